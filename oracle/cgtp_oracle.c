@@ -1,0 +1,488 @@
+/*
+ * cgtp_oracle.c -- FP64 CPU ORACLE for the contracted Clebsch-Gordan tensor product.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Only tests/, __graft_entry__.smoke() and the cpu_baseline /
+ * --impl reference legs of bench.py may build, load or call this file.  The product path
+ * (paper_2605_15073_b200/) never does and shares no code, header, table or constant with it.
+ *
+ * What it computes (citations are PAPER.md lines = /root/reference/PAPER.md):
+ *   - on-site bilinear contraction Eq.(1) at fixed CP rank Eq.(3) (:39), for
+ *     natural-parity inputs: "even" rank channels couple through the Gaunt coefficient Eq.(4)-(5)
+ *     (:49-:55), "odd" rank channels through the surface-curl coefficient Q = kappa^-1 * G,
+ *     Eq.(13)-(14) (:115-:119) with kappa^-1 from Eq.(A10) (:580).
+ *   - message-passing coupling Eq.(2) (:33): edge factor R~[e,c] * Y_{l1 m1}(r_hat_e) (factor 1)
+ *     times the sender's projected node feature (factor 2), summed over the in-edges of every
+ *     receiver (Eq.(52) :415, Eq.(57) :443).
+ * The method reaches these sums exactly (the grid quadrature is exact), so the oracle is the plain
+ * definition written out as a direct sparse sum over closed-form coefficients.  Nothing in this
+ * file touches a quadrature grid.
+ *
+ * Readings of the paper used here:
+ *   R1  spherical harmonics are orthonormal on S^2.
+ *   R2  real basis of Eq.(C1) (:663) without Condon-Shortley phase, order m=-l..l, flat index
+ *       l*l+l+m; (Y_{1,-1},Y_{1,0},Y_{1,1}) = sqrt(3/4pi) (y,z,x).
+ *   R4  with given weights the pipeline realises the Gaunt-weighted (even) / Q-weighted (odd)
+ *       coupling (the prefactors f, kappa are absorbed in the learnable weights, :157, :374-:381).
+ *   R5  l-shared weights W_a,W_b[C,N], W_out[N,C].   R6  parity_mask[c]: 0 even, 1 odd; two output
+ *       sectors.   R10 bracket {1,2} = d_phi A1 d_x A2 - d_x A1 d_phi A2, on-site A is factor 1,
+ *       message passing: edge is factor 1.   R11 edge_vec = r_j - r_i, edge_index row 0 sender,
+ *       row 1 receiver, receiver-sorted.   R12 l1-shared radial factor edge_radial[E,C].
+ *
+ * Pins (tests/test_oracle_*.py, all -m "not gpu"): Wigner 3j and Gaunt against sympy's exact values,
+ * Eq.(6) closed form, the printed kappa^-1 values (:600, :655) and worked example (A11)-(A13),
+ * real-basis tables against brute-force quadrature, (1,1,1) block = sqrt(3/4pi)*epsilon,
+ * real SH against scipy, whole-pipeline results against fine-grid quadrature, Wigner-D
+ * equivariance, inversion parity, self-coupled vanishing, Parseval.  No function here is
+ * "parity unpinned".
+ *
+ * Plain C99 + OpenMP, double precision (long double inside the Racah sum).
+ */
+#include <complex.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#ifndef M_PI
+#define M_PI 3.14159265358979323846264338327950288
+#endif
+
+/* ------------------------------------------------------------------------------------------ */
+/* Angular-momentum algebra                                                                   */
+/* ------------------------------------------------------------------------------------------ */
+
+static long double lfact(int n) { return lgammal((long double)n + 1.0L); }
+
+static int triangle_ok(int a, int b, int c) { return c >= abs(a - b) && c <= a + b; }
+
+/* Wigner 3j symbol (j1 j2 j3; m1 m2 m3), integer arguments, Racah's single-sum formula
+ * (the "standard 3-j/CG relation" the paper invokes at :578; ref. [41] of the paper). */
+double oracle_wigner3j(int j1, int j2, int j3, int m1, int m2, int m3)
+{
+    if (j1 < 0 || j2 < 0 || j3 < 0) return 0.0;
+    if (m1 + m2 + m3 != 0) return 0.0;
+    if (abs(m1) > j1 || abs(m2) > j2 || abs(m3) > j3) return 0.0;
+    if (!triangle_ok(j1, j2, j3)) return 0.0;
+    long double logpref = 0.5L * (lfact(j1 + j2 - j3) + lfact(j1 - j2 + j3) + lfact(-j1 + j2 + j3)
+                                  - lfact(j1 + j2 + j3 + 1)
+                                  + lfact(j1 + m1) + lfact(j1 - m1) + lfact(j2 + m2) + lfact(j2 - m2)
+                                  + lfact(j3 + m3) + lfact(j3 - m3));
+    int tmin = 0;
+    if (j2 - j3 - m1 > tmin) tmin = j2 - j3 - m1;
+    if (j1 - j3 + m2 > tmin) tmin = j1 - j3 + m2;
+    int tmax = j1 + j2 - j3;
+    if (j1 - m1 < tmax) tmax = j1 - m1;
+    if (j2 + m2 < tmax) tmax = j2 + m2;
+    long double sum = 0.0L;
+    for (int t = tmin; t <= tmax; ++t) {
+        long double logden = lfact(t) + lfact(j3 - j2 + t + m1) + lfact(j3 - j1 + t - m2)
+                             + lfact(j1 + j2 - j3 - t) + lfact(j1 - t - m1) + lfact(j2 - t + m2);
+        long double term = expl(logpref - logden);
+        sum += (t & 1) ? -term : term;
+    }
+    int ph = j1 - j2 - m3;
+    if (ph & 1) sum = -sum;
+    return (double)sum;
+}
+
+/* Clebsch-Gordan coefficient G^{l m}_{l1 m1 l2 m2} = <l1 m1 l2 m2 | l m> (Condon-Shortley). */
+double oracle_cg(int l1, int m1, int l2, int m2, int l, int m)
+{
+    if (m1 + m2 != m) return 0.0;
+    double w = oracle_wigner3j(l1, l2, l, m1, m2, -m);
+    int ph = l1 - l2 + m;
+    double s = (ph & 1) ? -1.0 : 1.0;
+    return s * sqrt(2.0 * l + 1.0) * w;
+}
+
+/* Eq.(6)-(7) (PAPER.md:59-:63): closed form of G^{l0}_{l1 0 l2 0}; Eq.(8) (:70): zero for odd sum. */
+double oracle_cg000_closed(int l1, int l2, int l)
+{
+    if (!triangle_ok(l1, l2, l)) return 0.0;
+    int s = l1 + l2 + l;
+    if (s & 1) return 0.0;
+    int g = s / 2;
+    long double logdelta = lfact(l1 + l2 - l) + lfact(l1 - l2 + l) + lfact(-l1 + l2 + l) - lfact(s + 1);
+    long double logv = 0.5L * logdelta + lfact(g) - lfact(g - l1) - lfact(g - l2) - lfact(g - l);
+    double v = sqrt(2.0 * l + 1.0) * (double)expl(logv);
+    int ph = l1 - l2 + g;
+    return (ph & 1) ? -v : v;
+}
+
+/* Eq.(4)-(5) (PAPER.md:49-:55): complex Gaunt coefficient  int Y_{l1m1} Y_{l2m2} Y*_{lm} dOmega. */
+double oracle_gaunt_complex(int l1, int m1, int l2, int m2, int l, int m)
+{
+    if (m1 + m2 != m) return 0.0;
+    double g0 = oracle_cg000_closed(l1, l2, l);
+    if (g0 == 0.0) return 0.0;
+    double pref = sqrt((2.0 * l1 + 1.0) * (2.0 * l2 + 1.0) / (4.0 * M_PI * (2.0 * l + 1.0)));
+    return pref * g0 * oracle_cg(l1, m1, l2, m2, l, m);
+}
+
+/* Eq.(A10): kappa^-1(l1,l2,l) is purely imaginary in the complex basis; this returns
+ * its imaginary part, i.e. kappa^-1 = i * oracle_kappa_inv_imag.  Support (:583-:585): l1,l2>=1,
+ * triangle, l1+l2+l odd; zero elsewhere (Eq.(A7) :560). */
+double oracle_kappa_inv_imag(int l1, int l2, int l)
+{
+    if (l1 < 1 || l2 < 1 || !triangle_ok(l1, l2, l)) return 0.0;
+    if (((l1 + l2 + l) & 1) == 0) return 0.0;
+    double pref = sqrt((2.0 * l1 + 1.0) * (2.0 * l2 + 1.0) * l1 * (l1 + 1.0) * l2 * (l2 + 1.0) / (4.0 * M_PI));
+    double w = oracle_wigner3j(l1, l2, l, -1, 1, 0);
+    int ph = l1 - l2;
+    double s = (ph & 1) ? -1.0 : 1.0;
+    /* kappa^-1 = -i * (-1)^{l1-l2} * pref * 3j  ->  imaginary part = -(-1)^{l1-l2} pref 3j */
+    return -s * pref * w;
+}
+
+/* Eq.(13)-(14) (PAPER.md:115-:119): complex surface-curl coefficient Q = kappa^-1 * G (purely
+ * imaginary); returns its imaginary part. */
+double oracle_q_complex_imag(int l1, int m1, int l2, int m2, int l, int m)
+{
+    if (m1 + m2 != m) return 0.0;
+    double k = oracle_kappa_inv_imag(l1, l2, l);
+    if (k == 0.0) return 0.0;
+    return k * oracle_cg(l1, m1, l2, m2, l, m);
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Complex -> real basis (reading R2; Eq.(C1), complex CS basis as in App. B :611) */
+/*   m>0 : Y^r_{l,m}  = ((-1)^m Y^c_{l,m} + Y^c_{l,-m}) / sqrt2                                 */
+/*   m=0 : Y^r_{l,0}  = Y^c_{l,0}                                                               */
+/*   m<0 : Y^r_{l,m}  = ((-1)^a Y^c_{l,a} - Y^c_{l,-a}) / (i sqrt2),  a=|m|                      */
+/* U(m, mu) is the coefficient of Y^c_{l,mu} in Y^r_{l,m}; only mu = +-|m| are non-zero.         */
+/* ------------------------------------------------------------------------------------------ */
+static double complex real_from_complex_U(int m, int mu)
+{
+    const double r = 0.70710678118654752440;
+    if (m == 0) return (mu == 0) ? 1.0 : 0.0;
+    int a = abs(m);
+    if (abs(mu) != a) return 0.0;
+    double sa = (a & 1) ? -1.0 : 1.0;
+    if (m > 0) return (mu > 0) ? sa * r : r;
+    /* m<0: 1/(i sqrt2) = -i/sqrt2 */
+    return (mu > 0) ? (-I * sa * r) : (I * r);
+}
+
+typedef struct {
+    int lmax, lmax_out, odd;
+    int64_t nnz;
+    int32_t *i1, *i2, *io;
+    double *val;
+    double max_imag; /* largest discarded imaginary part (must be round-off) */
+} coupling_t;
+
+#define MAX_CACHED 32
+static coupling_t g_cache[MAX_CACHED];
+static int g_ncache = 0;
+
+/* Real-basis coupling tensor, sparse COO:
+ *   odd=0:  Gr(a,b;c) = int Y_a Y_b Y_c dOmega                  (real Gaunt; Eq.(4)-(5) in the real basis)
+ *   odd=1:  Qr(a,b;c) = int r.[grad Y_a x grad Y_b] Y_c dOmega  (Eq.(13) in the real basis)
+ * via T^r_{abc} = sum U1(a,mu1) U2(b,mu2) conj(U3(c,mu)) T^c(mu1,mu2;mu). */
+static const coupling_t *get_coupling(int lmax, int lmax_out, int odd)
+{
+    const coupling_t *found = NULL;
+#pragma omp critical(cgtp_oracle_cache)
+    {
+        for (int i = 0; i < g_ncache; ++i)
+            if (g_cache[i].lmax == lmax && g_cache[i].lmax_out == lmax_out && g_cache[i].odd == odd)
+                found = &g_cache[i];
+        if (!found && g_ncache < MAX_CACHED) {
+            coupling_t t;
+            memset(&t, 0, sizeof t);
+            t.lmax = lmax; t.lmax_out = lmax_out; t.odd = odd;
+            int64_t cap = 1024;
+            t.i1 = malloc(cap * sizeof(int32_t)); t.i2 = malloc(cap * sizeof(int32_t));
+            t.io = malloc(cap * sizeof(int32_t)); t.val = malloc(cap * sizeof(double));
+            int W = 2 * lmax + 1;
+            double *tc = malloc((size_t)W * W * sizeof(double)); /* complex-basis table at fixed (l1,l2,l) */
+            for (int l1 = 0; l1 <= lmax; ++l1)
+            for (int l2 = 0; l2 <= lmax; ++l2)
+            for (int l = abs(l1 - l2); l <= l1 + l2 && l <= lmax_out; ++l) {
+                int par = (l1 + l2 + l) & 1;
+                if (par != odd) continue;
+                if (odd && (l1 < 1 || l2 < 1)) continue;
+                /* complex table: real number g (even) or imaginary part q (odd: value = i*q) */
+                for (int m1 = -l1; m1 <= l1; ++m1)
+                for (int m2 = -l2; m2 <= l2; ++m2) {
+                    int m = m1 + m2;
+                    double v = 0.0;
+                    if (abs(m) <= l)
+                        v = odd ? oracle_q_complex_imag(l1, m1, l2, m2, l, m)
+                                : oracle_gaunt_complex(l1, m1, l2, m2, l, m);
+                    tc[(m1 + l1) * W + (m2 + l2)] = v;
+                }
+                for (int a = -l1; a <= l1; ++a)
+                for (int b = -l2; b <= l2; ++b)
+                for (int c = -l; c <= l; ++c) {
+                    double complex acc = 0.0;
+                    for (int s1 = 0; s1 < 2; ++s1) {
+                        int mu1 = s1 ? -abs(a) : abs(a);
+                        if (a == 0 && s1) continue;
+                        double complex u1 = real_from_complex_U(a, mu1);
+                        for (int s2 = 0; s2 < 2; ++s2) {
+                            int mu2 = s2 ? -abs(b) : abs(b);
+                            if (b == 0 && s2) continue;
+                            int mu = mu1 + mu2;
+                            if (abs(mu) != abs(c)) continue;
+                            double complex u2 = real_from_complex_U(b, mu2);
+                            double complex u3 = real_from_complex_U(c, mu);
+                            double v = tc[(mu1 + l1) * W + (mu2 + l2)];
+                            double complex tcv = odd ? (I * v) : v;
+                            acc += u1 * u2 * conj(u3) * tcv;
+                        }
+                    }
+                    if (fabs(cimag(acc)) > t.max_imag) t.max_imag = fabs(cimag(acc));
+                    double r = creal(acc);
+                    if (fabs(r) > 1e-12) {
+                        if (t.nnz == cap) {
+                            cap *= 2;
+                            t.i1 = realloc(t.i1, cap * sizeof(int32_t)); t.i2 = realloc(t.i2, cap * sizeof(int32_t));
+                            t.io = realloc(t.io, cap * sizeof(int32_t)); t.val = realloc(t.val, cap * sizeof(double));
+                        }
+                        t.i1[t.nnz] = l1 * l1 + l1 + a;
+                        t.i2[t.nnz] = l2 * l2 + l2 + b;
+                        t.io[t.nnz] = l * l + l + c;
+                        t.val[t.nnz] = r;
+                        t.nnz++;
+                    }
+                }
+            }
+            free(tc);
+            g_cache[g_ncache] = t;
+            found = &g_cache[g_ncache];
+            g_ncache++;
+        }
+    }
+    return found;
+}
+
+/* Exported view of the real-basis coupling tensor.  Call with NULL arrays to get nnz. */
+int64_t oracle_real_coupling(int lmax, int lmax_out, int odd, int32_t *i1, int32_t *i2, int32_t *io,
+                             double *val, double *max_imag)
+{
+    const coupling_t *t = get_coupling(lmax, lmax_out, odd);
+    if (!t) return -1;
+    if (max_imag) *max_imag = t->max_imag;
+    if (i1 && i2 && io && val) {
+        memcpy(i1, t->i1, t->nnz * sizeof(int32_t));
+        memcpy(i2, t->i2, t->nnz * sizeof(int32_t));
+        memcpy(io, t->io, t->nnz * sizeof(int32_t));
+        memcpy(val, t->val, t->nnz * sizeof(double));
+    }
+    return t->nnz;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Real spherical harmonics of a direction (reading R1/R2), needed for the edge feature         */
+/* R(r) Y_{l1 m1}(r_hat) of Eq.(2) (PAPER.md:33-:35).                                           */
+/*   Y_{lm} = sqrt2 Pt_l^{|m|}(cos th) cos(m ph)  (m>0),  Pt_l^0  (m=0),  sqrt2 Pt sin(|m| ph) (m<0) */
+/*   Pt_l^m = sqrt((2l+1)/(4pi) (l-m)!/(l+m)!) P_l^m,  P_l^m WITHOUT the Condon-Shortley phase.  */
+/* ------------------------------------------------------------------------------------------ */
+void oracle_real_sh(int lmax, double x, double y, double z, double *Y /* [(lmax+1)^2] */)
+{
+    double r = sqrt(x * x + y * y + z * z);
+    double ct = z / r;
+    double st = sqrt(x * x + y * y) / r;
+    double ph = atan2(y, x);
+    int L = lmax + 1;
+    double *P = calloc((size_t)L * L, sizeof(double)); /* P[l*L+m] = Pt_l^m */
+    /* sectoral seeds Pt_m^m, then the standard three-term upward recurrence in l */
+    P[0] = sqrt(1.0 / (4.0 * M_PI));
+    for (int m = 1; m <= lmax; ++m)
+        P[m * L + m] = sqrt((2.0 * m + 1.0) / (2.0 * m)) * st * P[(m - 1) * L + (m - 1)];
+    for (int m = 0; m <= lmax; ++m) {
+        if (m + 1 <= lmax) P[(m + 1) * L + m] = sqrt(2.0 * m + 3.0) * ct * P[m * L + m];
+        for (int l = m + 2; l <= lmax; ++l) {
+            double a = sqrt((4.0 * l * l - 1.0) / ((double)l * l - (double)m * m));
+            double b = sqrt((((double)l - 1.0) * (l - 1.0) - (double)m * m) / (4.0 * (l - 1.0) * (l - 1.0) - 1.0));
+            P[l * L + m] = a * (ct * P[(l - 1) * L + m] - b * P[(l - 2) * L + m]);
+        }
+    }
+    const double s2 = sqrt(2.0);
+    for (int l = 0; l <= lmax; ++l) {
+        Y[l * l + l] = P[l * L];
+        for (int m = 1; m <= l; ++m) {
+            Y[l * l + l + m] = s2 * P[l * L + m] * cos(m * ph);
+            Y[l * l + l - m] = s2 * P[l * L + m] * sin(m * ph);
+        }
+    }
+    free(P);
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Segmentation (integer work): CSR offsets of a receiver-sorted edge list.                     */
+/* row_ptr[i] = first edge whose receiver is >= i;  row_ptr[nodes] = E.                         */
+/* Returns 0 if valid, 4 if not sorted / out of range (same code as the library's error 4).     */
+/* ------------------------------------------------------------------------------------------ */
+int oracle_segments(const int64_t *edge_index /* [2,E] */, int64_t E, int64_t nodes, int64_t *row_ptr)
+{
+    const int64_t *snd = edge_index, *rcv = edge_index + E;
+    for (int64_t e = 0; e < E; ++e) {
+        if (rcv[e] < 0 || rcv[e] >= nodes || snd[e] < 0 || snd[e] >= nodes) return 4;
+        if (e > 0 && rcv[e] < rcv[e - 1]) return 4;
+    }
+    int64_t e = 0;
+    for (int64_t i = 0; i <= nodes; ++i) {
+        while (e < E && rcv[e] < i) ++e;
+        row_ptr[i] = e;
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* On-site contraction, Eq.(1) with the CP factorisation Eq.(3).                                */
+/*   Ha[c,:] = W_a[c,:] . A[b]      Hb[c,:] = W_b[c,:] . B[b]                  (Eq.(35) :322)   */
+/*   T[c,lm] = sum coef(i1,i2;lm) Ha[c,i1] Hb[c,i2]   coef = Gr (mask 0) or Qr (mask 1)         */
+/*   out[b,s,n,lm] = sum_{c: mask[c]=s} W_out[n,c] T[c,lm]                     (Eq.(41) :346)   */
+/* Layouts: A,B [batch,N,(lmax+1)^2]; W_a,W_b [C,N]; W_out [N,C]; out [batch,2,N,(lmax_out+1)^2] */
+/* ------------------------------------------------------------------------------------------ */
+int oracle_onsite(const double *A, const double *B, const double *W_a, const double *W_b,
+                  const double *W_out, int lmax, int lmax_out, int N, int C, const uint8_t *parity_mask,
+                  double *out, int64_t batch)
+{
+    int L2 = (lmax + 1) * (lmax + 1), Lo2 = (lmax_out + 1) * (lmax_out + 1);
+    const coupling_t *tab[2];
+    tab[0] = get_coupling(lmax, lmax_out, 0);
+    tab[1] = get_coupling(lmax, lmax_out, 1);
+    if (!tab[0] || !tab[1]) return 2;
+#pragma omp parallel
+    {
+        double *Ha = malloc((size_t)C * L2 * sizeof(double));
+        double *Hb = malloc((size_t)C * L2 * sizeof(double));
+        double *T = malloc((size_t)C * Lo2 * sizeof(double));
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t b = 0; b < batch; ++b) {
+            const double *Ab = A + b * (int64_t)N * L2, *Bb = B + b * (int64_t)N * L2;
+            for (int c = 0; c < C; ++c)
+                for (int i = 0; i < L2; ++i) {
+                    double sa = 0.0, sb = 0.0;
+                    for (int n = 0; n < N; ++n) {
+                        sa += W_a[c * N + n] * Ab[n * L2 + i];
+                        sb += W_b[c * N + n] * Bb[n * L2 + i];
+                    }
+                    Ha[c * L2 + i] = sa;
+                    Hb[c * L2 + i] = sb;
+                }
+            for (int c = 0; c < C; ++c) {
+                const coupling_t *t = tab[parity_mask[c] ? 1 : 0];
+                double *Tc = T + (size_t)c * Lo2;
+                const double *ha = Ha + (size_t)c * L2, *hb = Hb + (size_t)c * L2;
+                for (int i = 0; i < Lo2; ++i) Tc[i] = 0.0;
+                for (int64_t k = 0; k < t->nnz; ++k)
+                    Tc[t->io[k]] += t->val[k] * ha[t->i1[k]] * hb[t->i2[k]];
+            }
+            double *ob = out + b * 2 * (int64_t)N * Lo2;
+            for (int s = 0; s < 2; ++s)
+                for (int n = 0; n < N; ++n)
+                    for (int i = 0; i < Lo2; ++i) {
+                        double acc = 0.0;
+                        for (int c = 0; c < C; ++c)
+                            if ((parity_mask[c] ? 1 : 0) == s) acc += W_out[n * C + c] * T[(size_t)c * Lo2 + i];
+                        ob[((size_t)s * N + n) * Lo2 + i] = acc;
+                    }
+        }
+        free(Ha); free(Hb); free(T);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Message passing, Eq.(2) with the CP factorisation Eq.(42)-(43) and the l1-shared radial      */
+/* factor (reading R12).  For receiver i with in-edges e (sender j = send(e)):                  */
+/*   a[e,c,l1m1] = edge_radial[e,c] * Y_{l1m1}(edge_vec[e]/|edge_vec[e]|)   (factor 1, Eq.(46),(48)) */
+/*   H[j,c,:]    = W_node[c,:] . node_feats[j]                              (factor 2, Eq.(47))  */
+/*   T[i,c,lm]   = sum_e sum coef(i1,i2;lm) a[e,c,i1] H[j,c,i2]             (Eq.(52) / Eq.(57))  */
+/*   out[i,s,n,lm] = sum_{c: mask[c]=s} W_out[n,c] T[i,c,lm]                (Eq.(55),(58),(59))  */
+/* recv_list/n_recv select the receivers that are evaluated (NULL = all nodes); out has one      */
+/* block [2,N,(lmax_out+1)^2] per evaluated receiver, in list order.                             */
+/* ------------------------------------------------------------------------------------------ */
+int oracle_message(const double *node_feats /* [nodes,N,L2] */, const int64_t *edge_index /* [2,E] */,
+                   const double *edge_vec /* [E,3] */, const double *edge_radial /* [E,C] */,
+                   const double *W_node /* [C,N] */, const double *W_out /* [N,C] */,
+                   int lmax, int lmax_out, int N, int C, const uint8_t *parity_mask,
+                   double *out, int64_t nodes, int64_t E, const int64_t *recv_list, int64_t n_recv)
+{
+    int L2 = (lmax + 1) * (lmax + 1), Lo2 = (lmax_out + 1) * (lmax_out + 1);
+    const coupling_t *tab[2];
+    tab[0] = get_coupling(lmax, lmax_out, 0);
+    tab[1] = get_coupling(lmax, lmax_out, 1);
+    if (!tab[0] || !tab[1]) return 2;
+    int64_t *row_ptr = malloc((size_t)(nodes + 1) * sizeof(int64_t));
+    int rc = oracle_segments(edge_index, E, nodes, row_ptr);
+    if (rc) { free(row_ptr); return rc; }
+    const int64_t *snd = edge_index;
+    int64_t nr = recv_list ? n_recv : nodes;
+    /* Eq.(47): project only the senders that the evaluated receivers need (once per node). */
+    int64_t *slot = malloc((size_t)nodes * sizeof(int64_t));
+    for (int64_t j = 0; j < nodes; ++j) slot[j] = -1;
+    int64_t n_need = 0;
+    for (int64_t r = 0; r < nr; ++r) {
+        int64_t i = recv_list ? recv_list[r] : r;
+        for (int64_t e = row_ptr[i]; e < row_ptr[i + 1]; ++e)
+            if (slot[snd[e]] < 0) slot[snd[e]] = n_need++;
+    }
+    double *H = malloc((size_t)(n_need > 0 ? n_need : 1) * C * L2 * sizeof(double));
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t j = 0; j < nodes; ++j) {
+        if (slot[j] < 0) continue;
+        const double *xj = node_feats + j * (int64_t)N * L2;
+        double *hj = H + slot[j] * (int64_t)C * L2;
+        for (int c = 0; c < C; ++c)
+            for (int q = 0; q < L2; ++q) {
+                double s = 0.0;
+                for (int n = 0; n < N; ++n) s += W_node[c * N + n] * xj[n * L2 + q];
+                hj[c * L2 + q] = s;
+            }
+    }
+#pragma omp parallel
+    {
+        double *Y = malloc((size_t)L2 * sizeof(double));
+        double *a = malloc((size_t)L2 * sizeof(double));
+        double *T = malloc((size_t)C * Lo2 * sizeof(double));
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t r = 0; r < nr; ++r) {
+            int64_t i = recv_list ? recv_list[r] : r;
+            for (size_t k = 0; k < (size_t)C * Lo2; ++k) T[k] = 0.0;
+            for (int64_t e = row_ptr[i]; e < row_ptr[i + 1]; ++e) {
+                const double *hj = H + slot[snd[e]] * (int64_t)C * L2;
+                oracle_real_sh(lmax, edge_vec[3 * e], edge_vec[3 * e + 1], edge_vec[3 * e + 2], Y);
+                for (int c = 0; c < C; ++c) {
+                    double rad = edge_radial[e * (int64_t)C + c];
+                    for (int q = 0; q < L2; ++q) a[q] = rad * Y[q];
+                    const double *h = hj + (size_t)c * L2;
+                    const coupling_t *t = tab[parity_mask[c] ? 1 : 0];
+                    double *Tc = T + (size_t)c * Lo2;
+                    for (int64_t k = 0; k < t->nnz; ++k)
+                        Tc[t->io[k]] += t->val[k] * a[t->i1[k]] * h[t->i2[k]];
+                }
+            }
+            double *ob = out + r * 2 * (int64_t)N * Lo2;
+            for (int s = 0; s < 2; ++s)
+                for (int n = 0; n < N; ++n)
+                    for (int q = 0; q < Lo2; ++q) {
+                        double acc = 0.0;
+                        for (int c = 0; c < C; ++c)
+                            if ((parity_mask[c] ? 1 : 0) == s) acc += W_out[n * C + c] * T[(size_t)c * Lo2 + q];
+                        ob[((size_t)s * N + n) * Lo2 + q] = acc;
+                    }
+        }
+        free(Y); free(a); free(T);
+    }
+    free(H); free(slot);
+    free(row_ptr);
+    return 0;
+}
+
+int oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

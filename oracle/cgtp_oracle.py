@@ -1,0 +1,182 @@
+"""ctypes front end of the FP64 CPU oracle (oracle/cgtp_oracle.c).
+
+TEST INFRASTRUCTURE ONLY: importable from tests/, __graft_entry__.smoke() and the cpu_baseline /
+--impl reference legs of bench.py.  The product package never imports this module and this
+module never imports the product package.
+
+Every function converts its inputs to float64 and calls the C routine of the same name; no
+arithmetic of the method lives in this file.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "cgtp_oracle.c")
+_LIB = os.path.join(_HERE, "libcgtp_oracle.so")
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (plain C99 + OpenMP).  Returns the path of the shared object."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    lib = ctypes.CDLL(build())
+    d, i, i64 = ctypes.c_double, ctypes.c_int, ctypes.c_int64
+    p = ctypes.c_void_p
+    lib.oracle_wigner3j.restype = d
+    lib.oracle_wigner3j.argtypes = [i] * 6
+    lib.oracle_cg.restype = d
+    lib.oracle_cg.argtypes = [i] * 6
+    lib.oracle_cg000_closed.restype = d
+    lib.oracle_cg000_closed.argtypes = [i] * 3
+    lib.oracle_gaunt_complex.restype = d
+    lib.oracle_gaunt_complex.argtypes = [i] * 6
+    lib.oracle_kappa_inv_imag.restype = d
+    lib.oracle_kappa_inv_imag.argtypes = [i] * 3
+    lib.oracle_q_complex_imag.restype = d
+    lib.oracle_q_complex_imag.argtypes = [i] * 6
+    lib.oracle_real_coupling.restype = i64
+    lib.oracle_real_coupling.argtypes = [i, i, i, p, p, p, p, p]
+    lib.oracle_real_sh.restype = None
+    lib.oracle_real_sh.argtypes = [i, d, d, d, p]
+    lib.oracle_segments.restype = i
+    lib.oracle_segments.argtypes = [p, i64, i64, p]
+    lib.oracle_onsite.restype = i
+    lib.oracle_onsite.argtypes = [p, p, p, p, p, i, i, i, i, p, p, i64]
+    lib.oracle_message.restype = i
+    lib.oracle_message.argtypes = [p, p, p, p, p, p, i, i, i, i, p, p, i64, i64, p, i64]
+    lib.oracle_num_threads.restype = i
+    lib.oracle_num_threads.argtypes = []
+    _lib = lib
+    return lib
+
+
+def _f64(a):
+    return np.ascontiguousarray(np.asarray(a), dtype=np.float64)
+
+
+def _ptr(a):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def wigner3j(j1, j2, j3, m1, m2, m3) -> float:
+    return _load().oracle_wigner3j(j1, j2, j3, m1, m2, m3)
+
+
+def cg(l1, m1, l2, m2, l, m) -> float:
+    return _load().oracle_cg(l1, m1, l2, m2, l, m)
+
+
+def cg000_closed(l1, l2, l) -> float:
+    return _load().oracle_cg000_closed(l1, l2, l)
+
+
+def gaunt_complex(l1, m1, l2, m2, l, m) -> float:
+    return _load().oracle_gaunt_complex(l1, m1, l2, m2, l, m)
+
+
+def kappa_inv_imag(l1, l2, l) -> float:
+    return _load().oracle_kappa_inv_imag(l1, l2, l)
+
+
+def q_complex_imag(l1, m1, l2, m2, l, m) -> float:
+    return _load().oracle_q_complex_imag(l1, m1, l2, m2, l, m)
+
+
+def real_coupling(lmax: int, lmax_out: int, odd: bool):
+    """Sparse real-basis coupling tensor (i1, i2, io, val, max_imag)."""
+    lib = _load()
+    mi = ctypes.c_double(0.0)
+    nnz = lib.oracle_real_coupling(lmax, lmax_out, int(odd), None, None, None, None, ctypes.byref(mi))
+    if nnz < 0:
+        raise RuntimeError("oracle coupling cache full")
+    i1 = np.empty(nnz, np.int32)
+    i2 = np.empty(nnz, np.int32)
+    io = np.empty(nnz, np.int32)
+    val = np.empty(nnz, np.float64)
+    lib.oracle_real_coupling(lmax, lmax_out, int(odd), _ptr(i1), _ptr(i2), _ptr(io), _ptr(val), ctypes.byref(mi))
+    return i1, i2, io, val, mi.value
+
+
+def real_coupling_dense(lmax: int, lmax_out: int, odd: bool) -> np.ndarray:
+    i1, i2, io, val, _ = real_coupling(lmax, lmax_out, odd)
+    t = np.zeros(((lmax + 1) ** 2, (lmax + 1) ** 2, (lmax_out + 1) ** 2))
+    t[i1, i2, io] = val
+    return t
+
+
+def real_sh(lmax: int, xyz) -> np.ndarray:
+    """Real spherical harmonics Y[(lmax+1)^2] of one direction (need not be normalised)."""
+    out = np.empty((lmax + 1) ** 2, np.float64)
+    x, y, z = (float(v) for v in xyz)
+    _load().oracle_real_sh(lmax, x, y, z, _ptr(out))
+    return out
+
+
+def segments(edge_index, nodes: int):
+    """CSR offsets row_ptr[nodes+1] of a receiver-sorted edge list; returns (status, row_ptr)."""
+    ei = np.ascontiguousarray(np.asarray(edge_index), dtype=np.int64)
+    E = ei.shape[1]
+    rp = np.zeros(nodes + 1, np.int64)
+    rc = _load().oracle_segments(_ptr(ei), E, nodes, _ptr(rp))
+    return rc, rp
+
+
+def onsite(A, B, W_a, W_b, W_out, lmax, lmax_out, parity_mask) -> np.ndarray:
+    """out[batch, 2, N, (lmax_out+1)^2] in float64."""
+    A, B, W_a, W_b, W_out = map(_f64, (A, B, W_a, W_b, W_out))
+    batch, N, L2 = A.shape
+    C = W_a.shape[0]
+    assert L2 == (lmax + 1) ** 2 and B.shape == A.shape
+    assert W_a.shape == (C, N) and W_b.shape == (C, N) and W_out.shape == (N, C)
+    mask = np.ascontiguousarray(np.asarray(parity_mask), dtype=np.uint8)
+    assert mask.shape == (C,)
+    out = np.zeros((batch, 2, N, (lmax_out + 1) ** 2), np.float64)
+    rc = _load().oracle_onsite(_ptr(A), _ptr(B), _ptr(W_a), _ptr(W_b), _ptr(W_out), lmax, lmax_out, N, C,
+                               _ptr(mask), _ptr(out), batch)
+    if rc:
+        raise RuntimeError(f"oracle_onsite failed with code {rc}")
+    return out
+
+
+def message(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, parity_mask,
+            recv_list=None) -> np.ndarray:
+    """out[n_recv or nodes, 2, N, (lmax_out+1)^2] in float64."""
+    X, ev, er, W_node, W_out = map(_f64, (node_feats, edge_vec, edge_radial, W_node, W_out))
+    ei = np.ascontiguousarray(np.asarray(edge_index), dtype=np.int64)
+    nodes, N, L2 = X.shape
+    E = ei.shape[1]
+    C = W_node.shape[0]
+    assert L2 == (lmax + 1) ** 2 and ev.shape == (E, 3) and er.shape == (E, C)
+    assert W_node.shape == (C, N) and W_out.shape == (N, C)
+    mask = np.ascontiguousarray(np.asarray(parity_mask), dtype=np.uint8)
+    if recv_list is None:
+        rl, nr, rlp = None, nodes, None
+    else:
+        rl = np.ascontiguousarray(np.asarray(recv_list), dtype=np.int64)
+        nr, rlp = rl.shape[0], _ptr(rl)
+    out = np.zeros((nr, 2, N, (lmax_out + 1) ** 2), np.float64)
+    rc = _load().oracle_message(_ptr(X), _ptr(ei), _ptr(ev), _ptr(er), _ptr(W_node), _ptr(W_out), lmax, lmax_out,
+                                N, C, _ptr(mask), _ptr(out), nodes, E, rlp, nr if rl is not None else 0)
+    if rc:
+        raise RuntimeError(f"oracle_message failed with code {rc}")
+    return out
+
+
+def num_threads() -> int:
+    return _load().oracle_num_threads()
