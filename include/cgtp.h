@@ -1,0 +1,164 @@
+/*
+ * cgtp.h -- C ABI of libcgtp: B200-native (sm_100a) contracted Clebsch-Gordan tensor products.
+ *
+ * The hot path of the SCALE-CG method (arxiv 2605.15073; citations "PAPER.md:<line>" refer to the
+ * paper text): the O(L^3) contracted Clebsch-Gordan tensor product at fixed CP rank, evaluated on a
+ * Gauss-Legendre (theta) x Fourier (phi) grid.
+ *
+ * Conventions ("Readings"):
+ *   - real spherical harmonics of Eq.(C1), orthonormal on S^2, no Condon-Shortley
+ *     phase, coefficient order m = -l..l, flat index l*l + l + m;
+ *   - all tensors row-major contiguous FP32; "device" pointers are CUDA device memory owned by the
+ *     caller (e.g. allocated by PyTorch), 16-byte aligned; the library never frees caller memory;
+ *   - parity_mask is a HOST array of C bytes: 0 = parity-even rank channel (pointwise grid product,
+ *     Gaunt coupling, Eq.(38) :332), 1 = parity-odd rank channel (surface-curl pairing
+ *     r.[grad A x grad B], Eq.(11)-(12) :107-:111, Eq.(57) :443).  It is structural (it selects the
+ *     kernels that run), like lmax;
+ *   - out has two parity sectors: sector 0 = sum over even channels (natural parity (-1)^l),
+ *     sector 1 = sum over odd channels (opposite parity); out is fully overwritten;
+ *   - every call is asynchronous on `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy
+ *     default stream) and does no host synchronisation, except where stated;
+ *   - results are bitwise reproducible run to run (no floating-point atomics anywhere).
+ *
+ * Return codes: CGTP_OK, or
+ *   CGTP_ERR_INVALID      null pointer, negative size, lmax < 0, lmax_out > 2*lmax, mask entry not in
+ *                         {0,1}, misaligned pointer, workspace too small;
+ *   CGTP_ERR_UNSUPPORTED  band limit above cgtp_max_lmax(), N or C above the compiled limits;
+ *   CGTP_ERR_CUDA         a CUDA runtime call failed (message in cgtp_last_error());
+ *   CGTP_ERR_GRAPH        edge_index not receiver-sorted or out of range (reported by
+ *                         cgtp_message_status / cgtp_build_segments' status word).
+ * No exception or abort ever crosses this boundary.
+ */
+#ifndef CGTP_H
+#define CGTP_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CGTP_OK 0
+#define CGTP_ERR_INVALID 1
+#define CGTP_ERR_UNSUPPORTED 2
+#define CGTP_ERR_CUDA 3
+#define CGTP_ERR_GRAPH 4
+
+/* Library version (major*10000 + minor*100 + patch). */
+int cgtp_version(void);
+
+/* Message of the last error raised on the calling thread ("" if none). Never NULL. */
+const char* cgtp_last_error(void);
+
+/* Largest band limit max(lmax, lmax_out) the compiled kernels support. */
+int cgtp_max_lmax(void);
+
+/* Quadrature grid used for (lmax, lmax_out): U Gauss-Legendre nodes in cos(theta) and V uniform
+ * azimuths, U = ceil((2 lmax + lmax_out + 1)/2), V = 2 lmax + lmax_out + 1 -- the exactness bound of
+ * PAPER.md:173 (U >= (3 lmax+1)/2, V >= 3 lmax+1) generalised to lmax_out != lmax. */
+int cgtp_grid_shape(int lmax, int lmax_out, int* U, int* V);
+
+/* ---------------------------------------------------------------------------------------------
+ * On-site bilinear contraction, Eq.(1) at CP rank C, Eq.(3) (:39), natural-parity
+ * inputs; the structured-grid pipeline of Sec. VII B, Eq.(35)-(41) (:322-:346), with the surface-curl
+ * pairing Eq.(12) (:111) for the odd channels (Sec. VII C e, :469):
+ *
+ *   Ha[b,c,:] = W_a[c,:] . A[b]     Hb[b,c,:] = W_b[c,:] . B[b]                       (Eq.(35))
+ *   even c:  T[b,c,lm] = int (Ha~ Hb~) Y_lm dOmega                                     (Eq.(36)-(40))
+ *   odd  c:  T[b,c,lm] = int r.[grad Ha~ x grad Hb~] Y_lm dOmega   (A factor 1, B factor 2)
+ *   out[b,s,n,lm] = sum_{c: mask[c]=s} W_out[n,c] T[b,c,lm],   l <= lmax_out           (Eq.(41))
+ *
+ * A, B      device [batch, N, (lmax+1)^2]
+ * W_a, W_b  device [C, N]        W_out  device [N, C]
+ * parity_mask  HOST [C]
+ * out       device [batch, 2, N, (lmax_out+1)^2]
+ * workspace device, >= cgtp_onsite_workspace_bytes(...) bytes, 256-byte aligned; contents are
+ *           scratch (projected coefficients H and rank-space results T) and may be reused by the
+ *           next call on the same stream.
+ * batch may be 0 (no work, CGTP_OK).  0 <= lmax_out <= 2*lmax.
+ * ------------------------------------------------------------------------------------------- */
+size_t cgtp_onsite_workspace_bytes(int lmax, int lmax_out, int N, int C, int64_t batch);
+
+int cgtp_onsite(const float* A, const float* B, const float* W_a, const float* W_b, const float* W_out,
+                int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask, float* out,
+                int64_t batch, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Parity-aware message passing, Eq.(2), pipeline of Sec. VII C, Eq.(46)-(59)
+ * (:396-:453), natural-parity node features (Cases A and B, :197-:217), l1-shared radial factor:
+ *
+ *   H[j,c,:]  = W_node[c,:] . node_feats[j]                                            (Eq.(47))
+ *   edge field (factor 1)  E_e(Omega) = edge_radial[e,c] * sum_{l1<=lmax,m1} Y_{l1m1}(r_e) Y_{l1m1}(Omega)
+ *                                                                                     (Eq.(46),(48),(50))
+ *   even c:  S[i,c,Omega] = sum_{e: recv(e)=i} E_e(Omega) H~[send(e),c](Omega)            (Eq.(52))
+ *   odd  c:  S[i,c,Omega] = sum_e r.[grad E_e x grad H~[send(e),c]](Omega)                (Eq.(57))
+ *   T[i,c,lm] = int S[i,c] Y_lm dOmega  (once per receiver, Eq.(53)-(54))
+ *   out[i,s,n,lm] = sum_{c: mask[c]=s} W_out[n,c] T[i,c,lm]                            (Eq.(55),(58),(59))
+ *
+ * node_feats  device [nodes, N, (lmax+1)^2]
+ * edge_index  device int64 [2, E]: row 0 = sender j, row 1 = receiver i; sorted by receiver
+ *             (ascending, ties in any fixed order -- the order of the sum within a receiver is the
+ *             input order, which makes the result bitwise reproducible)
+ * edge_vec    device [E, 3] = r_j - r_i; only the direction is used; must be non-zero
+ * edge_radial device [E, C] = R~ of Eq.(46), computed by the caller
+ * W_node      device [C, N]      W_out  device [N, C]      parity_mask  HOST [C]
+ * out         device [nodes, 2, N, (lmax_out+1)^2]; receivers without edges get zeros
+ * workspace   device, >= cgtp_message_workspace_bytes(...) bytes, 256-byte aligned
+ *
+ * Graph errors are detected on the device: the call still returns CGTP_OK, out is zero-filled, and
+ * cgtp_message_status() returns CGTP_ERR_GRAPH.
+ * ------------------------------------------------------------------------------------------- */
+size_t cgtp_message_workspace_bytes(int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask,
+                                    int64_t nodes, int64_t E);
+
+int cgtp_message(const float* node_feats, const int64_t* edge_index, const float* edge_vec,
+                 const float* edge_radial, const float* W_node, const float* W_out,
+                 int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask, float* out,
+                 int64_t nodes, int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Synchronises `cuda_stream` and returns the graph status the last cgtp_message on this workspace
+ * left: CGTP_OK or CGTP_ERR_GRAPH (CGTP_ERR_CUDA if the stream reports an error). */
+int cgtp_message_status(const void* workspace, void* cuda_stream);
+
+/* Segmentation step of cgtp_message on its own (integer work, bit-exact):
+ * row_ptr[i] = index of the first edge whose receiver is >= i, row_ptr[nodes] = E.
+ * edge_index device int64 [2,E]; row_ptr device int64 [nodes+1]; status device int32 [1], set to
+ * CGTP_OK or CGTP_ERR_GRAPH (receivers not ascending, or a sender/receiver outside [0,nodes)). */
+int cgtp_build_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int64_t* row_ptr,
+                        int32_t* status, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Host-buffer entry points (end-to-end path): same semantics as cgtp_onsite / cgtp_message, but
+ * every tensor pointer is HOST memory (pinned memory recommended; pageable works, slower).  The
+ * library allocates device memory from the CUDA stream-ordered pool, copies inputs host->device in
+ * batch chunks overlapped with compute, runs the device path, copies `out` device->host, and
+ * synchronises before returning.  Returns CGTP_ERR_GRAPH directly for a bad graph.
+ * ------------------------------------------------------------------------------------------- */
+int cgtp_onsite_host(const float* A, const float* B, const float* W_a, const float* W_b, const float* W_out,
+                     int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask, float* out,
+                     int64_t batch, void* cuda_stream);
+
+int cgtp_message_host(const float* node_feats, const int64_t* edge_index, const float* edge_vec,
+                      const float* edge_radial, const float* W_node, const float* W_out,
+                      int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask, float* out,
+                      int64_t nodes, int64_t E, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Instrumentation (used by bench.py; never needed for results).
+ * cgtp_launch_count: number of kernels this library has launched since it was loaded.
+ * cgtp_profile_enable(1): record a CUDA-event pair around every kernel launch (on the launching
+ * stream); cgtp_profile_collect synchronises those events, adds the elapsed milliseconds and launch
+ * counts per kernel kind into ms[kind], launches[kind] (arrays of cgtp_profile_kinds() entries), and
+ * clears the record.  cgtp_profile_kind_name(kind) names a kind.
+ * ------------------------------------------------------------------------------------------- */
+int64_t cgtp_launch_count(void);
+int cgtp_profile_kinds(void);
+const char* cgtp_profile_kind_name(int kind);
+int cgtp_profile_enable(int on);
+int cgtp_profile_collect(double* ms, int64_t* launches);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CGTP_H */

@@ -1,0 +1,269 @@
+"""Thin ctypes binding of libcgtp.so (the C ABI of include/cgtp.h).
+
+Argument marshalling only: every step of the hot path runs in the CUDA kernels of csrc/.  PyTorch is
+used for device memory (tensors, the workspace) and streams.  There is no CPU fallback: if the shared
+library is missing or the tensors are not CUDA tensors, the call raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libcgtp.so")
+
+OK, ERR_INVALID, ERR_UNSUPPORTED, ERR_CUDA, ERR_GRAPH = 0, 1, 2, 3, 4
+
+
+class CgtpError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"cgtp error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Loads libcgtp.so (built by `python -m paper_2605_15073_b200.build`).  Fails loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(f"{_LIB_PATH} not found: build it with `python -m paper_2605_15073_b200.build` "
+                          "(there is no CPU fallback)")
+    L = ctypes.CDLL(_LIB_PATH)
+    vp, i, i64, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_size_t
+    L.cgtp_version.restype = i
+    L.cgtp_last_error.restype = ctypes.c_char_p
+    L.cgtp_max_lmax.restype = i
+    L.cgtp_grid_shape.restype = i
+    L.cgtp_grid_shape.argtypes = [i, i, ctypes.POINTER(i), ctypes.POINTER(i)]
+    L.cgtp_onsite_workspace_bytes.restype = sz
+    L.cgtp_onsite_workspace_bytes.argtypes = [i, i, i, i, i64]
+    L.cgtp_onsite.restype = i
+    L.cgtp_onsite.argtypes = [vp, vp, vp, vp, vp, i, i, i, i, vp, vp, i64, vp, sz, vp]
+    L.cgtp_message_workspace_bytes.restype = sz
+    L.cgtp_message_workspace_bytes.argtypes = [i, i, i, i, vp, i64, i64]
+    L.cgtp_message.restype = i
+    L.cgtp_message.argtypes = [vp, vp, vp, vp, vp, vp, i, i, i, i, vp, vp, i64, i64, vp, sz, vp]
+    L.cgtp_message_status.restype = i
+    L.cgtp_message_status.argtypes = [vp, vp]
+    L.cgtp_build_segments.restype = i
+    L.cgtp_build_segments.argtypes = [vp, i64, i64, vp, vp, vp]
+    L.cgtp_onsite_host.restype = i
+    L.cgtp_onsite_host.argtypes = [vp, vp, vp, vp, vp, i, i, i, i, vp, vp, i64, vp]
+    L.cgtp_message_host.restype = i
+    L.cgtp_message_host.argtypes = [vp, vp, vp, vp, vp, vp, i, i, i, i, vp, vp, i64, i64, vp]
+    L.cgtp_launch_count.restype = i64
+    L.cgtp_profile_kinds.restype = i
+    L.cgtp_profile_kind_name.restype = ctypes.c_char_p
+    L.cgtp_profile_kind_name.argtypes = [i]
+    L.cgtp_profile_enable.restype = i
+    L.cgtp_profile_enable.argtypes = [i]
+    L.cgtp_profile_collect.restype = i
+    L.cgtp_profile_collect.argtypes = [vp, vp]
+    _lib = L
+    return L
+
+
+def _check(rc: int):
+    if rc != OK:
+        raise CgtpError(rc, lib().cgtp_last_error().decode())
+
+
+def _mask(parity_mask, C: int) -> np.ndarray:
+    m = np.ascontiguousarray(np.asarray(parity_mask), dtype=np.uint8)
+    if m.shape != (C,):
+        raise ValueError(f"parity_mask must have shape ({C},)")
+    return m
+
+
+def _dev(t: torch.Tensor, dtype, name: str) -> torch.Tensor:
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name} must be contiguous {dtype}")
+    return t
+
+
+def _stream_ptr(stream) -> int:
+    s = torch.cuda.current_stream() if stream is None else stream
+    return s.cuda_stream
+
+
+_ws_cache: dict = {}
+
+
+def _workspace(device, nbytes: int) -> torch.Tensor:
+    """One grow-only scratch buffer per device (torch allocations are 512-byte aligned)."""
+    key = (device.type, device.index)
+    ws = _ws_cache.get(key)
+    if ws is None or ws.numel() < nbytes:
+        _ws_cache.pop(key, None)
+        ws = None
+        ws = torch.empty(int(nbytes), dtype=torch.uint8, device=device)
+        _ws_cache[key] = ws
+    return ws
+
+
+def cgtp_version() -> int:
+    return lib().cgtp_version()
+
+
+def cgtp_max_lmax() -> int:
+    return lib().cgtp_max_lmax()
+
+
+def cgtp_grid_shape(lmax: int, lmax_out: int):
+    U, V = ctypes.c_int(0), ctypes.c_int(0)
+    _check(lib().cgtp_grid_shape(lmax, lmax_out, ctypes.byref(U), ctypes.byref(V)))
+    return U.value, V.value
+
+
+def cgtp_onsite_workspace_bytes(lmax, lmax_out, N, C, batch) -> int:
+    return lib().cgtp_onsite_workspace_bytes(lmax, lmax_out, N, C, batch)
+
+
+def cgtp_onsite(A, B, W_a, W_b, W_out, lmax, lmax_out, N, C, parity_mask, out=None, workspace=None, stream=None):
+    """out[batch, 2, N, (lmax_out+1)^2] = on-site contracted CG product (see include/cgtp.h)."""
+    f32 = torch.float32
+    A, B = _dev(A, f32, "A"), _dev(B, f32, "B")
+    W_a, W_b, W_out = _dev(W_a, f32, "W_a"), _dev(W_b, f32, "W_b"), _dev(W_out, f32, "W_out")
+    batch = A.shape[0]
+    L2, Lo2 = (lmax + 1) ** 2, (lmax_out + 1) ** 2
+    if tuple(A.shape) != (batch, N, L2) or tuple(B.shape) != (batch, N, L2):
+        raise ValueError("A, B must be [batch, N, (lmax+1)^2]")
+    if tuple(W_a.shape) != (C, N) or tuple(W_b.shape) != (C, N) or tuple(W_out.shape) != (N, C):
+        raise ValueError("W_a, W_b must be [C, N] and W_out [N, C]")
+    mask = _mask(parity_mask, C)
+    if out is None:
+        out = torch.empty((batch, 2, N, Lo2), dtype=f32, device=A.device)
+    else:
+        _dev(out, f32, "out")
+        if tuple(out.shape) != (batch, 2, N, Lo2):
+            raise ValueError("out must be [batch, 2, N, (lmax_out+1)^2]")
+    nbytes = cgtp_onsite_workspace_bytes(lmax, lmax_out, N, C, batch)
+    ws = _workspace(A.device, nbytes) if workspace is None else workspace
+    with torch.cuda.device(A.device):
+        rc = lib().cgtp_onsite(A.data_ptr(), B.data_ptr(), W_a.data_ptr(), W_b.data_ptr(), W_out.data_ptr(),
+                               lmax, lmax_out, N, C, mask.ctypes.data, out.data_ptr(), batch,
+                               ws.data_ptr(), ws.numel(), _stream_ptr(stream))
+    _check(rc)
+    return out
+
+
+def cgtp_message_workspace_bytes(lmax, lmax_out, N, C, parity_mask, nodes, E) -> int:
+    mask = _mask(parity_mask, C)
+    return lib().cgtp_message_workspace_bytes(lmax, lmax_out, N, C, mask.ctypes.data, nodes, E)
+
+
+def cgtp_message(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, N, C, parity_mask,
+                 out=None, workspace=None, stream=None, check: bool = False):
+    """out[nodes, 2, N, (lmax_out+1)^2] = parity-aware message passing (see include/cgtp.h).
+    check=True synchronises and raises CgtpError(ERR_GRAPH) for an unsorted / out-of-range edge list."""
+    f32 = torch.float32
+    X = _dev(node_feats, f32, "node_feats")
+    ei = _dev(edge_index, torch.int64, "edge_index")
+    ev, er = _dev(edge_vec, f32, "edge_vec"), _dev(edge_radial, f32, "edge_radial")
+    W_node, W_out = _dev(W_node, f32, "W_node"), _dev(W_out, f32, "W_out")
+    nodes, E = X.shape[0], ei.shape[1]
+    L2, Lo2 = (lmax + 1) ** 2, (lmax_out + 1) ** 2
+    if tuple(X.shape) != (nodes, N, L2):
+        raise ValueError("node_feats must be [nodes, N, (lmax+1)^2]")
+    if tuple(ei.shape) != (2, E) or tuple(ev.shape) != (E, 3) or tuple(er.shape) != (E, C):
+        raise ValueError("edge_index [2,E], edge_vec [E,3], edge_radial [E,C] expected")
+    if tuple(W_node.shape) != (C, N) or tuple(W_out.shape) != (N, C):
+        raise ValueError("W_node must be [C, N] and W_out [N, C]")
+    mask = _mask(parity_mask, C)
+    if out is None:
+        out = torch.empty((nodes, 2, N, Lo2), dtype=f32, device=X.device)
+    else:
+        _dev(out, f32, "out")
+    nbytes = lib().cgtp_message_workspace_bytes(lmax, lmax_out, N, C, mask.ctypes.data, nodes, E)
+    ws = _workspace(X.device, nbytes) if workspace is None else workspace
+    sp = _stream_ptr(stream)
+    with torch.cuda.device(X.device):
+        rc = lib().cgtp_message(X.data_ptr(), ei.data_ptr(), ev.data_ptr(), er.data_ptr(), W_node.data_ptr(),
+                                W_out.data_ptr(), lmax, lmax_out, N, C, mask.ctypes.data, out.data_ptr(), nodes, E,
+                                ws.data_ptr(), ws.numel(), sp)
+        _check(rc)
+        if check:
+            _check(lib().cgtp_message_status(ws.data_ptr(), sp))
+    return out
+
+
+def cgtp_message_status(workspace=None, device=None, stream=None) -> int:
+    ws = workspace if workspace is not None else _ws_cache[(device.type, device.index)]
+    return lib().cgtp_message_status(ws.data_ptr(), _stream_ptr(stream))
+
+
+def cgtp_build_segments(edge_index, nodes: int, stream=None):
+    """Returns (row_ptr int64 [nodes+1], status int32 [1]) on the device of edge_index."""
+    ei = _dev(edge_index, torch.int64, "edge_index")
+    E = ei.shape[1]
+    row_ptr = torch.empty(nodes + 1, dtype=torch.int64, device=ei.device)
+    status = torch.empty(1, dtype=torch.int32, device=ei.device)
+    with torch.cuda.device(ei.device):
+        _check(lib().cgtp_build_segments(ei.data_ptr(), E, nodes, row_ptr.data_ptr(), status.data_ptr(),
+                                         _stream_ptr(stream)))
+    return row_ptr, status
+
+
+def _host(t, dtype, name):
+    if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name} must be a contiguous CPU tensor of {dtype}")
+    return t
+
+
+def cgtp_onsite_host(A, B, W_a, W_b, W_out, lmax, lmax_out, N, C, parity_mask, out=None, stream=None):
+    """Host-buffer entry point (pinned CPU tensors recommended); returns a CPU tensor."""
+    f32 = torch.float32
+    A, B = _host(A, f32, "A"), _host(B, f32, "B")
+    W_a, W_b, W_out = _host(W_a, f32, "W_a"), _host(W_b, f32, "W_b"), _host(W_out, f32, "W_out")
+    batch = A.shape[0]
+    mask = _mask(parity_mask, C)
+    if out is None:
+        out = torch.empty((batch, 2, N, (lmax_out + 1) ** 2), dtype=f32, pin_memory=True)
+    rc = lib().cgtp_onsite_host(A.data_ptr(), B.data_ptr(), W_a.data_ptr(), W_b.data_ptr(), W_out.data_ptr(),
+                                lmax, lmax_out, N, C, mask.ctypes.data, out.data_ptr(), batch, _stream_ptr(stream))
+    _check(rc)
+    return out
+
+
+def cgtp_message_host(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, N, C,
+                      parity_mask, out=None, stream=None):
+    f32 = torch.float32
+    X = _host(node_feats, f32, "node_feats")
+    ei = _host(edge_index, torch.int64, "edge_index")
+    ev, er = _host(edge_vec, f32, "edge_vec"), _host(edge_radial, f32, "edge_radial")
+    W_node, W_out = _host(W_node, f32, "W_node"), _host(W_out, f32, "W_out")
+    nodes, E = X.shape[0], ei.shape[1]
+    mask = _mask(parity_mask, C)
+    if out is None:
+        out = torch.empty((nodes, 2, N, (lmax_out + 1) ** 2), dtype=f32, pin_memory=True)
+    rc = lib().cgtp_message_host(X.data_ptr(), ei.data_ptr(), ev.data_ptr(), er.data_ptr(), W_node.data_ptr(),
+                                 W_out.data_ptr(), lmax, lmax_out, N, C, mask.ctypes.data, out.data_ptr(), nodes, E,
+                                 _stream_ptr(stream))
+    _check(rc)
+    return out
+
+
+def cgtp_launch_count() -> int:
+    return lib().cgtp_launch_count()
+
+
+def cgtp_profile_enable(on: bool) -> None:
+    _check(lib().cgtp_profile_enable(int(on)))
+
+
+def cgtp_profile_collect() -> dict:
+    """{kind name: (milliseconds, launches)} accumulated since the last collect."""
+    n = lib().cgtp_profile_kinds()
+    ms = (ctypes.c_double * n)()
+    cnt = (ctypes.c_int64 * n)()
+    _check(lib().cgtp_profile_collect(ms, cnt))
+    return {lib().cgtp_profile_kind_name(k).decode(): (ms[k], cnt[k]) for k in range(n) if cnt[k]}

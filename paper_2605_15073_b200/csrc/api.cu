@@ -1,0 +1,470 @@
+// api.cu -- the C ABI of include/cgtp.h: argument validation, workspace carving, stage sequencing.
+#include <cstring>
+
+#include "common.cuh"
+
+namespace cgtp {
+const char* last_error();
+int64_t launch_count();
+void profile_enable(bool on);
+int profile_collect(double* ms, int64_t* launches);
+
+static const char* kKindNames[K_COUNT] = {
+    "proj_in",        "onsite_core_even", "onsite_core_odd", "proj_out",      "segments",      "node_synth_even",
+    "node_synth_odd", "edge_even",        "edge_odd",        "analysis_even", "analysis_odd",  "misc"};
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+struct Carver {
+    char* base;
+    size_t off;
+    explicit Carver(void* b) : base(static_cast<char*>(b)), off(0) {}
+    template <class T>
+    T* take(size_t count)
+    {
+        T* p = reinterpret_cast<T*>(base + off);
+        off = align_up(off + count * sizeof(T), 256);
+        return p;
+    }
+};
+
+static int check_common(int lmax, int lmax_out, int N, int C, const uint8_t* mask)
+{
+    if (lmax < 0 || lmax_out < 0 || lmax_out > 2 * lmax) {
+        set_error("invalid band limits lmax=%d lmax_out=%d (need 0 <= lmax_out <= 2*lmax)", lmax, lmax_out);
+        return CGTP_ERR_INVALID;
+    }
+    if (N <= 0 || C <= 0) { set_error("N and C must be positive (N=%d, C=%d)", N, C); return CGTP_ERR_INVALID; }
+    if (C > 1024) { set_error("C=%d exceeds the compiled limit 1024", C); return CGTP_ERR_UNSUPPORTED; }
+    if (kernel_band(lmax > lmax_out ? lmax : lmax_out) < 0) {
+        set_error("band limit max(lmax,lmax_out)=%d exceeds cgtp_max_lmax()=%d", lmax > lmax_out ? lmax : lmax_out, kMaxBand);
+        return CGTP_ERR_UNSUPPORTED;
+    }
+    if (!mask) { set_error("parity_mask is NULL"); return CGTP_ERR_INVALID; }
+    for (int c = 0; c < C; ++c)
+        if (mask[c] > 1) { set_error("parity_mask[%d]=%d is not 0 or 1", c, (int)mask[c]); return CGTP_ERR_INVALID; }
+    return CGTP_OK;
+}
+
+static size_t onsite_ws_bytes(int lmax, int lmax_out, int C, int64_t batch)
+{
+    const size_t L2p = round_up((lmax + 1) * (lmax + 1), 4), Lo2p = round_up((lmax_out + 1) * (lmax_out + 1), 4);
+    return (size_t)batch * C * (2 * L2p + Lo2p) * sizeof(float) + 8 * 256;
+}
+
+static size_t message_ws_bytes(int lmax, int lmax_out, int C, int Co, int64_t nodes)
+{
+    const size_t L2p = round_up((lmax + 1) * (lmax + 1), 4), Lo2p = round_up((lmax_out + 1) * (lmax_out + 1), 4);
+    const int U = (2 * lmax + lmax_out + 2) / 2, V = 2 * lmax + lmax_out + 1;
+    const size_t UVp = round_up(U * V, 4);
+    size_t fl = (size_t)nodes * C * (L2p + Lo2p) + (size_t)nodes * (C + Co) * UVp + (size_t)nodes * C * UVp;
+    return 256 + fl * sizeof(float) + (size_t)(nodes + 1) * sizeof(int64_t) + 12 * 256;
+}
+
+}  // namespace cgtp
+
+using namespace cgtp;
+
+extern "C" {
+
+int cgtp_version(void) { return 100; }
+const char* cgtp_last_error(void) { return cgtp::last_error(); }
+int cgtp_max_lmax(void) { return kMaxBand; }
+
+int cgtp_grid_shape(int lmax, int lmax_out, int* U, int* V)
+{
+    if (lmax < 0 || lmax_out < 0 || lmax_out > 2 * lmax) { set_error("invalid band limits"); return CGTP_ERR_INVALID; }
+    if (U) *U = (2 * lmax + lmax_out + 2) / 2;
+    if (V) *V = 2 * lmax + lmax_out + 1;
+    return CGTP_OK;
+}
+
+size_t cgtp_onsite_workspace_bytes(int lmax, int lmax_out, int N, int C, int64_t batch)
+{
+    (void)N;
+    if (lmax < 0 || lmax_out < 0 || C <= 0 || batch < 0) return 0;
+    return onsite_ws_bytes(lmax, lmax_out, C, batch);
+}
+
+int cgtp_onsite(const float* A, const float* B, const float* W_a, const float* W_b, const float* W_out, int lmax,
+                int lmax_out, int N, int C, const uint8_t* parity_mask, float* out, int64_t batch, void* workspace,
+                size_t workspace_bytes, void* cuda_stream)
+{
+    clear_error();
+    int rc = check_common(lmax, lmax_out, N, C, parity_mask);
+    if (rc) return rc;
+    if (batch < 0) { set_error("negative batch"); return CGTP_ERR_INVALID; }
+    if (batch == 0) return CGTP_OK;
+    if (!A || !B || !W_a || !W_b || !W_out || !out || !workspace) { set_error("null pointer argument"); return CGTP_ERR_INVALID; }
+    if (!aligned16(A) || !aligned16(B) || !aligned16(out) || !aligned16(W_a) || !aligned16(W_b) || !aligned16(W_out) ||
+        (reinterpret_cast<uintptr_t>(workspace) & 255u)) {
+        set_error("misaligned pointer (tensors need 16-byte, workspace 256-byte alignment)");
+        return CGTP_ERR_INVALID;
+    }
+    if (workspace_bytes < onsite_ws_bytes(lmax, lmax_out, C, batch)) {
+        set_error("workspace too small: %zu < %zu bytes", workspace_bytes, onsite_ws_bytes(lmax, lmax_out, C, batch));
+        return CGTP_ERR_INVALID;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const Plan* p = get_plan(lmax, lmax_out);
+    if (!p) return CGTP_ERR_CUDA;
+    const ChannelPlan* cp = get_channel_plan(C, parity_mask);
+    if (!cp) return CGTP_ERR_CUDA;
+    const int Ce = cp->Ce, Co = cp->Co;
+
+    Carver cv(workspace);
+    float* Ha_e = cv.take<float>((size_t)batch * Ce * p->L2p);
+    float* Ha_o = cv.take<float>((size_t)batch * Co * p->L2p);
+    float* Hb_e = cv.take<float>((size_t)batch * Ce * p->L2p);
+    float* Hb_o = cv.take<float>((size_t)batch * Co * p->L2p);
+    float* T_e = cv.take<float>((size_t)batch * Ce * p->Lo2p);
+    float* T_o = cv.take<float>((size_t)batch * Co * p->Lo2p);
+
+    // S1: H = W . A (Eq.(35)); rows are written in parity-sorted channel order, even block then odd block
+    ProjArgs pin[2];
+    for (int s = 0; s < 2; ++s) {
+        ProjArgs& a = pin[s];
+        a.X = s ? B : A;
+        a.x_bs = (int64_t)N * p->L2;
+        a.x_rs = p->L2;
+        a.W = s ? W_b : W_a;
+        a.ldw_m = N;
+        a.ldw_k = 1;
+        a.idx_m = cp->perm_dev;
+        a.idx_k = nullptr;
+        a.M = C;
+        a.K = N;
+        a.J = p->L2;
+        a.out0 = s ? Hb_e : Ha_e;
+        a.o_bs0 = (int64_t)Ce * p->L2p;
+        a.out1 = s ? Hb_o : Ha_o;
+        a.o_bs1 = (int64_t)Co * p->L2p;
+        a.m_split = Ce;
+        a.o_rs = p->L2p;
+        a.batch = batch;
+    }
+    rc = launch_proj(pin, 2, K_PROJ_IN, st);
+    if (rc) return rc;
+
+    // S2-S4 fused, one launch per parity
+    rc = launch_onsite_core(p, false, Ha_e, Hb_e, T_e, batch * Ce, st);
+    if (rc) return rc;
+    rc = launch_onsite_core(p, true, Ha_o, Hb_o, T_o, batch * Co, st);
+    if (rc) return rc;
+
+    // S5: out[b, s] = W_out[:, channels of sector s] . T_s (Eq.(41))
+    ProjArgs po[2];
+    for (int s = 0; s < 2; ++s) {
+        ProjArgs& a = po[s];
+        a.X = s ? T_o : T_e;
+        a.x_bs = (int64_t)(s ? Co : Ce) * p->Lo2p;
+        a.x_rs = p->Lo2p;
+        a.W = W_out;
+        a.ldw_m = C;
+        a.ldw_k = 1;
+        a.idx_m = nullptr;
+        a.idx_k = cp->perm_dev + (s ? Ce : 0);
+        a.M = N;
+        a.K = s ? Co : Ce;
+        a.J = p->Lo2;
+        a.out0 = out + (size_t)s * N * p->Lo2;
+        a.o_bs0 = (int64_t)2 * N * p->Lo2;
+        a.out1 = a.out0;
+        a.o_bs1 = a.o_bs0;
+        a.m_split = N;
+        a.o_rs = p->Lo2;
+        a.batch = batch;
+    }
+    return launch_proj(po, 2, K_PROJ_OUT, st);
+}
+
+size_t cgtp_message_workspace_bytes(int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask, int64_t nodes,
+                                    int64_t E)
+{
+    (void)N;
+    (void)E;
+    if (lmax < 0 || lmax_out < 0 || C <= 0 || nodes < 0 || !parity_mask) return 0;
+    int Co = 0;
+    for (int c = 0; c < C; ++c) Co += parity_mask[c] ? 1 : 0;
+    return message_ws_bytes(lmax, lmax_out, C, Co, nodes);
+}
+
+int cgtp_build_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int64_t* row_ptr, int32_t* status,
+                        void* cuda_stream)
+{
+    clear_error();
+    if (E < 0 || nodes < 0) { set_error("negative size"); return CGTP_ERR_INVALID; }
+    if ((!edge_index && E > 0) || !row_ptr || !status) { set_error("null pointer argument"); return CGTP_ERR_INVALID; }
+    return launch_segments(edge_index, E, nodes, row_ptr, status, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int cgtp_message(const float* node_feats, const int64_t* edge_index, const float* edge_vec, const float* edge_radial,
+                 const float* W_node, const float* W_out, int lmax, int lmax_out, int N, int C,
+                 const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* workspace,
+                 size_t workspace_bytes, void* cuda_stream)
+{
+    clear_error();
+    int rc = check_common(lmax, lmax_out, N, C, parity_mask);
+    if (rc) return rc;
+    if (nodes < 0 || E < 0) { set_error("negative size"); return CGTP_ERR_INVALID; }
+    if (nodes == 0) return CGTP_OK;
+    if (!node_feats || !W_node || !W_out || !out || !workspace || (E > 0 && (!edge_index || !edge_vec || !edge_radial))) {
+        set_error("null pointer argument");
+        return CGTP_ERR_INVALID;
+    }
+    if (!aligned16(node_feats) || !aligned16(out) || !aligned16(W_node) || !aligned16(W_out) ||
+        (E > 0 && (!aligned16(edge_index) || !aligned16(edge_vec) || !aligned16(edge_radial))) ||
+        (reinterpret_cast<uintptr_t>(workspace) & 255u)) {
+        set_error("misaligned pointer (tensors need 16-byte, workspace 256-byte alignment)");
+        return CGTP_ERR_INVALID;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const Plan* p = get_plan(lmax, lmax_out);
+    if (!p) return CGTP_ERR_CUDA;
+    const ChannelPlan* cp = get_channel_plan(C, parity_mask);
+    if (!cp) return CGTP_ERR_CUDA;
+    const int Ce = cp->Ce, Co = cp->Co;
+    if (workspace_bytes < message_ws_bytes(lmax, lmax_out, C, Co, nodes)) {
+        set_error("workspace too small: %zu < %zu bytes", workspace_bytes, message_ws_bytes(lmax, lmax_out, C, Co, nodes));
+        return CGTP_ERR_INVALID;
+    }
+
+    Carver cv(workspace);
+    int32_t* status = cv.take<int32_t>(1);
+    int64_t* row_ptr = cv.take<int64_t>((size_t)nodes + 1);
+    float* H_e = cv.take<float>((size_t)nodes * Ce * p->L2p);
+    float* H_o = cv.take<float>((size_t)nodes * Co * p->L2p);
+    float* G_e = cv.take<float>((size_t)nodes * Ce * p->UVp);
+    float* G_o = cv.take<float>((size_t)nodes * Co * 2 * p->UVp);
+    float* S_e = cv.take<float>((size_t)nodes * Ce * p->UVp);
+    float* S_o = cv.take<float>((size_t)nodes * Co * p->UVp);
+    float* T_e = cv.take<float>((size_t)nodes * Ce * p->Lo2p);
+    float* T_o = cv.take<float>((size_t)nodes * Co * p->Lo2p);
+
+    // M0
+    rc = launch_segments(edge_index, E, nodes, row_ptr, status, st);
+    if (rc) return rc;
+
+    // M1: H = W_node . node_feats (Eq.(47))
+    ProjArgs a;
+    a.X = node_feats;
+    a.x_bs = (int64_t)N * p->L2;
+    a.x_rs = p->L2;
+    a.W = W_node;
+    a.ldw_m = N;
+    a.ldw_k = 1;
+    a.idx_m = cp->perm_dev;
+    a.idx_k = nullptr;
+    a.M = C;
+    a.K = N;
+    a.J = p->L2;
+    a.out0 = H_e;
+    a.o_bs0 = (int64_t)Ce * p->L2p;
+    a.out1 = H_o;
+    a.o_bs1 = (int64_t)Co * p->L2p;
+    a.m_split = Ce;
+    a.o_rs = p->L2p;
+    a.batch = nodes;
+    rc = launch_proj(&a, 1, K_PROJ_IN, st);
+    if (rc) return rc;
+
+    // M2
+    rc = launch_node_synth(p, false, H_e, G_e, nodes * Ce, st);
+    if (rc) return rc;
+    rc = launch_node_synth(p, true, H_o, G_o, nodes * Co, st);
+    if (rc) return rc;
+
+    // M3 + M4
+    rc = launch_edge(p, false, G_e, row_ptr, edge_index, E, edge_vec, edge_radial, cp->perm_dev, Ce, C, S_e, nodes, status, st);
+    if (rc) return rc;
+    rc = launch_edge(p, true, G_o, row_ptr, edge_index, E, edge_vec, edge_radial, cp->perm_dev + Ce, Co, C, S_o, nodes, status, st);
+    if (rc) return rc;
+
+    // M5
+    rc = launch_analysis(p, false, S_e, T_e, nodes * Ce, st);
+    if (rc) return rc;
+    rc = launch_analysis(p, true, S_o, T_o, nodes * Co, st);
+    if (rc) return rc;
+
+    // M6
+    ProjArgs po[2];
+    for (int s = 0; s < 2; ++s) {
+        ProjArgs& b = po[s];
+        b.X = s ? T_o : T_e;
+        b.x_bs = (int64_t)(s ? Co : Ce) * p->Lo2p;
+        b.x_rs = p->Lo2p;
+        b.W = W_out;
+        b.ldw_m = C;
+        b.ldw_k = 1;
+        b.idx_m = nullptr;
+        b.idx_k = cp->perm_dev + (s ? Ce : 0);
+        b.M = N;
+        b.K = s ? Co : Ce;
+        b.J = p->Lo2;
+        b.out0 = out + (size_t)s * N * p->Lo2;
+        b.o_bs0 = (int64_t)2 * N * p->Lo2;
+        b.out1 = b.out0;
+        b.o_bs1 = b.o_bs0;
+        b.m_split = N;
+        b.o_rs = p->Lo2;
+        b.batch = nodes;
+    }
+    return launch_proj(po, 2, K_PROJ_OUT, st);
+}
+
+int cgtp_message_status(const void* workspace, void* cuda_stream)
+{
+    clear_error();
+    if (!workspace) { set_error("null workspace"); return CGTP_ERR_INVALID; }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    CGTP_CUDA_CHECK(cudaStreamSynchronize(st));
+    int32_t h = 0;
+    CGTP_CUDA_CHECK(cudaMemcpy(&h, workspace, sizeof h, cudaMemcpyDeviceToHost));
+    if (h != 0) {
+        set_error("edge_index is not receiver-sorted or has an index outside [0, nodes)");
+        return CGTP_ERR_GRAPH;
+    }
+    return CGTP_OK;
+}
+
+// ------------------------------------------------------------------------------ host-buffer entry points
+int cgtp_onsite_host(const float* A, const float* B, const float* W_a, const float* W_b, const float* W_out, int lmax,
+                     int lmax_out, int N, int C, const uint8_t* parity_mask, float* out, int64_t batch,
+                     void* cuda_stream)
+{
+    clear_error();
+    int rc = check_common(lmax, lmax_out, N, C, parity_mask);
+    if (rc) return rc;
+    if (batch < 0) { set_error("negative batch"); return CGTP_ERR_INVALID; }
+    if (batch == 0) return CGTP_OK;
+    if (!A || !B || !W_a || !W_b || !W_out || !out) { set_error("null pointer argument"); return CGTP_ERR_INVALID; }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t L2 = (size_t)(lmax + 1) * (lmax + 1), Lo2 = (size_t)(lmax_out + 1) * (lmax_out + 1);
+    const size_t wbytes = (size_t)C * N * 4;
+    float *dWa = nullptr, *dWb = nullptr, *dWo = nullptr;
+    CGTP_CUDA_CHECK(cudaMallocAsync(&dWa, wbytes, st));
+    CGTP_CUDA_CHECK(cudaMallocAsync(&dWb, wbytes, st));
+    CGTP_CUDA_CHECK(cudaMallocAsync(&dWo, wbytes, st));
+    CGTP_CUDA_CHECK(cudaMemcpyAsync(dWa, W_a, wbytes, cudaMemcpyHostToDevice, st));
+    CGTP_CUDA_CHECK(cudaMemcpyAsync(dWb, W_b, wbytes, cudaMemcpyHostToDevice, st));
+    CGTP_CUDA_CHECK(cudaMemcpyAsync(dWo, W_out, wbytes, cudaMemcpyHostToDevice, st));
+
+    // Batch chunks on two streams so the H2D copy of chunk k+1, the kernels of chunk k and the D2H copy
+    // of chunk k-1 overlap (PCIe is full duplex).
+    const size_t in_per = (size_t)N * L2 * 4, out_per = (size_t)2 * N * Lo2 * 4;
+    int64_t chunk = (int64_t)((64u << 20) / (in_per > 0 ? in_per : 1));
+    if (chunk < 1) chunk = 1;
+    if (chunk > batch) chunk = batch;
+    const int NS = 2;
+    cudaStream_t cs[NS];
+    cudaEvent_t ready, done[NS];
+    CGTP_CUDA_CHECK(cudaEventCreateWithFlags(&ready, cudaEventDisableTiming));
+    CGTP_CUDA_CHECK(cudaEventRecord(ready, st));
+    float *dA[NS], *dB[NS], *dO[NS];
+    void* dws[NS];
+    const size_t wsb = onsite_ws_bytes(lmax, lmax_out, C, chunk);
+    for (int s = 0; s < NS; ++s) {
+        CGTP_CUDA_CHECK(cudaStreamCreateWithFlags(&cs[s], cudaStreamNonBlocking));
+        CGTP_CUDA_CHECK(cudaEventCreateWithFlags(&done[s], cudaEventDisableTiming));
+        CGTP_CUDA_CHECK(cudaStreamWaitEvent(cs[s], ready, 0));
+        CGTP_CUDA_CHECK(cudaMallocAsync(&dA[s], chunk * in_per, cs[s]));
+        CGTP_CUDA_CHECK(cudaMallocAsync(&dB[s], chunk * in_per, cs[s]));
+        CGTP_CUDA_CHECK(cudaMallocAsync(&dO[s], chunk * out_per, cs[s]));
+        CGTP_CUDA_CHECK(cudaMallocAsync(&dws[s], wsb, cs[s]));
+    }
+    int k = 0;
+    for (int64_t b0 = 0; b0 < batch; b0 += chunk, ++k) {
+        const int s = k % NS;
+        const int64_t nb = (batch - b0 < chunk) ? (batch - b0) : chunk;
+        CGTP_CUDA_CHECK(cudaMemcpyAsync(dA[s], A + (size_t)b0 * N * L2, nb * in_per, cudaMemcpyHostToDevice, cs[s]));
+        CGTP_CUDA_CHECK(cudaMemcpyAsync(dB[s], B + (size_t)b0 * N * L2, nb * in_per, cudaMemcpyHostToDevice, cs[s]));
+        rc = cgtp_onsite(dA[s], dB[s], dWa, dWb, dWo, lmax, lmax_out, N, C, parity_mask, dO[s], nb, dws[s], wsb, cs[s]);
+        if (rc) return rc;
+        CGTP_CUDA_CHECK(cudaMemcpyAsync(out + (size_t)b0 * 2 * N * Lo2, dO[s], nb * out_per, cudaMemcpyDeviceToHost, cs[s]));
+    }
+    for (int s = 0; s < NS; ++s) {
+        CGTP_CUDA_CHECK(cudaFreeAsync(dA[s], cs[s]));
+        CGTP_CUDA_CHECK(cudaFreeAsync(dB[s], cs[s]));
+        CGTP_CUDA_CHECK(cudaFreeAsync(dO[s], cs[s]));
+        CGTP_CUDA_CHECK(cudaFreeAsync(dws[s], cs[s]));
+        CGTP_CUDA_CHECK(cudaEventRecord(done[s], cs[s]));
+        CGTP_CUDA_CHECK(cudaStreamWaitEvent(st, done[s], 0));
+    }
+    CGTP_CUDA_CHECK(cudaFreeAsync(dWa, st));
+    CGTP_CUDA_CHECK(cudaFreeAsync(dWb, st));
+    CGTP_CUDA_CHECK(cudaFreeAsync(dWo, st));
+    CGTP_CUDA_CHECK(cudaStreamSynchronize(st));
+    for (int s = 0; s < NS; ++s) {
+        cudaStreamDestroy(cs[s]);
+        cudaEventDestroy(done[s]);
+    }
+    cudaEventDestroy(ready);
+    return CGTP_OK;
+}
+
+int cgtp_message_host(const float* node_feats, const int64_t* edge_index, const float* edge_vec,
+                      const float* edge_radial, const float* W_node, const float* W_out, int lmax, int lmax_out, int N,
+                      int C, const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* cuda_stream)
+{
+    clear_error();
+    int rc = check_common(lmax, lmax_out, N, C, parity_mask);
+    if (rc) return rc;
+    if (nodes < 0 || E < 0) { set_error("negative size"); return CGTP_ERR_INVALID; }
+    if (nodes == 0) return CGTP_OK;
+    if (!node_feats || !W_node || !W_out || !out || (E > 0 && (!edge_index || !edge_vec || !edge_radial))) {
+        set_error("null pointer argument");
+        return CGTP_ERR_INVALID;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t L2 = (size_t)(lmax + 1) * (lmax + 1), Lo2 = (size_t)(lmax_out + 1) * (lmax_out + 1);
+    const size_t xb = (size_t)nodes * N * L2 * 4, ob = (size_t)nodes * 2 * N * Lo2 * 4, wb = (size_t)C * N * 4;
+    const size_t eib = (size_t)2 * (E > 0 ? E : 1) * 8, evb = (size_t)(E > 0 ? E : 1) * 3 * 4, erb = (size_t)(E > 0 ? E : 1) * C * 4;
+    const size_t wsb = cgtp_message_workspace_bytes(lmax, lmax_out, N, C, parity_mask, nodes, E);
+    float *dX, *dO, *dWn, *dWo, *dEv, *dEr;
+    int64_t* dEi;
+    void* dws;
+    CGTP_CUDA_CHECK(cudaMallocAsync(&dX, xb, st));
+    CGTP_CUDA_CHECK(cudaMallocAsync(&dO, ob, st));
+    CGTP_CUDA_CHECK(cudaMallocAsync(&dWn, wb, st));
+    CGTP_CUDA_CHECK(cudaMallocAsync(&dWo, wb, st));
+    CGTP_CUDA_CHECK(cudaMallocAsync(&dEi, eib, st));
+    CGTP_CUDA_CHECK(cudaMallocAsync(&dEv, evb, st));
+    CGTP_CUDA_CHECK(cudaMallocAsync(&dEr, erb, st));
+    CGTP_CUDA_CHECK(cudaMallocAsync(&dws, wsb, st));
+    CGTP_CUDA_CHECK(cudaMemcpyAsync(dX, node_feats, xb, cudaMemcpyHostToDevice, st));
+    CGTP_CUDA_CHECK(cudaMemcpyAsync(dWn, W_node, wb, cudaMemcpyHostToDevice, st));
+    CGTP_CUDA_CHECK(cudaMemcpyAsync(dWo, W_out, wb, cudaMemcpyHostToDevice, st));
+    if (E > 0) {
+        CGTP_CUDA_CHECK(cudaMemcpyAsync(dEi, edge_index, (size_t)2 * E * 8, cudaMemcpyHostToDevice, st));
+        CGTP_CUDA_CHECK(cudaMemcpyAsync(dEv, edge_vec, (size_t)E * 3 * 4, cudaMemcpyHostToDevice, st));
+        CGTP_CUDA_CHECK(cudaMemcpyAsync(dEr, edge_radial, (size_t)E * C * 4, cudaMemcpyHostToDevice, st));
+    }
+    rc = cgtp_message(dX, dEi, dEv, dEr, dWn, dWo, lmax, lmax_out, N, C, parity_mask, dO, nodes, E, dws, wsb, st);
+    if (rc) return rc;
+    CGTP_CUDA_CHECK(cudaMemcpyAsync(out, dO, ob, cudaMemcpyDeviceToHost, st));
+    int grc = cgtp_message_status(dws, st);
+    CGTP_CUDA_CHECK(cudaFreeAsync(dX, st));
+    CGTP_CUDA_CHECK(cudaFreeAsync(dO, st));
+    CGTP_CUDA_CHECK(cudaFreeAsync(dWn, st));
+    CGTP_CUDA_CHECK(cudaFreeAsync(dWo, st));
+    CGTP_CUDA_CHECK(cudaFreeAsync(dEi, st));
+    CGTP_CUDA_CHECK(cudaFreeAsync(dEv, st));
+    CGTP_CUDA_CHECK(cudaFreeAsync(dEr, st));
+    CGTP_CUDA_CHECK(cudaFreeAsync(dws, st));
+    CGTP_CUDA_CHECK(cudaStreamSynchronize(st));
+    return grc;
+}
+
+// ------------------------------------------------------------------------------------ instrumentation
+int64_t cgtp_launch_count(void) { return cgtp::launch_count(); }
+int cgtp_profile_kinds(void) { return K_COUNT; }
+const char* cgtp_profile_kind_name(int kind) { return (kind >= 0 && kind < K_COUNT) ? kKindNames[kind] : ""; }
+int cgtp_profile_enable(int on)
+{
+    cgtp::profile_enable(on != 0);
+    return CGTP_OK;
+}
+int cgtp_profile_collect(double* ms, int64_t* launches) { return cgtp::profile_collect(ms, launches); }
+
+}  // extern "C"

@@ -1,0 +1,156 @@
+// common.cuh -- shared host/device declarations of libcgtp (sm_100a only).
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <cstdio>
+
+#include "../../include/cgtp.h"
+
+namespace cgtp {
+
+// Band limits with a compiled kernel instantiation; max(lmax, lmax_out) is rounded up to the next one
+// (the extra coefficient rows are zero).  CGTP_FOR_EACH_BAND(X) expands X(LB) for each of them.
+#define CGTP_FOR_EACH_BAND(X) X(1) X(2) X(3) X(4) X(5) X(6) X(8) X(10) X(12) X(16) X(20)
+constexpr int kMaxBand = 20;
+inline int kernel_band(int b)
+{
+    const int bands[] = {1, 2, 3, 4, 5, 6, 8, 10, 12, 16, 20};
+    for (int v : bands)
+        if (b <= v) return v;
+    return -1;
+}
+
+__host__ __device__ constexpr int round_up(int x, int m) { return (x + m - 1) / m * m; }
+__host__ __device__ constexpr int tri_index(int l, int m) { return l * (l + 1) / 2 + m; }
+
+// ---------------------------------------------------------------------------------------------
+// Plan: quadrature grid + FP32 device tables for one (lmax, lmax_out).  Built once in FP64 on the
+// host (tables.cu), cached for the life of the process.
+//
+// Grid (R8): U Gauss-Legendre nodes x_u = cos(theta_u) (u = 0 is the
+// northernmost, x_{U-1-u} = -x_u), V azimuths phi_v = 2 pi v / V.
+// Folding: only the northern half u' < Uh = ceil(U/2) of the Legendre tables and only
+// v' < Vh = V/2 + 1 of the Fourier tables are stored; the southern / mirrored halves follow from
+// P~_l^m(-x) = (-1)^(l+m) P~_l^m(x) and cos/sin(m (2pi - phi)).
+// ---------------------------------------------------------------------------------------------
+struct Plan {
+    int lmax, lmax_out;
+    int LB;    // kernel band limit = kernel_band(max(lmax, lmax_out)); tables cover 0 <= m <= l <= LB
+    int U, V;  // grid
+    int Uh, Vh;
+    int UV, UVp;  // U*V and U*V rounded up to a multiple of 4 floats (16 bytes)
+    int NTRI;     // (LB+1)(LB+2)/2 rounded up to a multiple of 4: row length of the Legendre tables
+    int QSTR;     // LB+1 rounded up to a multiple of 4: row length of the Fourier tables
+    int L2, L2p, Lo2, Lo2p;  // (lmax+1)^2, (lmax_out+1)^2 and their multiples of 4
+    // Legendre tables, [Uh][NTRI], entry tri_index(l,m):
+    const float* PT;  // P~_l^m(x_u)                          (p_ulm of Eq.(22))
+    const float* DT;  // d/dtheta P~_l^m(cos theta) at theta_u (theta-form of d_x p_ulm, :445)
+    const float* ST;  // m P~_l^m(x_u) / sin(theta_u)         ((1/sin theta) d_phi of Eq.(11), :107)
+    const float* WP;  // w_u P~_l^m(x_u), equator row halved  (Eq.(40), :342)
+    // Fourier tables (real form, Eq.(C2) :668), [Vh][QSTR]:
+    const float* QC;  // QC[v'][0] = 1, QC[v'][m] = sqrt2 cos(m phi_v')
+    const float* QS;  // QS[v'][m] = sqrt2 sin(m phi_v'), zero for m = 0 and for self-mirrored v'
+    const float* WV;  // [round_up(Vh,4)]: (2 pi / V), halved for self-mirrored v'   (Eq.(39), :339)
+    // Grid geometry for the edge factor, [8][UVp]: Omega_xyz, theta_hat_xyz, phi_hat_xy (zero padded)
+    const float* geo;
+};
+
+// Returns the cached plan, creating it on first use (cudaMalloc + blocking copies, once).
+// nullptr + cgtp_last_error on failure.
+const Plan* get_plan(int lmax, int lmax_out);
+
+// ---------------------------------------------------------------------------------------------
+// Channel plan: parity_mask -> permutation that lists the even channels first (stable).
+// ---------------------------------------------------------------------------------------------
+struct ChannelPlan {
+    int C, Ce, Co;
+    const int* perm_dev;  // device [C]: perm[k] = original channel index of sorted position k
+    int perm_host[1024];
+};
+const ChannelPlan* get_channel_plan(int C, const uint8_t* parity_mask);
+
+// ---------------------------------------------------------------------------------------------
+// Errors, launch accounting, profiling
+// ---------------------------------------------------------------------------------------------
+void set_error(const char* fmt, ...);
+void clear_error();
+
+enum Kind {
+    K_PROJ_IN = 0,
+    K_ONSITE_EVEN,
+    K_ONSITE_ODD,
+    K_PROJ_OUT,
+    K_SEGMENTS,
+    K_NODE_SYNTH_EVEN,
+    K_NODE_SYNTH_ODD,
+    K_EDGE_EVEN,
+    K_EDGE_ODD,
+    K_ANALYSIS_EVEN,
+    K_ANALYSIS_ODD,
+    K_MISC,
+    K_COUNT
+};
+
+// RAII around one kernel launch: counts it and, when profiling is on, brackets it with events.
+struct LaunchScope {
+    LaunchScope(Kind kind, cudaStream_t stream);
+    ~LaunchScope();
+    Kind kind;
+    cudaStream_t stream;
+    void* rec;
+};
+
+#define CGTP_CUDA_CHECK(expr)                                                                    \
+    do {                                                                                         \
+        cudaError_t _e = (expr);                                                                 \
+        if (_e != cudaSuccess) {                                                                 \
+            ::cgtp::set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
+            return CGTP_ERR_CUDA;                                                                \
+        }                                                                                        \
+    } while (0)
+
+// ---------------------------------------------------------------------------------------------
+// Stage launchers (one per row of SURVEY.md 8(a)); all asynchronous on `st`.
+// ---------------------------------------------------------------------------------------------
+
+// S1/S5/M1/M6: Out[b][m][j] = sum_{kk<K} W[widx_m(m)*ldw_m + widx_k(kk)*ldw_k] * X[b*x_bs + kk*x_rs + j]
+// for j < J.  Rows m < m_split go to out0 + b*o_bs0 + m*o_rs, rows m >= m_split to
+// out1 + b*o_bs1 + (m-m_split)*o_rs.  idx arrays may be nullptr (identity).
+struct ProjArgs {
+    const float* X;
+    int64_t x_bs;
+    int x_rs;
+    const float* W;
+    int ldw_m, ldw_k;
+    const int* idx_m;
+    const int* idx_k;
+    int M, K, J;
+    float* out0;
+    int64_t o_bs0;
+    float* out1;
+    int64_t o_bs1;
+    int m_split;
+    int o_rs;
+    int64_t batch;
+};
+int launch_proj(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st);
+
+// S2-S4 fused: T[col][lm] from Ha[col], Hb[col]; ncols columns of one parity.
+int launch_onsite_core(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols,
+                       cudaStream_t st);
+
+// M0
+int launch_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int64_t* row_ptr, int32_t* status,
+                    cudaStream_t st);
+// M2: grid fields of the projected node features.  even: G[col][UVp]; odd: G[col][2][UVp] (d_theta, (1/sin)d_phi)
+int launch_node_synth(const Plan* p, bool odd, const float* H, float* G, int64_t ncols, cudaStream_t st);
+// M3+M4: S[i][kc][UVp] = sum_e radial * edge-field (x) sender grid, channels of one parity.
+int launch_edge(const Plan* p, bool odd, const float* G, const int64_t* row_ptr, const int64_t* edge_index,
+                int64_t E, const float* edge_vec, const float* edge_radial, const int* perm_par, int Cpar, int C,
+                float* S, int64_t nodes, const int32_t* status, cudaStream_t st);
+// M5: T[col][Lo2p] = analysis of S[col][UVp]
+int launch_analysis(const Plan* p, bool odd, const float* S, float* T, int64_t ncols, cudaStream_t st);
+
+}  // namespace cgtp

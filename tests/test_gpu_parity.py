@@ -1,0 +1,302 @@
+"""Parity of the CUDA path (through the C ABI, via paper_2605_15073_b200.binding) against the FP64 oracle.
+
+Bar (BASELINE.json north_star; R14): per parity sector, max|out - ref| / max|ref| <= 1e-5 for
+FP32; indexing / segmentation bit-exact.  All inputs are seeded and synthetic (synthetic.py).
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import cgtp_oracle as orc
+from paper_2605_15073_b200 import binding as cg
+from paper_2605_15073_b200 import synthetic
+from tests import shref
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5
+
+
+def _cuda(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def sector_err(got, ref):
+    got = np.asarray(got, np.float64)
+    errs = []
+    for s in (0, 1):
+        d = np.abs(got[:, s] - ref[:, s]).max() if got.size else 0.0
+        m = np.abs(ref[:, s]).max() if ref.size else 0.0
+        errs.append(d / m if m > 0 else d)
+    return errs
+
+
+def run_onsite(inp, **kw):
+    out = cg.cgtp_onsite(_cuda(inp.A), _cuda(inp.B), _cuda(inp.W_a), _cuda(inp.W_b), _cuda(inp.W_out),
+                         inp.lmax, inp.lmax_out, inp.N, inp.C, inp.parity_mask, **kw)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def run_message(m, **kw):
+    out = cg.cgtp_message(_cuda(m.node_feats), _cuda(m.edge_index), _cuda(m.edge_vec), _cuda(m.edge_radial),
+                          _cuda(m.W_node), _cuda(m.W_out), m.lmax, m.lmax_out, m.N, m.C, m.parity_mask, **kw)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def oracle_onsite(inp, idx=None):
+    A, B = (inp.A, inp.B) if idx is None else (inp.A[idx], inp.B[idx])
+    return orc.onsite(A, B, inp.W_a, inp.W_b, inp.W_out, inp.lmax, inp.lmax_out, inp.parity_mask)
+
+
+def oracle_message(m, recv=None):
+    return orc.message(m.node_feats, m.edge_index, m.edge_vec, m.edge_radial, m.W_node, m.W_out, m.lmax, m.lmax_out,
+                       m.parity_mask, recv)
+
+
+# ------------------------------------------------------------------------------------------ on-site
+def test_onsite_config0_full():
+    """BASELINE.json configs[0]: lmax=2, N=8, C=8, batch=64, even+odd, seed 0."""
+    inp = synthetic.config(0)
+    got, ref = run_onsite(inp), oracle_onsite(inp)
+    e = sector_err(got, ref)
+    assert max(e) < TOL, e
+    assert np.abs(ref[:, 1, :, 0]).max() == 0.0 and np.abs(got[:, 1, :, 0]).max() < 1e-6  # odd sector: no l=0
+
+
+@pytest.mark.parametrize("lmax,lmax_out,N,C,batch,mask", [
+    (0, 0, 4, 4, 3, [0, 1, 0, 1]),
+    (1, 1, 5, 6, 37, [0, 1, 1, 0, 1, 0]),
+    (1, 2, 4, 4, 9, [1, 0, 0, 1]),
+    (2, 4, 3, 5, 11, [1, 1, 0, 1, 0]),
+    (3, 3, 7, 9, 130, [0, 0, 1, 0, 1, 1, 1, 0, 0]),
+    (3, 5, 4, 4, 20, [0, 1, 0, 1]),
+    (4, 2, 6, 8, 33, [1, 0, 1, 0, 1, 0, 1, 0]),
+    (5, 5, 8, 8, 65, [0, 0, 0, 0, 1, 1, 1, 1]),
+    (7, 7, 4, 6, 19, [0, 1, 0, 1, 0, 1]),      # band 7 runs on the LB=8 instantiation
+    (9, 9, 4, 4, 7, [0, 0, 1, 1]),             # band 9 -> LB=10
+    (4, 4, 8, 8, 40, [0] * 8),                 # all even: sector 1 must be zero
+    (4, 4, 8, 8, 40, [1] * 8),                 # all odd: sector 0 must be zero
+    (6, 6, 40, 33, 50, None),                  # N, C not multiples of the GEMM tiles
+])
+def test_onsite_small_shapes(lmax, lmax_out, N, C, batch, mask):
+    inp = synthetic.make_onsite(lmax, lmax_out, N, C, batch, seed=100 + lmax * 7 + lmax_out, parity_mask=mask)
+    got, ref = run_onsite(inp), oracle_onsite(inp)
+    e = sector_err(got, ref)
+    assert max(e) < TOL, e
+    for s in (0, 1):
+        if np.abs(ref[:, s]).max() == 0.0:
+            assert np.abs(got[:, s]).max() == 0.0
+
+
+def test_onsite_config1_full():
+    """BASELINE.json configs[1] (the bench workload): lmax=6, N=C=64, batch=4096, every output checked."""
+    inp = synthetic.config(1)
+    got, ref = run_onsite(inp), oracle_onsite(inp)
+    e = sector_err(got, ref)
+    assert max(e) < TOL, e
+
+
+@pytest.mark.parametrize("lmax", [2, 4, 8, 12, 16, 20])
+def test_onsite_config3_sweep_sampled(lmax):
+    """BASELINE.json configs[3]: N=C=32, batch=16384 on the GPU; the oracle evaluates a deterministic
+    sample of atoms (first, last, strided, seeded random)."""
+    inp = synthetic.config(3, lmax=lmax)
+    got = run_onsite(inp)
+    n = {2: 512, 4: 512, 8: 256, 12: 128, 16: 64, 20: 48}[lmax]
+    rng = np.random.default_rng(lmax)
+    idx = np.unique(np.concatenate([[0, 1, inp.batch - 1, inp.batch - 2], np.arange(0, inp.batch, inp.batch // (n // 2)),
+                                    rng.integers(0, inp.batch, n // 2)]))
+    ref = oracle_onsite(inp, idx)
+    e = sector_err(got[idx], ref)
+    assert max(e) < TOL, e
+    assert np.isfinite(got).all()
+    # the whole batch has the same statistics as the checked sample (catches tiles that were never written)
+    assert abs(np.abs(got[:, 0]).mean() / np.abs(got[idx][:, 0]).mean() - 1) < 0.2
+
+
+def test_onsite_invariants_full_size():
+    """Properties that hold at any size, on the bench workload: exchange symmetry, self-coupled vanishing
+    (Eq.(27)) and bitwise run-to-run reproducibility."""
+    inp = synthetic.config(1)
+    A, B, Wa, Wb, Wo = map(_cuda, (inp.A, inp.B, inp.W_a, inp.W_b, inp.W_out))
+    f = lambda a, b, wa, wb: cg.cgtp_onsite(a, b, wa, wb, Wo, inp.lmax, inp.lmax_out, inp.N, inp.C, inp.parity_mask)
+    base = f(A, B, Wa, Wb).clone()
+    again = f(A, B, Wa, Wb)
+    assert torch.equal(base, again)
+    sw = f(B, A, Wb, Wa)
+    scale0, scale1 = base[:, 0].abs().max().item(), base[:, 1].abs().max().item()
+    assert (sw[:, 0] - base[:, 0]).abs().max().item() < TOL * scale0
+    assert (sw[:, 1] + base[:, 1]).abs().max().item() < TOL * scale1
+    selfc = f(A, A, Wa, Wa)
+    assert selfc[:, 1].abs().max().item() < TOL * scale1
+    assert selfc[:, 0].abs().max().item() > 0.1 * scale0
+
+
+def test_onsite_equivariance():
+    """R15: rotate A, B with the real Wigner-D of a random rotation; outputs rotate with D, per sector."""
+    lmax = 6
+    inp = synthetic.make_onsite(lmax, lmax, 16, 16, 64, seed=5)
+    base = run_onsite(inp).astype(np.float64)
+    R = shref.random_rotation(np.random.default_rng(17))
+    D = shref.wigner_D_real(lmax, R)
+    rot_in = synthetic.make_onsite(lmax, lmax, 16, 16, 64, seed=5)
+    rot_in.A = np.einsum("ab,...b->...a", D, inp.A.astype(np.float64)).astype(np.float32)
+    rot_in.B = np.einsum("ab,...b->...a", D, inp.B.astype(np.float64)).astype(np.float32)
+    rot = run_onsite(rot_in).astype(np.float64)
+    e = sector_err(rot, np.einsum("ab,...b->...a", D, base))
+    assert max(e) < TOL, e
+
+
+def test_onsite_host_entry_matches_device_entry():
+    inp = synthetic.make_onsite(4, 4, 16, 16, 3000, seed=9)
+    dev = run_onsite(inp)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    host = cg.cgtp_onsite_host(pin(inp.A), pin(inp.B), pin(inp.W_a), pin(inp.W_b), pin(inp.W_out), 4, 4, 16, 16,
+                               inp.parity_mask).numpy()
+    assert np.array_equal(dev, host)
+
+
+def test_onsite_argument_errors():
+    inp = synthetic.make_onsite(2, 2, 4, 4, 4, seed=1)
+    A, B, Wa, Wb, Wo = map(_cuda, (inp.A, inp.B, inp.W_a, inp.W_b, inp.W_out))
+    with pytest.raises(cg.CgtpError) as ei:
+        cg.cgtp_onsite(A, B, Wa, Wb, Wo, 2, 2, 4, 4, [0, 1, 2, 0])
+    assert ei.value.code == cg.ERR_INVALID
+    big = synthetic.make_onsite(2, 2, 4, 4, 1, seed=1)
+    with pytest.raises(cg.CgtpError) as ei:  # lmax_out > 2 lmax
+        cg.cgtp_onsite(A, B, Wa, Wb, Wo, 2, 5, 4, 4, big.parity_mask,
+                       out=torch.empty((4, 2, 4, 36), device="cuda"))
+    assert ei.value.code == cg.ERR_INVALID
+    with pytest.raises(cg.CgtpError) as ei:  # band limit above the compiled maximum
+        L2 = (cg.cgtp_max_lmax() + 2) ** 2
+        z = torch.zeros((1, 4, L2), device="cuda")
+        cg.cgtp_onsite(z, z, Wa, Wb, Wo, cg.cgtp_max_lmax() + 1, cg.cgtp_max_lmax() + 1, 4, 4, big.parity_mask)
+    assert ei.value.code == cg.ERR_UNSUPPORTED
+    with pytest.raises(TypeError):  # CPU tensors are refused: no CPU fallback
+        cg.cgtp_onsite(A.cpu(), B, Wa, Wb, Wo, 2, 2, 4, 4, inp.parity_mask)
+    empty = torch.zeros((0, 4, 9), device="cuda")
+    out = cg.cgtp_onsite(empty, empty, Wa, Wb, Wo, 2, 2, 4, 4, inp.parity_mask)
+    assert out.shape == (0, 2, 4, 9)
+
+
+# ------------------------------------------------------------------------------------- segmentation
+def test_segments_bit_exact_and_graph_errors():
+    rng = np.random.default_rng(0)
+    nodes = 1000
+    deg = rng.integers(0, 9, nodes)
+    deg[[0, 17, 999]] = 0
+    m = synthetic.make_message(2, 2, 4, 4, nodes, deg, seed=3)
+    rc, ref = orc.segments(m.edge_index, nodes)
+    assert rc == 0
+    row_ptr, status = cg.cgtp_build_segments(_cuda(m.edge_index), nodes)
+    assert status.item() == 0
+    assert np.array_equal(row_ptr.cpu().numpy(), ref)
+    # empty edge list
+    row_ptr, status = cg.cgtp_build_segments(torch.zeros((2, 0), dtype=torch.int64, device="cuda"), 5)
+    assert status.item() == 0 and np.array_equal(row_ptr.cpu().numpy(), np.zeros(6, np.int64))
+    # unsorted receivers / out-of-range sender
+    bad = m.edge_index.copy()
+    bad[1, 10], bad[1, 400] = bad[1, 400], bad[1, 10]
+    assert cg.cgtp_build_segments(_cuda(bad), nodes)[1].item() == cg.ERR_GRAPH
+    assert orc.segments(bad, nodes)[0] == 4
+    bad = m.edge_index.copy()
+    bad[0, 5] = nodes
+    assert cg.cgtp_build_segments(_cuda(bad), nodes)[1].item() == cg.ERR_GRAPH
+
+
+# ----------------------------------------------------------------------------------- message passing
+@pytest.mark.parametrize("lmax,lmax_out,N,C,nodes,mask", [
+    (0, 0, 4, 4, 6, [0, 1, 0, 1]),
+    (1, 1, 4, 4, 9, [0, 1, 1, 0]),
+    (2, 2, 5, 6, 40, [0, 1, 1, 0, 1, 0]),
+    (3, 3, 8, 8, 30, None),
+    (2, 4, 4, 4, 12, [1, 0, 0, 1]),
+    (4, 2, 4, 6, 12, [0, 0, 1, 1, 1, 0]),
+    (5, 5, 8, 8, 25, [1] * 8),
+    (6, 6, 8, 8, 25, [0] * 8),
+    (7, 7, 4, 4, 10, None),
+])
+def test_message_small_ragged_graphs(lmax, lmax_out, N, C, nodes, mask):
+    rng = np.random.default_rng(lmax * 13 + nodes)
+    deg = rng.integers(0, 20, nodes)
+    deg[0] = 0
+    deg[nodes // 2] = 0
+    deg[-1] = 0 if nodes % 2 else 11
+    m = synthetic.make_message(lmax, lmax_out, N, C, nodes, deg, seed=200 + lmax, parity_mask=mask)
+    got, ref = run_message(m, check=True), oracle_message(m)
+    e = sector_err(got, ref)
+    assert max(e) < TOL, e
+    assert np.abs(got[deg == 0]).max() == 0.0  # receivers without edges -> zeros
+
+
+def test_message_config2_full_even_and_halfhalf():
+    """BASELINE.json configs[2]: 2048 nodes x 16 in-edges, lmax=4, N=C=128; all-even as the config states
+    plus the half/half variant."""
+    m = synthetic.config(2)
+    got, ref = run_message(m, check=True), oracle_message(m)
+    e = sector_err(got, ref)
+    assert e[0] < TOL and np.abs(got[:, 1]).max() == 0.0, e
+    m.parity_mask = synthetic.half_mask(m.C)
+    got, ref = run_message(m, check=True), oracle_message(m)
+    e = sector_err(got, ref)
+    assert max(e) < TOL, e
+
+
+def test_message_config4_sampled():
+    """BASELINE.json configs[4]: 16384 nodes x 32 in-edges, lmax=8, N=C=128, half odd channels; the oracle
+    evaluates a deterministic sample of receiver segments."""
+    m = synthetic.config(4)
+    got = run_message(m, check=True)
+    rng = np.random.default_rng(4)
+    recv = np.unique(np.concatenate([[0, 1, m.nodes - 1], np.arange(0, m.nodes, m.nodes // 24), rng.integers(0, m.nodes, 24)]))
+    ref = oracle_message(m, recv)
+    e = sector_err(got[recv], ref)
+    assert max(e) < TOL, e
+    assert np.isfinite(got).all()
+    assert abs(np.abs(got[:, 1]).mean() / np.abs(got[recv][:, 1]).mean() - 1) < 0.2
+
+
+def test_message_reproducible_and_graph_error():
+    m = synthetic.make_message(4, 4, 16, 16, 300, 12, seed=8)
+    a = run_message(m)
+    b = run_message(m)
+    assert np.array_equal(a, b)
+    bad = synthetic.make_message(4, 4, 16, 16, 300, 12, seed=8)
+    bad.edge_index[1] = bad.edge_index[1][::-1].copy()
+    with pytest.raises(cg.CgtpError) as ei:
+        run_message(bad, check=True)
+    assert ei.value.code == cg.ERR_GRAPH
+    out = run_message(bad)
+    assert np.abs(out).max() == 0.0
+
+
+def test_message_equivariance_and_inversion():
+    lmax = 4
+    m = synthetic.make_message(lmax, lmax, 8, 8, 50, 10, seed=31)
+    base = run_message(m).astype(np.float64)
+    R = shref.random_rotation(np.random.default_rng(23))
+    D = shref.wigner_D_real(lmax, R)
+    mr = synthetic.make_message(lmax, lmax, 8, 8, 50, 10, seed=31)
+    mr.node_feats = np.einsum("ab,...b->...a", D, m.node_feats.astype(np.float64)).astype(np.float32)
+    mr.edge_vec = (m.edge_vec.astype(np.float64) @ R.T).astype(np.float32)
+    rot = run_message(mr).astype(np.float64)
+    e = sector_err(rot, np.einsum("ab,...b->...a", D, base))
+    assert max(e) < TOL, e
+    sign = np.concatenate([np.full(2 * l + 1, (-1.0) ** l) for l in range(lmax + 1)]).astype(np.float32)
+    mi = synthetic.make_message(lmax, lmax, 8, 8, 50, 10, seed=31)
+    mi.node_feats = m.node_feats * sign
+    mi.edge_vec = -m.edge_vec
+    inv = run_message(mi).astype(np.float64)
+    assert np.abs(inv[:, 0] - base[:, 0] * sign).max() < TOL * np.abs(base[:, 0]).max()
+    assert np.abs(inv[:, 1] + base[:, 1] * sign).max() < TOL * np.abs(base[:, 1]).max()
+
+
+def test_message_host_entry_matches_device_entry():
+    m = synthetic.make_message(3, 3, 8, 8, 200, 7, seed=2)
+    dev = run_message(m)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    host = cg.cgtp_message_host(pin(m.node_feats), pin(m.edge_index), pin(m.edge_vec), pin(m.edge_radial),
+                                pin(m.W_node), pin(m.W_out), 3, 3, 8, 8, m.parity_mask).numpy()
+    assert np.array_equal(dev, host)
