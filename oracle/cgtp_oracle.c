@@ -175,7 +175,7 @@ typedef struct {
     double max_imag; /* largest discarded imaginary part (must be round-off) */
 } coupling_t;
 
-#define MAX_CACHED 32
+#define MAX_CACHED 512
 static coupling_t g_cache[MAX_CACHED];
 static int g_ncache = 0;
 
