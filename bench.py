@@ -1,0 +1,453 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the B200 contracted Clebsch-Gordan hot path (contract: see README/DESIGN.md).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-extras]
+
+One "step" = one pass of the whole on-site hot path (S1..S5: projection, Legendre/Fourier synthesis,
+product / surface-curl pairing, analysis, output projection) over one batch of BASELINE.json configs[1]
+(lmax=6, N=C=64, 4096 atoms, 32 even + 32 odd rank channels).  Metric: on-site contractions/s
+(one contraction = one atom's full pipeline).  For N>1 (torchrun) every rank processes its own batch
+(weak scaling, no collective on the data path).
+
+Prints ONE JSON line on rank 0.  Extra objects on the line (N=1 only): "sweep" (configs[3], on-site vs
+lmax), "message" (configs[2] and configs[4], edges/s and HBM GB/s), "kernels" (per-kernel shares).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+SM_COUNT = 148
+FMA_LANES_PER_SM = 128  # 4 SMSPs x 32 FP32 lanes (B200_PROFILING.md / B300_MICROARCH.md unit counts)
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return d, "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+# ------------------------------------------------------------------------------------------------
+# algorithmic work (SURVEY.md 8(d) / DESIGN.md "Measurement"): fixed formulas, minimal grid, dense DFT
+# ------------------------------------------------------------------------------------------------
+def grid_shape(lmax, lmax_out):
+    return (2 * lmax + lmax_out + 2) // 2, 2 * lmax + lmax_out + 1
+
+
+def onsite_flops_per_atom(lmax, lmax_out, N, C, Ce, Co):
+    L2, Lo2 = (lmax + 1) ** 2, (lmax_out + 1) ** 2
+    U, V = grid_shape(lmax, lmax_out)
+    M, Mo = 2 * lmax + 1, 2 * lmax_out + 1
+    k = {
+        "proj_in": 4 * C * N * L2,
+        "onsite_core_even": Ce * (4 * U * L2 + 4 * U * V * M + U * V + 2 * U * V * Mo + 2 * U * Lo2),
+        "onsite_core_odd": Co * (8 * U * L2 + 8 * U * V * M + 3 * U * V + 2 * U * V * Mo + 2 * U * Lo2),
+        "proj_out": 2 * N * C * Lo2,
+    }
+    return k
+
+
+def onsite_bytes_per_atom(lmax, lmax_out, N):
+    return 4 * (2 * N * (lmax + 1) ** 2 + 2 * N * (lmax_out + 1) ** 2)
+
+
+def message_bytes(lmax, lmax_out, N, C, Ce, Co, nodes, E):
+    """Paper-faithful fused data flow: gather sender grids."""
+    U, V = grid_shape(lmax, lmax_out)
+    UV = U * V
+    L2, Lo2 = (lmax + 1) ** 2, (lmax_out + 1) ** 2
+    k = {
+        "edge_even": E * (4 * Ce * UV + 4 * Ce + 12 + 16) + nodes * 4 * Ce * UV,
+        "edge_odd": E * (4 * 2 * Co * UV + 4 * Co + 12 + 16) + nodes * 4 * Co * UV,
+    }
+    total = (E * (4 * (Ce + 2 * Co) * UV + 4 * C + 12 + 16)
+             + nodes * (4 * N * L2 + 4 * (Ce + 2 * Co) * UV + 8 * N * Lo2))
+    return k, total
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML in a background thread."""
+
+    def __init__(self, index: int, period: float = 0.02):
+        self.index, self.period = index, period
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._t = None
+        self.ok = False
+
+    def start(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            return self
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8)),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40)),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20)),
+            "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4)),
+        }
+        get_reasons = getattr(nv, "nvmlDeviceGetCurrentClocksEventReasons", None) or getattr(
+            nv, "nvmlDeviceGetCurrentClocksThrottleReasons")
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = int(get_reasons(self.h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop.set()
+        if self._t:
+            self._t.join()
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------------
+# reference arm = the oracle on the host cores
+# ------------------------------------------------------------------------------------------------
+def oracle_onsite_rate(inp, n_atoms):
+    from oracle import cgtp_oracle as orc
+    n = min(n_atoms, inp.batch)
+    orc.real_coupling(inp.lmax, inp.lmax_out, False)
+    orc.real_coupling(inp.lmax, inp.lmax_out, True)  # tables are set-up, not the timed work
+    t0 = time.perf_counter()
+    orc.onsite(inp.A[:n], inp.B[:n], inp.W_a, inp.W_b, inp.W_out, inp.lmax, inp.lmax_out, inp.parity_mask)
+    dt = time.perf_counter() - t0
+    return n / dt, dt, orc.num_threads()
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    from paper_2605_15073_b200 import synthetic
+    inp = synthetic.config(1)
+    n = 1024
+    from oracle import cgtp_oracle as orc
+    orc.real_coupling(inp.lmax, inp.lmax_out, False)
+    orc.real_coupling(inp.lmax, inp.lmax_out, True)
+    for _ in range(max(args.warmup, 1)):
+        oracle_onsite_rate(inp, n)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_onsite_rate(inp, n)
+    dt = time.perf_counter() - t0
+    val = n * args.steps / dt
+    line = {
+        "impl": "reference", "metric": "onsite_contractions_per_s", "value": val, "unit": "contractions/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "BASELINE.json configs[1]: on-site lmax=6 lmax_out=6 N=64 C=64 batch=4096 even+odd",
+                   "sample": f"first {n} atoms per step"},
+        "cpu_baseline": {"value": val, "unit": "contractions/s", "cores": orc.num_threads(), "kind": "oracle",
+                         "sample": f"{n} of 4096 atoms per step, {args.steps} steps"},
+        "e2e": {"value": val, "unit": "contractions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--sweep-batch", type=int, default=16384)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    from paper_2605_15073_b200 import binding as cg
+    from paper_2605_15073_b200 import synthetic
+
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    cg.lib()  # fails loudly if the CUDA library is missing
+
+    peaks, peak_src = load_peaks()
+    cu = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ------------------------------------------------------------------ main workload: configs[1]
+    NSETS = 4  # rotating input sets: 4 x (A,B) = 411 MB > 126 MB L2, so no step finds its inputs in L2
+    sets = []
+    base = None
+    for s in range(NSETS):
+        inp = synthetic.config(1, seed=1000 * rank + s)
+        base = base or inp
+        sets.append((cu(inp.A), cu(inp.B)))
+    Wa, Wb, Wo = cu(base.W_a), cu(base.W_b), cu(base.W_out)
+    lmax, lmax_out, N, C, batch, mask = base.lmax, base.lmax_out, base.N, base.C, base.batch, base.parity_mask
+    Ce, Co = int((mask == 0).sum()), int((mask == 1).sum())
+    out = torch.empty((batch, 2, N, (lmax_out + 1) ** 2), dtype=torch.float32, device=dev)
+
+    def step(i):
+        A, B = sets[i % NSETS]
+        cg.cgtp_onsite(A, B, Wa, Wb, Wo, lmax, lmax_out, N, C, mask, out=out)
+
+    sampler = ClockSampler(local_rank).start()
+    for i in range(args.warmup):
+        step(i)
+    barrier()
+    l0 = cg.cgtp_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for i in range(args.steps):
+        step(i)
+    ev1.record()
+    barrier()
+    ms_total = max_over_ranks(ev0.elapsed_time(ev1))
+    launches = cg.cgtp_launch_count() - l0
+    ms_per_step = ms_total / args.steps
+    value = world * batch / (ms_per_step * 1e-3)
+
+    # keep the same load running so that the clock record covers >= ~1 s of it
+    t_end = time.perf_counter() + 1.0
+    i = 0
+    while time.perf_counter() < t_end:
+        for _ in range(20):
+            step(i)
+            i += 1
+        torch.cuda.synchronize()
+    clocks = sampler.stop()
+
+    # per-kernel durations over another K steps (CUDA events around every launch, on the launch stream)
+    cg.cgtp_profile_enable(True)
+    for i in range(args.steps):
+        step(i)
+    torch.cuda.synchronize()
+    prof = cg.cgtp_profile_collect()
+    cg.cgtp_profile_enable(False)
+
+    fl = onsite_flops_per_atom(lmax, lmax_out, N, C, Ce, Co)
+    sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz", 1965.0)
+    fp32_peak_tflops = SM_COUNT * FMA_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    kernels = {}
+    for name, (ms, cnt) in prof.items():
+        avg_ms = ms / cnt
+        k = {"launches_per_step": cnt / args.steps, "avg_ms": avg_ms}
+        if name in fl:
+            k["alg_tflops"] = fl[name] * batch / (avg_ms * 1e-3) / 1e12
+            k["frac_fp32_peak"] = k["alg_tflops"] / fp32_peak_tflops
+        kernels[name] = k
+    tot_ms = sum(ms for ms, _ in prof.values())
+    for name, (ms, cnt) in prof.items():
+        kernels[name]["share"] = ms / tot_ms
+    dom = max(prof, key=lambda n: prof[n][0])
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp)).get(f"config1:{dom}")
+    roofline = {
+        "kernel": dom, "bound": "alu", "achieved": kernels[dom]["alg_tflops"], "peak": fp32_peak_tflops,
+        "unit": "TFLOP/s", "frac": kernels[dom]["alg_tflops"] / fp32_peak_tflops, "traffic": traffic,
+        "peak_source": f"derived: {SM_COUNT} SMs x {FMA_LANES_PER_SM} FP32 FMA lanes x 2 x {sm_max:.0f} MHz (DESIGN.md)",
+        "achieved_definition": "algorithmic FP32 flops of this kernel per launch (SURVEY.md 8(d) formula, dense DFT, "
+                               "no symmetry folding) / mean CUDA-event duration",
+        "step_alg_tflops": sum(fl.values()) * batch / (ms_per_step * 1e-3) / 1e12,
+        "step_frac_fp32_peak": sum(fl.values()) * batch / (ms_per_step * 1e-3) / 1e12 / fp32_peak_tflops,
+        "step_hbm_gbs_algorithmic": onsite_bytes_per_atom(lmax, lmax_out, N) * batch / (ms_per_step * 1e-3) / 1e9,
+        "hbm_peak_gbs": peaks["hbm_gbs"], "hbm_peak_source": peak_src,
+    }
+
+    # ------------------------------------------------------------------ end to end with host buffers
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    hA, hB = pin(base.A), pin(base.B)
+    hWa, hWb, hWo = pin(base.W_a), pin(base.W_b), pin(base.W_out)
+    hout = torch.empty((batch, 2, N, (lmax_out + 1) ** 2), dtype=torch.float32).pin_memory()
+    ke = max(3, min(args.steps, 20))
+    for _ in range(2):
+        cg.cgtp_onsite_host(hA, hB, hWa, hWb, hWo, lmax, lmax_out, N, C, mask, out=hout)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(ke):
+        cg.cgtp_onsite_host(hA, hB, hWa, hWb, hWo, lmax, lmax_out, N, C, mask, out=hout)
+    torch.cuda.synchronize()
+    dt = max_over_ranks(time.perf_counter() - t0)
+    e2e = {"value": world * batch * ke / dt, "unit": "contractions/s",
+           "h2d_bytes_per_step": int(hA.numel() + hB.numel() + hWa.numel() + hWb.numel() + hWo.numel()) * 4,
+           "d2h_bytes_per_step": int(hout.numel()) * 4, "steps": ke, "ms_per_step": 1e3 * dt / ke}
+
+    line = {
+        "metric": "onsite_contractions_per_s", "value": value, "unit": "contractions/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "BASELINE.json configs[1]: on-site lmax=6 lmax_out=6 N=64 C=64 batch=4096/GPU, "
+                               "32 even + 32 odd rank channels",
+                   "l2": f"{NSETS} rotating input sets (411 MB) + 360 MB touched per step > 126 MB L2",
+                   "parallelism": f"dp{world} (batch split, no collective)"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "kernels": kernels,
+    }
+
+    # ------------------------------------------------------------------ extras (rank 0, 1 GPU)
+    if world == 1 and not args.no_extras:
+        rate, dt_cpu, cores = oracle_onsite_rate(base, batch)
+        line["cpu_baseline"] = {"value": rate, "unit": "contractions/s", "cores": cores, "kind": "oracle",
+                                "sample": f"all {batch} atoms of configs[1] once ({dt_cpu:.1f} s wall)"}
+        line["sweep"] = run_sweep(args, cg, synthetic, dev, fp32_peak_tflops, peaks)
+        line["message"] = run_message(args, cg, synthetic, dev, peaks, peak_src)
+    elif world == 1:
+        rate, dt_cpu, cores = oracle_onsite_rate(base, 1024)
+        line["cpu_baseline"] = {"value": rate, "unit": "contractions/s", "cores": cores, "kind": "oracle",
+                                "sample": f"first 1024 atoms of configs[1] once ({dt_cpu:.1f} s wall)"}
+
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def time_steps(fn, steps, warmup):
+    import torch
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(steps):
+        fn()
+    ev1.record()
+    torch.cuda.synchronize()
+    return ev0.elapsed_time(ev1) / steps
+
+
+def run_sweep(args, cg, synthetic, dev, fp32_peak_tflops, peaks):
+    """BASELINE.json configs[3]: on-site, N=C=32, batch=16384, lmax in {2,4,8,12,16,20} (inputs drawn on the
+    device with a seeded torch generator: same distribution as synthetic.make_onsite)."""
+    import torch
+    res = []
+    N = C = 32
+    batch = args.sweep_batch
+    g = torch.Generator(device=dev)
+    g.manual_seed(3)
+    mask = synthetic.half_mask(C)
+    Wa = torch.randn((C, N), generator=g, device=dev) / N ** 0.5
+    Wb = torch.randn((C, N), generator=g, device=dev) / N ** 0.5
+    Wo = torch.randn((N, C), generator=g, device=dev) / C ** 0.5
+    for lmax in (2, 4, 8, 12, 16, 20):
+        L2 = (lmax + 1) ** 2
+        A = torch.randn((batch, N, L2), generator=g, device=dev)
+        B = torch.randn((batch, N, L2), generator=g, device=dev)
+        out = torch.empty((batch, 2, N, L2), device=dev)
+        fn = lambda: cg.cgtp_onsite(A, B, Wa, Wb, Wo, lmax, lmax, N, C, mask, out=out)
+        steps = 20 if lmax <= 8 else 5
+        ms = time_steps(fn, steps, 3)
+        fl = sum(onsite_flops_per_atom(lmax, lmax, N, C, C // 2, C // 2).values())
+        by = onsite_bytes_per_atom(lmax, lmax, N)
+        res.append({"lmax": lmax, "ms_per_step": ms, "contractions_per_s": batch / (ms * 1e-3),
+                    "alg_tflops": fl * batch / (ms * 1e-3) / 1e12,
+                    "frac_fp32_peak": fl * batch / (ms * 1e-3) / 1e12 / fp32_peak_tflops,
+                    "alg_hbm_gbs": by * batch / (ms * 1e-3) / 1e9,
+                    "frac_hbm_peak": by * batch / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"]})
+        del A, B, out
+    return {"workload": f"BASELINE.json configs[3]: on-site N=C=32 batch={batch} lmax_out=lmax, 16 even + 16 odd",
+            "points": res}
+
+
+def run_message(args, cg, synthetic, dev, peaks, peak_src):
+    import torch
+    cu = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    res = {}
+    for name, idx, halfhalf in (("config2_all_even", 2, False), ("config2_half_odd", 2, True), ("config4", 4, True)):
+        m = synthetic.config(idx)
+        if idx == 2 and halfhalf:
+            m.parity_mask = synthetic.half_mask(m.C)
+        Ce, Co = int((m.parity_mask == 0).sum()), int((m.parity_mask == 1).sum())
+        X, ei, ev, er = cu(m.node_feats), cu(m.edge_index), cu(m.edge_vec), cu(m.edge_radial)
+        Wn, Wo = cu(m.W_node), cu(m.W_out)
+        out = torch.empty((m.nodes, 2, m.N, (m.lmax_out + 1) ** 2), device=dev)
+        fn = lambda: cg.cgtp_message(X, ei, ev, er, Wn, Wo, m.lmax, m.lmax_out, m.N, m.C, m.parity_mask, out=out)
+        steps = 10 if idx == 2 else 3
+        ms = time_steps(fn, steps, 3)
+        cg.cgtp_profile_enable(True)
+        for _ in range(steps):
+            fn()
+        torch.cuda.synchronize()
+        prof = cg.cgtp_profile_collect()
+        cg.cgtp_profile_enable(False)
+        kb, total_bytes = message_bytes(m.lmax, m.lmax_out, m.N, m.C, Ce, Co, m.nodes, m.E)
+        kern = {}
+        tot = sum(v[0] for v in prof.values())
+        for k, (kms, cnt) in prof.items():
+            kern[k] = {"avg_ms": kms / cnt, "share": kms / tot}
+            if k in kb:
+                kern[k]["alg_gbs"] = kb[k] / (kms / cnt * 1e-3) / 1e9
+                kern[k]["frac_hbm_peak"] = kern[k]["alg_gbs"] / peaks["hbm_gbs"]
+        dom = max(prof, key=lambda n: prof[n][0])
+        res[name] = {
+            "workload": f"BASELINE.json configs[{idx}]: nodes={m.nodes} E={m.E} lmax={m.lmax} N=C={m.C} "
+                        f"even={Ce} odd={Co}",
+            "ms_per_step": ms, "edges_per_s": m.E / (ms * 1e-3),
+            "alg_hbm_gbs_whole_step": total_bytes / (ms * 1e-3) / 1e9,
+            "frac_hbm_peak_whole_step": total_bytes / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+            "roofline": {"kernel": dom, "bound": "hbm", "achieved": kern[dom].get("alg_gbs"),
+                         "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": kern[dom].get("frac_hbm_peak"),
+                         "peak_source": peak_src, "traffic": None},
+            "kernels": kern,
+        }
+        del X, ei, ev, er, out
+        torch.cuda.empty_cache()
+    return res
+
+
+if __name__ == "__main__":
+    main()

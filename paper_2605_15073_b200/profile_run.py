@@ -1,0 +1,57 @@
+"""Runs a few steps of one BASELINE.json config through the C ABI -- the small, fixed command that the
+ncu captures under profiles/ are made with.
+
+    python -m paper_2605_15073_b200.profile_run --config 1 --steps 2            # on-site, configs[1]
+    python -m paper_2605_15073_b200.profile_run --config 3 --lmax 20 --steps 1  # on-site sweep point
+    python -m paper_2605_15073_b200.profile_run --config 4 --steps 1            # message passing, configs[4]
+"""
+from __future__ import annotations
+
+import argparse
+
+import numpy as np
+import torch
+
+from . import binding as cg
+from . import synthetic
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--lmax", type=int, default=None)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--batch", type=int, default=None, help="override the batch / node count")
+    ap.add_argument("--all-even", action="store_true")
+    args = ap.parse_args()
+    dev = torch.device("cuda", 0)
+    cu = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    inp = synthetic.config(args.config, lmax=args.lmax)
+    if args.all_even:
+        inp.parity_mask = np.zeros_like(inp.parity_mask)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if isinstance(inp, synthetic.OnsiteInputs):
+        b = args.batch or inp.batch
+        A, B = cu(inp.A[:b]), cu(inp.B[:b])
+        Wa, Wb, Wo = cu(inp.W_a), cu(inp.W_b), cu(inp.W_out)
+        fn = lambda: cg.cgtp_onsite(A, B, Wa, Wb, Wo, inp.lmax, inp.lmax_out, inp.N, inp.C, inp.parity_mask)
+        units, unit = b, "contractions"
+    else:
+        X, ei, ev, er = cu(inp.node_feats), cu(inp.edge_index), cu(inp.edge_vec), cu(inp.edge_radial)
+        Wn, Wo = cu(inp.W_node), cu(inp.W_out)
+        fn = lambda: cg.cgtp_message(X, ei, ev, er, Wn, Wo, inp.lmax, inp.lmax_out, inp.N, inp.C, inp.parity_mask)
+        units, unit = inp.E, "edges"
+    fn()
+    torch.cuda.synchronize()
+    ev0.record()
+    for _ in range(args.steps):
+        fn()
+    ev1.record()
+    torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / args.steps
+    print(f"config {args.config}: {ms:.4f} ms/step, {units / ms * 1e3:.4g} {unit}/s, "
+          f"launches {cg.cgtp_launch_count()}")
+
+
+if __name__ == "__main__":
+    main()
