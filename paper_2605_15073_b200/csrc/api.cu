@@ -50,7 +50,8 @@ static int check_common(int lmax, int lmax_out, int N, int C, const uint8_t* mas
 static size_t onsite_ws_bytes(int lmax, int lmax_out, int C, int64_t batch)
 {
     const size_t L2p = round_up((lmax + 1) * (lmax + 1), 4), Lo2p = round_up((lmax_out + 1) * (lmax_out + 1), 4);
-    return (size_t)batch * C * (2 * L2p + Lo2p) * sizeof(float) + 8 * 256;
+    // rows may use the odd strides of the fast core (<= L2p + 1) and columns are padded to groups of 32
+    return ((size_t)batch * C + 64) * (2 * (L2p + 4) + (Lo2p + 4)) * sizeof(float) + 8 * 256;
 }
 
 static size_t message_ws_bytes(int lmax, int lmax_out, int C, int Co, int64_t nodes)
@@ -113,13 +114,32 @@ int cgtp_onsite(const float* A, const float* B, const float* W_a, const float* W
     if (!cp) return CGTP_ERR_CUDA;
     const int Ce = cp->Ce, Co = cp->Co;
 
+    // fast core (onsite_core.cu) when both parities fit; it wants odd row strides and 32-column groups
+    const bool fast = (Ce == 0 || onsite_fast_supported(p, false)) && (Co == 0 || onsite_fast_supported(p, true));
+    const int hstr = fast ? onsite_fast_hstride(p) : p->L2p;
+    const int tstr = fast ? onsite_fast_tstride(p) : p->Lo2p;
+    const size_t ncol_e = (size_t)round_up((int)((size_t)batch * Ce % 32), 32) + (size_t)batch * Ce / 32 * 32;
+    const size_t ncol_o = (size_t)round_up((int)((size_t)batch * Co % 32), 32) + (size_t)batch * Co / 32 * 32;
+
     Carver cv(workspace);
-    float* Ha_e = cv.take<float>((size_t)batch * Ce * p->L2p);
-    float* Ha_o = cv.take<float>((size_t)batch * Co * p->L2p);
-    float* Hb_e = cv.take<float>((size_t)batch * Ce * p->L2p);
-    float* Hb_o = cv.take<float>((size_t)batch * Co * p->L2p);
-    float* T_e = cv.take<float>((size_t)batch * Ce * p->Lo2p);
-    float* T_o = cv.take<float>((size_t)batch * Co * p->Lo2p);
+    float* Ha_e = cv.take<float>(ncol_e * hstr);
+    float* Ha_o = cv.take<float>(ncol_o * hstr);
+    float* Hb_e = cv.take<float>(ncol_e * hstr);
+    float* Hb_o = cv.take<float>(ncol_o * hstr);
+    float* T_e = cv.take<float>(ncol_e * tstr);
+    float* T_o = cv.take<float>(ncol_o * tstr);
+    if (fast) {
+        // columns that pad the last group: define them (their results are never read)
+        const size_t ne = (size_t)batch * Ce, no = (size_t)batch * Co;
+        if (ncol_e > ne) {
+            CGTP_CUDA_CHECK(cudaMemsetAsync(Ha_e + ne * hstr, 0, (ncol_e - ne) * hstr * 4, st));
+            CGTP_CUDA_CHECK(cudaMemsetAsync(Hb_e + ne * hstr, 0, (ncol_e - ne) * hstr * 4, st));
+        }
+        if (ncol_o > no) {
+            CGTP_CUDA_CHECK(cudaMemsetAsync(Ha_o + no * hstr, 0, (ncol_o - no) * hstr * 4, st));
+            CGTP_CUDA_CHECK(cudaMemsetAsync(Hb_o + no * hstr, 0, (ncol_o - no) * hstr * 4, st));
+        }
+    }
 
     // S1: H = W . A (Eq.(35)); rows are written in parity-sorted channel order, even block then odd block
     ProjArgs pin[2];
@@ -137,20 +157,22 @@ int cgtp_onsite(const float* A, const float* B, const float* W_a, const float* W
         a.K = N;
         a.J = p->L2;
         a.out0 = s ? Hb_e : Ha_e;
-        a.o_bs0 = (int64_t)Ce * p->L2p;
+        a.o_bs0 = (int64_t)Ce * hstr;
         a.out1 = s ? Hb_o : Ha_o;
-        a.o_bs1 = (int64_t)Co * p->L2p;
+        a.o_bs1 = (int64_t)Co * hstr;
         a.m_split = Ce;
-        a.o_rs = p->L2p;
+        a.o_rs = hstr;
         a.batch = batch;
     }
     rc = launch_proj(pin, 2, K_PROJ_IN, st);
     if (rc) return rc;
 
     // S2-S4 fused, one launch per parity
-    rc = launch_onsite_core(p, false, Ha_e, Hb_e, T_e, batch * Ce, st);
+    rc = fast ? launch_onsite_fast(p, false, Ha_e, Hb_e, T_e, batch * Ce, st)
+              : launch_onsite_generic(p, false, Ha_e, Hb_e, T_e, batch * Ce, st);
     if (rc) return rc;
-    rc = launch_onsite_core(p, true, Ha_o, Hb_o, T_o, batch * Co, st);
+    rc = fast ? launch_onsite_fast(p, true, Ha_o, Hb_o, T_o, batch * Co, st)
+              : launch_onsite_generic(p, true, Ha_o, Hb_o, T_o, batch * Co, st);
     if (rc) return rc;
 
     // S5: out[b, s] = W_out[:, channels of sector s] . T_s (Eq.(41))
@@ -158,8 +180,8 @@ int cgtp_onsite(const float* A, const float* B, const float* W_a, const float* W
     for (int s = 0; s < 2; ++s) {
         ProjArgs& a = po[s];
         a.X = s ? T_o : T_e;
-        a.x_bs = (int64_t)(s ? Co : Ce) * p->Lo2p;
-        a.x_rs = p->Lo2p;
+        a.x_bs = (int64_t)(s ? Co : Ce) * tstr;
+        a.x_rs = tstr;
         a.W = W_out;
         a.ldw_m = C;
         a.ldw_k = 1;

@@ -5,6 +5,7 @@
 
 #include <cstdint>
 #include <cstdio>
+#include <vector>
 
 #include "../../include/cgtp.h"
 
@@ -56,6 +57,10 @@ struct Plan {
     // Grid geometry for the edge factor, [8][UVp]: Omega_xyz, theta_hat_xyz, phi_hat_xy (zero padded)
     const float* geo;
 };
+
+// FP64 host helpers of the table builder (tables.cu), shared with the packed tables of onsite_core.cu.
+void gauss_legendre(int U, std::vector<double>& x, std::vector<double>& w);
+void legendre_values(int U, int LB, const std::vector<double>& x, std::vector<double>& P);  // P[u][l][m]
 
 // Returns the cached plan, creating it on first use (cudaMalloc + blocking copies, once).
 // nullptr + cgtp_last_error on failure.
@@ -138,7 +143,16 @@ struct ProjArgs {
 int launch_proj(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st);
 
 // S2-S4 fused: T[col][lm] from Ha[col], Hb[col]; ncols columns of one parity.
-int launch_onsite_core(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols,
+// Generic kernel (any compiled band limit): H rows of stride p->L2p, T rows of stride p->Lo2p.
+int launch_onsite_generic(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols,
+                          cudaStream_t st);
+// Fast kernel (onsite_core.cu): lane = column, packed FP32 FMAs.  H rows of stride onsite_fast_hstride(p),
+// T rows of stride onsite_fast_tstride(p) (both odd, so that lane-strided shared-memory accesses are
+// conflict-free); the column count is padded up to a multiple of 32 in both buffers.
+bool onsite_fast_supported(const Plan* p, bool odd);
+inline int onsite_fast_hstride(const Plan* p) { return p->L2 | 1; }
+inline int onsite_fast_tstride(const Plan* p) { return p->Lo2 | 1; }
+int launch_onsite_fast(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols,
                        cudaStream_t st);
 
 // M0

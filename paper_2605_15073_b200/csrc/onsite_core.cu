@@ -1,0 +1,653 @@
+// onsite_core.cu -- fast fused on-site core (rows S2a, S2b, S3, S4a, S4b of SURVEY.md 8(a)) for band
+// limits whose working set fits shared memory.  Same mathematics as onsite_generic.cu:
+//   Legendre synthesis (Eq.(36)) -> phi synthesis (Eq.(37) :327) -> pointwise product
+//   (even channels, Eq.(38) :332) or surface-curl pairing (odd channels, Eq.(11) :107, theta-form) ->
+//   inverse phi transform (Eq.(39) :339) -> Gauss-Legendre analysis (Eq.(40) :342),
+// with the grid fields in registers only.  What differs is the mapping to the machine:
+//   * lane = column: a CTA works on groups of 32 (atom, rank-channel) columns; every shared-memory array
+//     has the column as its fastest index (or an odd row stride), so all accesses are conflict-free;
+//   * packed FP32 FMAs (FFMA2, fma.rn.f32x2): the scalar FFMA issue rate of sm_100a tops out near 48
+//     TFLOP/s, the packed form reaches 66 TFLOP/s (measured); pairs are (+m,-m) rows, (A,B) factors or
+//     (d_theta, d_phi) components, with the tables stored in the duplicated / interleaved form each needs;
+//   * warps of a CTA split each stage by a static, host-computed schedule (longest-processing-time
+//     assignment of the ragged per-m work), CTAs are persistent over column groups and prefetch the
+//     next group's coefficients with TMA bulk copies while computing.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <mutex>
+
+#include "sht.cuh"
+
+namespace cgtp {
+
+constexpr int kMaxWarps = 8;
+
+// Byte offsets (multiples of 16) into the packed table blob of one (plan, parity).
+struct CoreTab {
+    int ta;     // stage A: [tri(l,m)][UP2] float2.  even: (P~,P~); odd: (d_theta P~, m P~/sin theta)
+    int wp;     // stage C: [tri(l,m)][UP2] float2 (w P~, w P~), equator row halved
+    int qf;     // stage B forward: [Vh][QFS] float2 (q,q); entry r<=LB: cos row r, r>LB: sin row r-LB
+    int qi;     // stage B inverse: [Vh][QIS] float, (2 pi/V) q folded in; cos m at m, sin m at SOFF+m-1
+    int sched;  // int: per stage s (A,B,C) and warp w: cnt[s][w] at s*kMaxWarps+w, then items[s][w][MAXI]
+    int bytes;
+    int UP2, QFS, QIS, SOFF, MAXI;
+    int NW;
+};
+
+struct CorePlan {
+    int lmax, lmax_out;
+    bool odd;
+    CoreTab tab;
+    const void* blob;  // device
+};
+
+__host__ __device__ constexpr int core_uhmax(int LB) { return ((3 * LB + 2) / 2 + 1) / 2; }
+
+// ------------------------------------------------------------------------------------------------
+// Host: packed tables + static schedules
+// ------------------------------------------------------------------------------------------------
+static void lpt_assign(const std::vector<std::pair<int, int>>& items /* (cost, id) */, int NW,
+                       std::vector<std::vector<int>>& out, int* makespan)
+{
+    std::vector<std::pair<int, int>> it = items;
+    std::stable_sort(it.begin(), it.end(), [](const std::pair<int, int>& a, const std::pair<int, int>& b) { return a.first > b.first; });
+    std::vector<int> load(NW, 0);
+    out.assign(NW, {});
+    for (auto& x : it) {
+        int w = 0;
+        for (int k = 1; k < NW; ++k)
+            if (load[k] < load[w]) w = k;
+        load[w] += x.first;
+        out[w].push_back(x.second);
+    }
+    *makespan = *std::max_element(load.begin(), load.end());
+}
+
+static void stage_items(const Plan* p, bool odd, std::vector<std::pair<int, int>> (&items)[3])
+{
+    const int LB = p->LB;
+    // stage A: one item per m <= LB (rows above lmax are zero-filled: cost 1); cost ~ number of l terms
+    for (int m = 0; m <= LB; ++m) items[0].push_back({m <= p->lmax ? 2 * (p->lmax - m + 1) + 1 : 1, m});
+    // stage B: one item per grid row u, equal cost
+    for (int u = 0; u < p->U; ++u) items[1].push_back({4, u});
+    // stage C: one item per m <= lmax_out
+    for (int m = 0; m <= p->lmax_out; ++m) items[2].push_back({(p->lmax_out - m + 1) + 1, m});
+    (void)odd;
+}
+
+static std::mutex g_core_mu;
+static std::vector<CorePlan*> g_core_plans;
+
+static size_t core_smem_bytes(const Plan* p, bool odd, const CoreTab& t, bool dbl)
+{
+    const int MR = 2 * p->LB + 1;
+    const size_t hs = (size_t)2 * 32 * onsite_fast_hstride(p) * 4;
+    const size_t f = (size_t)(odd ? 4 : 2) * MR * p->U * 32 * 4;
+    const size_t ts = (size_t)32 * onsite_fast_tstride(p) * 4;
+    return 64 + t.bytes + (dbl ? 2 : 1) * hs + f + ts;
+}
+
+static const CorePlan* get_core_plan(const Plan* p, bool odd)
+{
+    std::lock_guard<std::mutex> lk(g_core_mu);
+    for (CorePlan* c : g_core_plans)
+        if (c->lmax == p->lmax && c->lmax_out == p->lmax_out && c->odd == odd) return c;
+
+    const int LB = p->LB, U = p->U, Uh = p->Uh, V = p->V, Vh = p->Vh;
+    const int LL = LB + 1;
+    const int MR = 2 * LB + 1;
+    CoreTab t;
+    std::memset(&t, 0, sizeof t);
+    t.UP2 = round_up(core_uhmax(LB), 2);
+    t.QFS = round_up(MR, 2);
+    t.SOFF = round_up(LB + 1, 2);
+    t.QIS = round_up(t.SOFF + LB, 4);
+    const int ntri = (LB + 1) * (LB + 2) / 2;
+
+    std::vector<double> x, w, P;
+    gauss_legendre(U, x, w);
+    legendre_values(U, LB, x, P);
+    auto at = [&](int u, int l, int m) -> double { return P[((size_t)u * LL + l) * LL + m]; };
+
+    std::vector<float> TA((size_t)ntri * t.UP2 * 2, 0.f), WP(TA.size(), 0.f);
+    for (int u = 0; u < Uh; ++u) {
+        const double ct = x[u], st = std::sqrt(1.0 - ct * ct);
+        const double wu = w[u] * ((U % 2 && u == Uh - 1) ? 0.5 : 1.0);
+        for (int l = 0; l <= LB; ++l)
+            for (int m = 0; m <= l; ++m) {
+                const double pv = at(u, l, m);
+                const double pm1 = (l - 1 >= m) ? at(u, l - 1, m) : 0.0;
+                const double c = (l > 0) ? std::sqrt((2.0 * l + 1.0) * ((double)l * l - (double)m * m) / (2.0 * l - 1.0)) : 0.0;
+                const double dth = (l * ct * pv - c * pm1) / st;
+                const size_t k = ((size_t)tri_index(l, m) * t.UP2 + u) * 2;
+                if (!odd) {
+                    TA[k] = TA[k + 1] = (float)pv;
+                } else {
+                    TA[k] = (float)dth;
+                    TA[k + 1] = (float)(m * pv / st);
+                }
+                WP[k] = WP[k + 1] = (float)(wu * pv);
+            }
+    }
+    std::vector<float> QF((size_t)Vh * t.QFS * 2, 0.f), QI((size_t)Vh * t.QIS, 0.f);
+    for (int v = 0; v < Vh; ++v) {
+        const double ph = 2.0 * M_PI * v / V;
+        const bool paired = (v != 0) && !(V % 2 == 0 && v == V / 2);
+        const double wv = (2.0 * M_PI / V) * (paired ? 1.0 : 0.5);
+        for (int m = 0; m <= LB; ++m) {
+            const double qc = (m == 0) ? 1.0 : std::sqrt(2.0) * std::cos(m * ph);
+            const double qs = (m == 0 || !paired) ? 0.0 : std::sqrt(2.0) * std::sin(m * ph);
+            QF[((size_t)v * t.QFS + m) * 2] = QF[((size_t)v * t.QFS + m) * 2 + 1] = (float)qc;
+            QI[(size_t)v * t.QIS + m] = (float)(wv * qc);
+            if (m > 0) {
+                QF[((size_t)v * t.QFS + LB + m) * 2] = QF[((size_t)v * t.QFS + LB + m) * 2 + 1] = (float)qs;
+                QI[(size_t)v * t.QIS + t.SOFF + m - 1] = (float)(wv * qs);
+            }
+        }
+    }
+
+    // schedules: choose the warp count with the best work efficiency
+    std::vector<std::pair<int, int>> items[3];
+    stage_items(p, odd, items);
+    int bestNW = 4;
+    double best = -1.0;
+    for (int NW = 4; NW <= kMaxWarps; ++NW) {
+        double total = 0.0, span = 0.0;
+        for (int s = 0; s < 3; ++s) {
+            std::vector<std::vector<int>> asg;
+            int mk;
+            lpt_assign(items[s], NW, asg, &mk);
+            // stage B dominates the run time: weight it by its real share of the FMA work
+            const double wgt = (s == 1) ? 6.0 : 1.0;
+            int tot = 0;
+            for (auto& x2 : items[s]) tot += x2.first;
+            total += wgt * tot;
+            span += wgt * mk * NW;
+        }
+        const double eff = total / span;
+        if (eff > best + 1e-9) { best = eff; bestNW = NW; }
+    }
+    t.NW = bestNW;
+    std::vector<std::vector<int>> asg[3];
+    int maxi = 1;
+    for (int s = 0; s < 3; ++s) {
+        int mk;
+        lpt_assign(items[s], t.NW, asg[s], &mk);
+        for (auto& a : asg[s]) maxi = std::max(maxi, (int)a.size());
+    }
+    t.MAXI = maxi;
+    std::vector<int> sched((size_t)3 * kMaxWarps + (size_t)3 * kMaxWarps * maxi, 0);
+    for (int s = 0; s < 3; ++s)
+        for (int wi = 0; wi < t.NW; ++wi) {
+            sched[s * kMaxWarps + wi] = (int)asg[s][wi].size();
+            for (size_t k = 0; k < asg[s][wi].size(); ++k)
+                sched[3 * kMaxWarps + ((size_t)s * kMaxWarps + wi) * maxi + k] = asg[s][wi][k];
+        }
+
+    // pack
+    std::vector<unsigned char> blob;
+    auto append = [&](const void* src, size_t bytes) {
+        size_t off = blob.size();
+        blob.resize(off + round_up((int)bytes, 16));
+        std::memcpy(blob.data() + off, src, bytes);
+        return (int)off;
+    };
+    t.ta = append(TA.data(), TA.size() * 4);
+    t.wp = append(WP.data(), WP.size() * 4);
+    t.qf = append(QF.data(), QF.size() * 4);
+    t.qi = append(QI.data(), QI.size() * 4);
+    t.sched = append(sched.data(), sched.size() * 4);
+    t.bytes = (int)blob.size();
+
+    void* d = nullptr;
+    if (cudaMalloc(&d, blob.size()) != cudaSuccess ||
+        cudaMemcpy(d, blob.data(), blob.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
+        set_error("onsite core plan: device upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+        return nullptr;
+    }
+    CorePlan* c = new CorePlan;
+    c->lmax = p->lmax;
+    c->lmax_out = p->lmax_out;
+    c->odd = odd;
+    c->tab = t;
+    c->blob = d;
+    g_core_plans.push_back(c);
+    return c;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Device
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 fadd2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 fsub2(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+
+struct CoreArgs {
+    CoreTab tab;
+    const void* blob;
+    const float* Ha;
+    const float* Hb;
+    float* T;
+    long long ngroups;
+    int lmax, lmax_out, U, Uh, Vh;
+    int L2s, Lo2s;
+    int dbl;                         // 1: two H buffers (prefetch during the whole group), 0: one
+    int off_blob, off_hs, off_f, off_ts;  // byte offsets in dynamic shared memory
+    int hs_bytes;                    // bytes of one H buffer (both factors)
+};
+
+// Stage A (row S2a), even channels.  Thread = (column, |m|): rows m (cos) and LB+m (sin) of both factors
+// for all grid rows; pairs are (+m, -m), the table is stored duplicated.
+template <int LB>
+__device__ __forceinline__ void stage_a_even(const float* __restrict__ ta, int UP2, const float* __restrict__ ha,
+                                             const float* __restrict__ hb, float* __restrict__ Fa,
+                                             float* __restrict__ Fb, int m, int lmax, int U, int Uh, int lane)
+{
+    constexpr int UH = core_uhmax(LB);
+    float2 acc[2][2][UH];
+#pragma unroll
+    for (int f = 0; f < 2; ++f)
+#pragma unroll
+        for (int par = 0; par < 2; ++par)
+#pragma unroll
+            for (int e = 0; e < UH; ++e) acc[f][par][e] = make_float2(0.f, 0.f);
+    for (int l = m; l <= lmax; l += 2) {
+#pragma unroll
+        for (int par = 0; par < 2; ++par) {
+            const int ll = l + par;
+            if (ll > lmax) break;
+            const float4* tab = reinterpret_cast<const float4*>(ta + (size_t)tri_index(ll, m) * UP2 * 2);
+            const int ip = ll * ll + ll + m, im = ll * ll + ll - m;
+            const float2 xa = make_float2(ha[ip], ha[im]);
+            const float2 xb = make_float2(hb[ip], hb[im]);
+#pragma unroll
+            for (int e = 0; e < UH; e += 2) {
+                const float4 t4 = tab[e / 2];
+                acc[0][par][e] = ffma2(make_float2(t4.x, t4.y), xa, acc[0][par][e]);
+                acc[1][par][e] = ffma2(make_float2(t4.x, t4.y), xb, acc[1][par][e]);
+                if (e + 1 < UH) {
+                    acc[0][par][e + 1] = ffma2(make_float2(t4.z, t4.w), xa, acc[0][par][e + 1]);
+                    acc[1][par][e + 1] = ffma2(make_float2(t4.z, t4.w), xb, acc[1][par][e + 1]);
+                }
+            }
+        }
+    }
+    // P~(-x) = (-1)^(l+m) P~(x): north = even + odd part, south = even - odd part
+#pragma unroll
+    for (int e = 0; e < UH; ++e) {
+        if (e < Uh) {
+            const int rn = (m * U + e) * 32 + lane, rs = (m * U + (U - 1 - e)) * 32 + lane;
+            const int off = LB * U * 32;
+            const float2 na = fadd2(acc[0][0][e], acc[0][1][e]), sa = fsub2(acc[0][0][e], acc[0][1][e]);
+            const float2 nb = fadd2(acc[1][0][e], acc[1][1][e]), sb = fsub2(acc[1][0][e], acc[1][1][e]);
+            Fa[rn] = na.x; Fa[rs] = sa.x; Fb[rn] = nb.x; Fb[rs] = sb.x;
+            if (m > 0) { Fa[rn + off] = na.y; Fa[rs + off] = sa.y; Fb[rn + off] = nb.y; Fb[rs + off] = sb.y; }
+        }
+    }
+}
+
+// Stage A, odd channels.  Table pairs are (d_theta P~, m P~/sin theta); accumulator pairs are the
+// (theta, phi) components of the surface gradient.  The phi derivative swaps the cos and sin rows
+// (PAPER.md:679): cos row m takes +m * (sine coefficient), sin row takes -m * (cosine coefficient).
+// F planes: 2*f + 0 = d_theta, 2*f + 1 = (1/sin theta) d_phi of factor f.
+template <int LB>
+__device__ __forceinline__ void stage_a_odd(const float* __restrict__ ta, int UP2, const float* __restrict__ h,
+                                            float* __restrict__ Fth, float* __restrict__ Fph, int m, int lmax, int U,
+                                            int Uh, int lane)
+{
+    constexpr int UH = core_uhmax(LB);
+    float2 acc[2][2][UH];  // [row type: cos, sin][parity of l-m][u']
+#pragma unroll
+    for (int r = 0; r < 2; ++r)
+#pragma unroll
+        for (int par = 0; par < 2; ++par)
+#pragma unroll
+            for (int e = 0; e < UH; ++e) acc[r][par][e] = make_float2(0.f, 0.f);
+    for (int l = m; l <= lmax; l += 2) {
+#pragma unroll
+        for (int par = 0; par < 2; ++par) {
+            const int ll = l + par;
+            if (ll > lmax) break;
+            const float4* tab = reinterpret_cast<const float4*>(ta + (size_t)tri_index(ll, m) * UP2 * 2);
+            const float hp = h[ll * ll + ll + m], hm = h[ll * ll + ll - m];
+            const float2 xc = make_float2(hp, hm);   // cos row: d_theta from H[l,+m], d_phi from H[l,-m]
+            const float2 xs = make_float2(hm, -hp);  // sin row: d_theta from H[l,-m], d_phi from -H[l,+m]
+#pragma unroll
+            for (int e = 0; e < UH; e += 2) {
+                const float4 t4 = tab[e / 2];
+                acc[0][par][e] = ffma2(make_float2(t4.x, t4.y), xc, acc[0][par][e]);
+                acc[1][par][e] = ffma2(make_float2(t4.x, t4.y), xs, acc[1][par][e]);
+                if (e + 1 < UH) {
+                    acc[0][par][e + 1] = ffma2(make_float2(t4.z, t4.w), xc, acc[0][par][e + 1]);
+                    acc[1][par][e + 1] = ffma2(make_float2(t4.z, t4.w), xs, acc[1][par][e + 1]);
+                }
+            }
+        }
+    }
+    // d/dtheta flips the reflection parity; (1/sin) d_phi keeps it
+#pragma unroll
+    for (int e = 0; e < UH; ++e) {
+        if (e < Uh) {
+            const int rn = (m * U + e) * 32 + lane, rs = (m * U + (U - 1 - e)) * 32 + lane;
+            const int off = LB * U * 32;
+            const float2 n0 = fadd2(acc[0][0][e], acc[0][1][e]), d0 = fsub2(acc[0][0][e], acc[0][1][e]);
+            Fth[rn] = n0.x; Fth[rs] = -d0.x; Fph[rn] = n0.y; Fph[rs] = d0.y;
+            if (m > 0) {
+                const float2 n1 = fadd2(acc[1][0][e], acc[1][1][e]), d1 = fsub2(acc[1][0][e], acc[1][1][e]);
+                Fth[rn + off] = n1.x; Fth[rs + off] = -d1.x; Fph[rn + off] = n1.y; Fph[rs + off] = d1.y;
+            }
+        }
+    }
+}
+
+// Stage B (rows S2b + S3 + S4a) for one (column, grid row u): forward real DFT of the coefficient
+// rows, product (even) or curl pairing (odd) at every azimuth, inverse real DFT -- all in registers.
+// The azimuth pair (v', V-v') shares one table row: C = cosine part, S = sine part of the m-sum,
+// field(v') = C + S, field(V-v') = C - S.  The result rows overwrite plane 0 in place.
+template <int LB, bool ODD>
+__device__ __forceinline__ void stage_b(const float* __restrict__ qf, const float* __restrict__ qi, int QFS, int QIS,
+                                        int SOFF, float* __restrict__ F, int plane_stride, int U, int u, int Vh,
+                                        int lane)
+{
+    constexpr int MR = 2 * LB + 1;
+    constexpr int NTC = (LB + 2) / 2;  // pairs of cos rows m = 0..LB (+ pad)
+    constexpr int NTS = (LB + 1) / 2;  // pairs of sin rows m = 1..LB (+ pad)
+    constexpr int NP = ODD ? 2 : 1;
+    // f[k][r]: even: k = 0, pair (A, B); odd: k = 0 pair (A_theta, A_phi), k = 1 pair (B_theta, B_phi)
+    float2 f[NP][MR];
+#pragma unroll
+    for (int r = 0; r < MR; ++r) {
+        const int idx = (r * U + u) * 32 + lane;
+        f[0][r] = make_float2(F[idx], F[idx + plane_stride]);
+        if (ODD) f[NP - 1][r] = make_float2(F[idx + 2 * plane_stride], F[idx + 3 * plane_stride]);
+    }
+    float2 tc[NTC], ts[NTS > 0 ? NTS : 1];
+#pragma unroll
+    for (int k = 0; k < NTC; ++k) tc[k] = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int k = 0; k < NTS; ++k) ts[k] = make_float2(0.f, 0.f);
+
+    for (int vp = 0; vp < Vh; ++vp) {
+        const float4* q4 = reinterpret_cast<const float4*>(qf + (size_t)vp * QFS * 2);
+        float2 Cs[NP][2], Ss[NP][2];  // two chains each for ILP
+#pragma unroll
+        for (int k = 0; k < NP; ++k) {
+            Cs[k][0] = Cs[k][1] = make_float2(0.f, 0.f);
+            Ss[k][0] = Ss[k][1] = make_float2(0.f, 0.f);
+        }
+#pragma unroll
+        for (int r = 0; r < MR; r += 2) {
+            const float4 t4 = q4[r / 2];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int rr = r + h;
+                if (rr >= MR) break;
+                const float2 q2 = h ? make_float2(t4.z, t4.w) : make_float2(t4.x, t4.y);
+#pragma unroll
+                for (int k = 0; k < NP; ++k) {
+                    if (rr <= LB) Cs[k][rr & 1] = ffma2(q2, f[k][rr], Cs[k][rr & 1]);
+                    else Ss[k][rr & 1] = ffma2(q2, f[k][rr], Ss[k][rr & 1]);
+                }
+            }
+        }
+        float s1, s2;
+        if (!ODD) {
+            const float2 C = fadd2(Cs[0][0], Cs[0][1]), S = fadd2(Ss[0][0], Ss[0][1]);
+            const float2 g1 = fadd2(C, S), g2 = fsub2(C, S);
+            s1 = g1.x * g1.y;  // Eq.(38): A~ B~ at azimuth v'
+            s2 = g2.x * g2.y;  //          and at V - v'
+        } else {
+            const float2 Ca = fadd2(Cs[0][0], Cs[0][1]), Sa = fadd2(Ss[0][0], Ss[0][1]);
+            const float2 Cb = fadd2(Cs[1][0], Cs[1][1]), Sb = fadd2(Ss[1][0], Ss[1][1]);
+            const float2 a1 = fadd2(Ca, Sa), a2 = fsub2(Ca, Sa), b1 = fadd2(Cb, Sb), b2 = fsub2(Cb, Sb);
+            // Eq.(11): {A,B} = A_theta B_phi - A_phi B_theta  (A factor 1, B factor 2)
+            s1 = fmaf(a1.x, b1.y, -a1.y * b1.x);
+            s2 = fmaf(a2.x, b2.y, -a2.y * b2.x);
+        }
+        const float sp = s1 + s2, sm = s1 - s2;
+        const float2 sp2 = make_float2(sp, sp), sm2 = make_float2(sm, sm);
+        const float2* qc2 = reinterpret_cast<const float2*>(qi + (size_t)vp * QIS);
+        const float2* qs2 = reinterpret_cast<const float2*>(qi + (size_t)vp * QIS + SOFF);
+#pragma unroll
+        for (int k = 0; k < NTC; ++k) tc[k] = ffma2(qc2[k], sp2, tc[k]);
+#pragma unroll
+        for (int k = 0; k < NTS; ++k) ts[k] = ffma2(qs2[k], sm2, ts[k]);
+    }
+#pragma unroll
+    for (int m = 0; m <= LB; ++m) F[(m * U + u) * 32 + lane] = (m & 1) ? tc[m / 2].y : tc[m / 2].x;
+#pragma unroll
+    for (int m = 1; m <= LB; ++m) F[((LB + m) * U + u) * 32 + lane] = ((m - 1) & 1) ? ts[(m - 1) / 2].y : ts[(m - 1) / 2].x;
+}
+
+// Stage C (row S4b, Eq.(40)): Gauss-Legendre quadrature over the grid rows for one
+// (column, |m|); pairs are (+m, -m).  Ts: [32][Lo2s] staging for the bulk store.
+template <int LB>
+__device__ __forceinline__ void stage_c(const float* __restrict__ wp, int UP2, const float* __restrict__ F,
+                                        float* __restrict__ ts_col, int m, int lmax_out, int U, int Uh, int lane)
+{
+    constexpr int UH = core_uhmax(LB);
+    float2 tp[UH], tm[UH];
+#pragma unroll
+    for (int e = 0; e < UH; ++e) {
+        float2 n = make_float2(0.f, 0.f), s = make_float2(0.f, 0.f);
+        if (e < Uh) {
+            const int rn = (m * U + e) * 32 + lane, rs = (m * U + (U - 1 - e)) * 32 + lane;
+            const int off = LB * U * 32;
+            n.x = F[rn];
+            s.x = F[rs];
+            if (m > 0) { n.y = F[rn + off]; s.y = F[rs + off]; }
+        }
+        tp[e] = fadd2(n, s);
+        tm[e] = fsub2(n, s);
+    }
+    for (int l = m; l <= lmax_out; l += 2) {
+#pragma unroll
+        for (int par = 0; par < 2; ++par) {
+            const int ll = l + par;
+            if (ll > lmax_out) break;
+            const float4* tab = reinterpret_cast<const float4*>(wp + (size_t)tri_index(ll, m) * UP2 * 2);
+            float2 a0 = make_float2(0.f, 0.f), a1 = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int e = 0; e < UH; e += 2) {
+                const float4 t4 = tab[e / 2];
+                a0 = ffma2(make_float2(t4.x, t4.y), par ? tm[e] : tp[e], a0);
+                if (e + 1 < UH) a1 = ffma2(make_float2(t4.z, t4.w), par ? tm[e + 1] : tp[e + 1], a1);
+            }
+            const float2 r = fadd2(a0, a1);
+            ts_col[ll * ll + ll + m] = r.x;
+            if (m > 0) ts_col[ll * ll + ll - m] = r.y;
+        }
+    }
+}
+
+template <int LB, bool ODD>
+__global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    constexpr int MR = 2 * LB + 1;
+    uint64_t* bar_tab = reinterpret_cast<uint64_t*>(smem);
+    uint64_t* bar_h = reinterpret_cast<uint64_t*>(smem + 16);  // [2]
+    const unsigned char* blob = smem + a.off_blob;
+    const float* ta = reinterpret_cast<const float*>(blob + a.tab.ta);
+    const float* wp = reinterpret_cast<const float*>(blob + a.tab.wp);
+    const float* qf = reinterpret_cast<const float*>(blob + a.tab.qf);
+    const float* qi = reinterpret_cast<const float*>(blob + a.tab.qi);
+    const int* sched = reinterpret_cast<const int*>(blob + a.tab.sched);
+    float* F = reinterpret_cast<float*>(smem + a.off_f);
+    float* Ts = reinterpret_cast<float*>(smem + a.off_ts);
+    const int plane = MR * a.U * 32;
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int hfl = 32 * a.L2s;  // floats of one factor's H block
+    const uint32_t hbytes = (uint32_t)hfl * 4;
+
+    auto load_h = [&](long long g, int buf) {
+        float* dst = reinterpret_cast<float*>(smem + a.off_hs + (size_t)buf * a.hs_bytes);
+        mbar_arrive_expect_tx(&bar_h[buf], 2 * hbytes);
+        tma_load_span(dst, a.Ha + g * hfl, hbytes, &bar_h[buf]);
+        tma_load_span(dst + hfl, a.Hb + g * hfl, hbytes, &bar_h[buf]);
+    };
+
+    if (threadIdx.x == 0) {
+        mbar_init(bar_tab, 1);
+        mbar_init(&bar_h[0], 1);
+        mbar_init(&bar_h[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    long long g = blockIdx.x;
+    if (threadIdx.x == 0) {
+        mbar_arrive_expect_tx(bar_tab, (uint32_t)a.tab.bytes);
+        tma_load_span(smem + a.off_blob, a.blob, (uint32_t)a.tab.bytes, bar_tab);
+        if (g < a.ngroups) load_h(g, 0);
+    }
+    mbar_wait(bar_tab, 0);
+
+    const int MAXI = a.tab.MAXI;
+    const int na = sched[0 * kMaxWarps + warp], nb = sched[1 * kMaxWarps + warp], nc = sched[2 * kMaxWarps + warp];
+    const int* ia = sched + 3 * kMaxWarps + (0 * kMaxWarps + warp) * MAXI;
+    const int* ib = sched + 3 * kMaxWarps + (1 * kMaxWarps + warp) * MAXI;
+    const int* ic = sched + 3 * kMaxWarps + (2 * kMaxWarps + warp) * MAXI;
+
+    int buf = 0;
+    uint32_t phases = 0u;  // bit b = parity to wait for on bar_h[b]
+    for (; g < a.ngroups; g += gridDim.x) {
+        const long long gn = g + gridDim.x;
+        if (a.dbl && threadIdx.x == 0 && gn < a.ngroups) load_h(gn, buf ^ 1);
+        mbar_wait(&bar_h[buf], (phases >> buf) & 1u);
+        phases ^= 1u << buf;
+        const float* hs = reinterpret_cast<const float*>(smem + a.off_hs + (size_t)buf * a.hs_bytes);
+        const float* ha = hs + lane * a.L2s;
+        const float* hb = hs + hfl + lane * a.L2s;
+
+        // ---- stage A
+        for (int k = 0; k < na; ++k) {
+            const int m = ia[k];
+            if (!ODD) {
+                stage_a_even<LB>(ta, a.tab.UP2, ha, hb, F, F + plane, m, a.lmax, a.U, a.Uh, lane);
+            } else {
+#pragma unroll 1
+                for (int f = 0; f < 2; ++f)
+                    stage_a_odd<LB>(ta, a.tab.UP2, f ? hb : ha, F + (2 * f) * plane, F + (2 * f + 1) * plane, m, a.lmax,
+                                    a.U, a.Uh, lane);
+            }
+        }
+        __syncthreads();
+        if (!a.dbl && threadIdx.x == 0 && gn < a.ngroups) load_h(gn, 0);
+
+        // ---- stage B
+        for (int k = 0; k < nb; ++k)
+            stage_b<LB, ODD>(qf, qi, a.tab.QFS, a.tab.QIS, a.tab.SOFF, F, plane, a.U, ib[k], a.Vh, lane);
+        // the previous group's bulk store must have finished reading Ts before stage C rewrites it
+        if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        __syncthreads();
+
+        // ---- stage C
+        for (int k = 0; k < nc; ++k) stage_c<LB>(wp, a.tab.UP2, F, Ts + lane * a.Lo2s, ic[k], a.lmax_out, a.U, a.Uh, lane);
+        fence_async_smem();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            tma_store_1d(a.T + g * 32 * a.Lo2s, Ts, (uint32_t)(32 * a.Lo2s * 4));
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+        if (a.dbl) buf ^= 1;
+    }
+    if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+}
+
+// ------------------------------------------------------------------------------------------------
+// Launch
+// ------------------------------------------------------------------------------------------------
+static int g_num_sms = 0;
+static int num_sms()
+{
+    if (!g_num_sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
+        if (g_num_sms <= 0) g_num_sms = 148;
+    }
+    return g_num_sms;
+}
+
+constexpr size_t kSmemPerSm = 227 * 1024;
+
+// 0 if the fast kernel cannot run this plan; otherwise the dynamic shared memory per CTA, with *dbl set.
+static size_t core_config(const Plan* p, bool odd, const CorePlan* c, bool* dbl)
+{
+    if (p->LB > 8) return 0;  // instantiated for LB <= 8 only (register budget of stage B)
+    const size_t two = core_smem_bytes(p, odd, c->tab, true), one = core_smem_bytes(p, odd, c->tab, false);
+    // prefer double-buffered H when it does not cost a resident CTA
+    const size_t ctas_two = kSmemPerSm / (two + 1024), ctas_one = kSmemPerSm / (one + 1024);
+    if (ctas_one == 0) return 0;
+    *dbl = (ctas_two == ctas_one);
+    return *dbl ? two : one;
+}
+
+bool onsite_fast_supported(const Plan* p, bool odd)
+{
+    if (p->LB > 8) return false;
+    const CorePlan* c = get_core_plan(p, odd);
+    if (!c) return false;
+    bool dbl;
+    return core_config(p, odd, c, &dbl) != 0;
+}
+
+template <int LB, bool ODD>
+static int launch_fast_t(const Plan* p, const CorePlan* c, const float* Ha, const float* Hb, float* T, int64_t ncols,
+                         cudaStream_t st)
+{
+    bool dbl = false;
+    const size_t smem = core_config(p, ODD, c, &dbl);
+    if (!smem) { set_error("onsite fast core: plan does not fit shared memory"); return CGTP_ERR_UNSUPPORTED; }
+    CoreArgs a;
+    a.tab = c->tab;
+    a.blob = c->blob;
+    a.Ha = Ha;
+    a.Hb = Hb;
+    a.T = T;
+    a.ngroups = (ncols + 31) / 32;
+    a.lmax = p->lmax;
+    a.lmax_out = p->lmax_out;
+    a.U = p->U;
+    a.Uh = p->Uh;
+    a.Vh = p->Vh;
+    a.L2s = onsite_fast_hstride(p);
+    a.Lo2s = onsite_fast_tstride(p);
+    a.dbl = dbl ? 1 : 0;
+    a.hs_bytes = 2 * 32 * a.L2s * 4;
+    a.off_blob = 64;
+    a.off_hs = a.off_blob + c->tab.bytes;
+    a.off_f = a.off_hs + (dbl ? 2 : 1) * a.hs_bytes;
+    a.off_ts = a.off_f + (ODD ? 4 : 2) * (2 * LB + 1) * p->U * 32 * 4;
+    auto kern = onsite_fast_kernel<LB, ODD>;
+    CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int ctas_per_sm = (int)(kSmemPerSm / (smem + 1024));
+    int64_t grid = (int64_t)num_sms() * ctas_per_sm;
+    if (grid > a.ngroups) grid = a.ngroups;
+    LaunchScope scope(ODD ? K_ONSITE_ODD : K_ONSITE_EVEN, st);
+    kern<<<(unsigned)grid, 32 * c->tab.NW, smem, st>>>(a);
+    CGTP_CUDA_CHECK(cudaGetLastError());
+    return CGTP_OK;
+}
+
+int launch_onsite_fast(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols,
+                       cudaStream_t st)
+{
+    if (ncols <= 0) return CGTP_OK;
+    const CorePlan* c = get_core_plan(p, odd);
+    if (!c) return CGTP_ERR_CUDA;
+    switch (p->LB) {
+#define CGTP_CASE(B)                                                              \
+    case B:                                                                       \
+        return odd ? launch_fast_t<B, true>(p, c, Ha, Hb, T, ncols, st)           \
+                   : launch_fast_t<B, false>(p, c, Ha, Hb, T, ncols, st);
+        CGTP_CASE(1) CGTP_CASE(2) CGTP_CASE(3) CGTP_CASE(4) CGTP_CASE(5) CGTP_CASE(6) CGTP_CASE(8)
+#undef CGTP_CASE
+    }
+    set_error("onsite fast core: no kernel for band limit %d", p->LB);
+    return CGTP_ERR_UNSUPPORTED;
+}
+
+}  // namespace cgtp

@@ -140,7 +140,7 @@ static int launch_onsite_t(const Plan* p, const float* Ha, const float* Hb, floa
     return CGTP_OK;
 }
 
-int launch_onsite_core(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols,
+int launch_onsite_generic(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols,
                        cudaStream_t st)
 {
     if (ncols <= 0) return CGTP_OK;

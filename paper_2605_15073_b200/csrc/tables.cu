@@ -97,7 +97,7 @@ int profile_collect(double* ms, int64_t* launches)
 
 // ------------------------------------------------------------------------------ Gauss-Legendre
 // Nodes by Newton iteration on P_U, northern node first; exact mirror symmetry is enforced.
-static void gauss_legendre(int U, std::vector<double>& x, std::vector<double>& w)
+void gauss_legendre(int U, std::vector<double>& x, std::vector<double>& w)
 {
     x.assign(U, 0.0);
     w.assign(U, 0.0);
@@ -130,6 +130,27 @@ static void gauss_legendre(int U, std::vector<double>& x, std::vector<double>& w
         w[i] = w[U - 1 - i] = 2.0 / ((1.0 - z * z) * dp * dp);
     }
     if (U % 2) x[U / 2] = 0.0;
+}
+
+// P[u][l][m] = P~_l^m(x_u), 0 <= m <= l <= LB: orthonormal on S^2 (R1), no Condon-Shortley phase (R2).
+void legendre_values(int U, int LB, const std::vector<double>& x, std::vector<double>& P)
+{
+    const int LL = LB + 1;
+    P.assign((size_t)U * LL * LL, 0.0);
+    auto at = [&](int u, int l, int m) -> double& { return P[((size_t)u * LL + l) * LL + m]; };
+    for (int u = 0; u < U; ++u) {
+        double ct = x[u], st = std::sqrt(1.0 - ct * ct);
+        at(u, 0, 0) = std::sqrt(1.0 / (4.0 * M_PI));
+        for (int m = 1; m <= LB; ++m) at(u, m, m) = std::sqrt((2.0 * m + 1.0) / (2.0 * m)) * st * at(u, m - 1, m - 1);
+        for (int m = 0; m <= LB; ++m) {
+            if (m + 1 <= LB) at(u, m + 1, m) = std::sqrt(2.0 * m + 3.0) * ct * at(u, m, m);
+            for (int l = m + 2; l <= LB; ++l) {
+                double a = std::sqrt((4.0 * l * l - 1.0) / ((double)l * l - (double)m * m));
+                double b = std::sqrt(((l - 1.0) * (l - 1.0) - (double)m * m) / (4.0 * (l - 1.0) * (l - 1.0) - 1.0));
+                at(u, l, m) = a * (ct * at(u, l - 1, m) - b * at(u, l - 2, m));
+            }
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------ plan cache
@@ -174,21 +195,9 @@ const Plan* get_plan(int lmax, int lmax_out)
 
     // normalised associated Legendre functions at every node (FP64), P[u][l][m]
     const int LL = LB + 1;
-    std::vector<double> P((size_t)U * LL * LL, 0.0);
+    std::vector<double> P;
+    legendre_values(U, LB, x, P);
     auto at = [&](int u, int l, int m) -> double& { return P[((size_t)u * LL + l) * LL + m]; };
-    for (int u = 0; u < U; ++u) {
-        double ct = x[u], st = std::sqrt(1.0 - ct * ct);
-        at(u, 0, 0) = std::sqrt(1.0 / (4.0 * M_PI));
-        for (int m = 1; m <= LB; ++m) at(u, m, m) = std::sqrt((2.0 * m + 1.0) / (2.0 * m)) * st * at(u, m - 1, m - 1);
-        for (int m = 0; m <= LB; ++m) {
-            if (m + 1 <= LB) at(u, m + 1, m) = std::sqrt(2.0 * m + 3.0) * ct * at(u, m, m);
-            for (int l = m + 2; l <= LB; ++l) {
-                double a = std::sqrt((4.0 * l * l - 1.0) / ((double)l * l - (double)m * m));
-                double b = std::sqrt(((l - 1.0) * (l - 1.0) - (double)m * m) / (4.0 * (l - 1.0) * (l - 1.0) - 1.0));
-                at(u, l, m) = a * (ct * at(u, l - 1, m) - b * at(u, l - 2, m));
-            }
-        }
-    }
 
     std::vector<float> PT((size_t)Uh * NTRI, 0.f), DT(PT), ST(PT), WP(PT);
     for (int u = 0; u < Uh; ++u) {
