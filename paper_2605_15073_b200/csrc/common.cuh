@@ -141,6 +141,9 @@ struct ProjArgs {
     int64_t batch;
 };
 int launch_proj(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st);
+// Fast path of launch_proj (proj_fast.cu): TMA-staged features, packed FP32 FMAs; *handled = false when the
+// layout conditions (even K, 16-byte aligned atom blocks, ...) do not hold and the generic kernel must run.
+int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st, bool* handled);
 
 // S2-S4 fused: T[col][lm] from Ha[col], Hb[col]; ncols columns of one parity.
 // Generic kernel (any compiled band limit): H rows of stride p->L2p, T rows of stride p->Lo2p.

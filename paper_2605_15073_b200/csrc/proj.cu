@@ -126,6 +126,11 @@ int launch_proj(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st)
     }
     if (nargs == 1) pack.a[1] = args[0];
     if (max_cols == 0 || max_m == 0) return CGTP_OK;
+    {
+        bool handled = false;
+        const int rc = launch_proj_fast(args, nargs, kind, st, &handled);
+        if (rc != CGTP_OK || handled) return rc;
+    }
     constexpr int TM = 8, TN = 8;
     const int CW = 32 * TN;
     int64_t gx = (max_cols + CW - 1) / CW;
