@@ -167,6 +167,10 @@ int launch_node_synth(const Plan* p, bool odd, const float* H, float* G, int64_t
 int launch_edge(const Plan* p, bool odd, const float* G, const int64_t* row_ptr, const int64_t* edge_index,
                 int64_t E, const float* edge_vec, const float* edge_radial, const int* perm_par, int Cpar, int C,
                 float* S, int64_t nodes, const int32_t* status, cudaStream_t st);
+// Persistent TMA-ring form of launch_edge (edge_ring.cu); *handled = false -> use launch_edge's generic kernel.
+int launch_edge_ring(const Plan* p, bool odd, const float* G, const int64_t* row_ptr, const int64_t* edge_index,
+                     int64_t E, const float* edge_vec, const float* edge_radial, const int* perm_par, int Cpar, int C,
+                     float* S, int64_t nodes, const int32_t* status, cudaStream_t st, bool* handled);
 // M5: T[col][Lo2p] = analysis of S[col][UVp]
 int launch_analysis(const Plan* p, bool odd, const float* S, float* T, int64_t ncols, cudaStream_t st);
 

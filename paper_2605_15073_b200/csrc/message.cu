@@ -350,6 +350,12 @@ int launch_edge(const Plan* p, bool odd, const float* G, const int64_t* row_ptr,
                 int64_t nodes, const int32_t* status, cudaStream_t st)
 {
     if (Cpar <= 0 || nodes <= 0) return CGTP_OK;
+    {
+        bool handled = false;
+        const int rc = launch_edge_ring(p, odd, G, row_ptr, edge_index, E, edge_vec, edge_radial, perm_par, Cpar, C, S,
+                                        nodes, status, st, &handled);
+        if (rc != CGTP_OK || handled) return rc;
+    }
     const int QP = p->UVp / 4;
     int cbmax = EDGE_NI * EDGE_NT / QP;
     if (cbmax < 1) { set_error("edge kernel: grid of lmax=%d too large for the accumulator tile", p->lmax); return CGTP_ERR_UNSUPPORTED; }
