@@ -38,7 +38,7 @@ struct EdgeRingArgs {
     int cb;     // channels per CTA block
     int nblk;   // channel blocks
     int cs;     // channels per sub-block (one ring stage)
-    int G_;     // channel groups per sub-block pass (QT == 1): 512 / QP
+    int G_;     // channel groups per sub-block pass: 512 / QP
     int EC;     // edges per geometry chunk
     int NST;    // ring stages
     int geo_smem;  // 1: grid geometry staged in shared memory
@@ -54,11 +54,10 @@ __device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, %0;"
 __device__ __forceinline__ float2 lo2(const float4& v) { return make_float2(v.x, v.y); }
 __device__ __forceinline__ float2 hi2(const float4& v) { return make_float2(v.z, v.w); }
 
-// Thread <-> accumulator mapping.  QT == 1 (QP <= 512 quads per grid field): thread = (channel group cg,
-// quad q0), accumulator x of a sub-block = channel x*G + cg at quad q0, so the edge field at q0 stays in
-// registers for every channel of the edge.  QT > 1: thread owns quads tid + 512*j (j < QT), accumulator
-// x = channel x / QT at quad j = x % QT.
-template <bool ODD, int NSBT, int QT>
+// Thread <-> accumulator mapping (QP <= 512 float4 quads per grid field, true for every band limit the
+// library compiles): thread = (channel group cg, quad q0), accumulator x of a sub-block = channel
+// x*G + cg at quad q0, so the edge field at q0 stays in registers for every channel of the edge.
+template <bool ODD, int NSBT>
 __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
 {
     constexpr int NF = ODD ? 2 : 1;
@@ -129,23 +128,15 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
     }
 
     // ================================= consumer warps =================================
+    constexpr int QT = 1;
     int chl[ER_NA], qd[QT];
     bool qok[QT];
-    if (QT == 1) {
+    {
         const int cg = tid / QP;
         qd[0] = tid - cg * QP;
         qok[0] = cg < a.G_;
 #pragma unroll
         for (int x = 0; x < ER_NA; ++x) chl[x] = x * a.G_ + cg;
-    } else {
-#pragma unroll
-        for (int j = 0; j < QT; ++j) {
-            qd[j] = tid + ER_CONS * j;
-            qok[j] = qd[j] < QP;
-            if (!qok[j]) qd[j] = 0;
-        }
-#pragma unroll
-        for (int x = 0; x < ER_NA; ++x) chl[x] = x / QT;
     }
     const float* geo = a.geo_smem ? geo_s : a.p.geo;
     const int lmax = a.p.lmax;
@@ -227,9 +218,7 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
                         mbar_wait(&full[slot], phase);
 #pragma unroll
                         for (int x = 0; x < ER_NA; ++x) {
-                            constexpr int dummy = 0;
-                            (void)dummy;
-                            const int j = (QT == 1) ? 0 : (x % QT);
+                            constexpr int j = 0;
                             if (chl[x] < ncs && qok[j]) {
                                 const float r = rrow[sb * cs + chl[x]];
                                 if (!ODD) {
@@ -267,7 +256,7 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
                 float4* sdst = reinterpret_cast<float4*>(a.S + ((size_t)i * Cpar + kc0 + sb * cs) * UVp);
 #pragma unroll
                 for (int x = 0; x < ER_NA; ++x) {
-                    const int j = (QT == 1) ? 0 : (x % QT);
+                    constexpr int j = 0;
                     if (chl[x] < ncs && qok[j])
                         sdst[chl[x] * QP + qd[j]] =
                             make_float4(acc[sb][x][0].x, acc[sb][x][0].y, acc[sb][x][1].x, acc[sb][x][1].y);
@@ -292,10 +281,10 @@ static int er_num_sms()
     return n;
 }
 
-template <bool ODD, int NSBT, int QT>
+template <bool ODD, int NSBT>
 static int launch_ring_t(const EdgeRingArgs& a, size_t smem, int grid, cudaStream_t st)
 {
-    auto kern = edge_ring_kernel<ODD, NSBT, QT>;
+    auto kern = edge_ring_kernel<ODD, NSBT>;
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<grid, ER_NT, smem, st>>>(a);
     CGTP_CUDA_CHECK(cudaGetLastError());
@@ -313,15 +302,9 @@ int launch_edge_ring(const Plan* p, bool odd, const float* G, const int64_t* row
     if (p->lmax >= ER_LMAX) return CGTP_OK;
     const int nf = odd ? 2 : 1;
     const int QP = p->UVp / 4;
-    int QT = 1, G_ = 1, cs_max;
-    if (QP <= ER_CONS) {
-        G_ = ER_CONS / QP;
-        cs_max = ER_NA * G_;
-    } else {
-        QT = (QP + ER_CONS - 1) / ER_CONS;
-        if (QT > ER_NA) return CGTP_OK;
-        cs_max = ER_NA / QT;
-    }
+    if (QP > ER_CONS) return CGTP_OK;  // cannot happen for band limits <= 20 (QP <= 473)
+    const int G_ = ER_CONS / QP;
+    const int cs_max = ER_NA * G_;
     constexpr int NSB_MAX = 6;
     // channel blocks: as few as possible with at most NSB_MAX sub-blocks each
     const int cb_max = cs_max * NSB_MAX;
@@ -329,10 +312,9 @@ int launch_edge_ring(const Plan* p, bool odd, const float* G, const int64_t* row
     const int cb = (Cpar + nblk - 1) / nblk;
     int nsb = (cb + cs_max - 1) / cs_max;
     int cs = (cb + nsb - 1) / nsb;  // balanced sub-blocks
-    if (QT == 1) cs = std::min(cs_max, (cs + G_ - 1) / G_ * G_);  // whole channel groups
+    cs = std::min(cs_max, (cs + G_ - 1) / G_ * G_);  // whole channel groups
     nsb = (cb + cs - 1) / cs;
     int nsbt = nsb <= 1 ? 1 : nsb <= 2 ? 2 : nsb <= 3 ? 3 : nsb <= 4 ? 4 : 6;
-    if (QT > 1) nsbt = 6;
 
     const size_t budget = 200 * 1024;
     const size_t stage_bytes = (size_t)cs * nf * p->UVp * 4;
@@ -379,18 +361,14 @@ int launch_edge_ring(const Plan* p, bool odd, const float* G, const int64_t* row
 
     LaunchScope scope(odd ? K_EDGE_ODD : K_EDGE_EVEN, st);
     int rc = CGTP_OK;
-#define CGTP_RING(N, Q)                                                                                       \
-    rc = odd ? launch_ring_t<true, N, Q>(a, smem, grid, st) : launch_ring_t<false, N, Q>(a, smem, grid, st)
-    if (QT == 1) {
-        switch (nsbt) {
-        case 1: CGTP_RING(1, 1); break;
-        case 2: CGTP_RING(2, 1); break;
-        case 3: CGTP_RING(3, 1); break;
-        case 4: CGTP_RING(4, 1); break;
-        default: CGTP_RING(6, 1); break;
-        }
-    } else {
-        CGTP_RING(6, 2);
+#define CGTP_RING(N) \
+    rc = odd ? launch_ring_t<true, N>(a, smem, grid, st) : launch_ring_t<false, N>(a, smem, grid, st)
+    switch (nsbt) {
+    case 1: CGTP_RING(1); break;
+    case 2: CGTP_RING(2); break;
+    case 3: CGTP_RING(3); break;
+    case 4: CGTP_RING(4); break;
+    default: CGTP_RING(6); break;
     }
 #undef CGTP_RING
     if (rc == CGTP_OK) *handled = true;

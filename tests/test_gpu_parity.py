@@ -79,6 +79,10 @@ def test_onsite_config0_full():
     (4, 4, 8, 8, 40, [0] * 8),                 # all even: sector 1 must be zero
     (4, 4, 8, 8, 40, [1] * 8),                 # all odd: sector 0 must be zero
     (6, 6, 40, 33, 50, None),                  # N, C not multiples of the GEMM tiles
+    (16, 16, 40, 40, 3, None),                 # 289 coefficients > one 256-column tile of proj_fast (sub-tiles)
+    (2, 2, 72, 136, 61, None),                 # several row blocks, ragged last atom group and row slab
+    (5, 5, 12, 20, 9, [0] * 10 + [1] * 10),    # K = 12 / 10: small K chunks
+    (3, 3, 8, 8, 300, [0, 0, 0, 1, 1, 1, 1, 1]),  # odd number of even channels: generic projection kernel
 ])
 def test_onsite_small_shapes(lmax, lmax_out, N, C, batch, mask):
     inp = synthetic.make_onsite(lmax, lmax_out, N, C, batch, seed=100 + lmax * 7 + lmax_out, parity_mask=mask)
@@ -229,6 +233,26 @@ def test_message_small_ragged_graphs(lmax, lmax_out, N, C, nodes, mask):
     e = sector_err(got, ref)
     assert max(e) < TOL, e
     assert np.abs(got[deg == 0]).max() == 0.0  # receivers without edges -> zeros
+
+
+@pytest.mark.parametrize("lmax,lmax_out,N,C,deg,mask", [
+    # one receiver with more in-edges than the producer warp's batch (32) and the geometry chunk
+    (3, 3, 8, 8, [70, 0, 33, 1, 32, 8], None),
+    # more even channels than one CTA block of the edge kernel holds (several channel blocks)
+    (6, 6, 4, 132, [5, 0, 9, 3], [0] * 130 + [1] * 2),
+    # sub-blocks with a ragged last channel group
+    (8, 8, 4, 14, [4, 7, 0, 2], [0] * 9 + [1] * 5),
+    # the largest grid the library supports (lmax = lmax_out = 20: 473 float4 quads per field)
+    (20, 20, 4, 2, [2, 0, 3], [0, 1]),
+])
+def test_message_edge_kernel_shapes(lmax, lmax_out, N, C, deg, mask):
+    """Shapes that exercise the tiling limits of the TMA-ring edge kernel (edge_ring.cu)."""
+    deg = np.asarray(deg)
+    m = synthetic.make_message(lmax, lmax_out, N, C, len(deg), deg, seed=300 + lmax, parity_mask=mask)
+    got, ref = run_message(m, check=True), oracle_message(m)
+    e = sector_err(got, ref)
+    assert max(e) < TOL, e
+    assert np.abs(got[deg == 0]).max() == 0.0
 
 
 def test_message_config2_full_even_and_halfhalf():
