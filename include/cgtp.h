@@ -117,6 +117,23 @@ int cgtp_message(const float* node_feats, const int64_t* edge_index, const float
                  int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask, float* out,
                  int64_t nodes, int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Bipartite form of cgtp_message, the building block of receiver sharding: the
+ * sum of Eq.(2) runs over the in-edges of the n_recv receivers this call owns, while the
+ * senders j index a (possibly larger) set of n_send nodes whose features are given.
+ *   node_feats  device [n_send, N, (lmax+1)^2]
+ *   edge_index  device int64 [2, E]: row 0 = sender in [0, n_send), row 1 = receiver in [0, n_recv),
+ *               sorted by receiver
+ *   out         device [n_recv, 2, N, (lmax_out+1)^2]
+ * Everything else as cgtp_message, which is the case n_send = n_recv = nodes. */
+size_t cgtp_message_bipartite_workspace_bytes(int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask,
+                                              int64_t n_send, int64_t n_recv, int64_t E);
+
+int cgtp_message_bipartite(const float* node_feats, const int64_t* edge_index, const float* edge_vec,
+                           const float* edge_radial, const float* W_node, const float* W_out,
+                           int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask, float* out,
+                           int64_t n_send, int64_t n_recv, int64_t E, void* workspace, size_t workspace_bytes,
+                           void* cuda_stream);
+
 /* Synchronises `cuda_stream` and returns the graph status the last cgtp_message on this workspace
  * left: CGTP_OK or CGTP_ERR_GRAPH (CGTP_ERR_CUDA if the stream reports an error). */
 int cgtp_message_status(const void* workspace, void* cuda_stream);

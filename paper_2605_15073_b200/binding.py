@@ -50,6 +50,10 @@ def lib() -> ctypes.CDLL:
     L.cgtp_message_workspace_bytes.argtypes = [i, i, i, i, vp, i64, i64]
     L.cgtp_message.restype = i
     L.cgtp_message.argtypes = [vp, vp, vp, vp, vp, vp, i, i, i, i, vp, vp, i64, i64, vp, sz, vp]
+    L.cgtp_message_bipartite_workspace_bytes.restype = sz
+    L.cgtp_message_bipartite_workspace_bytes.argtypes = [i, i, i, i, vp, i64, i64, i64]
+    L.cgtp_message_bipartite.restype = i
+    L.cgtp_message_bipartite.argtypes = [vp, vp, vp, vp, vp, vp, i, i, i, i, vp, vp, i64, i64, i64, vp, sz, vp]
     L.cgtp_message_status.restype = i
     L.cgtp_message_status.argtypes = [vp, vp]
     L.cgtp_build_segments.restype = i
@@ -190,6 +194,43 @@ def cgtp_message(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, l
         rc = lib().cgtp_message(X.data_ptr(), ei.data_ptr(), ev.data_ptr(), er.data_ptr(), W_node.data_ptr(),
                                 W_out.data_ptr(), lmax, lmax_out, N, C, mask.ctypes.data, out.data_ptr(), nodes, E,
                                 ws.data_ptr(), ws.numel(), sp)
+        _check(rc)
+        if check:
+            _check(lib().cgtp_message_status(ws.data_ptr(), sp))
+    return out
+
+
+def cgtp_message_bipartite(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, N, C,
+                           parity_mask, n_recv: int, out=None, workspace=None, stream=None, check: bool = False):
+    """out[n_recv, 2, N, (lmax_out+1)^2]: message passing onto n_recv receivers from the n_send =
+    node_feats.shape[0] sender nodes (see include/cgtp.h); receivers in edge_index are local, in [0, n_recv)."""
+    f32 = torch.float32
+    X = _dev(node_feats, f32, "node_feats")
+    ei = _dev(edge_index, torch.int64, "edge_index")
+    ev, er = _dev(edge_vec, f32, "edge_vec"), _dev(edge_radial, f32, "edge_radial")
+    W_node, W_out = _dev(W_node, f32, "W_node"), _dev(W_out, f32, "W_out")
+    n_send, E = X.shape[0], ei.shape[1]
+    L2, Lo2 = (lmax + 1) ** 2, (lmax_out + 1) ** 2
+    if tuple(X.shape) != (n_send, N, L2):
+        raise ValueError("node_feats must be [n_send, N, (lmax+1)^2]")
+    if tuple(ei.shape) != (2, E) or tuple(ev.shape) != (E, 3) or tuple(er.shape) != (E, C):
+        raise ValueError("edge_index [2,E], edge_vec [E,3], edge_radial [E,C] expected")
+    if tuple(W_node.shape) != (C, N) or tuple(W_out.shape) != (N, C):
+        raise ValueError("W_node must be [C, N] and W_out [N, C]")
+    mask = _mask(parity_mask, C)
+    if out is None:
+        out = torch.empty((n_recv, 2, N, Lo2), dtype=f32, device=X.device)
+    else:
+        _dev(out, f32, "out")
+        if tuple(out.shape) != (n_recv, 2, N, Lo2):
+            raise ValueError("out must be [n_recv, 2, N, (lmax_out+1)^2]")
+    nbytes = lib().cgtp_message_bipartite_workspace_bytes(lmax, lmax_out, N, C, mask.ctypes.data, n_send, n_recv, E)
+    ws = _workspace(X.device, nbytes) if workspace is None else workspace
+    sp = _stream_ptr(stream)
+    with torch.cuda.device(X.device):
+        rc = lib().cgtp_message_bipartite(X.data_ptr(), ei.data_ptr(), ev.data_ptr(), er.data_ptr(), W_node.data_ptr(),
+                                          W_out.data_ptr(), lmax, lmax_out, N, C, mask.ctypes.data, out.data_ptr(),
+                                          n_send, n_recv, E, ws.data_ptr(), ws.numel(), sp)
         _check(rc)
         if check:
             _check(lib().cgtp_message_status(ws.data_ptr(), sp))

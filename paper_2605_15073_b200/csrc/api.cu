@@ -54,13 +54,14 @@ static size_t onsite_ws_bytes(int lmax, int lmax_out, int C, int64_t batch)
     return ((size_t)batch * C + 64) * (2 * (L2p + 4) + (Lo2p + 4)) * sizeof(float) + 8 * 256;
 }
 
-static size_t message_ws_bytes(int lmax, int lmax_out, int C, int Co, int64_t nodes)
+static size_t message_ws_bytes(int lmax, int lmax_out, int C, int Co, int64_t n_send, int64_t n_recv)
 {
     const size_t L2p = round_up((lmax + 1) * (lmax + 1), 4), Lo2p = round_up((lmax_out + 1) * (lmax_out + 1), 4);
     const int U = (2 * lmax + lmax_out + 2) / 2, V = 2 * lmax + lmax_out + 1;
     const size_t UVp = round_up(U * V, 4);
-    size_t fl = (size_t)nodes * C * (L2p + Lo2p) + (size_t)nodes * (C + Co) * UVp + (size_t)nodes * C * UVp;
-    return 256 + fl * sizeof(float) + (size_t)(nodes + 1) * sizeof(int64_t) + 12 * 256;
+    // H, G for the senders; S, T, row_ptr for the receivers
+    size_t fl = (size_t)n_send * C * L2p + (size_t)n_send * (C + Co) * UVp + (size_t)n_recv * C * (UVp + Lo2p);
+    return 256 + fl * sizeof(float) + (size_t)(n_recv + 1) * sizeof(int64_t) + 12 * 256;
 }
 
 }  // namespace cgtp
@@ -209,7 +210,18 @@ size_t cgtp_message_workspace_bytes(int lmax, int lmax_out, int N, int C, const 
     if (lmax < 0 || lmax_out < 0 || C <= 0 || nodes < 0 || !parity_mask) return 0;
     int Co = 0;
     for (int c = 0; c < C; ++c) Co += parity_mask[c] ? 1 : 0;
-    return message_ws_bytes(lmax, lmax_out, C, Co, nodes);
+    return message_ws_bytes(lmax, lmax_out, C, Co, nodes, nodes);
+}
+
+size_t cgtp_message_bipartite_workspace_bytes(int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask,
+                                              int64_t n_send, int64_t n_recv, int64_t E)
+{
+    (void)N;
+    (void)E;
+    if (lmax < 0 || lmax_out < 0 || C <= 0 || n_send < 0 || n_recv < 0 || !parity_mask) return 0;
+    int Co = 0;
+    for (int c = 0; c < C; ++c) Co += parity_mask[c] ? 1 : 0;
+    return message_ws_bytes(lmax, lmax_out, C, Co, n_send, n_recv);
 }
 
 int cgtp_build_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int64_t* row_ptr, int32_t* status,
@@ -218,20 +230,21 @@ int cgtp_build_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int
     clear_error();
     if (E < 0 || nodes < 0) { set_error("negative size"); return CGTP_ERR_INVALID; }
     if ((!edge_index && E > 0) || !row_ptr || !status) { set_error("null pointer argument"); return CGTP_ERR_INVALID; }
-    return launch_segments(edge_index, E, nodes, row_ptr, status, static_cast<cudaStream_t>(cuda_stream));
+    return launch_segments(edge_index, E, nodes, nodes, row_ptr, status, static_cast<cudaStream_t>(cuda_stream));
 }
 
-int cgtp_message(const float* node_feats, const int64_t* edge_index, const float* edge_vec, const float* edge_radial,
-                 const float* W_node, const float* W_out, int lmax, int lmax_out, int N, int C,
-                 const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* workspace,
-                 size_t workspace_bytes, void* cuda_stream)
+int cgtp_message_bipartite(const float* node_feats, const int64_t* edge_index, const float* edge_vec,
+                           const float* edge_radial, const float* W_node, const float* W_out, int lmax, int lmax_out,
+                           int N, int C, const uint8_t* parity_mask, float* out, int64_t n_send, int64_t nodes,
+                           int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     clear_error();
     int rc = check_common(lmax, lmax_out, N, C, parity_mask);
     if (rc) return rc;
-    if (nodes < 0 || E < 0) { set_error("negative size"); return CGTP_ERR_INVALID; }
+    if (nodes < 0 || n_send < 0 || E < 0) { set_error("negative size"); return CGTP_ERR_INVALID; }
     if (nodes == 0) return CGTP_OK;
-    if (!node_feats || !W_node || !W_out || !out || !workspace || (E > 0 && (!edge_index || !edge_vec || !edge_radial))) {
+    if (n_send == 0 && E > 0) { set_error("edges without sender nodes"); return CGTP_ERR_INVALID; }
+    if ((!node_feats && n_send > 0) || !W_node || !W_out || !out || !workspace || (E > 0 && (!edge_index || !edge_vec || !edge_radial))) {
         set_error("null pointer argument");
         return CGTP_ERR_INVALID;
     }
@@ -247,25 +260,25 @@ int cgtp_message(const float* node_feats, const int64_t* edge_index, const float
     const ChannelPlan* cp = get_channel_plan(C, parity_mask);
     if (!cp) return CGTP_ERR_CUDA;
     const int Ce = cp->Ce, Co = cp->Co;
-    if (workspace_bytes < message_ws_bytes(lmax, lmax_out, C, Co, nodes)) {
-        set_error("workspace too small: %zu < %zu bytes", workspace_bytes, message_ws_bytes(lmax, lmax_out, C, Co, nodes));
+    if (workspace_bytes < message_ws_bytes(lmax, lmax_out, C, Co, n_send, nodes)) {
+        set_error("workspace too small: %zu < %zu bytes", workspace_bytes, message_ws_bytes(lmax, lmax_out, C, Co, n_send, nodes));
         return CGTP_ERR_INVALID;
     }
 
     Carver cv(workspace);
     int32_t* status = cv.take<int32_t>(1);
     int64_t* row_ptr = cv.take<int64_t>((size_t)nodes + 1);
-    float* H_e = cv.take<float>((size_t)nodes * Ce * p->L2p);
-    float* H_o = cv.take<float>((size_t)nodes * Co * p->L2p);
-    float* G_e = cv.take<float>((size_t)nodes * Ce * p->UVp);
-    float* G_o = cv.take<float>((size_t)nodes * Co * 2 * p->UVp);
+    float* H_e = cv.take<float>((size_t)n_send * Ce * p->L2p);
+    float* H_o = cv.take<float>((size_t)n_send * Co * p->L2p);
+    float* G_e = cv.take<float>((size_t)n_send * Ce * p->UVp);
+    float* G_o = cv.take<float>((size_t)n_send * Co * 2 * p->UVp);
     float* S_e = cv.take<float>((size_t)nodes * Ce * p->UVp);
     float* S_o = cv.take<float>((size_t)nodes * Co * p->UVp);
     float* T_e = cv.take<float>((size_t)nodes * Ce * p->Lo2p);
     float* T_o = cv.take<float>((size_t)nodes * Co * p->Lo2p);
 
     // M0
-    rc = launch_segments(edge_index, E, nodes, row_ptr, status, st);
+    rc = launch_segments(edge_index, E, nodes, n_send, row_ptr, status, st);
     if (rc) return rc;
 
     // M1: H = W_node . node_feats (Eq.(47))
@@ -287,14 +300,14 @@ int cgtp_message(const float* node_feats, const int64_t* edge_index, const float
     a.o_bs1 = (int64_t)Co * p->L2p;
     a.m_split = Ce;
     a.o_rs = p->L2p;
-    a.batch = nodes;
+    a.batch = n_send;
     rc = launch_proj(&a, 1, K_PROJ_IN, st);
     if (rc) return rc;
 
     // M2
-    rc = launch_node_synth(p, false, H_e, G_e, nodes * Ce, st);
+    rc = launch_node_synth(p, false, H_e, G_e, n_send * Ce, st);
     if (rc) return rc;
-    rc = launch_node_synth(p, true, H_o, G_o, nodes * Co, st);
+    rc = launch_node_synth(p, true, H_o, G_o, n_send * Co, st);
     if (rc) return rc;
 
     // M3 + M4
@@ -333,6 +346,15 @@ int cgtp_message(const float* node_feats, const int64_t* edge_index, const float
         b.batch = nodes;
     }
     return launch_proj(po, 2, K_PROJ_OUT, st);
+}
+
+int cgtp_message(const float* node_feats, const int64_t* edge_index, const float* edge_vec, const float* edge_radial,
+                 const float* W_node, const float* W_out, int lmax, int lmax_out, int N, int C,
+                 const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* workspace,
+                 size_t workspace_bytes, void* cuda_stream)
+{
+    return cgtp_message_bipartite(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, N, C,
+                                  parity_mask, out, nodes, nodes, E, workspace, workspace_bytes, cuda_stream);
 }
 
 int cgtp_message_status(const void* workspace, void* cuda_stream)

@@ -158,9 +158,9 @@ inline int onsite_fast_tstride(const Plan* p) { return p->Lo2 | 1; }
 int launch_onsite_fast(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols,
                        cudaStream_t st);
 
-// M0
-int launch_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int64_t* row_ptr, int32_t* status,
-                    cudaStream_t st);
+// M0: row_ptr over `nodes` receivers; senders are validated against n_send
+int launch_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int64_t n_send, int64_t* row_ptr,
+                    int32_t* status, cudaStream_t st);
 // M2: grid fields of the projected node features.  even: G[col][UVp]; odd: G[col][2][UVp] (d_theta, (1/sin)d_phi)
 int launch_node_synth(const Plan* p, bool odd, const float* H, float* G, int64_t ncols, cudaStream_t st);
 // M3+M4: S[i][kc][UVp] = sum_e radial * edge-field (x) sender grid, channels of one parity.

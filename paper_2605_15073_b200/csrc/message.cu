@@ -20,7 +20,7 @@ namespace cgtp {
 // M0: segmentation
 // =============================================================================================
 __global__ void segments_kernel(const int64_t* __restrict__ edge_index, long long E, long long nodes,
-                                int64_t* __restrict__ row_ptr, int32_t* __restrict__ status)
+                                long long n_send, int64_t* __restrict__ row_ptr, int32_t* __restrict__ status)
 {
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (e > E) return;
@@ -31,7 +31,7 @@ __global__ void segments_kernel(const int64_t* __restrict__ edge_index, long lon
     bool bad = false;
     if (e < E) {
         const long long s = snd[e];
-        if (r < 0 || r >= nodes || s < 0 || s >= nodes) bad = true;
+        if (r < 0 || r >= nodes || s < 0 || s >= n_send) bad = true;
     }
     if (e > 0 && (r_prev < 0 || r_prev >= nodes)) bad = true;
     if (r < r_prev) bad = true;
@@ -45,8 +45,8 @@ __global__ void segments_kernel(const int64_t* __restrict__ edge_index, long lon
 
 __global__ void set_status_kernel(int32_t* status, int32_t v) { *status = v; }
 
-int launch_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int64_t* row_ptr, int32_t* status,
-                    cudaStream_t st)
+int launch_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int64_t n_send, int64_t* row_ptr,
+                    int32_t* status, cudaStream_t st)
 {
     {
         LaunchScope scope(K_MISC, st);
@@ -56,7 +56,8 @@ int launch_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int64_t
     const int NT = 256;
     int64_t grid = (E + 1 + NT - 1) / NT;
     LaunchScope scope(K_SEGMENTS, st);
-    segments_kernel<<<(unsigned)grid, NT, 0, st>>>(edge_index, (long long)E, (long long)nodes, row_ptr, status);
+    segments_kernel<<<(unsigned)grid, NT, 0, st>>>(edge_index, (long long)E, (long long)nodes, (long long)n_send, row_ptr,
+                                                    status);
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
 }

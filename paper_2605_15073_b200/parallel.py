@@ -1,0 +1,129 @@
+"""Host-side sharding of the hot path over ranks (one process per GPU, torch.distributed).
+
+The paper's implementation is single-GPU; DESIGN.md "Multi-GPU" derives the split:
+
+* on-site (Eq.(1)): atoms are independent -> split the batch, no collective;
+* message passing (Eq.(2)): the receiver-sorted edge list is cut into contiguous
+  receiver ranges balanced by work; every rank owns the node features, the in-edges and the output
+  rows of its range.  A sender may live on any rank, so the one exchange step is an all-gather of
+  the node features (NCCL over NVLink on GPUs) before `cgtp_message_bipartite`; outputs need no
+  reduction.
+
+Only index arithmetic and the collective live here; the arithmetic of the method stays in the CUDA
+kernels (`compute` defaults to binding.cgtp_message_bipartite).
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import Callable, Optional, Sequence
+
+import numpy as np
+import torch
+import torch.distributed as dist
+
+
+# ------------------------------------------------------------------------------------------ on-site
+def shard_batch(batch: int, world: int, rank: int) -> tuple[int, int]:
+    """[start, stop) of the atoms rank `rank` owns: contiguous, sizes differ by at most one."""
+    if world < 1 or not 0 <= rank < world or batch < 0:
+        raise ValueError("bad shard_batch arguments")
+    q, r = divmod(batch, world)
+    start = rank * q + min(rank, r)
+    return start, start + q + (1 if rank < r else 0)
+
+
+# ---------------------------------------------------------------------------------- message passing
+def row_ptr_from_receivers(receivers: np.ndarray, nodes: int) -> np.ndarray:
+    """CSR offsets of a receiver-sorted edge list (host copy of what cgtp_build_segments computes)."""
+    receivers = np.asarray(receivers, np.int64)
+    if receivers.size and (np.any(np.diff(receivers) < 0) or receivers[0] < 0 or receivers[-1] >= nodes):
+        raise ValueError("edge list is not receiver-sorted or has a receiver outside [0, nodes)")
+    return np.searchsorted(receivers, np.arange(nodes + 1, dtype=np.int64), side="left").astype(np.int64)
+
+
+def shard_receivers(row_ptr: np.ndarray, world: int, node_cost: float = 4.0) -> np.ndarray:
+    """Cuts [0, nodes) into `world` contiguous receiver ranges of near-equal cost.
+
+    cost(range) = edges in the range + node_cost * nodes in the range (the per-receiver analysis and
+    projections are not free).  Returns bounds int64 [world+1], bounds[0] = 0, bounds[-1] = nodes,
+    non-decreasing; the same on every rank (a pure function of row_ptr)."""
+    row_ptr = np.asarray(row_ptr, np.int64)
+    nodes = row_ptr.shape[0] - 1
+    if world < 1 or nodes < 0:
+        raise ValueError("bad shard_receivers arguments")
+    cum = row_ptr.astype(np.float64) + node_cost * np.arange(nodes + 1, dtype=np.float64)
+    total = cum[-1]
+    targets = total * np.arange(1, world, dtype=np.float64) / world
+    cuts = np.searchsorted(cum, targets, side="left")
+    # choose the nearer of the two neighbouring node boundaries
+    for k, (c, t) in enumerate(zip(cuts, targets)):
+        if 0 < c <= nodes and abs(cum[c - 1] - t) <= abs(cum[min(c, nodes)] - t):
+            cuts[k] = c - 1
+    bounds = np.concatenate([[0], np.clip(cuts, 0, nodes), [nodes]]).astype(np.int64)
+    return np.maximum.accumulate(bounds)
+
+
+def local_edge_slice(row_ptr: np.ndarray, lo: int, hi: int) -> tuple[int, int]:
+    """[e0, e1) of the receiver-sorted edge list whose receivers lie in [lo, hi)."""
+    return int(row_ptr[lo]), int(row_ptr[hi])
+
+
+@dataclass
+class MessageShard:
+    """What one rank holds: its receiver range, its in-edges (global sender ids, receivers rebased to
+    the range) and the features of its own nodes."""
+    lo: int
+    hi: int
+    edge_index: torch.Tensor   # int64 [2, E_local]; row 0 global sender, row 1 receiver - lo
+    edge_vec: torch.Tensor     # [E_local, 3]
+    edge_radial: torch.Tensor  # [E_local, C]
+    node_feats: torch.Tensor   # [hi - lo, N, (lmax+1)^2]
+
+
+def make_shard(node_feats: torch.Tensor, edge_index: torch.Tensor, edge_vec: torch.Tensor,
+               edge_radial: torch.Tensor, bounds: Sequence[int], rank: int) -> MessageShard:
+    """Cuts rank `rank`'s shard out of a full (replicated) problem; used by tests and by callers that
+    load the whole graph on every rank."""
+    nodes = node_feats.shape[0]
+    rp = row_ptr_from_receivers(edge_index[1].cpu().numpy(), nodes)
+    lo, hi = int(bounds[rank]), int(bounds[rank + 1])
+    e0, e1 = local_edge_slice(rp, lo, hi)
+    ei = edge_index[:, e0:e1].clone()
+    ei[1] -= lo
+    return MessageShard(lo, hi, ei.contiguous(), edge_vec[e0:e1].contiguous(), edge_radial[e0:e1].contiguous(),
+                        node_feats[lo:hi].contiguous())
+
+
+def all_gather_node_feats(local: torch.Tensor, bounds: Sequence[int], group=None) -> torch.Tensor:
+    """All-gather of the per-rank node-feature blocks into [nodes, N, L^2] (the one exchange step).
+
+    Ranges may differ in length, so every rank pads its block to the longest range, one
+    all_gather_into_tensor moves the padded blocks (NCCL on GPUs, gloo on CPU), and the padding is
+    dropped on arrival."""
+    world = dist.get_world_size(group)
+    rank = dist.get_rank(group)
+    sizes = [int(bounds[r + 1] - bounds[r]) for r in range(world)]
+    if local.shape[0] != sizes[rank]:
+        raise ValueError("local block does not match the receiver bounds")
+    longest = max(max(sizes), 1)
+    tail = tuple(local.shape[1:])
+    send = local.new_zeros((longest,) + tail)
+    send[: sizes[rank]] = local
+    recv = local.new_empty((world * longest,) + tail)
+    dist.all_gather_into_tensor(recv, send, group=group)
+    recv = recv.view((world, longest) + tail)
+    return torch.cat([recv[r, : sizes[r]] for r in range(world)], dim=0)
+
+
+def message_sharded(shard: MessageShard, bounds: Sequence[int], W_node: torch.Tensor, W_out: torch.Tensor,
+                    lmax: int, lmax_out: int, N: int, C: int, parity_mask, group=None,
+                    compute: Optional[Callable] = None) -> torch.Tensor:
+    """out rows [lo, hi) of the message-passing layer on this rank: all-gather node features, then the
+    bipartite kernel path over the local in-edges.  `compute(node_feats_all, edge_index, edge_vec,
+    edge_radial, W_node, W_out, lmax, lmax_out, N, C, parity_mask, n_recv)` defaults to the CUDA path."""
+    if compute is None:
+        from . import binding
+        compute = binding.cgtp_message_bipartite
+    feats = all_gather_node_feats(shard.node_feats, bounds, group)
+    return compute(feats, shard.edge_index, shard.edge_vec, shard.edge_radial, W_node, W_out, lmax, lmax_out, N, C,
+                   parity_mask, shard.hi - shard.lo)

@@ -324,3 +324,34 @@ def test_message_host_entry_matches_device_entry():
     host = cg.cgtp_message_host(pin(m.node_feats), pin(m.edge_index), pin(m.edge_vec), pin(m.edge_radial),
                                 pin(m.W_node), pin(m.W_out), 3, 3, 8, 8, m.parity_mask).numpy()
     assert np.array_equal(dev, host)
+
+
+def test_message_bipartite_shards_reproduce_the_full_call():
+    """Receiver sharding on one GPU: each shard's cgtp_message_bipartite call over its own
+    in-edges (global senders, local receivers) gives exactly the rows of the unsharded call, and matches the oracle."""
+    from paper_2605_15073_b200 import parallel
+    rng = np.random.default_rng(21)
+    deg = rng.integers(0, 14, 61)
+    deg[[0, 30]] = 0
+    m = synthetic.make_message(3, 3, 8, 8, 61, deg, seed=91)
+    full = run_message(m, check=True)
+    ref = oracle_message(m)
+    assert max(sector_err(full, ref)) < TOL
+    rp = parallel.row_ptr_from_receivers(m.edge_index[1], m.nodes)
+    bounds = parallel.shard_receivers(rp, 3)
+    t = torch.from_numpy
+    for r in range(3):
+        s = parallel.make_shard(t(m.node_feats), t(m.edge_index), t(m.edge_vec), t(m.edge_radial), bounds, r)
+        got = cg.cgtp_message_bipartite(_cuda(m.node_feats), s.edge_index.cuda(), s.edge_vec.cuda(), s.edge_radial.cuda(),
+                                        _cuda(m.W_node), _cuda(m.W_out), m.lmax, m.lmax_out, m.N, m.C, m.parity_mask,
+                                        s.hi - s.lo, check=True)
+        torch.cuda.synchronize()
+        assert np.array_equal(got.cpu().numpy(), full[s.lo:s.hi])
+    # a sender index outside [0, n_send) is a graph error
+    bad = m.edge_index.copy()
+    bad[0, 0] = m.nodes
+    with pytest.raises(cg.CgtpError) as ei:
+        cg.cgtp_message_bipartite(_cuda(m.node_feats), _cuda(bad), _cuda(m.edge_vec), _cuda(m.edge_radial),
+                                  _cuda(m.W_node), _cuda(m.W_out), m.lmax, m.lmax_out, m.N, m.C, m.parity_mask,
+                                  m.nodes, check=True)
+    assert ei.value.code == cg.ERR_GRAPH
