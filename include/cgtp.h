@@ -162,6 +162,23 @@ int cgtp_message_host(const float* node_feats, const int64_t* edge_index, const 
                       int64_t nodes, int64_t E, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * Arithmetic of the channel projections (Eq.(35), Eq.(41) :346, Eq.(47) :398, Eq.(55) :427),
+ * the dense GEMM-shaped stages of the path.  Process-wide, read at every call:
+ *   CGTP_MATH_FP32    FP32 fused multiply-adds on the CUDA cores (default; the path the 1e-5 parity bar is
+ *                     stated for);
+ *   CGTP_MATH_3XTF32  tcgen05 tensor cores, every FP32 operand split into two TF32 terms, three MMAs per
+ *                     product, FP32 accumulation in tensor memory (error ~1e-6 relative, reported separately);
+ *   CGTP_MATH_TF32    tcgen05 tensor cores, single TF32 pass (error ~1e-3 relative; fails the parity bar by
+ *                     design, for throughput comparison only).
+ * Every other stage always runs in FP32.  cgtp_set_math_mode returns CGTP_ERR_INVALID for an unknown mode.
+ * ------------------------------------------------------------------------------------------- */
+#define CGTP_MATH_FP32 0
+#define CGTP_MATH_3XTF32 1
+#define CGTP_MATH_TF32 2
+int cgtp_set_math_mode(int mode);
+int cgtp_get_math_mode(void);
+
+/* ---------------------------------------------------------------------------------------------
  * Instrumentation (used by bench.py; never needed for results).
  * cgtp_launch_count: number of kernels this library has launched since it was loaded.
  * cgtp_profile_enable(1): record a CUDA-event pair around every kernel launch (on the launching

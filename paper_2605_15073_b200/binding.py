@@ -62,6 +62,9 @@ def lib() -> ctypes.CDLL:
     L.cgtp_onsite_host.argtypes = [vp, vp, vp, vp, vp, i, i, i, i, vp, vp, i64, vp]
     L.cgtp_message_host.restype = i
     L.cgtp_message_host.argtypes = [vp, vp, vp, vp, vp, vp, i, i, i, i, vp, vp, i64, i64, vp]
+    L.cgtp_set_math_mode.restype = i
+    L.cgtp_set_math_mode.argtypes = [i]
+    L.cgtp_get_math_mode.restype = i
     L.cgtp_launch_count.restype = i64
     L.cgtp_profile_kinds.restype = i
     L.cgtp_profile_kind_name.restype = ctypes.c_char_p
@@ -291,6 +294,18 @@ def cgtp_message_host(node_feats, edge_index, edge_vec, edge_radial, W_node, W_o
                                  _stream_ptr(stream))
     _check(rc)
     return out
+
+
+MATH_FP32, MATH_3XTF32, MATH_TF32 = 0, 1, 2
+
+
+def cgtp_set_math_mode(mode: int) -> None:
+    """Arithmetic of the channel projections: MATH_FP32 (default), MATH_3XTF32 or MATH_TF32 (tcgen05)."""
+    _check(lib().cgtp_set_math_mode(int(mode)))
+
+
+def cgtp_get_math_mode() -> int:
+    return lib().cgtp_get_math_mode()
 
 
 def cgtp_launch_count() -> int:

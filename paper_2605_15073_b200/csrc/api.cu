@@ -500,6 +500,16 @@ int cgtp_message_host(const float* node_feats, const int64_t* edge_index, const 
     return grc;
 }
 
+// ------------------------------------------------------------------------------------------ math mode
+int cgtp_set_math_mode(int mode)
+{
+    clear_error();
+    if (mode < CGTP_MATH_FP32 || mode > CGTP_MATH_TF32) { set_error("unknown math mode %d", mode); return CGTP_ERR_INVALID; }
+    cgtp::set_math_mode(mode);
+    return CGTP_OK;
+}
+int cgtp_get_math_mode(void) { return cgtp::get_math_mode(); }
+
 // ------------------------------------------------------------------------------------ instrumentation
 int64_t cgtp_launch_count(void) { return cgtp::launch_count(); }
 int cgtp_profile_kinds(void) { return K_COUNT; }

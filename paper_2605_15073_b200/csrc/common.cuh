@@ -145,6 +145,12 @@ int launch_proj(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st);
 // layout conditions (even K, 16-byte aligned atom blocks, ...) do not hold and the generic kernel must run.
 int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st, bool* handled);
 
+// Tensor-core path of launch_proj (proj_tc.cu: tcgen05.mma kind::tf32, TMEM accumulators), taken only when
+// the math mode is CGTP_MATH_3XTF32 / CGTP_MATH_TF32; *handled = false otherwise.
+int launch_proj_tc(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st, bool* handled);
+void set_math_mode(int mode);
+int get_math_mode();
+
 // S2-S4 fused: T[col][lm] from Ha[col], Hb[col]; ncols columns of one parity.
 // Generic kernel (any compiled band limit): H rows of stride p->L2p, T rows of stride p->Lo2p.
 int launch_onsite_generic(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols,

@@ -6,9 +6,10 @@
 // with the grid fields in registers only.  What differs is the mapping to the machine:
 //   * lane = column: a CTA works on groups of 32 (atom, rank-channel) columns; every shared-memory array
 //     has the column as its fastest index (or an odd row stride), so all accesses are conflict-free;
-//   * packed FP32 FMAs (FFMA2, fma.rn.f32x2): the scalar FFMA issue rate of sm_100a tops out near 48
-//     TFLOP/s, the packed form reaches 66 TFLOP/s (measured); pairs are (+m,-m) rows, (A,B) factors or
-//     (d_theta, d_phi) components, with the tables stored in the duplicated / interleaved form each needs;
+//   * packed FP32 FMAs (FFMA2, fma.rn.f32x2; 65 TFLOP/s measured against 57 for scalar FFMA): pairs are
+//     (+m,-m) rows, (A,B) factors or (d_theta, d_phi) components.  Where the table value is common to both
+//     halves it is a plain scalar: FFMA2 takes a 32-bit register broadcast to both lanes (SASS `R.F32`), so
+//     one 128-bit broadcast load feeds four packed FMAs; only the odd stage A needs interleaved pairs;
 //   * warps of a CTA split each stage by a static, host-computed schedule (longest-processing-time
 //     assignment of the ragged per-m work), CTAs are persistent over column groups and prefetch the
 //     next group's coefficients with TMA bulk copies while computing.
@@ -25,13 +26,13 @@ constexpr int kMaxWarps = 8;
 
 // Byte offsets (multiples of 16) into the packed table blob of one (plan, parity).
 struct CoreTab {
-    int ta;     // stage A: [tri(l,m)][UP2] float2.  even: (P~,P~); odd: (d_theta P~, m P~/sin theta)
-    int wp;     // stage C: [tri(l,m)][UP2] float2 (w P~, w P~), equator row halved
-    int qf;     // stage B forward: [Vh][QFS] float2 (q,q); entry r<=LB: cos row r, r>LB: sin row r-LB
+    int ta;     // stage A: even [tri(l,m)][UP4] float P~; odd [tri(l,m)][UP2] float2 (d_theta P~, m P~/sin theta)
+    int wp;     // stage C: [tri(l,m)][UP4] float w P~, equator row halved
+    int qf;     // stage B forward: [Vh][QFS] float; entry r<=LB: cos row r, r>LB: sin row r-LB
     int qi;     // stage B inverse: [Vh][QIS] float, (2 pi/V) q folded in; cos m at m, sin m at SOFF+m-1
     int sched;  // int: per stage s (A,B,C) and warp w: cnt[s][w] at s*kMaxWarps+w, then items[s][w][MAXI]
     int bytes;
-    int UP2, QFS, QIS, SOFF, MAXI;
+    int UP2, UP4, QFS, QIS, SOFF, MAXI;
     int NW;
 };
 
@@ -100,7 +101,8 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
     CoreTab t;
     std::memset(&t, 0, sizeof t);
     t.UP2 = round_up(core_uhmax(LB), 2);
-    t.QFS = round_up(MR, 2);
+    t.UP4 = round_up(core_uhmax(LB), 4);
+    t.QFS = round_up(MR, 4);
     t.SOFF = round_up(LB + 1, 2);
     t.QIS = round_up(t.SOFF + LB, 4);
     const int ntri = (LB + 1) * (LB + 2) / 2;
@@ -110,7 +112,7 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
     legendre_values(U, LB, x, P);
     auto at = [&](int u, int l, int m) -> double { return P[((size_t)u * LL + l) * LL + m]; };
 
-    std::vector<float> TA((size_t)ntri * t.UP2 * 2, 0.f), WP(TA.size(), 0.f);
+    std::vector<float> TA((size_t)ntri * (odd ? t.UP2 * 2 : t.UP4), 0.f), WP((size_t)ntri * t.UP4, 0.f);
     for (int u = 0; u < Uh; ++u) {
         const double ct = x[u], st = std::sqrt(1.0 - ct * ct);
         const double wu = w[u] * ((U % 2 && u == Uh - 1) ? 0.5 : 1.0);
@@ -120,17 +122,17 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
                 const double pm1 = (l - 1 >= m) ? at(u, l - 1, m) : 0.0;
                 const double c = (l > 0) ? std::sqrt((2.0 * l + 1.0) * ((double)l * l - (double)m * m) / (2.0 * l - 1.0)) : 0.0;
                 const double dth = (l * ct * pv - c * pm1) / st;
-                const size_t k = ((size_t)tri_index(l, m) * t.UP2 + u) * 2;
                 if (!odd) {
-                    TA[k] = TA[k + 1] = (float)pv;
+                    TA[(size_t)tri_index(l, m) * t.UP4 + u] = (float)pv;
                 } else {
+                    const size_t k = ((size_t)tri_index(l, m) * t.UP2 + u) * 2;
                     TA[k] = (float)dth;
                     TA[k + 1] = (float)(m * pv / st);
                 }
-                WP[k] = WP[k + 1] = (float)(wu * pv);
+                WP[(size_t)tri_index(l, m) * t.UP4 + u] = (float)(wu * pv);
             }
     }
-    std::vector<float> QF((size_t)Vh * t.QFS * 2, 0.f), QI((size_t)Vh * t.QIS, 0.f);
+    std::vector<float> QF((size_t)Vh * t.QFS, 0.f), QI((size_t)Vh * t.QIS, 0.f);
     for (int v = 0; v < Vh; ++v) {
         const double ph = 2.0 * M_PI * v / V;
         const bool paired = (v != 0) && !(V % 2 == 0 && v == V / 2);
@@ -138,10 +140,10 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
         for (int m = 0; m <= LB; ++m) {
             const double qc = (m == 0) ? 1.0 : std::sqrt(2.0) * std::cos(m * ph);
             const double qs = (m == 0 || !paired) ? 0.0 : std::sqrt(2.0) * std::sin(m * ph);
-            QF[((size_t)v * t.QFS + m) * 2] = QF[((size_t)v * t.QFS + m) * 2 + 1] = (float)qc;
+            QF[(size_t)v * t.QFS + m] = (float)qc;
             QI[(size_t)v * t.QIS + m] = (float)(wv * qc);
             if (m > 0) {
-                QF[((size_t)v * t.QFS + LB + m) * 2] = QF[((size_t)v * t.QFS + LB + m) * 2 + 1] = (float)qs;
+                QF[(size_t)v * t.QFS + LB + m] = (float)qs;
                 QI[(size_t)v * t.QIS + t.SOFF + m - 1] = (float)(wv * qs);
             }
         }
@@ -240,7 +242,7 @@ struct CoreArgs {
 // Stage A (row S2a), even channels.  Thread = (column, |m|): rows m (cos) and LB+m (sin) of both factors
 // for all grid rows; pairs are (+m, -m), the table is stored duplicated.
 template <int LB>
-__device__ __forceinline__ void stage_a_even(const float* __restrict__ ta, int UP2, const float* __restrict__ ha,
+__device__ __forceinline__ void stage_a_even(const float* __restrict__ ta, int UP4, const float* __restrict__ ha,
                                              const float* __restrict__ hb, float* __restrict__ Fa,
                                              float* __restrict__ Fb, int m, int lmax, int U, int Uh, int lane)
 {
@@ -257,19 +259,20 @@ __device__ __forceinline__ void stage_a_even(const float* __restrict__ ta, int U
         for (int par = 0; par < 2; ++par) {
             const int ll = l + par;
             if (ll > lmax) break;
-            const float4* tab = reinterpret_cast<const float4*>(ta + (size_t)tri_index(ll, m) * UP2 * 2);
+            const float4* tab = reinterpret_cast<const float4*>(ta + (size_t)tri_index(ll, m) * UP4);
             const int ip = ll * ll + ll + m, im = ll * ll + ll - m;
             const float2 xa = make_float2(ha[ip], ha[im]);
             const float2 xb = make_float2(hb[ip], hb[im]);
 #pragma unroll
-            for (int e = 0; e < UH; e += 2) {
-                const float4 t4 = tab[e / 2];
-                acc[0][par][e] = ffma2(make_float2(t4.x, t4.y), xa, acc[0][par][e]);
-                acc[1][par][e] = ffma2(make_float2(t4.x, t4.y), xb, acc[1][par][e]);
-                if (e + 1 < UH) {
-                    acc[0][par][e + 1] = ffma2(make_float2(t4.z, t4.w), xa, acc[0][par][e + 1]);
-                    acc[1][par][e + 1] = ffma2(make_float2(t4.z, t4.w), xb, acc[1][par][e + 1]);
-                }
+            for (int e = 0; e < UH; e += 4) {
+                const float4 t4 = tab[e / 4];
+                const float tv[4] = {t4.x, t4.y, t4.z, t4.w};
+#pragma unroll
+                for (int h = 0; h < 4; ++h)
+                    if (e + h < UH) {
+                        acc[0][par][e + h] = ffma2(xa, make_float2(tv[h], tv[h]), acc[0][par][e + h]);
+                        acc[1][par][e + h] = ffma2(xb, make_float2(tv[h], tv[h]), acc[1][par][e + h]);
+                    }
             }
         }
     }
@@ -369,7 +372,7 @@ __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const floa
     for (int k = 0; k < NTS; ++k) ts[k] = make_float2(0.f, 0.f);
 
     for (int vp = 0; vp < Vh; ++vp) {
-        const float4* q4 = reinterpret_cast<const float4*>(qf + (size_t)vp * QFS * 2);
+        const float4* q4 = reinterpret_cast<const float4*>(qf + (size_t)vp * QFS);
         float2 Cs[NP][2], Ss[NP][2];  // two chains each for ILP
 #pragma unroll
         for (int k = 0; k < NP; ++k) {
@@ -377,17 +380,18 @@ __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const floa
             Ss[k][0] = Ss[k][1] = make_float2(0.f, 0.f);
         }
 #pragma unroll
-        for (int r = 0; r < MR; r += 2) {
-            const float4 t4 = q4[r / 2];
+        for (int r = 0; r < MR; r += 4) {
+            const float4 t4 = q4[r / 4];
+            const float qv[4] = {t4.x, t4.y, t4.z, t4.w};
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
+            for (int h = 0; h < 4; ++h) {
                 const int rr = r + h;
                 if (rr >= MR) break;
-                const float2 q2 = h ? make_float2(t4.z, t4.w) : make_float2(t4.x, t4.y);
+                const float2 q2 = make_float2(qv[h], qv[h]);
 #pragma unroll
                 for (int k = 0; k < NP; ++k) {
-                    if (rr <= LB) Cs[k][rr & 1] = ffma2(q2, f[k][rr], Cs[k][rr & 1]);
-                    else Ss[k][rr & 1] = ffma2(q2, f[k][rr], Ss[k][rr & 1]);
+                    if (rr <= LB) Cs[k][rr & 1] = ffma2(f[k][rr], q2, Cs[k][rr & 1]);
+                    else Ss[k][rr & 1] = ffma2(f[k][rr], q2, Ss[k][rr & 1]);
                 }
             }
         }
@@ -423,7 +427,7 @@ __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const floa
 // Stage C (row S4b, Eq.(40)): Gauss-Legendre quadrature over the grid rows for one
 // (column, |m|); pairs are (+m, -m).  Ts: [32][Lo2s] staging for the bulk store.
 template <int LB>
-__device__ __forceinline__ void stage_c(const float* __restrict__ wp, int UP2, const float* __restrict__ F,
+__device__ __forceinline__ void stage_c(const float* __restrict__ wp, int UP4, const float* __restrict__ F,
                                         float* __restrict__ ts_col, int m, int lmax_out, int U, int Uh, int lane)
 {
     constexpr int UH = core_uhmax(LB);
@@ -446,13 +450,19 @@ __device__ __forceinline__ void stage_c(const float* __restrict__ wp, int UP2, c
         for (int par = 0; par < 2; ++par) {
             const int ll = l + par;
             if (ll > lmax_out) break;
-            const float4* tab = reinterpret_cast<const float4*>(wp + (size_t)tri_index(ll, m) * UP2 * 2);
+            const float4* tab = reinterpret_cast<const float4*>(wp + (size_t)tri_index(ll, m) * UP4);
             float2 a0 = make_float2(0.f, 0.f), a1 = make_float2(0.f, 0.f);
 #pragma unroll
-            for (int e = 0; e < UH; e += 2) {
-                const float4 t4 = tab[e / 2];
-                a0 = ffma2(make_float2(t4.x, t4.y), par ? tm[e] : tp[e], a0);
-                if (e + 1 < UH) a1 = ffma2(make_float2(t4.z, t4.w), par ? tm[e + 1] : tp[e + 1], a1);
+            for (int e = 0; e < UH; e += 4) {
+                const float4 t4 = tab[e / 4];
+                const float tv[4] = {t4.x, t4.y, t4.z, t4.w};
+#pragma unroll
+                for (int h = 0; h < 4; ++h)
+                    if (e + h < UH) {
+                        const float2 x = par ? tm[e + h] : tp[e + h];
+                        if (h & 1) a1 = ffma2(x, make_float2(tv[h], tv[h]), a1);
+                        else a0 = ffma2(x, make_float2(tv[h], tv[h]), a0);
+                    }
             }
             const float2 r = fadd2(a0, a1);
             ts_col[ll * ll + ll + m] = r.x;
@@ -525,7 +535,7 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
         for (int k = 0; k < na; ++k) {
             const int m = ia[k];
             if (!ODD) {
-                stage_a_even<LB>(ta, a.tab.UP2, ha, hb, F, F + plane, m, a.lmax, a.U, a.Uh, lane);
+                stage_a_even<LB>(ta, a.tab.UP4, ha, hb, F, F + plane, m, a.lmax, a.U, a.Uh, lane);
             } else {
 #pragma unroll 1
                 for (int f = 0; f < 2; ++f)
@@ -544,7 +554,7 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
         __syncthreads();
 
         // ---- stage C
-        for (int k = 0; k < nc; ++k) stage_c<LB>(wp, a.tab.UP2, F, Ts + lane * a.Lo2s, ic[k], a.lmax_out, a.U, a.Uh, lane);
+        for (int k = 0; k < nc; ++k) stage_c<LB>(wp, a.tab.UP4, F, Ts + lane * a.Lo2s, ic[k], a.lmax_out, a.U, a.Uh, lane);
         fence_async_smem();
         __syncthreads();
         if (threadIdx.x == 0) {

@@ -128,6 +128,11 @@ int launch_proj(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st)
     if (max_cols == 0 || max_m == 0) return CGTP_OK;
     {
         bool handled = false;
+        const int rc = launch_proj_tc(args, nargs, kind, st, &handled);
+        if (rc != CGTP_OK || handled) return rc;
+    }
+    {
+        bool handled = false;
         const int rc = launch_proj_fast(args, nargs, kind, st, &handled);
         if (rc != CGTP_OK || handled) return rc;
     }

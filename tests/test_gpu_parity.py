@@ -355,3 +355,43 @@ def test_message_bipartite_shards_reproduce_the_full_call():
                                   _cuda(m.W_node), _cuda(m.W_out), m.lmax, m.lmax_out, m.N, m.C, m.parity_mask,
                                   m.nodes, check=True)
     assert ei.value.code == cg.ERR_GRAPH
+
+
+# ------------------------------------------------------------------------- tensor-core math modes
+@pytest.fixture
+def fp32_mode_after():
+    yield
+    cg.cgtp_set_math_mode(cg.MATH_FP32)
+
+
+@pytest.mark.parametrize("lmax,N,C,batch", [
+    (2, 8, 8, 64),       # configs[0] shape: one partial tile
+    (4, 24, 40, 70),     # K = 24 / 20: zero-padded K chunk; 40 channels padded to 64 TMEM columns
+    (6, 64, 64, 300),    # configs[1] shape, several tiles per CTA ring
+    (3, 136, 72, 40),    # K = 136: three K chunks accumulate in TMEM
+])
+def test_onsite_tensor_core_math_modes(lmax, N, C, batch, fp32_mode_after):
+    """cgtp_set_math_mode: the 3xTF32 tcgen05 projections meet the FP32 parity bar, single-pass TF32 lands at the
+    ~1e-3 the TF32 mantissa allows, and switching back restores the FP32 path bit for bit."""
+    inp = synthetic.make_onsite(lmax, lmax, N, C, batch, seed=500 + lmax)
+    ref = oracle_onsite(inp)
+    base = run_onsite(inp)
+    cg.cgtp_set_math_mode(cg.MATH_3XTF32)
+    assert cg.cgtp_get_math_mode() == cg.MATH_3XTF32
+    e3 = sector_err(run_onsite(inp), ref)
+    assert max(e3) < TOL, e3
+    cg.cgtp_set_math_mode(cg.MATH_TF32)
+    e1 = sector_err(run_onsite(inp), ref)
+    assert 1e-5 < max(e1) < 2e-2, e1
+    cg.cgtp_set_math_mode(cg.MATH_FP32)
+    assert np.array_equal(run_onsite(inp), base)
+    with pytest.raises(cg.CgtpError):
+        cg.cgtp_set_math_mode(7)
+
+
+def test_message_tensor_core_math_mode(fp32_mode_after):
+    m = synthetic.make_message(4, 4, 128, 128, 96, 6, seed=17)
+    ref = oracle_message(m)
+    cg.cgtp_set_math_mode(cg.MATH_3XTF32)
+    e3 = sector_err(run_message(m, check=True), ref)
+    assert max(e3) < TOL, e3
