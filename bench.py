@@ -343,6 +343,7 @@ def main():
         rate, dt_cpu, cores = oracle_onsite_rate(base, batch)
         line["cpu_baseline"] = {"value": rate, "unit": "contractions/s", "cores": cores, "kind": "oracle",
                                 "sample": f"all {batch} atoms of configs[1] once ({dt_cpu:.1f} s wall)"}
+        line["tensor_core"] = run_tensor_core(args, cg, step, out, lmax, lmax_out, N, C, Ce, Co, batch, peaks, peak_src)
         line["sweep"] = run_sweep(args, cg, synthetic, dev, fp32_peak_tflops, peaks)
         line["message"] = run_message(args, cg, synthetic, dev, peaks, peak_src)
     elif world == 1:
@@ -368,6 +369,44 @@ def time_steps(fn, steps, warmup):
     ev1.record()
     torch.cuda.synchronize()
     return ev0.elapsed_time(ev1) / steps
+
+
+def run_tensor_core(args, cg, step, out, lmax, lmax_out, N, C, Ce, Co, batch, peaks, peak_src):
+    """configs[1] with the channel projections (S1, S5) on tcgen05 tensor cores: 3xTF32 and single-pass TF32
+    (cgtp_set_math_mode).  Reported beside, never inside, the FP32 headline `value`."""
+    import torch
+    L2, Lo2 = (lmax + 1) ** 2, (lmax_out + 1) ** 2
+    fl = onsite_flops_per_atom(lmax, lmax_out, N, C, Ce, Co)
+    # compulsory bytes of the projection kernels: read X once, write the product once
+    by = {"proj_in": 4 * (2 * N * L2 + 2 * C * L2) * batch, "proj_out": 4 * (C * Lo2 + 2 * N * Lo2) * batch}
+    tf32_peak = peaks["bf16_tflops"] * 0.5  # nominal TF32 : bf16 ratio (B200_PROFILING.md table)
+    step(0)
+    torch.cuda.synchronize()
+    ref = out.clone()
+    res = {"tf32_peak_tflops": tf32_peak, "tf32_peak_source": f"{peak_src} bf16 peak x 0.5 (nominal TF32:bf16)"}
+    try:
+        for name, mode, passes in (("3xtf32", cg.MATH_3XTF32, 3), ("tf32", cg.MATH_TF32, 1)):
+            cg.cgtp_set_math_mode(mode)
+            ms = time_steps(lambda: step(0), max(args.steps // 2, 5), 3)
+            err = [float((out[:, s] - ref[:, s]).abs().max() / ref[:, s].abs().max()) for s in (0, 1)]
+            cg.cgtp_profile_enable(True)
+            for i in range(20):
+                step(i)
+            torch.cuda.synchronize()
+            prof = cg.cgtp_profile_collect()
+            cg.cgtp_profile_enable(False)
+            kern = {}
+            for k in ("proj_in", "proj_out"):
+                kms = prof[k][0] / prof[k][1]
+                kern[k] = {"avg_ms": kms, "alg_hbm_gbs": by[k] / (kms * 1e-3) / 1e9,
+                           "frac_hbm_peak": by[k] / (kms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                           "mma_tflops": passes * fl[k] * batch / (kms * 1e-3) / 1e12,
+                           "frac_tf32_peak": passes * fl[k] * batch / (kms * 1e-3) / 1e12 / tf32_peak}
+            res[name] = {"ms_per_step": ms, "contractions_per_s": batch / (ms * 1e-3),
+                         "max_rel_diff_vs_fp32_path": err, "bound": "hbm", "kernels": kern}
+    finally:
+        cg.cgtp_set_math_mode(cg.MATH_FP32)
+    return res
 
 
 def run_sweep(args, cg, synthetic, dev, fp32_peak_tflops, peaks):

@@ -186,45 +186,58 @@ __global__ void __launch_bounds__(TC_THREADS, 1) proj_tc_kernel(TcArgs a)
         const int col = lt & (TC_COLS - 1);            // column of the tile
         const int half = lt >> 7;                      // which half of the chunk's k-groups
         const int kg_begin = half * (KG / 2), kg_end = (half + 1) * (KG / 2);
-        int s = 0;
-        uint32_t ph = 0;
-        for (int64_t t = rank; t < ntiles; t += nctas) {
+        // unit = (tile, K chunk).  The loads of the next unit are issued before the current one is stored, so a
+        // thread keeps up to 2 x 32 independent 32-bit loads in flight (register double buffering).
+        auto load_unit = [&](int64_t t, int ch, float (&v)[8][4]) {
             const int64_t cc = t * TC_COLS + col;
             const bool live = cc < total_cols;
             const int64_t b = live ? cc / a.J : 0;
             const int j = live ? (int)(cc - b * a.J) : 0;
             const float* xcol = P.X + b * P.x_bs + j;
-            for (int ch = 0; ch < NCH; ++ch) {
-                mbar_wait(&empty[s], ph ^ 1u);
-                float4* dst_hi = As + (size_t)s * nsplit * a_f4;
-                float4* dst_lo = dst_hi + a_f4;
-                for (int kg0 = kg_begin; kg0 < kg_end; kg0 += 4) {
-                    float v[4][4];
 #pragma unroll
-                    for (int g = 0; g < 4; ++g)
+            for (int g = 0; g < 8; ++g)
 #pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            const int k = ch * KC + 4 * (kg0 + g) + q;
-                            v[g][q] = (live && kg0 + g < kg_end && k < K) ? __ldg(xcol + (int64_t)k * P.x_rs) : 0.f;
-                        }
-#pragma unroll
-                    for (int g = 0; g < 4; ++g) {
-                        if (kg0 + g >= kg_end) break;
-                        const int di = (kg0 + g) * TC_COLS + col;
-                        if (a.split) {
-                            const float4 hi = make_float4(tf32_hi(v[g][0]), tf32_hi(v[g][1]), tf32_hi(v[g][2]), tf32_hi(v[g][3]));
-                            dst_hi[di] = hi;
-                            dst_lo[di] = make_float4(v[g][0] - hi.x, v[g][1] - hi.y, v[g][2] - hi.z, v[g][3] - hi.w);
-                        } else {
-                            dst_hi[di] = make_float4(v[g][0], v[g][1], v[g][2], v[g][3]);
-                        }
-                    }
+                for (int q = 0; q < 4; ++q) {
+                    const int k = ch * KC + 4 * (kg_begin + g) + q;
+                    v[g][q] = (live && kg_begin + g < kg_end && k < K) ? __ldg(xcol + (int64_t)k * P.x_rs) : 0.f;
                 }
-                fence_async_smem();
-                __syncwarp();
-                if (lane == 0) mbar_arrive1(&full[s]);
-                if (++s == TC_STAGES) { s = 0; ph ^= 1u; }
+        };
+        int s = 0;
+        uint32_t ph = 0;
+        float cur[8][4], nxt[8][4];
+        int64_t t = rank;
+        int ch = 0;
+        if (t < ntiles) load_unit(t, ch, cur);
+        while (t < ntiles) {
+            int64_t tn = t;
+            int chn = ch + 1;
+            if (chn == NCH) { chn = 0; tn += nctas; }
+            if (tn < ntiles) load_unit(tn, chn, nxt);
+            mbar_wait(&empty[s], ph ^ 1u);
+            float4* dst_hi = As + (size_t)s * nsplit * a_f4;
+            float4* dst_lo = dst_hi + a_f4;
+#pragma unroll
+            for (int g = 0; g < 8; ++g) {
+                if (kg_begin + g >= kg_end) break;
+                const int di = (kg_begin + g) * TC_COLS + col;
+                if (a.split) {
+                    const float4 hi = make_float4(tf32_hi(cur[g][0]), tf32_hi(cur[g][1]), tf32_hi(cur[g][2]), tf32_hi(cur[g][3]));
+                    dst_hi[di] = hi;
+                    dst_lo[di] = make_float4(cur[g][0] - hi.x, cur[g][1] - hi.y, cur[g][2] - hi.z, cur[g][3] - hi.w);
+                } else {
+                    dst_hi[di] = make_float4(cur[g][0], cur[g][1], cur[g][2], cur[g][3]);
+                }
             }
+            fence_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive1(&full[s]);
+            if (++s == TC_STAGES) { s = 0; ph ^= 1u; }
+#pragma unroll
+            for (int g = 0; g < 8; ++g)
+#pragma unroll
+                for (int q = 0; q < 4; ++q) cur[g][q] = nxt[g][q];
+            t = tn;
+            ch = chn;
         }
     } else if (warp == TC_EPI_WARPS + TC_LD_WARPS) {
         // ======================================= MMA issuer =====================================
