@@ -19,8 +19,8 @@
 // D = A_hi B_lo + A_lo B_hi + A_hi B_hi accumulated in FP32 in TMEM; the dropped lo*lo term and the
 // truncation of lo are ~2^-21 relative per product.  TF32: the A_hi B_hi term alone (~2^-10).
 //
-// Roles (416 threads): warps 0-3 epilogue (TMEM lane quarter = warp index), warps 4-11 loaders,
-// warp 12 issues the MMAs (one elected thread).  Two shared-memory stages and two TMEM accumulators
+// Roles (544 threads): warps 0-7 epilogue (TMEM lane quarter = warp index % 4), warps 8-15 loaders,
+// warp 16 issues the MMAs (one elected thread).  Two shared-memory stages and two TMEM accumulators
 // are linked by mbarriers (tcgen05.commit arrives on them when the MMAs that read a stage finish).
 #include <algorithm>
 
@@ -29,7 +29,7 @@
 namespace cgtp {
 
 constexpr int TC_COLS = 128;     // columns per tile = UMMA M
-constexpr int TC_EPI_WARPS = 4;
+constexpr int TC_EPI_WARPS = 8;   // two warps per TMEM lane quarter, each takes alternate 32-channel slices
 constexpr int TC_LD_WARPS = 8;
 constexpr int TC_THREADS = 32 * (TC_EPI_WARPS + TC_LD_WARPS + 1);
 constexpr int TC_STAGES = 2;
@@ -281,24 +281,36 @@ __global__ void __launch_bounds__(TC_THREADS, 1) proj_tc_kernel(TcArgs a)
         // ======================================= epilogue =======================================
         int acc = 0;
         uint32_t aph = 0;
+        const int quarter = warp & 3, slice0 = warp >> 2;  // TMEM lanes 32*quarter..+31; channel slices slice0, slice0+2, ..
+        const int o_rs = P.o_rs, m_split = P.m_split;
         for (int64_t t = rank; t < ntiles; t += nctas) {
-            const int64_t cc = t * TC_COLS + 32 * warp + lane;
+            const int64_t cc = t * TC_COLS + 32 * quarter + lane;
             const bool live = cc < total_cols;
             const int64_t b = live ? cc / a.J : 0;
             const int j = live ? (int)(cc - b * a.J) : 0;
             float* o0 = P.out0 + b * P.o_bs0 + j;
-            float* o1 = P.out1 + b * P.o_bs1 + j - (int64_t)P.m_split * P.o_rs;
+            float* o1 = P.out1 + b * P.o_bs1 + j - (int64_t)m_split * o_rs;
             mbar_wait(&tfull[acc], aph);
             tc_fence_after();
-            const uint32_t taddr = tmem_base + ((uint32_t)(32 * warp) << 16) + (uint32_t)(acc * Npad);
-            for (int c0 = 0; c0 < M; c0 += 32) {
+            const uint32_t taddr = tmem_base + ((uint32_t)(32 * quarter) << 16) + (uint32_t)(acc * Npad);
+            for (int c0 = 32 * slice0; c0 < M; c0 += 32 * (TC_EPI_WARPS / 4)) {
                 uint32_t v[32];
                 tc_ld32(taddr + (uint32_t)c0, v);
                 if (live) {
+                    if (c0 + 32 <= m_split || c0 >= m_split) {  // the whole slice goes to one output tensor
+                        float* p = ((c0 < m_split) ? o0 : o1) + (int64_t)c0 * o_rs;
+                        const int nq = (M - c0 < 32) ? (M - c0) : 32;
 #pragma unroll
-                    for (int q = 0; q < 32; ++q) {
-                        const int m = c0 + q;
-                        if (m < M) ((m < P.m_split) ? o0 : o1)[(int64_t)m * P.o_rs] = __uint_as_float(v[q]);
+                        for (int q = 0; q < 32; ++q) {
+                            if (q < nq) *p = __uint_as_float(v[q]);
+                            p += o_rs;
+                        }
+                    } else {
+#pragma unroll
+                        for (int q = 0; q < 32; ++q) {
+                            const int m = c0 + q;
+                            if (m < M) ((m < m_split) ? o0 : o1)[(int64_t)m * o_rs] = __uint_as_float(v[q]);
+                        }
                     }
                 }
             }
