@@ -371,6 +371,7 @@ __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const floa
 #pragma unroll
     for (int k = 0; k < NTS; ++k) ts[k] = make_float2(0.f, 0.f);
 
+#pragma unroll 2
     for (int vp = 0; vp < Vh; ++vp) {
         const float4* q4 = reinterpret_cast<const float4*>(qf + (size_t)vp * QFS);
         float2 Cs[NP][2], Ss[NP][2];  // two chains each for ILP
@@ -633,7 +634,10 @@ static int launch_fast_t(const Plan* p, const CorePlan* c, const float* Ha, cons
     a.off_ts = a.off_f + (ODD ? 4 : 2) * (2 * LB + 1) * p->U * 32 * 4;
     auto kern = onsite_fast_kernel<LB, ODD>;
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const int ctas_per_sm = (int)(kSmemPerSm / (smem + 1024));
+    // persistent CTAs: exactly as many as are resident at once (shared memory and registers both count)
+    int ctas_per_sm = 0;
+    CGTP_CUDA_CHECK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, 32 * c->tab.NW, smem));
+    if (ctas_per_sm < 1) ctas_per_sm = 1;
     int64_t grid = (int64_t)num_sms() * ctas_per_sm;
     if (grid > a.ngroups) grid = a.ngroups;
     LaunchScope scope(ODD ? K_ONSITE_ODD : K_ONSITE_EVEN, st);
