@@ -68,13 +68,21 @@ static void lpt_assign(const std::vector<std::pair<int, int>>& items /* (cost, i
 static void stage_items(const Plan* p, bool odd, std::vector<std::pair<int, int>> (&items)[3])
 {
     const int LB = p->LB;
-    // stage A: one item per m <= LB (rows above lmax are zero-filled: cost 1); cost ~ number of l terms
-    for (int m = 0; m <= LB; ++m) items[0].push_back({m <= p->lmax ? 2 * (p->lmax - m + 1) + 1 : 1, m});
+    // stage A: cost ~ number of l terms (rows above lmax are zero-filled: cost 1).  even: one item per m <= LB
+    // (both factors at once, they share the table loads); odd: one item per (m, factor), id = 2 m + factor
+    for (int m = 0; m <= LB; ++m) {
+        const int cost = m <= p->lmax ? 2 * (p->lmax - m + 1) + 1 : 1;
+        if (!odd) {
+            items[0].push_back({cost, m});
+        } else {
+            items[0].push_back({cost, 2 * m});
+            items[0].push_back({cost, 2 * m + 1});
+        }
+    }
     // stage B: one item per grid row u, equal cost
     for (int u = 0; u < p->U; ++u) items[1].push_back({4, u});
     // stage C: one item per m <= lmax_out
     for (int m = 0; m <= p->lmax_out; ++m) items[2].push_back({(p->lmax_out - m + 1) + 1, m});
-    (void)odd;
 }
 
 static std::mutex g_core_mu;
@@ -534,14 +542,12 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
 
         // ---- stage A
         for (int k = 0; k < na; ++k) {
-            const int m = ia[k];
             if (!ODD) {
-                stage_a_even<LB>(ta, a.tab.UP4, ha, hb, F, F + plane, m, a.lmax, a.U, a.Uh, lane);
+                stage_a_even<LB>(ta, a.tab.UP4, ha, hb, F, F + plane, ia[k], a.lmax, a.U, a.Uh, lane);
             } else {
-#pragma unroll 1
-                for (int f = 0; f < 2; ++f)
-                    stage_a_odd<LB>(ta, a.tab.UP2, f ? hb : ha, F + (2 * f) * plane, F + (2 * f + 1) * plane, m, a.lmax,
-                                    a.U, a.Uh, lane);
+                const int m = ia[k] >> 1, f = ia[k] & 1;
+                stage_a_odd<LB>(ta, a.tab.UP2, f ? hb : ha, F + (2 * f) * plane, F + (2 * f + 1) * plane, m, a.lmax, a.U,
+                                a.Uh, lane);
             }
         }
         __syncthreads();
