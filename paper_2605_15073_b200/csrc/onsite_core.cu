@@ -28,11 +28,12 @@ constexpr int kMaxWarps = 8;
 struct CoreTab {
     int ta;     // stage A: even [tri(l,m)][UP4] float P~; odd [tri(l,m)][UP2] float2 (d_theta P~, m P~/sin theta)
     int wp;     // stage C: [tri(l,m)][UP4] float w P~, equator row halved
-    int qf;     // stage B forward: [Vh][QFS] float; entry r<=LB: cos row r, r>LB: sin row r-LB
-    int qi;     // stage B inverse: [Vh][QIS] float, (2 pi/V) q folded in; cos m at m, sin m at SOFF+m-1
+    int qf;     // stage B forward: [NQ][QFS] float; entry r<=LB: cos row r, r>LB: sin row r-LB
+    int qi;     // stage B inverse: [NQ][QIS] float, (2 pi/V4) q folded in; cos m at m, sin m at SOFF+m-1
     int sched;  // int: per stage s (A,B,C) and warp w: cnt[s][w] at s*kMaxWarps+w, then items[s][w][MAXI]
     int bytes;
     int UP2, UP4, QFS, QIS, SOFF, MAXI;
+    int NQ;     // rows of the azimuthal tables: V4/4 + 1, V4 = V rounded up to a multiple of 4
     int NW;
 };
 
@@ -140,14 +141,18 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
                 WP[(size_t)tri_index(l, m) * t.UP4 + u] = (float)(wu * pv);
             }
     }
-    std::vector<float> QF((size_t)Vh * t.QFS, 0.f), QI((size_t)Vh * t.QIS, 0.f);
-    for (int v = 0; v < Vh; ++v) {
-        const double ph = 2.0 * M_PI * v / V;
-        const bool paired = (v != 0) && !(V % 2 == 0 && v == V / 2);
-        const double wv = (2.0 * M_PI / V) * (paired ? 1.0 : 0.5);
+    // Azimuthal tables on the padded grid V4 = V rounded up to a multiple of 4 (exact as well, R8):
+    // row vq = 0..V4/4 serves the four azimuths phi, -phi, pi - phi, pi + phi (quarter-wave folding); rows 0 and
+    // V4/4 describe two distinct points each, visited twice -> half weight.
+    const int V4 = round_up(V, 4), NQ = V4 / 4 + 1;
+    (void)Vh;
+    std::vector<float> QF((size_t)NQ * t.QFS, 0.f), QI((size_t)NQ * t.QIS, 0.f);
+    for (int v = 0; v < NQ; ++v) {
+        const double ph = 2.0 * M_PI * v / V4;
+        const double wv = (2.0 * M_PI / V4) * ((v == 0 || v == NQ - 1) ? 0.5 : 1.0);
         for (int m = 0; m <= LB; ++m) {
             const double qc = (m == 0) ? 1.0 : std::sqrt(2.0) * std::cos(m * ph);
-            const double qs = (m == 0 || !paired) ? 0.0 : std::sqrt(2.0) * std::sin(m * ph);
+            const double qs = (m == 0) ? 0.0 : std::sqrt(2.0) * std::sin(m * ph);
             QF[(size_t)v * t.QFS + m] = (float)qc;
             QI[(size_t)v * t.QIS + m] = (float)(wv * qc);
             if (m > 0) {
@@ -156,6 +161,7 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
             }
         }
     }
+    t.NQ = NQ;
 
     // schedules: choose the warp count with the best work efficiency
     std::vector<std::pair<int, int>> items[3];
@@ -354,16 +360,19 @@ __device__ __forceinline__ void stage_a_odd(const float* __restrict__ ta, int UP
 
 // Stage B (rows S2b + S3 + S4a) for one (column, grid row u): forward real DFT of the coefficient
 // rows, product (even) or curl pairing (odd) at every azimuth, inverse real DFT -- all in registers.
-// The azimuth pair (v', V-v') shares one table row: C = cosine part, S = sine part of the m-sum,
-// field(v') = C + S, field(V-v') = C - S.  The result rows overwrite plane 0 in place.
+// Quarter-wave folding: with Ce/Co the cosine sums over even/odd m and Se/So the sine sums, one table row
+// gives the field at four azimuths,
+//   f(phi) = Ce+Co+Se+So,  f(-phi) = Ce+Co-Se-So,  f(pi+phi) = Ce-Co+Se-So,  f(pi-phi) = Ce-Co-Se+So,
+// and the inverse transform needs only  A+-B (cosine rows, even/odd m) and Cd+-D (sine rows) with
+// A = s1+s2, B = s3+s4, Cd = s1-s2, D = s4-s3.  The result rows overwrite plane 0 in place.
 template <int LB, bool ODD>
 __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const float* __restrict__ qi, int QFS, int QIS,
-                                        int SOFF, float* __restrict__ F, int plane_stride, int U, int u, int Vh,
+                                        int SOFF, float* __restrict__ F, int plane_stride, int U, int u, int NQ,
                                         int lane)
 {
     constexpr int MR = 2 * LB + 1;
-    constexpr int NTC = (LB + 2) / 2;  // pairs of cos rows m = 0..LB (+ pad)
-    constexpr int NTS = (LB + 1) / 2;  // pairs of sin rows m = 1..LB (+ pad)
+    constexpr int NTC = (LB + 2) / 2;  // pairs of cos rows (m = 2k, 2k+1)
+    constexpr int NTS = (LB + 1) / 2;  // pairs of sin rows (m = 2k+1, 2k+2)
     constexpr int NP = ODD ? 2 : 1;
     // f[k][r]: even: k = 0, pair (A, B); odd: k = 0 pair (A_theta, A_phi), k = 1 pair (B_theta, B_phi)
     float2 f[NP][MR];
@@ -380,14 +389,11 @@ __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const floa
     for (int k = 0; k < NTS; ++k) ts[k] = make_float2(0.f, 0.f);
 
 #pragma unroll 2
-    for (int vp = 0; vp < Vh; ++vp) {
-        const float4* q4 = reinterpret_cast<const float4*>(qf + (size_t)vp * QFS);
-        float2 Cs[NP][2], Ss[NP][2];  // two chains each for ILP
+    for (int vq = 0; vq < NQ; ++vq) {
+        const float4* q4 = reinterpret_cast<const float4*>(qf + (size_t)vq * QFS);
+        float2 Ce[NP], Co[NP], Se[NP], So[NP];
 #pragma unroll
-        for (int k = 0; k < NP; ++k) {
-            Cs[k][0] = Cs[k][1] = make_float2(0.f, 0.f);
-            Ss[k][0] = Ss[k][1] = make_float2(0.f, 0.f);
-        }
+        for (int k = 0; k < NP; ++k) Ce[k] = Co[k] = Se[k] = So[k] = make_float2(0.f, 0.f);
 #pragma unroll
         for (int r = 0; r < MR; r += 4) {
             const float4 t4 = q4[r / 4];
@@ -397,35 +403,52 @@ __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const floa
                 const int rr = r + h;
                 if (rr >= MR) break;
                 const float2 q2 = make_float2(qv[h], qv[h]);
+                const int m = (rr <= LB) ? rr : rr - LB;
 #pragma unroll
                 for (int k = 0; k < NP; ++k) {
-                    if (rr <= LB) Cs[k][rr & 1] = ffma2(f[k][rr], q2, Cs[k][rr & 1]);
-                    else Ss[k][rr & 1] = ffma2(f[k][rr], q2, Ss[k][rr & 1]);
+                    if (rr <= LB) {
+                        if (m & 1) Co[k] = ffma2(f[k][rr], q2, Co[k]);
+                        else Ce[k] = ffma2(f[k][rr], q2, Ce[k]);
+                    } else {
+                        if (m & 1) So[k] = ffma2(f[k][rr], q2, So[k]);
+                        else Se[k] = ffma2(f[k][rr], q2, Se[k]);
+                    }
                 }
             }
         }
-        float s1, s2;
-        if (!ODD) {
-            const float2 C = fadd2(Cs[0][0], Cs[0][1]), S = fadd2(Ss[0][0], Ss[0][1]);
-            const float2 g1 = fadd2(C, S), g2 = fsub2(C, S);
-            s1 = g1.x * g1.y;  // Eq.(38): A~ B~ at azimuth v'
-            s2 = g2.x * g2.y;  //          and at V - v'
-        } else {
-            const float2 Ca = fadd2(Cs[0][0], Cs[0][1]), Sa = fadd2(Ss[0][0], Ss[0][1]);
-            const float2 Cb = fadd2(Cs[1][0], Cs[1][1]), Sb = fadd2(Ss[1][0], Ss[1][1]);
-            const float2 a1 = fadd2(Ca, Sa), a2 = fsub2(Ca, Sa), b1 = fadd2(Cb, Sb), b2 = fsub2(Cb, Sb);
-            // Eq.(11): {A,B} = A_theta B_phi - A_phi B_theta  (A factor 1, B factor 2)
-            s1 = fmaf(a1.x, b1.y, -a1.y * b1.x);
-            s2 = fmaf(a2.x, b2.y, -a2.y * b2.x);
+        float2 g1[NP], g2[NP], g3[NP], g4[NP];
+#pragma unroll
+        for (int k = 0; k < NP; ++k) {
+            const float2 P = fadd2(Ce[k], Co[k]), Q = fsub2(Ce[k], Co[k]);
+            const float2 R = fadd2(Se[k], So[k]), T = fsub2(Se[k], So[k]);
+            g1[k] = fadd2(P, R);  // phi
+            g2[k] = fsub2(P, R);  // -phi
+            g4[k] = fadd2(Q, T);  // pi + phi
+            g3[k] = fsub2(Q, T);  // pi - phi
         }
-        const float sp = s1 + s2, sm = s1 - s2;
-        const float2 sp2 = make_float2(sp, sp), sm2 = make_float2(sm, sm);
-        const float2* qc2 = reinterpret_cast<const float2*>(qi + (size_t)vp * QIS);
-        const float2* qs2 = reinterpret_cast<const float2*>(qi + (size_t)vp * QIS + SOFF);
+        float s1, s2, s3, s4;
+        if (!ODD) {
+            // Eq.(38): A~ B~ at the four azimuths
+            s1 = g1[0].x * g1[0].y;
+            s2 = g2[0].x * g2[0].y;
+            s3 = g3[0].x * g3[0].y;
+            s4 = g4[0].x * g4[0].y;
+        } else {
+            // Eq.(11): {A,B} = A_theta B_phi - A_phi B_theta  (A factor 1, B factor 2)
+            s1 = fmaf(g1[0].x, g1[NP - 1].y, -g1[0].y * g1[NP - 1].x);
+            s2 = fmaf(g2[0].x, g2[NP - 1].y, -g2[0].y * g2[NP - 1].x);
+            s3 = fmaf(g3[0].x, g3[NP - 1].y, -g3[0].y * g3[NP - 1].x);
+            s4 = fmaf(g4[0].x, g4[NP - 1].y, -g4[0].y * g4[NP - 1].x);
+        }
+        const float A = s1 + s2, B = s3 + s4, Cd = s1 - s2, D = s4 - s3;
+        const float2 mc = make_float2(A + B, A - B);    // cosine rows: (even m, odd m)
+        const float2 ms = make_float2(Cd - D, Cd + D);  // sine rows:   (odd m, even m)
+        const float2* qc2 = reinterpret_cast<const float2*>(qi + (size_t)vq * QIS);
+        const float2* qs2 = reinterpret_cast<const float2*>(qi + (size_t)vq * QIS + SOFF);
 #pragma unroll
-        for (int k = 0; k < NTC; ++k) tc[k] = ffma2(qc2[k], sp2, tc[k]);
+        for (int k = 0; k < NTC; ++k) tc[k] = ffma2(qc2[k], mc, tc[k]);
 #pragma unroll
-        for (int k = 0; k < NTS; ++k) ts[k] = ffma2(qs2[k], sm2, ts[k]);
+        for (int k = 0; k < NTS; ++k) ts[k] = ffma2(qs2[k], ms, ts[k]);
     }
 #pragma unroll
     for (int m = 0; m <= LB; ++m) F[(m * U + u) * 32 + lane] = (m & 1) ? tc[m / 2].y : tc[m / 2].x;
@@ -629,7 +652,7 @@ static int launch_fast_t(const Plan* p, const CorePlan* c, const float* Ha, cons
     a.lmax_out = p->lmax_out;
     a.U = p->U;
     a.Uh = p->Uh;
-    a.Vh = p->Vh;
+    a.Vh = c->tab.NQ;  // rows of the quarter-wave azimuthal tables
     a.L2s = onsite_fast_hstride(p);
     a.Lo2s = onsite_fast_tstride(p);
     a.dbl = dbl ? 1 : 0;
