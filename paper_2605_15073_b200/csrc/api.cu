@@ -373,6 +373,21 @@ int cgtp_message_status(const void* workspace, void* cuda_stream)
 }
 
 // ------------------------------------------------------------------------------ host-buffer entry points
+// The host entry points allocate from the stream-ordered pool; without a release threshold the pool hands its
+// memory back to the driver at every synchronisation and the next call pays for a fresh allocation.
+static void keep_pool_memory()
+{
+    static bool done = false;
+    if (done) return;
+    int dev = 0;
+    cudaMemPool_t pool;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+        uint64_t keep = UINT64_MAX;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+    done = true;
+}
+
 int cgtp_onsite_host(const float* A, const float* B, const float* W_a, const float* W_b, const float* W_out, int lmax,
                      int lmax_out, int N, int C, const uint8_t* parity_mask, float* out, int64_t batch,
                      void* cuda_stream)
@@ -384,6 +399,7 @@ int cgtp_onsite_host(const float* A, const float* B, const float* W_a, const flo
     if (batch == 0) return CGTP_OK;
     if (!A || !B || !W_a || !W_b || !W_out || !out) { set_error("null pointer argument"); return CGTP_ERR_INVALID; }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    keep_pool_memory();
     const size_t L2 = (size_t)(lmax + 1) * (lmax + 1), Lo2 = (size_t)(lmax_out + 1) * (lmax_out + 1);
     const size_t wbytes = (size_t)C * N * 4;
     float *dWa = nullptr, *dWb = nullptr, *dWo = nullptr;
@@ -397,10 +413,13 @@ int cgtp_onsite_host(const float* A, const float* B, const float* W_a, const flo
     // Batch chunks on two streams so the H2D copy of chunk k+1, the kernels of chunk k and the D2H copy
     // of chunk k-1 overlap (PCIe is full duplex).
     const size_t in_per = (size_t)N * L2 * 4, out_per = (size_t)2 * N * Lo2 * 4;
-    int64_t chunk = (int64_t)((64u << 20) / (in_per > 0 ? in_per : 1));
-    if (chunk < 1) chunk = 1;
+    // <= 8 MB of each input per chunk, at least 8 chunks when the batch allows: PCIe is full duplex, so in steady
+    // state the H2D copy of chunk k+1, the kernels of chunk k and the D2H copy of chunk k-1 run together
+    int64_t chunk = (int64_t)((8u << 20) / (in_per > 0 ? in_per : 1));
+    if (chunk > (batch + 7) / 8) chunk = (batch + 7) / 8;
+    if (chunk < 64) chunk = 64;
     if (chunk > batch) chunk = batch;
-    const int NS = 2;
+    const int NS = 3;
     cudaStream_t cs[NS];
     cudaEvent_t ready, done[NS];
     CGTP_CUDA_CHECK(cudaEventCreateWithFlags(&ready, cudaEventDisableTiming));
@@ -461,6 +480,7 @@ int cgtp_message_host(const float* node_feats, const int64_t* edge_index, const 
         return CGTP_ERR_INVALID;
     }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    keep_pool_memory();
     const size_t L2 = (size_t)(lmax + 1) * (lmax + 1), Lo2 = (size_t)(lmax_out + 1) * (lmax_out + 1);
     const size_t xb = (size_t)nodes * N * L2 * 4, ob = (size_t)nodes * 2 * N * Lo2 * 4, wb = (size_t)C * N * 4;
     const size_t eib = (size_t)2 * (E > 0 ? E : 1) * 8, evb = (size_t)(E > 0 ? E : 1) * 3 * 4, erb = (size_t)(E > 0 ? E : 1) * C * 4;
