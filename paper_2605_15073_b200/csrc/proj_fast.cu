@@ -63,6 +63,11 @@ __device__ __forceinline__ float4 lds128(uint32_t addr)
     return v;
 }
 
+__device__ __forceinline__ void mbar_arrive_cta(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
 template <int RW, int CWP>
 __global__ void __launch_bounds__(kPfThreads, 2) proj_fast_kernel(PfArgs a)
 {
@@ -70,7 +75,8 @@ __global__ void __launch_bounds__(kPfThreads, 2) proj_fast_kernel(PfArgs a)
     constexpr int CWT = 128 * CWP;    // flattened columns per tile
     static_assert(RW * CWP == 8, "8 consumer warps");
     extern __shared__ __align__(128) unsigned char smem[];
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem);  // [NSTAGE <= 3]
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem);  // [NSTAGE <= 3]  TMA -> consumers
+    uint64_t* empty = full + 4;                          // [NSTAGE]       consumer warps -> producer (warp 0)
     float* Wd = reinterpret_cast<float*>(smem + 64);
     float* stages = Wd + a.w_floats;
 
@@ -93,7 +99,10 @@ __global__ void __launch_bounds__(kPfThreads, 2) proj_fast_kernel(PfArgs a)
     const uint32_t jmagic = a.jmagic;  // cc / J == umulhi(cc, jmagic) for cc < 2^16
 
     if (tid == 0) {
-        for (int s = 0; s < NSTAGE; ++s) mbar_init(&full[s], 1);
+        for (int s = 0; s < NSTAGE; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], kPfThreads / 32);
+        }
         mbar_fence_init();
     }
     __syncthreads();
@@ -165,11 +174,14 @@ __global__ void __launch_bounds__(kPfThreads, 2) proj_fast_kernel(PfArgs a)
     const uint32_t stage0 = smem_u32(stages), stage_bytes = (uint32_t)a.stage_floats * 4u, rs_bytes = (uint32_t)x_rs * 4u;
     const uint32_t w0 = smem_u32(Wd) + (uint32_t)wr * 64u;  // this warp's 16 rows
 
-    int ti = rank, kc = 0, s = 0;
-    uint32_t phase = 0;
+    int ti = rank, kc = 0, s = 0, prev_s = 0;
+    uint32_t phase = 0, prev_phase = 0;
     int b0 = 0, ncol = 0, cbase = 0;
     for (int c = 0; c < nchunks; ++c) {
-        __syncthreads();  // every warp is done with chunk c-1: its slot may be refilled
+        // The slot of chunk c-1 is refilled with chunk c+NSTAGE-1 once every warp has released it.  Only warp 0
+        // (the producer) waits for that; it is a consumer too, so the others have normally released the slot
+        // before warp 0 itself gets here, and no warp ever waits for a CTA-wide barrier in steady state.
+        if (warp == 0 && c > 0) mbar_wait(&empty[prev_s], prev_phase);
         produce();
 
         if (kc == 0) {
@@ -245,6 +257,10 @@ __global__ void __launch_bounds__(kPfThreads, 2) proj_fast_kernel(PfArgs a)
                 }
             }
         }
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cta(&empty[s]);
+        prev_s = s;
+        prev_phase = phase;
         if (++kc == NCH) { kc = 0; ti += cpr; }
         if (++s == NSTAGE) { s = 0; phase ^= 1u; }
     }
