@@ -4,6 +4,7 @@ ncu captures under profiles/ are made with.
     python -m paper_2605_15073_b200.profile_run --config 1 --steps 2            # on-site, configs[1]
     python -m paper_2605_15073_b200.profile_run --config 3 --lmax 20 --steps 1  # on-site sweep point
     python -m paper_2605_15073_b200.profile_run --config 4 --steps 1            # message passing, configs[4]
+    python -m paper_2605_15073_b200.profile_run --config 1 --math-mode 1        # 3xTF32 tensor-core projections
 """
 from __future__ import annotations
 
@@ -23,8 +24,10 @@ def main():
     ap.add_argument("--steps", type=int, default=2)
     ap.add_argument("--batch", type=int, default=None, help="override the batch / node count")
     ap.add_argument("--all-even", action="store_true")
+    ap.add_argument("--math-mode", type=int, default=0, help="0 FP32 (default), 1 3xTF32, 2 TF32 projections")
     args = ap.parse_args()
     dev = torch.device("cuda", 0)
+    cg.cgtp_set_math_mode(args.math_mode)
     cu = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     inp = synthetic.config(args.config, lmax=args.lmax)
     if args.all_even:
