@@ -45,6 +45,9 @@ struct CorePlan {
 };
 
 __host__ __device__ constexpr int core_uhmax(int LB) { return ((3 * LB + 2) / 2 + 1) / 2; }
+// Northern nodes per row block of the fast kernel: all of them (one block) for band limits <= 8; four for the
+// larger ones, two where four do not fit shared memory (odd channels at band limit 16).
+__host__ __device__ constexpr int core_ub(int LB, bool odd) { return LB <= 8 ? core_uhmax(LB) : (LB >= 16 && odd) ? 2 : 4; }
 
 // ------------------------------------------------------------------------------------------------
 // Host: packed tables + static schedules
@@ -80,8 +83,9 @@ static void stage_items(const Plan* p, bool odd, std::vector<std::pair<int, int>
             items[0].push_back({cost, 2 * m + 1});
         }
     }
-    // stage B: one item per grid row u, equal cost
-    for (int u = 0; u < p->U; ++u) items[1].push_back({4, u});
+    // stage B: one item per grid row of a row block, equal cost (the kernel deals them round-robin)
+    const int rows = LB <= 8 ? p->U : 2 * core_ub(LB, odd);
+    for (int u = 0; u < rows; ++u) items[1].push_back({4, u});
     // stage C: one item per m <= lmax_out
     for (int m = 0; m <= p->lmax_out; ++m) items[2].push_back({(p->lmax_out - m + 1) + 1, m});
 }
@@ -93,7 +97,7 @@ static size_t core_smem_bytes(const Plan* p, bool odd, const CoreTab& t, bool db
 {
     const int MR = 2 * p->LB + 1;
     const size_t hs = (size_t)2 * 32 * onsite_fast_hstride(p) * 4;
-    const size_t f = (size_t)(odd ? 4 : 2) * MR * p->U * 32 * 4;
+    const size_t f = (size_t)(odd ? 4 : 2) * MR * (2 * core_ub(p->LB, odd)) * 32 * 4;
     const size_t ts = (size_t)32 * onsite_fast_tstride(p) * 4;
     return 64 + t.bytes + (dbl ? 2 : 1) * hs + f + ts;
 }
@@ -253,37 +257,42 @@ struct CoreArgs {
     int hs_bytes;                    // bytes of one H buffer (both factors)
 };
 
+// Grid rows are processed in blocks of UB northern nodes u' = e0 .. e0+UB-1 together with their mirror images
+// U-1-u' (the pair shares one Legendre table row).  F holds one block: local row e (north) and UB+e (south),
+// RB = 2 UB rows per coefficient row.  Band limits <= 8 use a single block (UB = all northern nodes); larger band
+// limits use small blocks so that F fits shared memory, and stage C accumulates over the blocks.
+//
 // Stage A (row S2a), even channels.  Thread = (column, |m|): rows m (cos) and LB+m (sin) of both factors
-// for all grid rows; pairs are (+m, -m), the table is stored duplicated.
-template <int LB>
+// for the block's grid rows; pairs are (+m, -m), the table value is the broadcast scalar.
+template <int LB, int UB>
 __device__ __forceinline__ void stage_a_even(const float* __restrict__ ta, int UP4, const float* __restrict__ ha,
                                              const float* __restrict__ hb, float* __restrict__ Fa,
-                                             float* __restrict__ Fb, int m, int lmax, int U, int Uh, int lane)
+                                             float* __restrict__ Fb, int m, int lmax, int e0, int ne, int lane)
 {
-    constexpr int UH = core_uhmax(LB);
-    float2 acc[2][2][UH];
+    constexpr int RB = 2 * UB;
+    float2 acc[2][2][UB];
 #pragma unroll
     for (int f = 0; f < 2; ++f)
 #pragma unroll
         for (int par = 0; par < 2; ++par)
 #pragma unroll
-            for (int e = 0; e < UH; ++e) acc[f][par][e] = make_float2(0.f, 0.f);
+            for (int e = 0; e < UB; ++e) acc[f][par][e] = make_float2(0.f, 0.f);
     for (int l = m; l <= lmax; l += 2) {
 #pragma unroll
         for (int par = 0; par < 2; ++par) {
             const int ll = l + par;
             if (ll > lmax) break;
-            const float4* tab = reinterpret_cast<const float4*>(ta + (size_t)tri_index(ll, m) * UP4);
+            const float4* tab = reinterpret_cast<const float4*>(ta + (size_t)tri_index(ll, m) * UP4 + e0);
             const int ip = ll * ll + ll + m, im = ll * ll + ll - m;
             const float2 xa = make_float2(ha[ip], ha[im]);
             const float2 xb = make_float2(hb[ip], hb[im]);
 #pragma unroll
-            for (int e = 0; e < UH; e += 4) {
+            for (int e = 0; e < UB; e += 4) {
                 const float4 t4 = tab[e / 4];
                 const float tv[4] = {t4.x, t4.y, t4.z, t4.w};
 #pragma unroll
                 for (int h = 0; h < 4; ++h)
-                    if (e + h < UH) {
+                    if (e + h < UB) {
                         acc[0][par][e + h] = ffma2(xa, make_float2(tv[h], tv[h]), acc[0][par][e + h]);
                         acc[1][par][e + h] = ffma2(xb, make_float2(tv[h], tv[h]), acc[1][par][e + h]);
                     }
@@ -292,10 +301,10 @@ __device__ __forceinline__ void stage_a_even(const float* __restrict__ ta, int U
     }
     // P~(-x) = (-1)^(l+m) P~(x): north = even + odd part, south = even - odd part
 #pragma unroll
-    for (int e = 0; e < UH; ++e) {
-        if (e < Uh) {
-            const int rn = (m * U + e) * 32 + lane, rs = (m * U + (U - 1 - e)) * 32 + lane;
-            const int off = LB * U * 32;
+    for (int e = 0; e < UB; ++e) {
+        if (e < ne) {
+            const int rn = (m * RB + e) * 32 + lane, rs = (m * RB + UB + e) * 32 + lane;
+            const int off = LB * RB * 32;
             const float2 na = fadd2(acc[0][0][e], acc[0][1][e]), sa = fsub2(acc[0][0][e], acc[0][1][e]);
             const float2 nb = fadd2(acc[1][0][e], acc[1][1][e]), sb = fsub2(acc[1][0][e], acc[1][1][e]);
             Fa[rn] = na.x; Fa[rs] = sa.x; Fb[rn] = nb.x; Fb[rs] = sb.x;
@@ -308,34 +317,34 @@ __device__ __forceinline__ void stage_a_even(const float* __restrict__ ta, int U
 // (theta, phi) components of the surface gradient.  The phi derivative swaps the cos and sin rows
 // (PAPER.md:679): cos row m takes +m * (sine coefficient), sin row takes -m * (cosine coefficient).
 // F planes: 2*f + 0 = d_theta, 2*f + 1 = (1/sin theta) d_phi of factor f.
-template <int LB>
+template <int LB, int UB>
 __device__ __forceinline__ void stage_a_odd(const float* __restrict__ ta, int UP2, const float* __restrict__ h,
-                                            float* __restrict__ Fth, float* __restrict__ Fph, int m, int lmax, int U,
-                                            int Uh, int lane)
+                                            float* __restrict__ Fth, float* __restrict__ Fph, int m, int lmax, int e0,
+                                            int ne, int lane)
 {
-    constexpr int UH = core_uhmax(LB);
-    float2 acc[2][2][UH];  // [row type: cos, sin][parity of l-m][u']
+    constexpr int RB = 2 * UB;
+    float2 acc[2][2][UB];  // [row type: cos, sin][parity of l-m][u']
 #pragma unroll
     for (int r = 0; r < 2; ++r)
 #pragma unroll
         for (int par = 0; par < 2; ++par)
 #pragma unroll
-            for (int e = 0; e < UH; ++e) acc[r][par][e] = make_float2(0.f, 0.f);
+            for (int e = 0; e < UB; ++e) acc[r][par][e] = make_float2(0.f, 0.f);
     for (int l = m; l <= lmax; l += 2) {
 #pragma unroll
         for (int par = 0; par < 2; ++par) {
             const int ll = l + par;
             if (ll > lmax) break;
-            const float4* tab = reinterpret_cast<const float4*>(ta + (size_t)tri_index(ll, m) * UP2 * 2);
+            const float4* tab = reinterpret_cast<const float4*>(ta + ((size_t)tri_index(ll, m) * UP2 + e0) * 2);
             const float hp = h[ll * ll + ll + m], hm = h[ll * ll + ll - m];
             const float2 xc = make_float2(hp, hm);   // cos row: d_theta from H[l,+m], d_phi from H[l,-m]
             const float2 xs = make_float2(hm, -hp);  // sin row: d_theta from H[l,-m], d_phi from -H[l,+m]
 #pragma unroll
-            for (int e = 0; e < UH; e += 2) {
+            for (int e = 0; e < UB; e += 2) {
                 const float4 t4 = tab[e / 2];
                 acc[0][par][e] = ffma2(make_float2(t4.x, t4.y), xc, acc[0][par][e]);
                 acc[1][par][e] = ffma2(make_float2(t4.x, t4.y), xs, acc[1][par][e]);
-                if (e + 1 < UH) {
+                if (e + 1 < UB) {
                     acc[0][par][e + 1] = ffma2(make_float2(t4.z, t4.w), xc, acc[0][par][e + 1]);
                     acc[1][par][e + 1] = ffma2(make_float2(t4.z, t4.w), xs, acc[1][par][e + 1]);
                 }
@@ -344,10 +353,10 @@ __device__ __forceinline__ void stage_a_odd(const float* __restrict__ ta, int UP
     }
     // d/dtheta flips the reflection parity; (1/sin) d_phi keeps it
 #pragma unroll
-    for (int e = 0; e < UH; ++e) {
-        if (e < Uh) {
-            const int rn = (m * U + e) * 32 + lane, rs = (m * U + (U - 1 - e)) * 32 + lane;
-            const int off = LB * U * 32;
+    for (int e = 0; e < UB; ++e) {
+        if (e < ne) {
+            const int rn = (m * RB + e) * 32 + lane, rs = (m * RB + UB + e) * 32 + lane;
+            const int off = LB * RB * 32;
             const float2 n0 = fadd2(acc[0][0][e], acc[0][1][e]), d0 = fsub2(acc[0][0][e], acc[0][1][e]);
             Fth[rn] = n0.x; Fth[rs] = -d0.x; Fph[rn] = n0.y; Fph[rs] = d0.y;
             if (m > 0) {
@@ -365,10 +374,9 @@ __device__ __forceinline__ void stage_a_odd(const float* __restrict__ ta, int UP
 //   f(phi) = Ce+Co+Se+So,  f(-phi) = Ce+Co-Se-So,  f(pi+phi) = Ce-Co+Se-So,  f(pi-phi) = Ce-Co-Se+So,
 // and the inverse transform needs only  A+-B (cosine rows, even/odd m) and Cd+-D (sine rows) with
 // A = s1+s2, B = s3+s4, Cd = s1-s2, D = s4-s3.  The result rows overwrite plane 0 in place.
-template <int LB, bool ODD>
+template <int LB, bool ODD, int RB>
 __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const float* __restrict__ qi, int QFS, int QIS,
-                                        int SOFF, float* __restrict__ F, int plane_stride, int U, int u, int NQ,
-                                        int lane)
+                                        int SOFF, float* __restrict__ F, int plane_stride, int lr, int NQ, int lane)
 {
     constexpr int MR = 2 * LB + 1;
     constexpr int NTC = (LB + 2) / 2;  // pairs of cos rows (m = 2k, 2k+1)
@@ -378,7 +386,7 @@ __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const floa
     float2 f[NP][MR];
 #pragma unroll
     for (int r = 0; r < MR; ++r) {
-        const int idx = (r * U + u) * 32 + lane;
+        const int idx = (r * RB + lr) * 32 + lane;
         f[0][r] = make_float2(F[idx], F[idx + plane_stride]);
         if (ODD) f[NP - 1][r] = make_float2(F[idx + 2 * plane_stride], F[idx + 3 * plane_stride]);
     }
@@ -451,25 +459,29 @@ __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const floa
         for (int k = 0; k < NTS; ++k) ts[k] = ffma2(qs2[k], ms, ts[k]);
     }
 #pragma unroll
-    for (int m = 0; m <= LB; ++m) F[(m * U + u) * 32 + lane] = (m & 1) ? tc[m / 2].y : tc[m / 2].x;
+    for (int m = 0; m <= LB; ++m) F[(m * RB + lr) * 32 + lane] = (m & 1) ? tc[m / 2].y : tc[m / 2].x;
 #pragma unroll
-    for (int m = 1; m <= LB; ++m) F[((LB + m) * U + u) * 32 + lane] = ((m - 1) & 1) ? ts[(m - 1) / 2].y : ts[(m - 1) / 2].x;
+    for (int m = 1; m <= LB; ++m) F[((LB + m) * RB + lr) * 32 + lane] = ((m - 1) & 1) ? ts[(m - 1) / 2].y : ts[(m - 1) / 2].x;
 }
 
-// Stage C (row S4b, Eq.(40)): Gauss-Legendre quadrature over the grid rows for one
-// (column, |m|); pairs are (+m, -m).  Ts: [32][Lo2s] staging for the bulk store.
-template <int LB>
+// Stage C (row S4b, Eq.(40)): Gauss-Legendre quadrature over the block's grid rows for one
+// (column, |m|); pairs are (+m, -m).  Ts: [32][Lo2s] staging for the bulk store; `first` = first block of the
+// group (store), later blocks accumulate.  eq = index e of the equator row in this block (its mirror image is the
+// row itself and stage B ran on the northern copy only), or -1.
+template <int LB, int UB>
 __device__ __forceinline__ void stage_c(const float* __restrict__ wp, int UP4, const float* __restrict__ F,
-                                        float* __restrict__ ts_col, int m, int lmax_out, int U, int Uh, int lane)
+                                        float* __restrict__ ts_col, int m, int lmax_out, int e0, int ne, int eq,
+                                        bool first, int lane)
 {
-    constexpr int UH = core_uhmax(LB);
-    float2 tp[UH], tm[UH];
+    constexpr int RB = 2 * UB;
+    float2 tp[UB], tm[UB];
 #pragma unroll
-    for (int e = 0; e < UH; ++e) {
+    for (int e = 0; e < UB; ++e) {
         float2 n = make_float2(0.f, 0.f), s = make_float2(0.f, 0.f);
-        if (e < Uh) {
-            const int rn = (m * U + e) * 32 + lane, rs = (m * U + (U - 1 - e)) * 32 + lane;
-            const int off = LB * U * 32;
+        if (e < ne) {
+            const int rn = (m * RB + e) * 32 + lane;
+            const int rs = (e == eq) ? rn : (m * RB + UB + e) * 32 + lane;
+            const int off = LB * RB * 32;
             n.x = F[rn];
             s.x = F[rs];
             if (m > 0) { n.y = F[rn + off]; s.y = F[rs + off]; }
@@ -482,23 +494,30 @@ __device__ __forceinline__ void stage_c(const float* __restrict__ wp, int UP4, c
         for (int par = 0; par < 2; ++par) {
             const int ll = l + par;
             if (ll > lmax_out) break;
-            const float4* tab = reinterpret_cast<const float4*>(wp + (size_t)tri_index(ll, m) * UP4);
+            const float4* tab = reinterpret_cast<const float4*>(wp + (size_t)tri_index(ll, m) * UP4 + e0);
             float2 a0 = make_float2(0.f, 0.f), a1 = make_float2(0.f, 0.f);
+            if constexpr (UB == 2) {  // blocks of two rows start at even e0: 64-bit table loads
+                const float2 t2 = *reinterpret_cast<const float2*>(tab);
+                a0 = ffma2(par ? tm[0] : tp[0], make_float2(t2.x, t2.x), a0);
+                a1 = ffma2(par ? tm[1] : tp[1], make_float2(t2.y, t2.y), a1);
+            } else {
 #pragma unroll
-            for (int e = 0; e < UH; e += 4) {
-                const float4 t4 = tab[e / 4];
-                const float tv[4] = {t4.x, t4.y, t4.z, t4.w};
+                for (int e = 0; e < UB; e += 4) {
+                    const float4 t4 = tab[e / 4];
+                    const float tv[4] = {t4.x, t4.y, t4.z, t4.w};
 #pragma unroll
-                for (int h = 0; h < 4; ++h)
-                    if (e + h < UH) {
-                        const float2 x = par ? tm[e + h] : tp[e + h];
-                        if (h & 1) a1 = ffma2(x, make_float2(tv[h], tv[h]), a1);
-                        else a0 = ffma2(x, make_float2(tv[h], tv[h]), a0);
-                    }
+                    for (int h = 0; h < 4; ++h)
+                        if (e + h < UB) {
+                            const float2 x = par ? tm[e + h] : tp[e + h];
+                            if (h & 1) a1 = ffma2(x, make_float2(tv[h], tv[h]), a1);
+                            else a0 = ffma2(x, make_float2(tv[h], tv[h]), a0);
+                        }
+                }
             }
             const float2 r = fadd2(a0, a1);
-            ts_col[ll * ll + ll + m] = r.x;
-            if (m > 0) ts_col[ll * ll + ll - m] = r.y;
+            const int ip = ll * ll + ll + m, im = ll * ll + ll - m;
+            ts_col[ip] = first ? r.x : ts_col[ip] + r.x;
+            if (m > 0) ts_col[im] = first ? r.y : ts_col[im] + r.y;
         }
     }
 }
@@ -508,6 +527,7 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int MR = 2 * LB + 1;
+    constexpr int UB = core_ub(LB, ODD), RB = 2 * UB;
     uint64_t* bar_tab = reinterpret_cast<uint64_t*>(smem);
     uint64_t* bar_h = reinterpret_cast<uint64_t*>(smem + 16);  // [2]
     const unsigned char* blob = smem + a.off_blob;
@@ -518,9 +538,9 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
     const int* sched = reinterpret_cast<const int*>(blob + a.tab.sched);
     float* F = reinterpret_cast<float*>(smem + a.off_f);
     float* Ts = reinterpret_cast<float*>(smem + a.off_ts);
-    const int plane = MR * a.U * 32;
+    constexpr int plane = MR * RB * 32;
 
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, NW = blockDim.x >> 5;
     const int hfl = 32 * a.L2s;  // floats of one factor's H block
     const uint32_t hbytes = (uint32_t)hfl * 4;
 
@@ -547,10 +567,11 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
     mbar_wait(bar_tab, 0);
 
     const int MAXI = a.tab.MAXI;
-    const int na = sched[0 * kMaxWarps + warp], nb = sched[1 * kMaxWarps + warp], nc = sched[2 * kMaxWarps + warp];
+    const int na = sched[0 * kMaxWarps + warp], nc = sched[2 * kMaxWarps + warp];
     const int* ia = sched + 3 * kMaxWarps + (0 * kMaxWarps + warp) * MAXI;
-    const int* ib = sched + 3 * kMaxWarps + (1 * kMaxWarps + warp) * MAXI;
     const int* ic = sched + 3 * kMaxWarps + (2 * kMaxWarps + warp) * MAXI;
+    const int nblk = (a.Uh + UB - 1) / UB;
+    const int e_equator = (a.U & 1) ? a.Uh - 1 : -1;  // odd U: the last northern node is the equator, its own mirror image
 
     int buf = 0;
     uint32_t phases = 0u;  // bit b = parity to wait for on bar_h[b]
@@ -563,30 +584,41 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
         const float* ha = hs + lane * a.L2s;
         const float* hb = hs + hfl + lane * a.L2s;
 
-        // ---- stage A
-        for (int k = 0; k < na; ++k) {
-            if (!ODD) {
-                stage_a_even<LB>(ta, a.tab.UP4, ha, hb, F, F + plane, ia[k], a.lmax, a.U, a.Uh, lane);
-            } else {
-                const int m = ia[k] >> 1, f = ia[k] & 1;
-                stage_a_odd<LB>(ta, a.tab.UP2, f ? hb : ha, F + (2 * f) * plane, F + (2 * f + 1) * plane, m, a.lmax, a.U,
-                                a.Uh, lane);
+        for (int blk = 0; blk < nblk; ++blk) {
+            const int e0 = blk * UB;
+            const int ne = (a.Uh - e0 < UB) ? (a.Uh - e0) : UB;
+            const int eq = (e_equator >= e0 && e_equator < e0 + UB) ? e_equator - e0 : -1;
+
+            // ---- stage A: Legendre synthesis of the block's rows
+            for (int k = 0; k < na; ++k) {
+                if (!ODD) {
+                    stage_a_even<LB, UB>(ta, a.tab.UP4, ha, hb, F, F + plane, ia[k], a.lmax, e0, ne, lane);
+                } else {
+                    const int m = ia[k] >> 1, f = ia[k] & 1;
+                    stage_a_odd<LB, UB>(ta, a.tab.UP2, f ? hb : ha, F + (2 * f) * plane, F + (2 * f + 1) * plane, m, a.lmax,
+                                        e0, ne, lane);
+                }
             }
+            __syncthreads();
+            if (!a.dbl && blk == nblk - 1 && threadIdx.x == 0 && gn < a.ngroups) load_h(gn, 0);
+
+            // ---- stage B: one local grid row per warp pass (north rows 0..ne-1, south rows UB..UB+ne-1; the
+            // equator's southern copy is skipped)
+            for (int lr = warp; lr < RB; lr += NW) {
+                const int e = (lr < UB) ? lr : lr - UB;
+                if (e >= ne || (lr >= UB && e == eq)) continue;
+                stage_b<LB, ODD, RB>(qf, qi, a.tab.QFS, a.tab.QIS, a.tab.SOFF, F, plane, lr, a.Vh, lane);
+            }
+            // the previous group's bulk store must have finished reading Ts before stage C rewrites it
+            if (blk == 0 && threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+            __syncthreads();
+
+            // ---- stage C: quadrature over the block's rows, accumulated over the blocks
+            for (int k = 0; k < nc; ++k)
+                stage_c<LB, UB>(wp, a.tab.UP4, F, Ts + lane * a.Lo2s, ic[k], a.lmax_out, e0, ne, eq, blk == 0, lane);
+            if (blk == nblk - 1) fence_async_smem();
+            __syncthreads();
         }
-        __syncthreads();
-        if (!a.dbl && threadIdx.x == 0 && gn < a.ngroups) load_h(gn, 0);
-
-        // ---- stage B
-        for (int k = 0; k < nb; ++k)
-            stage_b<LB, ODD>(qf, qi, a.tab.QFS, a.tab.QIS, a.tab.SOFF, F, plane, a.U, ib[k], a.Vh, lane);
-        // the previous group's bulk store must have finished reading Ts before stage C rewrites it
-        if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-        __syncthreads();
-
-        // ---- stage C
-        for (int k = 0; k < nc; ++k) stage_c<LB>(wp, a.tab.UP4, F, Ts + lane * a.Lo2s, ic[k], a.lmax_out, a.U, a.Uh, lane);
-        fence_async_smem();
-        __syncthreads();
         if (threadIdx.x == 0) {
             tma_store_1d(a.T + g * 32 * a.Lo2s, Ts, (uint32_t)(32 * a.Lo2s * 4));
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
@@ -616,7 +648,7 @@ constexpr size_t kSmemPerSm = 227 * 1024;
 // 0 if the fast kernel cannot run this plan; otherwise the dynamic shared memory per CTA, with *dbl set.
 static size_t core_config(const Plan* p, bool odd, const CorePlan* c, bool* dbl)
 {
-    if (p->LB > 8) return 0;  // instantiated for LB <= 8 only (register budget of stage B)
+    if (p->LB > 16) return 0;  // band limit 20: H and T of a 32-column group alone exceed shared memory
     const size_t two = core_smem_bytes(p, odd, c->tab, true), one = core_smem_bytes(p, odd, c->tab, false);
     // prefer double-buffered H when it does not cost a resident CTA
     const size_t ctas_two = kSmemPerSm / (two + 1024), ctas_one = kSmemPerSm / (one + 1024);
@@ -627,7 +659,7 @@ static size_t core_config(const Plan* p, bool odd, const CorePlan* c, bool* dbl)
 
 bool onsite_fast_supported(const Plan* p, bool odd)
 {
-    if (p->LB > 8) return false;
+    if (p->LB > 16) return false;
     const CorePlan* c = get_core_plan(p, odd);
     if (!c) return false;
     bool dbl;
@@ -660,7 +692,7 @@ static int launch_fast_t(const Plan* p, const CorePlan* c, const float* Ha, cons
     a.off_blob = 64;
     a.off_hs = a.off_blob + c->tab.bytes;
     a.off_f = a.off_hs + (dbl ? 2 : 1) * a.hs_bytes;
-    a.off_ts = a.off_f + (ODD ? 4 : 2) * (2 * LB + 1) * p->U * 32 * 4;
+    a.off_ts = a.off_f + (ODD ? 4 : 2) * (2 * LB + 1) * (2 * core_ub(LB, ODD)) * 32 * 4;
     auto kern = onsite_fast_kernel<LB, ODD>;
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     // persistent CTAs: exactly as many as are resident at once (shared memory and registers both count)
@@ -686,7 +718,8 @@ int launch_onsite_fast(const Plan* p, bool odd, const float* Ha, const float* Hb
     case B:                                                                       \
         return odd ? launch_fast_t<B, true>(p, c, Ha, Hb, T, ncols, st)           \
                    : launch_fast_t<B, false>(p, c, Ha, Hb, T, ncols, st);
-        CGTP_CASE(1) CGTP_CASE(2) CGTP_CASE(3) CGTP_CASE(4) CGTP_CASE(5) CGTP_CASE(6) CGTP_CASE(8)
+        CGTP_CASE(1) CGTP_CASE(2) CGTP_CASE(3) CGTP_CASE(4) CGTP_CASE(5) CGTP_CASE(6) CGTP_CASE(8) CGTP_CASE(10)
+        CGTP_CASE(12) CGTP_CASE(16)
 #undef CGTP_CASE
     }
     set_error("onsite fast core: no kernel for band limit %d", p->LB);
