@@ -23,6 +23,7 @@
 namespace cgtp {
 
 constexpr int kMaxWarps = 8;
+constexpr int kMaxWorkers = 16;  // schedule slots: warps, or half-warps when a group has 16 columns
 
 // Byte offsets (multiples of 16) into the packed table blob of one (plan, parity).
 struct CoreTab {
@@ -30,7 +31,7 @@ struct CoreTab {
     int wp;     // stage C: [tri(l,m)][UP4] float w P~, equator row halved
     int qf;     // stage B forward: [NQ][QFS] float; entry r<=LB: cos row r, r>LB: sin row r-LB
     int qi;     // stage B inverse: [NQ][QIS] float, (2 pi/V4) q folded in; cos m at m, sin m at SOFF+m-1
-    int sched;  // int: per stage s (A,B,C) and warp w: cnt[s][w] at s*kMaxWarps+w, then items[s][w][MAXI]
+    int sched;  // int: per stage s (A,B,C) and worker w: cnt[s][w] at s*kMaxWorkers+w, then items[s][w][MAXI]
     int bytes;
     int UP2, UP4, QFS, QIS, SOFF, MAXI;
     int NQ;     // rows of the azimuthal tables: V4/4 + 1, V4 = V rounded up to a multiple of 4
@@ -45,6 +46,9 @@ struct CorePlan {
 };
 
 __host__ __device__ constexpr int core_uhmax(int LB) { return ((3 * LB + 2) / 2 + 1) / 2; }
+// Columns per group: 32 (lane = column); 16 at band limit 20, where a warp works on two items at once (one per
+// half-warp) because H, T and F of 32 columns do not fit shared memory.
+__host__ __device__ constexpr int core_gw(int LB) { return LB >= 20 ? 16 : 32; }
 // Northern nodes per row block of the fast kernel: all of them (one block) for band limits <= 8; four for the
 // larger ones, two where four do not fit shared memory (odd channels at band limit 16).
 __host__ __device__ constexpr int core_ub(int LB, bool odd) { return LB <= 8 ? core_uhmax(LB) : (LB >= 16 && odd) ? 2 : 4; }
@@ -96,9 +100,10 @@ static std::vector<CorePlan*> g_core_plans;
 static size_t core_smem_bytes(const Plan* p, bool odd, const CoreTab& t, bool dbl)
 {
     const int MR = 2 * p->LB + 1;
-    const size_t hs = (size_t)2 * 32 * onsite_fast_hstride(p) * 4;
-    const size_t f = (size_t)(odd ? 4 : 2) * MR * (2 * core_ub(p->LB, odd)) * 32 * 4;
-    const size_t ts = (size_t)32 * onsite_fast_tstride(p) * 4;
+    const size_t gw = core_gw(p->LB);
+    const size_t hs = (size_t)2 * gw * onsite_fast_hstride(p) * 4;
+    const size_t f = (size_t)(odd ? 4 : 2) * MR * (2 * core_ub(p->LB, odd)) * gw * 4;
+    const size_t ts = gw * onsite_fast_tstride(p) * 4;
     return 64 + t.bytes + (dbl ? 2 : 1) * hs + f + ts;
 }
 
@@ -172,18 +177,19 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
     stage_items(p, odd, items);
     int bestNW = 4;
     double best = -1.0;
+    const int NH = 32 / core_gw(LB);  // workers (schedule slots) per warp
     for (int NW = 4; NW <= kMaxWarps; ++NW) {
         double total = 0.0, span = 0.0;
         for (int s = 0; s < 3; ++s) {
             std::vector<std::vector<int>> asg;
             int mk;
-            lpt_assign(items[s], NW, asg, &mk);
+            lpt_assign(items[s], NW * NH, asg, &mk);
             // stage B dominates the run time: weight it by its real share of the FMA work
             const double wgt = (s == 1) ? 6.0 : 1.0;
             int tot = 0;
             for (auto& x2 : items[s]) tot += x2.first;
             total += wgt * tot;
-            span += wgt * mk * NW;
+            span += wgt * mk * NW * NH;
         }
         const double eff = total / span;
         if (eff > best + 1e-9) { best = eff; bestNW = NW; }
@@ -193,16 +199,16 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
     int maxi = 1;
     for (int s = 0; s < 3; ++s) {
         int mk;
-        lpt_assign(items[s], t.NW, asg[s], &mk);
+        lpt_assign(items[s], t.NW * NH, asg[s], &mk);
         for (auto& a : asg[s]) maxi = std::max(maxi, (int)a.size());
     }
     t.MAXI = maxi;
-    std::vector<int> sched((size_t)3 * kMaxWarps + (size_t)3 * kMaxWarps * maxi, 0);
+    std::vector<int> sched((size_t)3 * kMaxWorkers + (size_t)3 * kMaxWorkers * maxi, 0);
     for (int s = 0; s < 3; ++s)
-        for (int wi = 0; wi < t.NW; ++wi) {
-            sched[s * kMaxWarps + wi] = (int)asg[s][wi].size();
+        for (int wi = 0; wi < t.NW * NH; ++wi) {
+            sched[s * kMaxWorkers + wi] = (int)asg[s][wi].size();
             for (size_t k = 0; k < asg[s][wi].size(); ++k)
-                sched[3 * kMaxWarps + ((size_t)s * kMaxWarps + wi) * maxi + k] = asg[s][wi][k];
+                sched[3 * kMaxWorkers + ((size_t)s * kMaxWorkers + wi) * maxi + k] = asg[s][wi][k];
         }
 
     // pack
@@ -264,7 +270,7 @@ struct CoreArgs {
 //
 // Stage A (row S2a), even channels.  Thread = (column, |m|): rows m (cos) and LB+m (sin) of both factors
 // for the block's grid rows; pairs are (+m, -m), the table value is the broadcast scalar.
-template <int LB, int UB>
+template <int LB, int UB, int GW>
 __device__ __forceinline__ void stage_a_even(const float* __restrict__ ta, int UP4, const float* __restrict__ ha,
                                              const float* __restrict__ hb, float* __restrict__ Fa,
                                              float* __restrict__ Fb, int m, int lmax, int e0, int ne, int lane)
@@ -303,8 +309,8 @@ __device__ __forceinline__ void stage_a_even(const float* __restrict__ ta, int U
 #pragma unroll
     for (int e = 0; e < UB; ++e) {
         if (e < ne) {
-            const int rn = (m * RB + e) * 32 + lane, rs = (m * RB + UB + e) * 32 + lane;
-            const int off = LB * RB * 32;
+            const int rn = (m * RB + e) * GW + lane, rs = (m * RB + UB + e) * GW + lane;
+            const int off = LB * RB * GW;
             const float2 na = fadd2(acc[0][0][e], acc[0][1][e]), sa = fsub2(acc[0][0][e], acc[0][1][e]);
             const float2 nb = fadd2(acc[1][0][e], acc[1][1][e]), sb = fsub2(acc[1][0][e], acc[1][1][e]);
             Fa[rn] = na.x; Fa[rs] = sa.x; Fb[rn] = nb.x; Fb[rs] = sb.x;
@@ -317,7 +323,7 @@ __device__ __forceinline__ void stage_a_even(const float* __restrict__ ta, int U
 // (theta, phi) components of the surface gradient.  The phi derivative swaps the cos and sin rows
 // (PAPER.md:679): cos row m takes +m * (sine coefficient), sin row takes -m * (cosine coefficient).
 // F planes: 2*f + 0 = d_theta, 2*f + 1 = (1/sin theta) d_phi of factor f.
-template <int LB, int UB>
+template <int LB, int UB, int GW>
 __device__ __forceinline__ void stage_a_odd(const float* __restrict__ ta, int UP2, const float* __restrict__ h,
                                             float* __restrict__ Fth, float* __restrict__ Fph, int m, int lmax, int e0,
                                             int ne, int lane)
@@ -355,8 +361,8 @@ __device__ __forceinline__ void stage_a_odd(const float* __restrict__ ta, int UP
 #pragma unroll
     for (int e = 0; e < UB; ++e) {
         if (e < ne) {
-            const int rn = (m * RB + e) * 32 + lane, rs = (m * RB + UB + e) * 32 + lane;
-            const int off = LB * RB * 32;
+            const int rn = (m * RB + e) * GW + lane, rs = (m * RB + UB + e) * GW + lane;
+            const int off = LB * RB * GW;
             const float2 n0 = fadd2(acc[0][0][e], acc[0][1][e]), d0 = fsub2(acc[0][0][e], acc[0][1][e]);
             Fth[rn] = n0.x; Fth[rs] = -d0.x; Fph[rn] = n0.y; Fph[rs] = d0.y;
             if (m > 0) {
@@ -374,7 +380,7 @@ __device__ __forceinline__ void stage_a_odd(const float* __restrict__ ta, int UP
 //   f(phi) = Ce+Co+Se+So,  f(-phi) = Ce+Co-Se-So,  f(pi+phi) = Ce-Co+Se-So,  f(pi-phi) = Ce-Co-Se+So,
 // and the inverse transform needs only  A+-B (cosine rows, even/odd m) and Cd+-D (sine rows) with
 // A = s1+s2, B = s3+s4, Cd = s1-s2, D = s4-s3.  The result rows overwrite plane 0 in place.
-template <int LB, bool ODD, int RB>
+template <int LB, bool ODD, int RB, int GW>
 __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const float* __restrict__ qi, int QFS, int QIS,
                                         int SOFF, float* __restrict__ F, int plane_stride, int lr, int NQ, int lane)
 {
@@ -386,7 +392,7 @@ __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const floa
     float2 f[NP][MR];
 #pragma unroll
     for (int r = 0; r < MR; ++r) {
-        const int idx = (r * RB + lr) * 32 + lane;
+        const int idx = (r * RB + lr) * GW + lane;
         f[0][r] = make_float2(F[idx], F[idx + plane_stride]);
         if (ODD) f[NP - 1][r] = make_float2(F[idx + 2 * plane_stride], F[idx + 3 * plane_stride]);
     }
@@ -459,16 +465,85 @@ __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const floa
         for (int k = 0; k < NTS; ++k) ts[k] = ffma2(qs2[k], ms, ts[k]);
     }
 #pragma unroll
-    for (int m = 0; m <= LB; ++m) F[(m * RB + lr) * 32 + lane] = (m & 1) ? tc[m / 2].y : tc[m / 2].x;
+    for (int m = 0; m <= LB; ++m) F[(m * RB + lr) * GW + lane] = (m & 1) ? tc[m / 2].y : tc[m / 2].x;
 #pragma unroll
-    for (int m = 1; m <= LB; ++m) F[((LB + m) * RB + lr) * 32 + lane] = ((m - 1) & 1) ? ts[(m - 1) / 2].y : ts[(m - 1) / 2].x;
+    for (int m = 1; m <= LB; ++m) F[((LB + m) * RB + lr) * GW + lane] = ((m - 1) & 1) ? ts[(m - 1) / 2].y : ts[(m - 1) / 2].x;
+}
+
+// Stage B for odd channels at band limits whose four coefficient vectors do not fit the register file: the curl
+// pairing {A,B} = A_theta B_phi - A_phi B_theta is evaluated as two product terms, each with its own forward
+// transform of one (factor-1 field, factor-2 field) pair, sharing the inverse-transform accumulators by linearity.
+// F planes: 0 = A_theta, 1 = A_phi, 2 = B_theta, 3 = B_phi.
+template <int LB, int RB, int GW>
+__device__ __forceinline__ void stage_b_two_term(const float* __restrict__ qf, const float* __restrict__ qi, int QFS,
+                                                 int QIS, int SOFF, float* __restrict__ F, int plane_stride, int lr,
+                                                 int NQ, int lane)
+{
+    constexpr int MR = 2 * LB + 1;
+    constexpr int NTC = (LB + 2) / 2, NTS = (LB + 1) / 2;
+    float2 tc[NTC], ts[NTS];
+#pragma unroll
+    for (int k = 0; k < NTC; ++k) tc[k] = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int k = 0; k < NTS; ++k) ts[k] = make_float2(0.f, 0.f);
+#pragma unroll 1
+    for (int term = 0; term < 2; ++term) {
+        const int pa = term ? 1 : 0, pb = term ? 2 : 3;
+        const float sgn = term ? -1.f : 1.f;
+        float2 f[MR];
+#pragma unroll
+        for (int r = 0; r < MR; ++r) {
+            const int idx = (r * RB + lr) * GW + lane;
+            f[r] = make_float2(F[idx + pa * plane_stride], F[idx + pb * plane_stride]);
+        }
+#pragma unroll 2
+        for (int vq = 0; vq < NQ; ++vq) {
+            const float4* q4 = reinterpret_cast<const float4*>(qf + (size_t)vq * QFS);
+            float2 Ce = make_float2(0.f, 0.f), Co = Ce, Se = Ce, So = Ce;
+#pragma unroll
+            for (int r = 0; r < MR; r += 4) {
+                const float4 t4 = q4[r / 4];
+                const float qv[4] = {t4.x, t4.y, t4.z, t4.w};
+#pragma unroll
+                for (int h = 0; h < 4; ++h) {
+                    const int rr = r + h;
+                    if (rr >= MR) break;
+                    const float2 q2 = make_float2(qv[h], qv[h]);
+                    const int m = (rr <= LB) ? rr : rr - LB;
+                    if (rr <= LB) {
+                        if (m & 1) Co = ffma2(f[rr], q2, Co);
+                        else Ce = ffma2(f[rr], q2, Ce);
+                    } else {
+                        if (m & 1) So = ffma2(f[rr], q2, So);
+                        else Se = ffma2(f[rr], q2, Se);
+                    }
+                }
+            }
+            const float2 P = fadd2(Ce, Co), Q = fsub2(Ce, Co), R = fadd2(Se, So), T = fsub2(Se, So);
+            const float2 g1 = fadd2(P, R), g2 = fsub2(P, R), g4 = fadd2(Q, T), g3 = fsub2(Q, T);
+            const float s1 = sgn * (g1.x * g1.y), s2 = sgn * (g2.x * g2.y), s3 = sgn * (g3.x * g3.y),
+                        s4 = sgn * (g4.x * g4.y);
+            const float A = s1 + s2, B = s3 + s4, Cd = s1 - s2, D = s4 - s3;
+            const float2 mc = make_float2(A + B, A - B), ms = make_float2(Cd - D, Cd + D);
+            const float2* qc2 = reinterpret_cast<const float2*>(qi + (size_t)vq * QIS);
+            const float2* qs2 = reinterpret_cast<const float2*>(qi + (size_t)vq * QIS + SOFF);
+#pragma unroll
+            for (int k = 0; k < NTC; ++k) tc[k] = ffma2(qc2[k], mc, tc[k]);
+#pragma unroll
+            for (int k = 0; k < NTS; ++k) ts[k] = ffma2(qs2[k], ms, ts[k]);
+        }
+    }
+#pragma unroll
+    for (int m = 0; m <= LB; ++m) F[(m * RB + lr) * GW + lane] = (m & 1) ? tc[m / 2].y : tc[m / 2].x;
+#pragma unroll
+    for (int m = 1; m <= LB; ++m) F[((LB + m) * RB + lr) * GW + lane] = ((m - 1) & 1) ? ts[(m - 1) / 2].y : ts[(m - 1) / 2].x;
 }
 
 // Stage C (row S4b, Eq.(40)): Gauss-Legendre quadrature over the block's grid rows for one
 // (column, |m|); pairs are (+m, -m).  Ts: [32][Lo2s] staging for the bulk store; `first` = first block of the
 // group (store), later blocks accumulate.  eq = index e of the equator row in this block (its mirror image is the
 // row itself and stage B ran on the northern copy only), or -1.
-template <int LB, int UB>
+template <int LB, int UB, int GW>
 __device__ __forceinline__ void stage_c(const float* __restrict__ wp, int UP4, const float* __restrict__ F,
                                         float* __restrict__ ts_col, int m, int lmax_out, int e0, int ne, int eq,
                                         bool first, int lane)
@@ -479,9 +554,9 @@ __device__ __forceinline__ void stage_c(const float* __restrict__ wp, int UP4, c
     for (int e = 0; e < UB; ++e) {
         float2 n = make_float2(0.f, 0.f), s = make_float2(0.f, 0.f);
         if (e < ne) {
-            const int rn = (m * RB + e) * 32 + lane;
-            const int rs = (e == eq) ? rn : (m * RB + UB + e) * 32 + lane;
-            const int off = LB * RB * 32;
+            const int rn = (m * RB + e) * GW + lane;
+            const int rs = (e == eq) ? rn : (m * RB + UB + e) * GW + lane;
+            const int off = LB * RB * GW;
             n.x = F[rn];
             s.x = F[rs];
             if (m > 0) { n.y = F[rn + off]; s.y = F[rs + off]; }
@@ -528,6 +603,8 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int MR = 2 * LB + 1;
     constexpr int UB = core_ub(LB, ODD), RB = 2 * UB;
+    constexpr int GW = core_gw(LB), NH = 32 / GW;  // columns per group; schedule slots (workers) per warp
+    constexpr bool TWO_TERM = ODD && LB >= 20;     // four coefficient vectors of 2 LB + 1 pairs exceed the registers
     uint64_t* bar_tab = reinterpret_cast<uint64_t*>(smem);
     uint64_t* bar_h = reinterpret_cast<uint64_t*>(smem + 16);  // [2]
     const unsigned char* blob = smem + a.off_blob;
@@ -538,10 +615,12 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
     const int* sched = reinterpret_cast<const int*>(blob + a.tab.sched);
     float* F = reinterpret_cast<float*>(smem + a.off_f);
     float* Ts = reinterpret_cast<float*>(smem + a.off_ts);
-    constexpr int plane = MR * RB * 32;
+    constexpr int plane = MR * RB * GW;
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, NW = blockDim.x >> 5;
-    const int hfl = 32 * a.L2s;  // floats of one factor's H block
+    const int col = lane & (GW - 1);                 // column of the group this lane works on
+    const int worker = warp * NH + lane / GW, nworkers = NW * NH;
+    const int hfl = GW * a.L2s;  // floats of one factor's H block
     const uint32_t hbytes = (uint32_t)hfl * 4;
 
     auto load_h = [&](long long g, int buf) {
@@ -567,9 +646,9 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
     mbar_wait(bar_tab, 0);
 
     const int MAXI = a.tab.MAXI;
-    const int na = sched[0 * kMaxWarps + warp], nc = sched[2 * kMaxWarps + warp];
-    const int* ia = sched + 3 * kMaxWarps + (0 * kMaxWarps + warp) * MAXI;
-    const int* ic = sched + 3 * kMaxWarps + (2 * kMaxWarps + warp) * MAXI;
+    const int na = sched[0 * kMaxWorkers + worker], nc = sched[2 * kMaxWorkers + worker];
+    const int* ia = sched + 3 * kMaxWorkers + (0 * kMaxWorkers + worker) * MAXI;
+    const int* ic = sched + 3 * kMaxWorkers + (2 * kMaxWorkers + worker) * MAXI;
     const int nblk = (a.Uh + UB - 1) / UB;
     const int e_equator = (a.U & 1) ? a.Uh - 1 : -1;  // odd U: the last northern node is the equator, its own mirror image
 
@@ -581,8 +660,8 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
         mbar_wait(&bar_h[buf], (phases >> buf) & 1u);
         phases ^= 1u << buf;
         const float* hs = reinterpret_cast<const float*>(smem + a.off_hs + (size_t)buf * a.hs_bytes);
-        const float* ha = hs + lane * a.L2s;
-        const float* hb = hs + hfl + lane * a.L2s;
+        const float* ha = hs + col * a.L2s;
+        const float* hb = hs + hfl + col * a.L2s;
 
         for (int blk = 0; blk < nblk; ++blk) {
             const int e0 = blk * UB;
@@ -592,22 +671,25 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
             // ---- stage A: Legendre synthesis of the block's rows
             for (int k = 0; k < na; ++k) {
                 if (!ODD) {
-                    stage_a_even<LB, UB>(ta, a.tab.UP4, ha, hb, F, F + plane, ia[k], a.lmax, e0, ne, lane);
+                    stage_a_even<LB, UB, GW>(ta, a.tab.UP4, ha, hb, F, F + plane, ia[k], a.lmax, e0, ne, col);
                 } else {
                     const int m = ia[k] >> 1, f = ia[k] & 1;
-                    stage_a_odd<LB, UB>(ta, a.tab.UP2, f ? hb : ha, F + (2 * f) * plane, F + (2 * f + 1) * plane, m, a.lmax,
-                                        e0, ne, lane);
+                    stage_a_odd<LB, UB, GW>(ta, a.tab.UP2, f ? hb : ha, F + (2 * f) * plane, F + (2 * f + 1) * plane, m,
+                                            a.lmax, e0, ne, col);
                 }
             }
             __syncthreads();
             if (!a.dbl && blk == nblk - 1 && threadIdx.x == 0 && gn < a.ngroups) load_h(gn, 0);
 
-            // ---- stage B: one local grid row per warp pass (north rows 0..ne-1, south rows UB..UB+ne-1; the
+            // ---- stage B: one local grid row per worker pass (north rows 0..ne-1, south rows UB..UB+ne-1; the
             // equator's southern copy is skipped)
-            for (int lr = warp; lr < RB; lr += NW) {
+            for (int lr = worker; lr < RB; lr += nworkers) {
                 const int e = (lr < UB) ? lr : lr - UB;
                 if (e >= ne || (lr >= UB && e == eq)) continue;
-                stage_b<LB, ODD, RB>(qf, qi, a.tab.QFS, a.tab.QIS, a.tab.SOFF, F, plane, lr, a.Vh, lane);
+                if constexpr (TWO_TERM)
+                    stage_b_two_term<LB, RB, GW>(qf, qi, a.tab.QFS, a.tab.QIS, a.tab.SOFF, F, plane, lr, a.Vh, col);
+                else
+                    stage_b<LB, ODD, RB, GW>(qf, qi, a.tab.QFS, a.tab.QIS, a.tab.SOFF, F, plane, lr, a.Vh, col);
             }
             // the previous group's bulk store must have finished reading Ts before stage C rewrites it
             if (blk == 0 && threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
@@ -615,12 +697,12 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
 
             // ---- stage C: quadrature over the block's rows, accumulated over the blocks
             for (int k = 0; k < nc; ++k)
-                stage_c<LB, UB>(wp, a.tab.UP4, F, Ts + lane * a.Lo2s, ic[k], a.lmax_out, e0, ne, eq, blk == 0, lane);
+                stage_c<LB, UB, GW>(wp, a.tab.UP4, F, Ts + col * a.Lo2s, ic[k], a.lmax_out, e0, ne, eq, blk == 0, col);
             if (blk == nblk - 1) fence_async_smem();
             __syncthreads();
         }
         if (threadIdx.x == 0) {
-            tma_store_1d(a.T + g * 32 * a.Lo2s, Ts, (uint32_t)(32 * a.Lo2s * 4));
+            tma_store_1d(a.T + g * GW * a.Lo2s, Ts, (uint32_t)(GW * a.Lo2s * 4));
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
         if (a.dbl) buf ^= 1;
@@ -648,7 +730,6 @@ constexpr size_t kSmemPerSm = 227 * 1024;
 // 0 if the fast kernel cannot run this plan; otherwise the dynamic shared memory per CTA, with *dbl set.
 static size_t core_config(const Plan* p, bool odd, const CorePlan* c, bool* dbl)
 {
-    if (p->LB > 16) return 0;  // band limit 20: H and T of a 32-column group alone exceed shared memory
     const size_t two = core_smem_bytes(p, odd, c->tab, true), one = core_smem_bytes(p, odd, c->tab, false);
     // prefer double-buffered H when it does not cost a resident CTA
     const size_t ctas_two = kSmemPerSm / (two + 1024), ctas_one = kSmemPerSm / (one + 1024);
@@ -659,7 +740,6 @@ static size_t core_config(const Plan* p, bool odd, const CorePlan* c, bool* dbl)
 
 bool onsite_fast_supported(const Plan* p, bool odd)
 {
-    if (p->LB > 16) return false;
     const CorePlan* c = get_core_plan(p, odd);
     if (!c) return false;
     bool dbl;
@@ -679,7 +759,8 @@ static int launch_fast_t(const Plan* p, const CorePlan* c, const float* Ha, cons
     a.Ha = Ha;
     a.Hb = Hb;
     a.T = T;
-    a.ngroups = (ncols + 31) / 32;
+    constexpr int GW = core_gw(LB);
+    a.ngroups = (ncols + GW - 1) / GW;  // the caller pads the column count to a multiple of 32
     a.lmax = p->lmax;
     a.lmax_out = p->lmax_out;
     a.U = p->U;
@@ -688,11 +769,11 @@ static int launch_fast_t(const Plan* p, const CorePlan* c, const float* Ha, cons
     a.L2s = onsite_fast_hstride(p);
     a.Lo2s = onsite_fast_tstride(p);
     a.dbl = dbl ? 1 : 0;
-    a.hs_bytes = 2 * 32 * a.L2s * 4;
+    a.hs_bytes = 2 * GW * a.L2s * 4;
     a.off_blob = 64;
     a.off_hs = a.off_blob + c->tab.bytes;
     a.off_f = a.off_hs + (dbl ? 2 : 1) * a.hs_bytes;
-    a.off_ts = a.off_f + (ODD ? 4 : 2) * (2 * LB + 1) * (2 * core_ub(LB, ODD)) * 32 * 4;
+    a.off_ts = a.off_f + (ODD ? 4 : 2) * (2 * LB + 1) * (2 * core_ub(LB, ODD)) * GW * 4;
     auto kern = onsite_fast_kernel<LB, ODD>;
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     // persistent CTAs: exactly as many as are resident at once (shared memory and registers both count)
@@ -719,7 +800,7 @@ int launch_onsite_fast(const Plan* p, bool odd, const float* Ha, const float* Hb
         return odd ? launch_fast_t<B, true>(p, c, Ha, Hb, T, ncols, st)           \
                    : launch_fast_t<B, false>(p, c, Ha, Hb, T, ncols, st);
         CGTP_CASE(1) CGTP_CASE(2) CGTP_CASE(3) CGTP_CASE(4) CGTP_CASE(5) CGTP_CASE(6) CGTP_CASE(8) CGTP_CASE(10)
-        CGTP_CASE(12) CGTP_CASE(16)
+        CGTP_CASE(12) CGTP_CASE(16) CGTP_CASE(20)
 #undef CGTP_CASE
     }
     set_error("onsite fast core: no kernel for band limit %d", p->LB);
