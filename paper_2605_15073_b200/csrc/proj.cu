@@ -112,9 +112,37 @@ __global__ void __launch_bounds__(32 * WY) proj_kernel(ProjArgPack pack)
     }
 }
 
-int launch_proj(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st)
+// A problem with an empty contraction (K == 0: a parity sector without rank channels) has an all-zero result.
+// When its output rows are one dense block per batch entry it is written by a 2-D memset, so that the remaining
+// problem keeps the fast kernels; returns false when the layout is not of that form.
+static bool zero_fill(const ProjArgs& g, cudaStream_t st, int* rc)
 {
-    if (nargs < 1 || nargs > 2) { set_error("launch_proj: nargs"); return CGTP_ERR_INVALID; }
+    *rc = CGTP_OK;
+    if (g.batch <= 0 || g.M <= 0 || g.J <= 0) return true;
+    if (g.o_rs != g.J || g.m_split < g.M) return false;
+    const cudaError_t e = cudaMemset2DAsync(g.out0, (size_t)g.o_bs0 * 4, 0, (size_t)g.M * g.J * 4, (size_t)g.batch, st);
+    if (e != cudaSuccess) {
+        set_error("cudaMemset2DAsync failed: %s", cudaGetErrorString(e));
+        *rc = CGTP_ERR_CUDA;
+    }
+    return true;
+}
+
+int launch_proj(const ProjArgs* args_in, int nargs_in, Kind kind, cudaStream_t st)
+{
+    if (nargs_in < 1 || nargs_in > 2) { set_error("launch_proj: nargs"); return CGTP_ERR_INVALID; }
+    ProjArgs kept[2];
+    int nargs = 0;
+    for (int i = 0; i < nargs_in; ++i) {
+        int rc = CGTP_OK;
+        if (args_in[i].K == 0 && zero_fill(args_in[i], st, &rc)) {
+            if (rc != CGTP_OK) return rc;
+            continue;
+        }
+        kept[nargs++] = args_in[i];
+    }
+    if (nargs == 0) return CGTP_OK;
+    const ProjArgs* args = kept;
     ProjArgPack pack;
     int64_t max_cols = 0;
     int max_m = 0;
