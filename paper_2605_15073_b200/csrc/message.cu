@@ -74,7 +74,7 @@ static SynthSmem synth_smem_layout(const Plan* p, bool odd, int NC)
 {
     SynthSmem s;
     const int M = 2 * p->LB + 1;
-    const int J = NC * p->U;
+    const int J = (NC * p->U) | 1;  // odd row stride: rows of different m fall into different banks
     const int nf = odd ? 2 : 1;
     s.tab_bytes = p->Uh * p->NTRI * 4;
     s.q_bytes = p->Vh * p->QSTR * 4;
@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(256) node_synth_kernel(Plan p, SynthSmem lay, 
 
     const long long col0 = (long long)blockIdx.x * NC;
     const int nc = (int)((ncols - col0 < NC) ? (ncols - col0) : NC);
-    const int J = NC * p.U;
+    const int J = (NC * p.U) | 1;  // odd row stride (matches the host layout)
     const int hbytes = nc * p.L2p * 4;
 
     if (threadIdx.x == 0) {
@@ -400,7 +400,7 @@ static AnaSmem ana_smem_layout(const Plan* p, int NC)
 {
     AnaSmem s;
     const int M = 2 * p->LB + 1;
-    const int J = NC * p->U;
+    const int J = (NC * p->U) | 1;  // odd row stride: rows of different m fall into different banks
     s.tab_bytes = p->Uh * p->NTRI * 4;
     s.q_bytes = p->Vh * p->QSTR * 4;
     s.wv_bytes = round_up(p->Vh, 4) * 4;
@@ -431,7 +431,7 @@ __global__ void __launch_bounds__(256) analysis_kernel(Plan p, AnaSmem lay, cons
 
     const long long col0 = (long long)blockIdx.x * NC;
     const int nc = (int)((ncols - col0 < NC) ? (ncols - col0) : NC);
-    const int J = NC * p.U;
+    const int J = (NC * p.U) | 1;  // odd row stride (matches the host layout)
     const int sbytes = nc * p.UVp * 4;
 
     if (threadIdx.x == 0) {

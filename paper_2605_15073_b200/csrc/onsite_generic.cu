@@ -21,7 +21,7 @@ static OnsiteSmem onsite_smem_layout(const Plan* p, bool odd, int NC)
 {
     OnsiteSmem s;
     const int M = 2 * p->LB + 1;
-    const int J = NC * p->U;
+    const int J = (NC * p->U) | 1;  // odd row stride: rows of different m fall into different banks
     const int nterm = odd ? 2 : 1;
     s.tab_bytes = p->Uh * p->NTRI * 4;
     s.q_bytes = p->Vh * p->QSTR * 4;
@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(256) onsite_core_kernel(Plan p, OnsiteSmem lay
 
     const long long col0 = (long long)blockIdx.x * NC;
     const int nc = (int)((ncols - col0 < NC) ? (ncols - col0) : NC);
-    const int J = NC * p.U;
+    const int J = (NC * p.U) | 1;  // odd row stride (matches the host layout)
     const int hbytes = nc * p.L2p * 4;
 
     if (threadIdx.x == 0) {
