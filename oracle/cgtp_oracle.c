@@ -32,7 +32,9 @@
  * Eq.(6) closed form, the printed kappa^-1 values (:600, :655) and worked example (A11)-(A13),
  * real-basis tables against brute-force quadrature, (1,1,1) block = sqrt(3/4pi)*epsilon,
  * real SH against scipy, whole-pipeline results against fine-grid quadrature, Wigner-D
- * equivariance, inversion parity, self-coupled vanishing, Parseval.  No function here is
+ * equivariance, inversion parity, self-coupled vanishing, Parseval; the parity-slot functions
+ * (oracle_*_parity) against the paper's dispatch check B7 (:647), the reduction to the natural-parity
+ * functions, Eq.(44)-(45)/(56) slot rules, inversion and rotation.  No function here is
  * "parity unpinned".
  *
  * Plain C99 + OpenMP, double precision (long double inside the Racah sum).
@@ -475,6 +477,194 @@ int oracle_message(const double *node_feats /* [nodes,N,L2] */, const int64_t *e
     }
     free(H); free(slot);
     free(row_ptr);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Parity-labelled inputs (Sec. VI A-E :193-:240, Sec. VII C a-c, e :383-:469).                   */
+/*                                                                                              */
+/* A feature I_{n l m, p} carries an absolute parity label p = +-1 next to l.  Storage (reading   */
+/* R19): slot 0 of the slot axis holds the natural-parity part p = (-1)^l, slot 1 the  */
+/* opposite-parity part p = -(-1)^l -- for every l the same two numbers as the paper's (+1, -1)   */
+/* slots, indexed relative to (-1)^l.  The output uses the same two slots (= the two sectors of   */
+/* the natural-parity entry points).                                                            */
+/*                                                                                              */
+/* What is evaluated is Eq.(2) / Eq.(1) with the output parity p = p1 p2 (:29, :240; B7's         */
+/* dispatch rule p = (-1)^{l1} p2, :647) applied TERM BY TERM: every non-zero (l1m1, l2m2 -> lm)  */
+/* of the Gaunt table (l1+l2+l even, Category alpha, Cases A and C) and of the Q table (l1+l2+l   */
+/* odd, Category beta, Cases B and D) is routed to the output slot that p = p1 p2 and l select.   */
+/* Following Eq.(42)-(43), (45), (56) every run has independent CP weights; with the l-shared     */
+/* weights of reading R5 a run is one (category, slots, output-l parity sigma) combination:       */
+/*   message passing: run r = 4*cat + 2*s_out + tau, tau = 0 for sigma = +1 (even l), 1 for odd   */
+/*     l; cat 0 = alpha, 1 = beta; s_out the output slot.  (p, sigma) of Eq.(44)-(45) is          */
+/*     (s_out, tau) with p = (-1)^{s_out} sigma.  8 runs.                                        */
+/*   on-site (VII C e): run r = 8*cat + 4*s1 + 2*s2 + tau over the slots of both factors: 16 runs */
+/*     ("two pairs x two output sectors x two output-l parities" x {alpha, beta}, :469).          */
+/* Nothing below hard-codes which source slot feeds which output slot: that is decided per term   */
+/* from the parities, so Eq.(44), (45), (56) are consequences the tests can check.                */
+/* ------------------------------------------------------------------------------------------ */
+static int isqrt_floor(int i)
+{
+    int l = (int)floor(sqrt((double)i));
+    while ((l + 1) * (l + 1) <= i) ++l;
+    while (l * l > i) --l;
+    return l;
+}
+static int sgn_pow(int k) { return (k & 1) ? -1 : 1; }
+
+/* node_feats [nodes,2,N,L2]; edge_radial [E,8,C]; l1_weight [lmax+1] or NULL (an l1-dependent     */
+/* factor on the edge side, used by the dispatch pin B7 :647 to restrict the edge to one degree);  */
+/* W_node [8,C,N]; W_out [8,N,C]; out [n_recv or nodes, 2, N, Lo2].                                */
+int oracle_message_parity(const double *node_feats, const int64_t *edge_index, const double *edge_vec,
+                          const double *edge_radial, const double *l1_weight, const double *W_node,
+                          const double *W_out, int lmax, int lmax_out, int N, int C, double *out,
+                          int64_t nodes, int64_t E, const int64_t *recv_list, int64_t n_recv)
+{
+    enum { R = 8 };
+    int L2 = (lmax + 1) * (lmax + 1), Lo2 = (lmax_out + 1) * (lmax_out + 1);
+    const coupling_t *tab[2];
+    tab[0] = get_coupling(lmax, lmax_out, 0);
+    tab[1] = get_coupling(lmax, lmax_out, 1);
+    if (!tab[0] || !tab[1]) return 2;
+    int64_t *row_ptr = malloc((size_t)(nodes + 1) * sizeof(int64_t));
+    int rc = oracle_segments(edge_index, E, nodes, row_ptr);
+    if (rc) { free(row_ptr); return rc; }
+    const int64_t *snd = edge_index;
+    int64_t nr = recv_list ? n_recv : nodes;
+    int64_t *slot = malloc((size_t)nodes * sizeof(int64_t));
+    for (int64_t j = 0; j < nodes; ++j) slot[j] = -1;
+    int64_t n_need = 0;
+    for (int64_t r = 0; r < nr; ++r) {
+        int64_t i = recv_list ? recv_list[r] : r;
+        for (int64_t e = row_ptr[i]; e < row_ptr[i + 1]; ++e)
+            if (slot[snd[e]] < 0) slot[snd[e]] = n_need++;
+    }
+    /* Eq.(47) for every run and both source slots: H[j][run][s_in][c][l2m2] */
+    size_t hsz = (size_t)R * 2 * C * L2;
+    double *H = malloc((size_t)(n_need > 0 ? n_need : 1) * hsz * sizeof(double));
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t j = 0; j < nodes; ++j) {
+        if (slot[j] < 0) continue;
+        for (int run = 0; run < R; ++run)
+            for (int s = 0; s < 2; ++s) {
+                const double *xj = node_feats + (j * 2 + s) * (int64_t)N * L2;
+                double *hj = H + slot[j] * hsz + ((size_t)run * 2 + s) * C * L2;
+                for (int c = 0; c < C; ++c)
+                    for (int q = 0; q < L2; ++q) {
+                        double acc = 0.0;
+                        for (int n = 0; n < N; ++n) acc += W_node[((size_t)run * C + c) * N + n] * xj[n * L2 + q];
+                        hj[c * L2 + q] = acc;
+                    }
+            }
+    }
+#pragma omp parallel
+    {
+        double *Y = malloc((size_t)L2 * sizeof(double));
+        double *T = malloc((size_t)R * C * Lo2 * sizeof(double));
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t r = 0; r < nr; ++r) {
+            int64_t i = recv_list ? recv_list[r] : r;
+            for (size_t k = 0; k < (size_t)R * C * Lo2; ++k) T[k] = 0.0;
+            for (int64_t e = row_ptr[i]; e < row_ptr[i + 1]; ++e) {
+                oracle_real_sh(lmax, edge_vec[3 * e], edge_vec[3 * e + 1], edge_vec[3 * e + 2], Y);
+                if (l1_weight)
+                    for (int q = 0; q < L2; ++q) Y[q] *= l1_weight[isqrt_floor(q)];
+                for (int run = 0; run < R; ++run) {
+                    int cat = run >> 2, s_out = (run >> 1) & 1, tau = run & 1;
+                    const coupling_t *t = tab[cat];
+                    for (int s_in = 0; s_in < 2; ++s_in) {
+                        const double *hj = H + slot[snd[e]] * hsz + ((size_t)run * 2 + s_in) * C * L2;
+                        for (int64_t k = 0; k < t->nnz; ++k) {
+                            int l1 = isqrt_floor(t->i1[k]), l2 = isqrt_floor(t->i2[k]), l = isqrt_floor(t->io[k]);
+                            int p1 = sgn_pow(l1);              /* edge feature R Y_{l1}: natural parity (:370)      */
+                            int p2 = sgn_pow(s_in) * sgn_pow(l2); /* parity label of the source slot               */
+                            int p = p1 * p2;                   /* output parity, Eq.(2) / B7 (:647)                 */
+                            int so = (p == sgn_pow(l)) ? 0 : 1;
+                            if (so != s_out || (l & 1) != tau) continue; /* not a term of this run (Eq.(54): (-1)^l = sigma) */
+                            for (int c = 0; c < C; ++c)
+                                T[((size_t)run * C + c) * Lo2 + t->io[k]] +=
+                                    t->val[k] * edge_radial[(e * R + run) * (int64_t)C + c] * Y[t->i1[k]] *
+                                    hj[(size_t)c * L2 + t->i2[k]];
+                        }
+                    }
+                }
+            }
+            /* Eq.(55), (58), (59): channel projection per run, alpha + beta summed into the output slot */
+            double *ob = out + r * 2 * (int64_t)N * Lo2;
+            for (size_t k = 0; k < (size_t)2 * N * Lo2; ++k) ob[k] = 0.0;
+            for (int run = 0; run < R; ++run) {
+                int s_out = (run >> 1) & 1;
+                for (int n = 0; n < N; ++n)
+                    for (int q = 0; q < Lo2; ++q) {
+                        double acc = 0.0;
+                        for (int c = 0; c < C; ++c)
+                            acc += W_out[((size_t)run * N + n) * C + c] * T[((size_t)run * C + c) * Lo2 + q];
+                        ob[((size_t)s_out * N + n) * Lo2 + q] += acc;
+                    }
+            }
+        }
+        free(Y); free(T);
+    }
+    free(H); free(slot); free(row_ptr);
+    return 0;
+}
+
+/* A, B [batch,2,N,L2]; W_a, W_b [16,C,N]; W_out [16,N,C]; out [batch,2,N,Lo2].                    */
+int oracle_onsite_parity(const double *A, const double *B, const double *W_a, const double *W_b,
+                         const double *W_out, int lmax, int lmax_out, int N, int C, double *out, int64_t batch)
+{
+    enum { R = 16 };
+    int L2 = (lmax + 1) * (lmax + 1), Lo2 = (lmax_out + 1) * (lmax_out + 1);
+    const coupling_t *tab[2];
+    tab[0] = get_coupling(lmax, lmax_out, 0);
+    tab[1] = get_coupling(lmax, lmax_out, 1);
+    if (!tab[0] || !tab[1]) return 2;
+#pragma omp parallel
+    {
+        double *Ha = malloc((size_t)C * L2 * sizeof(double));
+        double *Hb = malloc((size_t)C * L2 * sizeof(double));
+        double *T = malloc((size_t)2 * C * Lo2 * sizeof(double)); /* [output slot][c][lm] of one run */
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t b = 0; b < batch; ++b) {
+            double *ob = out + b * 2 * (int64_t)N * Lo2;
+            for (size_t k = 0; k < (size_t)2 * N * Lo2; ++k) ob[k] = 0.0;
+            for (int run = 0; run < R; ++run) {
+                int cat = run >> 3, s1 = (run >> 2) & 1, s2 = (run >> 1) & 1, tau = run & 1;
+                const double *Ab = A + (b * 2 + s1) * (int64_t)N * L2, *Bb = B + (b * 2 + s2) * (int64_t)N * L2;
+                for (int c = 0; c < C; ++c)
+                    for (int q = 0; q < L2; ++q) {
+                        double sa = 0.0, sb = 0.0;
+                        for (int n = 0; n < N; ++n) {
+                            sa += W_a[((size_t)run * C + c) * N + n] * Ab[n * L2 + q];
+                            sb += W_b[((size_t)run * C + c) * N + n] * Bb[n * L2 + q];
+                        }
+                        Ha[c * L2 + q] = sa;
+                        Hb[c * L2 + q] = sb;
+                    }
+                for (size_t k = 0; k < (size_t)2 * C * Lo2; ++k) T[k] = 0.0;
+                const coupling_t *t = tab[cat];
+                for (int64_t k = 0; k < t->nnz; ++k) {
+                    int l1 = isqrt_floor(t->i1[k]), l2 = isqrt_floor(t->i2[k]), l = isqrt_floor(t->io[k]);
+                    int p1 = sgn_pow(s1) * sgn_pow(l1), p2 = sgn_pow(s2) * sgn_pow(l2);
+                    int p = p1 * p2;                        /* Eq.(1): output parity p = p1 p2 (:29)        */
+                    int so = (p == sgn_pow(l)) ? 0 : 1;
+                    if ((l & 1) != tau) continue;           /* this run feeds (-1)^l = sigma only           */
+                    for (int c = 0; c < C; ++c)
+                        T[((size_t)so * C + c) * Lo2 + t->io[k]] +=
+                            t->val[k] * Ha[(size_t)c * L2 + t->i1[k]] * Hb[(size_t)c * L2 + t->i2[k]];
+                }
+                for (int so = 0; so < 2; ++so)
+                    for (int n = 0; n < N; ++n)
+                        for (int q = 0; q < Lo2; ++q) {
+                            double acc = 0.0;
+                            for (int c = 0; c < C; ++c)
+                                acc += W_out[((size_t)run * N + n) * C + c] * T[((size_t)so * C + c) * Lo2 + q];
+                            ob[((size_t)so * N + n) * Lo2 + q] += acc;
+                        }
+            }
+        }
+        free(Ha); free(Hb); free(T);
+    }
     return 0;
 }
 

@@ -60,6 +60,10 @@ def _load():
     lib.oracle_onsite.argtypes = [p, p, p, p, p, i, i, i, i, p, p, i64]
     lib.oracle_message.restype = i
     lib.oracle_message.argtypes = [p, p, p, p, p, p, i, i, i, i, p, p, i64, i64, p, i64]
+    lib.oracle_message_parity.restype = i
+    lib.oracle_message_parity.argtypes = [p, p, p, p, p, p, p, i, i, i, i, p, i64, i64, p, i64]
+    lib.oracle_onsite_parity.restype = i
+    lib.oracle_onsite_parity.argtypes = [p, p, p, p, p, i, i, i, i, p, i64]
     lib.oracle_num_threads.restype = i
     lib.oracle_num_threads.argtypes = []
     _lib = lib
@@ -175,6 +179,49 @@ def message(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, 
                                 N, C, _ptr(mask), _ptr(out), nodes, E, rlp, nr if rl is not None else 0)
     if rc:
         raise RuntimeError(f"oracle_message failed with code {rc}")
+    return out
+
+
+def onsite_parity(A, B, W_a, W_b, W_out, lmax, lmax_out) -> np.ndarray:
+    """Parity-labelled on-site contraction (Sec. VII C e).  A, B [batch,2,N,L2] (slot 0 natural, 1 opposite parity);
+    W_a, W_b [16,C,N], W_out [16,N,C], run = 8*cat + 4*s1 + 2*s2 + tau.  out[batch,2,N,(lmax_out+1)^2]."""
+    A, B, W_a, W_b, W_out = map(_f64, (A, B, W_a, W_b, W_out))
+    batch, two, N, L2 = A.shape
+    C = W_a.shape[1]
+    assert two == 2 and L2 == (lmax + 1) ** 2 and B.shape == A.shape
+    assert W_a.shape == (16, C, N) and W_b.shape == (16, C, N) and W_out.shape == (16, N, C)
+    out = np.zeros((batch, 2, N, (lmax_out + 1) ** 2), np.float64)
+    rc = _load().oracle_onsite_parity(_ptr(A), _ptr(B), _ptr(W_a), _ptr(W_b), _ptr(W_out), lmax, lmax_out, N, C,
+                                      _ptr(out), batch)
+    if rc:
+        raise RuntimeError(f"oracle_onsite_parity failed with code {rc}")
+    return out
+
+
+def message_parity(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, recv_list=None,
+                   l1_weight=None) -> np.ndarray:
+    """Parity-labelled message passing (Sec. VII C a-c).  node_feats [nodes,2,N,L2]; edge_radial [E,8,C];
+    W_node [8,C,N]; W_out [8,N,C]; run = 4*cat + 2*s_out + tau.  out[n_recv or nodes,2,N,(lmax_out+1)^2]."""
+    X, ev, er, W_node, W_out = map(_f64, (node_feats, edge_vec, edge_radial, W_node, W_out))
+    ei = np.ascontiguousarray(np.asarray(edge_index), dtype=np.int64)
+    nodes, two, N, L2 = X.shape
+    E = ei.shape[1]
+    C = W_node.shape[1]
+    assert two == 2 and L2 == (lmax + 1) ** 2 and ev.shape == (E, 3) and er.shape == (E, 8, C)
+    assert W_node.shape == (8, C, N) and W_out.shape == (8, N, C)
+    if recv_list is None:
+        rl, nr, rlp = None, nodes, None
+    else:
+        rl = np.ascontiguousarray(np.asarray(recv_list), dtype=np.int64)
+        nr, rlp = rl.shape[0], _ptr(rl)
+    lw = None if l1_weight is None else _f64(l1_weight)
+    assert lw is None or lw.shape == (lmax + 1,)
+    out = np.zeros((nr, 2, N, (lmax_out + 1) ** 2), np.float64)
+    rc = _load().oracle_message_parity(_ptr(X), _ptr(ei), _ptr(ev), _ptr(er), None if lw is None else _ptr(lw),
+                                       _ptr(W_node), _ptr(W_out), lmax, lmax_out, N, C, _ptr(out), nodes, E, rlp,
+                                       nr if rl is not None else 0)
+    if rc:
+        raise RuntimeError(f"oracle_message_parity failed with code {rc}")
     return out
 
 

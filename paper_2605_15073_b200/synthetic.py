@@ -108,6 +108,70 @@ def make_message(lmax: int, lmax_out: int, N: int, C: int, nodes: int, degree, r
                          W_node, W_out, mask, deg)
 
 
+# ---------------------------------------------------------------------------------------------
+# Parity-labelled inputs (Sec. VI, VII C a-c, e): a parity-slot axis on the
+# features (slot 0 natural parity (-1)^l, slot 1 opposite) and one independent weight set per run.
+# ---------------------------------------------------------------------------------------------
+@dataclass
+class OnsiteParityInputs:
+    lmax: int
+    lmax_out: int
+    N: int
+    C: int
+    batch: int
+    A: np.ndarray      # [batch, 2, N, L2]
+    B: np.ndarray      # [batch, 2, N, L2]
+    W_a: np.ndarray    # [16, C, N]
+    W_b: np.ndarray    # [16, C, N]
+    W_out: np.ndarray  # [16, N, C]
+
+
+def make_onsite_parity(lmax: int, lmax_out: int, N: int, C: int, batch: int, seed: int = 0) -> OnsiteParityInputs:
+    """Same distributions as make_onsite, with both parity slots populated and 16 weight sets."""
+    L2 = (lmax + 1) ** 2
+    rA, rB, rWa, rWb, rWo = _streams(seed, 5)
+    A = rA.standard_normal((batch, 2, N, L2), dtype=np.float32)
+    B = rB.standard_normal((batch, 2, N, L2), dtype=np.float32)
+    W_a = (rWa.standard_normal((16, C, N), dtype=np.float32) / np.float32(np.sqrt(N))).astype(np.float32)
+    W_b = (rWb.standard_normal((16, C, N), dtype=np.float32) / np.float32(np.sqrt(N))).astype(np.float32)
+    W_out = (rWo.standard_normal((16, N, C), dtype=np.float32) / np.float32(np.sqrt(C))).astype(np.float32)
+    return OnsiteParityInputs(lmax, lmax_out, N, C, batch, A, B, W_a, W_b, W_out)
+
+
+@dataclass
+class MessageParityInputs:
+    lmax: int
+    lmax_out: int
+    N: int
+    C: int
+    nodes: int
+    E: int
+    node_feats: np.ndarray   # [nodes, 2, N, L2]
+    edge_index: np.ndarray   # [2, E]
+    edge_vec: np.ndarray     # [E, 3]
+    edge_radial: np.ndarray  # [E, 8, C]
+    W_node: np.ndarray       # [8, C, N]
+    W_out: np.ndarray        # [8, N, C]
+    degree: np.ndarray = field(default=None)
+
+
+def make_message_parity(lmax: int, lmax_out: int, N: int, C: int, nodes: int, degree, r_min: float = 0.8,
+                        r_max: float = 5.0, seed: int = 0) -> MessageParityInputs:
+    """The graph and edge vectors of make_message (same seed -> same graph); node features in both parity
+    slots; per run one Gaussian [8, C] radial weight matrix, W_node and W_out."""
+    g = make_message(lmax, lmax_out, 1, 1, nodes, degree, r_min, r_max, seed)
+    L2 = (lmax + 1) ** 2
+    rX, rRw, rWn, rWo = _streams(seed + 7919, 4)
+    length = np.linalg.norm(g.edge_vec.astype(np.float64), axis=1)
+    w_rad = rRw.standard_normal((8, 8 * C)) / np.sqrt(8.0)
+    edge_radial = (bessel_basis(length, r_max, 8) @ w_rad).astype(np.float32).reshape(g.E, 8, C)
+    node_feats = rX.standard_normal((nodes, 2, N, L2), dtype=np.float32)
+    W_node = (rWn.standard_normal((8, C, N), dtype=np.float32) / np.float32(np.sqrt(N))).astype(np.float32)
+    W_out = (rWo.standard_normal((8, N, C), dtype=np.float32) / np.float32(np.sqrt(C))).astype(np.float32)
+    return MessageParityInputs(lmax, lmax_out, N, C, nodes, g.E, node_feats, g.edge_index, g.edge_vec, edge_radial,
+                               W_node, W_out, g.degree)
+
+
 # BASELINE.json configs (index = position in BASELINE.json "configs").
 def config(idx: int, lmax: int | None = None, seed: int = 0):
     if idx == 0:
