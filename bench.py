@@ -430,9 +430,17 @@ def run_sweep(args, cg, synthetic, dev, fp32_peak_tflops, peaks):
         fn = lambda: cg.cgtp_onsite(A, B, Wa, Wb, Wo, lmax, lmax, N, C, mask, out=out)
         steps = 20 if lmax <= 8 else 5
         ms = time_steps(fn, steps, 3)
-        fl = sum(onsite_flops_per_atom(lmax, lmax, N, C, C // 2, C // 2).values())
+        cg.cgtp_profile_enable(True)
+        for _ in range(steps):
+            fn()
+        torch.cuda.synchronize()
+        prof = cg.cgtp_profile_collect()
+        cg.cgtp_profile_enable(False)
+        fls = onsite_flops_per_atom(lmax, lmax, N, C, C // 2, C // 2)
+        fl = sum(fls.values())
         by = onsite_bytes_per_atom(lmax, lmax, N)
         res.append({"lmax": lmax, "ms_per_step": ms, "contractions_per_s": batch / (ms * 1e-3),
+                    "kernel_ms": {k: v[0] / v[1] * (v[1] / steps) for k, v in prof.items()},
                     "alg_tflops": fl * batch / (ms * 1e-3) / 1e12,
                     "frac_fp32_peak": fl * batch / (ms * 1e-3) / 1e12 / fp32_peak_tflops,
                     "alg_hbm_gbs": by * batch / (ms * 1e-3) / 1e9,

@@ -146,6 +146,46 @@ int cgtp_build_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int
                         int32_t* status, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * Parity-labelled inputs (Sec. VI :193-:240; pipelines Sec. VII C a-c :383-:453 and e :469).
+ *
+ * Features carry a parity label p = +-1 next to l (Eq.(2) :33: I_{j n2 l2 m2, p2}).  Storage: a slot axis of
+ * length 2 in front of the channel axis, slot 0 = the natural-parity part p = (-1)^l, slot 1 = the
+ * opposite-parity part p = -(-1)^l (the paper's +1 / -1 slots, indexed relative to (-1)^l); `out` has the same
+ * two slots (they are the two sectors of cgtp_onsite / cgtp_message).  The output parity is p = p1 p2 (:29).
+ * Every output sector (l, p) is the sum of a Category-alpha run (direct Gaunt coupling, l1+l2+l even, Cases A
+ * and C) and a Category-beta run (surface curl, l1+l2+l odd, Cases B and D), Eq.(59); by the slot rules
+ * Eq.(44)-(45) an alpha run reads the source slot of its output sector and by Eq.(56) a beta run the other one.
+ * Each run has its own CP weights (Eq.(42)-(43), "fitted independently" :381, :437) and feeds only the output
+ * degrees with (-1)^l = sigma (Eq.(54)-(55)); tau = 0 for sigma = +1 (even l), 1 for sigma = -1 (odd l);
+ * cat = 0 alpha, 1 beta.
+ *
+ * cgtp_message_parity: run r = 4*cat + 2*s_out + tau (8 runs; the paper's (p, sigma) is (s_out, tau) with
+ * p = (-1)^{s_out} sigma); cost 4 alpha + 4 beta runs = the 12x of Eq.(60).
+ *   node_feats  device [nodes, 2, N, (lmax+1)^2]
+ *   edge_radial device [E, 8, C]  = R~ of Eq.(46) for every run
+ *   W_node      device [8, C, N]      W_out  device [8, N, C]
+ *   out         device [nodes, 2, N, (lmax_out+1)^2], fully overwritten
+ *   edge_index, edge_vec, workspace, graph status: as cgtp_message.  4*C <= 1024.
+ * cgtp_onsite_parity (VII C e): run r = 8*cat + 4*s1 + 2*s2 + tau over the slots s1 of A and s2 of B (16 runs,
+ * the paper's 24x); the run's alpha part lands in sector s1^s2, its beta part in sector 1^s1^s2.
+ *   A, B        device [batch, 2, N, (lmax+1)^2]
+ *   W_a, W_b    device [16, C, N]     W_out  device [16, N, C]
+ *   out         device [batch, 2, N, (lmax_out+1)^2], fully overwritten
+ * ------------------------------------------------------------------------------------------- */
+size_t cgtp_onsite_parity_workspace_bytes(int lmax, int lmax_out, int N, int C, int64_t batch);
+
+int cgtp_onsite_parity(const float* A, const float* B, const float* W_a, const float* W_b, const float* W_out,
+                       int lmax, int lmax_out, int N, int C, float* out, int64_t batch, void* workspace,
+                       size_t workspace_bytes, void* cuda_stream);
+
+size_t cgtp_message_parity_workspace_bytes(int lmax, int lmax_out, int N, int C, int64_t nodes, int64_t E);
+
+int cgtp_message_parity(const float* node_feats, const int64_t* edge_index, const float* edge_vec,
+                        const float* edge_radial, const float* W_node, const float* W_out,
+                        int lmax, int lmax_out, int N, int C, float* out, int64_t nodes, int64_t E,
+                        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Host-buffer entry points (end-to-end path): same semantics as cgtp_onsite / cgtp_message, but
  * every tensor pointer is HOST memory (pinned memory recommended; pageable works, slower).  The
  * library allocates device memory from the CUDA stream-ordered pool, copies inputs host->device in

@@ -64,6 +64,261 @@ static size_t message_ws_bytes(int lmax, int lmax_out, int C, int Co, int64_t n_
     return 256 + fl * sizeof(float) + (size_t)(n_recv + 1) * sizeof(int64_t) + 12 * 256;
 }
 
+// One run of the on-site pipeline S1-S5 over Ce even + Co odd rank channels (internal channel order: even block, then
+// odd block).  cgtp_onsite is one pass; the parity-slot entry point (cgtp_onsite_parity) is four passes that differ in
+// the input slots, the weight rows and the output sectors.
+struct OnsitePass {
+    const float *A, *B;   // first atom's [N, L2] block of each factor
+    int64_t x_bs;         // floats between consecutive atoms
+    const float *W_a, *W_b;
+    const int* idx_in;    // [Ce+Co] device: row of W_a / W_b (row length N) of internal channel k
+    const float* W_out;
+    int ldw_out;          // floats between output rows n of W_out
+    const int *idx_out_e, *idx_out_o;  // [Ce], [Co] device: offset of channel k inside a row of W_out
+    int Ce, Co;
+    float *out_e, *out_o; // first atom's [N, Lo2] block of the sector written by the even / odd channels
+    int64_t o_bs;
+    int accumulate;       // 1: add to the output sectors
+    int sigma_C;          // 0: none; > 0: channel k keeps only the output degrees l with (l & 1) == ((k / sigma_C) & 1)
+                          // inside its parity block (Eq.(54): (-1)^l = sigma)
+};
+
+static int onsite_pass(const Plan* p, int N, const OnsitePass& q, int64_t batch, void* workspace, cudaStream_t st)
+{
+    const int Ce = q.Ce, Co = q.Co;
+    // fast core (onsite_core.cu) when both parities fit; it wants odd row strides and 32-column groups
+    const bool fast = (Ce == 0 || onsite_fast_supported(p, false)) && (Co == 0 || onsite_fast_supported(p, true));
+    const int hstr = fast ? onsite_fast_hstride(p) : p->L2p;
+    const int tstr = fast ? onsite_fast_tstride(p) : p->Lo2p;
+    const size_t ncol_e = (size_t)round_up((int)((size_t)batch * Ce % 32), 32) + (size_t)batch * Ce / 32 * 32;
+    const size_t ncol_o = (size_t)round_up((int)((size_t)batch * Co % 32), 32) + (size_t)batch * Co / 32 * 32;
+
+    Carver cv(workspace);
+    float* Ha_e = cv.take<float>(ncol_e * hstr);
+    float* Ha_o = cv.take<float>(ncol_o * hstr);
+    float* Hb_e = cv.take<float>(ncol_e * hstr);
+    float* Hb_o = cv.take<float>(ncol_o * hstr);
+    float* T_e = cv.take<float>(ncol_e * tstr);
+    float* T_o = cv.take<float>(ncol_o * tstr);
+    if (fast) {
+        // columns that pad the last group: define them (their results are never read)
+        const size_t ne = (size_t)batch * Ce, no = (size_t)batch * Co;
+        if (ncol_e > ne) {
+            CGTP_CUDA_CHECK(cudaMemsetAsync(Ha_e + ne * hstr, 0, (ncol_e - ne) * hstr * 4, st));
+            CGTP_CUDA_CHECK(cudaMemsetAsync(Hb_e + ne * hstr, 0, (ncol_e - ne) * hstr * 4, st));
+        }
+        if (ncol_o > no) {
+            CGTP_CUDA_CHECK(cudaMemsetAsync(Ha_o + no * hstr, 0, (ncol_o - no) * hstr * 4, st));
+            CGTP_CUDA_CHECK(cudaMemsetAsync(Hb_o + no * hstr, 0, (ncol_o - no) * hstr * 4, st));
+        }
+    }
+
+    // S1: H = W . A (Eq.(35)); rows are written in parity-sorted channel order, even block then odd block
+    ProjArgs pin[2];
+    for (int s = 0; s < 2; ++s) {
+        ProjArgs& a = pin[s];
+        a.X = s ? q.B : q.A;
+        a.x_bs = q.x_bs;
+        a.x_rs = p->L2;
+        a.W = s ? q.W_b : q.W_a;
+        a.ldw_m = N;
+        a.ldw_k = 1;
+        a.idx_m = q.idx_in;
+        a.idx_k = nullptr;
+        a.M = Ce + Co;
+        a.K = N;
+        a.J = p->L2;
+        a.out0 = s ? Hb_e : Ha_e;
+        a.o_bs0 = (int64_t)Ce * hstr;
+        a.out1 = s ? Hb_o : Ha_o;
+        a.o_bs1 = (int64_t)Co * hstr;
+        a.m_split = Ce;
+        a.o_rs = hstr;
+        a.batch = batch;
+        a.accumulate = 0;
+    }
+    int rc = launch_proj(pin, 2, K_PROJ_IN, st);
+    if (rc) return rc;
+
+    // S2-S4 fused, one launch per parity
+    rc = fast ? launch_onsite_fast(p, false, Ha_e, Hb_e, T_e, batch * Ce, st)
+              : launch_onsite_generic(p, false, Ha_e, Hb_e, T_e, batch * Ce, st);
+    if (rc) return rc;
+    rc = fast ? launch_onsite_fast(p, true, Ha_o, Hb_o, T_o, batch * Co, st)
+              : launch_onsite_generic(p, true, Ha_o, Hb_o, T_o, batch * Co, st);
+    if (rc) return rc;
+    if (q.sigma_C > 0) {
+        rc = launch_sigma_mask(T_e, tstr, batch * Ce, Ce, q.sigma_C, p->Lo2, st);
+        if (rc) return rc;
+        rc = launch_sigma_mask(T_o, tstr, batch * Co, Co, q.sigma_C, p->Lo2, st);
+        if (rc) return rc;
+    }
+
+    // S5: out[b, s] = W_out[:, channels of sector s] . T_s (Eq.(41))
+    ProjArgs po[2];
+    for (int s = 0; s < 2; ++s) {
+        ProjArgs& a = po[s];
+        a.X = s ? T_o : T_e;
+        a.x_bs = (int64_t)(s ? Co : Ce) * tstr;
+        a.x_rs = tstr;
+        a.W = q.W_out;
+        a.ldw_m = q.ldw_out;
+        a.ldw_k = 1;
+        a.idx_m = nullptr;
+        a.idx_k = s ? q.idx_out_o : q.idx_out_e;
+        a.M = N;
+        a.K = s ? Co : Ce;
+        a.J = p->Lo2;
+        a.out0 = s ? q.out_o : q.out_e;
+        a.o_bs0 = q.o_bs;
+        a.out1 = a.out0;
+        a.o_bs1 = a.o_bs0;
+        a.m_split = N;
+        a.o_rs = p->Lo2;
+        a.batch = batch;
+        a.accumulate = q.accumulate;
+    }
+    return launch_proj(po, 2, K_PROJ_OUT, st);
+}
+
+static int check_message_args(const float* node_feats, const int64_t* edge_index, const float* edge_vec,
+                              const float* edge_radial, const float* W_node, const float* W_out, const float* out,
+                              int64_t n_send, int64_t nodes, int64_t E, const void* workspace)
+{
+    if (nodes < 0 || n_send < 0 || E < 0) { set_error("negative size"); return CGTP_ERR_INVALID; }
+    if (nodes == 0) return CGTP_OK;
+    if (n_send == 0 && E > 0) { set_error("edges without sender nodes"); return CGTP_ERR_INVALID; }
+    if ((!node_feats && n_send > 0) || !W_node || !W_out || !out || !workspace || (E > 0 && (!edge_index || !edge_vec || !edge_radial))) {
+        set_error("null pointer argument");
+        return CGTP_ERR_INVALID;
+    }
+    if (!aligned16(node_feats) || !aligned16(out) || !aligned16(W_node) || !aligned16(W_out) ||
+        (E > 0 && (!aligned16(edge_index) || !aligned16(edge_vec) || !aligned16(edge_radial))) ||
+        (reinterpret_cast<uintptr_t>(workspace) & 255u)) {
+        set_error("misaligned pointer (tensors need 16-byte, workspace 256-byte alignment)");
+        return CGTP_ERR_INVALID;
+    }
+    return CGTP_OK;
+}
+
+// One run of the message-passing pipeline M0-M6 over Ce even + Co odd rank channels; cgtp_message(_bipartite) is one
+// pass, cgtp_message_parity two (one per source slot).
+struct MessagePass {
+    const float* node_feats;  // first sender's [N, L2] block
+    int64_t x_bs;             // floats between consecutive senders
+    const float* W_node;
+    const int* idx_in;        // [Ce+Co] device: row of W_node (row length N) AND column of edge_radial of channel k
+    const float* edge_radial;
+    int radial_stride;        // floats between consecutive edges of edge_radial
+    const float* W_out;
+    int ldw_out;
+    const int *idx_out_e, *idx_out_o;
+    int Ce, Co;
+    float *out_e, *out_o;
+    int64_t o_bs;
+    int accumulate;
+    int sigma_C;              // as OnsitePass::sigma_C
+    bool segments_done;       // row_ptr / status of this workspace are already built (second pass)
+};
+
+static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_t* edge_index, const float* edge_vec,
+                        int64_t n_send, int64_t nodes, int64_t E, void* workspace, cudaStream_t st)
+{
+    const int Ce = q.Ce, Co = q.Co;
+    Carver cv(workspace);
+    int32_t* status = cv.take<int32_t>(1);
+    int64_t* row_ptr = cv.take<int64_t>((size_t)nodes + 1);
+    float* H_e = cv.take<float>((size_t)n_send * Ce * p->L2p);
+    float* H_o = cv.take<float>((size_t)n_send * Co * p->L2p);
+    float* G_e = cv.take<float>((size_t)n_send * Ce * p->UVp);
+    float* G_o = cv.take<float>((size_t)n_send * Co * 2 * p->UVp);
+    float* S_e = cv.take<float>((size_t)nodes * Ce * p->UVp);
+    float* S_o = cv.take<float>((size_t)nodes * Co * p->UVp);
+    float* T_e = cv.take<float>((size_t)nodes * Ce * p->Lo2p);
+    float* T_o = cv.take<float>((size_t)nodes * Co * p->Lo2p);
+
+    // M0
+    int rc = CGTP_OK;
+    if (!q.segments_done) {
+        rc = launch_segments(edge_index, E, nodes, n_send, row_ptr, status, st);
+        if (rc) return rc;
+    }
+
+    // M1: H = W_node . node_feats (Eq.(47))
+    ProjArgs a;
+    a.X = q.node_feats;
+    a.x_bs = q.x_bs;
+    a.x_rs = p->L2;
+    a.W = q.W_node;
+    a.ldw_m = N;
+    a.ldw_k = 1;
+    a.idx_m = q.idx_in;
+    a.idx_k = nullptr;
+    a.M = Ce + Co;
+    a.K = N;
+    a.J = p->L2;
+    a.out0 = H_e;
+    a.o_bs0 = (int64_t)Ce * p->L2p;
+    a.out1 = H_o;
+    a.o_bs1 = (int64_t)Co * p->L2p;
+    a.m_split = Ce;
+    a.o_rs = p->L2p;
+    a.batch = n_send;
+    a.accumulate = 0;
+    rc = launch_proj(&a, 1, K_PROJ_IN, st);
+    if (rc) return rc;
+
+    // M2
+    rc = launch_node_synth(p, false, H_e, G_e, n_send * Ce, st);
+    if (rc) return rc;
+    rc = launch_node_synth(p, true, H_o, G_o, n_send * Co, st);
+    if (rc) return rc;
+
+    // M3 + M4
+    rc = launch_edge(p, false, G_e, row_ptr, edge_index, E, edge_vec, q.edge_radial, q.idx_in, Ce, q.radial_stride, S_e, nodes, status, st);
+    if (rc) return rc;
+    rc = launch_edge(p, true, G_o, row_ptr, edge_index, E, edge_vec, q.edge_radial, q.idx_in + Ce, Co, q.radial_stride, S_o, nodes, status, st);
+    if (rc) return rc;
+
+    // M5
+    rc = launch_analysis(p, false, S_e, T_e, nodes * Ce, st);
+    if (rc) return rc;
+    rc = launch_analysis(p, true, S_o, T_o, nodes * Co, st);
+    if (rc) return rc;
+    if (q.sigma_C > 0) {
+        rc = launch_sigma_mask(T_e, p->Lo2p, nodes * Ce, Ce, q.sigma_C, p->Lo2, st);
+        if (rc) return rc;
+        rc = launch_sigma_mask(T_o, p->Lo2p, nodes * Co, Co, q.sigma_C, p->Lo2, st);
+        if (rc) return rc;
+    }
+
+    // M6
+    ProjArgs po[2];
+    for (int s = 0; s < 2; ++s) {
+        ProjArgs& b = po[s];
+        b.X = s ? T_o : T_e;
+        b.x_bs = (int64_t)(s ? Co : Ce) * p->Lo2p;
+        b.x_rs = p->Lo2p;
+        b.W = q.W_out;
+        b.ldw_m = q.ldw_out;
+        b.ldw_k = 1;
+        b.idx_m = nullptr;
+        b.idx_k = s ? q.idx_out_o : q.idx_out_e;
+        b.M = N;
+        b.K = s ? Co : Ce;
+        b.J = p->Lo2;
+        b.out0 = s ? q.out_o : q.out_e;
+        b.o_bs0 = q.o_bs;
+        b.out1 = b.out0;
+        b.o_bs1 = b.o_bs0;
+        b.m_split = N;
+        b.o_rs = p->Lo2;
+        b.batch = nodes;
+        b.accumulate = q.accumulate;
+    }
+    return launch_proj(po, 2, K_PROJ_OUT, st);
+}
+
 }  // namespace cgtp
 
 using namespace cgtp;
@@ -113,93 +368,25 @@ int cgtp_onsite(const float* A, const float* B, const float* W_a, const float* W
     if (!p) return CGTP_ERR_CUDA;
     const ChannelPlan* cp = get_channel_plan(C, parity_mask);
     if (!cp) return CGTP_ERR_CUDA;
-    const int Ce = cp->Ce, Co = cp->Co;
-
-    // fast core (onsite_core.cu) when both parities fit; it wants odd row strides and 32-column groups
-    const bool fast = (Ce == 0 || onsite_fast_supported(p, false)) && (Co == 0 || onsite_fast_supported(p, true));
-    const int hstr = fast ? onsite_fast_hstride(p) : p->L2p;
-    const int tstr = fast ? onsite_fast_tstride(p) : p->Lo2p;
-    const size_t ncol_e = (size_t)round_up((int)((size_t)batch * Ce % 32), 32) + (size_t)batch * Ce / 32 * 32;
-    const size_t ncol_o = (size_t)round_up((int)((size_t)batch * Co % 32), 32) + (size_t)batch * Co / 32 * 32;
-
-    Carver cv(workspace);
-    float* Ha_e = cv.take<float>(ncol_e * hstr);
-    float* Ha_o = cv.take<float>(ncol_o * hstr);
-    float* Hb_e = cv.take<float>(ncol_e * hstr);
-    float* Hb_o = cv.take<float>(ncol_o * hstr);
-    float* T_e = cv.take<float>(ncol_e * tstr);
-    float* T_o = cv.take<float>(ncol_o * tstr);
-    if (fast) {
-        // columns that pad the last group: define them (their results are never read)
-        const size_t ne = (size_t)batch * Ce, no = (size_t)batch * Co;
-        if (ncol_e > ne) {
-            CGTP_CUDA_CHECK(cudaMemsetAsync(Ha_e + ne * hstr, 0, (ncol_e - ne) * hstr * 4, st));
-            CGTP_CUDA_CHECK(cudaMemsetAsync(Hb_e + ne * hstr, 0, (ncol_e - ne) * hstr * 4, st));
-        }
-        if (ncol_o > no) {
-            CGTP_CUDA_CHECK(cudaMemsetAsync(Ha_o + no * hstr, 0, (ncol_o - no) * hstr * 4, st));
-            CGTP_CUDA_CHECK(cudaMemsetAsync(Hb_o + no * hstr, 0, (ncol_o - no) * hstr * 4, st));
-        }
-    }
-
-    // S1: H = W . A (Eq.(35)); rows are written in parity-sorted channel order, even block then odd block
-    ProjArgs pin[2];
-    for (int s = 0; s < 2; ++s) {
-        ProjArgs& a = pin[s];
-        a.X = s ? B : A;
-        a.x_bs = (int64_t)N * p->L2;
-        a.x_rs = p->L2;
-        a.W = s ? W_b : W_a;
-        a.ldw_m = N;
-        a.ldw_k = 1;
-        a.idx_m = cp->perm_dev;
-        a.idx_k = nullptr;
-        a.M = C;
-        a.K = N;
-        a.J = p->L2;
-        a.out0 = s ? Hb_e : Ha_e;
-        a.o_bs0 = (int64_t)Ce * hstr;
-        a.out1 = s ? Hb_o : Ha_o;
-        a.o_bs1 = (int64_t)Co * hstr;
-        a.m_split = Ce;
-        a.o_rs = hstr;
-        a.batch = batch;
-    }
-    rc = launch_proj(pin, 2, K_PROJ_IN, st);
-    if (rc) return rc;
-
-    // S2-S4 fused, one launch per parity
-    rc = fast ? launch_onsite_fast(p, false, Ha_e, Hb_e, T_e, batch * Ce, st)
-              : launch_onsite_generic(p, false, Ha_e, Hb_e, T_e, batch * Ce, st);
-    if (rc) return rc;
-    rc = fast ? launch_onsite_fast(p, true, Ha_o, Hb_o, T_o, batch * Co, st)
-              : launch_onsite_generic(p, true, Ha_o, Hb_o, T_o, batch * Co, st);
-    if (rc) return rc;
-
-    // S5: out[b, s] = W_out[:, channels of sector s] . T_s (Eq.(41))
-    ProjArgs po[2];
-    for (int s = 0; s < 2; ++s) {
-        ProjArgs& a = po[s];
-        a.X = s ? T_o : T_e;
-        a.x_bs = (int64_t)(s ? Co : Ce) * tstr;
-        a.x_rs = tstr;
-        a.W = W_out;
-        a.ldw_m = C;
-        a.ldw_k = 1;
-        a.idx_m = nullptr;
-        a.idx_k = cp->perm_dev + (s ? Ce : 0);
-        a.M = N;
-        a.K = s ? Co : Ce;
-        a.J = p->Lo2;
-        a.out0 = out + (size_t)s * N * p->Lo2;
-        a.o_bs0 = (int64_t)2 * N * p->Lo2;
-        a.out1 = a.out0;
-        a.o_bs1 = a.o_bs0;
-        a.m_split = N;
-        a.o_rs = p->Lo2;
-        a.batch = batch;
-    }
-    return launch_proj(po, 2, K_PROJ_OUT, st);
+    OnsitePass q;
+    q.A = A;
+    q.B = B;
+    q.x_bs = (int64_t)N * p->L2;
+    q.W_a = W_a;
+    q.W_b = W_b;
+    q.idx_in = cp->perm_dev;
+    q.W_out = W_out;
+    q.ldw_out = C;
+    q.idx_out_e = cp->perm_dev;
+    q.idx_out_o = cp->perm_dev + cp->Ce;
+    q.Ce = cp->Ce;
+    q.Co = cp->Co;
+    q.out_e = out;
+    q.out_o = out + (size_t)N * p->Lo2;
+    q.o_bs = (int64_t)2 * N * p->Lo2;
+    q.accumulate = 0;
+    q.sigma_C = 0;
+    return onsite_pass(p, N, q, batch, workspace, st);
 }
 
 size_t cgtp_message_workspace_bytes(int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask, int64_t nodes,
@@ -241,19 +428,8 @@ int cgtp_message_bipartite(const float* node_feats, const int64_t* edge_index, c
     clear_error();
     int rc = check_common(lmax, lmax_out, N, C, parity_mask);
     if (rc) return rc;
-    if (nodes < 0 || n_send < 0 || E < 0) { set_error("negative size"); return CGTP_ERR_INVALID; }
-    if (nodes == 0) return CGTP_OK;
-    if (n_send == 0 && E > 0) { set_error("edges without sender nodes"); return CGTP_ERR_INVALID; }
-    if ((!node_feats && n_send > 0) || !W_node || !W_out || !out || !workspace || (E > 0 && (!edge_index || !edge_vec || !edge_radial))) {
-        set_error("null pointer argument");
-        return CGTP_ERR_INVALID;
-    }
-    if (!aligned16(node_feats) || !aligned16(out) || !aligned16(W_node) || !aligned16(W_out) ||
-        (E > 0 && (!aligned16(edge_index) || !aligned16(edge_vec) || !aligned16(edge_radial))) ||
-        (reinterpret_cast<uintptr_t>(workspace) & 255u)) {
-        set_error("misaligned pointer (tensors need 16-byte, workspace 256-byte alignment)");
-        return CGTP_ERR_INVALID;
-    }
+    rc = check_message_args(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, out, n_send, nodes, E, workspace);
+    if (rc || nodes == 0) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const Plan* p = get_plan(lmax, lmax_out);
     if (!p) return CGTP_ERR_CUDA;
@@ -264,88 +440,26 @@ int cgtp_message_bipartite(const float* node_feats, const int64_t* edge_index, c
         set_error("workspace too small: %zu < %zu bytes", workspace_bytes, message_ws_bytes(lmax, lmax_out, C, Co, n_send, nodes));
         return CGTP_ERR_INVALID;
     }
-
-    Carver cv(workspace);
-    int32_t* status = cv.take<int32_t>(1);
-    int64_t* row_ptr = cv.take<int64_t>((size_t)nodes + 1);
-    float* H_e = cv.take<float>((size_t)n_send * Ce * p->L2p);
-    float* H_o = cv.take<float>((size_t)n_send * Co * p->L2p);
-    float* G_e = cv.take<float>((size_t)n_send * Ce * p->UVp);
-    float* G_o = cv.take<float>((size_t)n_send * Co * 2 * p->UVp);
-    float* S_e = cv.take<float>((size_t)nodes * Ce * p->UVp);
-    float* S_o = cv.take<float>((size_t)nodes * Co * p->UVp);
-    float* T_e = cv.take<float>((size_t)nodes * Ce * p->Lo2p);
-    float* T_o = cv.take<float>((size_t)nodes * Co * p->Lo2p);
-
-    // M0
-    rc = launch_segments(edge_index, E, nodes, n_send, row_ptr, status, st);
-    if (rc) return rc;
-
-    // M1: H = W_node . node_feats (Eq.(47))
-    ProjArgs a;
-    a.X = node_feats;
-    a.x_bs = (int64_t)N * p->L2;
-    a.x_rs = p->L2;
-    a.W = W_node;
-    a.ldw_m = N;
-    a.ldw_k = 1;
-    a.idx_m = cp->perm_dev;
-    a.idx_k = nullptr;
-    a.M = C;
-    a.K = N;
-    a.J = p->L2;
-    a.out0 = H_e;
-    a.o_bs0 = (int64_t)Ce * p->L2p;
-    a.out1 = H_o;
-    a.o_bs1 = (int64_t)Co * p->L2p;
-    a.m_split = Ce;
-    a.o_rs = p->L2p;
-    a.batch = n_send;
-    rc = launch_proj(&a, 1, K_PROJ_IN, st);
-    if (rc) return rc;
-
-    // M2
-    rc = launch_node_synth(p, false, H_e, G_e, n_send * Ce, st);
-    if (rc) return rc;
-    rc = launch_node_synth(p, true, H_o, G_o, n_send * Co, st);
-    if (rc) return rc;
-
-    // M3 + M4
-    rc = launch_edge(p, false, G_e, row_ptr, edge_index, E, edge_vec, edge_radial, cp->perm_dev, Ce, C, S_e, nodes, status, st);
-    if (rc) return rc;
-    rc = launch_edge(p, true, G_o, row_ptr, edge_index, E, edge_vec, edge_radial, cp->perm_dev + Ce, Co, C, S_o, nodes, status, st);
-    if (rc) return rc;
-
-    // M5
-    rc = launch_analysis(p, false, S_e, T_e, nodes * Ce, st);
-    if (rc) return rc;
-    rc = launch_analysis(p, true, S_o, T_o, nodes * Co, st);
-    if (rc) return rc;
-
-    // M6
-    ProjArgs po[2];
-    for (int s = 0; s < 2; ++s) {
-        ProjArgs& b = po[s];
-        b.X = s ? T_o : T_e;
-        b.x_bs = (int64_t)(s ? Co : Ce) * p->Lo2p;
-        b.x_rs = p->Lo2p;
-        b.W = W_out;
-        b.ldw_m = C;
-        b.ldw_k = 1;
-        b.idx_m = nullptr;
-        b.idx_k = cp->perm_dev + (s ? Ce : 0);
-        b.M = N;
-        b.K = s ? Co : Ce;
-        b.J = p->Lo2;
-        b.out0 = out + (size_t)s * N * p->Lo2;
-        b.o_bs0 = (int64_t)2 * N * p->Lo2;
-        b.out1 = b.out0;
-        b.o_bs1 = b.o_bs0;
-        b.m_split = N;
-        b.o_rs = p->Lo2;
-        b.batch = nodes;
-    }
-    return launch_proj(po, 2, K_PROJ_OUT, st);
+    MessagePass q;
+    q.node_feats = node_feats;
+    q.x_bs = (int64_t)N * p->L2;
+    q.W_node = W_node;
+    q.idx_in = cp->perm_dev;
+    q.edge_radial = edge_radial;
+    q.radial_stride = C;
+    q.W_out = W_out;
+    q.ldw_out = C;
+    q.idx_out_e = cp->perm_dev;
+    q.idx_out_o = cp->perm_dev + Ce;
+    q.Ce = Ce;
+    q.Co = Co;
+    q.out_e = out;
+    q.out_o = out + (size_t)N * p->Lo2;
+    q.o_bs = (int64_t)2 * N * p->Lo2;
+    q.accumulate = 0;
+    q.sigma_C = 0;
+    q.segments_done = false;
+    return message_pass(p, N, q, edge_index, edge_vec, n_send, nodes, E, workspace, st);
 }
 
 int cgtp_message(const float* node_feats, const int64_t* edge_index, const float* edge_vec, const float* edge_radial,
@@ -368,6 +482,125 @@ int cgtp_message_status(const void* workspace, void* cuda_stream)
     if (h != 0) {
         set_error("edge_index is not receiver-sorted or has an index outside [0, nodes)");
         return CGTP_ERR_GRAPH;
+    }
+    return CGTP_OK;
+}
+
+// ------------------------------------------------------------------------------ parity-slot entry points
+size_t cgtp_onsite_parity_workspace_bytes(int lmax, int lmax_out, int N, int C, int64_t batch)
+{
+    (void)N;
+    if (lmax < 0 || lmax_out < 0 || C <= 0 || batch < 0) return 0;
+    return onsite_ws_bytes(lmax, lmax_out, 4 * C, batch);
+}
+
+int cgtp_onsite_parity(const float* A, const float* B, const float* W_a, const float* W_b, const float* W_out, int lmax,
+                       int lmax_out, int N, int C, float* out, int64_t batch, void* workspace, size_t workspace_bytes,
+                       void* cuda_stream)
+{
+    clear_error();
+    if (C <= 0 || C > 256) { set_error("C=%d outside [1, 256] (4*C internal rank channels per pass)", C); return C <= 0 ? CGTP_ERR_INVALID : CGTP_ERR_UNSUPPORTED; }
+    uint8_t mask[1024];
+    for (int k = 0; k < 4 * C; ++k) mask[k] = k >= 2 * C;
+    int rc = check_common(lmax, lmax_out, N, 4 * C, mask);
+    if (rc) return rc;
+    if (batch < 0) { set_error("negative batch"); return CGTP_ERR_INVALID; }
+    if (batch == 0) return CGTP_OK;
+    if (!A || !B || !W_a || !W_b || !W_out || !out || !workspace) { set_error("null pointer argument"); return CGTP_ERR_INVALID; }
+    if (!aligned16(A) || !aligned16(B) || !aligned16(out) || !aligned16(W_a) || !aligned16(W_b) || !aligned16(W_out) ||
+        (reinterpret_cast<uintptr_t>(workspace) & 255u)) {
+        set_error("misaligned pointer (tensors need 16-byte, workspace 256-byte alignment)");
+        return CGTP_ERR_INVALID;
+    }
+    if (workspace_bytes < onsite_ws_bytes(lmax, lmax_out, 4 * C, batch)) {
+        set_error("workspace too small: %zu < %zu bytes", workspace_bytes, onsite_ws_bytes(lmax, lmax_out, 4 * C, batch));
+        return CGTP_ERR_INVALID;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const Plan* p = get_plan(lmax, lmax_out);
+    if (!p) return CGTP_ERR_CUDA;
+    const ParityPlan* pp = get_parity_plan(C, N, false);
+    if (!pp) return CGTP_ERR_CUDA;
+    const size_t slot = (size_t)N * p->L2, sector = (size_t)N * p->Lo2;
+    for (int ps = 0; ps < 4; ++ps) {
+        const int s1 = ps >> 1, s2 = ps & 1;
+        OnsitePass q;
+        q.A = A + (size_t)s1 * slot;
+        q.B = B + (size_t)s2 * slot;
+        q.x_bs = (int64_t)2 * slot;
+        q.W_a = W_a;
+        q.W_b = W_b;
+        q.idx_in = pp->idx_in(ps);
+        q.W_out = W_out;
+        q.ldw_out = C;
+        q.idx_out_e = pp->idx_out(ps);
+        q.idx_out_o = pp->idx_out(ps) + 2 * C;
+        q.Ce = 2 * C;
+        q.Co = 2 * C;
+        q.out_e = out + (size_t)(s1 ^ s2) * sector;      // alpha: p = p1 p2 with l1+l2+l even -> slot s1 ^ s2
+        q.out_o = out + (size_t)(1 ^ s1 ^ s2) * sector;  // beta: l1+l2+l odd -> the other slot
+        q.o_bs = (int64_t)2 * sector;
+        q.accumulate = ps > 0;  // pass (0,0) writes both sectors, the others add to them
+        q.sigma_C = C;
+        rc = onsite_pass(p, N, q, batch, workspace, st);
+        if (rc) return rc;
+    }
+    return CGTP_OK;
+}
+
+size_t cgtp_message_parity_workspace_bytes(int lmax, int lmax_out, int N, int C, int64_t nodes, int64_t E)
+{
+    (void)N;
+    (void)E;
+    if (lmax < 0 || lmax_out < 0 || C <= 0 || nodes < 0) return 0;
+    return message_ws_bytes(lmax, lmax_out, 4 * C, 2 * C, nodes, nodes);
+}
+
+int cgtp_message_parity(const float* node_feats, const int64_t* edge_index, const float* edge_vec,
+                        const float* edge_radial, const float* W_node, const float* W_out, int lmax, int lmax_out,
+                        int N, int C, float* out, int64_t nodes, int64_t E, void* workspace, size_t workspace_bytes,
+                        void* cuda_stream)
+{
+    clear_error();
+    if (C <= 0 || C > 256) { set_error("C=%d outside [1, 256] (4*C internal rank channels per pass)", C); return C <= 0 ? CGTP_ERR_INVALID : CGTP_ERR_UNSUPPORTED; }
+    uint8_t mask[1024];
+    for (int k = 0; k < 4 * C; ++k) mask[k] = k >= 2 * C;
+    int rc = check_common(lmax, lmax_out, N, 4 * C, mask);
+    if (rc) return rc;
+    rc = check_message_args(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, out, nodes, nodes, E, workspace);
+    if (rc || nodes == 0) return rc;
+    if (workspace_bytes < message_ws_bytes(lmax, lmax_out, 4 * C, 2 * C, nodes, nodes)) {
+        set_error("workspace too small: %zu < %zu bytes", workspace_bytes, message_ws_bytes(lmax, lmax_out, 4 * C, 2 * C, nodes, nodes));
+        return CGTP_ERR_INVALID;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const Plan* p = get_plan(lmax, lmax_out);
+    if (!p) return CGTP_ERR_CUDA;
+    const ParityPlan* pp = get_parity_plan(C, N, true);
+    if (!pp) return CGTP_ERR_CUDA;
+    const size_t slot = (size_t)N * p->L2, sector = (size_t)N * p->Lo2;
+    for (int s_in = 0; s_in < 2; ++s_in) {
+        MessagePass q;
+        q.node_feats = node_feats + (size_t)s_in * slot;
+        q.x_bs = (int64_t)2 * slot;
+        q.W_node = W_node;
+        q.idx_in = pp->idx_in(s_in);
+        q.edge_radial = edge_radial;
+        q.radial_stride = 8 * C;
+        q.W_out = W_out;
+        q.ldw_out = C;
+        q.idx_out_e = pp->idx_out(s_in);
+        q.idx_out_o = pp->idx_out(s_in) + 2 * C;
+        q.Ce = 2 * C;
+        q.Co = 2 * C;
+        q.out_e = out + (size_t)s_in * sector;        // Eq.(45): alpha reads the slot of its output sector
+        q.out_o = out + (size_t)(1 - s_in) * sector;  // Eq.(56): beta reads the opposite slot
+        q.o_bs = (int64_t)2 * sector;
+        q.accumulate = s_in > 0;
+        q.sigma_C = C;
+        q.segments_done = s_in > 0;
+        rc = message_pass(p, N, q, edge_index, edge_vec, nodes, nodes, E, workspace, st);
+        if (rc) return rc;
     }
     return CGTP_OK;
 }

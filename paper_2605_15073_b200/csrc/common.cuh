@@ -77,6 +77,21 @@ struct ChannelPlan {
 const ChannelPlan* get_channel_plan(int C, const uint8_t* parity_mask);
 
 // ---------------------------------------------------------------------------------------------
+// Parity plan (parity.cu): weight-row / weight-column index tables of the passes of the parity-slot entry points.
+// ---------------------------------------------------------------------------------------------
+struct ParityPlan {
+    int C, N;
+    bool message;
+    int npass;       // 4 on-site passes (s1, s2), 2 message passes (s_in)
+    const int* dev;  // device [npass][2][4C]: idx_in, idx_out of pass ps
+    const int* idx_in(int ps) const { return dev + (size_t)ps * 8 * C; }
+    const int* idx_out(int ps) const { return dev + (size_t)ps * 8 * C + 4 * C; }
+};
+const ParityPlan* get_parity_plan(int C, int N, bool message);
+// Clears T[col][lm] for the degrees l whose parity is not the sigma of the column's channel (Eq.(54)).
+int launch_sigma_mask(float* T, int stride, int64_t ncols, int Cpar, int Cs, int Lo2, cudaStream_t st);
+
+// ---------------------------------------------------------------------------------------------
 // Errors, launch accounting, profiling
 // ---------------------------------------------------------------------------------------------
 void set_error(const char* fmt, ...);
@@ -139,6 +154,7 @@ struct ProjArgs {
     int m_split;
     int o_rs;
     int64_t batch;
+    int accumulate;  // 1: add to the output instead of overwriting it (second pass of the parity-slot entry points)
 };
 int launch_proj(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st);
 // Fast path of launch_proj (proj_fast.cu): TMA-staged features, packed FP32 FMAs; *handled = false when the

@@ -1,0 +1,82 @@
+// parity.cu -- routing layer of the parity-slot entry points (Sec. VI :193-:240,
+// Sec. VII C a-c, e :383-:469): the index tables that select, for every pass, the weight rows of the runs
+// (category, slots, output-l parity sigma) it evaluates, and the kernel that applies Eq.(54)'s restriction
+// (-1)^l = sigma to the analysed coefficients.
+#include <mutex>
+#include <vector>
+
+#include "common.cuh"
+
+namespace cgtp {
+
+// T[col][lm], col = b * Cpar + k: internal channel k belongs to output-l parity tau = (k / Cs) & 1; coefficients of
+// the other l-parity are not part of the run (Eq.(54)) and are cleared so that S5 / M6 (Eq.(55), (58))
+// sums the two sigma runs of a sector in one contraction.
+__global__ void __launch_bounds__(256) sigma_mask_kernel(float* __restrict__ T, int stride, int64_t ncols, int Cpar,
+                                                         int Cs, int Lo2)
+{
+    const int64_t total = ncols * Lo2;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t col = i / Lo2;
+        const int lm = (int)(i - col * Lo2);
+        int l = (int)sqrtf((float)lm);  // exact for lm < 2^23
+        const int tau = ((int)(col % Cpar) / Cs) & 1;
+        if ((l & 1) != tau) T[col * stride + lm] = 0.f;
+    }
+}
+
+int launch_sigma_mask(float* T, int stride, int64_t ncols, int Cpar, int Cs, int Lo2, cudaStream_t st)
+{
+    if (ncols <= 0 || Cpar <= 0) return CGTP_OK;
+    const int64_t total = ncols * Lo2;
+    int64_t blocks = (total + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    LaunchScope scope(K_MISC, st);
+    sigma_mask_kernel<<<(unsigned)blocks, 256, 0, st>>>(T, stride, ncols, Cpar, Cs, Lo2);
+    CGTP_CUDA_CHECK(cudaGetLastError());
+    return CGTP_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Index tables.  Internal channel order of a pass: [alpha tau=0 | alpha tau=1 | beta tau=0 | beta tau=1], C each;
+// the alpha half is the "even" block of the pipeline (pointwise product), the beta half the "odd" block (curl).
+//   on-site pass (s1, s2):  run = 8 cat + 4 s1 + 2 s2 + tau          (16 runs, weights [16, C, N] / [16, N, C])
+//   message pass s_in:      run = 4 cat + 2 (s_in ^ cat) + tau       ( 8 runs): Eq.(45): alpha reads the slot of
+//                           its output sector, Eq.(56): beta the opposite one.
+// idx_in[k] = run * C + c (row of the stacked [R*C, N] input weights; column of edge_radial [E, R*C]);
+// idx_out[k] = run * N * C + c (offset of the channel inside row n of the stacked W_out; rows are C apart).
+// ------------------------------------------------------------------------------------------------
+static std::mutex g_pp_mutex;
+static std::vector<ParityPlan*> g_pp;
+
+const ParityPlan* get_parity_plan(int C, int N, bool message)
+{
+    std::lock_guard<std::mutex> lock(g_pp_mutex);
+    for (ParityPlan* q : g_pp)
+        if (q->C == C && q->N == N && q->message == message) return q;
+    const int npass = message ? 2 : 4;
+    std::vector<int> h((size_t)npass * 8 * C);
+    for (int ps = 0; ps < npass; ++ps)
+        for (int k = 0; k < 4 * C; ++k) {
+            const int g = k / C, c = k % C, cat = g >> 1, tau = g & 1;
+            const int run = message ? 4 * cat + 2 * (ps ^ cat) + tau : 8 * cat + 4 * (ps >> 1) + 2 * (ps & 1) + tau;
+            h[((size_t)ps * 2 + 0) * 4 * C + k] = run * C + c;
+            h[((size_t)ps * 2 + 1) * 4 * C + k] = run * N * C + c;
+        }
+    int* d = nullptr;
+    if (cudaMalloc(&d, h.size() * sizeof(int)) != cudaSuccess ||
+        cudaMemcpy(d, h.data(), h.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) {
+        set_error("parity plan: device allocation / upload failed");
+        return nullptr;
+    }
+    ParityPlan* q = new ParityPlan;
+    q->C = C;
+    q->N = N;
+    q->message = message;
+    q->npass = npass;
+    q->dev = d;
+    g_pp.push_back(q);
+    return q;
+}
+
+}  // namespace cgtp

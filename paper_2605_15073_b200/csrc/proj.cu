@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(32 * WY) proj_kernel(ProjArgPack pack)
             if (m >= a.M) continue;
             float* dst = (m < a.m_split) ? a.out0 + b * a.o_bs0 + (int64_t)m * a.o_rs + j
                                          : a.out1 + b * a.o_bs1 + (int64_t)(m - a.m_split) * a.o_rs + j;
-            *dst = acc[r][t];
+            *dst = a.accumulate ? *dst + acc[r][t] : acc[r][t];
         }
     }
 }
@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(32 * WY) proj_kernel(ProjArgPack pack)
 static bool zero_fill(const ProjArgs& g, cudaStream_t st, int* rc)
 {
     *rc = CGTP_OK;
-    if (g.batch <= 0 || g.M <= 0 || g.J <= 0) return true;
+    if (g.batch <= 0 || g.M <= 0 || g.J <= 0 || g.accumulate) return true;  // adding zero: nothing to do
     if (g.o_rs != g.J || g.m_split < g.M) return false;
     const cudaError_t e = cudaMemset2DAsync(g.out0, (size_t)g.o_bs0 * 4, 0, (size_t)g.M * g.J * 4, (size_t)g.batch, st);
     if (e != cudaSuccess) {

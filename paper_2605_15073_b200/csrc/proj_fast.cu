@@ -71,7 +71,7 @@ __device__ __forceinline__ void mbar_arrive_cta(uint64_t* bar)
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
-template <int RW, int CWP>
+template <int RW, int CWP, bool ACC>
 __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
 {
     constexpr int MW = 16 * RW;       // rows per CTA
@@ -246,7 +246,11 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
                     float* dst = ob + b * obs + j;
 #pragma unroll
                     for (int r = 0; r < 16; ++r)
-                        if (r < nrow_live) dst[(int64_t)r * o_rs] = (r & 1) ? acc[r >> 1][t].y : acc[r >> 1][t].x;
+                        if (r < nrow_live) {
+                            const float v = (r & 1) ? acc[r >> 1][t].y : acc[r >> 1][t].x;
+                            float* q = dst + (int64_t)r * o_rs;
+                            *q = ACC ? *q + v : v;
+                        }
                 } else {
 #pragma unroll
                     for (int r = 0; r < 16; ++r) {
@@ -255,7 +259,8 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
                         const int m = mrow0 + r;
                         float* dst = (m < m_split) ? P.out0 + b * P.o_bs0 + (int64_t)m * o_rs + j
                                                    : P.out1 + b * P.o_bs1 + (int64_t)(m - m_split) * o_rs + j;
-                        *dst = (r & 1) ? acc[r >> 1][t].y : acc[r >> 1][t].x;
+                        const float v = (r & 1) ? acc[r >> 1][t].y : acc[r >> 1][t].x;
+                        *dst = ACC ? *dst + v : v;
                     }
                 }
             }
@@ -297,7 +302,7 @@ int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st
     int maxM = 0, maxK = 0;
     for (int i = 0; i < nargs; ++i) {
         const ProjArgs& g = args[i];
-        if (g.J != J || g.batch != batch || g.x_rs != args[0].x_rs) return CGTP_OK;
+        if (g.J != J || g.batch != batch || g.x_rs != args[0].x_rs || g.accumulate != args[0].accumulate) return CGTP_OK;
         if (g.K < 2 || (g.K & 1) || g.M < 1 || g.x_rs < J) return CGTP_OK;
         if (!al16(g.X) || (g.x_bs & 3)) return CGTP_OK;
         maxM = std::max(maxM, g.M);
@@ -390,15 +395,11 @@ int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st
     const int grid = begin;
 
     LaunchScope scope(kind, st);
-    if (wide) {
-        auto kern = proj_fast_kernel<2, 4>;
-        CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kern<<<grid, kPfThreads, smem, st>>>(a);
-    } else {
-        auto kern = proj_fast_kernel<4, 2>;
-        CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kern<<<grid, kPfThreads, smem, st>>>(a);
-    }
+    const bool acc = args[0].accumulate != 0;  // out += result (second pass of the parity-slot entry points)
+    void (*kern)(PfArgs) = wide ? (acc ? proj_fast_kernel<2, 4, true> : proj_fast_kernel<2, 4, false>)
+                                : (acc ? proj_fast_kernel<4, 2, true> : proj_fast_kernel<4, 2, false>);
+    CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<grid, kPfThreads, smem, st>>>(a);
     CGTP_CUDA_CHECK(cudaGetLastError());
     *handled = true;
     return CGTP_OK;

@@ -109,6 +109,7 @@ __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32])
 
 __device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
 
+template <bool ACC>
 __global__ void __launch_bounds__(TC_THREADS, 1) proj_tc_kernel(TcArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -302,14 +303,17 @@ __global__ void __launch_bounds__(TC_THREADS, 1) proj_tc_kernel(TcArgs a)
                         const int nq = (M - c0 < 32) ? (M - c0) : 32;
 #pragma unroll
                         for (int q = 0; q < 32; ++q) {
-                            if (q < nq) *p = __uint_as_float(v[q]);
+                            if (q < nq) *p = ACC ? *p + __uint_as_float(v[q]) : __uint_as_float(v[q]);
                             p += o_rs;
                         }
                     } else {
 #pragma unroll
                         for (int q = 0; q < 32; ++q) {
                             const int m = c0 + q;
-                            if (m < M) ((m < m_split) ? o0 : o1)[(int64_t)m * o_rs] = __uint_as_float(v[q]);
+                            if (m < M) {
+                                float* w = ((m < m_split) ? o0 : o1) + (int64_t)m * o_rs;
+                                *w = ACC ? *w + __uint_as_float(v[q]) : __uint_as_float(v[q]);
+                            }
                         }
                     }
                 }
@@ -358,7 +362,9 @@ int launch_proj_tc(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st, 
     const int64_t batch = args[0].batch;
     int maxM = 0, maxK = 0;
     for (int i = 0; i < nargs; ++i) {
-        if (args[i].J != J || args[i].batch != batch || args[i].M < 1 || args[i].K < 1) return CGTP_OK;
+        if (args[i].J != J || args[i].batch != batch || args[i].M < 1 || args[i].K < 1 ||
+            args[i].accumulate != args[0].accumulate)
+            return CGTP_OK;
         maxM = std::max(maxM, args[i].M);
         maxK = std::max(maxK, args[i].K);
     }
@@ -411,8 +417,9 @@ int launch_proj_tc(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st, 
     if (nargs == 1) a.p[1] = a.p[0];
 
     LaunchScope scope(kind, st);
-    CGTP_CUDA_CHECK(cudaFuncSetAttribute(proj_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    proj_tc_kernel<<<begin, TC_THREADS, smem, st>>>(a);
+    void (*kern)(TcArgs) = args[0].accumulate ? proj_tc_kernel<true> : proj_tc_kernel<false>;  // out += result
+    CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<begin, TC_THREADS, smem, st>>>(a);
     CGTP_CUDA_CHECK(cudaGetLastError());
     *handled = true;
     return CGTP_OK;

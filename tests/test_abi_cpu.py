@@ -49,6 +49,10 @@ def test_validation_codes_without_gpu():
     rc = L.cgtp_onsite(None, None, None, None, None, 2, 2, 4, 4, mask.ctypes.data_as(ctypes.c_void_p), None, i64(0),
                        None, sz(0), None)
     assert rc == 0  # empty batch is a no-op
+    rc = L.cgtp_onsite_parity(None, None, None, None, None, 2, 2, 4, 300, None, i64(1), None, sz(0), None)
+    assert rc == 2  # 4*C internal channels above the compiled limit
+    rc = L.cgtp_message_parity(None, None, None, None, None, None, 2, 5, 4, 4, None, i64(1), i64(0), None, sz(0), None)
+    assert rc == 1 and b"band" in L.cgtp_last_error()
     L.cgtp_onsite_workspace_bytes.restype = sz
     L.cgtp_onsite_workspace_bytes.argtypes = [ctypes.c_int] * 4 + [i64]
     assert L.cgtp_onsite_workspace_bytes(6, 6, 64, 64, 4096) >= 4096 * 64 * (2 * 52 + 52) * 4

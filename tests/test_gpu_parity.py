@@ -395,3 +395,93 @@ def test_message_tensor_core_math_mode(fp32_mode_after):
     cg.cgtp_set_math_mode(cg.MATH_3XTF32)
     e3 = sector_err(run_message(m, check=True), ref)
     assert max(e3) < TOL, e3
+
+
+# ------------------------------------------------------------- parity-labelled inputs
+def run_onsite_parity(q):
+    out = cg.cgtp_onsite_parity(_cuda(q.A), _cuda(q.B), _cuda(q.W_a), _cuda(q.W_b), _cuda(q.W_out), q.lmax,
+                                q.lmax_out, q.N, q.C)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def run_message_parity(m, **kw):
+    out = cg.cgtp_message_parity(_cuda(m.node_feats), _cuda(m.edge_index), _cuda(m.edge_vec), _cuda(m.edge_radial),
+                                 _cuda(m.W_node), _cuda(m.W_out), m.lmax, m.lmax_out, m.N, m.C, **kw)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+@pytest.mark.parametrize("lmax,lmax_out,N,C,batch", [
+    (0, 0, 2, 2, 5),
+    (1, 2, 3, 2, 37),     # odd N * L2: slot blocks not 16-byte aligned -> generic projection kernel
+    (2, 2, 8, 8, 64),     # configs[0] shape with both slots
+    (3, 5, 4, 3, 33),
+    (6, 6, 16, 8, 300),   # fast core + fast projections, several tiles and a ragged tail
+    (10, 10, 4, 2, 9),
+])
+def test_onsite_parity_slots(lmax, lmax_out, N, C, batch):
+    """cgtp_onsite_parity (PAPER.md VII C e :469) against the term-by-term oracle, 16 runs."""
+    q = synthetic.make_onsite_parity(lmax, lmax_out, N, C, batch, seed=400 + lmax)
+    got = run_onsite_parity(q)
+    ref = orc.onsite_parity(q.A, q.B, q.W_a, q.W_b, q.W_out, lmax, lmax_out)
+    e = sector_err(got, ref)
+    assert max(e) < TOL, e
+    assert np.array_equal(got, run_onsite_parity(q))  # bitwise reproducible
+
+
+def test_onsite_parity_reduces_to_natural_call():
+    """Slot 1 of both inputs empty: sector 0 / 1 at (-1)^l = sigma equal cgtp_onsite with the weights of the runs
+    (alpha, 0, 0, tau) / (beta, 0, 0, tau) -- the two entry points agree to rounding."""
+    lmax, N, C, batch = 4, 8, 4, 50
+    q = synthetic.make_onsite_parity(lmax, lmax, N, C, batch, seed=77)
+    q.A[:, 1] = 0
+    q.B[:, 1] = 0
+    got = run_onsite_parity(q)
+    lv = np.concatenate([np.full(2 * l + 1, l) for l in range(lmax + 1)])
+    for tau in (0, 1):
+        Wa = np.concatenate([q.W_a[tau], q.W_a[8 + tau]])
+        Wb = np.concatenate([q.W_b[tau], q.W_b[8 + tau]])
+        Wo = np.concatenate([q.W_out[tau], q.W_out[8 + tau]], axis=1)
+        nat = cg.cgtp_onsite(_cuda(q.A[:, 0]), _cuda(q.B[:, 0]), _cuda(Wa), _cuda(Wb), _cuda(Wo), lmax, lmax, N, 2 * C,
+                             [0] * C + [1] * C).cpu().numpy()
+        sel = (lv % 2) == tau
+        for s in (0, 1):
+            d = np.abs(got[:, s][:, :, sel] - nat[:, s][:, :, sel]).max()
+            assert d <= 2e-6 * np.abs(nat[:, s]).max(), (tau, s, d)
+
+
+@pytest.mark.parametrize("lmax,lmax_out,N,C,nodes", [
+    (0, 0, 2, 2, 5),
+    (2, 2, 3, 3, 17),
+    (3, 4, 4, 2, 12),
+    (4, 4, 8, 8, 40),
+    (8, 8, 4, 5, 10),
+])
+def test_message_parity_slots(lmax, lmax_out, N, C, nodes):
+    """cgtp_message_parity (PAPER.md VII C a-c) against the term-by-term oracle, 8 runs, ragged graphs."""
+    rng = np.random.default_rng(500 + lmax)
+    deg = rng.integers(0, 12, nodes)
+    deg[0] = 0
+    deg[-1] = 35
+    m = synthetic.make_message_parity(lmax, lmax_out, N, C, nodes, deg, seed=500 + lmax)
+    got = run_message_parity(m, check=True)
+    ref = orc.message_parity(m.node_feats, m.edge_index, m.edge_vec, m.edge_radial, m.W_node, m.W_out, lmax, lmax_out)
+    e = sector_err(got, ref)
+    assert max(e) < TOL, e
+    assert np.abs(got[deg == 0]).max() == 0.0
+    assert np.array_equal(got, run_message_parity(m))
+
+
+def test_message_parity_inversion_on_gpu():
+    """Parity labels on the device path: slot s at degree l carries (-1)^(s+l) (Table I PAPER.md:86-:93)."""
+    lmax, N, C, nodes = 5, 8, 4, 20
+    m = synthetic.make_message_parity(lmax, lmax, N, C, nodes, 6, seed=91)
+    base = run_message_parity(m)
+    sign = np.concatenate([np.full(2 * l + 1, (-1.0) ** l) for l in range(lmax + 1)]).astype(np.float32)
+    m.node_feats[:, 0] *= sign
+    m.node_feats[:, 1] *= -sign
+    m.edge_vec = -m.edge_vec
+    inv = run_message_parity(m)
+    assert np.abs(inv[:, 0] - base[:, 0] * sign).max() < 1e-5 * np.abs(base[:, 0]).max()
+    assert np.abs(inv[:, 1] + base[:, 1] * sign).max() < 1e-5 * np.abs(base[:, 1]).max()
