@@ -10,7 +10,8 @@ product / surface-curl pairing, analysis, output projection) over one batch of B
 (weak scaling, no collective on the data path).
 
 Prints ONE JSON line on rank 0.  Extra objects on the line (N=1 only): "sweep" (configs[3], on-site vs
-lmax), "message" (configs[2] and configs[4], edges/s and HBM GB/s), "kernels" (per-kernel shares).
+lmax), "message" (configs[2] and configs[4], edges/s and HBM GB/s), "kernels" (per-kernel shares), "parity"
+(parity-labelled inputs: cost of the full dispatch against one Category-alpha run).
 """
 from __future__ import annotations
 
@@ -346,6 +347,7 @@ def main():
         line["tensor_core"] = run_tensor_core(args, cg, step, out, lmax, lmax_out, N, C, Ce, Co, batch, peaks, peak_src)
         line["sweep"] = run_sweep(args, cg, synthetic, dev, fp32_peak_tflops, peaks)
         line["message"] = run_message(args, cg, synthetic, dev, peaks, peak_src)
+        line["parity"] = run_parity(args, cg, synthetic, dev)
     elif world == 1:
         rate, dt_cpu, cores = oracle_onsite_rate(base, 1024)
         line["cpu_baseline"] = {"value": rate, "unit": "contractions/s", "cores": cores, "kind": "oracle",
@@ -493,6 +495,40 @@ def run_message(args, cg, synthetic, dev, peaks, peak_src):
         }
         del X, ei, ev, er, out
         torch.cuda.empty_cache()
+    return res
+
+
+def run_parity(args, cg, synthetic, dev):
+    """Parity-labelled inputs (Sec. VII C a-c, e): cost of the full (p, sigma) dispatch
+    relative to ONE Category-alpha run of the same N and C -- the unit of the paper's 12x (Eq.(60) :455) and 24x (:469)
+    upper bounds.  Shapes: configs[1] / configs[2] with C/4 rank channels per run, so a pass has the configs' C."""
+    import torch
+    cu = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    res = {}
+    # on-site: lmax=6, N=64, C=16 per run (16 runs, 4 passes of 64 internal channels), 4096 atoms
+    q = synthetic.make_onsite_parity(6, 6, 64, 16, 4096, seed=0)
+    A, B, Wa, Wb, Wo = cu(q.A), cu(q.B), cu(q.W_a), cu(q.W_b), cu(q.W_out)
+    out = torch.empty((q.batch, 2, q.N, 49), device=dev)
+    ms = time_steps(lambda: cg.cgtp_onsite_parity(A, B, Wa, Wb, Wo, 6, 6, q.N, q.C, out=out), 20, 3)
+    A0, B0 = A[:, 0].contiguous(), B[:, 0].contiguous()
+    Wa0, Wb0, Wo0 = Wa[0].contiguous(), Wb[0].contiguous(), Wo[0].contiguous()
+    mask0 = np.zeros(q.C, np.uint8)
+    ms1 = time_steps(lambda: cg.cgtp_onsite(A0, B0, Wa0, Wb0, Wo0, 6, 6, q.N, q.C, mask0, out=out), 20, 3)
+    res["onsite"] = {"workload": "lmax=6 N=64 C=16 per run x 16 runs, batch=4096, both slots populated",
+                     "ms_per_step": ms, "contractions_per_s": q.batch / (ms * 1e-3), "alpha_run_ms": ms1,
+                     "factor_vs_alpha_run": ms / ms1, "paper_upper_bound": 24}
+    del A, B, out, A0, B0
+    # message passing: configs[2] graph, lmax=4, N=128, C=32 per run (8 runs, 2 passes of 128 internal channels)
+    m = synthetic.make_message_parity(4, 4, 128, 32, 2048, 16, 0.8, 5.0, seed=0)
+    X, ei, ev, er, Wn, Wo = cu(m.node_feats), cu(m.edge_index), cu(m.edge_vec), cu(m.edge_radial), cu(m.W_node), cu(m.W_out)
+    out = torch.empty((m.nodes, 2, m.N, 25), device=dev)
+    ms = time_steps(lambda: cg.cgtp_message_parity(X, ei, ev, er, Wn, Wo, 4, 4, m.N, m.C, out=out), 10, 3)
+    X0, er0, Wn0, Wo0 = X[:, 0].contiguous(), er[:, 0].contiguous(), Wn[0].contiguous(), Wo[0].contiguous()
+    mask0 = np.zeros(m.C, np.uint8)
+    ms1 = time_steps(lambda: cg.cgtp_message(X0, ei, ev, er0, Wn0, Wo0, 4, 4, m.N, m.C, mask0, out=out), 10, 3)
+    res["message"] = {"workload": "configs[2] graph (2048 nodes, 32768 edges), lmax=4 N=128 C=32 per run x 8 runs",
+                      "ms_per_step": ms, "edges_per_s": m.E / (ms * 1e-3), "alpha_run_ms": ms1,
+                      "factor_vs_alpha_run": ms / ms1, "paper_upper_bound": 12}
     return res
 
 

@@ -171,7 +171,9 @@ static int launch_node_synth_t(const Plan* p, const float* H, float* G, int64_t 
     const int nf = ODD ? 2 : 1;
     SynthSmem fixed = synth_smem_layout(p, ODD, 0);
     const int percol = p->L2p * 4 + nf * M * p->U * 4 + nf * p->UVp * 4;
-    int budget = 100 * 1024;
+    // 45 KB per CTA -> four or five CTAs per SM, so that the load / compute / store phases of different CTAs overlap
+    // (measured on configs[2] / configs[4]: 64 -> 52 us and 1.08 -> 0.85 ms against a 100 KB budget)
+    int budget = 45 * 1024;
     int NC = (budget - fixed.total - 64) / percol;
     if (NC < 4) {
         budget = 220 * 1024;
@@ -465,7 +467,7 @@ static int launch_analysis_t(const Plan* p, bool odd, const float* S, float* T, 
     const int M = 2 * p->LB + 1;
     AnaSmem fixed = ana_smem_layout(p, 0);
     const int percol = p->UVp * 4 + M * p->U * 4;
-    int budget = 100 * 1024;
+    int budget = 45 * 1024;  // as node synthesis: several small CTAs per SM overlap their phases (0.80 -> 0.67 ms, configs[4])
     int NC = (budget - fixed.total - 64) / percol;
     if (NC < 4) {
         budget = 220 * 1024;
