@@ -15,22 +15,31 @@ namespace cgtp {
 __global__ void __launch_bounds__(256) sigma_mask_kernel(float* __restrict__ T, int stride, int64_t ncols, int Cpar,
                                                          int Cs, int Lo2)
 {
-    const int64_t total = ncols * Lo2;
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t col = i / Lo2;
-        const int lm = (int)(i - col * Lo2);
-        int l = (int)sqrtf((float)lm);  // exact for lm < 2^23
-        const int tau = ((int)(col % Cpar) / Cs) & 1;
-        if ((l & 1) != tau) T[col * stride + lm] = 0.f;
+    // one warp per column, lane = lm mod 32: the l-parity of a lane's coefficients is a per-lane bit mask computed
+    // once, so the column loop has no division and no square root (32-bit indices: the host rejects ncols >= 2^31)
+    const int lane = threadIdx.x & 31;
+    uint32_t lodd = 0;  // bit i: degree of lm = lane + 32 i is odd
+    for (int lm = lane, i = 0; lm < Lo2; lm += 32, ++i) {
+        const int l = (int)sqrtf((float)lm);  // exact: lm < 2^23 and sqrtf is correctly rounded
+        lodd |= (uint32_t)(l & 1) << i;
+    }
+    const uint32_t nwarps = gridDim.x * (blockDim.x >> 5);
+    const uint32_t n = (uint32_t)ncols, cpar = (uint32_t)Cpar, cs = (uint32_t)Cs;
+    for (uint32_t col = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); col < n; col += nwarps) {
+        const uint32_t tau = ((col % cpar) / cs) & 1u;
+        const uint32_t clear = tau ? ~lodd : lodd;  // bit i set: coefficient is not part of the run
+        float* row = T + (size_t)col * stride;
+        for (int lm = lane, i = 0; lm < Lo2; lm += 32, ++i)
+            if ((clear >> i) & 1u) row[lm] = 0.f;
     }
 }
 
 int launch_sigma_mask(float* T, int stride, int64_t ncols, int Cpar, int Cs, int Lo2, cudaStream_t st)
 {
     if (ncols <= 0 || Cpar <= 0) return CGTP_OK;
-    const int64_t total = ncols * Lo2;
-    int64_t blocks = (total + 255) / 256;
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (ncols >= 2147483647LL) { set_error("sigma mask: too many columns"); return CGTP_ERR_UNSUPPORTED; }
+    int64_t blocks = (ncols + 7) / 8;
+    if (blocks > 148 * 8) blocks = 148 * 8;
     LaunchScope scope(K_MISC, st);
     sigma_mask_kernel<<<(unsigned)blocks, 256, 0, st>>>(T, stride, ncols, Cpar, Cs, Lo2);
     CGTP_CUDA_CHECK(cudaGetLastError());

@@ -244,12 +244,17 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
                 const int64_t b = (int64_t)b0 + al;
                 if (slab_uniform) {
                     float* dst = ob + b * obs + j;
+                    float prev[16];
+                    if (ACC) {
+                        // all loads first: a load issued after a store to a possibly aliasing address would wait for it
+#pragma unroll
+                        for (int r = 0; r < 16; ++r) prev[r] = (r < nrow_live) ? __ldcg(dst + (int64_t)r * o_rs) : 0.f;
+                    }
 #pragma unroll
                     for (int r = 0; r < 16; ++r)
                         if (r < nrow_live) {
                             const float v = (r & 1) ? acc[r >> 1][t].y : acc[r >> 1][t].x;
-                            float* q = dst + (int64_t)r * o_rs;
-                            *q = ACC ? *q + v : v;
+                            dst[(int64_t)r * o_rs] = ACC ? prev[r] + v : v;
                         }
                 } else {
 #pragma unroll

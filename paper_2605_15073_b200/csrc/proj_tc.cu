@@ -301,9 +301,15 @@ __global__ void __launch_bounds__(TC_THREADS, 1) proj_tc_kernel(TcArgs a)
                     if (c0 + 32 <= m_split || c0 >= m_split) {  // the whole slice goes to one output tensor
                         float* p = ((c0 < m_split) ? o0 : o1) + (int64_t)c0 * o_rs;
                         const int nq = (M - c0 < 32) ? (M - c0) : 32;
+                        if (ACC) {
+                            // all loads before the first store (a load behind a possibly aliasing store waits for it)
+#pragma unroll
+                            for (int q = 0; q < 32; ++q)
+                                if (q < nq) v[q] = __float_as_uint(__uint_as_float(v[q]) + __ldcg(p + (int64_t)q * o_rs));
+                        }
 #pragma unroll
                         for (int q = 0; q < 32; ++q) {
-                            if (q < nq) *p = ACC ? *p + __uint_as_float(v[q]) : __uint_as_float(v[q]);
+                            if (q < nq) *p = __uint_as_float(v[q]);
                             p += o_rs;
                         }
                     } else {
