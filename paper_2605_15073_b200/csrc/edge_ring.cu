@@ -19,7 +19,10 @@ namespace cgtp {
 
 constexpr int ER_CONS = 512;            // consumer threads
 constexpr int ER_NT = ER_CONS + 32;     // + producer warp
-constexpr int ER_NA = 2;                // float4 accumulators per thread per sub-block
+// float4 accumulators per thread per sub-block (template parameter NA): 2 for the odd kernel (two fields per channel),
+// 4 for the even one, so that a ring stage carries the same ~31 KB and a thread has the same number of independent
+// load -> multiply -> accumulate chains per mbarrier hand-over in both (with 2 the even kernel was latency-bound at
+// 5.6 TB/s against 7.1 TB/s for the odd one)
 constexpr int ER_MAXST = 16;            // ring stages (upper bound)
 constexpr int ER_LMAX = 24;             // recurrence coefficient table length
 
@@ -57,7 +60,7 @@ __device__ __forceinline__ float2 hi2(const float4& v) { return make_float2(v.z,
 // Thread <-> accumulator mapping (QP <= 512 float4 quads per grid field, true for every band limit the
 // library compiles): thread = (channel group cg, quad q0), accumulator x of a sub-block = channel
 // x*G + cg at quad q0, so the edge field at q0 stays in registers for every channel of the edge.
-template <bool ODD, int NSBT>
+template <bool ODD, int NSBT, int NA>
 __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
 {
     constexpr int NF = ODD ? 2 : 1;
@@ -129,14 +132,14 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
 
     // ================================= consumer warps =================================
     constexpr int QT = 1;
-    int chl[ER_NA], qd[QT];
+    int chl[NA], qd[QT];
     bool qok[QT];
     {
         const int cg = tid / QP;
         qd[0] = tid - cg * QP;
         qok[0] = cg < a.G_;
 #pragma unroll
-        for (int x = 0; x < ER_NA; ++x) chl[x] = x * a.G_ + cg;
+        for (int x = 0; x < NA; ++x) chl[x] = x * a.G_ + cg;
     }
     const float* geo = a.geo_smem ? geo_s : a.p.geo;
     const int lmax = a.p.lmax;
@@ -148,11 +151,11 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
         const int nsb = (ncb + cs - 1) / cs;
         const long long e_begin = graph_ok ? a.row_ptr[i] : 0, e_end = graph_ok ? a.row_ptr[i + 1] : 0;
 
-        float2 acc[NSBT][ER_NA][2];
+        float2 acc[NSBT][NA][2];
 #pragma unroll
         for (int sb = 0; sb < NSBT; ++sb)
 #pragma unroll
-            for (int x = 0; x < ER_NA; ++x) acc[sb][x][0] = acc[sb][x][1] = make_float2(0.f, 0.f);
+            for (int x = 0; x < NA; ++x) acc[sb][x][0] = acc[sb][x][1] = make_float2(0.f, 0.f);
 
         for (long long e0 = e_begin; e0 < e_end; e0 += a.EC) {
             const int ne = (int)((e_end - e0 < a.EC) ? (e_end - e0) : a.EC);
@@ -217,7 +220,7 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
                         const float4* g4 = reinterpret_cast<const float4*>(ring + (size_t)slot * a.stage_bytes);
                         mbar_wait(&full[slot], phase);
 #pragma unroll
-                        for (int x = 0; x < ER_NA; ++x) {
+                        for (int x = 0; x < NA; ++x) {
                             constexpr int j = 0;
                             if (chl[x] < ncs && qok[j]) {
                                 const float r = rrow[sb * cs + chl[x]];
@@ -255,7 +258,7 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
                 const int ncs = (ncb - sb * cs < cs) ? (ncb - sb * cs) : cs;
                 float4* sdst = reinterpret_cast<float4*>(a.S + ((size_t)i * Cpar + kc0 + sb * cs) * UVp);
 #pragma unroll
-                for (int x = 0; x < ER_NA; ++x) {
+                for (int x = 0; x < NA; ++x) {
                     constexpr int j = 0;
                     if (chl[x] < ncs && qok[j])
                         sdst[chl[x] * QP + qd[j]] =
@@ -281,10 +284,10 @@ static int er_num_sms()
     return n;
 }
 
-template <bool ODD, int NSBT>
+template <bool ODD, int NSBT, int NA>
 static int launch_ring_t(const EdgeRingArgs& a, size_t smem, int grid, cudaStream_t st)
 {
-    auto kern = edge_ring_kernel<ODD, NSBT>;
+    auto kern = edge_ring_kernel<ODD, NSBT, NA>;
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<grid, ER_NT, smem, st>>>(a);
     CGTP_CUDA_CHECK(cudaGetLastError());
@@ -304,8 +307,12 @@ int launch_edge_ring(const Plan* p, bool odd, const float* G, const int64_t* row
     const int QP = p->UVp / 4;
     if (QP > ER_CONS) return CGTP_OK;  // cannot happen for band limits <= 20 (QP <= 473)
     const int G_ = ER_CONS / QP;
-    const int cs_max = ER_NA * G_;
-    constexpr int NSB_MAX = 6;
+    // even kernel: 4 accumulators per thread and sub-block; 6 when that turns the whole channel set into one
+    // sub-block (one ring stage per edge: configs[2] all-even 225 -> 192 us), measured slower otherwise
+    int NA = odd ? 2 : 4;
+    if (!odd && Cpar > 4 * G_ && Cpar <= 6 * G_ && (size_t)6 * G_ * p->UVp * 4 * 3 <= 150 * 1024) NA = 6;
+    const int cs_max = NA * G_;
+    const int NSB_MAX = 12 / NA;  // NA * NSBT <= 12 float4 accumulators per thread
     // channel blocks: as few as possible with at most NSB_MAX sub-blocks each
     const int cb_max = cs_max * NSB_MAX;
     const int nblk = (Cpar + cb_max - 1) / cb_max;
@@ -361,16 +368,25 @@ int launch_edge_ring(const Plan* p, bool odd, const float* G, const int64_t* row
 
     LaunchScope scope(odd ? K_EDGE_ODD : K_EDGE_EVEN, st);
     int rc = CGTP_OK;
-#define CGTP_RING(N) \
-    rc = odd ? launch_ring_t<true, N>(a, smem, grid, st) : launch_ring_t<false, N>(a, smem, grid, st)
-    switch (nsbt) {
-    case 1: CGTP_RING(1); break;
-    case 2: CGTP_RING(2); break;
-    case 3: CGTP_RING(3); break;
-    case 4: CGTP_RING(4); break;
-    default: CGTP_RING(6); break;
+    if (odd) {
+        switch (nsbt) {
+        case 1: rc = launch_ring_t<true, 1, 2>(a, smem, grid, st); break;
+        case 2: rc = launch_ring_t<true, 2, 2>(a, smem, grid, st); break;
+        case 3: rc = launch_ring_t<true, 3, 2>(a, smem, grid, st); break;
+        case 4: rc = launch_ring_t<true, 4, 2>(a, smem, grid, st); break;
+        default: rc = launch_ring_t<true, 6, 2>(a, smem, grid, st); break;
+        }
+    } else {
+        if (NA == 6) {
+            rc = launch_ring_t<false, 1, 6>(a, smem, grid, st);
+        } else {
+            switch (nsbt) {
+            case 1: rc = launch_ring_t<false, 1, 4>(a, smem, grid, st); break;
+            case 2: rc = launch_ring_t<false, 2, 4>(a, smem, grid, st); break;
+            default: rc = launch_ring_t<false, 3, 4>(a, smem, grid, st); break;
+            }
+        }
     }
-#undef CGTP_RING
     if (rc == CGTP_OK) *handled = true;
     return rc;
 }
