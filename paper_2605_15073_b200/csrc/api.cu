@@ -59,8 +59,8 @@ static size_t message_ws_bytes(int lmax, int lmax_out, int C, int Co, int64_t n_
     const size_t L2p = round_up((lmax + 1) * (lmax + 1), 4), Lo2p = round_up((lmax_out + 1) * (lmax_out + 1), 4);
     const int U = (2 * lmax + lmax_out + 2) / 2, V = 2 * lmax + lmax_out + 1;
     const size_t UVp = round_up(U * V, 4);
-    // H, G for the senders; S, T, row_ptr for the receivers
-    size_t fl = (size_t)n_send * C * L2p + (size_t)n_send * (C + Co) * UVp + (size_t)n_recv * C * (UVp + Lo2p);
+    // H, G (value grid, both parities) for the senders; S (two pooled grids per odd channel), T, row_ptr for the receivers
+    size_t fl = (size_t)n_send * C * (L2p + UVp) + (size_t)n_recv * ((C + Co) * UVp + (size_t)C * Lo2p);
     return 256 + fl * sizeof(float) + (size_t)(n_recv + 1) * sizeof(int64_t) + 12 * 256;
 }
 
@@ -231,9 +231,9 @@ static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_
     float* H_e = cv.take<float>((size_t)n_send * Ce * p->L2p);
     float* H_o = cv.take<float>((size_t)n_send * Co * p->L2p);
     float* G_e = cv.take<float>((size_t)n_send * Ce * p->UVp);
-    float* G_o = cv.take<float>((size_t)n_send * Co * 2 * p->UVp);
+    float* G_o = cv.take<float>((size_t)n_send * Co * p->UVp);
     float* S_e = cv.take<float>((size_t)nodes * Ce * p->UVp);
-    float* S_o = cv.take<float>((size_t)nodes * Co * p->UVp);
+    float* S_o = cv.take<float>((size_t)nodes * Co * 2 * p->UVp);
     float* T_e = cv.take<float>((size_t)nodes * Ce * p->Lo2p);
     float* T_o = cv.take<float>((size_t)nodes * Co * p->Lo2p);
 
@@ -268,7 +268,7 @@ static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_
     rc = launch_proj(&a, 1, K_PROJ_IN, st);
     if (rc) return rc;
 
-    // M2
+    // M2 (value fields for both parities: the odd channels take their derivatives on the edge side and in M5)
     rc = launch_node_synth(p, false, H_e, G_e, n_send * Ce, st);
     if (rc) return rc;
     rc = launch_node_synth(p, true, H_o, G_o, n_send * Co, st);

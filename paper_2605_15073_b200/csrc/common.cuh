@@ -50,6 +50,8 @@ struct Plan {
     const float* DT;  // d/dtheta P~_l^m(cos theta) at theta_u (theta-form of d_x p_ulm, :445)
     const float* ST;  // m P~_l^m(x_u) / sin(theta_u)         ((1/sin theta) d_phi of Eq.(11), :107)
     const float* WP;  // w_u P~_l^m(x_u), equator row halved  (Eq.(40), :342)
+    const float* WD;  // w_u d/dtheta P~_l^m, equator row halved      (analysis of the by-parts curl pairing, M5 odd)
+    const float* WS;  // w_u m P~_l^m / sin(theta), equator row halved
     // Fourier tables (real form, Eq.(C2) :668), [Vh][QSTR]:
     const float* QC;  // QC[v'][0] = 1, QC[v'][m] = sqrt2 cos(m phi_v')
     const float* QS;  // QS[v'][m] = sqrt2 sin(m phi_v'), zero for m = 0 and for self-mirrored v'
@@ -183,9 +185,12 @@ int launch_onsite_fast(const Plan* p, bool odd, const float* Ha, const float* Hb
 // M0: row_ptr over `nodes` receivers; senders are validated against n_send
 int launch_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int64_t n_send, int64_t* row_ptr,
                     int32_t* status, cudaStream_t st);
-// M2: grid fields of the projected node features.  even: G[col][UVp]; odd: G[col][2][UVp] (d_theta, (1/sin)d_phi)
+// M2: value grid field of the projected node features, G[col][UVp], for the channels of either parity (`odd` only
+// labels the launch for the profiler: the odd channels pair the edge's derivative fields with the sender's VALUE
+// field and move the derivatives onto Y_lm in the analysis).
 int launch_node_synth(const Plan* p, bool odd, const float* H, float* G, int64_t ncols, cudaStream_t st);
-// M3+M4: S[i][kc][UVp] = sum_e radial * edge-field (x) sender grid, channels of one parity.
+// M3+M4: channels of one parity.  even: S[i][kc][UVp] = sum_e R~ K_e G[send(e)];
+// odd: S[i][kc][2][UVp] = sum_e R~ (d_theta K_e, -(1/sin) d_phi K_e) G[send(e)].
 int launch_edge(const Plan* p, bool odd, const float* G, const int64_t* row_ptr, const int64_t* edge_index,
                 int64_t E, const float* edge_vec, const float* edge_radial, const int* perm_par, int Cpar, int C,
                 float* S, int64_t nodes, const int32_t* status, cudaStream_t st);
@@ -193,7 +198,7 @@ int launch_edge(const Plan* p, bool odd, const float* G, const int64_t* row_ptr,
 int launch_edge_ring(const Plan* p, bool odd, const float* G, const int64_t* row_ptr, const int64_t* edge_index,
                      int64_t E, const float* edge_vec, const float* edge_radial, const int* perm_par, int Cpar, int C,
                      float* S, int64_t nodes, const int32_t* status, cudaStream_t st, bool* handled);
-// M5: T[col][Lo2p] = analysis of S[col][UVp]
+// M5: T[col][Lo2p] = analysis of S[col][UVp] (even) or of the field pair S[col][2][UVp] against {., Y_lm} (odd)
 int launch_analysis(const Plan* p, bool odd, const float* S, float* T, int64_t ncols, cudaStream_t st);
 
 }  // namespace cgtp

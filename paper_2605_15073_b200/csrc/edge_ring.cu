@@ -25,6 +25,7 @@ constexpr int ER_NT = ER_CONS + 32;     // + producer warp
 // 5.6 TB/s against 7.1 TB/s for the odd one)
 constexpr int ER_MAXST = 16;            // ring stages (upper bound)
 constexpr int ER_LMAX = 24;             // recurrence coefficient table length
+constexpr int ER_HDR = 256 + ER_LMAX * 16 + 8 * 16;  // barriers, coefficient table, edge unit vectors
 
 struct EdgeRingArgs {
     Plan p;
@@ -67,9 +68,10 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);   // [ER_MAXST]
     uint64_t* empty = full + ER_MAXST;                    // [ER_MAXST]
-    float* coef = reinterpret_cast<float*>(smem + 256);   // [3][ER_LMAX]: (2l-1)/l, (l-1)/l, (2l+1)/(4 pi)
-    float* geo_s = coef + 3 * ER_LMAX;
-    float* Kbuf = reinterpret_cast<float*>(smem + 256 + 3 * ER_LMAX * 4 + a.geo_bytes);  // [EC][NF][UVp]
+    float4* coef = reinterpret_cast<float4*>(smem + 256);  // [ER_LMAX]: (2l-1)/l, -(l-1)/l, (2l+1)/(4 pi), l
+    float4* Ebuf = coef + ER_LMAX;                         // [8]: unit vectors of the chunk's edges
+    float* geo_s = reinterpret_cast<float*>(Ebuf + 8);
+    float* Kbuf = reinterpret_cast<float*>(smem + ER_HDR + a.geo_bytes);  // [EC][NF][UVp]
     float* Rbuf = Kbuf + a.k_bytes / 4;                                                   // [EC][cb]
     unsigned char* ring = reinterpret_cast<unsigned char*>(Rbuf) + a.r_bytes;
 
@@ -86,9 +88,7 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
     }
     if (tid < ER_LMAX) {
         const float l = (float)(tid > 0 ? tid : 1);
-        coef[tid] = (2.f * l - 1.f) / l;
-        coef[ER_LMAX + tid] = (l - 1.f) / l;
-        coef[2 * ER_LMAX + tid] = (2.f * tid + 1.f) * 0.07957747154594767f;
+        coef[tid] = make_float4((2.f * l - 1.f) / l, -(l - 1.f) / l, (2.f * tid + 1.f) * 0.07957747154594767f, l);
     }
     if (a.geo_smem)
         for (int idx = tid; idx < a.geo_bytes / 4; idx += ER_NT) geo_s[idx] = a.p.geo[idx];
@@ -113,13 +113,13 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
                 for (int el = 0; el < n; ++el) {
                     const long long s = __shfl_sync(0xffffffffu, s_mine, el);
                     if (lane == 0) {
-                        const float* src = a.G + ((size_t)s * Cpar + kc0) * NF * UVp;
+                        const float* src = a.G + ((size_t)s * Cpar + kc0) * UVp;
                         for (int sb = 0; sb < nsb; ++sb) {
                             const int ncs = (ncb - sb * cs < cs) ? (ncb - sb * cs) : cs;
-                            const uint32_t bytes = (uint32_t)ncs * NF * UVp * 4u;
+                            const uint32_t bytes = (uint32_t)ncs * UVp * 4u;
                             mbar_wait(&empty[slot], phase ^ 1u);
                             mbar_arrive_expect_tx(&full[slot], bytes);
-                            tma_load_1d(ring + (size_t)slot * a.stage_bytes, src + (size_t)sb * cs * NF * UVp, bytes,
+                            tma_load_1d(ring + (size_t)slot * a.stage_bytes, src + (size_t)sb * cs * UVp, bytes,
                                         &full[slot]);
                             if (++slot == NST) { slot = 0; phase ^= 1u; }
                         }
@@ -151,51 +151,91 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
         const int nsb = (ncb + cs - 1) / cs;
         const long long e_begin = graph_ok ? a.row_ptr[i] : 0, e_end = graph_ok ? a.row_ptr[i + 1] : 0;
 
-        float2 acc[NSBT][NA][2];
+        float2 acc[NSBT][NA][NF][2];
 #pragma unroll
         for (int sb = 0; sb < NSBT; ++sb)
 #pragma unroll
-            for (int x = 0; x < NA; ++x) acc[sb][x][0] = acc[sb][x][1] = make_float2(0.f, 0.f);
+            for (int x = 0; x < NA; ++x)
+#pragma unroll
+                for (int f = 0; f < NF; ++f) acc[sb][x][f][0] = acc[sb][x][f][1] = make_float2(0.f, 0.f);
+
+        // unit vectors of a chunk's edges (only the direction of edge_vec is used, R11)
+        auto load_edges = [&](long long e0, long long e_end_) {
+            const int n = (int)((e_end_ - e0 < a.EC) ? (e_end_ - e0) : a.EC);
+            if (tid < n) {
+                const long long e = e0 + tid;
+                const float ex = a.edge_vec[3 * e], ey = a.edge_vec[3 * e + 1], ez = a.edge_vec[3 * e + 2];
+                const float rn = rsqrtf(ex * ex + ey * ey + ez * ez);
+                Ebuf[tid] = make_float4(ex * rn, ey * rn, ez * rn, 0.f);
+            }
+        };
+        if (e_begin < e_end) {
+            load_edges(e_begin, e_end);
+            consumer_sync();
+        }
 
         for (long long e0 = e_begin; e0 < e_end; e0 += a.EC) {
             const int ne = (int)((e_end - e0 < a.EC) ? (e_end - e0) : a.EC);
             // ---- M3: edge fields of the chunk on the grid (Eq.(48),(50); addition theorem, R12):
-            // K(t) = sum_l (2l+1)/(4 pi) P_l(t), K'(t) likewise with P'_l = t P'_{l-1} + l P_{l-1}, t = r_e . Omega
-            for (int idx = tid; idx < ne * UVp; idx += ER_CONS) {
-                const int el = idx / UVp, q = idx - el * UVp;
-                const long long e = e0 + el;
-                float k0 = 0.f, k1 = 0.f;
-                if (q < a.p.UV) {
-                    float ex = a.edge_vec[3 * e], ey = a.edge_vec[3 * e + 1], ez = a.edge_vec[3 * e + 2];
-                    const float rn = rsqrtf(ex * ex + ey * ey + ez * ez);
-                    ex *= rn; ey *= rn; ez *= rn;
-                    const float t = ex * geo[q] + ey * geo[UVp + q] + ez * geo[2 * UVp + q];
-                    float pm = 1.f, pc = t, dc = 1.f;
-                    float ks = coef[2 * ER_LMAX], kd = 0.f;
-                    if (lmax >= 1) { ks = fmaf(coef[2 * ER_LMAX + 1], pc, ks); kd = coef[2 * ER_LMAX + 1]; }
-                    for (int l = 2; l <= lmax; ++l) {
-                        const float pn = fmaf(coef[l] * t, pc, -(coef[ER_LMAX + l] * pm));
-                        const float c = coef[2 * ER_LMAX + l];
-                        if (!ODD) {
-                            ks = fmaf(c, pn, ks);
-                        } else {
-                            const float dn = fmaf(t, dc, (float)l * pc);
-                            kd = fmaf(c, dn, kd);
-                            dc = dn;
+            // K(t) = sum_l (2l+1)/(4 pi) P_l(t), K'(t) likewise with P'_l = t P'_{l-1} + l P_{l-1}, t = r_e . Omega.
+            // Thread = grid point (geometry read once per chunk), two edges per pass in the halves of packed
+            // FP32 operations; ER_CONS / UVp thread sets share the edge pairs when the grid is small.
+            {
+                const int qs = (UVp <= ER_CONS) ? UVp : ER_CONS;
+                const int nset = (UVp <= ER_CONS) ? ER_CONS / UVp : 1;
+                const int set = tid / qs;
+                if (set < nset) {
+                    for (int q = tid - set * qs; q < UVp; q += qs) {
+                        const bool live = q < a.p.UV;
+                        const float gx = geo[q], gy = geo[UVp + q], gz = geo[2 * UVp + q];
+                        float tx = 0.f, ty = 0.f, tz = 0.f, fx = 0.f, fy = 0.f;
+                        if (ODD) {
+                            tx = geo[3 * UVp + q]; ty = geo[4 * UVp + q]; tz = geo[5 * UVp + q];
+                            fx = geo[6 * UVp + q]; fy = geo[7 * UVp + q];
                         }
-                        pm = pc; pc = pn;
-                    }
-                    if (!ODD) {
-                        k0 = ks;
-                    } else {
-                        const float dth = ex * geo[3 * UVp + q] + ey * geo[4 * UVp + q] + ez * geo[5 * UVp + q];
-                        const float dph = ex * geo[6 * UVp + q] + ey * geo[7 * UVp + q];
-                        k0 = kd * dth;
-                        k1 = -(kd * dph);  // stored negated: {E,I} = E_theta I_phi + (-E_phi) I_theta
+                        for (int el = 2 * set; el < ne; el += 2 * nset) {
+                            const int el1 = (el + 1 < ne) ? el + 1 : el;
+                            const float4 ea = Ebuf[el], eb = Ebuf[el1];
+                            const float2 t = make_float2(fmaf(ea.x, gx, fmaf(ea.y, gy, ea.z * gz)),
+                                                         fmaf(eb.x, gx, fmaf(eb.y, gy, eb.z * gz)));
+                            float2 pm = make_float2(1.f, 1.f), pc = t, dc = make_float2(1.f, 1.f);
+                            const float c0 = coef[0].z, c1 = coef[1].z;
+                            float2 ks = make_float2(c0, c0), kd = make_float2(0.f, 0.f);
+                            if (lmax >= 1) {
+                                ks = __ffma2_rn(make_float2(c1, c1), pc, ks);
+                                kd = make_float2(c1, c1);
+                            }
+                            for (int l = 2; l <= lmax; ++l) {
+                                const float4 c = coef[l];
+                                const float2 pn = __ffma2_rn(make_float2(c.x, c.x), __fmul2_rn(t, pc),
+                                                             __fmul2_rn(make_float2(c.y, c.y), pm));
+                                if (!ODD) {
+                                    ks = __ffma2_rn(make_float2(c.z, c.z), pn, ks);
+                                } else {
+                                    const float2 dn = __ffma2_rn(t, dc, __fmul2_rn(make_float2(c.w, c.w), pc));
+                                    kd = __ffma2_rn(make_float2(c.z, c.z), dn, kd);
+                                    dc = dn;
+                                }
+                                pm = pc; pc = pn;
+                            }
+                            float2 k0 = ks, k1 = make_float2(0.f, 0.f);
+                            if (ODD) {
+                                const float2 dth = make_float2(fmaf(ea.x, tx, fmaf(ea.y, ty, ea.z * tz)),
+                                                               fmaf(eb.x, tx, fmaf(eb.y, ty, eb.z * tz)));
+                                const float2 dph = make_float2(fmaf(ea.x, fx, ea.y * fy), fmaf(eb.x, fx, eb.y * fy));
+                                k0 = __fmul2_rn(kd, dth);
+                                k1 = __fmul2_rn(kd, make_float2(-dph.x, -dph.y));  // stored negated (X1 = -sum R~ E_phi I)
+                            }
+                            if (!live) k0 = k1 = make_float2(0.f, 0.f);
+                            Kbuf[((size_t)el * NF) * UVp + q] = k0.x;
+                            if (ODD) Kbuf[((size_t)el * NF + 1) * UVp + q] = k1.x;
+                            if (el1 != el) {
+                                Kbuf[((size_t)el1 * NF) * UVp + q] = k0.y;
+                                if (ODD) Kbuf[((size_t)el1 * NF + 1) * UVp + q] = k1.y;
+                            }
+                        }
                     }
                 }
-                Kbuf[((size_t)el * NF) * UVp + q] = k0;
-                if (ODD) Kbuf[((size_t)el * NF + 1) * UVp + q] = k1;
             }
             for (int idx = tid; idx < ne * ncb; idx += ER_CONS) {
                 const int el = idx / ncb, k = idx - el * ncb;
@@ -224,21 +264,22 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
                             constexpr int j = 0;
                             if (chl[x] < ncs && qok[j]) {
                                 const float r = rrow[sb * cs + chl[x]];
+                                const float4 g = g4[chl[x] * QP + qd[j]];
                                 if (!ODD) {
-                                    const float4 g = g4[chl[x] * QP + qd[j]];
                                     const float2 p0 = __fmul2_rn(lo2(kr[j][0]), lo2(g));
                                     const float2 p1 = __fmul2_rn(hi2(kr[j][0]), hi2(g));
-                                    acc[sb][x][0] = __ffma2_rn(p0, make_float2(r, r), acc[sb][x][0]);
-                                    acc[sb][x][1] = __ffma2_rn(p1, make_float2(r, r), acc[sb][x][1]);
+                                    acc[sb][x][0][0] = __ffma2_rn(p0, make_float2(r, r), acc[sb][x][0][0]);
+                                    acc[sb][x][0][1] = __ffma2_rn(p1, make_float2(r, r), acc[sb][x][0][1]);
                                 } else {
-                                    // {E, I} = E_theta I_phi - E_phi I_theta   (edge = factor 1, Eq.(57))
-                                    const float4 g0 = g4[chl[x] * 2 * QP + qd[j]], g1 = g4[chl[x] * 2 * QP + QP + qd[j]];
-                                    float2 p0 = __fmul2_rn(lo2(kr[j][0]), lo2(g1));
-                                    float2 p1 = __fmul2_rn(hi2(kr[j][0]), hi2(g1));
-                                    p0 = __ffma2_rn(lo2(kr[j][NF - 1]), lo2(g0), p0);
-                                    p1 = __ffma2_rn(hi2(kr[j][NF - 1]), hi2(g0), p1);
-                                    acc[sb][x][0] = __ffma2_rn(p0, make_float2(r, r), acc[sb][x][0]);
-                                    acc[sb][x][1] = __ffma2_rn(p1, make_float2(r, r), acc[sb][x][1]);
+                                    // surface-curl pairing by parts: the sender's VALUE field is
+                                    // gathered once and paired with both derivative fields of the edge,
+                                    // X0 += R~ E_theta I,  X1 += R~ (-E_phi) I; the analysis applies {., Y_lm}
+                                    const float2 g0 = __fmul2_rn(lo2(g), make_float2(r, r));
+                                    const float2 g1 = __fmul2_rn(hi2(g), make_float2(r, r));
+                                    acc[sb][x][0][0] = __ffma2_rn(lo2(kr[j][0]), g0, acc[sb][x][0][0]);
+                                    acc[sb][x][0][1] = __ffma2_rn(hi2(kr[j][0]), g1, acc[sb][x][0][1]);
+                                    acc[sb][x][NF - 1][0] = __ffma2_rn(lo2(kr[j][NF - 1]), g0, acc[sb][x][NF - 1][0]);
+                                    acc[sb][x][NF - 1][1] = __ffma2_rn(hi2(kr[j][NF - 1]), g1, acc[sb][x][NF - 1][1]);
                                 }
                             }
                         }
@@ -248,6 +289,7 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
                     }
                 }
             }
+            if (e0 + a.EC < e_end) load_edges(e0 + a.EC, e_end);  // Ebuf was last read before the first sync of this chunk
             consumer_sync();  // Kbuf / Rbuf are rewritten by the next chunk
         }
 
@@ -256,13 +298,16 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
         for (int sb = 0; sb < NSBT; ++sb) {
             if (sb < nsb) {
                 const int ncs = (ncb - sb * cs < cs) ? (ncb - sb * cs) : cs;
-                float4* sdst = reinterpret_cast<float4*>(a.S + ((size_t)i * Cpar + kc0 + sb * cs) * UVp);
+                float4* sdst = reinterpret_cast<float4*>(a.S + ((size_t)i * Cpar + kc0 + sb * cs) * NF * UVp);
 #pragma unroll
                 for (int x = 0; x < NA; ++x) {
                     constexpr int j = 0;
-                    if (chl[x] < ncs && qok[j])
-                        sdst[chl[x] * QP + qd[j]] =
-                            make_float4(acc[sb][x][0].x, acc[sb][x][0].y, acc[sb][x][1].x, acc[sb][x][1].y);
+                    if (chl[x] < ncs && qok[j]) {
+#pragma unroll
+                        for (int f = 0; f < NF; ++f)
+                            sdst[(chl[x] * NF + f) * QP + qd[j]] = make_float4(acc[sb][x][f][0].x, acc[sb][x][f][0].y,
+                                                                               acc[sb][x][f][1].x, acc[sb][x][f][1].y);
+                    }
                 }
             }
         }
@@ -309,10 +354,16 @@ int launch_edge_ring(const Plan* p, bool odd, const float* G, const int64_t* row
     const int G_ = ER_CONS / QP;
     // even kernel: 4 accumulators per thread and sub-block; 6 when that turns the whole channel set into one
     // sub-block (one ring stage per edge: configs[2] all-even 225 -> 192 us), measured slower otherwise
-    int NA = odd ? 2 : 4;
+    // odd: two accumulator fields per channel (X0, X1), so NA * NSBT <= 6: channel blocks of up to 6 G_ channels, as
+    // one sub-block of 6 per thread when a block needs more than 3 G_ (configs[4]: 10.0 -> 9.4 ms), else 3 per thread
+    int NA = odd ? 3 : 4;
+    if (odd) {
+        const int nb = (Cpar + 6 * G_ - 1) / (6 * G_);
+        if ((Cpar + nb - 1) / nb > 3 * G_) NA = 6;
+    }
     if (!odd && Cpar > 4 * G_ && Cpar <= 6 * G_ && (size_t)6 * G_ * p->UVp * 4 * 3 <= 150 * 1024) NA = 6;
     const int cs_max = NA * G_;
-    const int NSB_MAX = 12 / NA;  // NA * NSBT <= 12 float4 accumulators per thread
+    const int NSB_MAX = (odd ? 6 : 12) / NA;  // at most 12 float4 accumulators per thread
     // channel blocks: as few as possible with at most NSB_MAX sub-blocks each
     const int cb_max = cs_max * NSB_MAX;
     const int nblk = (Cpar + cb_max - 1) / cb_max;
@@ -324,7 +375,7 @@ int launch_edge_ring(const Plan* p, bool odd, const float* G, const int64_t* row
     int nsbt = nsb <= 1 ? 1 : nsb <= 2 ? 2 : nsb <= 3 ? 3 : nsb <= 4 ? 4 : 6;
 
     const size_t budget = 200 * 1024;
-    const size_t stage_bytes = (size_t)cs * nf * p->UVp * 4;
+    const size_t stage_bytes = (size_t)cs * p->UVp * 4;  // one gathered field per channel for both parities
     size_t geo_bytes = (size_t)(odd ? 8 : 3) * p->UVp * 4;
     const int geo_smem = geo_bytes <= 32 * 1024 ? 1 : 0;
     if (!geo_smem) geo_bytes = 0;
@@ -332,7 +383,7 @@ int launch_edge_ring(const Plan* p, bool odd, const float* G, const int64_t* row
     while (EC > 1 && (size_t)EC * nf * p->UVp * 4 > 40 * 1024) EC >>= 1;
     const size_t k_bytes = (size_t)EC * nf * p->UVp * 4;
     const size_t r_bytes = (size_t)round_up(EC * cb, 4) * 4;
-    const size_t fixed = 256 + 3 * ER_LMAX * 4 + geo_bytes + k_bytes + r_bytes;
+    const size_t fixed = ER_HDR + geo_bytes + k_bytes + r_bytes;
     if (fixed + 2 * stage_bytes > budget) return CGTP_OK;
     int NST = (int)((budget - fixed) / stage_bytes);
     if (NST > ER_MAXST) NST = ER_MAXST;
@@ -369,12 +420,14 @@ int launch_edge_ring(const Plan* p, bool odd, const float* G, const int64_t* row
     LaunchScope scope(odd ? K_EDGE_ODD : K_EDGE_EVEN, st);
     int rc = CGTP_OK;
     if (odd) {
-        switch (nsbt) {
-        case 1: rc = launch_ring_t<true, 1, 2>(a, smem, grid, st); break;
-        case 2: rc = launch_ring_t<true, 2, 2>(a, smem, grid, st); break;
-        case 3: rc = launch_ring_t<true, 3, 2>(a, smem, grid, st); break;
-        case 4: rc = launch_ring_t<true, 4, 2>(a, smem, grid, st); break;
-        default: rc = launch_ring_t<true, 6, 2>(a, smem, grid, st); break;
+        if (NA == 3) {
+            rc = nsbt <= 1 ? launch_ring_t<true, 1, 3>(a, smem, grid, st) : launch_ring_t<true, 2, 3>(a, smem, grid, st);
+        } else if (NA == 6) {
+            rc = launch_ring_t<true, 1, 6>(a, smem, grid, st);
+        } else {
+            rc = nsbt <= 1 ? launch_ring_t<true, 1, 2>(a, smem, grid, st)
+               : nsbt <= 2 ? launch_ring_t<true, 2, 2>(a, smem, grid, st)
+                           : launch_ring_t<true, 3, 2>(a, smem, grid, st);
         }
     } else {
         if (NA == 6) {

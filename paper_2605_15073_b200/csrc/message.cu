@@ -70,18 +70,18 @@ struct SynthSmem {
     int tab_bytes, q_bytes;
 };
 
-static SynthSmem synth_smem_layout(const Plan* p, bool odd, int NC)
+static SynthSmem synth_smem_layout(const Plan* p, int NC)
 {
     SynthSmem s;
     const int M = 2 * p->LB + 1;
     const int J = (NC * p->U) | 1;  // odd row stride: rows of different m fall into different banks
-    const int nf = odd ? 2 : 1;
+    const int nf = 1;
     s.tab_bytes = p->Uh * p->NTRI * 4;
     s.q_bytes = p->Vh * p->QSTR * 4;
     int off = 0;
     s.bar = off; off += 16;
     s.tab0 = off; off += s.tab_bytes;
-    s.tab1 = off; off += odd ? s.tab_bytes : 0;
+    s.tab1 = off;
     s.qc = off; off += s.q_bytes;
     s.qs = off; off += s.q_bytes;
     s.hs = off; off += NC * p->L2p * 4;
@@ -91,16 +91,15 @@ static SynthSmem synth_smem_layout(const Plan* p, bool odd, int NC)
     return s;
 }
 
-template <int LB, bool ODD>
+template <int LB>
 __global__ void __launch_bounds__(256) node_synth_kernel(Plan p, SynthSmem lay, const float* __restrict__ H,
                                                         float* __restrict__ G, long long ncols, int NC)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int M = 2 * LB + 1;
-    constexpr int NF = ODD ? 2 : 1;
+    constexpr int NF = 1;
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + lay.bar);
     float* tab0 = reinterpret_cast<float*>(smem + lay.tab0);
-    float* tab1 = reinterpret_cast<float*>(smem + lay.tab1);
     float* qc = reinterpret_cast<float*>(smem + lay.qc);
     float* qs = reinterpret_cast<float*>(smem + lay.qs);
     float* hs = reinterpret_cast<float*>(smem + lay.hs);
@@ -118,10 +117,9 @@ __global__ void __launch_bounds__(256) node_synth_kernel(Plan p, SynthSmem lay, 
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        const uint32_t total = (ODD ? 2 : 1) * lay.tab_bytes + 2 * lay.q_bytes + hbytes;
+        const uint32_t total = lay.tab_bytes + 2 * lay.q_bytes + hbytes;
         mbar_arrive_expect_tx(bar, total);
-        tma_load_span(tab0, ODD ? p.DT : p.PT, lay.tab_bytes, bar);
-        if (ODD) tma_load_span(tab1, p.ST, lay.tab_bytes, bar);
+        tma_load_span(tab0, p.PT, lay.tab_bytes, bar);
         tma_load_span(qc, p.QC, lay.q_bytes, bar);
         tma_load_span(qs, p.QS, lay.q_bytes, bar);
         tma_load_span(hs, H + col0 * p.L2p, hbytes, bar);
@@ -138,12 +136,9 @@ __global__ void __launch_bounds__(256) node_synth_kernel(Plan p, SynthSmem lay, 
     }
     mbar_wait(bar, 0);
 
-    if (!ODD) {
+    {
         const LegDst dst[1][2] = {{{F, 1.f}, {nullptr, 0.f}}};
         legendre_synthesis<LB, false, 1, 4>(tab0, nullptr, hs, 0, p.L2p, dst, nc, p.lmax, p.U, p.Uh, p.NTRI, J);
-    } else {
-        const LegDst dst[1][2] = {{{F, 1.f}, {F + (size_t)M * J, 1.f}}};
-        legendre_synthesis<LB, true, 1, 4>(tab0, tab1, hs, 0, p.L2p, dst, nc, p.lmax, p.U, p.Uh, p.NTRI, J);
     }
     __syncthreads();
 
@@ -164,12 +159,12 @@ __global__ void __launch_bounds__(256) node_synth_kernel(Plan p, SynthSmem lay, 
     for (int i = threadIdx.x; i < n4; i += blockDim.x) dst4[i] = src4[i];
 }
 
-template <int LB, bool ODD>
-static int launch_node_synth_t(const Plan* p, const float* H, float* G, int64_t ncols, cudaStream_t st)
+template <int LB>
+static int launch_node_synth_t(const Plan* p, Kind kind, const float* H, float* G, int64_t ncols, cudaStream_t st)
 {
     const int M = 2 * p->LB + 1;
-    const int nf = ODD ? 2 : 1;
-    SynthSmem fixed = synth_smem_layout(p, ODD, 0);
+    const int nf = 1;
+    SynthSmem fixed = synth_smem_layout(p, 0);
     const int percol = p->L2p * 4 + nf * M * p->U * 4 + nf * p->UVp * 4;
     // 45 KB per CTA -> four or five CTAs per SM, so that the load / compute / store phases of different CTAs overlap
     // (measured on configs[2] / configs[4]: 64 -> 52 us and 1.08 -> 0.85 ms against a 100 KB budget)
@@ -182,11 +177,11 @@ static int launch_node_synth_t(const Plan* p, const float* H, float* G, int64_t 
     if (NC < 1) { set_error("node synthesis: shared memory too small for lmax=%d", p->lmax); return CGTP_ERR_UNSUPPORTED; }
     if (NC > 128) NC = 128;
     if ((int64_t)NC > ncols) NC = (int)ncols;
-    SynthSmem lay = synth_smem_layout(p, ODD, NC);
-    auto kern = node_synth_kernel<LB, ODD>;
+    SynthSmem lay = synth_smem_layout(p, NC);
+    auto kern = node_synth_kernel<LB>;
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, lay.total));
     int64_t grid = (ncols + NC - 1) / NC;
-    LaunchScope scope(ODD ? K_NODE_SYNTH_ODD : K_NODE_SYNTH_EVEN, st);
+    LaunchScope scope(kind, st);
     kern<<<(unsigned)grid, 256, lay.total, st>>>(*p, lay, H, G, (long long)ncols, NC);
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
@@ -196,10 +191,9 @@ int launch_node_synth(const Plan* p, bool odd, const float* H, float* G, int64_t
 {
     if (ncols <= 0) return CGTP_OK;
     switch (p->LB) {
-#define CGTP_CASE(B)                                                       \
-    case B:                                                                \
-        return odd ? launch_node_synth_t<B, true>(p, H, G, ncols, st)      \
-                   : launch_node_synth_t<B, false>(p, H, G, ncols, st);
+#define CGTP_CASE(B) \
+    case B:          \
+        return launch_node_synth_t<B>(p, odd ? K_NODE_SYNTH_ODD : K_NODE_SYNTH_EVEN, H, G, ncols, st);
         CGTP_FOR_EACH_BAND(CGTP_CASE)
 #undef CGTP_CASE
     }
@@ -223,8 +217,8 @@ __device__ __forceinline__ float4 ldg_stream(const float4* p)
     return r;
 }
 
-// G   : even [nodes][Cpar][UVp]          odd [nodes][Cpar][2][UVp]
-// S   : [nodes][Cpar][UVp]
+// G   : [nodes][Cpar][UVp] (value field, both parities)
+// S   : even [nodes][Cpar][UVp]          odd [nodes][Cpar][2][UVp] = (X0, X1) of the by-parts pairing
 // grid: (channel blocks, receivers)
 template <bool ODD>
 __global__ void __launch_bounds__(EDGE_NT) edge_kernel(Plan p, const float* __restrict__ G,
@@ -249,13 +243,14 @@ __global__ void __launch_bounds__(EDGE_NT) edge_kernel(Plan p, const float* __re
 
     // ownership: accumulator a of this thread is float4 index f = tid + a*NT -> (channel kc, quad q)
     int kcl[EDGE_NI], qd[EDGE_NI];
-    float4 acc[EDGE_NI];
+    float4 acc[EDGE_NI][NF];
 #pragma unroll
     for (int a = 0; a < EDGE_NI; ++a) {
         const int f = threadIdx.x + a * EDGE_NT;
         kcl[a] = (f < n4) ? f / QP : -1;
         qd[a] = (f < n4) ? f - kcl[a] * QP : 0;
-        acc[a] = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int x = 0; x < NF; ++x) acc[a][x] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
 
     const bool graph_ok = (*status == 0);
@@ -293,7 +288,7 @@ __global__ void __launch_bounds__(EDGE_NT) edge_kernel(Plan p, const float* __re
                     const float dth = ex * p.geo[3 * UVp + q] + ey * p.geo[4 * UVp + q] + ez * p.geo[5 * UVp + q];
                     const float dph = ex * p.geo[6 * UVp + q] + ey * p.geo[7 * UVp + q];
                     k0 = kd * dth;
-                    k1 = kd * dph;
+                    k1 = -(kd * dph);
                 }
             }
             Kbuf[((size_t)el * NF) * UVp + q] = k0;
@@ -308,33 +303,24 @@ __global__ void __launch_bounds__(EDGE_NT) edge_kernel(Plan p, const float* __re
 
         // ---- M4: gather the sender's grid fields, multiply, accumulate (fixed edge order)
         for (int el = 0; el < ne; ++el) {
-            const float4* gsrc = reinterpret_cast<const float4*>(G + ((size_t)Sbuf[el] * Cpar + kc0) * NF * UVp);
+            const float4* gsrc = reinterpret_cast<const float4*>(G + ((size_t)Sbuf[el] * Cpar + kc0) * UVp);
             const float4* k4 = reinterpret_cast<const float4*>(Kbuf + (size_t)el * NF * UVp);
-            float4 g0[EDGE_NI], g1[EDGE_NI];
+            float4 g0[EDGE_NI];
 #pragma unroll
-            for (int a = 0; a < EDGE_NI; ++a) {
-                if (kcl[a] >= 0) {
-                    g0[a] = ldg_stream(gsrc + (size_t)kcl[a] * NF * QP + qd[a]);
-                    if (ODD) g1[a] = ldg_stream(gsrc + (size_t)kcl[a] * NF * QP + QP + qd[a]);
-                }
-            }
+            for (int a = 0; a < EDGE_NI; ++a)
+                if (kcl[a] >= 0) g0[a] = ldg_stream(gsrc + (size_t)kcl[a] * QP + qd[a]);
 #pragma unroll
             for (int a = 0; a < EDGE_NI; ++a) {
                 if (kcl[a] >= 0) {
                     const float r = Rbuf[el * cb + kcl[a]];
-                    if (!ODD) {
-                        const float4 k = k4[qd[a]];
-                        acc[a].x = fmaf(r * k.x, g0[a].x, acc[a].x);
-                        acc[a].y = fmaf(r * k.y, g0[a].y, acc[a].y);
-                        acc[a].z = fmaf(r * k.z, g0[a].z, acc[a].z);
-                        acc[a].w = fmaf(r * k.w, g0[a].w, acc[a].w);
-                    } else {
-                        // {E, I} = E_theta I_phi - E_phi I_theta   (edge = factor 1, Eq.(57))
-                        const float4 et = k4[qd[a]], ep = k4[QP + qd[a]];
-                        acc[a].x = fmaf(r, et.x * g1[a].x - ep.x * g0[a].x, acc[a].x);
-                        acc[a].y = fmaf(r, et.y * g1[a].y - ep.y * g0[a].y, acc[a].y);
-                        acc[a].z = fmaf(r, et.z * g1[a].z - ep.z * g0[a].z, acc[a].z);
-                        acc[a].w = fmaf(r, et.w * g1[a].w - ep.w * g0[a].w, acc[a].w);
+#pragma unroll
+                    for (int x = 0; x < NF; ++x) {
+                        // even: K_e; odd: (d_theta K_e, -(1/sin) d_phi K_e) against the sender's value field
+                        const float4 k = k4[x * QP + qd[a]];
+                        acc[a][x].x = fmaf(r * k.x, g0[a].x, acc[a][x].x);
+                        acc[a][x].y = fmaf(r * k.y, g0[a].y, acc[a][x].y);
+                        acc[a][x].z = fmaf(r * k.z, g0[a].z, acc[a][x].z);
+                        acc[a][x].w = fmaf(r * k.w, g0[a].w, acc[a][x].w);
                     }
                 }
             }
@@ -342,10 +328,13 @@ __global__ void __launch_bounds__(EDGE_NT) edge_kernel(Plan p, const float* __re
         __syncthreads();
     }
 
-    float4* sdst = reinterpret_cast<float4*>(S + ((size_t)i * Cpar + kc0) * UVp);
+    float4* sdst = reinterpret_cast<float4*>(S + ((size_t)i * Cpar + kc0) * NF * UVp);
 #pragma unroll
     for (int a = 0; a < EDGE_NI; ++a)
-        if (kcl[a] >= 0) sdst[(size_t)kcl[a] * QP + qd[a]] = acc[a];
+        if (kcl[a] >= 0) {
+#pragma unroll
+            for (int x = 0; x < NF; ++x) sdst[((size_t)kcl[a] * NF + x) * QP + qd[a]] = acc[a][x];
+        }
 }
 
 int launch_edge(const Plan* p, bool odd, const float* G, const int64_t* row_ptr, const int64_t* edge_index, int64_t E,
@@ -378,7 +367,7 @@ int launch_edge(const Plan* p, bool odd, const float* G, const int64_t* row_ptr,
         if (odd) {
             CGTP_CUDA_CHECK(cudaFuncSetAttribute(edge_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             edge_kernel<true><<<grid, EDGE_NT, smem, st>>>(*p, G, row_ptr + n0, edge_index, edge_vec, edge_radial, perm_par,
-                                                          Cpar, C, cb, S + (size_t)n0 * Cpar * p->UVp, status);
+                                                          Cpar, C, cb, S + (size_t)n0 * Cpar * 2 * p->UVp, status);
         } else {
             CGTP_CUDA_CHECK(cudaFuncSetAttribute(edge_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             edge_kernel<false><<<grid, EDGE_NT, smem, st>>>(*p, G, row_ptr + n0, edge_index, edge_vec, edge_radial, perm_par,
@@ -398,31 +387,34 @@ struct AnaSmem {
     int tab_bytes, q_bytes, wv_bytes;
 };
 
-static AnaSmem ana_smem_layout(const Plan* p, int NC)
+static AnaSmem ana_smem_layout(const Plan* p, bool odd, int NC)
 {
     AnaSmem s;
     const int M = 2 * p->LB + 1;
     const int J = (NC * p->U) | 1;  // odd row stride: rows of different m fall into different banks
+    const int nf = odd ? 2 : 1;     // odd channels: the field pair (X0, X1) and the table pair (WD, WS)
     s.tab_bytes = p->Uh * p->NTRI * 4;
     s.q_bytes = p->Vh * p->QSTR * 4;
     s.wv_bytes = round_up(p->Vh, 4) * 4;
     int off = 0;
     s.bar = off; off += 16;
-    s.wp = off; off += s.tab_bytes;
+    s.wp = off; off += nf * s.tab_bytes;
     s.qc = off; off += s.q_bytes;
     s.qs = off; off += s.q_bytes;
     s.wv = off; off += s.wv_bytes;
-    s.ss = off; off += NC * p->UVp * 4;
-    s.t = off; off += round_up(M * J, 4) * 4;
+    s.ss = off; off += NC * nf * p->UVp * 4;
+    s.t = off; off += nf * round_up(M * J, 4) * 4;
     s.total = off;
     return s;
 }
 
-template <int LB>
+template <int LB, bool ODD>
 __global__ void __launch_bounds__(256) analysis_kernel(Plan p, AnaSmem lay, const float* __restrict__ S,
                                                       float* __restrict__ T, long long ncols, int NC)
 {
     extern __shared__ __align__(128) unsigned char smem[];
+    constexpr int M = 2 * LB + 1;
+    constexpr int NF = ODD ? 2 : 1;
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + lay.bar);
     float* wp = reinterpret_cast<float*>(smem + lay.wp);
     float* qc = reinterpret_cast<float*>(smem + lay.qc);
@@ -434,7 +426,8 @@ __global__ void __launch_bounds__(256) analysis_kernel(Plan p, AnaSmem lay, cons
     const long long col0 = (long long)blockIdx.x * NC;
     const int nc = (int)((ncols - col0 < NC) ? (ncols - col0) : NC);
     const int J = (NC * p.U) | 1;  // odd row stride (matches the host layout)
-    const int sbytes = nc * p.UVp * 4;
+    const int MJ = round_up(M * J, 4);
+    const int sbytes = nc * NF * p.UVp * 4;
 
     if (threadIdx.x == 0) {
         mbar_init(bar, 1);
@@ -442,31 +435,42 @@ __global__ void __launch_bounds__(256) analysis_kernel(Plan p, AnaSmem lay, cons
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        const uint32_t total = lay.tab_bytes + 2 * lay.q_bytes + lay.wv_bytes + sbytes;
+        const uint32_t total = NF * lay.tab_bytes + 2 * lay.q_bytes + lay.wv_bytes + sbytes;
         mbar_arrive_expect_tx(bar, total);
-        tma_load_span(wp, p.WP, lay.tab_bytes, bar);
+        if (!ODD) {
+            tma_load_span(wp, p.WP, lay.tab_bytes, bar);
+        } else {
+            tma_load_span(wp, p.WD, lay.tab_bytes, bar);
+            tma_load_span(wp + lay.tab_bytes / 4, p.WS, lay.tab_bytes, bar);
+        }
         tma_load_span(qc, p.QC, lay.q_bytes, bar);
         tma_load_span(qs, p.QS, lay.q_bytes, bar);
         tma_load_span(wv, p.WV, lay.wv_bytes, bar);
-        tma_load_span(Ss, S + col0 * p.UVp, sbytes, bar);
+        tma_load_span(Ss, S + col0 * NF * p.UVp, sbytes, bar);
     }
     mbar_wait(bar, 0);
 
     const int rows = nc * p.U;
-    for (int j = threadIdx.x; j < rows; j += blockDim.x) {
+    for (int item = threadIdx.x; item < NF * rows; item += blockDim.x) {
+        const int f = item / rows, j = item - f * rows;
         const int col = j / p.U, u = j - col * p.U;
-        dft_inverse_row<LB>(Ss + (size_t)col * p.UVp + u * p.V, Tm, J, j, qc, qs, wv, p.V, p.Vh);
+        dft_inverse_row<LB>(Ss + ((size_t)col * NF + f) * p.UVp + u * p.V, Tm + (size_t)f * MJ, J, j, qc, qs, wv, p.V, p.Vh);
     }
     __syncthreads();
-    legendre_analysis<LB>(Tm, nullptr, wp, T + col0 * p.Lo2p, p.Lo2p, nc, p.lmax_out, p.U, p.Uh, p.NTRI, J);
+    if (!ODD)
+        legendre_analysis<LB>(Tm, nullptr, wp, T + col0 * p.Lo2p, p.Lo2p, nc, p.lmax_out, p.U, p.Uh, p.NTRI, J);
+    else
+        legendre_analysis_curl<LB>(Tm, Tm + MJ, wp, wp + lay.tab_bytes / 4, T + col0 * p.Lo2p, p.Lo2p, nc, p.lmax_out, p.U,
+                                   p.Uh, p.NTRI, J);
 }
 
-template <int LB>
-static int launch_analysis_t(const Plan* p, bool odd, const float* S, float* T, int64_t ncols, cudaStream_t st)
+template <int LB, bool ODD>
+static int launch_analysis_t(const Plan* p, const float* S, float* T, int64_t ncols, cudaStream_t st)
 {
     const int M = 2 * p->LB + 1;
-    AnaSmem fixed = ana_smem_layout(p, 0);
-    const int percol = p->UVp * 4 + M * p->U * 4;
+    const int nf = ODD ? 2 : 1;
+    AnaSmem fixed = ana_smem_layout(p, ODD, 0);
+    const int percol = nf * (p->UVp * 4 + M * p->U * 4);
     int budget = 45 * 1024;  // as node synthesis: several small CTAs per SM overlap their phases (0.80 -> 0.67 ms, configs[4])
     int NC = (budget - fixed.total - 64) / percol;
     if (NC < 4) {
@@ -476,11 +480,11 @@ static int launch_analysis_t(const Plan* p, bool odd, const float* S, float* T, 
     if (NC < 1) { set_error("analysis: shared memory too small for lmax=%d", p->lmax); return CGTP_ERR_UNSUPPORTED; }
     if (NC > 128) NC = 128;
     if ((int64_t)NC > ncols) NC = (int)ncols;
-    AnaSmem lay = ana_smem_layout(p, NC);
-    auto kern = analysis_kernel<LB>;
+    AnaSmem lay = ana_smem_layout(p, ODD, NC);
+    auto kern = analysis_kernel<LB, ODD>;
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, lay.total));
     int64_t grid = (ncols + NC - 1) / NC;
-    LaunchScope scope(odd ? K_ANALYSIS_ODD : K_ANALYSIS_EVEN, st);
+    LaunchScope scope(ODD ? K_ANALYSIS_ODD : K_ANALYSIS_EVEN, st);
     kern<<<(unsigned)grid, 256, lay.total, st>>>(*p, lay, S, T, (long long)ncols, NC);
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
@@ -492,7 +496,7 @@ int launch_analysis(const Plan* p, bool odd, const float* S, float* T, int64_t n
     switch (p->LB) {
 #define CGTP_CASE(B) \
     case B:          \
-        return launch_analysis_t<B>(p, odd, S, T, ncols, st);
+        return odd ? launch_analysis_t<B, true>(p, S, T, ncols, st) : launch_analysis_t<B, false>(p, S, T, ncols, st);
         CGTP_FOR_EACH_BAND(CGTP_CASE)
 #undef CGTP_CASE
     }

@@ -407,4 +407,68 @@ __device__ __forceinline__ void legendre_analysis(const float* T0, const float* 
     }
 }
 
+// Row M5 second half for the odd (surface-curl) channels, by parts.  With the pooled grids
+//   X0 = sum_e R~ (d_theta E_e) I_j,   X1 = -sum_e R~ ((1/sin) d_phi E_e) I_j       (edge_ring.cu / message.cu)
+// the coupling  T_lm = int r.[grad E x grad I] Y_lm  (Eq.(57) PAPER.md:443 under Eq.(53)-(54)) equals, because the
+// bracket of two functions integrates to zero over the sphere,
+//   T_lm = -int I {E, Y_lm} = -int [ X1 d_theta Y_lm + X0 (1/sin) d_phi Y_lm ] dOmega ,
+// and with (1/sin) d_phi Y_{l,+m} = -(m P~/sin) q_{-m}, (1/sin) d_phi Y_{l,-m} = +(m P~/sin) q_{+m}  (:679):
+//   T_{l,+m} = sum_u w_u [ -dP~_l^m x1_{+m}(u) + (m P~_l^m/sin) x0_{-m}(u) ]
+//   T_{l,-m} = sum_u w_u [ -dP~_l^m x1_{-m}(u) - (m P~_l^m/sin) x0_{+m}(u) ] .
+// X0r, X1r: [M][J] shared azimuthal coefficients per grid row; WD, WS: [Uh][NTRI] weighted tables.
+// Reflection x -> -x: m P~/sin has the parity (-1)^(l-m) of P~, d_theta P~ the opposite one.
+template <int LB>
+__device__ __forceinline__ void legendre_analysis_curl(const float* X0r, const float* X1r,
+                                                       const float* __restrict__ WD, const float* __restrict__ WS,
+                                                       float* __restrict__ out, int Lo2p, int NC, int lmax_out, int U,
+                                                       int Uh, int NTRI, int J)
+{
+    constexpr int UHMAX = ((3 * LB + 2) / 2 + 1) / 2;
+    const int items = NC * (lmax_out + 1);
+    for (int item = threadIdx.x; item < items; item += blockDim.x) {
+        const int col = item / (lmax_out + 1);
+        const int mm = item - col * (lmax_out + 1);
+        // [field][cos / sin row][north + south, north - south][u']
+        float f[2][2][2][UHMAX];
+#pragma unroll
+        for (int x = 0; x < 2; ++x) {
+            const float* X = x ? X1r : X0r;
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                const int row = (s == 0) ? mm : (LB + mm);
+#pragma unroll
+                for (int up = 0; up < UHMAX; ++up) {
+                    float n = 0.f, so = 0.f;
+                    if (up < Uh && !(s == 1 && mm == 0)) {
+                        n = X[row * J + col * U + up];
+                        so = X[row * J + col * U + (U - 1 - up)];
+                    }
+                    f[x][s][0][up] = n + so;
+                    f[x][s][1][up] = n - so;
+                }
+            }
+        }
+        float* ocol = out + (size_t)col * Lo2p;
+        for (int l = mm; l <= lmax_out; ++l) {
+            const int par = (l - mm) & 1;  // 0: P~ symmetric, d_theta P~ antisymmetric under x -> -x
+            const int t0 = tri_index(l, mm);
+            float ap = 0.f, an = 0.f;
+#pragma unroll
+            for (int up = 0; up < UHMAX; ++up) {
+                if (up < Uh) {
+                    const float wd = WD[up * NTRI + t0], ws = WS[up * NTRI + t0];
+                    const float x1c = par ? f[1][0][0][up] : f[1][0][1][up];  // x1_{+m} folded for d_theta P~
+                    const float x1s = par ? f[1][1][0][up] : f[1][1][1][up];  // x1_{-m}
+                    const float x0c = par ? f[0][0][1][up] : f[0][0][0][up];  // x0_{+m} folded for m P~/sin
+                    const float x0s = par ? f[0][1][1][up] : f[0][1][0][up];  // x0_{-m}
+                    ap = fmaf(ws, x0s, fmaf(-wd, x1c, ap));
+                    an = fmaf(-ws, x0c, fmaf(-wd, x1s, an));
+                }
+            }
+            ocol[l * l + l + mm] = ap;
+            if (mm > 0) ocol[l * l + l - mm] = an;
+        }
+    }
+}
+
 }  // namespace cgtp

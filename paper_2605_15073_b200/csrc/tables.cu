@@ -199,7 +199,7 @@ const Plan* get_plan(int lmax, int lmax_out)
     legendre_values(U, LB, x, P);
     auto at = [&](int u, int l, int m) -> double& { return P[((size_t)u * LL + l) * LL + m]; };
 
-    std::vector<float> PT((size_t)Uh * NTRI, 0.f), DT(PT), ST(PT), WP(PT);
+    std::vector<float> PT((size_t)Uh * NTRI, 0.f), DT(PT), ST(PT), WP(PT), WD(PT), WS(PT);
     for (int u = 0; u < Uh; ++u) {
         double ct = x[u], st = std::sqrt(1.0 - ct * ct);
         double wu = w[u] * ((U % 2 && u == Uh - 1) ? 0.5 : 1.0);
@@ -215,6 +215,8 @@ const Plan* get_plan(int lmax, int lmax_out)
                 DT[k] = (float)dth;
                 ST[k] = (float)(m * pv / st);
                 WP[k] = (float)(wu * pv);
+                WD[k] = (float)(wu * dth);
+                WS[k] = (float)(wu * m * pv / st);
             }
     }
 
@@ -251,6 +253,8 @@ const Plan* get_plan(int lmax, int lmax_out)
     p->DT = upload(DT, &ok);
     p->ST = upload(ST, &ok);
     p->WP = upload(WP, &ok);
+    p->WD = upload(WD, &ok);
+    p->WS = upload(WS, &ok);
     p->QC = upload(QC, &ok);
     p->QS = upload(QS, &ok);
     p->WV = upload(WV, &ok);
