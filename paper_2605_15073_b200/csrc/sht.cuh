@@ -424,49 +424,54 @@ __device__ __forceinline__ void legendre_analysis_curl(const float* X0r, const f
                                                        int Uh, int NTRI, int J)
 {
     constexpr int UHMAX = ((3 * LB + 2) / 2 + 1) / 2;
-    const int items = NC * (lmax_out + 1);
+    // work item = (column, |m|, sign of m): T_{l,+m} needs x1_{+m} and x0_{-m}, T_{l,-m} needs x1_{-m} and x0_{+m}
+    const int items = NC * (lmax_out + 1) * 2;
     for (int item = threadIdx.x; item < items; item += blockDim.x) {
-        const int col = item / (lmax_out + 1);
-        const int mm = item - col * (lmax_out + 1);
-        // [field][cos / sin row][north + south, north - south][u']
-        float f[2][2][2][UHMAX];
+        const int neg = item & 1;
+        const int cm = item >> 1;
+        const int col = cm / (lmax_out + 1);
+        const int mm = cm - col * (lmax_out + 1);
+        if (neg && mm == 0) continue;
+        const int row1 = neg ? (LB + mm) : mm;  // row of X1 with the sign of the output m
+        const int row0 = neg ? mm : (LB + mm);  // row of X0 with the opposite sign
+        const float sgn0 = neg ? -1.f : 1.f;
+        // [north + south, north - south][u']
+        float f1[2][UHMAX], f0[2][UHMAX];
 #pragma unroll
-        for (int x = 0; x < 2; ++x) {
-            const float* X = x ? X1r : X0r;
-#pragma unroll
-            for (int s = 0; s < 2; ++s) {
-                const int row = (s == 0) ? mm : (LB + mm);
-#pragma unroll
-                for (int up = 0; up < UHMAX; ++up) {
-                    float n = 0.f, so = 0.f;
-                    if (up < Uh && !(s == 1 && mm == 0)) {
-                        n = X[row * J + col * U + up];
-                        so = X[row * J + col * U + (U - 1 - up)];
-                    }
-                    f[x][s][0][up] = n + so;
-                    f[x][s][1][up] = n - so;
+        for (int up = 0; up < UHMAX; ++up) {
+            float n1 = 0.f, s1 = 0.f, n0 = 0.f, s0 = 0.f;
+            if (up < Uh) {
+                n1 = X1r[row1 * J + col * U + up];
+                s1 = X1r[row1 * J + col * U + (U - 1 - up)];
+                if (mm > 0) {
+                    n0 = sgn0 * X0r[row0 * J + col * U + up];
+                    s0 = sgn0 * X0r[row0 * J + col * U + (U - 1 - up)];
                 }
             }
+            f1[0][up] = n1 + s1;
+            f1[1][up] = n1 - s1;
+            f0[0][up] = n0 + s0;
+            f0[1][up] = n0 - s0;
         }
         float* ocol = out + (size_t)col * Lo2p;
-        for (int l = mm; l <= lmax_out; ++l) {
-            const int par = (l - mm) & 1;  // 0: P~ symmetric, d_theta P~ antisymmetric under x -> -x
-            const int t0 = tri_index(l, mm);
-            float ap = 0.f, an = 0.f;
+        // degrees in pairs so that the reflection parity of (l - m) is a compile-time constant:
+        // par = 0: P~ symmetric, d_theta P~ antisymmetric under x -> -x; par = 1 the other way round
+        for (int l0 = mm; l0 <= lmax_out; l0 += 2) {
 #pragma unroll
-            for (int up = 0; up < UHMAX; ++up) {
-                if (up < Uh) {
-                    const float wd = WD[up * NTRI + t0], ws = WS[up * NTRI + t0];
-                    const float x1c = par ? f[1][0][0][up] : f[1][0][1][up];  // x1_{+m} folded for d_theta P~
-                    const float x1s = par ? f[1][1][0][up] : f[1][1][1][up];  // x1_{-m}
-                    const float x0c = par ? f[0][0][1][up] : f[0][0][0][up];  // x0_{+m} folded for m P~/sin
-                    const float x0s = par ? f[0][1][1][up] : f[0][1][0][up];  // x0_{-m}
-                    ap = fmaf(ws, x0s, fmaf(-wd, x1c, ap));
-                    an = fmaf(-ws, x0c, fmaf(-wd, x1s, an));
+            for (int par = 0; par < 2; ++par) {
+                const int l = l0 + par;
+                if (l > lmax_out) break;
+                const int t0 = tri_index(l, mm);
+                float acc = 0.f;
+#pragma unroll
+                for (int up = 0; up < UHMAX; ++up) {
+                    if (up < Uh) {
+                        const float wd = WD[up * NTRI + t0], ws = WS[up * NTRI + t0];
+                        acc = fmaf(ws, f0[par][up], fmaf(-wd, f1[1 - par][up], acc));
+                    }
                 }
+                ocol[l * l + l + (neg ? -mm : mm)] = acc;
             }
-            ocol[l * l + l + mm] = ap;
-            if (mm > 0) ocol[l * l + l - mm] = an;
         }
     }
 }
