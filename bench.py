@@ -65,17 +65,21 @@ def onsite_bytes_per_atom(lmax, lmax_out, N):
 
 
 def message_bytes(lmax, lmax_out, N, C, Ce, Co, nodes, E):
-    """Paper-faithful fused data flow: gather sender grids."""
+    """Algorithmic HBM bytes of the implemented data flow: every edge gathers ONE value grid per rank
+    channel of either parity (the odd channels pair it with both derivative fields of the edge and pool two grids per
+    receiver).  Also returns the total of SURVEY.md 8(d)'s "gather sender grids" flow (two gathered derivative fields per
+    odd channel), which this build no longer moves, for comparison."""
     U, V = grid_shape(lmax, lmax_out)
     UV = U * V
     L2, Lo2 = (lmax + 1) ** 2, (lmax_out + 1) ** 2
     k = {
         "edge_even": E * (4 * Ce * UV + 4 * Ce + 12 + 16) + nodes * 4 * Ce * UV,
-        "edge_odd": E * (4 * 2 * Co * UV + 4 * Co + 12 + 16) + nodes * 4 * Co * UV,
+        "edge_odd": E * (4 * Co * UV + 4 * Co + 12 + 16) + nodes * 8 * Co * UV,
     }
-    total = (E * (4 * (Ce + 2 * Co) * UV + 4 * C + 12 + 16)
-             + nodes * (4 * N * L2 + 4 * (Ce + 2 * Co) * UV + 8 * N * Lo2))
-    return k, total
+    total = E * (4 * C * UV + 4 * C + 12 + 16) + nodes * (4 * N * L2 + 4 * C * UV + 8 * N * Lo2)
+    total_paper_flow = (E * (4 * (Ce + 2 * Co) * UV + 4 * C + 12 + 16)
+                        + nodes * (4 * N * L2 + 4 * (Ce + 2 * Co) * UV + 8 * N * Lo2))
+    return k, total, total_paper_flow
 
 
 # ------------------------------------------------------------------------------------------------
@@ -473,7 +477,7 @@ def run_message(args, cg, synthetic, dev, peaks, peak_src):
         torch.cuda.synchronize()
         prof = cg.cgtp_profile_collect()
         cg.cgtp_profile_enable(False)
-        kb, total_bytes = message_bytes(m.lmax, m.lmax_out, m.N, m.C, Ce, Co, m.nodes, m.E)
+        kb, total_bytes, paper_bytes = message_bytes(m.lmax, m.lmax_out, m.N, m.C, Ce, Co, m.nodes, m.E)
         kern = {}
         tot = sum(v[0] for v in prof.values())
         for k, (kms, cnt) in prof.items():
@@ -488,6 +492,9 @@ def run_message(args, cg, synthetic, dev, peaks, peak_src):
             "ms_per_step": ms, "edges_per_s": m.E / (ms * 1e-3),
             "alg_hbm_gbs_whole_step": total_bytes / (ms * 1e-3) / 1e9,
             "frac_hbm_peak_whole_step": total_bytes / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+            "paper_flow_equiv_gbs": paper_bytes / (ms * 1e-3) / 1e9,
+            "numerator": "implemented flow: one gathered value grid per (edge, channel); paper_flow_equiv_gbs uses "
+                         "SURVEY.md 8(d)'s two-derivative-field gather for the odd channels",
             "roofline": {"kernel": dom, "bound": "hbm", "achieved": kern[dom].get("alg_gbs"),
                          "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": kern[dom].get("frac_hbm_peak"),
                          "peak_source": peak_src, "traffic": None},

@@ -51,6 +51,8 @@ struct PfArgs {
     int stage_floats;  // AB * KC * x_rs
     uint32_t jmagic;   // floor(2^32 / J) + 1
     int w_floats;      // Kmax * MW
+    int window;        // 1: tile = window of CWT flattened (atom, j) columns, atoms may straddle tiles (NSUB = 1)
+    int ntiles;        // tiles per (problem, row block)
 };
 
 __device__ __forceinline__ float lds32(uint32_t addr)
@@ -71,7 +73,7 @@ __device__ __forceinline__ void mbar_arrive_cta(uint64_t* bar)
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
-template <int RW, int CWP, bool ACC>
+template <int RW, int CWP, bool ACC, bool WIN>
 __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
 {
     constexpr int MW = 16 * RW;       // rows per CTA
@@ -112,8 +114,21 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
 
     // tiles of this CTA: ti = rank + i * cpr (32-bit: the host rejects larger problems); chunk counters
     // advance incrementally (no divisions in the loop)
-    const int ngroups = (int)((a.batch + AB - 1) / AB);
-    const int ntiles = ngroups * NSUB;
+    // tiles of a (problem, row block): WIN = false: (atom group, sub-tile); WIN = true: windows of CWT flattened
+    // (atom, j) columns (NSUB = 1), atoms may straddle tiles.  A template flag so that the group form keeps its code.
+    const int ntiles = a.ntiles;
+    // first atom of tile ti and the tile's first column inside the staged atoms
+    auto tile_origin = [&](int ti, int& b0, int& off0) {
+        if (WIN) {
+            const int64_t c0 = (int64_t)ti * CWT;
+            b0 = (int)(c0 / J);
+            off0 = (int)(c0 - (int64_t)b0 * J);
+        } else {
+            const int g = ti / NSUB;
+            b0 = g * AB;
+            off0 = (ti - g * NSUB) * CWT;
+        }
+    };
     const int my_tiles = (ntiles > rank) ? (ntiles - rank + cpr - 1) / cpr : 0;
     const int NCH = K / KC;
     const int nchunks = my_tiles * NCH;
@@ -122,13 +137,14 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
 
     // warp 0 issues the bulk copies of the chunk (tile ti, K-chunk kc) into slot s (lane = atom within the group)
     auto issue = [&](int ti, int kc, int s) {
-        const int64_t b0 = (int64_t)(ti / NSUB) * AB;
+        int b0, off0;
+        tile_origin(ti, b0, off0);
         const int nb = (int)((a.batch - b0 < AB) ? (a.batch - b0) : AB);
         float* dst = stages + (size_t)s * a.stage_floats;
         if (lane == 0) mbar_arrive_expect_tx(&full[s], chunk_bytes * (uint32_t)nb);
         __syncwarp();
         for (int al = lane; al < nb; al += 32)
-            tma_load_1d(dst + (size_t)al * chunk_floats, X + (b0 + al) * x_bs + (int64_t)kc * chunk_floats, chunk_bytes,
+            tma_load_1d(dst + (size_t)al * chunk_floats, X + ((int64_t)b0 + al) * x_bs + (int64_t)kc * chunk_floats, chunk_bytes,
                         &full[s]);
     };
 
@@ -188,11 +204,12 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
         produce();
 
         if (kc == 0) {
-            const int g = ti / NSUB, sub = ti - g * NSUB;
-            b0 = g * AB;
+            int off0;
+            tile_origin(ti, b0, off0);
             const int nb = (int)((a.batch - b0 < AB) ? (a.batch - b0) : AB);
             ncol = nb * J;
-            cbase = sub * CWT + wc * 128 + lane;
+            if (WIN && ncol > off0 + CWT) ncol = off0 + CWT;  // the columns beyond belong to the next tile
+            cbase = off0 + wc * 128 + lane;
 #pragma unroll
             for (int r = 0; r < 8; ++r)
 #pragma unroll
@@ -354,6 +371,44 @@ int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st
         }
     }
     if (best < 0.0) return CGTP_OK;
+    const int slots_total = pf_num_sms();
+
+    // Window tiles: a tile is CWT consecutive flattened (atom, j) columns, so every tile is full and atoms straddle
+    // tile boundaries; the stage then holds every atom the window touches (up to ABw).  Taken when it saves rounds of
+    // the persistent CTAs after charging the extra staging traffic (boundary atoms are staged by two tiles).
+    int window = 0;
+    {
+        const int ABw = (CWT + 2 * J - 2) / J;
+        int wKC = 0, wNS = 0;
+        for (int NS = 3; NS >= 2 && !wKC; --NS)
+            for (int i = 0; i < nkc; ++i)
+                if (kcs[i] >= 8 && 64 + wbytes + (size_t)NS * ABw * kcs[i] * x_rs * 4 <= budget) { wKC = kcs[i]; wNS = NS; break; }
+        if (wKC && batch * (int64_t)J >= 4 * (int64_t)CWT) {
+            const int nsub_g = (bAB * J + CWT - 1) / CWT;
+            const int64_t tiles_g = (batch + bAB - 1) / bAB * nsub_g;
+            const int64_t tiles_w = (batch * (int64_t)J + CWT - 1) / CWT;
+            int nrb_tot = 0;
+            for (int i = 0; i < nargs; ++i) nrb_tot += (args[i].M + MW - 1) / MW;
+            const int per = std::max(1, slots_total / std::max(1, nrb_tot));
+            // staging traffic per tile relative to the columns it computes: sub-tiles of a group re-stage the whole
+            // group (factor nsub), a window stages the atoms it straddles (factor ABw J / CWT).  Measured (configs[3]):
+            // the window pays off where it replaces sub-tiles (lmax = 16: 772 -> 588 us) and where it saves at least
+            // ~6 % of the rounds at a factor <= 1.4 (configs[1]); elsewhere the extra staging costs more than it saves
+            const double lf_g = nsub_g, lf_w = (double)ABw * J / CWT;
+            const int64_t rounds_g = (tiles_g + per - 1) / per, rounds_w = (tiles_w + per - 1) / per;
+            // sub-tiles of a group run on neighbouring CTAs at about the same time, so their re-staging is served by L2
+            // as long as the CTAs do not drift apart; with operands of several times the L2 size it is not
+            double xbytes = 0.0;
+            for (int i = 0; i < nargs; ++i) xbytes += (double)batch * args[i].K * x_rs * 4.0;
+            const bool beyond_l2 = xbytes > 4.0 * 126e6;
+            if ((nsub_g > 1 && lf_w < lf_g && beyond_l2) || (lf_w <= 1.4 && 1.05 * rounds_w < (double)rounds_g)) {
+                window = 1;
+                bAB = ABw;
+                bKC = wKC;
+                bNS = wNS;
+            }
+        }
+    }
 
     PfArgs a;
     a.nprob = nargs;
@@ -362,9 +417,10 @@ int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st
     a.AB = bAB;
     a.KC = bKC;
     a.NSTAGE = bNS;
-    a.NSUB = (bAB * J + CWT - 1) / CWT;
+    a.NSUB = window ? 1 : (bAB * J + CWT - 1) / CWT;
     a.stage_floats = bAB * bKC * x_rs;
     a.w_floats = maxK * MW;
+    a.window = window;
     a.jmagic = (uint32_t)((1ull << 32) / (uint64_t)J) + 1u;
     const size_t smem = 64 + wbytes + (size_t)bNS * a.stage_floats * 4;
     const int ctas_per_sm = 1;
@@ -378,9 +434,9 @@ int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st
         tot_rb += nrb[i];
         wsum += (double)nrb[i] * args[i].K;
     }
-    const int64_t ngroups = (batch + bAB - 1) / bAB;
-    const int64_t ntiles = ngroups * a.NSUB;
-    if (ntiles * 8 > 2147483647LL) return CGTP_OK;  // 32-bit tile / chunk counters in the kernel
+    const int64_t ntiles = window ? (batch * (int64_t)J + CWT - 1) / CWT : (batch + bAB - 1) / bAB * a.NSUB;
+    if (ntiles * 64 > 2147483647LL) return CGTP_OK;  // 32-bit tile / chunk counters in the kernel
+    a.ntiles = (int)ntiles;
     int begin = 0;
     for (int i = 0; i < nargs; ++i) {
         const ProjArgs& g = args[i];
@@ -401,8 +457,13 @@ int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st
 
     LaunchScope scope(kind, st);
     const bool acc = args[0].accumulate != 0;  // out += result (second pass of the parity-slot entry points)
-    void (*kern)(PfArgs) = wide ? (acc ? proj_fast_kernel<2, 4, true> : proj_fast_kernel<2, 4, false>)
-                                : (acc ? proj_fast_kernel<4, 2, true> : proj_fast_kernel<4, 2, false>);
+    void (*kern)(PfArgs);
+    if (window)
+        kern = wide ? (acc ? proj_fast_kernel<2, 4, true, true> : proj_fast_kernel<2, 4, false, true>)
+                    : (acc ? proj_fast_kernel<4, 2, true, true> : proj_fast_kernel<4, 2, false, true>);
+    else
+        kern = wide ? (acc ? proj_fast_kernel<2, 4, true, false> : proj_fast_kernel<2, 4, false, false>)
+                    : (acc ? proj_fast_kernel<4, 2, true, false> : proj_fast_kernel<4, 2, false, false>);
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<grid, kPfThreads, smem, st>>>(a);
     CGTP_CUDA_CHECK(cudaGetLastError());

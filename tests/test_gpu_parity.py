@@ -102,6 +102,16 @@ def test_onsite_config1_full():
     assert max(e) < TOL, e
 
 
+@pytest.mark.parametrize("lmax,N,C,batch", [(6, 64, 64, 4099), (5, 32, 32, 9001)])
+def test_onsite_window_tiles_ragged(lmax, N, C, batch):
+    """Projection tiles that are windows of the flattened (atom, lm) columns (proj_fast.cu): atoms straddle tile
+    boundaries and the last window is ragged; every output checked."""
+    inp = synthetic.make_onsite(lmax, lmax, N, C, batch, seed=610 + lmax)
+    got, ref = run_onsite(inp), oracle_onsite(inp)
+    e = sector_err(got, ref)
+    assert max(e) < TOL, e
+
+
 @pytest.mark.parametrize("lmax", [2, 4, 8, 12, 16, 20])
 def test_onsite_config3_sweep_sampled(lmax):
     """BASELINE.json configs[3]: N=C=32, batch=16384 on the GPU; the oracle evaluates a deterministic
