@@ -460,6 +460,8 @@ def run_message(args, cg, synthetic, dev, peaks, peak_src):
     import torch
     cu = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     res = {}
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    ncu_traffic = json.load(open(tp)) if os.path.exists(tp) else {}
     for name, idx, halfhalf in (("config2_all_even", 2, False), ("config2_half_odd", 2, True), ("config4", 4, True)):
         m = synthetic.config(idx)
         if idx == 2 and halfhalf:
@@ -497,7 +499,7 @@ def run_message(args, cg, synthetic, dev, peaks, peak_src):
                          "SURVEY.md 8(d)'s two-derivative-field gather for the odd channels",
             "roofline": {"kernel": dom, "bound": "hbm", "achieved": kern[dom].get("alg_gbs"),
                          "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": kern[dom].get("frac_hbm_peak"),
-                         "peak_source": peak_src, "traffic": None},
+                         "peak_source": peak_src, "traffic": ncu_traffic.get(f"config{idx}:{dom}") if halfhalf else None},
             "kernels": kern,
         }
         del X, ei, ev, er, out
