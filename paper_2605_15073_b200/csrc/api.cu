@@ -14,6 +14,7 @@ static const char* kKindNames[K_COUNT] = {
     "node_synth_odd", "edge_even",        "edge_odd",        "analysis_even", "analysis_odd",  "misc"};
 
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+static inline int64_t round_up64(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 struct Carver {
@@ -60,7 +61,8 @@ static size_t message_ws_bytes(int lmax, int lmax_out, int C, int Co, int64_t n_
     const int U = (2 * lmax + lmax_out + 2) / 2, V = 2 * lmax + lmax_out + 1;
     const size_t UVp = round_up(U * V, 4);
     // H, G (value grid, both parities) for the senders; S (two pooled grids per odd channel), T, row_ptr for the receivers
-    size_t fl = (size_t)n_send * C * (L2p + UVp) + (size_t)n_recv * ((C + Co) * UVp + (size_t)C * Lo2p);
+    // (H rows may use the odd stride of the fast synthesis, <= L2p + 1, with the columns padded to groups of 32)
+    size_t fl = ((size_t)n_send * C + 64) * (L2p + 4 + UVp) + (size_t)n_recv * ((C + Co) * UVp + (size_t)C * Lo2p);
     return 256 + fl * sizeof(float) + (size_t)(n_recv + 1) * sizeof(int64_t) + 12 * 256;
 }
 
@@ -228,8 +230,10 @@ static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_
     Carver cv(workspace);
     int32_t* status = cv.take<int32_t>(1);
     int64_t* row_ptr = cv.take<int64_t>((size_t)nodes + 1);
-    float* H_e = cv.take<float>((size_t)n_send * Ce * p->L2p);
-    float* H_o = cv.take<float>((size_t)n_send * Co * p->L2p);
+    const bool fast_synth = synth_fast_supported(p);
+    const int hstr = fast_synth ? synth_fast_hstride(p) : p->L2p;
+    float* H_e = cv.take<float>((size_t)round_up64(n_send * Ce, 32) * hstr);
+    float* H_o = cv.take<float>((size_t)round_up64(n_send * Co, 32) * hstr);
     float* G_e = cv.take<float>((size_t)n_send * Ce * p->UVp);
     float* G_o = cv.take<float>((size_t)n_send * Co * p->UVp);
     float* S_e = cv.take<float>((size_t)nodes * Ce * p->UVp);
@@ -258,20 +262,22 @@ static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_
     a.K = N;
     a.J = p->L2;
     a.out0 = H_e;
-    a.o_bs0 = (int64_t)Ce * p->L2p;
+    a.o_bs0 = (int64_t)Ce * hstr;
     a.out1 = H_o;
-    a.o_bs1 = (int64_t)Co * p->L2p;
+    a.o_bs1 = (int64_t)Co * hstr;
     a.m_split = Ce;
-    a.o_rs = p->L2p;
+    a.o_rs = hstr;
     a.batch = n_send;
     a.accumulate = 0;
     rc = launch_proj(&a, 1, K_PROJ_IN, st);
     if (rc) return rc;
 
     // M2 (value fields for both parities: the odd channels take their derivatives on the edge side and in M5)
-    rc = launch_node_synth(p, false, H_e, G_e, n_send * Ce, st);
+    rc = fast_synth ? launch_node_synth_fast(p, false, H_e, hstr, G_e, n_send * Ce, st)
+                    : launch_node_synth(p, false, H_e, G_e, n_send * Ce, st);
     if (rc) return rc;
-    rc = launch_node_synth(p, true, H_o, G_o, n_send * Co, st);
+    rc = fast_synth ? launch_node_synth_fast(p, true, H_o, hstr, G_o, n_send * Co, st)
+                    : launch_node_synth(p, true, H_o, G_o, n_send * Co, st);
     if (rc) return rc;
 
     // M3 + M4

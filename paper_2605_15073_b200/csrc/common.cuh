@@ -189,6 +189,11 @@ int launch_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int64_t
 // labels the launch for the profiler: the odd channels pair the edge's derivative fields with the sender's VALUE
 // field and move the derivatives onto Y_lm in the analysis).
 int launch_node_synth(const Plan* p, bool odd, const float* H, float* G, int64_t ncols, cudaStream_t st);
+// Lane = column form of M2 (sht_fast.cu) for band limits whose 32-column tile fits shared memory: H rows of stride
+// synth_fast_hstride(p) (odd), the H buffer padded to whole groups of 32 columns.
+bool synth_fast_supported(const Plan* p);
+inline int synth_fast_hstride(const Plan* p) { return p->L2 | 1; }
+int launch_node_synth_fast(const Plan* p, bool odd, const float* H, int hstride, float* G, int64_t ncols, cudaStream_t st);
 // M3+M4: channels of one parity.  even: S[i][kc][UVp] = sum_e R~ K_e G[send(e)];
 // odd: S[i][kc][2][UVp] = sum_e R~ (d_theta K_e, -(1/sin) d_phi K_e) G[send(e)].
 int launch_edge(const Plan* p, bool odd, const float* G, const int64_t* row_ptr, const int64_t* edge_index,
