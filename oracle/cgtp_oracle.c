@@ -34,8 +34,9 @@
  * real SH against scipy, whole-pipeline results against fine-grid quadrature, Wigner-D
  * equivariance, inversion parity, self-coupled vanishing, Parseval; the parity-slot functions
  * (oracle_*_parity) against the paper's dispatch check B7 (:647), the reduction to the natural-parity
- * functions, Eq.(44)-(45)/(56) slot rules, inversion and rotation.  No function here is
- * "parity unpinned".
+ * functions, Eq.(44)-(45)/(56) slot rules, inversion and rotation; the l-dependent-weight functions
+ * (oracle_*_lw) against the l-shared functions (equal weights, degree selection, per-degree numpy
+ * projections around them) and rotation.  No function here is "parity unpinned".
  *
  * Plain C99 + OpenMP, double precision (long double inside the Racah sum).
  */
@@ -665,6 +666,128 @@ int oracle_onsite_parity(const double *A, const double *B, const double *W_a, co
         }
         free(Ha); free(Hb); free(T);
     }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* l-dependent CP weights (the paper's own parameterisation: c_{cnl} in Eq.(35) :322 and Eq.(47)  */
+/* :398, lambda_c^{(nl)} in Eq.(41) :346 and Eq.(55) :427; reading R5 made them l-shared for the  */
+/* BASELINE configs).  W_a, W_b, W_node: [lmax+1, C, N]; W_out: [lmax_out+1, N, C]:               */
+/*   H[c,lm] = sum_n W[l][c,n] A[n,lm]          out[s,n,lm] = sum_{c in s} W_out[l][n,c] T[c,lm]  */
+/* The radial factor of the edge stays l1-shared (reading R12).  Everything else as oracle_onsite */
+/* / oracle_message.                                                                            */
+/* ------------------------------------------------------------------------------------------ */
+int oracle_onsite_lw(const double *A, const double *B, const double *W_a, const double *W_b,
+                     const double *W_out, int lmax, int lmax_out, int N, int C, const uint8_t *parity_mask,
+                     double *out, int64_t batch)
+{
+    int L2 = (lmax + 1) * (lmax + 1), Lo2 = (lmax_out + 1) * (lmax_out + 1);
+    const coupling_t *tab[2];
+    tab[0] = get_coupling(lmax, lmax_out, 0);
+    tab[1] = get_coupling(lmax, lmax_out, 1);
+    if (!tab[0] || !tab[1]) return 2;
+#pragma omp parallel
+    {
+        double *Ha = malloc((size_t)C * L2 * sizeof(double));
+        double *Hb = malloc((size_t)C * L2 * sizeof(double));
+        double *T = malloc((size_t)C * Lo2 * sizeof(double));
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t b = 0; b < batch; ++b) {
+            const double *Ab = A + b * (int64_t)N * L2, *Bb = B + b * (int64_t)N * L2;
+            for (int c = 0; c < C; ++c)
+                for (int i = 0; i < L2; ++i) {
+                    int l = isqrt_floor(i);
+                    double sa = 0.0, sb = 0.0;
+                    for (int n = 0; n < N; ++n) {
+                        sa += W_a[((size_t)l * C + c) * N + n] * Ab[n * L2 + i];
+                        sb += W_b[((size_t)l * C + c) * N + n] * Bb[n * L2 + i];
+                    }
+                    Ha[c * L2 + i] = sa;
+                    Hb[c * L2 + i] = sb;
+                }
+            for (int c = 0; c < C; ++c) {
+                const coupling_t *t = tab[parity_mask[c] ? 1 : 0];
+                double *Tc = T + (size_t)c * Lo2;
+                for (int i = 0; i < Lo2; ++i) Tc[i] = 0.0;
+                for (int64_t k = 0; k < t->nnz; ++k)
+                    Tc[t->io[k]] += t->val[k] * Ha[(size_t)c * L2 + t->i1[k]] * Hb[(size_t)c * L2 + t->i2[k]];
+            }
+            double *ob = out + b * 2 * (int64_t)N * Lo2;
+            for (int s = 0; s < 2; ++s)
+                for (int n = 0; n < N; ++n)
+                    for (int i = 0; i < Lo2; ++i) {
+                        int l = isqrt_floor(i);
+                        double acc = 0.0;
+                        for (int c = 0; c < C; ++c)
+                            if ((parity_mask[c] ? 1 : 0) == s)
+                                acc += W_out[((size_t)l * N + n) * C + c] * T[(size_t)c * Lo2 + i];
+                        ob[((size_t)s * N + n) * Lo2 + i] = acc;
+                    }
+        }
+        free(Ha); free(Hb); free(T);
+    }
+    return 0;
+}
+
+int oracle_message_lw(const double *node_feats, const int64_t *edge_index, const double *edge_vec,
+                      const double *edge_radial, const double *W_node, const double *W_out, int lmax,
+                      int lmax_out, int N, int C, const uint8_t *parity_mask, double *out, int64_t nodes,
+                      int64_t E)
+{
+    int L2 = (lmax + 1) * (lmax + 1), Lo2 = (lmax_out + 1) * (lmax_out + 1);
+    const coupling_t *tab[2];
+    tab[0] = get_coupling(lmax, lmax_out, 0);
+    tab[1] = get_coupling(lmax, lmax_out, 1);
+    if (!tab[0] || !tab[1]) return 2;
+    int64_t *row_ptr = malloc((size_t)(nodes + 1) * sizeof(int64_t));
+    int rc = oracle_segments(edge_index, E, nodes, row_ptr);
+    if (rc) { free(row_ptr); return rc; }
+    const int64_t *snd = edge_index;
+    double *H = malloc((size_t)(nodes > 0 ? nodes : 1) * C * L2 * sizeof(double));
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t j = 0; j < nodes; ++j) {
+        const double *xj = node_feats + j * (int64_t)N * L2;
+        double *hj = H + j * (int64_t)C * L2;
+        for (int c = 0; c < C; ++c)
+            for (int q = 0; q < L2; ++q) {
+                int l = isqrt_floor(q);
+                double s = 0.0;
+                for (int n = 0; n < N; ++n) s += W_node[((size_t)l * C + c) * N + n] * xj[n * L2 + q];
+                hj[c * L2 + q] = s;
+            }
+    }
+#pragma omp parallel
+    {
+        double *Y = malloc((size_t)L2 * sizeof(double));
+        double *T = malloc((size_t)C * Lo2 * sizeof(double));
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t i = 0; i < nodes; ++i) {
+            for (size_t k = 0; k < (size_t)C * Lo2; ++k) T[k] = 0.0;
+            for (int64_t e = row_ptr[i]; e < row_ptr[i + 1]; ++e) {
+                const double *hj = H + snd[e] * (int64_t)C * L2;
+                oracle_real_sh(lmax, edge_vec[3 * e], edge_vec[3 * e + 1], edge_vec[3 * e + 2], Y);
+                for (int c = 0; c < C; ++c) {
+                    double rad = edge_radial[e * (int64_t)C + c];
+                    const coupling_t *t = tab[parity_mask[c] ? 1 : 0];
+                    for (int64_t k = 0; k < t->nnz; ++k)
+                        T[(size_t)c * Lo2 + t->io[k]] += t->val[k] * rad * Y[t->i1[k]] * hj[(size_t)c * L2 + t->i2[k]];
+                }
+            }
+            double *ob = out + i * 2 * (int64_t)N * Lo2;
+            for (int s = 0; s < 2; ++s)
+                for (int n = 0; n < N; ++n)
+                    for (int q = 0; q < Lo2; ++q) {
+                        int l = isqrt_floor(q);
+                        double acc = 0.0;
+                        for (int c = 0; c < C; ++c)
+                            if ((parity_mask[c] ? 1 : 0) == s)
+                                acc += W_out[((size_t)l * N + n) * C + c] * T[(size_t)c * Lo2 + q];
+                        ob[((size_t)s * N + n) * Lo2 + q] = acc;
+                    }
+        }
+        free(Y); free(T);
+    }
+    free(H); free(row_ptr);
     return 0;
 }
 

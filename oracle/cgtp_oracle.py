@@ -64,6 +64,10 @@ def _load():
     lib.oracle_message_parity.argtypes = [p, p, p, p, p, p, p, i, i, i, i, p, i64, i64, p, i64]
     lib.oracle_onsite_parity.restype = i
     lib.oracle_onsite_parity.argtypes = [p, p, p, p, p, i, i, i, i, p, i64]
+    lib.oracle_onsite_lw.restype = i
+    lib.oracle_onsite_lw.argtypes = [p, p, p, p, p, i, i, i, i, p, p, i64]
+    lib.oracle_message_lw.restype = i
+    lib.oracle_message_lw.argtypes = [p, p, p, p, p, p, i, i, i, i, p, p, i64, i64]
     lib.oracle_num_threads.restype = i
     lib.oracle_num_threads.argtypes = []
     _lib = lib
@@ -222,6 +226,41 @@ def message_parity(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out,
                                        nr if rl is not None else 0)
     if rc:
         raise RuntimeError(f"oracle_message_parity failed with code {rc}")
+    return out
+
+
+def onsite_lw(A, B, W_a, W_b, W_out, lmax, lmax_out, parity_mask) -> np.ndarray:
+    """On-site contraction with l-dependent CP weights (Eq.(35), (41)): W_a, W_b [lmax+1, C, N], W_out [lmax_out+1, N, C]."""
+    A, B, W_a, W_b, W_out = map(_f64, (A, B, W_a, W_b, W_out))
+    batch, N, L2 = A.shape
+    C = W_a.shape[1]
+    assert L2 == (lmax + 1) ** 2 and B.shape == A.shape
+    assert W_a.shape == (lmax + 1, C, N) and W_b.shape == (lmax + 1, C, N) and W_out.shape == (lmax_out + 1, N, C)
+    mask = np.ascontiguousarray(np.asarray(parity_mask), dtype=np.uint8)
+    assert mask.shape == (C,)
+    out = np.zeros((batch, 2, N, (lmax_out + 1) ** 2), np.float64)
+    rc = _load().oracle_onsite_lw(_ptr(A), _ptr(B), _ptr(W_a), _ptr(W_b), _ptr(W_out), lmax, lmax_out, N, C,
+                                  _ptr(mask), _ptr(out), batch)
+    if rc:
+        raise RuntimeError(f"oracle_onsite_lw failed with code {rc}")
+    return out
+
+
+def message_lw(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, parity_mask) -> np.ndarray:
+    """Message passing with l-dependent node / output weights: W_node [lmax+1, C, N], W_out [lmax_out+1, N, C]."""
+    X, ev, er, W_node, W_out = map(_f64, (node_feats, edge_vec, edge_radial, W_node, W_out))
+    ei = np.ascontiguousarray(np.asarray(edge_index), dtype=np.int64)
+    nodes, N, L2 = X.shape
+    E = ei.shape[1]
+    C = W_node.shape[1]
+    assert L2 == (lmax + 1) ** 2 and ev.shape == (E, 3) and er.shape == (E, C)
+    assert W_node.shape == (lmax + 1, C, N) and W_out.shape == (lmax_out + 1, N, C)
+    mask = np.ascontiguousarray(np.asarray(parity_mask), dtype=np.uint8)
+    out = np.zeros((nodes, 2, N, (lmax_out + 1) ** 2), np.float64)
+    rc = _load().oracle_message_lw(_ptr(X), _ptr(ei), _ptr(ev), _ptr(er), _ptr(W_node), _ptr(W_out), lmax, lmax_out,
+                                   N, C, _ptr(mask), _ptr(out), nodes, E)
+    if rc:
+        raise RuntimeError(f"oracle_message_lw failed with code {rc}")
     return out
 
 

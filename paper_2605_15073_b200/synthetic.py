@@ -172,6 +172,19 @@ def make_message_parity(lmax: int, lmax_out: int, N: int, C: int, nodes: int, de
                                W_node, W_out, g.degree)
 
 
+# ---------------------------------------------------------------------------------------------
+# l-dependent CP weights (Eq.(35) :322, Eq.(41) :346, Eq.(47) :398): the same inputs as
+# make_onsite / make_message with one weight matrix per degree l.
+# ---------------------------------------------------------------------------------------------
+def lw_weights(lmax: int, lmax_out: int, N: int, C: int, seed: int, n_in: int = 2):
+    """n_in input weight stacks [lmax+1, C, N] ~ N(0, 1/sqrt(N)) and one output stack [lmax_out+1, N, C] ~ N(0, 1/sqrt(C))."""
+    rs = _streams(seed + 104729, n_in + 1)
+    w_in = [(r.standard_normal((lmax + 1, C, N), dtype=np.float32) / np.float32(np.sqrt(N))).astype(np.float32)
+            for r in rs[:n_in]]
+    w_out = (rs[n_in].standard_normal((lmax_out + 1, N, C), dtype=np.float32) / np.float32(np.sqrt(C))).astype(np.float32)
+    return w_in, w_out
+
+
 # BASELINE.json configs (index = position in BASELINE.json "configs").
 def config(idx: int, lmax: int | None = None, seed: int = 0):
     if idx == 0:
