@@ -11,7 +11,7 @@ product / surface-curl pairing, analysis, output projection) over one batch of B
 
 Prints ONE JSON line on rank 0.  Extra objects on the line (N=1 only): "sweep" (configs[3], on-site vs
 lmax), "message" (configs[2] and configs[4], edges/s and HBM GB/s), "kernels" (per-kernel shares), "parity"
-(parity-labelled inputs: cost of the full dispatch against one Category-alpha run).
+(parity-labelled inputs: cost of the full dispatch against one Category-alpha run), "l_dependent_weights".
 """
 from __future__ import annotations
 
@@ -352,6 +352,7 @@ def main():
         line["sweep"] = run_sweep(args, cg, synthetic, dev, fp32_peak_tflops, peaks)
         line["message"] = run_message(args, cg, synthetic, dev, peaks, peak_src)
         line["parity"] = run_parity(args, cg, synthetic, dev)
+        line["l_dependent_weights"] = run_lw(args, cg, synthetic, dev, ms_per_step)
     elif world == 1:
         rate, dt_cpu, cores = oracle_onsite_rate(base, 1024)
         line["cpu_baseline"] = {"value": rate, "unit": "contractions/s", "cores": cores, "kind": "oracle",
@@ -539,6 +540,30 @@ def run_parity(args, cg, synthetic, dev):
                       "ms_per_step": ms, "edges_per_s": m.E / (ms * 1e-3), "alpha_run_ms": ms1,
                       "factor_vs_alpha_run": ms / ms1, "paper_upper_bound": 12}
     return res
+
+
+def run_lw(args, cg, synthetic, dev, shared_ms):
+    """l-dependent CP weights (Eq.(35), Eq.(41) :346): configs[1] with one weight
+    matrix per degree; the channel projections run once per degree."""
+    import torch
+    cu = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    inp = synthetic.config(1)
+    (Wa, Wb), Wo = synthetic.lw_weights(inp.lmax, inp.lmax_out, inp.N, inp.C, seed=0)
+    A, B, Wa, Wb, Wo = cu(inp.A), cu(inp.B), cu(Wa), cu(Wb), cu(Wo)
+    out = torch.empty((inp.batch, 2, inp.N, (inp.lmax_out + 1) ** 2), device=dev)
+    fn = lambda: cg.cgtp_onsite_lw(A, B, Wa, Wb, Wo, inp.lmax, inp.lmax_out, inp.N, inp.C, inp.parity_mask, out=out)
+    ms = time_steps(fn, 20, 3)
+    cg.cgtp_profile_enable(True)
+    for _ in range(10):
+        fn()
+    torch.cuda.synchronize()
+    prof = cg.cgtp_profile_collect()
+    cg.cgtp_profile_enable(False)
+    return {"workload": "BASELINE.json configs[1] with W_a, W_b [7, 64, 64] and W_out [7, 64, 64] (one matrix per degree)",
+            "ms_per_step": ms, "contractions_per_s": inp.batch / (ms * 1e-3), "l_shared_ms_per_step": shared_ms,
+            "factor_vs_l_shared": ms / shared_ms,
+            "kernel_ms": {k: v[0] / 10 for k, v in prof.items()},
+            "launches_per_step": int(sum(v[1] for v in prof.values()) // 10)}
 
 
 if __name__ == "__main__":

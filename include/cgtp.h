@@ -186,6 +186,24 @@ int cgtp_message_parity(const float* node_feats, const int64_t* edge_index, cons
                         void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * l-dependent CP weights, the paper's own parameterisation (c_{cnl} in Eq.(35) PAPER.md:322 and Eq.(47) :398,
+ * lambda_c^{(nl)} in Eq.(41) :346 and Eq.(55) :427; cgtp_onsite / cgtp_message take one matrix for all degrees):
+ *   H[b,c,lm] = sum_n W[l][c,n] A[b,n,lm]         out[b,s,n,lm] = sum_{c: mask[c]=s} W_out[l][n,c] T[b,c,lm]
+ *   W_a, W_b, W_node  device [lmax+1, C, N]        W_out  device [lmax_out+1, N, C]
+ * The radial factor of the edge stays l1-shared, edge_radial [E, C].  Every other argument, the workspace size
+ * (cgtp_onsite_workspace_bytes / cgtp_message_workspace_bytes) and the error behaviour are those of cgtp_onsite /
+ * cgtp_message.  The channel projections run once per degree l over the coefficient columns l^2 .. l^2 + 2l.
+ * ------------------------------------------------------------------------------------------- */
+int cgtp_onsite_lw(const float* A, const float* B, const float* W_a, const float* W_b, const float* W_out,
+                   int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask, float* out,
+                   int64_t batch, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+int cgtp_message_lw(const float* node_feats, const int64_t* edge_index, const float* edge_vec,
+                    const float* edge_radial, const float* W_node, const float* W_out,
+                    int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask, float* out,
+                    int64_t nodes, int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Host-buffer entry points (end-to-end path): same semantics as cgtp_onsite / cgtp_message, but
  * every tensor pointer is HOST memory (pinned memory recommended; pageable works, slower).  The
  * library allocates device memory from the CUDA stream-ordered pool, copies inputs host->device in

@@ -62,6 +62,10 @@ def lib() -> ctypes.CDLL:
     L.cgtp_message_parity_workspace_bytes.argtypes = [i, i, i, i, i64, i64]
     L.cgtp_message_parity.restype = i
     L.cgtp_message_parity.argtypes = [vp, vp, vp, vp, vp, vp, i, i, i, i, vp, i64, i64, vp, sz, vp]
+    L.cgtp_onsite_lw.restype = i
+    L.cgtp_onsite_lw.argtypes = L.cgtp_onsite.argtypes
+    L.cgtp_message_lw.restype = i
+    L.cgtp_message_lw.argtypes = L.cgtp_message.argtypes
     L.cgtp_message_status.restype = i
     L.cgtp_message_status.argtypes = [vp, vp]
     L.cgtp_build_segments.restype = i
@@ -306,6 +310,68 @@ def cgtp_message_parity(node_feats, edge_index, edge_vec, edge_radial, W_node, W
         rc = lib().cgtp_message_parity(X.data_ptr(), ei.data_ptr(), ev.data_ptr(), er.data_ptr(), W_node.data_ptr(),
                                        W_out.data_ptr(), lmax, lmax_out, N, C, out.data_ptr(), nodes, E,
                                        ws.data_ptr(), ws.numel(), sp)
+        _check(rc)
+        if check:
+            _check(lib().cgtp_message_status(ws.data_ptr(), sp))
+    return out
+
+
+def cgtp_onsite_lw(A, B, W_a, W_b, W_out, lmax, lmax_out, N, C, parity_mask, out=None, workspace=None, stream=None):
+    """cgtp_onsite with l-dependent CP weights: W_a, W_b [lmax+1, C, N], W_out [lmax_out+1, N, C] (see include/cgtp.h)."""
+    f32 = torch.float32
+    A, B = _dev(A, f32, "A"), _dev(B, f32, "B")
+    W_a, W_b, W_out = _dev(W_a, f32, "W_a"), _dev(W_b, f32, "W_b"), _dev(W_out, f32, "W_out")
+    batch = A.shape[0]
+    L2, Lo2 = (lmax + 1) ** 2, (lmax_out + 1) ** 2
+    if tuple(A.shape) != (batch, N, L2) or tuple(B.shape) != (batch, N, L2):
+        raise ValueError("A, B must be [batch, N, (lmax+1)^2]")
+    if tuple(W_a.shape) != (lmax + 1, C, N) or tuple(W_b.shape) != (lmax + 1, C, N) or tuple(W_out.shape) != (lmax_out + 1, N, C):
+        raise ValueError("W_a, W_b must be [lmax+1, C, N] and W_out [lmax_out+1, N, C]")
+    mask = _mask(parity_mask, C)
+    if out is None:
+        out = torch.empty((batch, 2, N, Lo2), dtype=f32, device=A.device)
+    else:
+        _dev(out, f32, "out")
+        if tuple(out.shape) != (batch, 2, N, Lo2):
+            raise ValueError("out must be [batch, 2, N, (lmax_out+1)^2]")
+    nbytes = cgtp_onsite_workspace_bytes(lmax, lmax_out, N, C, batch)
+    ws = _workspace(A.device, nbytes) if workspace is None else workspace
+    with torch.cuda.device(A.device):
+        rc = lib().cgtp_onsite_lw(A.data_ptr(), B.data_ptr(), W_a.data_ptr(), W_b.data_ptr(), W_out.data_ptr(),
+                                  lmax, lmax_out, N, C, mask.ctypes.data, out.data_ptr(), batch,
+                                  ws.data_ptr(), ws.numel(), _stream_ptr(stream))
+    _check(rc)
+    return out
+
+
+def cgtp_message_lw(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, N, C, parity_mask,
+                    out=None, workspace=None, stream=None, check: bool = False):
+    """cgtp_message with l-dependent weights: W_node [lmax+1, C, N], W_out [lmax_out+1, N, C] (see include/cgtp.h)."""
+    f32 = torch.float32
+    X = _dev(node_feats, f32, "node_feats")
+    ei = _dev(edge_index, torch.int64, "edge_index")
+    ev, er = _dev(edge_vec, f32, "edge_vec"), _dev(edge_radial, f32, "edge_radial")
+    W_node, W_out = _dev(W_node, f32, "W_node"), _dev(W_out, f32, "W_out")
+    nodes, E = X.shape[0], ei.shape[1]
+    L2, Lo2 = (lmax + 1) ** 2, (lmax_out + 1) ** 2
+    if tuple(X.shape) != (nodes, N, L2):
+        raise ValueError("node_feats must be [nodes, N, (lmax+1)^2]")
+    if tuple(ei.shape) != (2, E) or tuple(ev.shape) != (E, 3) or tuple(er.shape) != (E, C):
+        raise ValueError("edge_index [2,E], edge_vec [E,3], edge_radial [E,C] expected")
+    if tuple(W_node.shape) != (lmax + 1, C, N) or tuple(W_out.shape) != (lmax_out + 1, N, C):
+        raise ValueError("W_node must be [lmax+1, C, N] and W_out [lmax_out+1, N, C]")
+    mask = _mask(parity_mask, C)
+    if out is None:
+        out = torch.empty((nodes, 2, N, Lo2), dtype=f32, device=X.device)
+    else:
+        _dev(out, f32, "out")
+    nbytes = lib().cgtp_message_workspace_bytes(lmax, lmax_out, N, C, mask.ctypes.data, nodes, E)
+    ws = _workspace(X.device, nbytes) if workspace is None else workspace
+    sp = _stream_ptr(stream)
+    with torch.cuda.device(X.device):
+        rc = lib().cgtp_message_lw(X.data_ptr(), ei.data_ptr(), ev.data_ptr(), er.data_ptr(), W_node.data_ptr(),
+                                   W_out.data_ptr(), lmax, lmax_out, N, C, mask.ctypes.data, out.data_ptr(), nodes, E,
+                                   ws.data_ptr(), ws.numel(), sp)
         _check(rc)
         if check:
             _check(lib().cgtp_message_status(ws.data_ptr(), sp))

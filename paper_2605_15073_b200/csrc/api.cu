@@ -83,6 +83,8 @@ struct OnsitePass {
     int accumulate;       // 1: add to the output sectors
     int sigma_C;          // 0: none; > 0: channel k keeps only the output degrees l with (l & 1) == ((k / sigma_C) & 1)
                           // inside its parity block (Eq.(54): (-1)^l = sigma)
+    int64_t lw_in, lw_out;  // 0: l-shared weights; else floats between the weight matrices of consecutive degrees l
+                          // (c_{cnl} of Eq.(35) :322, lambda_c^{(nl)} of Eq.(41) :346): S1 / S5 run once per degree
 };
 
 static int onsite_pass(const Plan* p, int N, const OnsitePass& q, int64_t batch, void* workspace, cudaStream_t st)
@@ -115,32 +117,38 @@ static int onsite_pass(const Plan* p, int N, const OnsitePass& q, int64_t batch,
         }
     }
 
-    // S1: H = W . A (Eq.(35)); rows are written in parity-sorted channel order, even block then odd block
-    ProjArgs pin[2];
-    for (int s = 0; s < 2; ++s) {
-        ProjArgs& a = pin[s];
-        a.X = s ? q.B : q.A;
-        a.x_bs = q.x_bs;
-        a.x_rs = p->L2;
-        a.W = s ? q.W_b : q.W_a;
-        a.ldw_m = N;
-        a.ldw_k = 1;
-        a.idx_m = q.idx_in;
-        a.idx_k = nullptr;
-        a.M = Ce + Co;
-        a.K = N;
-        a.J = p->L2;
-        a.out0 = s ? Hb_e : Ha_e;
-        a.o_bs0 = (int64_t)Ce * hstr;
-        a.out1 = s ? Hb_o : Ha_o;
-        a.o_bs1 = (int64_t)Co * hstr;
-        a.m_split = Ce;
-        a.o_rs = hstr;
-        a.batch = batch;
-        a.accumulate = 0;
+    // S1: H = W . A (Eq.(35)); rows are written in parity-sorted channel order, even block then odd block.  With
+    // l-dependent weights one launch per degree l over the columns l^2 .. l^2 + 2l of every row.
+    int rc = CGTP_OK;
+    for (int l = 0; l < (q.lw_in ? p->lmax + 1 : 1); ++l) {
+        ProjArgs pin[2];
+        for (int s = 0; s < 2; ++s) {
+            ProjArgs& a = pin[s];
+            const int jo = q.lw_in ? l * l : 0;
+            a.X = s ? q.B : q.A;
+            a.x_bs = q.x_bs;
+            a.x_rs = p->L2;
+            a.W = (s ? q.W_b : q.W_a) + (size_t)l * q.lw_in;
+            a.ldw_m = N;
+            a.ldw_k = 1;
+            a.idx_m = q.idx_in;
+            a.idx_k = nullptr;
+            a.M = Ce + Co;
+            a.K = N;
+            a.J = q.lw_in ? 2 * l + 1 : p->L2;
+            a.out0 = (s ? Hb_e : Ha_e) + jo;
+            a.o_bs0 = (int64_t)Ce * hstr;
+            a.out1 = (s ? Hb_o : Ha_o) + jo;
+            a.o_bs1 = (int64_t)Co * hstr;
+            a.m_split = Ce;
+            a.o_rs = hstr;
+            a.batch = batch;
+            a.accumulate = 0;
+            a.j0 = jo;
+        }
+        rc = launch_proj(pin, 2, K_PROJ_IN, st);
+        if (rc) return rc;
     }
-    int rc = launch_proj(pin, 2, K_PROJ_IN, st);
-    if (rc) return rc;
 
     // S2-S4 fused, one launch per parity
     rc = fast ? launch_onsite_fast(p, false, Ha_e, Hb_e, T_e, batch * Ce, st)
@@ -156,31 +164,37 @@ static int onsite_pass(const Plan* p, int N, const OnsitePass& q, int64_t batch,
         if (rc) return rc;
     }
 
-    // S5: out[b, s] = W_out[:, channels of sector s] . T_s (Eq.(41))
-    ProjArgs po[2];
-    for (int s = 0; s < 2; ++s) {
-        ProjArgs& a = po[s];
-        a.X = s ? T_o : T_e;
-        a.x_bs = (int64_t)(s ? Co : Ce) * tstr;
-        a.x_rs = tstr;
-        a.W = q.W_out;
-        a.ldw_m = q.ldw_out;
-        a.ldw_k = 1;
-        a.idx_m = nullptr;
-        a.idx_k = s ? q.idx_out_o : q.idx_out_e;
-        a.M = N;
-        a.K = s ? Co : Ce;
-        a.J = p->Lo2;
-        a.out0 = s ? q.out_o : q.out_e;
-        a.o_bs0 = q.o_bs;
-        a.out1 = a.out0;
-        a.o_bs1 = a.o_bs0;
-        a.m_split = N;
-        a.o_rs = p->Lo2;
-        a.batch = batch;
-        a.accumulate = q.accumulate;
+    // S5: out[b, s] = W_out[:, channels of sector s] . T_s (Eq.(41)); per degree with l-dependent weights
+    for (int l = 0; l < (q.lw_out ? p->lmax_out + 1 : 1); ++l) {
+        ProjArgs po[2];
+        for (int s = 0; s < 2; ++s) {
+            ProjArgs& a = po[s];
+            const int jo = q.lw_out ? l * l : 0;
+            a.X = s ? T_o : T_e;
+            a.x_bs = (int64_t)(s ? Co : Ce) * tstr;
+            a.x_rs = tstr;
+            a.W = q.W_out + (size_t)l * q.lw_out;
+            a.ldw_m = q.ldw_out;
+            a.ldw_k = 1;
+            a.idx_m = nullptr;
+            a.idx_k = s ? q.idx_out_o : q.idx_out_e;
+            a.M = N;
+            a.K = s ? Co : Ce;
+            a.J = q.lw_out ? 2 * l + 1 : p->Lo2;
+            a.out0 = (s ? q.out_o : q.out_e) + jo;
+            a.o_bs0 = q.o_bs;
+            a.out1 = a.out0;
+            a.o_bs1 = a.o_bs0;
+            a.m_split = N;
+            a.o_rs = p->Lo2;
+            a.batch = batch;
+            a.accumulate = q.accumulate;
+            a.j0 = jo;
+        }
+        rc = launch_proj(po, 2, K_PROJ_OUT, st);
+        if (rc) return rc;
     }
-    return launch_proj(po, 2, K_PROJ_OUT, st);
+    return CGTP_OK;
 }
 
 static int check_message_args(const float* node_feats, const int64_t* edge_index, const float* edge_vec,
@@ -221,6 +235,7 @@ struct MessagePass {
     int accumulate;
     int sigma_C;              // as OnsitePass::sigma_C
     bool segments_done;       // row_ptr / status of this workspace are already built (second pass)
+    int64_t lw_in, lw_out;    // as OnsitePass: l-dependent W_node (Eq.(47) :398) / W_out (Eq.(55), (58))
 };
 
 static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_t* edge_index, const float* edge_vec,
@@ -248,29 +263,33 @@ static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_
         if (rc) return rc;
     }
 
-    // M1: H = W_node . node_feats (Eq.(47))
-    ProjArgs a;
-    a.X = q.node_feats;
-    a.x_bs = q.x_bs;
-    a.x_rs = p->L2;
-    a.W = q.W_node;
-    a.ldw_m = N;
-    a.ldw_k = 1;
-    a.idx_m = q.idx_in;
-    a.idx_k = nullptr;
-    a.M = Ce + Co;
-    a.K = N;
-    a.J = p->L2;
-    a.out0 = H_e;
-    a.o_bs0 = (int64_t)Ce * hstr;
-    a.out1 = H_o;
-    a.o_bs1 = (int64_t)Co * hstr;
-    a.m_split = Ce;
-    a.o_rs = hstr;
-    a.batch = n_send;
-    a.accumulate = 0;
-    rc = launch_proj(&a, 1, K_PROJ_IN, st);
-    if (rc) return rc;
+    // M1: H = W_node . node_feats (Eq.(47)); one launch per degree with l-dependent weights
+    for (int l = 0; l < (q.lw_in ? p->lmax + 1 : 1); ++l) {
+        const int jo = q.lw_in ? l * l : 0;
+        ProjArgs a;
+        a.X = q.node_feats;
+        a.x_bs = q.x_bs;
+        a.x_rs = p->L2;
+        a.W = q.W_node + (size_t)l * q.lw_in;
+        a.ldw_m = N;
+        a.ldw_k = 1;
+        a.idx_m = q.idx_in;
+        a.idx_k = nullptr;
+        a.M = Ce + Co;
+        a.K = N;
+        a.J = q.lw_in ? 2 * l + 1 : p->L2;
+        a.out0 = H_e + jo;
+        a.o_bs0 = (int64_t)Ce * hstr;
+        a.out1 = H_o + jo;
+        a.o_bs1 = (int64_t)Co * hstr;
+        a.m_split = Ce;
+        a.o_rs = hstr;
+        a.batch = n_send;
+        a.accumulate = 0;
+        a.j0 = jo;
+        rc = launch_proj(&a, 1, K_PROJ_IN, st);
+        if (rc) return rc;
+    }
 
     // M2 (value fields for both parities: the odd channels take their derivatives on the edge side and in M5)
     rc = fast_synth ? launch_node_synth_fast(p, false, H_e, hstr, G_e, n_send * Ce, st)
@@ -298,31 +317,37 @@ static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_
         if (rc) return rc;
     }
 
-    // M6
-    ProjArgs po[2];
-    for (int s = 0; s < 2; ++s) {
-        ProjArgs& b = po[s];
-        b.X = s ? T_o : T_e;
-        b.x_bs = (int64_t)(s ? Co : Ce) * p->Lo2p;
-        b.x_rs = p->Lo2p;
-        b.W = q.W_out;
-        b.ldw_m = q.ldw_out;
-        b.ldw_k = 1;
-        b.idx_m = nullptr;
-        b.idx_k = s ? q.idx_out_o : q.idx_out_e;
-        b.M = N;
-        b.K = s ? Co : Ce;
-        b.J = p->Lo2;
-        b.out0 = s ? q.out_o : q.out_e;
-        b.o_bs0 = q.o_bs;
-        b.out1 = b.out0;
-        b.o_bs1 = b.o_bs0;
-        b.m_split = N;
-        b.o_rs = p->Lo2;
-        b.batch = nodes;
-        b.accumulate = q.accumulate;
+    // M6 (per degree with l-dependent weights)
+    for (int l = 0; l < (q.lw_out ? p->lmax_out + 1 : 1); ++l) {
+        const int jo = q.lw_out ? l * l : 0;
+        ProjArgs po[2];
+        for (int s = 0; s < 2; ++s) {
+            ProjArgs& b = po[s];
+            b.X = s ? T_o : T_e;
+            b.x_bs = (int64_t)(s ? Co : Ce) * p->Lo2p;
+            b.x_rs = p->Lo2p;
+            b.W = q.W_out + (size_t)l * q.lw_out;
+            b.ldw_m = q.ldw_out;
+            b.ldw_k = 1;
+            b.idx_m = nullptr;
+            b.idx_k = s ? q.idx_out_o : q.idx_out_e;
+            b.M = N;
+            b.K = s ? Co : Ce;
+            b.J = q.lw_out ? 2 * l + 1 : p->Lo2;
+            b.out0 = (s ? q.out_o : q.out_e) + jo;
+            b.o_bs0 = q.o_bs;
+            b.out1 = b.out0;
+            b.o_bs1 = b.o_bs0;
+            b.m_split = N;
+            b.o_rs = p->Lo2;
+            b.batch = nodes;
+            b.accumulate = q.accumulate;
+            b.j0 = jo;
+        }
+        rc = launch_proj(po, 2, K_PROJ_OUT, st);
+        if (rc) return rc;
     }
-    return launch_proj(po, 2, K_PROJ_OUT, st);
+    return CGTP_OK;
 }
 
 }  // namespace cgtp
@@ -350,9 +375,9 @@ size_t cgtp_onsite_workspace_bytes(int lmax, int lmax_out, int N, int C, int64_t
     return onsite_ws_bytes(lmax, lmax_out, C, batch);
 }
 
-int cgtp_onsite(const float* A, const float* B, const float* W_a, const float* W_b, const float* W_out, int lmax,
-                int lmax_out, int N, int C, const uint8_t* parity_mask, float* out, int64_t batch, void* workspace,
-                size_t workspace_bytes, void* cuda_stream)
+static int onsite_entry(bool lw, const float* A, const float* B, const float* W_a, const float* W_b, const float* W_out,
+                        int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask, float* out, int64_t batch,
+                        void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     clear_error();
     int rc = check_common(lmax, lmax_out, N, C, parity_mask);
@@ -392,6 +417,8 @@ int cgtp_onsite(const float* A, const float* B, const float* W_a, const float* W
     q.o_bs = (int64_t)2 * N * p->Lo2;
     q.accumulate = 0;
     q.sigma_C = 0;
+    q.lw_in = lw ? (int64_t)C * N : 0;
+    q.lw_out = lw ? (int64_t)N * C : 0;
     return onsite_pass(p, N, q, batch, workspace, st);
 }
 
@@ -426,10 +453,10 @@ int cgtp_build_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int
     return launch_segments(edge_index, E, nodes, nodes, row_ptr, status, static_cast<cudaStream_t>(cuda_stream));
 }
 
-int cgtp_message_bipartite(const float* node_feats, const int64_t* edge_index, const float* edge_vec,
-                           const float* edge_radial, const float* W_node, const float* W_out, int lmax, int lmax_out,
-                           int N, int C, const uint8_t* parity_mask, float* out, int64_t n_send, int64_t nodes,
-                           int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream)
+static int message_entry(bool lw, const float* node_feats, const int64_t* edge_index, const float* edge_vec,
+                         const float* edge_radial, const float* W_node, const float* W_out, int lmax, int lmax_out,
+                         int N, int C, const uint8_t* parity_mask, float* out, int64_t n_send, int64_t nodes,
+                         int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     clear_error();
     int rc = check_common(lmax, lmax_out, N, C, parity_mask);
@@ -465,7 +492,43 @@ int cgtp_message_bipartite(const float* node_feats, const int64_t* edge_index, c
     q.accumulate = 0;
     q.sigma_C = 0;
     q.segments_done = false;
+    q.lw_in = lw ? (int64_t)C * N : 0;
+    q.lw_out = lw ? (int64_t)N * C : 0;
     return message_pass(p, N, q, edge_index, edge_vec, n_send, nodes, E, workspace, st);
+}
+
+int cgtp_onsite(const float* A, const float* B, const float* W_a, const float* W_b, const float* W_out, int lmax,
+                int lmax_out, int N, int C, const uint8_t* parity_mask, float* out, int64_t batch, void* workspace,
+                size_t workspace_bytes, void* cuda_stream)
+{
+    return onsite_entry(false, A, B, W_a, W_b, W_out, lmax, lmax_out, N, C, parity_mask, out, batch, workspace,
+                        workspace_bytes, cuda_stream);
+}
+
+int cgtp_onsite_lw(const float* A, const float* B, const float* W_a, const float* W_b, const float* W_out, int lmax,
+                   int lmax_out, int N, int C, const uint8_t* parity_mask, float* out, int64_t batch, void* workspace,
+                   size_t workspace_bytes, void* cuda_stream)
+{
+    return onsite_entry(true, A, B, W_a, W_b, W_out, lmax, lmax_out, N, C, parity_mask, out, batch, workspace,
+                        workspace_bytes, cuda_stream);
+}
+
+int cgtp_message_bipartite(const float* node_feats, const int64_t* edge_index, const float* edge_vec,
+                           const float* edge_radial, const float* W_node, const float* W_out, int lmax, int lmax_out,
+                           int N, int C, const uint8_t* parity_mask, float* out, int64_t n_send, int64_t nodes,
+                           int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    return message_entry(false, node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, N, C,
+                         parity_mask, out, n_send, nodes, E, workspace, workspace_bytes, cuda_stream);
+}
+
+int cgtp_message_lw(const float* node_feats, const int64_t* edge_index, const float* edge_vec, const float* edge_radial,
+                    const float* W_node, const float* W_out, int lmax, int lmax_out, int N, int C,
+                    const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* workspace,
+                    size_t workspace_bytes, void* cuda_stream)
+{
+    return message_entry(true, node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, N, C,
+                         parity_mask, out, nodes, nodes, E, workspace, workspace_bytes, cuda_stream);
 }
 
 int cgtp_message(const float* node_feats, const int64_t* edge_index, const float* edge_vec, const float* edge_radial,
@@ -548,6 +611,7 @@ int cgtp_onsite_parity(const float* A, const float* B, const float* W_a, const f
         q.o_bs = (int64_t)2 * sector;
         q.accumulate = ps > 0;  // pass (0,0) writes both sectors, the others add to them
         q.sigma_C = C;
+        q.lw_in = q.lw_out = 0;
         rc = onsite_pass(p, N, q, batch, workspace, st);
         if (rc) return rc;
     }
@@ -605,6 +669,7 @@ int cgtp_message_parity(const float* node_feats, const int64_t* edge_index, cons
         q.accumulate = s_in > 0;
         q.sigma_C = C;
         q.segments_done = s_in > 0;
+        q.lw_in = q.lw_out = 0;
         rc = message_pass(p, N, q, edge_index, edge_vec, nodes, nodes, E, workspace, st);
         if (rc) return rc;
     }

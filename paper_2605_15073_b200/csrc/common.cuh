@@ -157,6 +157,8 @@ struct ProjArgs {
     int o_rs;
     int64_t batch;
     int accumulate;  // 1: add to the output instead of overwriting it (second pass of the parity-slot entry points)
+    int j0;          // first column of every X row that is used: X[.. + j0 + j], j < J (l-dependent weights: one degree l
+                     // per launch, j0 = l^2, J = 2l+1); the output pointers are given already offset by the caller
 };
 int launch_proj(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st);
 // Fast path of launch_proj (proj_fast.cu): TMA-staged features, packed FP32 FMAs; *handled = false when the

@@ -154,7 +154,9 @@ int launch_proj(const ProjArgs* args_in, int nargs_in, Kind kind, cudaStream_t s
     }
     if (nargs == 1) pack.a[1] = args[0];
     if (max_cols == 0 || max_m == 0) return CGTP_OK;
-    {
+    bool offset = false;
+    for (int i = 0; i < nargs; ++i) offset = offset || args[i].j0 != 0;
+    if (!offset) {
         bool handled = false;
         const int rc = launch_proj_tc(args, nargs, kind, st, &handled);
         if (rc != CGTP_OK || handled) return rc;
@@ -163,6 +165,10 @@ int launch_proj(const ProjArgs* args_in, int nargs_in, Kind kind, cudaStream_t s
         bool handled = false;
         const int rc = launch_proj_fast(args, nargs, kind, st, &handled);
         if (rc != CGTP_OK || handled) return rc;
+    }
+    for (int i = 0; i < 2; ++i) {  // the generic kernel loads scalars: fold the column offset into the pointer
+        pack.a[i].X += pack.a[i].j0;
+        pack.a[i].j0 = 0;
     }
     constexpr int TM = 8, TN = 8;
     const int CW = 32 * TN;

@@ -37,6 +37,7 @@ struct PfProblem {
     int64_t o_bs1;
     int m_split;
     int o_rs;
+    int j0;        // first used column of every X row
     int nrb;       // row blocks of this problem
     int cta_begin; // first CTA (blockIdx.x) serving this problem
     int ctas_per_rb;
@@ -97,6 +98,7 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
     const int M = pi ? a.p[1].M : a.p[0].M;
     const int K = pi ? a.p[1].K : a.p[0].K;
     const int cpr = pi ? a.p[1].ctas_per_rb : a.p[0].ctas_per_rb;
+    const int j0 = pi ? a.p[1].j0 : a.p[0].j0;
     const int local = blockIdx.x - (pi ? a.p[1].cta_begin : 0);
     const int rb = local / cpr, rank = local - rb * cpr;
     const int m0 = rb * MW;
@@ -218,7 +220,7 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
             for (int t = 0; t < 4; ++t) {
                 const int cc = cbase + 32 * t;
                 const int al = (J == 1) ? cc : (int)__umulhi((uint32_t)cc, jmagic);
-                xoff[t] = (cc < ncol) ? 4 * (al * chunk_floats + (cc - al * J)) : 0;  // bytes
+                xoff[t] = (cc < ncol) ? 4 * (al * chunk_floats + j0 + (cc - al * J)) : 0;  // bytes
             }
         }
         mbar_wait(&full[s], phase);
@@ -325,7 +327,7 @@ int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st
     for (int i = 0; i < nargs; ++i) {
         const ProjArgs& g = args[i];
         if (g.J != J || g.batch != batch || g.x_rs != args[0].x_rs || g.accumulate != args[0].accumulate) return CGTP_OK;
-        if (g.K < 2 || (g.K & 1) || g.M < 1 || g.x_rs < J) return CGTP_OK;
+        if (g.K < 2 || (g.K & 1) || g.M < 1 || g.x_rs < g.j0 + J || g.j0 < 0) return CGTP_OK;
         if (!al16(g.X) || (g.x_bs & 3)) return CGTP_OK;
         maxM = std::max(maxM, g.M);
         maxK = std::max(maxK, g.K);
@@ -442,7 +444,7 @@ int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st
         const ProjArgs& g = args[i];
         PfProblem& q = a.p[i];
         q.X = g.X; q.x_bs = g.x_bs; q.x_rs = g.x_rs; q.W = g.W; q.ldw_m = g.ldw_m; q.ldw_k = g.ldw_k;
-        q.idx_m = g.idx_m; q.idx_k = g.idx_k; q.M = g.M; q.K = g.K;
+        q.idx_m = g.idx_m; q.idx_k = g.idx_k; q.M = g.M; q.K = g.K; q.j0 = g.j0;
         q.out0 = g.out0; q.o_bs0 = g.o_bs0; q.out1 = g.out1; q.o_bs1 = g.o_bs1; q.m_split = g.m_split; q.o_rs = g.o_rs;
         q.nrb = nrb[i];
         int per = (int)((double)slots * g.K / wsum);

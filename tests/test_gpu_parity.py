@@ -495,3 +495,52 @@ def test_message_parity_inversion_on_gpu():
     inv = run_message_parity(m)
     assert np.abs(inv[:, 0] - base[:, 0] * sign).max() < 1e-5 * np.abs(base[:, 0]).max()
     assert np.abs(inv[:, 1] + base[:, 1] * sign).max() < 1e-5 * np.abs(base[:, 1]).max()
+
+
+# --------------------------------------------------------------- l-dependent CP weights
+@pytest.mark.parametrize("lmax,lmax_out,N,C,batch,mask", [
+    (0, 0, 2, 2, 5, [0, 1]),
+    (2, 2, 8, 8, 64, None),
+    (3, 5, 5, 3, 33, [1, 0, 1]),      # odd N: unaligned atom blocks -> generic projection kernel
+    (6, 6, 16, 16, 700, None),        # fast projections with a column offset, several tiles, ragged tail
+    (10, 10, 4, 4, 9, None),
+])
+def test_onsite_lw(lmax, lmax_out, N, C, batch, mask):
+    """cgtp_onsite_lw: c_{cnl} / lambda_c^{(nl)} per degree (Eq.(35), Eq.(41) :346) against the oracle."""
+    inp = synthetic.make_onsite(lmax, lmax_out, N, C, batch, seed=700 + lmax, parity_mask=mask)
+    (Wa, Wb), Wo = synthetic.lw_weights(lmax, lmax_out, N, C, seed=700 + lmax)
+    out = cg.cgtp_onsite_lw(_cuda(inp.A), _cuda(inp.B), _cuda(Wa), _cuda(Wb), _cuda(Wo), lmax, lmax_out, N, C,
+                            inp.parity_mask)
+    got = out.cpu().numpy()
+    ref = orc.onsite_lw(inp.A, inp.B, Wa, Wb, Wo, lmax, lmax_out, inp.parity_mask)
+    e = sector_err(got, ref)
+    assert max(e) < TOL, e
+    # equal weights for every degree: the l-shared entry point, to rounding
+    rep = lambda W, n: np.ascontiguousarray(np.repeat(W[None], n, axis=0))
+    same = cg.cgtp_onsite_lw(_cuda(inp.A), _cuda(inp.B), _cuda(rep(inp.W_a, lmax + 1)), _cuda(rep(inp.W_b, lmax + 1)),
+                             _cuda(rep(inp.W_out, lmax_out + 1)), lmax, lmax_out, N, C, inp.parity_mask).cpu().numpy()
+    base = run_onsite(inp)
+    for s in (0, 1):
+        assert np.abs(same[:, s] - base[:, s]).max() <= 2e-6 * max(np.abs(base[:, s]).max(), 1e-30)
+
+
+@pytest.mark.parametrize("lmax,lmax_out,N,C,nodes,mask", [
+    (1, 1, 4, 4, 9, [0, 1, 1, 0]),
+    (3, 4, 4, 6, 20, None),
+    (6, 6, 8, 8, 40, None),
+    (8, 8, 16, 8, 30, [0] * 3 + [1] * 5),
+])
+def test_message_lw(lmax, lmax_out, N, C, nodes, mask):
+    """cgtp_message_lw: W_node[l], W_out[l] per degree (Eq.(47), Eq.(55) :427) against the oracle."""
+    rng = np.random.default_rng(800 + lmax)
+    deg = rng.integers(0, 10, nodes)
+    deg[0] = 0
+    m = synthetic.make_message(lmax, lmax_out, N, C, nodes, deg, seed=800 + lmax, parity_mask=mask)
+    (Wn,), Wo = synthetic.lw_weights(lmax, lmax_out, N, C, seed=800 + lmax, n_in=1)
+    out = cg.cgtp_message_lw(_cuda(m.node_feats), _cuda(m.edge_index), _cuda(m.edge_vec), _cuda(m.edge_radial), _cuda(Wn),
+                             _cuda(Wo), lmax, lmax_out, N, C, m.parity_mask, check=True)
+    got = out.cpu().numpy()
+    ref = orc.message_lw(m.node_feats, m.edge_index, m.edge_vec, m.edge_radial, Wn, Wo, lmax, lmax_out, m.parity_mask)
+    e = sector_err(got, ref)
+    assert max(e) < TOL, e
+    assert np.abs(got[deg == 0]).max() == 0.0
