@@ -1,5 +1,6 @@
 // api.cu -- the C ABI of include/cgtp.h: argument validation, workspace carving, stage sequencing.
 #include <cstring>
+#include <vector>
 
 #include "common.cuh"
 
@@ -66,6 +67,22 @@ static size_t message_ws_bytes(int lmax, int lmax_out, int C, int Co, int64_t n_
     return 256 + fl * sizeof(float) + (size_t)(n_recv + 1) * sizeof(int64_t) + 12 * 256;
 }
 
+// Projection problems of all degrees (l-dependent weights): one launch when the multi-problem kernel takes them, else
+// `group` problems per launch (the factors / sectors of one degree).
+static int launch_proj_degrees(const std::vector<ProjArgs>& v, int group, Kind kind, cudaStream_t st)
+{
+    if ((int)v.size() > group && get_math_mode() == CGTP_MATH_FP32) {
+        bool handled = false;
+        const int rc = launch_proj_multi(v.data(), (int)v.size(), kind, st, &handled);
+        if (rc != CGTP_OK || handled) return rc;
+    }
+    for (size_t i = 0; i < v.size(); i += group) {
+        const int rc = launch_proj(&v[i], group, kind, st);
+        if (rc) return rc;
+    }
+    return CGTP_OK;
+}
+
 // One run of the on-site pipeline S1-S5 over Ce even + Co odd rank channels (internal channel order: even block, then
 // odd block).  cgtp_onsite is one pass; the parity-slot entry point (cgtp_onsite_parity) is four passes that differ in
 // the input slots, the weight rows and the output sectors.
@@ -120,10 +137,11 @@ static int onsite_pass(const Plan* p, int N, const OnsitePass& q, int64_t batch,
     // S1: H = W . A (Eq.(35)); rows are written in parity-sorted channel order, even block then odd block.  With
     // l-dependent weights one launch per degree l over the columns l^2 .. l^2 + 2l of every row.
     int rc = CGTP_OK;
+    std::vector<ProjArgs> pv;
     for (int l = 0; l < (q.lw_in ? p->lmax + 1 : 1); ++l) {
-        ProjArgs pin[2];
         for (int s = 0; s < 2; ++s) {
-            ProjArgs& a = pin[s];
+            pv.emplace_back();
+            ProjArgs& a = pv.back();
             const int jo = q.lw_in ? l * l : 0;
             a.X = s ? q.B : q.A;
             a.x_bs = q.x_bs;
@@ -146,9 +164,9 @@ static int onsite_pass(const Plan* p, int N, const OnsitePass& q, int64_t batch,
             a.accumulate = 0;
             a.j0 = jo;
         }
-        rc = launch_proj(pin, 2, K_PROJ_IN, st);
-        if (rc) return rc;
     }
+    rc = launch_proj_degrees(pv, 2, K_PROJ_IN, st);
+    if (rc) return rc;
 
     // S2-S4 fused, one launch per parity
     rc = fast ? launch_onsite_fast(p, false, Ha_e, Hb_e, T_e, batch * Ce, st)
@@ -165,10 +183,11 @@ static int onsite_pass(const Plan* p, int N, const OnsitePass& q, int64_t batch,
     }
 
     // S5: out[b, s] = W_out[:, channels of sector s] . T_s (Eq.(41)); per degree with l-dependent weights
+    pv.clear();
     for (int l = 0; l < (q.lw_out ? p->lmax_out + 1 : 1); ++l) {
-        ProjArgs po[2];
         for (int s = 0; s < 2; ++s) {
-            ProjArgs& a = po[s];
+            pv.emplace_back();
+            ProjArgs& a = pv.back();
             const int jo = q.lw_out ? l * l : 0;
             a.X = s ? T_o : T_e;
             a.x_bs = (int64_t)(s ? Co : Ce) * tstr;
@@ -191,10 +210,8 @@ static int onsite_pass(const Plan* p, int N, const OnsitePass& q, int64_t batch,
             a.accumulate = q.accumulate;
             a.j0 = jo;
         }
-        rc = launch_proj(po, 2, K_PROJ_OUT, st);
-        if (rc) return rc;
     }
-    return CGTP_OK;
+    return launch_proj_degrees(pv, 2, K_PROJ_OUT, st);
 }
 
 static int check_message_args(const float* node_feats, const int64_t* edge_index, const float* edge_vec,
@@ -264,9 +281,11 @@ static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_
     }
 
     // M1: H = W_node . node_feats (Eq.(47)); one launch per degree with l-dependent weights
+    std::vector<ProjArgs> pv;
     for (int l = 0; l < (q.lw_in ? p->lmax + 1 : 1); ++l) {
         const int jo = q.lw_in ? l * l : 0;
-        ProjArgs a;
+        pv.emplace_back();
+        ProjArgs& a = pv.back();
         a.X = q.node_feats;
         a.x_bs = q.x_bs;
         a.x_rs = p->L2;
@@ -287,9 +306,9 @@ static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_
         a.batch = n_send;
         a.accumulate = 0;
         a.j0 = jo;
-        rc = launch_proj(&a, 1, K_PROJ_IN, st);
-        if (rc) return rc;
     }
+    rc = launch_proj_degrees(pv, 1, K_PROJ_IN, st);
+    if (rc) return rc;
 
     // M2 (value fields for both parities: the odd channels take their derivatives on the edge side and in M5)
     rc = fast_synth ? launch_node_synth_fast(p, false, H_e, hstr, G_e, n_send * Ce, st)
@@ -318,11 +337,12 @@ static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_
     }
 
     // M6 (per degree with l-dependent weights)
+    pv.clear();
     for (int l = 0; l < (q.lw_out ? p->lmax_out + 1 : 1); ++l) {
         const int jo = q.lw_out ? l * l : 0;
-        ProjArgs po[2];
         for (int s = 0; s < 2; ++s) {
-            ProjArgs& b = po[s];
+            pv.emplace_back();
+            ProjArgs& b = pv.back();
             b.X = s ? T_o : T_e;
             b.x_bs = (int64_t)(s ? Co : Ce) * p->Lo2p;
             b.x_rs = p->Lo2p;
@@ -344,10 +364,8 @@ static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_
             b.accumulate = q.accumulate;
             b.j0 = jo;
         }
-        rc = launch_proj(po, 2, K_PROJ_OUT, st);
-        if (rc) return rc;
     }
-    return CGTP_OK;
+    return launch_proj_degrees(pv, 2, K_PROJ_OUT, st);
 }
 
 }  // namespace cgtp

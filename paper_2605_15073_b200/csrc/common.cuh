@@ -165,6 +165,10 @@ int launch_proj(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st);
 // layout conditions (even K, 16-byte aligned atom blocks, ...) do not hold and the generic kernel must run.
 int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st, bool* handled);
 
+// All degrees of an l-dependent-weight projection in one launch (proj_multi.cu); FP32 path only; *handled = false ->
+// launch the problems one by one.
+int launch_proj_multi(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st, bool* handled);
+
 // Tensor-core path of launch_proj (proj_tc.cu: tcgen05.mma kind::tf32, TMEM accumulators), taken only when
 // the math mode is CGTP_MATH_3XTF32 / CGTP_MATH_TF32; *handled = false otherwise.
 int launch_proj_tc(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st, bool* handled);
