@@ -729,10 +729,12 @@ int oracle_onsite_lw(const double *A, const double *B, const double *W_a, const 
     return 0;
 }
 
-int oracle_message_lw(const double *node_feats, const int64_t *edge_index, const double *edge_vec,
-                      const double *edge_radial, const double *W_node, const double *W_out, int lmax,
-                      int lmax_out, int N, int C, const uint8_t *parity_mask, double *out, int64_t nodes,
-                      int64_t E)
+/* radial_l1 = 0: edge_radial [E,C] (l1-shared, reading R12); radial_l1 = 1: edge_radial [E,C,lmax+1], the paper's  */
+/* R~_{jicl1} of Eq.(46) (:396): a[e,c,l1m1] = edge_radial[e,c,l1] Y_{l1m1}(r_hat_e) (Eq.(48) :402).                   */
+static int message_lw_impl(const double *node_feats, const int64_t *edge_index, const double *edge_vec,
+                           const double *edge_radial, int radial_l1, const double *W_node, const double *W_out,
+                           int lmax, int lmax_out, int N, int C, const uint8_t *parity_mask, double *out,
+                           int64_t nodes, int64_t E)
 {
     int L2 = (lmax + 1) * (lmax + 1), Lo2 = (lmax_out + 1) * (lmax_out + 1);
     const coupling_t *tab[2];
@@ -767,10 +769,12 @@ int oracle_message_lw(const double *node_feats, const int64_t *edge_index, const
                 const double *hj = H + snd[e] * (int64_t)C * L2;
                 oracle_real_sh(lmax, edge_vec[3 * e], edge_vec[3 * e + 1], edge_vec[3 * e + 2], Y);
                 for (int c = 0; c < C; ++c) {
-                    double rad = edge_radial[e * (int64_t)C + c];
                     const coupling_t *t = tab[parity_mask[c] ? 1 : 0];
-                    for (int64_t k = 0; k < t->nnz; ++k)
+                    for (int64_t k = 0; k < t->nnz; ++k) {
+                        double rad = radial_l1 ? edge_radial[(e * (int64_t)C + c) * (lmax + 1) + isqrt_floor(t->i1[k])]
+                                               : edge_radial[e * (int64_t)C + c];
                         T[(size_t)c * Lo2 + t->io[k]] += t->val[k] * rad * Y[t->i1[k]] * hj[(size_t)c * L2 + t->i2[k]];
+                    }
                 }
             }
             double *ob = out + i * 2 * (int64_t)N * Lo2;
@@ -789,6 +793,26 @@ int oracle_message_lw(const double *node_feats, const int64_t *edge_index, const
     }
     free(H); free(row_ptr);
     return 0;
+}
+
+int oracle_message_lw(const double *node_feats, const int64_t *edge_index, const double *edge_vec,
+                      const double *edge_radial, const double *W_node, const double *W_out, int lmax,
+                      int lmax_out, int N, int C, const uint8_t *parity_mask, double *out, int64_t nodes,
+                      int64_t E)
+{
+    return message_lw_impl(node_feats, edge_index, edge_vec, edge_radial, 0, W_node, W_out, lmax, lmax_out, N, C,
+                           parity_mask, out, nodes, E);
+}
+
+/* The message-passing coupling in the paper's full parameterisation: l-dependent c_{cnl}, lambda_c^{(nl)} and the   */
+/* l1-dependent radial factor R~_{jicl1} (Eq.(46)-(48) :396-:402).  edge_radial [E, C, lmax+1].                        */
+int oracle_message_lwr(const double *node_feats, const int64_t *edge_index, const double *edge_vec,
+                       const double *edge_radial, const double *W_node, const double *W_out, int lmax,
+                       int lmax_out, int N, int C, const uint8_t *parity_mask, double *out, int64_t nodes,
+                       int64_t E)
+{
+    return message_lw_impl(node_feats, edge_index, edge_vec, edge_radial, 1, W_node, W_out, lmax, lmax_out, N, C,
+                           parity_mask, out, nodes, E);
 }
 
 int oracle_num_threads(void)

@@ -68,6 +68,8 @@ def _load():
     lib.oracle_onsite_lw.argtypes = [p, p, p, p, p, i, i, i, i, p, p, i64]
     lib.oracle_message_lw.restype = i
     lib.oracle_message_lw.argtypes = [p, p, p, p, p, p, i, i, i, i, p, p, i64, i64]
+    lib.oracle_message_lwr.restype = i
+    lib.oracle_message_lwr.argtypes = lib.oracle_message_lw.argtypes
     lib.oracle_num_threads.restype = i
     lib.oracle_num_threads.argtypes = []
     _lib = lib
@@ -261,6 +263,25 @@ def message_lw(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lma
                                    N, C, _ptr(mask), _ptr(out), nodes, E)
     if rc:
         raise RuntimeError(f"oracle_message_lw failed with code {rc}")
+    return out
+
+
+def message_lwr(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, parity_mask) -> np.ndarray:
+    """Message passing in the paper's full parameterisation: W_node [lmax+1, C, N], W_out [lmax_out+1, N, C] and the
+    l1-dependent radial factor edge_radial [E, C, lmax+1] (Eq.(46))."""
+    X, ev, er, W_node, W_out = map(_f64, (node_feats, edge_vec, edge_radial, W_node, W_out))
+    ei = np.ascontiguousarray(np.asarray(edge_index), dtype=np.int64)
+    nodes, N, L2 = X.shape
+    E = ei.shape[1]
+    C = W_node.shape[1]
+    assert L2 == (lmax + 1) ** 2 and ev.shape == (E, 3) and er.shape == (E, C, lmax + 1)
+    assert W_node.shape == (lmax + 1, C, N) and W_out.shape == (lmax_out + 1, N, C)
+    mask = np.ascontiguousarray(np.asarray(parity_mask), dtype=np.uint8)
+    out = np.zeros((nodes, 2, N, (lmax_out + 1) ** 2), np.float64)
+    rc = _load().oracle_message_lwr(_ptr(X), _ptr(ei), _ptr(ev), _ptr(er), _ptr(W_node), _ptr(W_out), lmax, lmax_out,
+                                    N, C, _ptr(mask), _ptr(out), nodes, E)
+    if rc:
+        raise RuntimeError(f"oracle_message_lwr failed with code {rc}")
     return out
 
 

@@ -75,3 +75,32 @@ def test_message_lw_reduces_and_matches_numpy_projections():
     T = orc.message(H, m.edge_index, m.edge_vec, m.edge_radial, eye, eye, lmax, lmax, m.parity_mask)
     ref = np.einsum("qnc,iscq->isnq", Wo[lv].astype(float), T)
     assert np.abs(got - ref).max() < 1e-12 and np.abs(ref).max() > 1e-2
+
+
+def test_message_lwr_radial_per_degree():
+    """l1-dependent radial factor (Eq.(46)): equal values for every l1 reduce to message_lw; the general
+    case against a direct contraction of the pinned real coupling tables (real_coupling_dense) in numpy."""
+    lmax, N, C = 3, 3, 4
+    m = synthetic.make_message(lmax, lmax, N, C, nodes=5, degree=np.array([2, 0, 3, 1, 2]), seed=47,
+                               parity_mask=[1, 0, 0, 1])
+    (Wn,), Wo = synthetic.lw_weights(lmax, lmax, N, C, seed=47, n_in=1)
+    rep = np.repeat(m.edge_radial[:, :, None].astype(float), lmax + 1, axis=2)
+    a = orc.message_lwr(m.node_feats, m.edge_index, m.edge_vec, rep, Wn, Wo, lmax, lmax, m.parity_mask)
+    b = orc.message_lw(m.node_feats, m.edge_index, m.edge_vec, m.edge_radial, Wn, Wo, lmax, lmax, m.parity_mask)
+    assert np.abs(a - b).max() < 1e-13
+    rad = np.random.default_rng(3).standard_normal((m.E, C, lmax + 1))
+    got = orc.message_lwr(m.node_feats, m.edge_index, m.edge_vec, rad, Wn, Wo, lmax, lmax, m.parity_mask)
+    lv = _lof(lmax)
+    H = np.einsum("qcn,jnq->jcq", Wn[lv].astype(float), m.node_feats.astype(float))
+    tabs = [orc.real_coupling_dense(lmax, lmax, False), orc.real_coupling_dense(lmax, lmax, True)]
+    T = np.zeros((m.nodes, C, (lmax + 1) ** 2))
+    for e in range(m.E):
+        j, i = m.edge_index[:, e]
+        Y = shref.real_sh_xyz(lmax, m.edge_vec[e].astype(float))
+        for c in range(C):
+            T[i, c] += np.einsum("abo,a,b->o", tabs[int(m.parity_mask[c])], rad[e, c][lv] * Y, H[j, c])
+    ref = np.zeros_like(got)
+    for s in (0, 1):
+        sel = m.parity_mask == s
+        ref[:, s] = np.einsum("qnc,icq->inq", Wo[lv].astype(float)[:, :, sel], T[:, sel])
+    assert np.abs(got - ref).max() < 1e-12 and np.abs(ref).max() > 1e-2
