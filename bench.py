@@ -559,7 +559,28 @@ def run_lw(args, cg, synthetic, dev, shared_ms):
     torch.cuda.synchronize()
     prof = cg.cgtp_profile_collect()
     cg.cgtp_profile_enable(False)
-    return {"workload": "BASELINE.json configs[1] with W_a, W_b [7, 64, 64] and W_out [7, 64, 64] (one matrix per degree)",
+    res_msg = {}
+    for idx in (2, 4):
+        m = synthetic.config(idx)
+        if idx == 2:
+            m.parity_mask = synthetic.half_mask(m.C)
+        (Wn,), Wom = synthetic.lw_weights(m.lmax, m.lmax_out, m.N, m.C, seed=0, n_in=1)
+        X, ei, ev, er = cu(m.node_feats), cu(m.edge_index), cu(m.edge_vec), cu(m.edge_radial)
+        Wn, Wom = cu(Wn), cu(Wom)
+        # R~[e, c, l1]: the configs' Bessel x Gaussian radial factor with a smooth l1 profile
+        rad = (er[:, :, None] * torch.linspace(0.5, 1.5, m.lmax + 1, device=dev)[None, None, :]).contiguous()
+        outm = torch.empty((m.nodes, 2, m.N, (m.lmax_out + 1) ** 2), device=dev)
+        f_lw = lambda: cg.cgtp_message_lw(X, ei, ev, er, Wn, Wom, m.lmax, m.lmax_out, m.N, m.C, m.parity_mask, out=outm)
+        f_lwr = lambda: cg.cgtp_message_lwr(X, ei, ev, rad, Wn, Wom, m.lmax, m.lmax_out, m.N, m.C, m.parity_mask, out=outm)
+        ms_lw, ms_lwr = time_steps(f_lw, 3, 2), time_steps(f_lwr, 3, 2)
+        res_msg[f"config{idx}"] = {
+            "workload": f"BASELINE.json configs[{idx}] (half odd) with W_node [L, C, N], W_out [L, N, C]; lwr: edge_radial [E, C, L]",
+            "lw_ms_per_step": ms_lw, "lw_edges_per_s": m.E / (ms_lw * 1e-3),
+            "lwr_ms_per_step": ms_lwr, "lwr_edges_per_s": m.E / (ms_lwr * 1e-3)}
+        del X, ei, ev, er, rad, outm
+        torch.cuda.empty_cache()
+    return {"message": res_msg,
+            "workload": "BASELINE.json configs[1] with W_a, W_b [7, 64, 64] and W_out [7, 64, 64] (one matrix per degree)",
             "ms_per_step": ms, "contractions_per_s": inp.batch / (ms * 1e-3), "l_shared_ms_per_step": shared_ms,
             "factor_vs_l_shared": ms / shared_ms,
             "kernel_ms": {k: v[0] / 10 for k, v in prof.items()},

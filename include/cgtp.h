@@ -203,6 +203,15 @@ int cgtp_message_lw(const float* node_feats, const int64_t* edge_index, const fl
                     int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask, float* out,
                     int64_t nodes, int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Message passing in the paper's full parameterisation: the l-dependent weights of cgtp_message_lw AND the l1-dependent
+ * radial factor R~_{jicl1} of Eq.(46): the edge field of channel c is
+ *   E_{e,c}(Omega) = sum_{l1 <= lmax} edge_radial[e,c,l1] sum_{m1} Y_{l1m1}(r_e) Y_{l1m1}(Omega)          (Eq.(48), (50))
+ * edge_radial  device [E, C, lmax+1]; everything else as cgtp_message_lw (same workspace size). */
+int cgtp_message_lwr(const float* node_feats, const int64_t* edge_index, const float* edge_vec,
+                     const float* edge_radial, const float* W_node, const float* W_out,
+                     int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask, float* out,
+                     int64_t nodes, int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* ---------------------------------------------------------------------------------------------
  * Host-buffer entry points (end-to-end path): same semantics as cgtp_onsite / cgtp_message, but
  * every tensor pointer is HOST memory (pinned memory recommended; pageable works, slower).  The

@@ -64,6 +64,8 @@ def lib() -> ctypes.CDLL:
     L.cgtp_message_parity.argtypes = [vp, vp, vp, vp, vp, vp, i, i, i, i, vp, i64, i64, vp, sz, vp]
     L.cgtp_onsite_lw.restype = i
     L.cgtp_onsite_lw.argtypes = L.cgtp_onsite.argtypes
+    L.cgtp_message_lwr.restype = i
+    L.cgtp_message_lwr.argtypes = L.cgtp_message.argtypes
     L.cgtp_message_lw.restype = i
     L.cgtp_message_lw.argtypes = L.cgtp_message.argtypes
     L.cgtp_message_status.restype = i
@@ -345,8 +347,9 @@ def cgtp_onsite_lw(A, B, W_a, W_b, W_out, lmax, lmax_out, N, C, parity_mask, out
 
 
 def cgtp_message_lw(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, N, C, parity_mask,
-                    out=None, workspace=None, stream=None, check: bool = False):
-    """cgtp_message with l-dependent weights: W_node [lmax+1, C, N], W_out [lmax_out+1, N, C] (see include/cgtp.h)."""
+                    out=None, workspace=None, stream=None, check: bool = False, radial_l1: bool = False):
+    """cgtp_message with l-dependent weights: W_node [lmax+1, C, N], W_out [lmax_out+1, N, C]; radial_l1=True calls
+    cgtp_message_lwr: edge_radial [E, C, lmax+1], the l1-dependent radial factor (see include/cgtp.h)."""
     f32 = torch.float32
     X = _dev(node_feats, f32, "node_feats")
     ei = _dev(edge_index, torch.int64, "edge_index")
@@ -356,8 +359,8 @@ def cgtp_message_lw(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out
     L2, Lo2 = (lmax + 1) ** 2, (lmax_out + 1) ** 2
     if tuple(X.shape) != (nodes, N, L2):
         raise ValueError("node_feats must be [nodes, N, (lmax+1)^2]")
-    if tuple(ei.shape) != (2, E) or tuple(ev.shape) != (E, 3) or tuple(er.shape) != (E, C):
-        raise ValueError("edge_index [2,E], edge_vec [E,3], edge_radial [E,C] expected")
+    if tuple(ei.shape) != (2, E) or tuple(ev.shape) != (E, 3) or tuple(er.shape) != ((E, C, lmax + 1) if radial_l1 else (E, C)):
+        raise ValueError("edge_index [2,E], edge_vec [E,3], edge_radial [E,C] ([E,C,lmax+1] with radial_l1) expected")
     if tuple(W_node.shape) != (lmax + 1, C, N) or tuple(W_out.shape) != (lmax_out + 1, N, C):
         raise ValueError("W_node must be [lmax+1, C, N] and W_out [lmax_out+1, N, C]")
     mask = _mask(parity_mask, C)
@@ -369,13 +372,21 @@ def cgtp_message_lw(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out
     ws = _workspace(X.device, nbytes) if workspace is None else workspace
     sp = _stream_ptr(stream)
     with torch.cuda.device(X.device):
-        rc = lib().cgtp_message_lw(X.data_ptr(), ei.data_ptr(), ev.data_ptr(), er.data_ptr(), W_node.data_ptr(),
-                                   W_out.data_ptr(), lmax, lmax_out, N, C, mask.ctypes.data, out.data_ptr(), nodes, E,
-                                   ws.data_ptr(), ws.numel(), sp)
+        fn = lib().cgtp_message_lwr if radial_l1 else lib().cgtp_message_lw
+        rc = fn(X.data_ptr(), ei.data_ptr(), ev.data_ptr(), er.data_ptr(), W_node.data_ptr(),
+                W_out.data_ptr(), lmax, lmax_out, N, C, mask.ctypes.data, out.data_ptr(), nodes, E,
+                ws.data_ptr(), ws.numel(), sp)
         _check(rc)
         if check:
             _check(lib().cgtp_message_status(ws.data_ptr(), sp))
     return out
+
+
+def cgtp_message_lwr(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, N, C, parity_mask,
+                     out=None, workspace=None, stream=None, check: bool = False):
+    """Message passing with l-dependent weights and the l1-dependent radial factor edge_radial [E, C, lmax+1]."""
+    return cgtp_message_lw(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, N, C, parity_mask,
+                           out=out, workspace=workspace, stream=stream, check=check, radial_l1=True)
 
 
 def cgtp_message_status(workspace=None, device=None, stream=None) -> int:

@@ -253,6 +253,7 @@ struct MessagePass {
     int sigma_C;              // as OnsitePass::sigma_C
     bool segments_done;       // row_ptr / status of this workspace are already built (second pass)
     int64_t lw_in, lw_out;    // as OnsitePass: l-dependent W_node (Eq.(47) :398) / W_out (Eq.(55), (58))
+    bool radial_l1;           // edge_radial is [E][radial_stride][lmax+1]: l1-dependent R~ (Eq.(46) :396)
 };
 
 static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_t* edge_index, const float* edge_vec,
@@ -319,10 +320,17 @@ static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_
     if (rc) return rc;
 
     // M3 + M4
-    rc = launch_edge(p, false, G_e, row_ptr, edge_index, E, edge_vec, q.edge_radial, q.idx_in, Ce, q.radial_stride, S_e, nodes, status, st);
-    if (rc) return rc;
-    rc = launch_edge(p, true, G_o, row_ptr, edge_index, E, edge_vec, q.edge_radial, q.idx_in + Ce, Co, q.radial_stride, S_o, nodes, status, st);
-    if (rc) return rc;
+    if (q.radial_l1) {
+        rc = launch_edge_lr(p, false, G_e, row_ptr, edge_index, E, edge_vec, q.edge_radial, q.idx_in, Ce, q.radial_stride, S_e, nodes, status, st);
+        if (rc) return rc;
+        rc = launch_edge_lr(p, true, G_o, row_ptr, edge_index, E, edge_vec, q.edge_radial, q.idx_in + Ce, Co, q.radial_stride, S_o, nodes, status, st);
+        if (rc) return rc;
+    } else {
+        rc = launch_edge(p, false, G_e, row_ptr, edge_index, E, edge_vec, q.edge_radial, q.idx_in, Ce, q.radial_stride, S_e, nodes, status, st);
+        if (rc) return rc;
+        rc = launch_edge(p, true, G_o, row_ptr, edge_index, E, edge_vec, q.edge_radial, q.idx_in + Ce, Co, q.radial_stride, S_o, nodes, status, st);
+        if (rc) return rc;
+    }
 
     // M5
     rc = launch_analysis(p, false, S_e, T_e, nodes * Ce, st);
@@ -471,7 +479,7 @@ int cgtp_build_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int
     return launch_segments(edge_index, E, nodes, nodes, row_ptr, status, static_cast<cudaStream_t>(cuda_stream));
 }
 
-static int message_entry(bool lw, const float* node_feats, const int64_t* edge_index, const float* edge_vec,
+static int message_entry(int lw, const float* node_feats, const int64_t* edge_index, const float* edge_vec,
                          const float* edge_radial, const float* W_node, const float* W_out, int lmax, int lmax_out,
                          int N, int C, const uint8_t* parity_mask, float* out, int64_t n_send, int64_t nodes,
                          int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream)
@@ -512,6 +520,7 @@ static int message_entry(bool lw, const float* node_feats, const int64_t* edge_i
     q.segments_done = false;
     q.lw_in = lw ? (int64_t)C * N : 0;
     q.lw_out = lw ? (int64_t)N * C : 0;
+    q.radial_l1 = lw == 2;
     return message_pass(p, N, q, edge_index, edge_vec, n_send, nodes, E, workspace, st);
 }
 
@@ -536,7 +545,7 @@ int cgtp_message_bipartite(const float* node_feats, const int64_t* edge_index, c
                            int N, int C, const uint8_t* parity_mask, float* out, int64_t n_send, int64_t nodes,
                            int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
-    return message_entry(false, node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, N, C,
+    return message_entry(0, node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, N, C,
                          parity_mask, out, n_send, nodes, E, workspace, workspace_bytes, cuda_stream);
 }
 
@@ -545,7 +554,16 @@ int cgtp_message_lw(const float* node_feats, const int64_t* edge_index, const fl
                     const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* workspace,
                     size_t workspace_bytes, void* cuda_stream)
 {
-    return message_entry(true, node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, N, C,
+    return message_entry(1, node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, N, C,
+                         parity_mask, out, nodes, nodes, E, workspace, workspace_bytes, cuda_stream);
+}
+
+int cgtp_message_lwr(const float* node_feats, const int64_t* edge_index, const float* edge_vec, const float* edge_radial,
+                     const float* W_node, const float* W_out, int lmax, int lmax_out, int N, int C,
+                     const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* workspace,
+                     size_t workspace_bytes, void* cuda_stream)
+{
+    return message_entry(2, node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lmax, lmax_out, N, C,
                          parity_mask, out, nodes, nodes, E, workspace, workspace_bytes, cuda_stream);
 }
 
@@ -688,6 +706,7 @@ int cgtp_message_parity(const float* node_feats, const int64_t* edge_index, cons
         q.sigma_C = C;
         q.segments_done = s_in > 0;
         q.lw_in = q.lw_out = 0;
+        q.radial_l1 = false;
         rc = message_pass(p, N, q, edge_index, edge_vec, nodes, nodes, E, workspace, st);
         if (rc) return rc;
     }

@@ -209,6 +209,10 @@ int launch_edge(const Plan* p, bool odd, const float* G, const int64_t* row_ptr,
 int launch_edge_ring(const Plan* p, bool odd, const float* G, const int64_t* row_ptr, const int64_t* edge_index,
                      int64_t E, const float* edge_vec, const float* edge_radial, const int* perm_par, int Cpar, int C,
                      float* S, int64_t nodes, const int32_t* status, cudaStream_t st, bool* handled);
+// M3+M4 with the l1-dependent radial factor edge_radial [E][C][lmax+1] (edge_lr.cu; Eq.(46)).
+int launch_edge_lr(const Plan* p, bool odd, const float* G, const int64_t* row_ptr, const int64_t* edge_index, int64_t E,
+                   const float* edge_vec, const float* edge_radial, const int* perm_par, int Cpar, int C, float* S,
+                   int64_t nodes, const int32_t* status, cudaStream_t st);
 // M5: T[col][Lo2p] = analysis of S[col][UVp] (even) or of the field pair S[col][2][UVp] against {., Y_lm} (odd)
 int launch_analysis(const Plan* p, bool odd, const float* S, float* T, int64_t ncols, cudaStream_t st);
 

@@ -544,3 +544,32 @@ def test_message_lw(lmax, lmax_out, N, C, nodes, mask):
     e = sector_err(got, ref)
     assert max(e) < TOL, e
     assert np.abs(got[deg == 0]).max() == 0.0
+
+
+@pytest.mark.parametrize("lmax,lmax_out,N,C,nodes,mask", [
+    (0, 0, 4, 4, 6, [0, 1, 0, 1]),
+    (1, 2, 4, 4, 9, [0, 1, 1, 0]),
+    (3, 3, 4, 6, 20, None),
+    (4, 4, 8, 40, 12, [0] * 30 + [1] * 10),   # several channel blocks per receiver
+    (8, 8, 8, 8, 16, None),
+    (12, 12, 4, 3, 5, [0, 1, 1]),
+])
+def test_message_lwr(lmax, lmax_out, N, C, nodes, mask):
+    """cgtp_message_lwr: l-dependent weights and the l1-dependent radial factor R~_{jicl1} (Eq.(46))."""
+    rng = np.random.default_rng(900 + lmax)
+    deg = rng.integers(0, 12, nodes)
+    deg[0] = 0
+    deg[-1] = 19
+    m = synthetic.make_message(lmax, lmax_out, N, C, nodes, deg, seed=900 + lmax, parity_mask=mask)
+    (Wn,), Wo = synthetic.lw_weights(lmax, lmax_out, N, C, seed=900 + lmax, n_in=1)
+    rad = (m.edge_radial[:, :, None] * rng.uniform(0.5, 1.5, (m.E, C, lmax + 1))).astype(np.float32)
+    out = cg.cgtp_message_lwr(_cuda(m.node_feats), _cuda(m.edge_index), _cuda(m.edge_vec), _cuda(rad), _cuda(Wn),
+                              _cuda(Wo), lmax, lmax_out, N, C, m.parity_mask, check=True)
+    got = out.cpu().numpy()
+    ref = orc.message_lwr(m.node_feats, m.edge_index, m.edge_vec, rad, Wn, Wo, lmax, lmax_out, m.parity_mask)
+    e = sector_err(got, ref)
+    assert max(e) < TOL, e
+    assert np.abs(got[deg == 0]).max() == 0.0
+    again = cg.cgtp_message_lwr(_cuda(m.node_feats), _cuda(m.edge_index), _cuda(m.edge_vec), _cuda(rad), _cuda(Wn),
+                                _cuda(Wo), lmax, lmax_out, N, C, m.parity_mask).cpu().numpy()
+    assert np.array_equal(got, again)  # bitwise reproducible
