@@ -17,7 +17,7 @@
 namespace cgtp {
 
 constexpr int LR_NT = 512;
-constexpr int LR_EC = 8;     // edges per chunk
+constexpr int LR_EC = 32;    // edges per chunk (upper bound; the launcher picks EC <= LR_EC that fits shared memory)
 constexpr int LR_LMAX = 24;  // recurrence coefficient table length
 
 __device__ __forceinline__ float4 lr_ldg_stream(const float4* p)
@@ -42,25 +42,29 @@ __device__ __forceinline__ void lr_fma4(float4& a, const float4& u, const float4
     a.x = fmaf(u.x, v.x, a.x); a.y = fmaf(u.y, v.y, a.y); a.z = fmaf(u.z, v.z, a.z); a.w = fmaf(u.w, v.w, a.w);
 }
 
-template <bool ODD, int NA>
+template <bool ODD, int NA, int LB>
 __global__ void __launch_bounds__(LR_NT, 1) edge_lr_kernel(Plan p, const float* __restrict__ G,
                                                           const int64_t* __restrict__ row_ptr,
                                                           const int64_t* __restrict__ snd,
                                                           const float* __restrict__ edge_vec,
                                                           const float* __restrict__ radial,
                                                           const int* __restrict__ perm_par, int Cpar, int C, int cb,
-                                                          int nblk, int G_, float* __restrict__ S,
+                                                          int nblk, int G_, int EC, float* __restrict__ S,
                                                           const int32_t* __restrict__ status)
 {
     constexpr int NF = ODD ? 2 : 1;
+    constexpr int NG = ODD ? 8 : 3;  // geometry fields: Omega_xyz (+ theta_hat_xyz, phi_hat_xy)
     extern __shared__ __align__(16) unsigned char smem_lr[];
-    float4* coef = reinterpret_cast<float4*>(smem_lr);             // [LR_LMAX]: (2l-1)/l, -(l-1)/l, (2l+1)/(4 pi), l
-    float4* Es = coef + LR_LMAX;                                   // [EC] unit vectors
+    float4* Es = reinterpret_cast<float4*>(smem_lr);               // [LR_EC] unit vectors
     long long* Ss = reinterpret_cast<long long*>(Es + LR_EC);      // [EC] senders
-    float* Rs = reinterpret_cast<float*>(Ss + LR_EC);              // [EC][cb][L1]
+    // the degree loop is unrolled to the kernel band limit LB >= lmax: recurrence coefficients are immediates and the
+    // R~ rows are zero beyond lmax
+    const int UVp = p.UVp, QP = UVp / 4, lmax = p.lmax, L1 = lmax + 1;
+    constexpr int L1p = round_up(LB + 1, 4);
+    float4* geo_s = reinterpret_cast<float4*>(Ss + LR_EC);         // [NG][QP]
+    float4* Rs = geo_s + NG * QP;                                  // [EC][cb][L1p / 4]: c_l R~[e, ch, l], zero padded
 
     const int tid = threadIdx.x;
-    const int UVp = p.UVp, QP = UVp / 4, lmax = p.lmax, L1 = lmax + 1;
     const long long item = blockIdx.x;
     const long long i = item / nblk;
     const int kc0 = (int)(item - i * nblk) * cb;
@@ -75,36 +79,34 @@ __global__ void __launch_bounds__(LR_NT, 1) edge_lr_kernel(Plan p, const float* 
         ch[x] = x * G_ + cg;
         live[x] = active && ch[x] < ncb;
     }
-    if (tid < LR_LMAX) {
-        const float l = (float)(tid > 0 ? tid : 1);
-        coef[tid] = make_float4((2.f * l - 1.f) / l, -(l - 1.f) / l, (2.f * tid + 1.f) * 0.07957747154594767f, l);
+    {
+        const float4* geo4 = reinterpret_cast<const float4*>(p.geo);
+        for (int idx = tid; idx < NG * QP; idx += LR_NT) geo_s[idx] = geo4[idx];
     }
-    // grid geometry of the thread's quad (zero beyond the U*V real points: those columns stay zero)
-    const float4* geo4 = reinterpret_cast<const float4*>(p.geo);
-    const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
-    const float4 gx = active ? geo4[q] : zero4, gy = active ? geo4[QP + q] : zero4, gz = active ? geo4[2 * QP + q] : zero4;
-    float4 thx = zero4, thy = zero4, thz = zero4, phx = zero4, phy = zero4;
-    if (ODD && active) {
-        thx = geo4[3 * QP + q]; thy = geo4[4 * QP + q]; thz = geo4[5 * QP + q];
-        phx = geo4[6 * QP + q]; phy = geo4[7 * QP + q];
-    }
-    const bool pad = 4 * q + 3 >= p.UV;  // quad touches the zero padding of the field
-    float4 acc[NA][NF];
+    const int qq = active ? q : 0;
+    int roff[NA];  // row of the thread's channels in the staged R~ (float4 units); dead lanes read row 0, never stored
+#pragma unroll
+    for (int x = 0; x < NA; ++x) roff[x] = live[x] ? ch[x] * (L1p / 4) : 0;
+    const float2 z2 = make_float2(0.f, 0.f);
+    float2 acc[NA][NF][2];
 #pragma unroll
     for (int x = 0; x < NA; ++x)
 #pragma unroll
-        for (int f = 0; f < NF; ++f) acc[x][f] = zero4;
+        for (int f = 0; f < NF; ++f) acc[x][f][0] = acc[x][f][1] = z2;
 
     const bool graph_ok = (*status == 0);
     const long long e_begin = graph_ok ? row_ptr[i] : 0, e_end = graph_ok ? row_ptr[i + 1] : 0;
     __syncthreads();
 
-    for (long long e0 = e_begin; e0 < e_end; e0 += LR_EC) {
-        const int ne = (int)((e_end - e0 < LR_EC) ? (e_end - e0) : LR_EC);
-        for (int idx = tid; idx < ne * ncb * L1; idx += LR_NT) {
-            const int el = idx / (ncb * L1), rem = idx - el * (ncb * L1);
-            const int k = rem / L1, l = rem - k * L1;
-            Rs[(el * cb + k) * L1 + l] = radial[((e0 + el) * (long long)C + perm_par[kc0 + k]) * L1 + l];
+    for (long long e0 = e_begin; e0 < e_end; e0 += EC) {
+        const int ne = (int)((e_end - e0 < EC) ? (e_end - e0) : EC);
+        // c_l R~[e, ch, l] of the chunk (the (2l+1)/(4 pi) of the addition theorem folded in), rows padded to float4s
+        for (int idx = tid; idx < ne * ncb * L1p; idx += LR_NT) {
+            const int el = idx / (ncb * L1p), rem = idx - el * (ncb * L1p);
+            const int k = rem / L1p, l = rem - k * L1p;
+            float v = 0.f;
+            if (l < L1) v = (2.f * l + 1.f) * 0.07957747154594767f * radial[((e0 + el) * (long long)C + perm_par[kc0 + k]) * L1 + l];
+            reinterpret_cast<float*>(Rs)[(el * cb + k) * L1p + l] = v;
         }
         if (tid < ne) {
             const long long e = e0 + tid;
@@ -120,63 +122,81 @@ __global__ void __launch_bounds__(LR_NT, 1) edge_lr_kernel(Plan p, const float* 
             const float4* gsrc = reinterpret_cast<const float4*>(G + ((size_t)Ss[el] * Cpar + kc0) * UVp);
             float4 g[NA];
 #pragma unroll
-            for (int x = 0; x < NA; ++x) g[x] = live[x] ? lr_ldg_stream(gsrc + (size_t)ch[x] * QP + q) : zero4;
+            for (int x = 0; x < NA; ++x) g[x] = live[x] ? lr_ldg_stream(gsrc + (size_t)ch[x] * QP + q) : make_float4(0.f, 0.f, 0.f, 0.f);
 
-            // E[x] = sum_l R~[e, ch_x, l] c_l P_l(t)   (even)   or   sum_l R~ c_l P'_l(t)   (odd), at the quad's points
-            const float4 t = lr_dot3(ev.x, ev.y, ev.z, gx, gy, gz);
-            float4 Ex[NA];
+            // E[x] = sum_l (c_l R~[e, ch_x, l]) P_l(t)  (even)  or  sum_l (c_l R~) P'_l(t)  (odd) at the quad's four points,
+            // two points per packed operation
+            const float4 t4 = lr_dot3(ev.x, ev.y, ev.z, geo_s[qq], geo_s[QP + qq], geo_s[2 * QP + qq]);
+            const float2 t[2] = {make_float2(t4.x, t4.y), make_float2(t4.z, t4.w)};
+            float2 Ex[NA][2];
 #pragma unroll
-            for (int x = 0; x < NA; ++x) Ex[x] = zero4;
-            const float* rrow = Rs + (size_t)el * cb * L1;
-            float4 pm = make_float4(1.f, 1.f, 1.f, 1.f), pc = t, dc = make_float4(1.f, 1.f, 1.f, 1.f);
+            for (int x = 0; x < NA; ++x) Ex[x][0] = Ex[x][1] = z2;
+            const float4* rrow = Rs + (size_t)el * cb * (L1p / 4);
+            const float2 one2 = make_float2(1.f, 1.f);
+            float2 pm[2] = {one2, one2}, pc[2] = {t[0], t[1]}, dc[2] = {one2, one2};
+#pragma unroll
+            for (int l0 = 0; l0 <= LB; l0 += 4) {
+                float r[NA][4];
+#pragma unroll
+                for (int x = 0; x < NA; ++x) {
+                    const float4 r4 = rrow[roff[x] + l0 / 4];
+                    r[x][0] = r4.x; r[x][1] = r4.y; r[x][2] = r4.z; r[x][3] = r4.w;
+                }
+#pragma unroll
+                for (int dl = 0; dl < 4; ++dl) {
+                    const int l = l0 + dl;
+                    if (l > LB) break;
+                    float2 term[2];
+                    if (l == 0) {
+                        term[0] = term[1] = ODD ? z2 : one2;  // P_0 = 1, P'_0 = 0
+                    } else if (l == 1) {
+                        term[0] = ODD ? one2 : t[0];          // P_1 = t, P'_1 = 1
+                        term[1] = ODD ? one2 : t[1];
+                    } else {
+                        const float ca = (2.f * l - 1.f) / l, cb2 = -(l - 1.f) / l, cl = (float)l;
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+                            const float2 pn = __ffma2_rn(__fmul2_rn(make_float2(ca, ca), t[h]), pc[h],
+                                                         __fmul2_rn(make_float2(cb2, cb2), pm[h]));
+                            if (ODD) {
+                                const float2 dn = __ffma2_rn(t[h], dc[h], __fmul2_rn(make_float2(cl, cl), pc[h]));
+                                dc[h] = dn;
+                                term[h] = dn;
+                            } else {
+                                term[h] = pn;
+                            }
+                            pm[h] = pc[h];
+                            pc[h] = pn;
+                        }
+                    }
+#pragma unroll
+                    for (int x = 0; x < NA; ++x) {
+                        const float2 r2 = make_float2(r[x][dl], r[x][dl]);
+                        Ex[x][0] = __ffma2_rn(r2, term[0], Ex[x][0]);
+                        Ex[x][1] = __ffma2_rn(r2, term[1], Ex[x][1]);
+                    }
+                }
+            }
             if (!ODD) {
-                const float c0 = coef[0].z;
 #pragma unroll
                 for (int x = 0; x < NA; ++x) {
-                    const float r = live[x] ? rrow[ch[x] * L1] : 0.f;
-                    lr_axpy(Ex[x], r * c0, pm);
+                    acc[x][0][0] = __ffma2_rn(Ex[x][0], make_float2(g[x].x, g[x].y), acc[x][0][0]);
+                    acc[x][0][1] = __ffma2_rn(Ex[x][1], make_float2(g[x].z, g[x].w), acc[x][0][1]);
                 }
-            }
-            if (lmax >= 1) {
-                const float c1 = coef[1].z;
-                const float4 term = ODD ? dc : pc;  // P'_1 = 1, P_1 = t
-#pragma unroll
-                for (int x = 0; x < NA; ++x) {
-                    const float r = live[x] ? rrow[ch[x] * L1 + 1] : 0.f;
-                    lr_axpy(Ex[x], r * c1, term);
-                }
-            }
-            for (int l = 2; l <= lmax; ++l) {
-                const float4 c = coef[l];
-                float4 pn, dn = zero4;
-                pn.x = fmaf(c.x * t.x, pc.x, c.y * pm.x); pn.y = fmaf(c.x * t.y, pc.y, c.y * pm.y);
-                pn.z = fmaf(c.x * t.z, pc.z, c.y * pm.z); pn.w = fmaf(c.x * t.w, pc.w, c.y * pm.w);
-                if (ODD) {
-                    dn.x = fmaf(t.x, dc.x, c.w * pc.x); dn.y = fmaf(t.y, dc.y, c.w * pc.y);
-                    dn.z = fmaf(t.z, dc.z, c.w * pc.z); dn.w = fmaf(t.w, dc.w, c.w * pc.w);
-                }
-                const float4 term = ODD ? dn : pn;
-#pragma unroll
-                for (int x = 0; x < NA; ++x) {
-                    const float r = live[x] ? rrow[ch[x] * L1 + l] : 0.f;
-                    lr_axpy(Ex[x], r * c.z, term);
-                }
-                pm = pc; pc = pn; dc = dn;
-            }
-            if (!ODD) {
-#pragma unroll
-                for (int x = 0; x < NA; ++x) lr_fma4(acc[x][0], Ex[x], g[x]);
             } else {
                 // X0 += (d_theta E) I,  X1 += -((1/sin) d_phi E) I
-                const float4 dth = lr_dot3(ev.x, ev.y, ev.z, thx, thy, thz);
-                const float4 dph = make_float4(-fmaf(ev.x, phx.x, ev.y * phy.x), -fmaf(ev.x, phx.y, ev.y * phy.y),
-                                               -fmaf(ev.x, phx.z, ev.y * phy.z), -fmaf(ev.x, phx.w, ev.y * phy.w));
+                const float4 dth = lr_dot3(ev.x, ev.y, ev.z, geo_s[3 * QP + qq], geo_s[4 * QP + qq], geo_s[5 * QP + qq]);
+                const float4 fx = geo_s[6 * QP + qq], fy = geo_s[7 * QP + qq];
+                const float4 dph = make_float4(-fmaf(ev.x, fx.x, ev.y * fy.x), -fmaf(ev.x, fx.y, ev.y * fy.y),
+                                               -fmaf(ev.x, fx.z, ev.y * fy.z), -fmaf(ev.x, fx.w, ev.y * fy.w));
 #pragma unroll
                 for (int x = 0; x < NA; ++x) {
-                    const float4 a = make_float4(Ex[x].x * dth.x, Ex[x].y * dth.y, Ex[x].z * dth.z, Ex[x].w * dth.w);
-                    const float4 b = make_float4(Ex[x].x * dph.x, Ex[x].y * dph.y, Ex[x].z * dph.z, Ex[x].w * dph.w);
-                    lr_fma4(acc[x][0], a, g[x]);
-                    lr_fma4(acc[x][NF - 1], b, g[x]);
+                    const float2 g0 = make_float2(g[x].x, g[x].y), g1 = make_float2(g[x].z, g[x].w);
+                    const float2 a0 = __fmul2_rn(Ex[x][0], g0), a1 = __fmul2_rn(Ex[x][1], g1);
+                    acc[x][0][0] = __ffma2_rn(a0, make_float2(dth.x, dth.y), acc[x][0][0]);
+                    acc[x][0][1] = __ffma2_rn(a1, make_float2(dth.z, dth.w), acc[x][0][1]);
+                    acc[x][NF - 1][0] = __ffma2_rn(a0, make_float2(dph.x, dph.y), acc[x][NF - 1][0]);
+                    acc[x][NF - 1][1] = __ffma2_rn(a1, make_float2(dph.z, dph.w), acc[x][NF - 1][1]);
                 }
             }
         }
@@ -188,17 +208,9 @@ __global__ void __launch_bounds__(LR_NT, 1) edge_lr_kernel(Plan p, const float* 
     for (int x = 0; x < NA; ++x) {
         if (!live[x]) continue;
 #pragma unroll
-        for (int f = 0; f < NF; ++f) {
-            float4 v = acc[x][f];
-            if (pad) {  // the even field K(t) does not vanish at the padded points (their geometry is zero, t = 0)
-                const int b = 4 * q;
-                if (b + 0 >= p.UV) v.x = 0.f;
-                if (b + 1 >= p.UV) v.y = 0.f;
-                if (b + 2 >= p.UV) v.z = 0.f;
-                if (b + 3 >= p.UV) v.w = 0.f;
-            }
-            sdst[((size_t)ch[x] * NF + f) * QP + q] = v;
-        }
+        for (int f = 0; f < NF; ++f)
+            sdst[((size_t)ch[x] * NF + f) * QP + q] =
+                make_float4(acc[x][f][0].x, acc[x][f][0].y, acc[x][f][1].x, acc[x][f][1].y);
     }
 }
 
@@ -211,29 +223,37 @@ int launch_edge_lr(const Plan* p, bool odd, const float* G, const int64_t* row_p
     const int QP = p->UVp / 4;
     if (QP > LR_NT || p->lmax >= LR_LMAX) { set_error("edge kernel (l1-dependent radial): grid of lmax=%d too large", p->lmax); return CGTP_ERR_UNSUPPORTED; }
     const int G_ = LR_NT / QP;
-    const int NA = odd ? 2 : 4;
+    const int NA = 4;
     const int cb_max = NA * G_;
     const int nblk = (Cpar + cb_max - 1) / cb_max;
     int cb = (Cpar + nblk - 1) / nblk;
     cb = std::min(cb_max, (cb + G_ - 1) / G_ * G_);
-    const int L1 = p->lmax + 1;
-    const size_t smem = (size_t)LR_LMAX * 16 + LR_EC * 16 + LR_EC * 8 + (size_t)LR_EC * cb * L1 * 4;
+    // whole in-edge lists in one chunk where they fit: the staging of R~ (two dependent global loads and two barriers
+    // per chunk) is exposed, one CTA per SM
+    const size_t fixed = (size_t)LR_EC * 16 + LR_EC * 8 + (size_t)(odd ? 8 : 3) * QP * 16;
+    const int L1p = round_up(p->LB + 1, 4);
+    int EC = LR_EC;
+    while (EC > 1 && fixed + (size_t)EC * cb * L1p * 4 > 160 * 1024) EC >>= 1;
+    const size_t smem = fixed + (size_t)EC * cb * L1p * 4;
     if (smem > 200 * 1024) { set_error("edge kernel (l1-dependent radial): channel block too large"); return CGTP_ERR_UNSUPPORTED; }
     const int64_t grid = nodes * (int64_t)((Cpar + cb - 1) / cb);
     if (grid > 2147483647LL) { set_error("edge kernel (l1-dependent radial): too many work items"); return CGTP_ERR_UNSUPPORTED; }
     const int nb = (Cpar + cb - 1) / cb;
     LaunchScope scope(odd ? K_EDGE_ODD : K_EDGE_EVEN, st);
-    if (odd) {
-        auto kern = edge_lr_kernel<true, 2>;
-        CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kern<<<(unsigned)grid, LR_NT, smem, st>>>(*p, G, row_ptr, edge_index, edge_vec, edge_radial, perm_par, Cpar, C, cb, nb,
-                                                  G_, S, status);
-    } else {
-        auto kern = edge_lr_kernel<false, 4>;
-        CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kern<<<(unsigned)grid, LR_NT, smem, st>>>(*p, G, row_ptr, edge_index, edge_vec, edge_radial, perm_par, Cpar, C, cb, nb,
-                                                  G_, S, status);
+    void (*kern)(Plan, const float*, const int64_t*, const int64_t*, const float*, const float*, const int*, int, int, int, int,
+                 int, int, float*, const int32_t*) = nullptr;
+    switch (p->LB) {
+#define CGTP_CASE(B) \
+    case B:          \
+        kern = odd ? edge_lr_kernel<true, 4, B> : edge_lr_kernel<false, 4, B>; \
+        break;
+        CGTP_FOR_EACH_BAND(CGTP_CASE)
+#undef CGTP_CASE
     }
+    if (!kern) { set_error("edge kernel (l1-dependent radial): no kernel for band limit %d", p->LB); return CGTP_ERR_UNSUPPORTED; }
+    CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<(unsigned)grid, LR_NT, smem, st>>>(*p, G, row_ptr, edge_index, edge_vec, edge_radial, perm_par, Cpar, C, cb, nb, G_, EC,
+                                              S, status);
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
 }
