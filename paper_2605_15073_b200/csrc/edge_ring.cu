@@ -5,9 +5,11 @@
 //     in-edges and streams the sender's grid block from HBM into a shared-memory ring with TMA bulk
 //     copies (cp.async.bulk + mbarrier complete_tx), one stage = one (edge, channel sub-block) span,
 //     contiguous and 16-byte aligned in the G layout of message.cu;
-//   * eight consumer warps evaluate the channel-independent edge field K_e on the grid (Legendre
-//     recurrence in r_e . Omega, chunks of edges), multiply it and R~[e,c] with the staged sender grid
-//     and accumulate in registers in input edge order -- deterministic, no floating-point atomics;
+//   * sixteen consumer warps evaluate the channel-independent edge field(s) K_e on the grid (Legendre
+//     recurrence in r_e . Omega, chunks of edges, two edges per packed operation), multiply them and R~[e,c]
+//     with the staged sender VALUE grid and accumulate in registers in input edge order -- deterministic, no
+//     floating-point atomics; odd channels pair the value grid with (d_theta K_e, -(1/sin) d_phi K_e) into two
+//     pooled grids, the derivatives of Y_lm being applied by the analysis (curl pairing by parts);
 //   * the ring keeps tens of KB per SM in flight independent of occupancy, which is what an
 //     HBM-latency-bound gather needs; S is written once per receiver with 128-bit stores.
 // The arithmetic per grid point is identical to edge_kernel in message.cu (kept as the fallback).

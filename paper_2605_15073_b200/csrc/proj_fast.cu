@@ -337,8 +337,7 @@ int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st
     const bool wide = maxM <= 32;          // 32 rows x 512 columns, else 64 rows x 256 columns
     const int MW = wide ? 32 : 64, CWT = wide ? 512 : 256;
     const size_t wbytes = (size_t)maxK * MW * 4;
-    const size_t kTwo = 113 * 1024, kOne = 226 * 1024;
-    const size_t budget = kOne;
+    const size_t budget = 226 * 1024;  // one CTA per SM
     if (wbytes + 2 * 4096 + 64 > budget) return CGTP_OK;
 
     // K chunk: divides every K, chunk bytes a multiple of 16
