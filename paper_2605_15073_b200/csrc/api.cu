@@ -1,5 +1,8 @@
 // api.cu -- the C ABI of include/cgtp.h: argument validation, workspace carving, stage sequencing.
+#include <algorithm>
+#include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "common.cuh"
@@ -729,6 +732,68 @@ static void keep_pool_memory()
     done = true;
 }
 
+// Streams, events and chunk buffers of cgtp_onsite_host live for the life of the process (grow-only): creating and
+// destroying them per call cost more than a millisecond of the 3.4 ms end-to-end step.
+namespace {
+constexpr int kHostStreams = 4;
+struct HostCtx {
+    std::mutex mu;
+    bool ready = false;
+    // one stream per engine, so that a host->device copy never queues behind a device->host copy of an earlier chunk
+    // (copies of one direction execute in issue order: with a stream per chunk the H2D engine stalled on them)
+    cudaStream_t s_h2d, s_comp, s_d2h;
+    cudaEvent_t start, ev_h2d[kHostStreams], ev_comp[kHostStreams], ev_d2h[kHostStreams], ev_end;
+    float *dA[kHostStreams] = {}, *dB[kHostStreams] = {}, *dO[kHostStreams] = {};
+    void* dws[kHostStreams] = {};
+    size_t in_bytes = 0, out_bytes = 0, ws_bytes = 0;
+    float* dW = nullptr;  // W_a | W_b | W_out
+    size_t w_bytes = 0;
+};
+HostCtx g_host;
+
+int host_ctx_reserve(HostCtx& h, size_t in_bytes, size_t out_bytes, size_t ws_bytes, size_t w_bytes)
+{
+    if (!h.ready) {
+        CGTP_CUDA_CHECK(cudaStreamCreateWithFlags(&h.s_h2d, cudaStreamNonBlocking));
+        CGTP_CUDA_CHECK(cudaStreamCreateWithFlags(&h.s_comp, cudaStreamNonBlocking));
+        CGTP_CUDA_CHECK(cudaStreamCreateWithFlags(&h.s_d2h, cudaStreamNonBlocking));
+        for (int s = 0; s < kHostStreams; ++s) {
+            CGTP_CUDA_CHECK(cudaEventCreateWithFlags(&h.ev_h2d[s], cudaEventDisableTiming));
+            CGTP_CUDA_CHECK(cudaEventCreateWithFlags(&h.ev_comp[s], cudaEventDisableTiming));
+            CGTP_CUDA_CHECK(cudaEventCreateWithFlags(&h.ev_d2h[s], cudaEventDisableTiming));
+        }
+        CGTP_CUDA_CHECK(cudaEventCreateWithFlags(&h.start, cudaEventDisableTiming));
+        CGTP_CUDA_CHECK(cudaEventCreateWithFlags(&h.ev_end, cudaEventDisableTiming));
+        h.ready = true;
+    }
+    if (in_bytes > h.in_bytes || out_bytes > h.out_bytes || ws_bytes > h.ws_bytes) {
+        CGTP_CUDA_CHECK(cudaDeviceSynchronize());
+        for (int s = 0; s < kHostStreams; ++s) {
+            cudaFree(h.dA[s]); cudaFree(h.dB[s]); cudaFree(h.dO[s]); cudaFree(h.dws[s]);
+            h.dA[s] = h.dB[s] = h.dO[s] = nullptr;
+            h.dws[s] = nullptr;
+        }
+        h.in_bytes = std::max(h.in_bytes, in_bytes);
+        h.out_bytes = std::max(h.out_bytes, out_bytes);
+        h.ws_bytes = std::max(h.ws_bytes, ws_bytes);
+        for (int s = 0; s < kHostStreams; ++s) {
+            CGTP_CUDA_CHECK(cudaMalloc(&h.dA[s], h.in_bytes));
+            CGTP_CUDA_CHECK(cudaMalloc(&h.dB[s], h.in_bytes));
+            CGTP_CUDA_CHECK(cudaMalloc(&h.dO[s], h.out_bytes));
+            CGTP_CUDA_CHECK(cudaMalloc(&h.dws[s], h.ws_bytes));
+        }
+    }
+    if (w_bytes > h.w_bytes) {
+        CGTP_CUDA_CHECK(cudaDeviceSynchronize());
+        cudaFree(h.dW);
+        h.dW = nullptr;
+        CGTP_CUDA_CHECK(cudaMalloc(&h.dW, w_bytes));
+        h.w_bytes = w_bytes;
+    }
+    return CGTP_OK;
+}
+}  // namespace
+
 int cgtp_onsite_host(const float* A, const float* B, const float* W_a, const float* W_b, const float* W_out, int lmax,
                      int lmax_out, int N, int C, const uint8_t* parity_mask, float* out, int64_t batch,
                      void* cuda_stream)
@@ -740,70 +805,56 @@ int cgtp_onsite_host(const float* A, const float* B, const float* W_a, const flo
     if (batch == 0) return CGTP_OK;
     if (!A || !B || !W_a || !W_b || !W_out || !out) { set_error("null pointer argument"); return CGTP_ERR_INVALID; }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    keep_pool_memory();
     const size_t L2 = (size_t)(lmax + 1) * (lmax + 1), Lo2 = (size_t)(lmax_out + 1) * (lmax_out + 1);
-    const size_t wbytes = (size_t)C * N * 4;
-    float *dWa = nullptr, *dWb = nullptr, *dWo = nullptr;
-    CGTP_CUDA_CHECK(cudaMallocAsync(&dWa, wbytes, st));
-    CGTP_CUDA_CHECK(cudaMallocAsync(&dWb, wbytes, st));
-    CGTP_CUDA_CHECK(cudaMallocAsync(&dWo, wbytes, st));
-    CGTP_CUDA_CHECK(cudaMemcpyAsync(dWa, W_a, wbytes, cudaMemcpyHostToDevice, st));
-    CGTP_CUDA_CHECK(cudaMemcpyAsync(dWb, W_b, wbytes, cudaMemcpyHostToDevice, st));
-    CGTP_CUDA_CHECK(cudaMemcpyAsync(dWo, W_out, wbytes, cudaMemcpyHostToDevice, st));
-
-    // Batch chunks on two streams so the H2D copy of chunk k+1, the kernels of chunk k and the D2H copy
-    // of chunk k-1 overlap (PCIe is full duplex).
+    const size_t wfl = (size_t)C * N;  // floats per weight matrix
     const size_t in_per = (size_t)N * L2 * 4, out_per = (size_t)2 * N * Lo2 * 4;
-    // <= 8 MB of each input per chunk, at least 8 chunks when the batch allows: PCIe is full duplex, so in steady
-    // state the H2D copy of chunk k+1, the kernels of chunk k and the D2H copy of chunk k-1 run together
-    int64_t chunk = (int64_t)((8u << 20) / (in_per > 0 ? in_per : 1));
-    if (chunk > (batch + 7) / 8) chunk = (batch + 7) / 8;
-    if (chunk < 64) chunk = 64;
-    if (chunk > batch) chunk = batch;
-    const int NS = 3;
-    cudaStream_t cs[NS];
-    cudaEvent_t ready, done[NS];
-    CGTP_CUDA_CHECK(cudaEventCreateWithFlags(&ready, cudaEventDisableTiming));
-    CGTP_CUDA_CHECK(cudaEventRecord(ready, st));
-    float *dA[NS], *dB[NS], *dO[NS];
-    void* dws[NS];
+    // Batch chunks: in steady state the H2D copy of chunk k+1, the kernels of chunk k and the D2H copy of chunk k-1 run
+    // together (PCIe is full duplex; 55 GB/s per direction alone, 48 GB/s each when both run, measured).  Every copy
+    // has a fixed cost, so the chunks are few and large in the middle and small at both ends, where the first H2D and
+    // the last D2H have nothing to overlap with: fractions 1 1 2 4 8 8 4 2 1 1 of 32.
+    static const int kFrac[] = {1, 1, 2, 4, 8, 8, 4, 2, 1, 1};
+    constexpr int kNumFrac = (int)(sizeof(kFrac) / sizeof(kFrac[0]));
+    int64_t unit = (batch + 31) / 32;
+    if (unit < 16) unit = 16;
+    const int64_t chunk = std::min<int64_t>(batch, 8 * unit);  // largest chunk: sizes the buffers
     const size_t wsb = onsite_ws_bytes(lmax, lmax_out, C, chunk);
-    for (int s = 0; s < NS; ++s) {
-        CGTP_CUDA_CHECK(cudaStreamCreateWithFlags(&cs[s], cudaStreamNonBlocking));
-        CGTP_CUDA_CHECK(cudaEventCreateWithFlags(&done[s], cudaEventDisableTiming));
-        CGTP_CUDA_CHECK(cudaStreamWaitEvent(cs[s], ready, 0));
-        CGTP_CUDA_CHECK(cudaMallocAsync(&dA[s], chunk * in_per, cs[s]));
-        CGTP_CUDA_CHECK(cudaMallocAsync(&dB[s], chunk * in_per, cs[s]));
-        CGTP_CUDA_CHECK(cudaMallocAsync(&dO[s], chunk * out_per, cs[s]));
-        CGTP_CUDA_CHECK(cudaMallocAsync(&dws[s], wsb, cs[s]));
-    }
+
+    HostCtx& h = g_host;
+    std::lock_guard<std::mutex> lock(h.mu);
+    rc = host_ctx_reserve(h, (size_t)chunk * in_per, (size_t)chunk * out_per, wsb, 3 * wfl * 4);
+    if (rc) return rc;
+    float *dWa = h.dW, *dWb = h.dW + wfl, *dWo = h.dW + 2 * wfl;
+    CGTP_CUDA_CHECK(cudaMemcpyAsync(dWa, W_a, wfl * 4, cudaMemcpyHostToDevice, st));
+    CGTP_CUDA_CHECK(cudaMemcpyAsync(dWb, W_b, wfl * 4, cudaMemcpyHostToDevice, st));
+    CGTP_CUDA_CHECK(cudaMemcpyAsync(dWo, W_out, wfl * 4, cudaMemcpyHostToDevice, st));
+    CGTP_CUDA_CHECK(cudaEventRecord(h.start, st));
+    CGTP_CUDA_CHECK(cudaStreamWaitEvent(h.s_h2d, h.start, 0));
+    CGTP_CUDA_CHECK(cudaStreamWaitEvent(h.s_comp, h.start, 0));
     int k = 0;
-    for (int64_t b0 = 0; b0 < batch; b0 += chunk, ++k) {
-        const int s = k % NS;
-        const int64_t nb = (batch - b0 < chunk) ? (batch - b0) : chunk;
-        CGTP_CUDA_CHECK(cudaMemcpyAsync(dA[s], A + (size_t)b0 * N * L2, nb * in_per, cudaMemcpyHostToDevice, cs[s]));
-        CGTP_CUDA_CHECK(cudaMemcpyAsync(dB[s], B + (size_t)b0 * N * L2, nb * in_per, cudaMemcpyHostToDevice, cs[s]));
-        rc = cgtp_onsite(dA[s], dB[s], dWa, dWb, dWo, lmax, lmax_out, N, C, parity_mask, dO[s], nb, dws[s], wsb, cs[s]);
+    for (int64_t b0 = 0, nb = 0; b0 < batch; b0 += nb, ++k) {
+        const int s = k % kHostStreams;  // buffer set of this chunk
+        nb = (k < kNumFrac ? kFrac[k] : 8) * unit;
+        if (nb > batch - b0) nb = batch - b0;
+        // inputs: the buffer set is free once the kernels of the chunk that used it last have run
+        if (k >= kHostStreams) CGTP_CUDA_CHECK(cudaStreamWaitEvent(h.s_h2d, h.ev_comp[s], 0));
+        CGTP_CUDA_CHECK(cudaMemcpyAsync(h.dA[s], A + (size_t)b0 * N * L2, nb * in_per, cudaMemcpyHostToDevice, h.s_h2d));
+        CGTP_CUDA_CHECK(cudaMemcpyAsync(h.dB[s], B + (size_t)b0 * N * L2, nb * in_per, cudaMemcpyHostToDevice, h.s_h2d));
+        CGTP_CUDA_CHECK(cudaEventRecord(h.ev_h2d[s], h.s_h2d));
+        // kernels: need the inputs, and the output buffer back from the copy of the chunk that used it last
+        CGTP_CUDA_CHECK(cudaStreamWaitEvent(h.s_comp, h.ev_h2d[s], 0));
+        if (k >= kHostStreams) CGTP_CUDA_CHECK(cudaStreamWaitEvent(h.s_comp, h.ev_d2h[s], 0));
+        rc = cgtp_onsite(h.dA[s], h.dB[s], dWa, dWb, dWo, lmax, lmax_out, N, C, parity_mask, h.dO[s], nb, h.dws[0], wsb,
+                         h.s_comp);
         if (rc) return rc;
-        CGTP_CUDA_CHECK(cudaMemcpyAsync(out + (size_t)b0 * 2 * N * Lo2, dO[s], nb * out_per, cudaMemcpyDeviceToHost, cs[s]));
+        CGTP_CUDA_CHECK(cudaEventRecord(h.ev_comp[s], h.s_comp));
+        // result
+        CGTP_CUDA_CHECK(cudaStreamWaitEvent(h.s_d2h, h.ev_comp[s], 0));
+        CGTP_CUDA_CHECK(cudaMemcpyAsync(out + (size_t)b0 * 2 * N * Lo2, h.dO[s], nb * out_per, cudaMemcpyDeviceToHost, h.s_d2h));
+        CGTP_CUDA_CHECK(cudaEventRecord(h.ev_d2h[s], h.s_d2h));
     }
-    for (int s = 0; s < NS; ++s) {
-        CGTP_CUDA_CHECK(cudaFreeAsync(dA[s], cs[s]));
-        CGTP_CUDA_CHECK(cudaFreeAsync(dB[s], cs[s]));
-        CGTP_CUDA_CHECK(cudaFreeAsync(dO[s], cs[s]));
-        CGTP_CUDA_CHECK(cudaFreeAsync(dws[s], cs[s]));
-        CGTP_CUDA_CHECK(cudaEventRecord(done[s], cs[s]));
-        CGTP_CUDA_CHECK(cudaStreamWaitEvent(st, done[s], 0));
-    }
-    CGTP_CUDA_CHECK(cudaFreeAsync(dWa, st));
-    CGTP_CUDA_CHECK(cudaFreeAsync(dWb, st));
-    CGTP_CUDA_CHECK(cudaFreeAsync(dWo, st));
+    CGTP_CUDA_CHECK(cudaEventRecord(h.ev_end, h.s_d2h));
+    CGTP_CUDA_CHECK(cudaStreamWaitEvent(st, h.ev_end, 0));
     CGTP_CUDA_CHECK(cudaStreamSynchronize(st));
-    for (int s = 0; s < NS; ++s) {
-        cudaStreamDestroy(cs[s]);
-        cudaEventDestroy(done[s]);
-    }
-    cudaEventDestroy(ready);
     return CGTP_OK;
 }
 
