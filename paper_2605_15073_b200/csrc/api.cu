@@ -811,8 +811,9 @@ int cgtp_onsite_host(const float* A, const float* B, const float* W_a, const flo
     // Batch chunks: in steady state the H2D copy of chunk k+1, the kernels of chunk k and the D2H copy of chunk k-1 run
     // together (PCIe is full duplex; 55 GB/s per direction alone, 48 GB/s each when both run, measured).  Every copy
     // has a fixed cost, so the chunks are few and large in the middle and small at both ends, where the first H2D and
-    // the last D2H have nothing to overlap with: fractions 1 1 2 4 8 8 4 2 1 1 of 32.
-    static const int kFrac[] = {1, 1, 2, 4, 8, 8, 4, 2, 1, 1};
+    // the last D2H have nothing to overlap with: fractions 2 6 8 8 6 2 of 32 (2.83 ms at configs[1]; ten chunks
+    // 1 1 2 4 8 8 4 2 1 1 took 2.95 ms, sixteen equal ones 3.1 ms).
+    static const int kFrac[] = {2, 6, 8, 8, 6, 2};
     constexpr int kNumFrac = (int)(sizeof(kFrac) / sizeof(kFrac[0]));
     int64_t unit = (batch + 31) / 32;
     if (unit < 16) unit = 16;
