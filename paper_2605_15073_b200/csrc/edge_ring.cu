@@ -180,22 +180,22 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
             const int ne = (int)((e_end - e0 < a.EC) ? (e_end - e0) : a.EC);
             // ---- M3: edge fields of the chunk on the grid (Eq.(48),(50); addition theorem, R12):
             // K(t) = sum_l (2l+1)/(4 pi) P_l(t), K'(t) likewise with P'_l = t P'_{l-1} + l P_{l-1}, t = r_e . Omega.
-            // Thread = grid point (geometry read once per chunk), two edges per pass in the halves of packed
-            // FP32 operations; ER_CONS / UVp thread sets share the edge pairs when the grid is small.
+            // Two edges per work item in the halves of packed FP32 operations.
             {
-                const int qs = (UVp <= ER_CONS) ? UVp : ER_CONS;
-                const int nset = (UVp <= ER_CONS) ? ER_CONS / UVp : 1;
-                const int set = tid / qs;
-                if (set < nset) {
-                    for (int q = tid - set * qs; q < UVp; q += qs) {
-                        const bool live = q < a.p.UV;
-                        const float gx = geo[q], gy = geo[UVp + q], gz = geo[2 * UVp + q];
-                        float tx = 0.f, ty = 0.f, tz = 0.f, fx = 0.f, fy = 0.f;
-                        if (ODD) {
-                            tx = geo[3 * UVp + q]; ty = geo[4 * UVp + q]; tz = geo[5 * UVp + q];
-                            fx = geo[6 * UVp + q]; fy = geo[7 * UVp + q];
-                        }
-                        for (int el = 2 * set; el < ne; el += 2 * nset) {
+                // work items = (edge pair, grid point), dealt over all consumer threads
+                const int total = ((ne + 1) >> 1) * UVp;
+                {
+                    {
+                        for (int w = tid; w < total; w += ER_CONS) {
+                            const int pr = w / UVp, q = w - pr * UVp;
+                            const int el = 2 * pr;
+                            const bool live = q < a.p.UV;
+                            const float gx = geo[q], gy = geo[UVp + q], gz = geo[2 * UVp + q];
+                            float tx = 0.f, ty = 0.f, tz = 0.f, fx = 0.f, fy = 0.f;
+                            if (ODD) {
+                                tx = geo[3 * UVp + q]; ty = geo[4 * UVp + q]; tz = geo[5 * UVp + q];
+                                fx = geo[6 * UVp + q]; fy = geo[7 * UVp + q];
+                            }
                             const int el1 = (el + 1 < ne) ? el + 1 : el;
                             const float4 ea = Ebuf[el], eb = Ebuf[el1];
                             const float2 t = make_float2(fmaf(ea.x, gx, fmaf(ea.y, gy, ea.z * gz)),
