@@ -1,14 +1,15 @@
-// sht_fast.cu -- lane = column forms of node synthesis (row M2 of SURVEY.md 8(a); Eq.(49), (51) PAPER.md:404-:410) and of
-// the per-receiver analysis (row M5; Eq.(53)-(54) :420-:422) for band limits whose 32-column tile fits shared memory.
-// Same mathematics and the same folding as the generic kernels of message.cu / sht.cuh; what differs is the mapping:
+// sht_fast.cu -- lane = column form of node synthesis (row M2 of SURVEY.md 8(a); Eq.(49), (51) PAPER.md:404-:410) for
+// band limits whose 32-column tile fits shared memory.  Same mathematics and the same folding as the generic kernel of
+// message.cu / sht.cuh; what differs is the mapping:
 //   * a CTA works on groups of 32 (node, rank-channel) columns, lane = column: every shared-memory array has the
 //     column as its fastest index or an odd column stride, so no access has a bank conflict, and every table value is
 //     a warp-wide broadcast (one 128-bit load feeds four packed FMAs);
-//   * packed FP32 FMAs: the pair is (+m, -m) in the Legendre stages and (north row u, south row U-1-u) in the
-//     Fourier stages;
-//   * the grid tile of the group is staged in shared memory and moved to / from HBM with coalesced accesses.
-// The generic kernels shared one table row among lanes of different m (conflicts, divergent trip counts) and ran the
-// shared-memory pipe at 78 % for 25 % FMA-pipe activity (profiles/r01f_message_config4_ncu.txt).
+//   * packed FP32 FMAs: the pair is (+m, -m) in the Legendre stage and (north row u, south row U-1-u) in the
+//     Fourier stage;
+//   * the grid tile of the group is staged in shared memory and written to HBM with coalesced stores.
+// The generic kernel shares one table row among lanes of different m (conflicts, divergent trip counts) and runs the
+// shared-memory pipe at 78 % for 25 % FMA-pipe activity (profiles/r01f_message_config4_ncu.txt); this one is
+// issue-bound at 61 % (profiles/r01g_message_config4_ncu.txt).  The per-receiver analysis (M5) still uses the generic form.
 #include <algorithm>
 
 #include "sht.cuh"
