@@ -573,3 +573,28 @@ def test_message_lwr(lmax, lmax_out, N, C, nodes, mask):
     again = cg.cgtp_message_lwr(_cuda(m.node_feats), _cuda(m.edge_index), _cuda(m.edge_vec), _cuda(rad), _cuda(Wn),
                                 _cuda(Wo), lmax, lmax_out, N, C, m.parity_mask).cpu().numpy()
     assert np.array_equal(got, again)  # bitwise reproducible
+
+
+def test_message_lwr_equivariance_and_inversion():
+    """The full parameterisation on the device path (cgtp_message_lwr) under a random rotation and under inversion: weights
+    and radial factor act within a degree, so both sectors still rotate with D^l (App. B test 5 PAPER.md:633) and pick up
+    their parity labels (Table I :86-:93)."""
+    lmax, N, C, nodes = 5, 8, 8, 40
+    m = synthetic.make_message(lmax, lmax, N, C, nodes, 9, seed=33)
+    (Wn,), Wo = synthetic.lw_weights(lmax, lmax, N, C, seed=33, n_in=1)
+    rad = (m.edge_radial[:, :, None] * np.random.default_rng(4).uniform(0.5, 1.5, (m.E, C, lmax + 1))).astype(np.float32)
+
+    def run(X, ev):
+        return cg.cgtp_message_lwr(_cuda(X.astype(np.float32)), _cuda(m.edge_index), _cuda(ev.astype(np.float32)), _cuda(rad),
+                                   _cuda(Wn), _cuda(Wo), lmax, lmax, N, C, m.parity_mask).cpu().numpy().astype(np.float64)
+
+    base = run(m.node_feats, m.edge_vec)
+    R = shref.random_rotation(np.random.default_rng(29))
+    D = shref.wigner_D_real(lmax, R)
+    rot = run(np.einsum("ab,...b->...a", D, m.node_feats.astype(np.float64)), m.edge_vec.astype(np.float64) @ R.T)
+    e = sector_err(rot, np.einsum("ab,...b->...a", D, base))
+    assert max(e) < TOL, e
+    sign = np.concatenate([np.full(2 * l + 1, (-1.0) ** l) for l in range(lmax + 1)])
+    inv = run(m.node_feats * sign, -m.edge_vec)
+    assert np.abs(inv[:, 0] - base[:, 0] * sign).max() < TOL * np.abs(base[:, 0]).max()
+    assert np.abs(inv[:, 1] + base[:, 1] * sign).max() < TOL * np.abs(base[:, 1]).max()
