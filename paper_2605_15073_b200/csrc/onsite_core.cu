@@ -46,12 +46,16 @@ struct CorePlan {
 };
 
 __host__ __device__ constexpr int core_uhmax(int LB) { return ((3 * LB + 2) / 2 + 1) / 2; }
-// Columns per group: 32 (lane = column); 16 at band limit 20, where a warp works on two items at once (one per
-// half-warp) because H, T and F of 32 columns do not fit shared memory.
-__host__ __device__ constexpr int core_gw(int LB) { return LB >= 20 ? 16 : 32; }
+// Columns per group: 32 (lane = column) at the small band limits; 16 from band limit 8 up (and for the odd channels at
+// 6), where a warp works on two schedule items at once, one per half-warp: twice as many schedule slots balance the
+// ragged per-m work and halve the shared memory per group.  Measured (configs[3], core even / odd, 32 -> 16 columns):
+// lmax 8: 226 / 527 -> 205 / 402 us; 12: 1.25 / 1.80 -> 0.67 / 1.15 ms; 16: 3.16 / 4.77 -> 2.04 / 3.80 ms (odd with
+// four-node row blocks); 20 odd (four-node row blocks): 11.2 -> 6.0 ms; configs[1] odd 106 -> 97 us, even 56 -> 63 us
+// (kept at 32); lmax 2 and 4 are slower with 16.
+__host__ __device__ constexpr int core_gw(int LB, bool odd) { return (LB >= 8 || (LB == 6 && odd)) ? 16 : 32; }
 // Northern nodes per row block of the fast kernel: all of them (one block) for band limits <= 8; four for the
-// larger ones, two where four do not fit shared memory (odd channels at band limit 16).
-__host__ __device__ constexpr int core_ub(int LB, bool odd) { return LB <= 8 ? core_uhmax(LB) : (LB >= 16 && odd) ? 2 : 4; }
+// larger ones.
+__host__ __device__ constexpr int core_ub(int LB, bool odd) { return LB <= 8 ? core_uhmax(LB) : 4; }
 
 // ------------------------------------------------------------------------------------------------
 // Host: packed tables + static schedules
@@ -100,7 +104,7 @@ static std::vector<CorePlan*> g_core_plans;
 static size_t core_smem_bytes(const Plan* p, bool odd, const CoreTab& t, bool dbl)
 {
     const int MR = 2 * p->LB + 1;
-    const size_t gw = core_gw(p->LB);
+    const size_t gw = core_gw(p->LB, odd);
     const size_t hs = (size_t)2 * gw * onsite_fast_hstride(p) * 4;
     const size_t f = (size_t)(odd ? 4 : 2) * MR * (2 * core_ub(p->LB, odd)) * gw * 4;
     const size_t ts = gw * onsite_fast_tstride(p) * 4;
@@ -177,7 +181,7 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
     stage_items(p, odd, items);
     int bestNW = 4;
     double best = -1.0;
-    const int NH = 32 / core_gw(LB);  // workers (schedule slots) per warp
+    const int NH = 32 / core_gw(LB, odd);  // workers (schedule slots) per warp
     for (int NW = 4; NW <= kMaxWarps; ++NW) {
         double total = 0.0, span = 0.0;
         for (int s = 0; s < 3; ++s) {
@@ -603,7 +607,7 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int MR = 2 * LB + 1;
     constexpr int UB = core_ub(LB, ODD), RB = 2 * UB;
-    constexpr int GW = core_gw(LB), NH = 32 / GW;  // columns per group; schedule slots (workers) per warp
+    constexpr int GW = core_gw(LB, ODD), NH = 32 / GW;  // columns per group; schedule slots (workers) per warp
     constexpr bool TWO_TERM = ODD && LB >= 20;     // four coefficient vectors of 2 LB + 1 pairs exceed the registers
     uint64_t* bar_tab = reinterpret_cast<uint64_t*>(smem);
     uint64_t* bar_h = reinterpret_cast<uint64_t*>(smem + 16);  // [2]
@@ -759,7 +763,7 @@ static int launch_fast_t(const Plan* p, const CorePlan* c, const float* Ha, cons
     a.Ha = Ha;
     a.Hb = Hb;
     a.T = T;
-    constexpr int GW = core_gw(LB);
+    constexpr int GW = core_gw(LB, ODD);
     a.ngroups = (ncols + GW - 1) / GW;  // the caller pads the column count to a multiple of 32
     a.lmax = p->lmax;
     a.lmax_out = p->lmax_out;
