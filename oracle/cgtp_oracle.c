@@ -36,7 +36,10 @@
  * (oracle_*_parity) against the paper's dispatch check B7 (:647), the reduction to the natural-parity
  * functions, Eq.(44)-(45)/(56) slot rules, inversion and rotation; the l-dependent-weight functions
  * (oracle_*_lw) against the l-shared functions (equal weights, degree selection, per-degree numpy
- * projections around them) and rotation.  No function here is "parity unpinned".
+ * projections around them) and rotation; the nu-body function (oracle_onsite_nbody) against fine-grid
+ * quadrature of the pointwise product, the closed form Y_10^3 = (3/4pi)^(3/2) (3/5 z + 2/5 P_3(z)), the
+ * reduction to oracle_onsite at nu = 2, factor permutation and rotation (tests/test_oracle_nbody.py).
+ * No function here is "parity unpinned".
  *
  * Plain C99 + OpenMP, double precision (long double inside the Racah sum).
  */
@@ -813,6 +816,86 @@ int oracle_message_lwr(const double *node_feats, const int64_t *edge_index, cons
 {
     return message_lw_impl(node_feats, edge_index, edge_vec, edge_radial, 1, W_node, W_out, lmax, lmax_out, N, C,
                            parity_mask, out, nodes, E);
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* nu-body on-site product (end of Sec. VI): "The grid pointwise product extends */
+/* to nu-body features through additional pointwise multiplications on the grid followed by a  */
+/* single inverse transform".  What that reaches exactly is the plain definition                */
+/*   T[c,lm] = int prod_{s=1..nu} A~(s)_c(Omega) Y_lm(Omega) dOmega,  A~(s)_c = sum_i H(s)[c,i] Y_i, */
+/*   H(s)[c,:] = W_in[s][c,:] . X[s][b]   (Eq.(35) :322 per factor),                            */
+/*   out[b,n,lm] = sum_c W_out[n,c] T[c,lm]   (Eq.(41) :346; a product of natural-parity fields  */
+/*   has natural parity: one sector).                                                           */
+/* Written out with the real Gaunt tensor Gr (Eq.(4)-(5)) applied nu-1 times, the intermediate   */
+/* products kept at their FULL band k*lmax (a product of k fields of band lmax has band k*lmax;  */
+/* truncating it earlier would change the result):                                               */
+/*   P_1 = H(1);  P_k[i] = sum_{a,b} Gr(a,b;i) P_{k-1}[a] H(k)[b],  band k*lmax;                 */
+/*   T = P_nu restricted to l <= lmax_out.                                                       */
+/* Nothing here touches a quadrature grid.  Reading R19: l-shared weights, rank       */
+/* channels of the pointwise (even) kind only -- the curl pairing is bilinear and the paper       */
+/* gives no nu-body form of it.  Layouts: X [nu,batch,N,(lmax+1)^2]; W_in [nu,C,N]; W_out [N,C];  */
+/* out [batch,N,(lmax_out+1)^2].                                                                  */
+/* ------------------------------------------------------------------------------------------ */
+int oracle_onsite_nbody(const double *X, const double *W_in, const double *W_out, int nu, int lmax, int lmax_out,
+                        int N, int C, double *out, int64_t batch)
+{
+    if (nu < 1 || nu > 8 || lmax < 0 || lmax_out < 0 || lmax_out > nu * lmax) return 1;
+    int L2 = (lmax + 1) * (lmax + 1), Lo2 = (lmax_out + 1) * (lmax_out + 1);
+    /* step k (2..nu): left band (k-1)*lmax, right band lmax, output band k*lmax (last step: lmax_out) */
+    const coupling_t *tab[9];
+    int lin[9], lout[9];
+    for (int k = 2; k <= nu; ++k) {
+        lin[k] = (k - 1) * lmax;
+        lout[k] = (k == nu) ? lmax_out : k * lmax;
+        tab[k] = get_coupling(lin[k], lout[k], 0);
+        if (!tab[k]) return 2;
+    }
+    int Pmax = (nu * lmax + 1) * (nu * lmax + 1);
+#pragma omp parallel
+    {
+        double *H = malloc((size_t)nu * C * L2 * sizeof(double));
+        double *P = malloc((size_t)Pmax * sizeof(double));
+        double *Pn = malloc((size_t)Pmax * sizeof(double));
+        double *T = malloc((size_t)C * Lo2 * sizeof(double));
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t b = 0; b < batch; ++b) {
+            for (int s = 0; s < nu; ++s) {
+                const double *Xb = X + ((int64_t)s * batch + b) * N * L2;
+                const double *W = W_in + (size_t)s * C * N;
+                for (int c = 0; c < C; ++c)
+                    for (int i = 0; i < L2; ++i) {
+                        double acc = 0.0;
+                        for (int n = 0; n < N; ++n) acc += W[c * N + n] * Xb[n * L2 + i];
+                        H[((size_t)s * C + c) * L2 + i] = acc;
+                    }
+            }
+            for (int c = 0; c < C; ++c) {
+                for (int i = 0; i < Pmax; ++i) P[i] = 0.0;
+                for (int i = 0; i < L2; ++i) P[i] = H[(size_t)c * L2 + i];
+                if (nu == 1) { /* single field: T = H restricted to lmax_out (lmax_out <= lmax) */ }
+                for (int k = 2; k <= nu; ++k) {
+                    const coupling_t *t = tab[k];
+                    const double *h = H + ((size_t)(k - 1) * C + c) * L2;
+                    int no = (lout[k] + 1) * (lout[k] + 1);
+                    for (int i = 0; i < Pmax; ++i) Pn[i] = 0.0;
+                    for (int64_t q = 0; q < t->nnz; ++q)
+                        if (t->i2[q] < L2) /* factor k has band lmax; the table covers band (k-1)*lmax on both sides */
+                            Pn[t->io[q]] += t->val[q] * P[t->i1[q]] * h[t->i2[q]];
+                    for (int i = 0; i < Pmax; ++i) P[i] = (i < no) ? Pn[i] : 0.0;
+                }
+                for (int i = 0; i < Lo2; ++i) T[(size_t)c * Lo2 + i] = P[i];
+            }
+            double *ob = out + b * (int64_t)N * Lo2;
+            for (int n = 0; n < N; ++n)
+                for (int i = 0; i < Lo2; ++i) {
+                    double acc = 0.0;
+                    for (int c = 0; c < C; ++c) acc += W_out[n * C + c] * T[(size_t)c * Lo2 + i];
+                    ob[(size_t)n * Lo2 + i] = acc;
+                }
+        }
+        free(H); free(P); free(Pn); free(T);
+    }
+    return 0;
 }
 
 int oracle_num_threads(void)

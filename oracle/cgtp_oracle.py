@@ -70,6 +70,8 @@ def _load():
     lib.oracle_message_lw.argtypes = [p, p, p, p, p, p, i, i, i, i, p, p, i64, i64]
     lib.oracle_message_lwr.restype = i
     lib.oracle_message_lwr.argtypes = lib.oracle_message_lw.argtypes
+    lib.oracle_onsite_nbody.restype = i
+    lib.oracle_onsite_nbody.argtypes = [p, p, p, i, i, i, i, i, p, i64]
     lib.oracle_num_threads.restype = i
     lib.oracle_num_threads.argtypes = []
     _lib = lib
@@ -282,6 +284,20 @@ def message_lwr(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, lm
                                     N, C, _ptr(mask), _ptr(out), nodes, E)
     if rc:
         raise RuntimeError(f"oracle_message_lwr failed with code {rc}")
+    return out
+
+
+def onsite_nbody(X, W_in, W_out, lmax, lmax_out) -> np.ndarray:
+    """nu-body pointwise product: X [nu, batch, N, (lmax+1)^2], W_in [nu, C, N], W_out [N, C]
+    -> out[batch, N, (lmax_out+1)^2] in float64."""
+    X, W_in, W_out = map(_f64, (X, W_in, W_out))
+    nu, batch, N, L2 = X.shape
+    C = W_in.shape[1]
+    assert L2 == (lmax + 1) ** 2 and W_in.shape == (nu, C, N) and W_out.shape == (N, C)
+    out = np.zeros((batch, N, (lmax_out + 1) ** 2), np.float64)
+    rc = _load().oracle_onsite_nbody(_ptr(X), _ptr(W_in), _ptr(W_out), nu, lmax, lmax_out, N, C, _ptr(out), batch)
+    if rc:
+        raise RuntimeError(f"oracle_onsite_nbody failed with code {rc}")
     return out
 
 

@@ -54,6 +54,29 @@ def make_onsite(lmax: int, lmax_out: int, N: int, C: int, batch: int, seed: int 
 
 
 @dataclass
+class NbodyInputs:
+    nu: int
+    lmax: int
+    lmax_out: int
+    N: int
+    C: int
+    batch: int
+    X: np.ndarray      # [nu, batch, N, (lmax+1)^2]
+    W_in: np.ndarray   # [nu, C, N]
+    W_out: np.ndarray  # [N, C]
+
+
+def make_nbody(nu: int, lmax: int, lmax_out: int, N: int, C: int, batch: int, seed: int = 0) -> NbodyInputs:
+    """nu feature sets ~ N(0,1) per real-SH coefficient; W_in[s][C,N] ~ N(0,1/sqrt(N)); W_out[N,C] ~ N(0,1/sqrt(C))."""
+    L2 = (lmax + 1) ** 2
+    rX, rW, rWo = _streams(seed, 3)
+    X = rX.standard_normal((nu, batch, N, L2), dtype=np.float32)
+    W_in = (rW.standard_normal((nu, C, N), dtype=np.float32) / np.float32(np.sqrt(N))).astype(np.float32)
+    W_out = (rWo.standard_normal((N, C), dtype=np.float32) / np.float32(np.sqrt(C))).astype(np.float32)
+    return NbodyInputs(nu, lmax, lmax_out, N, C, batch, X, W_in, W_out)
+
+
+@dataclass
 class MessageInputs:
     lmax: int
     lmax_out: int
