@@ -85,6 +85,35 @@ int cgtp_onsite(const float* A, const float* B, const float* W_a, const float* W
                 int64_t batch, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * nu-body on-site product (end of Sec. VI): "The grid pointwise product
+ * extends to nu-body features through additional pointwise multiplications on the grid followed by a single
+ * inverse transform", on the grid U = ceil((nu lmax + lmax_out + 1)/2), V = nu lmax + lmax_out + 1 that the
+ * degree-(nu lmax + lmax_out) integrand needs ("tighten this requirement linearly in the body order nu"):
+ *
+ *   H(s)[b,c,:] = W_in[s][c,:] . X[s][b]                     s = 1..nu                  (Eq.(35) per factor)
+ *   T[b,c,lm]   = int prod_s H(s)~[b,c](Omega) Y_lm dOmega   l <= lmax_out              (Eq.(36)-(40))
+ *   out[b,n,lm] = sum_c W_out[n,c] T[b,c,lm]                                            (Eq.(41))
+ *
+ * Pointwise (parity-even) rank channels only -- the curl pairing is bilinear and the paper gives no nu-body
+ * form of it -- so there is one output sector (natural parity).  nu = 2 equals sector 0 of cgtp_onsite with an
+ * all-even mask.
+ *
+ * X      device [nu, batch, N, (lmax+1)^2]     W_in  device [nu, C, N]     W_out  device [N, C]
+ * out    device [batch, N, (lmax_out+1)^2]
+ * workspace device, >= cgtp_onsite_nbody_workspace_bytes(...) bytes, 256-byte aligned (scratch)
+ * 1 <= nu <= 4, max(lmax, lmax_out) <= 8 (CGTP_ERR_UNSUPPORTED beyond), 0 <= lmax_out <= nu*lmax
+ * (CGTP_ERR_INVALID otherwise).  batch may be 0.  Asynchronous on cuda_stream, bitwise reproducible.
+ * ------------------------------------------------------------------------------------------- */
+size_t cgtp_onsite_nbody_workspace_bytes(int nu, int lmax, int lmax_out, int N, int C, int64_t batch);
+
+int cgtp_onsite_nbody(const float* X, const float* W_in, const float* W_out, int nu, int lmax, int lmax_out,
+                      int N, int C, float* out, int64_t batch, void* workspace, size_t workspace_bytes,
+                      void* cuda_stream);
+
+/* Grid of the nu-body product (cgtp_grid_shape is the case nu = 2). */
+int cgtp_grid_shape_nu(int lmax, int lmax_out, int nu, int* U, int* V);
+
+/* ---------------------------------------------------------------------------------------------
  * Parity-aware message passing, Eq.(2), pipeline of Sec. VII C, Eq.(46)-(59)
  * (:396-:453), natural-parity node features (Cases A and B, :197-:217), l1-shared radial factor:
  *

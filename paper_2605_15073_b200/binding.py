@@ -62,6 +62,12 @@ def lib() -> ctypes.CDLL:
     L.cgtp_message_parity_workspace_bytes.argtypes = [i, i, i, i, i64, i64]
     L.cgtp_message_parity.restype = i
     L.cgtp_message_parity.argtypes = [vp, vp, vp, vp, vp, vp, i, i, i, i, vp, i64, i64, vp, sz, vp]
+    L.cgtp_onsite_nbody_workspace_bytes.restype = sz
+    L.cgtp_onsite_nbody_workspace_bytes.argtypes = [i, i, i, i, i, i64]
+    L.cgtp_onsite_nbody.restype = i
+    L.cgtp_onsite_nbody.argtypes = [vp, vp, vp, i, i, i, i, i, vp, i64, vp, sz, vp]
+    L.cgtp_grid_shape_nu.restype = i
+    L.cgtp_grid_shape_nu.argtypes = [i, i, i, ctypes.POINTER(i), ctypes.POINTER(i)]
     L.cgtp_onsite_lw.restype = i
     L.cgtp_onsite_lw.argtypes = L.cgtp_onsite.argtypes
     L.cgtp_message_lwr.restype = i
@@ -173,6 +179,41 @@ def cgtp_onsite(A, B, W_a, W_b, W_out, lmax, lmax_out, N, C, parity_mask, out=No
         rc = lib().cgtp_onsite(A.data_ptr(), B.data_ptr(), W_a.data_ptr(), W_b.data_ptr(), W_out.data_ptr(),
                                lmax, lmax_out, N, C, mask.ctypes.data, out.data_ptr(), batch,
                                ws.data_ptr(), ws.numel(), _stream_ptr(stream))
+    _check(rc)
+    return out
+
+
+def cgtp_grid_shape_nu(lmax: int, lmax_out: int, nu: int):
+    U, V = ctypes.c_int(0), ctypes.c_int(0)
+    _check(lib().cgtp_grid_shape_nu(lmax, lmax_out, nu, ctypes.byref(U), ctypes.byref(V)))
+    return U.value, V.value
+
+
+def cgtp_onsite_nbody_workspace_bytes(nu, lmax, lmax_out, N, C, batch) -> int:
+    return lib().cgtp_onsite_nbody_workspace_bytes(nu, lmax, lmax_out, N, C, batch)
+
+
+def cgtp_onsite_nbody(X, W_in, W_out, nu, lmax, lmax_out, N, C, out=None, workspace=None, stream=None):
+    """out[batch, N, (lmax_out+1)^2] = nu-body pointwise product of X[nu, batch, N, (lmax+1)^2] (see include/cgtp.h)."""
+    f32 = torch.float32
+    X, W_in, W_out = _dev(X, f32, "X"), _dev(W_in, f32, "W_in"), _dev(W_out, f32, "W_out")
+    L2, Lo2 = (lmax + 1) ** 2, (lmax_out + 1) ** 2
+    if X.dim() != 4 or X.shape[0] != nu or X.shape[2] != N or X.shape[3] != L2:
+        raise ValueError("X must be [nu, batch, N, (lmax+1)^2]")
+    batch = X.shape[1]
+    if tuple(W_in.shape) != (nu, C, N) or tuple(W_out.shape) != (N, C):
+        raise ValueError("W_in must be [nu, C, N] and W_out [N, C]")
+    if out is None:
+        out = torch.empty((batch, N, Lo2), dtype=f32, device=X.device)
+    else:
+        _dev(out, f32, "out")
+        if tuple(out.shape) != (batch, N, Lo2):
+            raise ValueError("out must be [batch, N, (lmax_out+1)^2]")
+    nbytes = cgtp_onsite_nbody_workspace_bytes(nu, lmax, lmax_out, N, C, batch)
+    ws = _workspace(X.device, nbytes) if workspace is None else workspace
+    with torch.cuda.device(X.device):
+        rc = lib().cgtp_onsite_nbody(X.data_ptr(), W_in.data_ptr(), W_out.data_ptr(), nu, lmax, lmax_out, N, C,
+                                     out.data_ptr(), batch, ws.data_ptr(), ws.numel(), _stream_ptr(stream))
     _check(rc)
     return out
 

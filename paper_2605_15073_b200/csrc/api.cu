@@ -80,7 +80,8 @@ static int launch_proj_degrees(const std::vector<ProjArgs>& v, int group, Kind k
         if (rc != CGTP_OK || handled) return rc;
     }
     for (size_t i = 0; i < v.size(); i += group) {
-        const int rc = launch_proj(&v[i], group, kind, st);
+        const int n = (int)(v.size() - i) < group ? (int)(v.size() - i) : group;
+        const int rc = launch_proj(&v[i], n, kind, st);
         if (rc) return rc;
     }
     return CGTP_OK;
@@ -397,6 +398,17 @@ int cgtp_grid_shape(int lmax, int lmax_out, int* U, int* V)
     return CGTP_OK;
 }
 
+int cgtp_grid_shape_nu(int lmax, int lmax_out, int nu, int* U, int* V)
+{
+    if (nu < 1 || lmax < 0 || lmax_out < 0 || (int64_t)lmax_out > (int64_t)nu * lmax) {
+        set_error("invalid band limits / body order");
+        return CGTP_ERR_INVALID;
+    }
+    if (U) *U = (nu * lmax + lmax_out + 2) / 2;
+    if (V) *V = nu * lmax + lmax_out + 1;
+    return CGTP_OK;
+}
+
 size_t cgtp_onsite_workspace_bytes(int lmax, int lmax_out, int N, int C, int64_t batch)
 {
     (void)N;
@@ -592,6 +604,114 @@ int cgtp_message_status(const void* workspace, void* cuda_stream)
         return CGTP_ERR_GRAPH;
     }
     return CGTP_OK;
+}
+
+// ------------------------------------------------------------------------------ nu-body on-site product
+static size_t nbody_ws_bytes(int nu, int lmax, int lmax_out, int C, int64_t batch)
+{
+    const size_t L2p = round_up((lmax + 1) * (lmax + 1), 4), Lo2p = round_up((lmax_out + 1) * (lmax_out + 1), 4);
+    return (size_t)batch * C * ((size_t)nu * L2p + Lo2p) * sizeof(float) + 4 * 256;
+}
+
+size_t cgtp_onsite_nbody_workspace_bytes(int nu, int lmax, int lmax_out, int N, int C, int64_t batch)
+{
+    (void)N;
+    if (nu < 1 || lmax < 0 || lmax_out < 0 || C <= 0 || batch < 0) return 0;
+    return nbody_ws_bytes(nu, lmax, lmax_out, C, batch);
+}
+
+int cgtp_onsite_nbody(const float* X, const float* W_in, const float* W_out, int nu, int lmax, int lmax_out, int N,
+                      int C, float* out, int64_t batch, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    clear_error();
+    if (nu < 1) { set_error("body order nu=%d must be >= 1", nu); return CGTP_ERR_INVALID; }
+    if (lmax < 0 || lmax_out < 0 || (int64_t)lmax_out > (int64_t)nu * lmax) {
+        set_error("invalid band limits lmax=%d lmax_out=%d (need 0 <= lmax_out <= nu*lmax)", lmax, lmax_out);
+        return CGTP_ERR_INVALID;
+    }
+    if (N <= 0 || C <= 0) { set_error("N and C must be positive (N=%d, C=%d)", N, C); return CGTP_ERR_INVALID; }
+    const int LB = kernel_band(lmax > lmax_out ? lmax : lmax_out);
+    if (!nbody_supported(LB, nu)) {
+        set_error("nu-body product: max(lmax,lmax_out)=%d / nu=%d exceed the compiled limits (band limit 8, nu 4)",
+                  lmax > lmax_out ? lmax : lmax_out, nu);
+        return CGTP_ERR_UNSUPPORTED;
+    }
+    if (batch < 0) { set_error("negative batch"); return CGTP_ERR_INVALID; }
+    if (batch == 0) return CGTP_OK;
+    if (!X || !W_in || !W_out || !out || !workspace) { set_error("null pointer argument"); return CGTP_ERR_INVALID; }
+    if (!aligned16(X) || !aligned16(out) || !aligned16(W_in) || !aligned16(W_out) ||
+        (reinterpret_cast<uintptr_t>(workspace) & 255u)) {
+        set_error("misaligned pointer (tensors need 16-byte, workspace 256-byte alignment)");
+        return CGTP_ERR_INVALID;
+    }
+    if (workspace_bytes < nbody_ws_bytes(nu, lmax, lmax_out, C, batch)) {
+        set_error("workspace too small: %zu < %zu bytes", workspace_bytes, nbody_ws_bytes(nu, lmax, lmax_out, C, batch));
+        return CGTP_ERR_INVALID;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const Plan* p = get_plan_nu(lmax, lmax_out, nu);
+    if (!p) return CGTP_ERR_CUDA;
+    const int64_t ncols = batch * C;
+    Carver cv(workspace);
+    float* H = cv.take<float>((size_t)nu * ncols * p->L2p);
+    float* T = cv.take<float>((size_t)ncols * p->Lo2p);
+
+    // S1 per factor: H[s] = W_in[s] . X[s] (Eq.(35)), one launch over the nu problems
+    std::vector<ProjArgs> pv(nu);
+    for (int s = 0; s < nu; ++s) {
+        ProjArgs& a = pv[s];
+        a.X = X + (size_t)s * batch * N * p->L2;
+        a.x_bs = (int64_t)N * p->L2;
+        a.x_rs = p->L2;
+        a.W = W_in + (size_t)s * C * N;
+        a.ldw_m = N;
+        a.ldw_k = 1;
+        a.idx_m = nullptr;
+        a.idx_k = nullptr;
+        a.M = C;
+        a.K = N;
+        a.J = p->L2;
+        a.out0 = H + (size_t)s * ncols * p->L2p;
+        a.o_bs0 = (int64_t)C * p->L2p;
+        a.out1 = a.out0;
+        a.o_bs1 = a.o_bs0;
+        a.m_split = C;
+        a.o_rs = p->L2p;
+        a.batch = batch;
+        a.accumulate = 0;
+        a.j0 = 0;
+    }
+    int rc = launch_proj_degrees(pv, 2, K_PROJ_IN, st);
+    if (rc) return rc;
+    // S2-S4 with nu factors
+    rc = launch_nbody(p, H, T, ncols, st);
+    if (rc) return rc;
+    // S5: out[b] = W_out . T[b] (Eq.(41) :346)
+    std::vector<ProjArgs> po(1);
+    {
+        ProjArgs& a = po[0];
+        a.X = T;
+        a.x_bs = (int64_t)C * p->Lo2p;
+        a.x_rs = p->Lo2p;
+        a.W = W_out;
+        a.ldw_m = C;
+        a.ldw_k = 1;
+        a.idx_m = nullptr;
+        a.idx_k = nullptr;
+        a.M = N;
+        a.K = C;
+        a.J = p->Lo2;
+        a.out0 = out;
+        a.o_bs0 = (int64_t)N * p->Lo2;
+        a.out1 = a.out0;
+        a.o_bs1 = a.o_bs0;
+        a.m_split = N;
+        a.o_rs = p->Lo2;
+        a.batch = batch;
+        a.accumulate = 0;
+        a.j0 = 0;
+    }
+    return launch_proj_degrees(po, 1, K_PROJ_OUT, st);
 }
 
 // ------------------------------------------------------------------------------ parity-slot entry points

@@ -38,6 +38,7 @@ __host__ __device__ constexpr int tri_index(int l, int m) { return l * (l + 1) /
 // ---------------------------------------------------------------------------------------------
 struct Plan {
     int lmax, lmax_out;
+    int nu;    // body order the grid is exact for (2 everywhere except the nu-body entry point)
     int LB;    // kernel band limit = kernel_band(max(lmax, lmax_out)); tables cover 0 <= m <= l <= LB
     int U, V;  // grid
     int Uh, Vh;
@@ -67,6 +68,9 @@ void legendre_values(int U, int LB, const std::vector<double>& x, std::vector<do
 // Returns the cached plan, creating it on first use (cudaMalloc + blocking copies, once).
 // nullptr + cgtp_last_error on failure.
 const Plan* get_plan(int lmax, int lmax_out);
+// Same with the grid of a nu-body product: U = ceil((nu lmax + lmax_out + 1)/2), V = nu lmax + lmax_out + 1
+// ("Higher-body-order products tighten this requirement linearly in the body order nu").
+const Plan* get_plan_nu(int lmax, int lmax_out, int nu);
 
 // ---------------------------------------------------------------------------------------------
 // Channel plan: parity_mask -> permutation that lists the even channels first (stable).
@@ -187,6 +191,11 @@ inline int onsite_fast_hstride(const Plan* p) { return p->L2 | 1; }
 inline int onsite_fast_tstride(const Plan* p) { return p->Lo2 | 1; }
 int launch_onsite_fast(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols,
                        cudaStream_t st);
+
+// nu-body form of S2-S4 (nbody.cu): T[col][Lo2p] = analysis of prod_s synthesis(H[s][col]); H is [nu][ncols][L2p],
+// p a plan of get_plan_nu.  CGTP_ERR_UNSUPPORTED above band limit 8 or body order 4.
+bool nbody_supported(int LB, int nu);
+int launch_nbody(const Plan* p, const float* H, float* T, int64_t ncols, cudaStream_t st);
 
 // M0: row_ptr over `nodes` receivers; senders are validated against n_send
 int launch_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int64_t n_send, int64_t* row_ptr,

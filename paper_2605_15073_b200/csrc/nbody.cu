@@ -1,0 +1,201 @@
+// nbody.cu -- nu-body on-site core (end of Sec. VI): "The grid pointwise
+// product extends to nu-body features through additional pointwise multiplications on the grid followed by a single
+// inverse transform ... Higher-body-order products tighten this requirement linearly in the body order nu."
+//
+// Rows S2a, S2b, S3, S4a, S4b with nu factors instead of two, for NC (atom, rank-channel) columns per CTA:
+// Legendre synthesis of every factor (Eq.(36) :325) -> per (column, grid row u): forward real DFT of the nu coefficient
+// vectors (Eq.(37) :327), product of the nu grid values (Eq.(38) :332 with nu - 1 multiplications), inverse real DFT
+// (Eq.(39) :339), all in registers -> Gauss-Legendre analysis (Eq.(40) :342).  The grid is the plan's
+// U = ceil((nu lmax + lmax_out + 1)/2) x V = nu lmax + lmax_out + 1, on which the quadrature of the degree
+// nu lmax + lmax_out integrand is exact.  Grid fields exist only in registers, the per-row azimuthal coefficients only
+// in shared memory.  Pointwise (even) channels only: the curl pairing is bilinear (R19).
+#include "sht.cuh"
+
+namespace cgtp {
+
+constexpr int kNbodyMaxBand = 8;
+constexpr int kNbodyMaxNu = 4;
+
+bool nbody_supported(int LB, int nu) { return LB >= 1 && LB <= kNbodyMaxBand && nu >= 1 && nu <= kNbodyMaxNu; }
+
+struct NbodySmem {
+    // byte offsets into dynamic shared memory (all multiples of 16)
+    int bar, tab, wp, qc, qs, wv, hs, f, total;
+    int tab_bytes, q_bytes, wv_bytes;
+};
+
+static NbodySmem nbody_smem_layout(const Plan* p, int NC)
+{
+    NbodySmem s;
+    const int M = 2 * p->LB + 1;
+    const int J = (NC * p->U) | 1;  // odd row stride: rows of different m fall into different banks
+    s.tab_bytes = p->Uh * p->NTRI * 4;
+    s.q_bytes = p->Vh * p->QSTR * 4;
+    s.wv_bytes = round_up(p->Vh, 4) * 4;
+    int off = 0;
+    s.bar = off; off += 16;
+    s.tab = off; off += s.tab_bytes;
+    s.wp = off; off += s.tab_bytes;
+    s.qc = off; off += s.q_bytes;
+    s.qs = off; off += s.q_bytes;
+    s.wv = off; off += s.wv_bytes;
+    s.hs = off; off += p->nu * NC * p->L2p * 4;
+    s.f = off; off += round_up(p->nu * M * J, 4) * 4;
+    s.total = off;
+    return s;
+}
+
+// Rows S2b + S3 + S4a for one (column, u): forward real DFT of the NU coefficient vectors, product of the NU grid
+// values at the azimuth pair (v', V - v'), inverse real DFT.  F: NU fields [M][J] at distance FS; the result T[m]
+// overwrites field 0 at [.][j].
+template <int LB, int NU>
+__device__ __forceinline__ void dft_nproduct_idft(float* F, int FS, int J, int j, const float* __restrict__ QC,
+                                                  const float* __restrict__ QS, const float* __restrict__ WV, int Vh)
+{
+    constexpr int M = 2 * LB + 1;
+    constexpr int QSTR = round_up(LB + 1, 4);
+    float f[NU][M], t[M];
+#pragma unroll
+    for (int s = 0; s < NU; ++s)
+#pragma unroll
+        for (int r = 0; r < M; ++r) f[s][r] = F[(size_t)s * FS + r * J + j];
+#pragma unroll
+    for (int r = 0; r < M; ++r) t[r] = 0.f;
+    for (int vp = 0; vp < Vh; ++vp) {
+        float qc[QSTR], qs[QSTR];
+        load_q_row<LB>(QC, vp, qc);
+        load_q_row<LB>(QS, vp, qs);
+        float s1 = 1.f, s2 = 1.f;
+#pragma unroll
+        for (int s = 0; s < NU; ++s) {
+            float ce = 0.f, so = 0.f;
+#pragma unroll
+            for (int m = 0; m <= LB; ++m) ce = fmaf(qc[m], f[s][m], ce);
+#pragma unroll
+            for (int m = 1; m <= LB; ++m) so = fmaf(qs[m], f[s][LB + m], so);
+            s1 *= ce + so;  // grid point v'
+            s2 *= ce - so;  // mirrored grid point V - v'
+        }
+        const float w = WV[vp];
+        const float sp = w * (s1 + s2), sm = w * (s1 - s2);
+#pragma unroll
+        for (int m = 0; m <= LB; ++m) t[m] = fmaf(qc[m], sp, t[m]);
+#pragma unroll
+        for (int m = 1; m <= LB; ++m) t[LB + m] = fmaf(qs[m], sm, t[LB + m]);
+    }
+#pragma unroll
+    for (int r = 0; r < M; ++r) F[r * J + j] = t[r];
+}
+
+template <int LB, int NU>
+__global__ void __launch_bounds__(256) nbody_core_kernel(Plan p, NbodySmem lay, const float* __restrict__ H,
+                                                         float* __restrict__ T, long long ncols, int NC)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    constexpr int M = 2 * LB + 1;
+    constexpr int UHMAX = (((NU + 1) * LB + 2) / 2 + 1) / 2;  // Uh for lmax = lmax_out = LB
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem + lay.bar);
+    float* tab = reinterpret_cast<float*>(smem + lay.tab);
+    float* wp = reinterpret_cast<float*>(smem + lay.wp);
+    float* qc = reinterpret_cast<float*>(smem + lay.qc);
+    float* qs = reinterpret_cast<float*>(smem + lay.qs);
+    float* wv = reinterpret_cast<float*>(smem + lay.wv);
+    float* hs = reinterpret_cast<float*>(smem + lay.hs);
+    float* F = reinterpret_cast<float*>(smem + lay.f);
+
+    const long long col0 = (long long)blockIdx.x * NC;
+    const int nc = (int)((ncols - col0 < NC) ? (ncols - col0) : NC);
+    const int J = (NC * p.U) | 1;
+    const int FS = M * J;
+    const int hbytes = nc * p.L2p * 4;
+
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const uint32_t total = 2 * lay.tab_bytes + 2 * lay.q_bytes + lay.wv_bytes + NU * hbytes;
+        mbar_arrive_expect_tx(bar, total);
+        tma_load_span(tab, p.PT, lay.tab_bytes, bar);
+        tma_load_span(wp, p.WP, lay.tab_bytes, bar);
+        tma_load_span(qc, p.QC, lay.q_bytes, bar);
+        tma_load_span(qs, p.QS, lay.q_bytes, bar);
+        tma_load_span(wv, p.WV, lay.wv_bytes, bar);
+#pragma unroll
+        for (int s = 0; s < NU; ++s)
+            tma_load_span(hs + (size_t)s * NC * p.L2p, H + ((size_t)s * ncols + col0) * p.L2p, hbytes, bar);
+    }
+#pragma unroll
+    for (int s = 0; s < NU; ++s) zero_high_rows<LB>(F + (size_t)s * FS, p.lmax, J);
+    mbar_wait(bar, 0);
+
+    // ---- S2a: Legendre synthesis of the NU factors
+    {
+        LegDst dst[NU][2];
+#pragma unroll
+        for (int s = 0; s < NU; ++s) {
+            dst[s][0] = LegDst{F + (size_t)s * FS, 1.f};
+            dst[s][1] = LegDst{nullptr, 0.f};
+        }
+        legendre_synthesis<LB, false, NU, 2>(tab, nullptr, hs, NC * p.L2p, p.L2p, dst, nc, p.lmax, p.U, p.Uh, p.NTRI, J);
+    }
+    __syncthreads();
+
+    // ---- S2b + S3 + S4a: one (column, u) per thread
+    const int rows = nc * p.U;
+    for (int j = threadIdx.x; j < rows; j += blockDim.x) dft_nproduct_idft<LB, NU>(F, FS, J, j, qc, qs, wv, p.Vh);
+    __syncthreads();
+
+    // ---- S4b: Gauss-Legendre analysis
+    legendre_analysis<LB, UHMAX>(F, nullptr, wp, T + col0 * p.Lo2p, p.Lo2p, nc, p.lmax_out, p.U, p.Uh, p.NTRI, J);
+}
+
+template <int LB, int NU>
+static int launch_nbody_t(const Plan* p, const float* H, float* T, int64_t ncols, cudaStream_t st)
+{
+    const int M = 2 * p->LB + 1;
+    // columns per CTA: fill ~100 KB of shared memory (two CTAs per SM), at least 1 column
+    NbodySmem fixed = nbody_smem_layout(p, 0);
+    const int percol = NU * p->L2p * 4 + NU * M * p->U * 4;
+    int NC = (100 * 1024 - fixed.total - 64) / percol;
+    if (NC < 4) NC = (220 * 1024 - fixed.total - 64) / percol;
+    if (NC < 1) { set_error("nbody core: shared memory too small for lmax=%d nu=%d", p->lmax, NU); return CGTP_ERR_UNSUPPORTED; }
+    if (NC > 128) NC = 128;
+    // at least ~2 CTAs per SM when the problem is small
+    while (NC > 8 && (ncols + NC - 1) / NC < 296) NC /= 2;
+    if ((int64_t)NC > ncols) NC = (int)ncols;
+    NbodySmem lay = nbody_smem_layout(p, NC);
+    auto kern = nbody_core_kernel<LB, NU>;
+    CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, lay.total));
+    int64_t grid = (ncols + NC - 1) / NC;
+    LaunchScope scope(K_ONSITE_EVEN, st);
+    kern<<<(unsigned)grid, 256, lay.total, st>>>(*p, lay, H, T, (long long)ncols, NC);
+    CGTP_CUDA_CHECK(cudaGetLastError());
+    return CGTP_OK;
+}
+
+#define CGTP_FOR_EACH_NBODY_BAND(X) X(1) X(2) X(3) X(4) X(5) X(6) X(8)
+
+int launch_nbody(const Plan* p, const float* H, float* T, int64_t ncols, cudaStream_t st)
+{
+    if (ncols <= 0) return CGTP_OK;
+    if (!nbody_supported(p->LB, p->nu)) {
+        set_error("nbody core: band limit %d / body order %d not supported (max %d / %d)", p->LB, p->nu, kNbodyMaxBand,
+                  kNbodyMaxNu);
+        return CGTP_ERR_UNSUPPORTED;
+    }
+    switch (p->LB * 8 + p->nu) {
+#define CGTP_CASE(B)                                                        \
+    case B * 8 + 1: return launch_nbody_t<B, 1>(p, H, T, ncols, st);        \
+    case B * 8 + 2: return launch_nbody_t<B, 2>(p, H, T, ncols, st);        \
+    case B * 8 + 3: return launch_nbody_t<B, 3>(p, H, T, ncols, st);        \
+    case B * 8 + 4: return launch_nbody_t<B, 4>(p, H, T, ncols, st);
+        CGTP_FOR_EACH_NBODY_BAND(CGTP_CASE)
+#undef CGTP_CASE
+    }
+    set_error("nbody core: no kernel for band limit %d, body order %d", p->LB, p->nu);
+    return CGTP_ERR_UNSUPPORTED;
+}
+
+}  // namespace cgtp

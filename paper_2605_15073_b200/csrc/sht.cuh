@@ -346,12 +346,12 @@ __device__ __forceinline__ void dft_inverse_row(const float* srow, float* T, int
 // Rows S4b / M5 second half (Eq.(40), Eq.(54) :422): Gauss-Legendre quadrature.
 // T0 (+ T1 if not null): [M][J] shared, the azimuthal coefficients per grid row; WP: [Uh][NTRI] table
 // (weights folded in, equator halved); out: global [NC][Lo2p].
-template <int LB>
+// UHMAX: upper bound of Uh; the default is Uh for lmax = lmax_out = LB on the bilinear grid, the largest possible there.
+template <int LB, int UHMAX = ((3 * LB + 2) / 2 + 1) / 2>
 __device__ __forceinline__ void legendre_analysis(const float* T0, const float* T1, const float* __restrict__ WP,
                                                   float* __restrict__ out, int Lo2p, int NC, int lmax_out, int U,
                                                   int Uh, int NTRI, int J)
 {
-    constexpr int UHMAX = ((3 * LB + 2) / 2 + 1) / 2;  // Uh for lmax = lmax_out = LB is the largest possible
     const int items = NC * (lmax_out + 1);
     for (int item = threadIdx.x; item < items; item += blockDim.x) {
         const int col = item / (lmax_out + 1);

@@ -166,19 +166,23 @@ static const float* upload(const std::vector<float>& h, bool* ok)
     return d;
 }
 
-const Plan* get_plan(int lmax, int lmax_out)
+const Plan* get_plan(int lmax, int lmax_out) { return get_plan_nu(lmax, lmax_out, 2); }
+
+const Plan* get_plan_nu(int lmax, int lmax_out, int nu)
 {
     std::lock_guard<std::mutex> lk(g_plan_mu);
     for (Plan* p : g_plans)
-        if (p->lmax == lmax && p->lmax_out == lmax_out) return p;
+        if (p->lmax == lmax && p->lmax_out == lmax_out && p->nu == nu) return p;
 
     Plan* p = new Plan;
     std::memset(p, 0, sizeof *p);
     p->lmax = lmax;
     p->lmax_out = lmax_out;
+    p->nu = nu;
     const int LB = p->LB = kernel_band(lmax > lmax_out ? lmax : lmax_out);
-    const int U = p->U = (2 * lmax + lmax_out + 2) / 2;  // ceil((2 lmax + lmax_out + 1)/2)
-    const int V = p->V = 2 * lmax + lmax_out + 1;
+    // a product of nu fields of band lmax against Y_lm, l <= lmax_out, is a polynomial of degree nu lmax + lmax_out
+    const int U = p->U = (nu * lmax + lmax_out + 2) / 2;  // ceil((nu lmax + lmax_out + 1)/2)
+    const int V = p->V = nu * lmax + lmax_out + 1;
     const int Uh = p->Uh = (U + 1) / 2;
     const int Vh = p->Vh = V / 2 + 1;
     p->UV = U * V;
