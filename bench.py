@@ -11,7 +11,8 @@ product / surface-curl pairing, analysis, output projection) over one batch of B
 
 Prints ONE JSON line on rank 0.  Extra objects on the line (N=1 only): "sweep" (configs[3], on-site vs
 lmax), "message" (configs[2] and configs[4], edges/s and HBM GB/s), "kernels" (per-kernel shares), "parity"
-(parity-labelled inputs: cost of the full dispatch against one Category-alpha run), "l_dependent_weights".
+(parity-labelled inputs: cost of the full dispatch against one Category-alpha run), "l_dependent_weights", "nbody"
+(nu-body pointwise products).
 """
 from __future__ import annotations
 
@@ -353,6 +354,7 @@ def main():
         line["message"] = run_message(args, cg, synthetic, dev, peaks, peak_src)
         line["parity"] = run_parity(args, cg, synthetic, dev)
         line["l_dependent_weights"] = run_lw(args, cg, synthetic, dev, ms_per_step)
+        line["nbody"] = run_nbody(args, cg, synthetic, dev, fp32_peak_tflops)
     elif world == 1:
         rate, dt_cpu, cores = oracle_onsite_rate(base, 1024)
         line["cpu_baseline"] = {"value": rate, "unit": "contractions/s", "cores": cores, "kind": "oracle",
@@ -585,6 +587,51 @@ def run_lw(args, cg, synthetic, dev, shared_ms):
             "factor_vs_l_shared": ms / shared_ms,
             "kernel_ms": {k: v[0] / 10 for k, v in prof.items()},
             "launches_per_step": int(sum(v[1] for v in prof.values()) // 10)}
+
+
+def run_nbody(args, cg, synthetic, dev, fp32_peak_tflops):
+    """nu-body pointwise products at the shape of configs[1] (all 64 rank channels
+    pointwise) and at an ACE-like small band limit.  Algorithmic flops per atom, dense transforms on the minimal grid
+    U x V = ceil((nu lmax + lmax_out + 1)/2) x (nu lmax + lmax_out + 1):
+    2 nu C N L^2 (S1) + C [2 nu U L^2 + 2 nu U V M + (nu - 1) U V + 2 U V M_o + 2 U L_o^2] + 2 N C L_o^2 (S5)."""
+    import torch
+    res = []
+    for (nu, lmax, N, C, batch) in [(2, 6, 64, 64, 4096), (3, 6, 64, 64, 4096), (4, 6, 64, 64, 4096),
+                                    (3, 3, 32, 32, 16384), (4, 3, 32, 32, 16384)]:
+        inp = synthetic.make_nbody(nu, lmax, lmax, N, C, batch, seed=0)
+        # rotating input sets so that no step finds its inputs in L2
+        nsets = max(2, int(300e6 // inp.X.nbytes) + 1)
+        Xs = [torch.from_numpy(inp.X).to(dev) for _ in range(nsets)]
+        W_in, W_out = torch.from_numpy(inp.W_in).to(dev), torch.from_numpy(inp.W_out).to(dev)
+        out = torch.empty((batch, N, (lmax + 1) ** 2), device=dev)
+        it = [0]
+
+        def fn():
+            it[0] += 1
+            cg.cgtp_onsite_nbody(Xs[it[0] % nsets], W_in, W_out, nu, lmax, lmax, N, C, out=out)
+        ms = time_steps(fn, 20, 3)
+        cg.cgtp_profile_enable(True)
+        for _ in range(10):
+            fn()
+        torch.cuda.synchronize()
+        prof = cg.cgtp_profile_collect()
+        cg.cgtp_profile_enable(False)
+        L2 = (lmax + 1) ** 2
+        U, V = (nu * lmax + lmax + 2) // 2, nu * lmax + lmax + 1
+        M = 2 * lmax + 1
+        core = C * (2 * nu * U * L2 + 2 * nu * U * V * M + (nu - 1) * U * V + 2 * U * V * M + 2 * U * L2)
+        flops = 2 * nu * C * N * L2 + core + 2 * N * C * L2
+        kms = {k: v[0] / 10 for k, v in prof.items() if v[1]}
+        core_ms = kms.get("onsite_core_even", float("nan"))
+        res.append({"workload": f"nu={nu} lmax=lmax_out={lmax} N=C={N} batch={batch}, grid {U}x{V}, {nsets} rotating input sets",
+                    "ms_per_step": ms, "products_per_s": batch / (ms * 1e-3), "alg_tflops": flops * batch / (ms * 1e-3) / 1e12,
+                    "frac_fp32_peak": flops * batch / (ms * 1e-3) / 1e12 / fp32_peak_tflops,
+                    "core_alg_tflops": core * batch / (core_ms * 1e-3) / 1e12,
+                    "core_frac_fp32_peak": core * batch / (core_ms * 1e-3) / 1e12 / fp32_peak_tflops,
+                    "kernel_ms": kms})
+        del Xs, out
+        torch.cuda.empty_cache()
+    return res
 
 
 if __name__ == "__main__":

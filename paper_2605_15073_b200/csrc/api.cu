@@ -610,7 +610,8 @@ int cgtp_message_status(const void* workspace, void* cuda_stream)
 static size_t nbody_ws_bytes(int nu, int lmax, int lmax_out, int C, int64_t batch)
 {
     const size_t L2p = round_up((lmax + 1) * (lmax + 1), 4), Lo2p = round_up((lmax_out + 1) * (lmax_out + 1), 4);
-    return (size_t)batch * C * ((size_t)nu * L2p + Lo2p) * sizeof(float) + 4 * 256;
+    // H rows have the odd stride L2 | 1 <= L2p + 1; every factor block is padded to whole groups of 4 columns
+    return (((size_t)batch * C + 4) * (size_t)nu * (L2p + 1) + 4 * (L2p + 1) + (size_t)batch * C * Lo2p) * sizeof(float) + 4 * 256;
 }
 
 size_t cgtp_onsite_nbody_workspace_bytes(int nu, int lmax, int lmax_out, int N, int C, int64_t batch)
@@ -653,7 +654,9 @@ int cgtp_onsite_nbody(const float* X, const float* W_in, const float* W_out, int
     if (!p) return CGTP_ERR_CUDA;
     const int64_t ncols = batch * C;
     Carver cv(workspace);
-    float* H = cv.take<float>((size_t)nu * ncols * p->L2p);
+    const int hstr = nbody_hstride(p);
+    const int64_t hfs = nbody_hfstride(p, ncols);
+    float* H = cv.take<float>((size_t)nu * hfs + 4 * hstr);
     float* T = cv.take<float>((size_t)ncols * p->Lo2p);
 
     // S1 per factor: H[s] = W_in[s] . X[s] (Eq.(35)), one launch over the nu problems
@@ -671,12 +674,12 @@ int cgtp_onsite_nbody(const float* X, const float* W_in, const float* W_out, int
         a.M = C;
         a.K = N;
         a.J = p->L2;
-        a.out0 = H + (size_t)s * ncols * p->L2p;
-        a.o_bs0 = (int64_t)C * p->L2p;
+        a.out0 = H + (size_t)s * hfs;
+        a.o_bs0 = (int64_t)C * hstr;
         a.out1 = a.out0;
         a.o_bs1 = a.o_bs0;
         a.m_split = C;
-        a.o_rs = p->L2p;
+        a.o_rs = hstr;
         a.batch = batch;
         a.accumulate = 0;
         a.j0 = 0;

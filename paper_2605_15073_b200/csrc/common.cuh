@@ -192,9 +192,12 @@ inline int onsite_fast_tstride(const Plan* p) { return p->Lo2 | 1; }
 int launch_onsite_fast(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols,
                        cudaStream_t st);
 
-// nu-body form of S2-S4 (nbody.cu): T[col][Lo2p] = analysis of prod_s synthesis(H[s][col]); H is [nu][ncols][L2p],
-// p a plan of get_plan_nu.  CGTP_ERR_UNSUPPORTED above band limit 8 or body order 4.
+// nu-body form of S2-S4 (nbody.cu): T[col][Lo2p] = analysis of prod_s synthesis(H[s][col]); H holds nu blocks at
+// distance nbody_hfstride(p, ncols) floats, each [ncols][nbody_hstride(p)] (odd row stride), plus 4 rows of padding at
+// the end; p a plan of get_plan_nu.  CGTP_ERR_UNSUPPORTED above band limit 8 or body order 4.
 bool nbody_supported(int LB, int nu);
+int nbody_hstride(const Plan* p);
+int64_t nbody_hfstride(const Plan* p, int64_t ncols);
 int launch_nbody(const Plan* p, const float* H, float* T, int64_t ncols, cudaStream_t st);
 
 // M0: row_ptr over `nodes` receivers; senders are validated against n_send

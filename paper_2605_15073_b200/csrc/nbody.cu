@@ -16,6 +16,12 @@ namespace cgtp {
 constexpr int kNbodyMaxBand = 8;
 constexpr int kNbodyMaxNu = 4;
 
+// H rows have the odd stride L2 | 1 (written so by S1): with lane = column the coefficient loads of the synthesis are
+// then free of bank conflicts; a CTA's tile of every factor is one contiguous bulk copy of whole groups of 4 columns.
+int nbody_hstride(const Plan* p) { return p->L2 | 1; }
+// floats between the H blocks of consecutive factors (whole groups of 4 columns)
+int64_t nbody_hfstride(const Plan* p, int64_t ncols) { return (ncols + 3) / 4 * 4 * (int64_t)nbody_hstride(p); }
+
 bool nbody_supported(int LB, int nu) { return LB >= 1 && LB <= kNbodyMaxBand && nu >= 1 && nu <= kNbodyMaxNu; }
 
 struct NbodySmem {
@@ -39,10 +45,83 @@ static NbodySmem nbody_smem_layout(const Plan* p, int NC)
     s.qc = off; off += s.q_bytes;
     s.qs = off; off += s.q_bytes;
     s.wv = off; off += s.wv_bytes;
-    s.hs = off; off += p->nu * NC * p->L2p * 4;
+    s.hs = off; off += p->nu * round_up(NC, 4) * nbody_hstride(p) * 4;
     s.f = off; off += round_up(p->nu * M * J, 4) * 4;
     s.total = off;
     return s;
+}
+
+// Row S2a for the NU factors (Eq.(36)).  Work item = (|m|, block of UB northern nodes, column), the column
+// fastest: a warp shares |m| and the node block (the table loads are broadcasts, the loop trip counts agree), and items
+// of the same cost sit next to one another, so that the strided item -> thread map deals every thread the same mix of
+// cheap and expensive |m|.  Per degree: 2 NU coefficient loads and UB table loads feed 2 NU UB FMAs.  The sums are split
+// into the parts even / odd under x -> -x (P~_l^m(-x) = (-1)^(l+m) P~_l^m(x)), one table row serves the node pair
+// (u', U-1-u').  Table rows past Uh read by the last block are inside the shared-memory allocation; their sums are dropped.
+template <int LB, int NU, int UB>
+__device__ __forceinline__ void nbody_synthesis(const float* __restrict__ tab, const float* __restrict__ Hs,
+                                                int h_in_stride, int L2p, float* F, int FS, int NC, int lmax, int U,
+                                                int Uh, int J)
+{
+    constexpr int NTRI = round_up((LB + 1) * (LB + 2) / 2, 4);
+    const int nub = (Uh + UB - 1) / UB;
+    const int items = (lmax + 1) * nub * NC;
+    for (int item = threadIdx.x; item < items; item += blockDim.x) {
+        const int mm = item / (nub * NC);
+        const int rest = item - mm * (nub * NC);
+        const int ub = rest / NC;
+        const int col = rest - ub * NC;
+        const float* hcol = Hs + (size_t)col * L2p;
+        const float* trow = tab + (size_t)ub * UB * NTRI;
+        float acc[NU][2][2][UB];  // [factor][+m, -m][parity of l - m][node]
+#pragma unroll
+        for (int a = 0; a < NU; ++a)
+#pragma unroll
+            for (int c = 0; c < 2; ++c)
+#pragma unroll
+                for (int d = 0; d < 2; ++d)
+#pragma unroll
+                    for (int e = 0; e < UB; ++e) acc[a][c][d][e] = 0.f;
+        for (int l0 = mm; l0 <= lmax; l0 += 2) {
+#pragma unroll
+            for (int par = 0; par < 2; ++par) {
+                const int l = l0 + par;
+                if (l <= lmax) {
+                    const int t = tri_index(l, mm);
+                    const int c0 = l * l + l;
+                    float pv[UB];
+#pragma unroll
+                    for (int e = 0; e < UB; ++e) pv[e] = trow[e * NTRI + t];
+#pragma unroll
+                    for (int a = 0; a < NU; ++a) {
+                        const float hp = hcol[a * h_in_stride + c0 + mm];
+                        const float hn = hcol[a * h_in_stride + c0 - mm];
+#pragma unroll
+                        for (int e = 0; e < UB; ++e) {
+                            acc[a][0][par][e] = fmaf(pv[e], hp, acc[a][0][par][e]);
+                            acc[a][1][par][e] = fmaf(pv[e], hn, acc[a][1][par][e]);
+                        }
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int e = 0; e < UB; ++e) {
+            const int up = ub * UB + e;
+            if (up < Uh) {
+                const int jn = col * U + up, js = col * U + (U - 1 - up);
+#pragma unroll
+                for (int a = 0; a < NU; ++a) {
+                    float* Fa = F + (size_t)a * FS;
+                    Fa[mm * J + jn] = acc[a][0][0][e] + acc[a][0][1][e];
+                    Fa[mm * J + js] = acc[a][0][0][e] - acc[a][0][1][e];
+                    if (mm > 0) {
+                        Fa[(LB + mm) * J + jn] = acc[a][1][0][e] + acc[a][1][1][e];
+                        Fa[(LB + mm) * J + js] = acc[a][1][0][e] - acc[a][1][1][e];
+                    }
+                }
+            }
+        }
+    }
 }
 
 // Rows S2b + S3 + S4a for one (column, u): forward real DFT of the NU coefficient vectors, product of the NU grid
@@ -88,8 +167,8 @@ __device__ __forceinline__ void dft_nproduct_idft(float* F, int FS, int J, int j
 }
 
 template <int LB, int NU>
-__global__ void __launch_bounds__(256) nbody_core_kernel(Plan p, NbodySmem lay, const float* __restrict__ H,
-                                                         float* __restrict__ T, long long ncols, int NC)
+__global__ void __launch_bounds__(256, 2) nbody_core_kernel(Plan p, NbodySmem lay, const float* __restrict__ H,
+                                                            long long hfs, float* __restrict__ T, long long ncols, int NC)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int M = 2 * LB + 1;
@@ -107,7 +186,9 @@ __global__ void __launch_bounds__(256) nbody_core_kernel(Plan p, NbodySmem lay, 
     const int nc = (int)((ncols - col0 < NC) ? (ncols - col0) : NC);
     const int J = (NC * p.U) | 1;
     const int FS = M * J;
-    const int hbytes = nc * p.L2p * 4;
+    const int hstr = p.L2 | 1;
+    const int NC4 = round_up(NC, 4);
+    const int hbytes = round_up(nc, 4) * hstr * 4;  // whole groups of 4 columns (16-byte granularity); H is padded
 
     if (threadIdx.x == 0) {
         mbar_init(bar, 1);
@@ -124,22 +205,14 @@ __global__ void __launch_bounds__(256) nbody_core_kernel(Plan p, NbodySmem lay, 
         tma_load_span(wv, p.WV, lay.wv_bytes, bar);
 #pragma unroll
         for (int s = 0; s < NU; ++s)
-            tma_load_span(hs + (size_t)s * NC * p.L2p, H + ((size_t)s * ncols + col0) * p.L2p, hbytes, bar);
+            tma_load_span(hs + (size_t)s * NC4 * hstr, H + (size_t)s * hfs + (size_t)col0 * hstr, hbytes, bar);
     }
 #pragma unroll
     for (int s = 0; s < NU; ++s) zero_high_rows<LB>(F + (size_t)s * FS, p.lmax, J);
     mbar_wait(bar, 0);
 
     // ---- S2a: Legendre synthesis of the NU factors
-    {
-        LegDst dst[NU][2];
-#pragma unroll
-        for (int s = 0; s < NU; ++s) {
-            dst[s][0] = LegDst{F + (size_t)s * FS, 1.f};
-            dst[s][1] = LegDst{nullptr, 0.f};
-        }
-        legendre_synthesis<LB, false, NU, 2>(tab, nullptr, hs, NC * p.L2p, p.L2p, dst, nc, p.lmax, p.U, p.Uh, p.NTRI, J);
-    }
+    nbody_synthesis<LB, NU, 4>(tab, hs, NC4 * hstr, hstr, F, FS, nc, p.lmax, p.U, p.Uh, J);
     __syncthreads();
 
     // ---- S2b + S3 + S4a: one (column, u) per thread
@@ -156,8 +229,8 @@ static int launch_nbody_t(const Plan* p, const float* H, float* T, int64_t ncols
 {
     const int M = 2 * p->LB + 1;
     // columns per CTA: fill ~100 KB of shared memory (two CTAs per SM), at least 1 column
-    NbodySmem fixed = nbody_smem_layout(p, 0);
-    const int percol = NU * p->L2p * 4 + NU * M * p->U * 4;
+    NbodySmem fixed = nbody_smem_layout(p, 4);  // includes the padding of the H tiles to whole groups of 4 columns
+    const int percol = NU * nbody_hstride(p) * 4 + NU * M * p->U * 4;
     int NC = (100 * 1024 - fixed.total - 64) / percol;
     if (NC < 4) NC = (220 * 1024 - fixed.total - 64) / percol;
     if (NC < 1) { set_error("nbody core: shared memory too small for lmax=%d nu=%d", p->lmax, NU); return CGTP_ERR_UNSUPPORTED; }
@@ -165,12 +238,31 @@ static int launch_nbody_t(const Plan* p, const float* H, float* T, int64_t ncols
     // at least ~2 CTAs per SM when the problem is small
     while (NC > 8 && (ncols + NC - 1) / NC < 296) NC /= 2;
     if ((int64_t)NC > ncols) NC = (int)ncols;
+    {
+        // every stage deals its items over the 256 threads in strided passes: among the column counts near the one
+        // that fills shared memory take the one with the fewest idle thread slots in the last passes (estimated
+        // instruction cost per item: synthesis ~ 10 NU per degree, transform ~ Vh (2 NU + 2) LB, analysis ~ 3 Uh per degree)
+        const int nub = (p->Uh + 3) / 4;
+        const double c_syn = 10.0 * NU * (p->lmax + 2) / 2.0, c_dft = (double)p->Vh * (2 * NU + 2) * (p->LB + 1),
+                     c_ana = 3.0 * p->Uh * (p->lmax_out + 2) / 2.0;
+        auto passes = [](int items) { return (items + 255) / 256; };
+        int best = NC;
+        double bestc = 1e300;
+        for (int n = NC; n >= 1 && n >= NC * 2 / 3; --n) {
+            const double c = (passes((p->lmax + 1) * nub * n) * c_syn + passes(n * p->U) * c_dft +
+                              passes(n * (p->lmax_out + 1)) * c_ana) / n;
+            if ((n % 4 == 0 || n < 4) && c < bestc * 0.999) { bestc = c; best = n; }
+        }
+        NC = best;
+    }
+    if (NC >= 4 && (int64_t)NC < ncols) NC &= ~3;  // tiles start at 16-byte boundaries of H
+    if (NC < 4 && (int64_t)NC < ncols) { set_error("nbody core: fewer than 4 columns per CTA fit shared memory (lmax=%d nu=%d)", p->lmax, NU); return CGTP_ERR_UNSUPPORTED; }
     NbodySmem lay = nbody_smem_layout(p, NC);
     auto kern = nbody_core_kernel<LB, NU>;
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, lay.total));
     int64_t grid = (ncols + NC - 1) / NC;
     LaunchScope scope(K_ONSITE_EVEN, st);
-    kern<<<(unsigned)grid, 256, lay.total, st>>>(*p, lay, H, T, (long long)ncols, NC);
+    kern<<<(unsigned)grid, 256, lay.total, st>>>(*p, lay, H, (long long)nbody_hfstride(p, ncols), T, (long long)ncols, NC);
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
 }

@@ -5,6 +5,7 @@ ncu captures under profiles/ are made with.
     python -m paper_2605_15073_b200.profile_run --config 3 --lmax 20 --steps 1  # on-site sweep point
     python -m paper_2605_15073_b200.profile_run --config 4 --steps 1            # message passing, configs[4]
     python -m paper_2605_15073_b200.profile_run --config 1 --math-mode 1        # 3xTF32 tensor-core projections
+    python -m paper_2605_15073_b200.profile_run --config 1 --nu 3               # nu-body product at the shape of configs[1]
 """
 from __future__ import annotations
 
@@ -25,6 +26,8 @@ def main():
     ap.add_argument("--batch", type=int, default=None, help="override the batch / node count")
     ap.add_argument("--all-even", action="store_true")
     ap.add_argument("--math-mode", type=int, default=0, help="0 FP32 (default), 1 3xTF32, 2 TF32 projections")
+    ap.add_argument("--nu", type=int, default=0, help="> 0: cgtp_onsite_nbody with this body order at the on-site "
+                    "config's lmax, N, C, batch (all rank channels pointwise)")
     args = ap.parse_args()
     dev = torch.device("cuda", 0)
     cg.cgtp_set_math_mode(args.math_mode)
@@ -33,7 +36,13 @@ def main():
     if args.all_even:
         inp.parity_mask = np.zeros_like(inp.parity_mask)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    if isinstance(inp, synthetic.OnsiteInputs):
+    if args.nu > 0:
+        b = args.batch or inp.batch
+        nb = synthetic.make_nbody(args.nu, inp.lmax, inp.lmax_out, inp.N, inp.C, b, seed=0)
+        X, Wi, Wo = cu(nb.X), cu(nb.W_in), cu(nb.W_out)
+        fn = lambda: cg.cgtp_onsite_nbody(X, Wi, Wo, nb.nu, nb.lmax, nb.lmax_out, nb.N, nb.C)
+        units, unit = b, "products"
+    elif isinstance(inp, synthetic.OnsiteInputs):
         b = args.batch or inp.batch
         A, B = cu(inp.A[:b]), cu(inp.B[:b])
         Wa, Wb, Wo = cu(inp.W_a), cu(inp.W_b), cu(inp.W_out)
