@@ -59,8 +59,8 @@ static NbodySmem nbody_smem_layout(const Plan* p, int NC)
 // (u', U-1-u').  Table rows past Uh read by the last block are inside the shared-memory allocation; their sums are dropped.
 template <int LB, int NU, int UB>
 __device__ __forceinline__ void nbody_synthesis(const float* __restrict__ tab, const float* __restrict__ Hs,
-                                                int h_in_stride, int L2p, float* F, int FS, int NC, int lmax, int U,
-                                                int Uh, int J)
+                                                int h_in_stride, int L2p, float* F, int FS, int NC, int NCS, int lmax,
+                                                int U, int Uh, int J)
 {
     constexpr int NTRI = round_up((LB + 1) * (LB + 2) / 2, 4);
     const int nub = (Uh + UB - 1) / UB;
@@ -108,7 +108,7 @@ __device__ __forceinline__ void nbody_synthesis(const float* __restrict__ tab, c
         for (int e = 0; e < UB; ++e) {
             const int up = ub * UB + e;
             if (up < Uh) {
-                const int jn = col * U + up, js = col * U + (U - 1 - up);
+                const int jn = up * NCS + col, js = (U - 1 - up) * NCS + col;  // j = u * NCS + col: lanes = columns
 #pragma unroll
                 for (int a = 0; a < NU; ++a) {
                     float* Fa = F + (size_t)a * FS;
@@ -166,6 +166,57 @@ __device__ __forceinline__ void dft_nproduct_idft(float* F, int FS, int J, int j
     for (int r = 0; r < M; ++r) F[r * J + j] = t[r];
 }
 
+// Row S4b (Eq.(40)): legendre_analysis of sht.cuh on the column-fastest row layout j = u * NCS + col.
+// Work item = (column, |m|), |m| fastest: lanes read different coefficient rows (odd row stride J, no bank conflicts)
+// and store neighbouring output coefficients.  North and south node are folded with the reflection parity (-1)^(l-m).
+template <int LB, int UHMAX>
+__device__ __forceinline__ void nbody_analysis(const float* Tr, const float* __restrict__ WP, float* __restrict__ out,
+                                               int Lo2p, int NC, int NCS, int lmax_out, int U, int Uh, int J)
+{
+    constexpr int NTRI = round_up((LB + 1) * (LB + 2) / 2, 4);
+    const int items = NC * (lmax_out + 1);
+    for (int item = threadIdx.x; item < items; item += blockDim.x) {
+        const int col = item / (lmax_out + 1);
+        const int mm = item - col * (lmax_out + 1);
+        float tp[2][UHMAX], tm[2][UHMAX];  // [+m, -m][u']: north + south, north - south
+#pragma unroll
+        for (int sg = 0; sg < 2; ++sg) {
+            const int row = (sg == 0) ? mm : (LB + mm);
+#pragma unroll
+            for (int up = 0; up < UHMAX; ++up) {
+                float n = 0.f, so = 0.f;
+                if (up < Uh && !(sg == 1 && mm == 0)) {
+                    n = Tr[row * J + up * NCS + col];
+                    so = Tr[row * J + (U - 1 - up) * NCS + col];
+                }
+                tp[sg][up] = n + so;
+                tm[sg][up] = n - so;
+            }
+        }
+        float* ocol = out + (size_t)col * Lo2p;
+        for (int l0 = mm; l0 <= lmax_out; l0 += 2) {
+#pragma unroll
+            for (int par = 0; par < 2; ++par) {
+                const int l = l0 + par;
+                if (l <= lmax_out) {
+                    const int t = tri_index(l, mm);
+                    float ap = 0.f, an = 0.f;
+#pragma unroll
+                    for (int up = 0; up < UHMAX; ++up) {
+                        if (up < Uh) {
+                            const float w = WP[up * NTRI + t];
+                            ap = fmaf(w, par ? tm[0][up] : tp[0][up], ap);
+                            an = fmaf(w, par ? tm[1][up] : tp[1][up], an);
+                        }
+                    }
+                    ocol[l * l + l + mm] = ap;
+                    if (mm > 0) ocol[l * l + l - mm] = an;
+                }
+            }
+        }
+    }
+}
+
 template <int LB, int NU>
 __global__ void __launch_bounds__(256, 2) nbody_core_kernel(Plan p, NbodySmem lay, const float* __restrict__ H,
                                                             long long hfs, float* __restrict__ T, long long ncols, int NC)
@@ -212,26 +263,29 @@ __global__ void __launch_bounds__(256, 2) nbody_core_kernel(Plan p, NbodySmem la
     mbar_wait(bar, 0);
 
     // ---- S2a: Legendre synthesis of the NU factors
-    nbody_synthesis<LB, NU, 4>(tab, hs, NC4 * hstr, hstr, F, FS, nc, p.lmax, p.U, p.Uh, J);
+    nbody_synthesis<LB, NU, 4>(tab, hs, NC4 * hstr, hstr, F, FS, nc, NC, p.lmax, p.U, p.Uh, J);
     __syncthreads();
 
     // ---- S2b + S3 + S4a: one (column, u) per thread
     const int rows = nc * p.U;
-    for (int j = threadIdx.x; j < rows; j += blockDim.x) dft_nproduct_idft<LB, NU>(F, FS, J, j, qc, qs, wv, p.Vh);
+    for (int item = threadIdx.x; item < rows; item += blockDim.x) {
+        const int u = item / nc, col = item - u * nc;
+        dft_nproduct_idft<LB, NU>(F, FS, J, u * NC + col, qc, qs, wv, p.Vh);
+    }
     __syncthreads();
 
     // ---- S4b: Gauss-Legendre analysis
-    legendre_analysis<LB, UHMAX>(F, nullptr, wp, T + col0 * p.Lo2p, p.Lo2p, nc, p.lmax_out, p.U, p.Uh, p.NTRI, J);
+    nbody_analysis<LB, UHMAX>(F, wp, T + col0 * p.Lo2p, p.Lo2p, nc, NC, p.lmax_out, p.U, p.Uh, J);
 }
 
 template <int LB, int NU>
 static int launch_nbody_t(const Plan* p, const float* H, float* T, int64_t ncols, cudaStream_t st)
 {
     const int M = 2 * p->LB + 1;
-    // columns per CTA: fill ~100 KB of shared memory (two CTAs per SM), at least 1 column
+    // columns per CTA: fill ~112 KB of shared memory (two CTAs per SM), at least 1 column
     NbodySmem fixed = nbody_smem_layout(p, 4);  // includes the padding of the H tiles to whole groups of 4 columns
     const int percol = NU * nbody_hstride(p) * 4 + NU * M * p->U * 4;
-    int NC = (100 * 1024 - fixed.total - 64) / percol;
+    int NC = (112 * 1024 - fixed.total - 64) / percol;
     if (NC < 4) NC = (220 * 1024 - fixed.total - 64) / percol;
     if (NC < 1) { set_error("nbody core: shared memory too small for lmax=%d nu=%d", p->lmax, NU); return CGTP_ERR_UNSUPPORTED; }
     if (NC > 128) NC = 128;
