@@ -133,11 +133,19 @@ __device__ __forceinline__ void dft_nproduct_idft(float* F, int FS, int J, int j
 {
     constexpr int M = 2 * LB + 1;
     constexpr int QSTR = round_up(LB + 1, 4);
-    float f[NU][M], t[M];
+    constexpr int NP = NU / 2, NR = NU % 2;  // factors are transformed two at a time in packed FP32 (FFMA2: the
+                                             // Fourier coefficient is the scalar broadcast to both halves)
+    float2 f2[NP > 0 ? NP : 1][M];
+    float fr[M], t[M];
 #pragma unroll
-    for (int s = 0; s < NU; ++s)
+    for (int q = 0; q < NP; ++q)
 #pragma unroll
-        for (int r = 0; r < M; ++r) f[s][r] = F[(size_t)s * FS + r * J + j];
+        for (int r = 0; r < M; ++r)
+            f2[q][r] = make_float2(F[(size_t)(2 * q) * FS + r * J + j], F[(size_t)(2 * q + 1) * FS + r * J + j]);
+    if (NR) {
+#pragma unroll
+        for (int r = 0; r < M; ++r) fr[r] = F[(size_t)(NU - 1) * FS + r * J + j];
+    }
 #pragma unroll
     for (int r = 0; r < M; ++r) t[r] = 0.f;
     for (int vp = 0; vp < Vh; ++vp) {
@@ -146,14 +154,23 @@ __device__ __forceinline__ void dft_nproduct_idft(float* F, int FS, int J, int j
         load_q_row<LB>(QS, vp, qs);
         float s1 = 1.f, s2 = 1.f;
 #pragma unroll
-        for (int s = 0; s < NU; ++s) {
+        for (int q = 0; q < NP; ++q) {
+            float2 ce = make_float2(0.f, 0.f), so = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int m = 0; m <= LB; ++m) ce = __ffma2_rn(make_float2(qc[m], qc[m]), f2[q][m], ce);
+#pragma unroll
+            for (int m = 1; m <= LB; ++m) so = __ffma2_rn(make_float2(qs[m], qs[m]), f2[q][LB + m], so);
+            s1 *= (ce.x + so.x) * (ce.y + so.y);  // grid point v'
+            s2 *= (ce.x - so.x) * (ce.y - so.y);  // mirrored grid point V - v'
+        }
+        if (NR) {
             float ce = 0.f, so = 0.f;
 #pragma unroll
-            for (int m = 0; m <= LB; ++m) ce = fmaf(qc[m], f[s][m], ce);
+            for (int m = 0; m <= LB; ++m) ce = fmaf(qc[m], fr[m], ce);
 #pragma unroll
-            for (int m = 1; m <= LB; ++m) so = fmaf(qs[m], f[s][LB + m], so);
-            s1 *= ce + so;  // grid point v'
-            s2 *= ce - so;  // mirrored grid point V - v'
+            for (int m = 1; m <= LB; ++m) so = fmaf(qs[m], fr[LB + m], so);
+            s1 *= ce + so;
+            s2 *= ce - so;
         }
         const float w = WV[vp];
         const float sp = w * (s1 + s2), sm = w * (s1 - s2);
