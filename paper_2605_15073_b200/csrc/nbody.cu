@@ -26,7 +26,7 @@ bool nbody_supported(int LB, int nu) { return LB >= 1 && LB <= kNbodyMaxBand && 
 
 struct NbodySmem {
     // byte offsets into dynamic shared memory (all multiples of 16)
-    int bar, tab, wp, qc, qs, wv, hs, f, total;
+    int bar, tab, wp, qc, qs, qi, wv, hs, f, total;
     int tab_bytes, q_bytes, wv_bytes;
 };
 
@@ -44,6 +44,7 @@ static NbodySmem nbody_smem_layout(const Plan* p, int NC)
     s.wp = off; off += s.tab_bytes;
     s.qc = off; off += s.q_bytes;
     s.qs = off; off += s.q_bytes;
+    s.qi = off; off += p->Vh * round_up(p->LB + 1, 2) * 8;
     s.wv = off; off += s.wv_bytes;
     s.hs = off; off += p->nu * round_up(NC, 4) * nbody_hstride(p) * 4;
     s.f = off; off += round_up(p->nu * M * J, 4) * 4;
@@ -127,60 +128,70 @@ __device__ __forceinline__ void nbody_synthesis(const float* __restrict__ tab, c
 // Rows S2b + S3 + S4a for one (column, u): forward real DFT of the NU coefficient vectors, product of the NU grid
 // values at the azimuth pair (v', V - v'), inverse real DFT.  F: NU fields [M][J] at distance FS; the result T[m]
 // overwrites field 0 at [.][j].
+// QI: interleaved Fourier table [Vh][QP] of pairs (qc[m], qs[m]), QP = LB + 1 rounded up to 2 pairs (16 bytes).
+// Packed FP32 throughout (FFMA2): factors two at a time with the Fourier coefficient broadcast to both halves; an odd
+// last factor and the inverse transform as (cosine part, sine part) pairs against the (qc, qs) pair.
 template <int LB, int NU>
-__device__ __forceinline__ void dft_nproduct_idft(float* F, int FS, int J, int j, const float* __restrict__ QC,
-                                                  const float* __restrict__ QS, const float* __restrict__ WV, int Vh)
+__device__ __forceinline__ void dft_nproduct_idft(float* F, int FS, int J, int j, const float2* __restrict__ QI,
+                                                  const float* __restrict__ WV, int Vh)
 {
     constexpr int M = 2 * LB + 1;
-    constexpr int QSTR = round_up(LB + 1, 4);
-    constexpr int NP = NU / 2, NR = NU % 2;  // factors are transformed two at a time in packed FP32 (FFMA2: the
-                                             // Fourier coefficient is the scalar broadcast to both halves)
-    float2 f2[NP > 0 ? NP : 1][M];
-    float fr[M], t[M];
+    constexpr int QP = round_up(LB + 1, 2);
+    constexpr int NP = NU / 2, NR = NU % 2;
+    float2 f2[NP > 0 ? NP : 1][M];  // (factor 2q, factor 2q+1)[row]
+    float2 fr[LB + 1];              // odd last factor: (cosine row m, sine row m)
+    float2 t[LB + 1];               // result: (cosine row m, sine row m)
 #pragma unroll
     for (int q = 0; q < NP; ++q)
 #pragma unroll
         for (int r = 0; r < M; ++r)
             f2[q][r] = make_float2(F[(size_t)(2 * q) * FS + r * J + j], F[(size_t)(2 * q + 1) * FS + r * J + j]);
     if (NR) {
+        const float* Fl = F + (size_t)(NU - 1) * FS;
+        fr[0] = make_float2(Fl[j], 0.f);
 #pragma unroll
-        for (int r = 0; r < M; ++r) fr[r] = F[(size_t)(NU - 1) * FS + r * J + j];
+        for (int m = 1; m <= LB; ++m) fr[m] = make_float2(Fl[m * J + j], Fl[(LB + m) * J + j]);
     }
 #pragma unroll
-    for (int r = 0; r < M; ++r) t[r] = 0.f;
+    for (int m = 0; m <= LB; ++m) t[m] = make_float2(0.f, 0.f);
     for (int vp = 0; vp < Vh; ++vp) {
-        float qc[QSTR], qs[QSTR];
-        load_q_row<LB>(QC, vp, qc);
-        load_q_row<LB>(QS, vp, qs);
+        float2 qi[QP];
+        const float4* src = reinterpret_cast<const float4*>(QI + vp * QP);
+#pragma unroll
+        for (int i = 0; i < QP / 2; ++i) {
+            const float4 v = src[i];
+            qi[2 * i] = make_float2(v.x, v.y);
+            qi[2 * i + 1] = make_float2(v.z, v.w);
+        }
         float s1 = 1.f, s2 = 1.f;
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
             float2 ce = make_float2(0.f, 0.f), so = make_float2(0.f, 0.f);
 #pragma unroll
-            for (int m = 0; m <= LB; ++m) ce = __ffma2_rn(make_float2(qc[m], qc[m]), f2[q][m], ce);
+            for (int m = 0; m <= LB; ++m) ce = __ffma2_rn(make_float2(qi[m].x, qi[m].x), f2[q][m], ce);
 #pragma unroll
-            for (int m = 1; m <= LB; ++m) so = __ffma2_rn(make_float2(qs[m], qs[m]), f2[q][LB + m], so);
+            for (int m = 1; m <= LB; ++m) so = __ffma2_rn(make_float2(qi[m].y, qi[m].y), f2[q][LB + m], so);
             s1 *= (ce.x + so.x) * (ce.y + so.y);  // grid point v'
             s2 *= (ce.x - so.x) * (ce.y - so.y);  // mirrored grid point V - v'
         }
         if (NR) {
-            float ce = 0.f, so = 0.f;
+            float2 cs = make_float2(0.f, 0.f);  // (cosine part, sine part)
 #pragma unroll
-            for (int m = 0; m <= LB; ++m) ce = fmaf(qc[m], fr[m], ce);
-#pragma unroll
-            for (int m = 1; m <= LB; ++m) so = fmaf(qs[m], fr[LB + m], so);
-            s1 *= ce + so;
-            s2 *= ce - so;
+            for (int m = 0; m <= LB; ++m) cs = __ffma2_rn(qi[m], fr[m], cs);
+            s1 *= cs.x + cs.y;
+            s2 *= cs.x - cs.y;
         }
         const float w = WV[vp];
-        const float sp = w * (s1 + s2), sm = w * (s1 - s2);
+        const float2 spm = make_float2(w * (s1 + s2), w * (s1 - s2));
 #pragma unroll
-        for (int m = 0; m <= LB; ++m) t[m] = fmaf(qc[m], sp, t[m]);
-#pragma unroll
-        for (int m = 1; m <= LB; ++m) t[LB + m] = fmaf(qs[m], sm, t[LB + m]);
+        for (int m = 0; m <= LB; ++m) t[m] = __ffma2_rn(qi[m], spm, t[m]);  // qs[0] = 0: t[0].y stays 0
     }
+    F[j] = t[0].x;
 #pragma unroll
-    for (int r = 0; r < M; ++r) F[r * J + j] = t[r];
+    for (int m = 1; m <= LB; ++m) {
+        F[m * J + j] = t[m].x;
+        F[(LB + m) * J + j] = t[m].y;
+    }
 }
 
 // Row S4b (Eq.(40)): legendre_analysis of sht.cuh on the column-fastest row layout j = u * NCS + col.
@@ -278,6 +289,15 @@ __global__ void __launch_bounds__(256, 2) nbody_core_kernel(Plan p, NbodySmem la
 #pragma unroll
     for (int s = 0; s < NU; ++s) zero_high_rows<LB>(F + (size_t)s * FS, p.lmax, J);
     mbar_wait(bar, 0);
+    // interleaved Fourier table for the packed azimuthal stage (read after the barrier that ends the synthesis)
+    float2* qi = reinterpret_cast<float2*>(smem + lay.qi);
+    {
+        constexpr int QP = round_up(LB + 1, 2);
+        for (int i = threadIdx.x; i < p.Vh * QP; i += blockDim.x) {
+            const int vp = i / QP, m = i - vp * QP;
+            qi[i] = (m <= LB) ? make_float2(qc[vp * p.QSTR + m], qs[vp * p.QSTR + m]) : make_float2(0.f, 0.f);
+        }
+    }
 
     // ---- S2a: Legendre synthesis of the NU factors
     nbody_synthesis<LB, NU, 4>(tab, hs, NC4 * hstr, hstr, F, FS, nc, NC, p.lmax, p.U, p.Uh, J);
@@ -287,7 +307,7 @@ __global__ void __launch_bounds__(256, 2) nbody_core_kernel(Plan p, NbodySmem la
     const int rows = nc * p.U;
     for (int item = threadIdx.x; item < rows; item += blockDim.x) {
         const int u = item / nc, col = item - u * nc;
-        dft_nproduct_idft<LB, NU>(F, FS, J, u * NC + col, qc, qs, wv, p.Vh);
+        dft_nproduct_idft<LB, NU>(F, FS, J, u * NC + col, qi, wv, p.Vh);
     }
     __syncthreads();
 
