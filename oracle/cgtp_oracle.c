@@ -38,7 +38,10 @@
  * (oracle_*_lw) against the l-shared functions (equal weights, degree selection, per-degree numpy
  * projections around them) and rotation; the nu-body function (oracle_onsite_nbody) against fine-grid
  * quadrature of the pointwise product, the closed form Y_10^3 = (3/4pi)^(3/2) (3/5 z + 2/5 P_3(z)), the
- * reduction to oracle_onsite at nu = 2, factor permutation and rotation (tests/test_oracle_nbody.py).
+ * reduction to oracle_onsite at nu = 2, factor permutation and rotation (tests/test_oracle_nbody.py); the
+ * two-field function (oracle_message_field, Eq.(28)) against oracle_message for edge fields of the form R.Y,
+ * fine-grid quadrature of the pooled pointwise product, one-edge receivers = oracle_onsite, edge order inside a
+ * segment and rotation (tests/test_oracle_field.py).
  * No function here is "parity unpinned".
  *
  * Plain C99 + OpenMP, double precision (long double inside the Racah sum).
@@ -895,6 +898,77 @@ int oracle_onsite_nbody(const double *X, const double *W_in, const double *W_out
         }
         free(H); free(P); free(Pn); free(T);
     }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Two feature fields, Eq.(28) (Sec. VII C f :471): the edge side is a general      */
+/* feature field I^(E)[e,n1,l1m1] that no longer factors as R.Y, the node side the sender's       */
+/* feature I^(N)[j,n2,l2m2].  With the CP factorisation (Eq.(3) :39; "an explicit radial          */
+/* contraction ... on the edge side, replacing R~ by an analogue of Eq.(47)", :471):              */
+/*   a[e,c,:]  = W_edge[c,:] . edge_feats[e]                 (factor 1, analogue of Eq.(47))      */
+/*   H[j,c,:]  = W_node[c,:] . node_feats[j]                 (factor 2, Eq.(47) :398)             */
+/*   T[i,c,lm] = sum_{e: recv(e)=i} sum coef(i1,i2;lm) a[e,c,i1] H[send(e),c,i2]                  */
+/*               coef = Gr (mask 0, Category alpha) or Qr (mask 1, Category beta, Eq.(57) :443)   */
+/*   out[i,s,n,lm] = sum_{c: mask[c]=s} W_out[n,c] T[i,c,lm]                                      */
+/* Reading R21: natural-parity slots on both fields (the (p1,p2) slot dispatch of     */
+/* :471 is a routing layer over this coupling, as in oracle_*_parity), l-shared weights (R5).     */
+/* Layouts: node_feats [nodes,N,L2]; edge_feats [E,Ne,L2]; W_edge [C,Ne]; W_node [C,N];           */
+/* W_out [N,C]; out [nodes,2,N,Lo2].                                                              */
+/* ------------------------------------------------------------------------------------------ */
+int oracle_message_field(const double *node_feats, const int64_t *edge_index /* [2,E] */, const double *edge_feats,
+                         const double *W_edge, const double *W_node, const double *W_out, int lmax, int lmax_out,
+                         int N, int Ne, int C, const uint8_t *parity_mask, double *out, int64_t nodes, int64_t E)
+{
+    int L2 = (lmax + 1) * (lmax + 1), Lo2 = (lmax_out + 1) * (lmax_out + 1);
+    const coupling_t *tab[2];
+    tab[0] = get_coupling(lmax, lmax_out, 0);
+    tab[1] = get_coupling(lmax, lmax_out, 1);
+    if (!tab[0] || !tab[1]) return 2;
+    int64_t *row_ptr = malloc((size_t)(nodes + 1) * sizeof(int64_t));
+    int rc = oracle_segments(edge_index, E, nodes, row_ptr);
+    if (rc) { free(row_ptr); return rc; }
+    const int64_t *snd = edge_index;
+#pragma omp parallel
+    {
+        double *a = malloc((size_t)C * L2 * sizeof(double));
+        double *h = malloc((size_t)C * L2 * sizeof(double));
+        double *T = malloc((size_t)C * Lo2 * sizeof(double));
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t i = 0; i < nodes; ++i) {
+            for (size_t k = 0; k < (size_t)C * Lo2; ++k) T[k] = 0.0;
+            for (int64_t e = row_ptr[i]; e < row_ptr[i + 1]; ++e) {
+                const double *xe = edge_feats + e * (int64_t)Ne * L2;
+                const double *xj = node_feats + snd[e] * (int64_t)N * L2;
+                for (int c = 0; c < C; ++c)
+                    for (int q = 0; q < L2; ++q) {
+                        double sa = 0.0, sh = 0.0;
+                        for (int n = 0; n < Ne; ++n) sa += W_edge[c * Ne + n] * xe[n * L2 + q];
+                        for (int n = 0; n < N; ++n) sh += W_node[c * N + n] * xj[n * L2 + q];
+                        a[c * L2 + q] = sa;
+                        h[c * L2 + q] = sh;
+                    }
+                for (int c = 0; c < C; ++c) {
+                    const coupling_t *t = tab[parity_mask[c] ? 1 : 0];
+                    double *Tc = T + (size_t)c * Lo2;
+                    const double *ac = a + (size_t)c * L2, *hc = h + (size_t)c * L2;
+                    for (int64_t k = 0; k < t->nnz; ++k)
+                        Tc[t->io[k]] += t->val[k] * ac[t->i1[k]] * hc[t->i2[k]];
+                }
+            }
+            double *ob = out + i * 2 * (int64_t)N * Lo2;
+            for (int s = 0; s < 2; ++s)
+                for (int n = 0; n < N; ++n)
+                    for (int q = 0; q < Lo2; ++q) {
+                        double acc = 0.0;
+                        for (int c = 0; c < C; ++c)
+                            if ((parity_mask[c] ? 1 : 0) == s) acc += W_out[n * C + c] * T[(size_t)c * Lo2 + q];
+                        ob[((size_t)s * N + n) * Lo2 + q] = acc;
+                    }
+        }
+        free(a); free(h); free(T);
+    }
+    free(row_ptr);
     return 0;
 }
 

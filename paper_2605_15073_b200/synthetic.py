@@ -131,6 +131,17 @@ def make_message(lmax: int, lmax_out: int, N: int, C: int, nodes: int, degree, r
                          W_node, W_out, mask, deg)
 
 
+def make_edge_field(m: MessageInputs, Ne: int, seed: int = 0):
+    """Edge feature field of the two-field coupling Eq.(28) for the graph `m`: edge_feats [E, Ne, L2]
+    ~N(0,1) per real-SH coefficient (a deeper layer's edge message, no longer of the form R.Y) and its CP projection
+    weights W_edge [C, Ne] ~N(0, 1/sqrt(Ne)).  Holds none of the method's arithmetic."""
+    rF, rW = _streams(seed + 7919, 2)
+    L2 = (m.lmax + 1) ** 2
+    edge_feats = rF.standard_normal((m.E, Ne, L2), dtype=np.float32)
+    W_edge = (rW.standard_normal((m.C, Ne), dtype=np.float32) / np.float32(np.sqrt(Ne))).astype(np.float32)
+    return edge_feats, W_edge
+
+
 # ---------------------------------------------------------------------------------------------
 # Parity-labelled inputs (SURVEY.md 8(f) NEXT-1; PAPER.md Sec. VI, VII C a-c, e): a parity-slot axis on the
 # features (slot 0 natural parity (-1)^l, slot 1 opposite) and one independent weight set per run.
