@@ -85,6 +85,39 @@ int cgtp_onsite(const float* A, const float* B, const float* W_a, const float* W
                 int64_t batch, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * Two feature fields (Eq.(28) :236, Sec. VI E :232-:240, Sec. VII C f :471):
+ * "the deeper message-passing variant in which the edge-side message ... no longer factors as R.Y", written with
+ * an edge field I^(E)[e, n1, l1 m1] and a node field I^(N)[j, n2, l2 m2].  At fixed CP rank (Eq.(3) :39; "an
+ * explicit radial contraction is required on the edge side, replacing R~ by an analogue of Eq.(47)", :471):
+ *
+ *   a[e,c,:]      = W_edge[c,:] . edge_feats[e]                                  (factor 1)
+ *   H[j,c,:]      = W_node[c,:] . node_feats[j]                                  (factor 2, Eq.(47) :398)
+ *   T[i,c,lm]     = sum_{e: recv(e)=i} int P(a~[e,c], H~[send(e),c])(Omega) Y_lm dOmega
+ *                   P = pointwise product (parity_mask[c] = 0, Category alpha, Eq.(52) :415) or the surface-curl
+ *                   pairing {a~, H~} (parity_mask[c] = 1, Category beta, Eq.(57) :443; the edge field is factor 1)
+ *   out[i,s,n,lm] = sum_{c: mask[c]=s} W_out[n,c] T[i,c,lm]                      (Eq.(55), (58))
+ *
+ * Both fields sit in their natural-parity slots and the weights are l-shared; sector 0 / 1 of `out` as in
+ * cgtp_message.  Every edge is one fused synthesis-product-analysis pass (the grids stay on chip); the per-edge
+ * coefficients are pooled per receiver in edge order (fixed order, no float atomics, bitwise reproducible).
+ *
+ * node_feats device [nodes, N, (lmax+1)^2]      edge_feats device [E, Ne, (lmax+1)^2]
+ * edge_index device int64 [2, E], row 0 sender, row 1 receiver, receiver-sorted (validated on the device: query
+ *            cgtp_message_status(workspace, stream); on CGTP_ERR_GRAPH `out` is undefined)
+ * W_edge device [C, Ne]    W_node device [C, N]    W_out device [N, C]    parity_mask HOST [C]
+ * out    device [nodes, 2, N, (lmax_out+1)^2]; receivers without in-edges get zeros
+ * workspace device, >= cgtp_message_field_workspace_bytes(...) bytes, 256-byte aligned (scratch; edges are
+ *           processed in chunks of at most 2^22 / C, so the size is bounded in E)
+ * nodes or E may be 0.  Errors as cgtp_message.  Asynchronous on cuda_stream.
+ * ------------------------------------------------------------------------------------------- */
+size_t cgtp_message_field_workspace_bytes(int lmax, int lmax_out, int N, int Ne, int C, int64_t nodes, int64_t E);
+
+int cgtp_message_field(const float* node_feats, const int64_t* edge_index, const float* edge_feats, const float* W_edge,
+                       const float* W_node, const float* W_out, int lmax, int lmax_out, int N, int Ne, int C,
+                       const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* workspace,
+                       size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * nu-body on-site product (end of Sec. VI): "The grid pointwise product
  * extends to nu-body features through additional pointwise multiplications on the grid followed by a single
  * inverse transform", on the grid U = ceil((nu lmax + lmax_out + 1)/2), V = nu lmax + lmax_out + 1 that the

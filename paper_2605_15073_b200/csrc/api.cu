@@ -717,6 +717,177 @@ int cgtp_onsite_nbody(const float* X, const float* W_in, const float* W_out, int
     return launch_proj_degrees(po, 1, K_PROJ_OUT, st);
 }
 
+// ------------------------------------------------------------------------------ two feature fields, Eq.(28)
+// Edges are processed in chunks of at most field_chunk(C) so that the per-edge buffers stay bounded (<= 2^22 columns).
+static int64_t field_chunk(int C, int64_t E)
+{
+    const int64_t cap = ((int64_t)1 << 22) / C;
+    return E < cap ? E : cap;
+}
+
+static size_t field_ws_bytes(int lmax, int lmax_out, int C, int64_t nodes, int64_t E)
+{
+    const size_t L2p = round_up((lmax + 1) * (lmax + 1), 4), Lo2p = round_up((lmax_out + 1) * (lmax_out + 1), 4);
+    const size_t ec = (size_t)field_chunk(C, E);
+    // per chunk: Ha, Hb (two parities, columns padded to groups of 32), T; per node: Hn, Tn; status, row_ptr
+    const size_t fl = (ec * C + 128) * (2 * (L2p + 4) + (Lo2p + 4)) + ((size_t)nodes * C + 128) * ((L2p + 4) + (Lo2p + 4));
+    return 256 + fl * sizeof(float) + (size_t)(nodes + 1) * sizeof(int64_t) + 16 * 256;
+}
+
+size_t cgtp_message_field_workspace_bytes(int lmax, int lmax_out, int N, int Ne, int C, int64_t nodes, int64_t E)
+{
+    (void)N;
+    (void)Ne;
+    if (lmax < 0 || lmax_out < 0 || C <= 0 || nodes < 0 || E < 0) return 0;
+    return field_ws_bytes(lmax, lmax_out, C, nodes, E);
+}
+
+int cgtp_message_field(const float* node_feats, const int64_t* edge_index, const float* edge_feats, const float* W_edge,
+                       const float* W_node, const float* W_out, int lmax, int lmax_out, int N, int Ne, int C,
+                       const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* workspace,
+                       size_t workspace_bytes, void* cuda_stream)
+{
+    clear_error();
+    int rc = check_common(lmax, lmax_out, N, C, parity_mask);
+    if (rc) return rc;
+    if (Ne <= 0) { set_error("Ne must be positive (Ne=%d)", Ne); return CGTP_ERR_INVALID; }
+    if (nodes < 0 || E < 0) { set_error("negative size"); return CGTP_ERR_INVALID; }
+    if (nodes == 0) return CGTP_OK;
+    if (!node_feats || !W_edge || !W_node || !W_out || !out || !workspace || (E > 0 && (!edge_index || !edge_feats))) {
+        set_error("null pointer argument");
+        return CGTP_ERR_INVALID;
+    }
+    if (!aligned16(node_feats) || !aligned16(out) || !aligned16(W_edge) || !aligned16(W_node) || !aligned16(W_out) ||
+        (E > 0 && (!aligned16(edge_index) || !aligned16(edge_feats))) || (reinterpret_cast<uintptr_t>(workspace) & 255u)) {
+        set_error("misaligned pointer (tensors need 16-byte, workspace 256-byte alignment)");
+        return CGTP_ERR_INVALID;
+    }
+    if (workspace_bytes < field_ws_bytes(lmax, lmax_out, C, nodes, E)) {
+        set_error("workspace too small: %zu < %zu bytes", workspace_bytes, field_ws_bytes(lmax, lmax_out, C, nodes, E));
+        return CGTP_ERR_INVALID;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const Plan* p = get_plan(lmax, lmax_out);
+    if (!p) return CGTP_ERR_CUDA;
+    const ChannelPlan* cp = get_channel_plan(C, parity_mask);
+    if (!cp) return CGTP_ERR_CUDA;
+    const int Cpar[2] = {cp->Ce, cp->Co};
+    const bool fast = (Cpar[0] == 0 || onsite_fast_supported(p, false)) && (Cpar[1] == 0 || onsite_fast_supported(p, true));
+    const int hstr = fast ? onsite_fast_hstride(p) : p->L2p;
+    const int tstr = fast ? onsite_fast_tstride(p) : p->Lo2p;
+    const int64_t ec_max = field_chunk(C, E);
+
+    Carver cv(workspace);
+    int32_t* status = cv.take<int32_t>(1);
+    int64_t* row_ptr = cv.take<int64_t>((size_t)nodes + 1);
+    float *Hn[2], *Tn[2], *Ha[2], *Hb[2], *T[2];
+    size_t ncol[2];
+    for (int s = 0; s < 2; ++s) {
+        ncol[s] = (size_t)round_up64(ec_max * Cpar[s], 32);
+        Hn[s] = cv.take<float>((size_t)nodes * Cpar[s] * hstr);
+        Tn[s] = cv.take<float>((size_t)nodes * Cpar[s] * tstr);
+        Ha[s] = cv.take<float>(ncol[s] * hstr);
+        Hb[s] = cv.take<float>(ncol[s] * hstr);
+        T[s] = cv.take<float>(ncol[s] * tstr);
+    }
+
+    // M0
+    rc = launch_segments(edge_index, E, nodes, nodes, row_ptr, status, st);
+    if (rc) return rc;
+
+    // factor 2: Hn = W_node . node_feats, once per node (Eq.(47) :398)
+    ProjArgs a;
+    a.X = node_feats;
+    a.x_bs = (int64_t)N * p->L2;
+    a.x_rs = p->L2;
+    a.W = W_node;
+    a.ldw_m = N;
+    a.ldw_k = 1;
+    a.idx_m = cp->perm_dev;
+    a.idx_k = nullptr;
+    a.M = C;
+    a.K = N;
+    a.J = p->L2;
+    a.out0 = Hn[0];
+    a.o_bs0 = (int64_t)Cpar[0] * hstr;
+    a.out1 = Hn[1];
+    a.o_bs1 = (int64_t)Cpar[1] * hstr;
+    a.m_split = Cpar[0];
+    a.o_rs = hstr;
+    a.batch = nodes;
+    a.accumulate = 0;
+    a.j0 = 0;
+    rc = launch_proj(&a, 1, K_PROJ_IN, st);
+    if (rc) return rc;
+
+    for (int64_t e0 = 0; e0 == 0 || e0 < E; e0 += ec_max) {
+        const int64_t ec = E - e0 < ec_max ? E - e0 : ec_max;
+        if (ec > 0) {
+            // factor 1: Ha = W_edge . edge_feats ("an explicit radial contraction ... on the edge side", :471)
+            ProjArgs b = a;
+            b.X = edge_feats + (size_t)e0 * Ne * p->L2;
+            b.x_bs = (int64_t)Ne * p->L2;
+            b.W = W_edge;
+            b.ldw_m = Ne;
+            b.K = Ne;
+            b.out0 = Ha[0];
+            b.out1 = Ha[1];
+            b.batch = ec;
+            rc = launch_proj(&b, 1, K_PROJ_IN, st);
+            if (rc) return rc;
+        }
+        for (int s = 0; s < 2; ++s) {
+            const int64_t nc = ec * Cpar[s];
+            if (nc > 0) {
+                const size_t pad = (size_t)round_up64(nc, 32) - (size_t)nc;
+                if (pad) {  // columns that pad the last group of 32: defined, never read back
+                    CGTP_CUDA_CHECK(cudaMemsetAsync(Ha[s] + (size_t)nc * hstr, 0, pad * hstr * 4, st));
+                    CGTP_CUDA_CHECK(cudaMemsetAsync(Hb[s] + (size_t)nc * hstr, 0, pad * hstr * 4, st));
+                }
+                rc = launch_field_gather(Hn[s], edge_index + e0, Hb[s], ec, Cpar[s] * hstr, status, st);
+                if (rc) return rc;
+                // S2-S4 per edge: the edge field is factor 1 (R10), the sender's field factor 2
+                rc = fast ? launch_onsite_fast(p, s == 1, Ha[s], Hb[s], T[s], nc, st)
+                          : launch_onsite_generic(p, s == 1, Ha[s], Hb[s], T[s], nc, st);
+                if (rc) return rc;
+            }
+            // sum over the in-edges of every receiver (Eq.(28) sum_j), in edge order
+            if (Cpar[s] > 0) {
+                rc = launch_field_pool(T[s], row_ptr, Tn[s], nodes, e0, e0 + ec, Cpar[s] * tstr, status, st);
+                if (rc) return rc;
+            }
+        }
+        if (E == 0) break;
+    }
+
+    // output projection per receiver (Eq.(55), (58))
+    std::vector<ProjArgs> pv(2);
+    for (int s = 0; s < 2; ++s) {
+        ProjArgs& o = pv[s];
+        o.X = Tn[s];
+        o.x_bs = (int64_t)Cpar[s] * tstr;
+        o.x_rs = tstr;
+        o.W = W_out;
+        o.ldw_m = C;
+        o.ldw_k = 1;
+        o.idx_m = nullptr;
+        o.idx_k = cp->perm_dev + (s ? cp->Ce : 0);
+        o.M = N;
+        o.K = Cpar[s];
+        o.J = p->Lo2;
+        o.out0 = out + (size_t)s * N * p->Lo2;
+        o.o_bs0 = (int64_t)2 * N * p->Lo2;
+        o.out1 = o.out0;
+        o.o_bs1 = o.o_bs0;
+        o.m_split = N;
+        o.o_rs = p->Lo2;
+        o.batch = nodes;
+        o.accumulate = 0;
+        o.j0 = 0;
+    }
+    return launch_proj_degrees(pv, 2, K_PROJ_OUT, st);
+}
+
 // ------------------------------------------------------------------------------ parity-slot entry points
 size_t cgtp_onsite_parity_workspace_bytes(int lmax, int lmax_out, int N, int C, int64_t batch)
 {

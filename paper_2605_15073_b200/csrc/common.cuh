@@ -225,6 +225,12 @@ int launch_edge_ring(const Plan* p, bool odd, const float* G, const int64_t* row
 int launch_edge_lr(const Plan* p, bool odd, const float* G, const int64_t* row_ptr, const int64_t* edge_index, int64_t E,
                    const float* edge_vec, const float* edge_radial, const int* perm_par, int Cpar, int C, float* S,
                    int64_t nodes, const int32_t* status, cudaStream_t st);
+// Two-field coupling (edge_field.cu; Eq.(28)): block gather Hb[e] = Hn[send[e]] and the pooled sum
+// Tn[i] (+)= sum of T[e - e0] over the edges of receiver i inside [e0, e1); blocks of `blk` contiguous floats.
+int launch_field_gather(const float* Hn, const int64_t* send, float* Hb, int64_t ne, int blk, const int32_t* status,
+                        cudaStream_t st);
+int launch_field_pool(const float* T, const int64_t* row_ptr, float* Tn, int64_t nodes, int64_t e0, int64_t e1, int blk,
+                      const int32_t* status, cudaStream_t st);
 // M5: T[col][Lo2p] = analysis of S[col][UVp] (even) or of the field pair S[col][2][UVp] against {., Y_lm} (odd)
 int launch_analysis(const Plan* p, bool odd, const float* S, float* T, int64_t ncols, cudaStream_t st);
 

@@ -1,0 +1,141 @@
+"""Parity of cgtp_message_field (two feature fields, Eq.(28) :236, Sec. VII C f :471)
+against the FP64 oracle, through the C ABI.  Bar: max|out - ref| / max|ref| <= 1e-5 per sector (FP32); segmentation
+bit-exact (an edge attributed to the wrong receiver fails the value check at O(1))."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import cgtp_oracle as orc
+from paper_2605_15073_b200 import binding as cg
+from paper_2605_15073_b200 import synthetic
+from tests import shref
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5
+
+
+def _cuda(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run_field(m, XE, W_edge, **kw):
+    out = cg.cgtp_message_field(_cuda(m.node_feats), _cuda(m.edge_index), _cuda(XE), _cuda(W_edge), _cuda(m.W_node),
+                                _cuda(m.W_out), m.lmax, m.lmax_out, m.N, W_edge.shape[1], m.C, m.parity_mask, **kw)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def oracle_field(m, XE, W_edge):
+    return orc.message_field(m.node_feats, m.edge_index, XE, W_edge, m.W_node, m.W_out, m.lmax, m.lmax_out, m.parity_mask)
+
+
+def sector_err(got, ref):
+    """max|got - ref| / max|ref| per sector; a sector that vanishes identically in the reference (the curl pairing has
+    no l = 0 component, so the odd sector is zero at lmax_out = 0) is measured against the norm of the whole output."""
+    errs = []
+    whole = np.abs(ref).max()
+    for s in range(2):
+        den = np.abs(ref[:, s]).max()
+        if den == 0.0:
+            den = whole
+        if den > 0:
+            errs.append(np.abs(got[:, s].astype(np.float64) - ref[:, s]).max() / den)
+        else:
+            assert np.abs(got[:, s]).max() == 0.0
+    return max(errs) if errs else 0.0
+
+
+def _ragged(nodes, hi, seed):
+    d = np.random.default_rng(seed).integers(0, hi + 1, size=nodes)
+    d[0] = 0
+    d[-1] = 0
+    return d
+
+
+# several CTAs and a ragged tail of columns; compiled and non-compiled bands (5 -> 6, 7 -> 8); lmax_out != lmax;
+# band 12 takes the generic core; ragged degrees with empty receivers (first and last node included)
+@pytest.mark.parametrize("lmax,lmax_out,N,Ne,C,nodes,degree", [
+    (2, 2, 8, 4, 8, 40, 3), (4, 4, 16, 8, 12, 61, "ragged"), (6, 6, 16, 16, 16, 50, 5), (8, 8, 8, 8, 8, 20, 4),
+    (3, 5, 6, 3, 5, 33, "ragged"), (5, 3, 4, 4, 6, 17, 2), (7, 7, 8, 2, 4, 9, 3), (1, 2, 2, 2, 2, 5, 1),
+    (12, 12, 4, 4, 4, 6, 2), (4, 0, 8, 8, 8, 12, 3),
+])
+def test_field_vs_oracle(lmax, lmax_out, N, Ne, C, nodes, degree):
+    deg = _ragged(nodes, 6, lmax) if degree == "ragged" else degree
+    m = synthetic.make_message(lmax, lmax_out, N, C, nodes, deg, seed=100 * lmax + lmax_out)
+    XE, W_edge = synthetic.make_edge_field(m, Ne, seed=lmax)
+    got = run_field(m, XE, W_edge, check=True)
+    ref = oracle_field(m, XE, W_edge)
+    assert got.shape == ref.shape
+    assert sector_err(got, ref) <= TOL, sector_err(got, ref)
+    assert np.array_equal(got, run_field(m, XE, W_edge))  # bitwise reproducible
+
+
+@pytest.mark.parametrize("mask_kind", ["even", "odd", "mixed"])
+def test_field_masks(mask_kind):
+    lmax, lmax_out, N, Ne, C, nodes = 3, 3, 8, 4, 7, 25
+    mask = {"even": np.zeros(C, np.uint8), "odd": np.ones(C, np.uint8),
+            "mixed": np.array([1, 0, 0, 1, 1, 0, 1], np.uint8)}[mask_kind]
+    m = synthetic.make_message(lmax, lmax_out, N, C, nodes, 4, seed=2, parity_mask=mask)
+    XE, W_edge = synthetic.make_edge_field(m, Ne, seed=2)
+    got = run_field(m, XE, W_edge)
+    ref = oracle_field(m, XE, W_edge)
+    assert sector_err(got, ref) <= TOL
+
+
+def test_field_edge_chunks_straddle_segments():
+    # C = 1024 -> chunks of 4096 edges; degree 7 puts segment boundaries inside chunks and segments across them
+    lmax, lmax_out, N, Ne, C, nodes = 1, 1, 2, 2, 1024, 1300
+    m = synthetic.make_message(lmax, lmax_out, N, C, nodes, 7, seed=4)
+    assert m.E > 2 * 4096 and 4096 % 7 != 0
+    XE, W_edge = synthetic.make_edge_field(m, Ne, seed=4)
+    got = run_field(m, XE, W_edge, check=True)
+    ref = oracle_field(m, XE, W_edge)
+    assert sector_err(got, ref) <= TOL
+
+
+def test_field_no_edges_and_bad_graph():
+    lmax, lmax_out, N, Ne, C, nodes = 2, 2, 4, 4, 4, 6
+    m = synthetic.make_message(lmax, lmax_out, N, C, nodes, 0, seed=1)
+    XE, W_edge = synthetic.make_edge_field(m, Ne, seed=1)
+    assert m.E == 0
+    got = run_field(m, XE, W_edge, check=True)
+    assert got.shape == (nodes, 2, N, 9) and np.abs(got).max() == 0.0
+    m = synthetic.make_message(lmax, lmax_out, N, C, nodes, 2, seed=1)
+    XE, W_edge = synthetic.make_edge_field(m, Ne, seed=1)
+    m.edge_index = m.edge_index[:, ::-1].copy()  # receivers descending
+    with pytest.raises(cg.CgtpError):
+        run_field(m, XE, W_edge, check=True)
+    with pytest.raises(cg.CgtpError):  # workspace too small
+        m2 = synthetic.make_message(lmax, lmax_out, N, C, nodes, 2, seed=1)
+        run_field(m2, XE, W_edge, workspace=torch.empty(512, dtype=torch.uint8, device="cuda"))
+
+
+def test_field_RY_edge_fields_match_cgtp_message():
+    lmax, lmax_out, N, Ne, C, nodes = 4, 4, 16, 8, 16, 64
+    m = synthetic.make_message(lmax, lmax_out, N, C, nodes, 5, seed=7)
+    _, W_edge = synthetic.make_edge_field(m, Ne, seed=7)
+    R = np.random.default_rng(3).standard_normal((m.E, Ne)).astype(np.float32)
+    ev = m.edge_vec.astype(np.float64)
+    Y = shref.real_sh_xyz(lmax, ev / np.linalg.norm(ev, axis=1, keepdims=True))
+    XE = (R[:, :, None] * Y[:, None, :]).astype(np.float32)
+    got = run_field(m, XE, W_edge)
+    er = (R.astype(np.float64) @ W_edge.astype(np.float64).T).astype(np.float32)
+    ref = cg.cgtp_message(_cuda(m.node_feats), _cuda(m.edge_index), _cuda(m.edge_vec), _cuda(er), _cuda(m.W_node),
+                          _cuda(m.W_out), lmax, lmax_out, N, C, m.parity_mask)
+    torch.cuda.synchronize()
+    assert sector_err(got, ref.cpu().numpy().astype(np.float64)) <= 2 * TOL
+
+
+def test_field_rotation_equivariance_on_device():
+    lmax, lmax_out, N, Ne, C, nodes = 4, 4, 8, 8, 8, 30
+    m = synthetic.make_message(lmax, lmax_out, N, C, nodes, 4, seed=9)
+    XE, W_edge = synthetic.make_edge_field(m, Ne, seed=9)
+    base = run_field(m, XE, W_edge).astype(np.float64)
+    D = shref.wigner_D_real(lmax_out, shref.random_rotation(np.random.default_rng(4)))
+    L2 = (lmax + 1) ** 2
+    rot = lambda x: np.einsum("ab,...b->...a", D[:L2, :L2], x.astype(np.float64)).astype(np.float32)
+    m.node_feats = rot(m.node_feats)
+    got = run_field(m, rot(XE), W_edge).astype(np.float64)
+    want = np.einsum("ab,...b->...a", D, base)
+    assert sector_err(got, want) <= TOL
