@@ -12,7 +12,7 @@ product / surface-curl pairing, analysis, output projection) over one batch of B
 Prints ONE JSON line on rank 0.  Extra objects on the line (N=1 only): "sweep" (configs[3], on-site vs
 lmax), "message" (configs[2] and configs[4], edges/s and HBM GB/s), "kernels" (per-kernel shares), "parity"
 (parity-labelled inputs: cost of the full dispatch against one Category-alpha run), "l_dependent_weights", "nbody"
-(nu-body pointwise products).
+(nu-body pointwise products), "edge_field" (two feature fields, Eq.(28)).
 """
 from __future__ import annotations
 
@@ -355,6 +355,7 @@ def main():
         line["parity"] = run_parity(args, cg, synthetic, dev)
         line["l_dependent_weights"] = run_lw(args, cg, synthetic, dev, ms_per_step)
         line["nbody"] = run_nbody(args, cg, synthetic, dev, fp32_peak_tflops)
+        line["edge_field"] = run_edge_field(args, cg, synthetic, dev, fp32_peak_tflops)
     elif world == 1:
         rate, dt_cpu, cores = oracle_onsite_rate(base, 1024)
         line["cpu_baseline"] = {"value": rate, "unit": "contractions/s", "cores": cores, "kind": "oracle",
@@ -630,6 +631,52 @@ def run_nbody(args, cg, synthetic, dev, fp32_peak_tflops):
                     "core_frac_fp32_peak": core * batch / (core_ms * 1e-3) / 1e12 / fp32_peak_tflops,
                     "kernel_ms": kms})
         del Xs, out
+        torch.cuda.empty_cache()
+    return res
+
+
+def run_edge_field(args, cg, synthetic, dev, fp32_peak_tflops):
+    """Two feature fields, Eq.(28) on the graph of BASELINE.json configs[2]
+    with an edge feature field [E, Ne, L^2] in place of R.Y.  Algorithmic flops: per edge the on-site S2-S4 work of all
+    C channels plus the edge projection 2 C Ne L^2; per node 2 C N L^2 (node projection) + 2 N C L_o^2 (output)."""
+    import torch
+    res = []
+    for (lmax, N, Ne, C, nodes, degree) in [(4, 128, 128, 128, 2048, 16), (4, 128, 8, 128, 2048, 16)]:
+        m = synthetic.make_message(lmax, lmax, N, C, nodes, degree, seed=0)
+        XE, W_edge = synthetic.make_edge_field(m, Ne, seed=0)
+        nsets = max(2, int(300e6 // XE.nbytes) + 1)   # rotating edge fields so that no step finds them in L2
+        XEs = [torch.from_numpy(XE).to(dev) for _ in range(nsets)]
+        t = {k: torch.from_numpy(getattr(m, k)).to(dev) for k in ("node_feats", "edge_index", "W_node", "W_out")}
+        W_e = torch.from_numpy(W_edge).to(dev)
+        out = torch.empty((nodes, 2, N, (lmax + 1) ** 2), device=dev)
+        it = [0]
+
+        def fn():
+            it[0] += 1
+            cg.cgtp_message_field(t["node_feats"], t["edge_index"], XEs[it[0] % nsets], W_e, t["W_node"], t["W_out"],
+                                  lmax, lmax, N, Ne, C, m.parity_mask, out=out)
+        ms = time_steps(fn, 20, 3)
+        cg.cgtp_profile_enable(True)
+        for _ in range(10):
+            fn()
+        torch.cuda.synchronize()
+        prof = cg.cgtp_profile_collect()
+        cg.cgtp_profile_enable(False)
+        Ce = int((m.parity_mask == 0).sum())
+        k = onsite_flops_per_atom(lmax, lmax, N, C, Ce, C - Ce)
+        L2 = (lmax + 1) ** 2
+        core = k["onsite_core_even"] + k["onsite_core_odd"]
+        flops = m.E * (core + 2 * C * Ne * L2) + nodes * (2 * C * N * L2 + k["proj_out"])
+        kms = {kk: v[0] / 10 for kk, v in prof.items() if v[1]}
+        core_ms = kms.get("onsite_core_even", 0.0) + kms.get("onsite_core_odd", 0.0)
+        res.append({"workload": f"configs[2] graph ({nodes} nodes, {m.E} edges), lmax=lmax_out={lmax}, N=C={N}, edge field "
+                                f"[E, {Ne}, {L2}] ({XE.nbytes / 1e6:.0f} MB, {nsets} rotating sets), half odd channels",
+                    "ms_per_step": ms, "edges_per_s": m.E / (ms * 1e-3),
+                    "alg_tflops": flops / (ms * 1e-3) / 1e12, "frac_fp32_peak": flops / (ms * 1e-3) / 1e12 / fp32_peak_tflops,
+                    "core_alg_tflops": m.E * core / (core_ms * 1e-3) / 1e12 if core_ms else None,
+                    "core_frac_fp32_peak": m.E * core / (core_ms * 1e-3) / 1e12 / fp32_peak_tflops if core_ms else None,
+                    "kernel_ms": kms, "launches_per_step": int(sum(v[1] for v in prof.values()) // 10)})
+        del XEs, out
         torch.cuda.empty_cache()
     return res
 

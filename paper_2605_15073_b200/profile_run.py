@@ -6,6 +6,7 @@ ncu captures under profiles/ are made with.
     python -m paper_2605_15073_b200.profile_run --config 4 --steps 1            # message passing, configs[4]
     python -m paper_2605_15073_b200.profile_run --config 1 --math-mode 1        # 3xTF32 tensor-core projections
     python -m paper_2605_15073_b200.profile_run --config 1 --nu 3               # nu-body product at the shape of configs[1]
+    python -m paper_2605_15073_b200.profile_run --config 2 --edge-field 128     # two-field coupling on the graph of configs[2]
 """
 from __future__ import annotations
 
@@ -28,6 +29,8 @@ def main():
     ap.add_argument("--math-mode", type=int, default=0, help="0 FP32 (default), 1 3xTF32, 2 TF32 projections")
     ap.add_argument("--nu", type=int, default=0, help="> 0: cgtp_onsite_nbody with this body order at the on-site "
                     "config's lmax, N, C, batch (all rank channels pointwise)")
+    ap.add_argument("--edge-field", type=int, default=0, help="> 0: cgtp_message_field on the graph of a message "
+                    "config with an edge feature field of this many channels (Ne)")
     args = ap.parse_args()
     dev = torch.device("cuda", 0)
     cg.cgtp_set_math_mode(args.math_mode)
@@ -48,6 +51,13 @@ def main():
         Wa, Wb, Wo = cu(inp.W_a), cu(inp.W_b), cu(inp.W_out)
         fn = lambda: cg.cgtp_onsite(A, B, Wa, Wb, Wo, inp.lmax, inp.lmax_out, inp.N, inp.C, inp.parity_mask)
         units, unit = b, "contractions"
+    elif args.edge_field > 0:
+        XE, W_edge = synthetic.make_edge_field(inp, args.edge_field, seed=0)
+        X, ei, XEd, We = cu(inp.node_feats), cu(inp.edge_index), cu(XE), cu(W_edge)
+        Wn, Wo = cu(inp.W_node), cu(inp.W_out)
+        fn = lambda: cg.cgtp_message_field(X, ei, XEd, We, Wn, Wo, inp.lmax, inp.lmax_out, inp.N, args.edge_field, inp.C,
+                                           inp.parity_mask)
+        units, unit = inp.E, "edges"
     else:
         X, ei, ev, er = cu(inp.node_feats), cu(inp.edge_index), cu(inp.edge_vec), cu(inp.edge_radial)
         Wn, Wo = cu(inp.W_node), cu(inp.W_out)
