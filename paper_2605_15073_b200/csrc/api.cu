@@ -839,17 +839,26 @@ int cgtp_message_field(const float* node_feats, const int64_t* edge_index, const
         for (int s = 0; s < 2; ++s) {
             const int64_t nc = ec * Cpar[s];
             if (nc > 0) {
-                const size_t pad = (size_t)round_up64(nc, 32) - (size_t)nc;
-                if (pad) {  // columns that pad the last group of 32: defined, never read back
-                    CGTP_CUDA_CHECK(cudaMemsetAsync(Ha[s] + (size_t)nc * hstr, 0, pad * hstr * 4, st));
-                    CGTP_CUDA_CHECK(cudaMemsetAsync(Hb[s] + (size_t)nc * hstr, 0, pad * hstr * 4, st));
+                // S2-S4 per edge: the edge field is factor 1 (R10), the sender's field factor 2 -- read in place through
+                // the edge list when the core's column groups do not straddle edges, else gathered into Hb first
+                bool handled = false;
+                if (fast) {
+                    rc = launch_onsite_fast_gather(p, s == 1, Ha[s], Hn[s], edge_index + e0, Cpar[s], status, T[s], nc, st,
+                                                   &handled);
+                    if (rc) return rc;
                 }
-                rc = launch_field_gather(Hn[s], edge_index + e0, Hb[s], ec, Cpar[s] * hstr, status, st);
-                if (rc) return rc;
-                // S2-S4 per edge: the edge field is factor 1 (R10), the sender's field factor 2
-                rc = fast ? launch_onsite_fast(p, s == 1, Ha[s], Hb[s], T[s], nc, st)
-                          : launch_onsite_generic(p, s == 1, Ha[s], Hb[s], T[s], nc, st);
-                if (rc) return rc;
+                if (!handled) {
+                    const size_t pad = (size_t)round_up64(nc, 32) - (size_t)nc;
+                    if (pad) {  // columns that pad the last group of 32: defined, never read back
+                        CGTP_CUDA_CHECK(cudaMemsetAsync(Ha[s] + (size_t)nc * hstr, 0, pad * hstr * 4, st));
+                        CGTP_CUDA_CHECK(cudaMemsetAsync(Hb[s] + (size_t)nc * hstr, 0, pad * hstr * 4, st));
+                    }
+                    rc = launch_field_gather(Hn[s], edge_index + e0, Hb[s], ec, Cpar[s] * hstr, status, st);
+                    if (rc) return rc;
+                    rc = fast ? launch_onsite_fast(p, s == 1, Ha[s], Hb[s], T[s], nc, st)
+                              : launch_onsite_generic(p, s == 1, Ha[s], Hb[s], T[s], nc, st);
+                    if (rc) return rc;
+                }
             }
             // sum over the in-edges of every receiver (Eq.(28) sum_j), in edge order
             if (Cpar[s] > 0) {

@@ -192,6 +192,11 @@ inline int onsite_fast_tstride(const Plan* p) { return p->Lo2 | 1; }
 int launch_onsite_fast(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols,
                        cudaStream_t st);
 
+// Same core with factor 2 read through the edge list (two-field coupling, Eq.(28)): column e * cpar + k of
+// Ha pairs with column send[e] * cpar + k of Hn.  *handled = false when the kernel's group width does not divide cpar.
+int launch_onsite_fast_gather(const Plan* p, bool odd, const float* Ha, const float* Hn, const int64_t* send, int cpar,
+                              const int32_t* status, float* T, int64_t ncols, cudaStream_t st, bool* handled);
+
 // nu-body form of S2-S4 (nbody.cu): T[col][Lo2p] = analysis of prod_s synthesis(H[s][col]); H holds nu blocks at
 // distance nbody_hfstride(p, ncols) floats, each [ncols][nbody_hstride(p)] (odd row stride), plus 4 rows of padding at
 // the end; p a plan of get_plan_nu.  CGTP_ERR_UNSUPPORTED above band limit 8 or body order 4.

@@ -265,6 +265,13 @@ struct CoreArgs {
     int dbl;                         // 1: two H buffers (prefetch during the whole group), 0: one
     int off_blob, off_hs, off_f, off_ts;  // byte offsets in dynamic shared memory
     int hs_bytes;                    // bytes of one H buffer (both factors)
+    // Two-field coupling (Eq.(28)): column = edge * cpar + channel and factor 2 of edge e is the block of
+    // sender send[e] in Hb [senders][cpar][L2s]; cpar is a multiple of the group width, so a group never straddles two
+    // edges.  send == nullptr: factor 2 is indexed like factor 1.  status != nullptr: leave when *status != 0 (M0 found
+    // the edge list invalid, so send[] may not be dereferenced).
+    const long long* send;
+    int cpar;
+    const int32_t* status;
 };
 
 // Grid rows are processed in blocks of UB northern nodes u' = e0 .. e0+UB-1 together with their mirror images
@@ -631,8 +638,14 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
         float* dst = reinterpret_cast<float*>(smem + a.off_hs + (size_t)buf * a.hs_bytes);
         mbar_arrive_expect_tx(&bar_h[buf], 2 * hbytes);
         tma_load_span(dst, a.Ha + g * hfl, hbytes, &bar_h[buf]);
-        tma_load_span(dst + hfl, a.Hb + g * hfl, hbytes, &bar_h[buf]);
+        const float* hb = a.Hb + g * hfl;
+        if (a.send) {
+            const long long c0 = g * GW, e = c0 / a.cpar;
+            hb = a.Hb + ((size_t)a.send[e] * a.cpar + (size_t)(c0 - e * a.cpar)) * a.L2s;
+        }
+        tma_load_span(dst + hfl, hb, hbytes, &bar_h[buf]);
     };
+    if (a.status && *a.status != 0) return;
 
     if (threadIdx.x == 0) {
         mbar_init(bar_tab, 1);
@@ -752,7 +765,7 @@ bool onsite_fast_supported(const Plan* p, bool odd)
 
 template <int LB, bool ODD>
 static int launch_fast_t(const Plan* p, const CorePlan* c, const float* Ha, const float* Hb, float* T, int64_t ncols,
-                         cudaStream_t st)
+                         cudaStream_t st, const int64_t* send = nullptr, int cpar = 0, const int32_t* status = nullptr)
 {
     bool dbl = false;
     const size_t smem = core_config(p, ODD, c, &dbl);
@@ -763,6 +776,9 @@ static int launch_fast_t(const Plan* p, const CorePlan* c, const float* Ha, cons
     a.Ha = Ha;
     a.Hb = Hb;
     a.T = T;
+    a.send = reinterpret_cast<const long long*>(send);
+    a.cpar = cpar;
+    a.status = status;
     constexpr int GW = core_gw(LB, ODD);
     a.ngroups = (ncols + GW - 1) / GW;  // the caller pads the column count to a multiple of 32
     a.lmax = p->lmax;
@@ -803,6 +819,31 @@ int launch_onsite_fast(const Plan* p, bool odd, const float* Ha, const float* Hb
     case B:                                                                       \
         return odd ? launch_fast_t<B, true>(p, c, Ha, Hb, T, ncols, st)           \
                    : launch_fast_t<B, false>(p, c, Ha, Hb, T, ncols, st);
+        CGTP_CASE(1) CGTP_CASE(2) CGTP_CASE(3) CGTP_CASE(4) CGTP_CASE(5) CGTP_CASE(6) CGTP_CASE(8) CGTP_CASE(10)
+        CGTP_CASE(12) CGTP_CASE(16) CGTP_CASE(20)
+#undef CGTP_CASE
+    }
+    set_error("onsite fast core: no kernel for band limit %d", p->LB);
+    return CGTP_ERR_UNSUPPORTED;
+}
+
+// Factor 2 gathered through the edge list (two-field coupling): column e * cpar + k pairs Ha's column with the block
+// of sender send[e] in Hn.  *handled = false when the group width does not divide cpar (the caller gathers into a
+// dense Hb and uses launch_onsite_fast).
+int launch_onsite_fast_gather(const Plan* p, bool odd, const float* Ha, const float* Hn, const int64_t* send, int cpar,
+                              const int32_t* status, float* T, int64_t ncols, cudaStream_t st, bool* handled)
+{
+    *handled = false;
+    if (cpar <= 0 || cpar % core_gw(p->LB, odd) != 0) return CGTP_OK;
+    *handled = true;
+    if (ncols <= 0) return CGTP_OK;
+    const CorePlan* c = get_core_plan(p, odd);
+    if (!c) return CGTP_ERR_CUDA;
+    switch (p->LB) {
+#define CGTP_CASE(B)                                                                                   \
+    case B:                                                                                            \
+        return odd ? launch_fast_t<B, true>(p, c, Ha, Hn, T, ncols, st, send, cpar, status)            \
+                   : launch_fast_t<B, false>(p, c, Ha, Hn, T, ncols, st, send, cpar, status);
         CGTP_CASE(1) CGTP_CASE(2) CGTP_CASE(3) CGTP_CASE(4) CGTP_CASE(5) CGTP_CASE(6) CGTP_CASE(8) CGTP_CASE(10)
         CGTP_CASE(12) CGTP_CASE(16) CGTP_CASE(20)
 #undef CGTP_CASE

@@ -59,6 +59,9 @@ def _ragged(nodes, hi, seed):
     (2, 2, 8, 4, 8, 40, 3), (4, 4, 16, 8, 12, 61, "ragged"), (6, 6, 16, 16, 16, 50, 5), (8, 8, 8, 8, 8, 20, 4),
     (3, 5, 6, 3, 5, 33, "ragged"), (5, 3, 4, 4, 6, 17, 2), (7, 7, 8, 2, 4, 9, 3), (1, 2, 2, 2, 2, 5, 1),
     (12, 12, 4, 4, 4, 6, 2), (4, 0, 8, 8, 8, 12, 3),
+    # channel counts per parity that are multiples of the core's column-group width (32, or 16 from band 8 up and for
+    # the odd channels at 6): the sender's field is read in place through the edge list, no gathered copy
+    (4, 4, 16, 8, 64, 37, "ragged"), (8, 8, 8, 4, 32, 11, 3), (6, 6, 8, 8, 64, 13, 4), (2, 3, 8, 8, 64, 29, "ragged"),
 ])
 def test_field_vs_oracle(lmax, lmax_out, N, Ne, C, nodes, degree):
     deg = _ragged(nodes, 6, lmax) if degree == "ragged" else degree
@@ -106,6 +109,13 @@ def test_field_no_edges_and_bad_graph():
     m.edge_index = m.edge_index[:, ::-1].copy()  # receivers descending
     with pytest.raises(cg.CgtpError):
         run_field(m, XE, W_edge, check=True)
+    m = synthetic.make_message(lmax, lmax_out, N, 64, nodes, 2, seed=1)   # in-place sender reads (C/2 = 32)
+    XE, W_edge = synthetic.make_edge_field(m, Ne, seed=1)
+    m.edge_index[0, 3] = nodes + 5                                        # sender out of range
+    with pytest.raises(cg.CgtpError):
+        run_field(m, XE, W_edge, check=True)
+    m = synthetic.make_message(lmax, lmax_out, N, C, nodes, 2, seed=1)
+    XE, W_edge = synthetic.make_edge_field(m, Ne, seed=1)
     with pytest.raises(cg.CgtpError):  # workspace too small
         m2 = synthetic.make_message(lmax, lmax_out, N, C, nodes, 2, seed=1)
         run_field(m2, XE, W_edge, workspace=torch.empty(512, dtype=torch.uint8, device="cuda"))
