@@ -117,6 +117,21 @@ int cgtp_message_field(const float* node_feats, const int64_t* edge_index, const
                        const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* workspace,
                        size_t workspace_bytes, void* cuda_stream);
 
+/* Bipartite form (one shard of a receiver-partitioned graph, as cgtp_message_bipartite): senders index node_feats
+ * [n_send, N, (lmax+1)^2] (all nodes, after the all-gather), receivers are the local rows 0 .. nodes-1 of
+ * out [nodes, 2, N, (lmax_out+1)^2]; edge_index row 0 in [0, n_send), row 1 in [0, nodes), receiver-sorted;
+ * edge_feats [E, Ne, (lmax+1)^2] holds the shard's in-edges.  cgtp_message_field is the case n_send = nodes, and the
+ * shards' outputs are the rows of the single call bit for bit (the per-receiver arithmetic does not depend on the
+ * shard as long as no receiver's edges are split between edge chunks differently, i.e. E <= 2^22 / C per shard
+ * and in the single call; otherwise equal within rounding). */
+size_t cgtp_message_field_bipartite_workspace_bytes(int lmax, int lmax_out, int N, int Ne, int C, int64_t n_send,
+                                                    int64_t nodes, int64_t E);
+
+int cgtp_message_field_bipartite(const float* node_feats, const int64_t* edge_index, const float* edge_feats,
+                                 const float* W_edge, const float* W_node, const float* W_out, int lmax, int lmax_out, int N,
+                                 int Ne, int C, const uint8_t* parity_mask, float* out, int64_t n_send, int64_t nodes,
+                                 int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* ---------------------------------------------------------------------------------------------
  * nu-body on-site product (end of Sec. VI): "The grid pointwise product
  * extends to nu-body features through additional pointwise multiplications on the grid followed by a single

@@ -66,6 +66,10 @@ def lib() -> ctypes.CDLL:
     L.cgtp_message_field_workspace_bytes.argtypes = [i, i, i, i, i, i64, i64]
     L.cgtp_message_field.restype = i
     L.cgtp_message_field.argtypes = [vp, vp, vp, vp, vp, vp, i, i, i, i, i, vp, vp, i64, i64, vp, sz, vp]
+    L.cgtp_message_field_bipartite_workspace_bytes.restype = sz
+    L.cgtp_message_field_bipartite_workspace_bytes.argtypes = [i, i, i, i, i, i64, i64, i64]
+    L.cgtp_message_field_bipartite.restype = i
+    L.cgtp_message_field_bipartite.argtypes = [vp, vp, vp, vp, vp, vp, i, i, i, i, i, vp, vp, i64, i64, i64, vp, sz, vp]
     L.cgtp_onsite_nbody_workspace_bytes.restype = sz
     L.cgtp_onsite_nbody_workspace_bytes.argtypes = [i, i, i, i, i, i64]
     L.cgtp_onsite_nbody.restype = i
@@ -292,6 +296,39 @@ def cgtp_message_field(node_feats, edge_index, edge_feats, W_edge, W_node, W_out
         rc = lib().cgtp_message_field(X.data_ptr(), ei.data_ptr(), XE.data_ptr(), W_edge.data_ptr(), W_node.data_ptr(),
                                       W_out.data_ptr(), lmax, lmax_out, N, Ne, C, mask.ctypes.data, out.data_ptr(),
                                       nodes, E, ws.data_ptr(), ws.numel(), sp)
+        _check(rc)
+        if check:
+            _check(lib().cgtp_message_status(ws.data_ptr(), sp))
+    return out
+
+
+def cgtp_message_field_bipartite(node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C,
+                                 parity_mask, n_recv, out=None, workspace=None, stream=None, check: bool = False):
+    """out[n_recv, 2, N, (lmax_out+1)^2]: cgtp_message_field for one receiver shard -- senders index node_feats
+    [n_send, N, L2] (all nodes), receivers are the local rows 0 .. n_recv-1 (see include/cgtp.h)."""
+    f32 = torch.float32
+    X, XE = _dev(node_feats, f32, "node_feats"), _dev(edge_feats, f32, "edge_feats")
+    ei = _dev(edge_index, torch.int64, "edge_index")
+    W_edge, W_node, W_out = _dev(W_edge, f32, "W_edge"), _dev(W_node, f32, "W_node"), _dev(W_out, f32, "W_out")
+    n_send, E = X.shape[0], ei.shape[1]
+    L2, Lo2 = (lmax + 1) ** 2, (lmax_out + 1) ** 2
+    if tuple(X.shape) != (n_send, N, L2) or tuple(XE.shape) != (E, Ne, L2) or tuple(ei.shape) != (2, E):
+        raise ValueError("node_feats [n_send,N,(lmax+1)^2], edge_feats [E,Ne,(lmax+1)^2], edge_index [2,E] expected")
+    if tuple(W_edge.shape) != (C, Ne) or tuple(W_node.shape) != (C, N) or tuple(W_out.shape) != (N, C):
+        raise ValueError("W_edge must be [C, Ne], W_node [C, N] and W_out [N, C]")
+    mask = _mask(parity_mask, C)
+    if out is None:
+        out = torch.empty((n_recv, 2, N, Lo2), dtype=f32, device=X.device)
+    else:
+        _dev(out, f32, "out")
+    nbytes = lib().cgtp_message_field_bipartite_workspace_bytes(lmax, lmax_out, N, Ne, C, n_send, n_recv, E)
+    ws = _workspace(X.device, nbytes) if workspace is None else workspace
+    sp = _stream_ptr(stream)
+    with torch.cuda.device(X.device):
+        rc = lib().cgtp_message_field_bipartite(X.data_ptr(), ei.data_ptr(), XE.data_ptr(), W_edge.data_ptr(),
+                                                W_node.data_ptr(), W_out.data_ptr(), lmax, lmax_out, N, Ne, C,
+                                                mask.ctypes.data, out.data_ptr(), n_send, n_recv, E, ws.data_ptr(),
+                                                ws.numel(), sp)
         _check(rc)
         if check:
             _check(lib().cgtp_message_status(ws.data_ptr(), sp))

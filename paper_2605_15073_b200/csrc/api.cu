@@ -725,21 +725,28 @@ static int64_t field_chunk(int C, int64_t E)
     return E < cap ? E : cap;
 }
 
-static size_t field_ws_bytes(int lmax, int lmax_out, int C, int64_t nodes, int64_t E)
+static size_t field_ws_bytes(int lmax, int lmax_out, int C, int64_t n_send, int64_t nodes, int64_t E)
 {
     const size_t L2p = round_up((lmax + 1) * (lmax + 1), 4), Lo2p = round_up((lmax_out + 1) * (lmax_out + 1), 4);
     const size_t ec = (size_t)field_chunk(C, E);
     // per chunk: Ha, Hb (two parities, columns padded to groups of 32), T; per node: Hn, Tn; status, row_ptr
-    const size_t fl = (ec * C + 128) * (2 * (L2p + 4) + (Lo2p + 4)) + ((size_t)nodes * C + 128) * ((L2p + 4) + (Lo2p + 4));
+    const size_t fl = (ec * C + 128) * (2 * (L2p + 4) + (Lo2p + 4)) + ((size_t)n_send * C + 128) * (L2p + 4) +
+                      ((size_t)nodes * C + 128) * (Lo2p + 4);
     return 256 + fl * sizeof(float) + (size_t)(nodes + 1) * sizeof(int64_t) + 16 * 256;
+}
+
+size_t cgtp_message_field_bipartite_workspace_bytes(int lmax, int lmax_out, int N, int Ne, int C, int64_t n_send,
+                                                    int64_t nodes, int64_t E)
+{
+    (void)N;
+    (void)Ne;
+    if (lmax < 0 || lmax_out < 0 || C <= 0 || n_send < 0 || nodes < 0 || E < 0) return 0;
+    return field_ws_bytes(lmax, lmax_out, C, n_send, nodes, E);
 }
 
 size_t cgtp_message_field_workspace_bytes(int lmax, int lmax_out, int N, int Ne, int C, int64_t nodes, int64_t E)
 {
-    (void)N;
-    (void)Ne;
-    if (lmax < 0 || lmax_out < 0 || C <= 0 || nodes < 0 || E < 0) return 0;
-    return field_ws_bytes(lmax, lmax_out, C, nodes, E);
+    return cgtp_message_field_bipartite_workspace_bytes(lmax, lmax_out, N, Ne, C, nodes, nodes, E);
 }
 
 int cgtp_message_field(const float* node_feats, const int64_t* edge_index, const float* edge_feats, const float* W_edge,
@@ -747,13 +754,23 @@ int cgtp_message_field(const float* node_feats, const int64_t* edge_index, const
                        const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* workspace,
                        size_t workspace_bytes, void* cuda_stream)
 {
+    return cgtp_message_field_bipartite(node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C,
+                                        parity_mask, out, nodes, nodes, E, workspace, workspace_bytes, cuda_stream);
+}
+
+int cgtp_message_field_bipartite(const float* node_feats, const int64_t* edge_index, const float* edge_feats,
+                                 const float* W_edge, const float* W_node, const float* W_out, int lmax, int lmax_out, int N,
+                                 int Ne, int C, const uint8_t* parity_mask, float* out, int64_t n_send, int64_t nodes,
+                                 int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
     clear_error();
     int rc = check_common(lmax, lmax_out, N, C, parity_mask);
     if (rc) return rc;
     if (Ne <= 0) { set_error("Ne must be positive (Ne=%d)", Ne); return CGTP_ERR_INVALID; }
-    if (nodes < 0 || E < 0) { set_error("negative size"); return CGTP_ERR_INVALID; }
+    if (nodes < 0 || n_send < 0 || E < 0) { set_error("negative size"); return CGTP_ERR_INVALID; }
     if (nodes == 0) return CGTP_OK;
-    if (!node_feats || !W_edge || !W_node || !W_out || !out || !workspace || (E > 0 && (!edge_index || !edge_feats))) {
+    if (n_send == 0 && E > 0) { set_error("edges without sender nodes"); return CGTP_ERR_INVALID; }
+    if ((!node_feats && n_send > 0) || !W_edge || !W_node || !W_out || !out || !workspace || (E > 0 && (!edge_index || !edge_feats))) {
         set_error("null pointer argument");
         return CGTP_ERR_INVALID;
     }
@@ -762,8 +779,8 @@ int cgtp_message_field(const float* node_feats, const int64_t* edge_index, const
         set_error("misaligned pointer (tensors need 16-byte, workspace 256-byte alignment)");
         return CGTP_ERR_INVALID;
     }
-    if (workspace_bytes < field_ws_bytes(lmax, lmax_out, C, nodes, E)) {
-        set_error("workspace too small: %zu < %zu bytes", workspace_bytes, field_ws_bytes(lmax, lmax_out, C, nodes, E));
+    if (workspace_bytes < field_ws_bytes(lmax, lmax_out, C, n_send, nodes, E)) {
+        set_error("workspace too small: %zu < %zu bytes", workspace_bytes, field_ws_bytes(lmax, lmax_out, C, n_send, nodes, E));
         return CGTP_ERR_INVALID;
     }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -784,7 +801,7 @@ int cgtp_message_field(const float* node_feats, const int64_t* edge_index, const
     size_t ncol[2];
     for (int s = 0; s < 2; ++s) {
         ncol[s] = (size_t)round_up64(ec_max * Cpar[s], 32);
-        Hn[s] = cv.take<float>((size_t)nodes * Cpar[s] * hstr);
+        Hn[s] = cv.take<float>((size_t)n_send * Cpar[s] * hstr);
         Tn[s] = cv.take<float>((size_t)nodes * Cpar[s] * tstr);
         Ha[s] = cv.take<float>(ncol[s] * hstr);
         Hb[s] = cv.take<float>(ncol[s] * hstr);
@@ -792,7 +809,7 @@ int cgtp_message_field(const float* node_feats, const int64_t* edge_index, const
     }
 
     // M0
-    rc = launch_segments(edge_index, E, nodes, nodes, row_ptr, status, st);
+    rc = launch_segments(edge_index, E, nodes, n_send, row_ptr, status, st);
     if (rc) return rc;
 
     // factor 2: Hn = W_node . node_feats, once per node (Eq.(47) :398)
@@ -814,11 +831,13 @@ int cgtp_message_field(const float* node_feats, const int64_t* edge_index, const
     a.o_bs1 = (int64_t)Cpar[1] * hstr;
     a.m_split = Cpar[0];
     a.o_rs = hstr;
-    a.batch = nodes;
+    a.batch = n_send;
     a.accumulate = 0;
     a.j0 = 0;
-    rc = launch_proj(&a, 1, K_PROJ_IN, st);
-    if (rc) return rc;
+    if (n_send > 0) {
+        rc = launch_proj(&a, 1, K_PROJ_IN, st);
+        if (rc) return rc;
+    }
 
     for (int64_t e0 = 0; e0 == 0 || e0 < E; e0 += ec_max) {
         const int64_t ec = E - e0 < ec_max ? E - e0 : ec_max;

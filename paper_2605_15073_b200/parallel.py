@@ -127,3 +127,40 @@ def message_sharded(shard: MessageShard, bounds: Sequence[int], W_node: torch.Te
     feats = all_gather_node_feats(shard.node_feats, bounds, group)
     return compute(feats, shard.edge_index, shard.edge_vec, shard.edge_radial, W_node, W_out, lmax, lmax_out, N, C,
                    parity_mask, shard.hi - shard.lo)
+
+
+# ------------------------------------------------------------------ two feature fields, Eq.(28)
+@dataclass
+class FieldShard:
+    """One rank's part of the two-field coupling: its receiver range, its in-edges with their edge feature field
+    (global sender ids, receivers rebased) and the features of its own nodes."""
+    lo: int
+    hi: int
+    edge_index: torch.Tensor   # int64 [2, E_local]
+    edge_feats: torch.Tensor   # [E_local, Ne, (lmax+1)^2]
+    node_feats: torch.Tensor   # [hi - lo, N, (lmax+1)^2]
+
+
+def make_field_shard(node_feats: torch.Tensor, edge_index: torch.Tensor, edge_feats: torch.Tensor,
+                     bounds: Sequence[int], rank: int) -> FieldShard:
+    nodes = node_feats.shape[0]
+    rp = row_ptr_from_receivers(edge_index[1].cpu().numpy(), nodes)
+    lo, hi = int(bounds[rank]), int(bounds[rank + 1])
+    e0, e1 = local_edge_slice(rp, lo, hi)
+    ei = edge_index[:, e0:e1].clone()
+    ei[1] -= lo
+    return FieldShard(lo, hi, ei.contiguous(), edge_feats[e0:e1].contiguous(), node_feats[lo:hi].contiguous())
+
+
+def message_field_sharded(shard: FieldShard, bounds: Sequence[int], W_edge: torch.Tensor, W_node: torch.Tensor,
+                          W_out: torch.Tensor, lmax: int, lmax_out: int, N: int, Ne: int, C: int, parity_mask, group=None,
+                          compute: Optional[Callable] = None) -> torch.Tensor:
+    """out rows [lo, hi) of the two-field coupling on this rank: the edge feature field is local to the receiver's rank,
+    so the one exchange step is again the all-gather of the node features.  `compute(node_feats_all, edge_index,
+    edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C, parity_mask, n_recv)` defaults to the CUDA path."""
+    if compute is None:
+        from . import binding
+        compute = binding.cgtp_message_field_bipartite
+    feats = all_gather_node_feats(shard.node_feats, bounds, group)
+    return compute(feats, shard.edge_index, shard.edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C, parity_mask,
+                   shard.hi - shard.lo)

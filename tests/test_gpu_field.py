@@ -149,3 +149,41 @@ def test_field_rotation_equivariance_on_device():
     got = run_field(m, rot(XE), W_edge).astype(np.float64)
     want = np.einsum("ab,...b->...a", D, base)
     assert sector_err(got, want) <= TOL
+
+
+def test_field_full_size_bench_configuration_sampled_receivers():
+    """The workload bench.py times (`edge_field`: graph of BASELINE.json configs[2], N = C = Ne = 128, lmax 4, half odd
+    channels, in-place sender reads): sampled receivers (first, last, strided, seeded-random) against the oracle, which
+    evaluates the same edge list restricted to those receivers; exchange-free invariant on the full output: the odd
+    sector has no l = 0 component."""
+    lmax, N, Ne, C, nodes, degree = 4, 128, 128, 128, 2048, 16
+    m = synthetic.make_message(lmax, lmax, N, C, nodes, degree, seed=0)
+    XE, W_edge = synthetic.make_edge_field(m, Ne, seed=0)
+    got = run_field(m, XE, W_edge, check=True)
+    rng = np.random.default_rng(0)
+    recv = np.unique(np.concatenate([[0, nodes - 1], np.arange(0, nodes, 257), rng.integers(0, nodes, 6)]))
+    keep = np.isin(m.edge_index[1], recv)
+    ref = orc.message_field(m.node_feats, m.edge_index[:, keep], XE[keep], W_edge, m.W_node, m.W_out, lmax, lmax,
+                            m.parity_mask)
+    assert sector_err(got[recv], ref[recv]) <= TOL, sector_err(got[recv], ref[recv])
+    assert np.abs(got[:, 1, :, 0]).max() <= TOL * np.abs(got[:, 1]).max()
+
+
+def test_field_bipartite_shards_reproduce_the_full_call():
+    from paper_2605_15073_b200 import parallel
+    lmax, lmax_out, N, Ne, C, nodes = 4, 4, 8, 8, 64, 50
+    m = synthetic.make_message(lmax, lmax_out, N, C, nodes, _ragged(nodes, 7, 3), seed=12)
+    XE, W_edge = synthetic.make_edge_field(m, Ne, seed=12)
+    full = run_field(m, XE, W_edge)
+    rp = parallel.row_ptr_from_receivers(m.edge_index[1], nodes)
+    bounds = parallel.shard_receivers(rp, 3)
+    rows = []
+    for r in range(3):
+        sh = parallel.make_field_shard(torch.from_numpy(m.node_feats), torch.from_numpy(m.edge_index), torch.from_numpy(XE),
+                                       bounds, r)
+        out = cg.cgtp_message_field_bipartite(_cuda(m.node_feats), sh.edge_index.cuda(), sh.edge_feats.cuda(), _cuda(W_edge),
+                                              _cuda(m.W_node), _cuda(m.W_out), lmax, lmax_out, N, Ne, C, m.parity_mask,
+                                              sh.hi - sh.lo, check=True)
+        torch.cuda.synchronize()
+        rows.append(out.cpu().numpy())
+    assert np.array_equal(np.concatenate(rows), full)  # bit-identical rows

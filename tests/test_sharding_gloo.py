@@ -59,6 +59,44 @@ def _worker(rank: int, world: int, port: int, result_dir: str):
         dist.destroy_process_group()
 
 
+def _field_oracle_compute(feats, ei, xe, We, Wn, Wo, lmax, lmax_out, N, Ne, C, mask, n_recv):
+    # receivers are local rows 0 .. n_recv-1 of a graph whose senders index all nodes: evaluate on the sender count
+    out = orc.message_field(feats.numpy(), ei.numpy(), xe.numpy(), We.numpy(), Wn.numpy(), Wo.numpy(), lmax, lmax_out, mask)
+    return torch.from_numpy(out[:n_recv])
+
+
+def _field_worker(rank: int, world: int, port: int, result_dir: str):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        m = _problem()
+        XE, W_edge = synthetic.make_edge_field(m, 2, seed=5)
+        t = torch.from_numpy
+        rp = parallel.row_ptr_from_receivers(m.edge_index[1], m.nodes)
+        bounds = parallel.shard_receivers(rp, world)
+        shard = parallel.make_field_shard(t(m.node_feats), t(m.edge_index), t(XE), bounds, rank)
+        assert shard.edge_feats.shape[0] == shard.edge_index.shape[1]
+        out = parallel.message_field_sharded(shard, bounds, t(W_edge), t(m.W_node), t(m.W_out), m.lmax, m.lmax_out, m.N, 2,
+                                             m.C, m.parity_mask, compute=_field_oracle_compute)
+        np.save(os.path.join(result_dir, f"fout{rank}.npy"), out.numpy())
+        dist.barrier()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.timeout(300)
+def test_message_field_sharded_world2_matches_unsharded(tmp_path):
+    world = 2
+    mp.spawn(_field_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    m = _problem()
+    XE, W_edge = synthetic.make_edge_field(m, 2, seed=5)
+    ref = orc.message_field(m.node_feats, m.edge_index, XE, W_edge, m.W_node, m.W_out, m.lmax, m.lmax_out, m.parity_mask)
+    got = np.concatenate([np.load(tmp_path / f"fout{r}.npy") for r in range(world)])
+    assert got.shape == ref.shape
+    assert np.array_equal(got, ref)
+
+
 @pytest.mark.timeout(300)
 def test_message_sharded_world2_matches_unsharded(tmp_path):
     world = 2
