@@ -669,13 +669,31 @@ def run_edge_field(args, cg, synthetic, dev, fp32_peak_tflops):
         flops = m.E * (core + 2 * C * Ne * L2) + nodes * (2 * C * N * L2 + k["proj_out"])
         kms = {kk: v[0] / 10 for kk, v in prof.items() if v[1]}
         core_ms = kms.get("onsite_core_even", 0.0) + kms.get("onsite_core_odd", 0.0)
+        # projections on tcgen05 tensor cores (3xTF32), reported beside the FP32 path, never instead of it (the rotating
+        # edge-field sets hold the same values, so any two calls are comparable)
+        tc = None
+        try:
+            cg.cgtp_set_math_mode(cg.MATH_3XTF32)
+            tc_ms = time_steps(fn, 10, 3)
+            torch.cuda.synchronize()
+            got_tc = out.clone()
+            cg.cgtp_set_math_mode(cg.MATH_FP32)
+            fn()
+            torch.cuda.synchronize()
+            tc = {"ms_per_step": tc_ms, "edges_per_s": m.E / (tc_ms * 1e-3),
+                  "max_rel_diff_vs_fp32_path": [float((got_tc[:, s_] - out[:, s_]).abs().max() / out[:, s_].abs().max())
+                                                for s_ in (0, 1)]}
+            del got_tc
+        finally:
+            cg.cgtp_set_math_mode(cg.MATH_FP32)
         res.append({"workload": f"configs[2] graph ({nodes} nodes, {m.E} edges), lmax=lmax_out={lmax}, N=C={N}, edge field "
                                 f"[E, {Ne}, {L2}] ({XE.nbytes / 1e6:.0f} MB, {nsets} rotating sets), half odd channels",
                     "ms_per_step": ms, "edges_per_s": m.E / (ms * 1e-3),
                     "alg_tflops": flops / (ms * 1e-3) / 1e12, "frac_fp32_peak": flops / (ms * 1e-3) / 1e12 / fp32_peak_tflops,
                     "core_alg_tflops": m.E * core / (core_ms * 1e-3) / 1e12 if core_ms else None,
                     "core_frac_fp32_peak": m.E * core / (core_ms * 1e-3) / 1e12 / fp32_peak_tflops if core_ms else None,
-                    "kernel_ms": kms, "launches_per_step": int(sum(v[1] for v in prof.values()) // 10)})
+                    "kernel_ms": kms, "launches_per_step": int(sum(v[1] for v in prof.values()) // 10),
+                    "projections_3xtf32": tc})
         del XEs, out
         torch.cuda.empty_cache()
     return res
