@@ -41,7 +41,8 @@
  * reduction to oracle_onsite at nu = 2, factor permutation and rotation (tests/test_oracle_nbody.py); the
  * two-field function (oracle_message_field, Eq.(28)) against oracle_message for edge fields of the form R.Y,
  * fine-grid quadrature of the pooled pointwise product, one-edge receivers = oracle_onsite, edge order inside a
- * segment and rotation (tests/test_oracle_field.py).
+ * segment and rotation, and its l-dependent-weight form (oracle_message_field_lw) against it (equal weights, degree
+ * selection, per-degree numpy projections around it) (tests/test_oracle_field.py).
  * No function here is "parity unpinned".
  *
  * Plain C99 + OpenMP, double precision (long double inside the Racah sum).
@@ -916,9 +917,13 @@ int oracle_onsite_nbody(const double *X, const double *W_in, const double *W_out
 /* Layouts: node_feats [nodes,N,L2]; edge_feats [E,Ne,L2]; W_edge [C,Ne]; W_node [C,N];           */
 /* W_out [N,C]; out [nodes,2,N,Lo2].                                                              */
 /* ------------------------------------------------------------------------------------------ */
-int oracle_message_field(const double *node_feats, const int64_t *edge_index /* [2,E] */, const double *edge_feats,
-                         const double *W_edge, const double *W_node, const double *W_out, int lmax, int lmax_out,
-                         int N, int Ne, int C, const uint8_t *parity_mask, double *out, int64_t nodes, int64_t E)
+/* lw = 1: l-dependent weights (the paper's own parameterisation, Eq.(35) :322, (41) :346, (47) :398, (55) :427):  */
+/* W_edge [lmax+1,C,Ne], W_node [lmax+1,C,N] act on the coefficients of their degree l, W_out [lmax_out+1,N,C] on   */
+/* the output coefficients of its degree.                                                                          */
+static int message_field_impl(const double *node_feats, const int64_t *edge_index /* [2,E] */, const double *edge_feats,
+                              const double *W_edge, const double *W_node, const double *W_out, int lmax, int lmax_out,
+                              int N, int Ne, int C, const uint8_t *parity_mask, double *out, int64_t nodes, int64_t E,
+                              int lw)
 {
     int L2 = (lmax + 1) * (lmax + 1), Lo2 = (lmax_out + 1) * (lmax_out + 1);
     const coupling_t *tab[2];
@@ -942,9 +947,11 @@ int oracle_message_field(const double *node_feats, const int64_t *edge_index /* 
                 const double *xj = node_feats + snd[e] * (int64_t)N * L2;
                 for (int c = 0; c < C; ++c)
                     for (int q = 0; q < L2; ++q) {
+                        const int l = lw ? isqrt_floor(q) : 0;
+                        const double *We = W_edge + (size_t)l * C * Ne, *Wn = W_node + (size_t)l * C * N;
                         double sa = 0.0, sh = 0.0;
-                        for (int n = 0; n < Ne; ++n) sa += W_edge[c * Ne + n] * xe[n * L2 + q];
-                        for (int n = 0; n < N; ++n) sh += W_node[c * N + n] * xj[n * L2 + q];
+                        for (int n = 0; n < Ne; ++n) sa += We[c * Ne + n] * xe[n * L2 + q];
+                        for (int n = 0; n < N; ++n) sh += Wn[c * N + n] * xj[n * L2 + q];
                         a[c * L2 + q] = sa;
                         h[c * L2 + q] = sh;
                     }
@@ -960,9 +967,10 @@ int oracle_message_field(const double *node_feats, const int64_t *edge_index /* 
             for (int s = 0; s < 2; ++s)
                 for (int n = 0; n < N; ++n)
                     for (int q = 0; q < Lo2; ++q) {
+                        const double *Wo = W_out + (size_t)(lw ? isqrt_floor(q) : 0) * N * C;
                         double acc = 0.0;
                         for (int c = 0; c < C; ++c)
-                            if ((parity_mask[c] ? 1 : 0) == s) acc += W_out[n * C + c] * T[(size_t)c * Lo2 + q];
+                            if ((parity_mask[c] ? 1 : 0) == s) acc += Wo[n * C + c] * T[(size_t)c * Lo2 + q];
                         ob[((size_t)s * N + n) * Lo2 + q] = acc;
                     }
         }
@@ -970,6 +978,22 @@ int oracle_message_field(const double *node_feats, const int64_t *edge_index /* 
     }
     free(row_ptr);
     return 0;
+}
+
+int oracle_message_field(const double *node_feats, const int64_t *edge_index, const double *edge_feats,
+                         const double *W_edge, const double *W_node, const double *W_out, int lmax, int lmax_out,
+                         int N, int Ne, int C, const uint8_t *parity_mask, double *out, int64_t nodes, int64_t E)
+{
+    return message_field_impl(node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C,
+                              parity_mask, out, nodes, E, 0);
+}
+
+int oracle_message_field_lw(const double *node_feats, const int64_t *edge_index, const double *edge_feats,
+                            const double *W_edge, const double *W_node, const double *W_out, int lmax, int lmax_out,
+                            int N, int Ne, int C, const uint8_t *parity_mask, double *out, int64_t nodes, int64_t E)
+{
+    return message_field_impl(node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C,
+                              parity_mask, out, nodes, E, 1);
 }
 
 int oracle_num_threads(void)

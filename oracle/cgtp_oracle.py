@@ -74,6 +74,8 @@ def _load():
     lib.oracle_onsite_nbody.argtypes = [p, p, p, i, i, i, i, i, p, i64]
     lib.oracle_message_field.restype = i
     lib.oracle_message_field.argtypes = [p, p, p, p, p, p, i, i, i, i, i, p, p, i64, i64]
+    lib.oracle_message_field_lw.restype = i
+    lib.oracle_message_field_lw.argtypes = lib.oracle_message_field.argtypes
     lib.oracle_num_threads.restype = i
     lib.oracle_num_threads.argtypes = []
     _lib = lib
@@ -320,6 +322,25 @@ def message_field(node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lma
                                       lmax_out, N, Ne, C, _ptr(mask), _ptr(out), nodes, E)
     if rc:
         raise RuntimeError(f"oracle_message_field failed with code {rc}")
+    return out
+
+
+def message_field_lw(node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out, parity_mask) -> np.ndarray:
+    """Two-field coupling with l-dependent weights: W_edge [lmax+1,C,Ne], W_node [lmax+1,C,N], W_out [lmax_out+1,N,C]."""
+    X, XE, W_edge, W_node, W_out = map(_f64, (node_feats, edge_feats, W_edge, W_node, W_out))
+    ei = np.ascontiguousarray(np.asarray(edge_index), dtype=np.int64)
+    nodes, N, L2 = X.shape
+    E, Ne, _ = XE.shape
+    C = W_node.shape[1]
+    assert L2 == (lmax + 1) ** 2 and XE.shape == (E, Ne, L2) and ei.shape == (2, E)
+    assert W_edge.shape == (lmax + 1, C, Ne) and W_node.shape == (lmax + 1, C, N) and W_out.shape == (lmax_out + 1, N, C)
+    mask = np.ascontiguousarray(np.asarray(parity_mask), dtype=np.uint8)
+    assert mask.shape == (C,)
+    out = np.zeros((nodes, 2, N, (lmax_out + 1) ** 2), np.float64)
+    rc = _load().oracle_message_field_lw(_ptr(X), _ptr(ei), _ptr(XE), _ptr(W_edge), _ptr(W_node), _ptr(W_out), lmax,
+                                         lmax_out, N, Ne, C, _ptr(mask), _ptr(out), nodes, E)
+    if rc:
+        raise RuntimeError(f"oracle_message_field_lw failed with code {rc}")
     return out
 
 

@@ -97,3 +97,54 @@ def test_field_equivariance_and_inversion():
     got = _run(m, XE * sgn_in, W_edge, node_feats=m.node_feats * sgn_in)
     assert np.abs(got[:, 0] - base[:, 0] * sgn_out).max() < 1e-13 * np.abs(base).max()
     assert np.abs(got[:, 1] + base[:, 1] * sgn_out).max() < 1e-13 * np.abs(base).max()
+
+
+# ------------------------------------------------------------------ l-dependent weights on the two-field coupling
+def _lof(lmax):
+    return np.concatenate([np.full(2 * l + 1, l) for l in range(lmax + 1)])
+
+
+def test_field_lw_reduces_and_selects_degrees():
+    lmax, lo = 3, 4
+    m, XE, W_edge = _case(lmax, lo, N=3, Ne=2, C=4, nodes=5, degree=3, seed=21)
+    base = _run(m, XE, W_edge)
+    rep = lambda W, n: np.repeat(W[None].astype(np.float64), n, axis=0)
+    run_lw = lambda We, Wn, Wo, xe=XE, x=m.node_feats: orc.message_field_lw(x, m.edge_index, xe, We, Wn, Wo, lmax, lo, m.parity_mask)
+    assert np.array_equal(run_lw(rep(W_edge, lmax + 1), rep(m.W_node, lmax + 1), rep(m.W_out, lo + 1)), base)
+    lv, lvo = _lof(lmax), _lof(lo)
+    for l0 in range(lmax + 1):
+        We = np.zeros((lmax + 1,) + W_edge.shape)
+        We[l0] = W_edge
+        got = run_lw(We, rep(m.W_node, lmax + 1), rep(m.W_out, lo + 1))
+        ref = _run(m, XE * (lv == l0), W_edge)
+        assert np.abs(got - ref).max() < 1e-13 and np.abs(ref).max() > 1e-3
+        Wn = np.zeros((lmax + 1,) + m.W_node.shape)
+        Wn[l0] = m.W_node
+        got = run_lw(rep(W_edge, lmax + 1), Wn, rep(m.W_out, lo + 1))
+        ref = _run(m, XE, W_edge, node_feats=m.node_feats * (lv == l0))
+        assert np.abs(got - ref).max() < 1e-13 and np.abs(ref).max() > 1e-3
+    for l0 in range(lo + 1):
+        Wo = np.zeros((lo + 1,) + m.W_out.shape)
+        Wo[l0] = m.W_out
+        got = run_lw(rep(W_edge, lmax + 1), rep(m.W_node, lmax + 1), Wo)
+        assert np.abs(got - base * (lvo == l0)).max() < 1e-13
+
+
+def test_field_lw_vs_numpy_projections_around_the_shared_oracle():
+    lmax, N, Ne, C = 3, 3, 2, 4
+    m, XE, _ = _case(lmax, lmax, N=N, Ne=Ne, C=C, nodes=6, degree=np.array([2, 0, 3, 1, 4, 2]), seed=23)
+    (Wn,), Wo = synthetic.lw_weights(lmax, lmax, N, C, seed=23, n_in=1)
+    (We,), _ = synthetic.lw_weights(lmax, lmax, Ne, C, seed=29, n_in=1)
+    got = orc.message_field_lw(m.node_feats, m.edge_index, XE, We, Wn, Wo, lmax, lmax, m.parity_mask)
+    lv = _lof(lmax)
+    a = np.einsum("qcn,enq->ecq", We[lv].astype(float), XE.astype(float))
+    H = np.einsum("qcn,jnq->jcq", Wn[lv].astype(float), m.node_feats.astype(float))
+    eye = np.eye(C)
+    T = orc.message_field(H, m.edge_index, a, eye, eye, eye, lmax, lmax, m.parity_mask)  # [i, s, c, lm]
+    ref = np.einsum("qnc,iscq->isnq", Wo[lv].astype(float), T)
+    assert np.abs(got - ref).max() < 1e-12 and np.abs(ref).max() > 1e-2
+    R = shref.random_rotation(np.random.default_rng(6))
+    D = shref.wigner_D_real(lmax, R)
+    rot = lambda x: np.einsum("ab,...b->...a", D, x.astype(float))
+    got_r = orc.message_field_lw(rot(m.node_feats), m.edge_index, rot(XE), We, Wn, Wo, lmax, lmax, m.parity_mask)
+    assert np.abs(got_r - rot(got)).max() < 1e-11
