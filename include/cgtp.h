@@ -117,6 +117,16 @@ int cgtp_message_field(const float* node_feats, const int64_t* edge_index, const
                        const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* workspace,
                        size_t workspace_bytes, void* cuda_stream);
 
+/* The same coupling in the paper's own parameterisation, l-dependent CP weights (c_{cnl} of Eq.(35) :322 / Eq.(47) :398 on
+ * both fields, lambda_c^{(nl)} of Eq.(41) :346 / Eq.(55) :427 on the output), as cgtp_message_lw:
+ * W_edge device [lmax+1, C, Ne], W_node device [lmax+1, C, N], W_out device [lmax_out+1, N, C]; the matrix of degree l
+ * acts on the coefficients l^2 .. l^2 + 2l.  Workspace: cgtp_message_field_workspace_bytes.  Everything else as
+ * cgtp_message_field. */
+int cgtp_message_field_lw(const float* node_feats, const int64_t* edge_index, const float* edge_feats, const float* W_edge,
+                          const float* W_node, const float* W_out, int lmax, int lmax_out, int N, int Ne, int C,
+                          const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* workspace,
+                          size_t workspace_bytes, void* cuda_stream);
+
 /* Bipartite form (one shard of a receiver-partitioned graph, as cgtp_message_bipartite): senders index node_feats
  * [n_send, N, (lmax+1)^2] (all nodes, after the all-gather), receivers are the local rows 0 .. nodes-1 of
  * out [nodes, 2, N, (lmax_out+1)^2]; edge_index row 0 in [0, n_send), row 1 in [0, nodes), receiver-sorted;

@@ -66,6 +66,8 @@ def lib() -> ctypes.CDLL:
     L.cgtp_message_field_workspace_bytes.argtypes = [i, i, i, i, i, i64, i64]
     L.cgtp_message_field.restype = i
     L.cgtp_message_field.argtypes = [vp, vp, vp, vp, vp, vp, i, i, i, i, i, vp, vp, i64, i64, vp, sz, vp]
+    L.cgtp_message_field_lw.restype = i
+    L.cgtp_message_field_lw.argtypes = L.cgtp_message_field.argtypes
     L.cgtp_message_field_bipartite_workspace_bytes.restype = sz
     L.cgtp_message_field_bipartite_workspace_bytes.argtypes = [i, i, i, i, i, i64, i64, i64]
     L.cgtp_message_field_bipartite.restype = i
@@ -270,8 +272,15 @@ def cgtp_message_field_workspace_bytes(lmax, lmax_out, N, Ne, C, nodes, E) -> in
     return lib().cgtp_message_field_workspace_bytes(lmax, lmax_out, N, Ne, C, nodes, E)
 
 
+def cgtp_message_field_lw(node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C,
+                          parity_mask, out=None, workspace=None, stream=None, check: bool = False):
+    """cgtp_message_field with l-dependent weights W_edge [lmax+1,C,Ne], W_node [lmax+1,C,N], W_out [lmax_out+1,N,C]."""
+    return cgtp_message_field(node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C,
+                              parity_mask, out=out, workspace=workspace, stream=stream, check=check, _lw=True)
+
+
 def cgtp_message_field(node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C,
-                       parity_mask, out=None, workspace=None, stream=None, check: bool = False):
+                       parity_mask, out=None, workspace=None, stream=None, check: bool = False, _lw: bool = False):
     """out[nodes, 2, N, (lmax_out+1)^2] = two-field coupling Eq.(28) (edge feature field x sender feature; see
     include/cgtp.h).  check=True synchronises and raises CgtpError(ERR_GRAPH) for an invalid edge list."""
     f32 = torch.float32
@@ -282,8 +291,10 @@ def cgtp_message_field(node_feats, edge_index, edge_feats, W_edge, W_node, W_out
     L2, Lo2 = (lmax + 1) ** 2, (lmax_out + 1) ** 2
     if tuple(X.shape) != (nodes, N, L2) or tuple(XE.shape) != (E, Ne, L2) or tuple(ei.shape) != (2, E):
         raise ValueError("node_feats [nodes,N,(lmax+1)^2], edge_feats [E,Ne,(lmax+1)^2], edge_index [2,E] expected")
-    if tuple(W_edge.shape) != (C, Ne) or tuple(W_node.shape) != (C, N) or tuple(W_out.shape) != (N, C):
-        raise ValueError("W_edge must be [C, Ne], W_node [C, N] and W_out [N, C]")
+    pre_in, pre_out = ((lmax + 1,), (lmax_out + 1,)) if _lw else ((), ())
+    if (tuple(W_edge.shape) != pre_in + (C, Ne) or tuple(W_node.shape) != pre_in + (C, N)
+            or tuple(W_out.shape) != pre_out + (N, C)):
+        raise ValueError("W_edge must be [C, Ne], W_node [C, N] and W_out [N, C] (with a leading degree axis for _lw)")
     mask = _mask(parity_mask, C)
     if out is None:
         out = torch.empty((nodes, 2, N, Lo2), dtype=f32, device=X.device)
@@ -293,7 +304,8 @@ def cgtp_message_field(node_feats, edge_index, edge_feats, W_edge, W_node, W_out
     ws = _workspace(X.device, nbytes) if workspace is None else workspace
     sp = _stream_ptr(stream)
     with torch.cuda.device(X.device):
-        rc = lib().cgtp_message_field(X.data_ptr(), ei.data_ptr(), XE.data_ptr(), W_edge.data_ptr(), W_node.data_ptr(),
+        entry = lib().cgtp_message_field_lw if _lw else lib().cgtp_message_field
+        rc = entry(X.data_ptr(), ei.data_ptr(), XE.data_ptr(), W_edge.data_ptr(), W_node.data_ptr(),
                                       W_out.data_ptr(), lmax, lmax_out, N, Ne, C, mask.ctypes.data, out.data_ptr(),
                                       nodes, E, ws.data_ptr(), ws.numel(), sp)
         _check(rc)

@@ -749,19 +749,12 @@ size_t cgtp_message_field_workspace_bytes(int lmax, int lmax_out, int N, int Ne,
     return cgtp_message_field_bipartite_workspace_bytes(lmax, lmax_out, N, Ne, C, nodes, nodes, E);
 }
 
-int cgtp_message_field(const float* node_feats, const int64_t* edge_index, const float* edge_feats, const float* W_edge,
-                       const float* W_node, const float* W_out, int lmax, int lmax_out, int N, int Ne, int C,
-                       const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* workspace,
-                       size_t workspace_bytes, void* cuda_stream)
-{
-    return cgtp_message_field_bipartite(node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C,
-                                        parity_mask, out, nodes, nodes, E, workspace, workspace_bytes, cuda_stream);
-}
-
-int cgtp_message_field_bipartite(const float* node_feats, const int64_t* edge_index, const float* edge_feats,
-                                 const float* W_edge, const float* W_node, const float* W_out, int lmax, int lmax_out, int N,
-                                 int Ne, int C, const uint8_t* parity_mask, float* out, int64_t n_send, int64_t nodes,
-                                 int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream)
+// lw: l-dependent weights W_edge [lmax+1, C, Ne], W_node [lmax+1, C, N], W_out [lmax_out+1, N, C] (Eq.(35), (41), (47), (55)):
+// every projection becomes one problem per degree l over the columns l^2 .. l^2 + 2l (one launch with proj_multi).
+static int field_entry(bool lw, const float* node_feats, const int64_t* edge_index, const float* edge_feats,
+                       const float* W_edge, const float* W_node, const float* W_out, int lmax, int lmax_out, int N, int Ne,
+                       int C, const uint8_t* parity_mask, float* out, int64_t n_send, int64_t nodes, int64_t E,
+                       void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     clear_error();
     int rc = check_common(lmax, lmax_out, N, C, parity_mask);
@@ -834,8 +827,23 @@ int cgtp_message_field_bipartite(const float* node_feats, const int64_t* edge_in
     a.batch = n_send;
     a.accumulate = 0;
     a.j0 = 0;
+    // one problem per degree with l-dependent weights, else the whole row
+    auto per_degree = [&](const ProjArgs& base, const float* W, int K) {
+        std::vector<ProjArgs> v;
+        for (int l = 0; l < (lw ? p->lmax + 1 : 1); ++l) {
+            ProjArgs d = base;
+            const int jo = lw ? l * l : 0;
+            d.W = W + (lw ? (size_t)l * C * K : 0);
+            d.J = lw ? 2 * l + 1 : p->L2;
+            d.out0 = base.out0 + jo;
+            d.out1 = base.out1 + jo;
+            d.j0 = jo;
+            v.push_back(d);
+        }
+        return v;
+    };
     if (n_send > 0) {
-        rc = launch_proj(&a, 1, K_PROJ_IN, st);
+        rc = launch_proj_degrees(per_degree(a, W_node, N), 1, K_PROJ_IN, st);
         if (rc) return rc;
     }
 
@@ -852,7 +860,7 @@ int cgtp_message_field_bipartite(const float* node_feats, const int64_t* edge_in
             b.out0 = Ha[0];
             b.out1 = Ha[1];
             b.batch = ec;
-            rc = launch_proj(&b, 1, K_PROJ_IN, st);
+            rc = launch_proj_degrees(per_degree(b, W_edge, Ne), 1, K_PROJ_IN, st);
             if (rc) return rc;
         }
         for (int s = 0; s < 2; ++s) {
@@ -889,31 +897,62 @@ int cgtp_message_field_bipartite(const float* node_feats, const int64_t* edge_in
     }
 
     // output projection per receiver (Eq.(55), (58))
-    std::vector<ProjArgs> pv(2);
-    for (int s = 0; s < 2; ++s) {
-        ProjArgs& o = pv[s];
-        o.X = Tn[s];
-        o.x_bs = (int64_t)Cpar[s] * tstr;
-        o.x_rs = tstr;
-        o.W = W_out;
-        o.ldw_m = C;
-        o.ldw_k = 1;
-        o.idx_m = nullptr;
-        o.idx_k = cp->perm_dev + (s ? cp->Ce : 0);
-        o.M = N;
-        o.K = Cpar[s];
-        o.J = p->Lo2;
-        o.out0 = out + (size_t)s * N * p->Lo2;
-        o.o_bs0 = (int64_t)2 * N * p->Lo2;
-        o.out1 = o.out0;
-        o.o_bs1 = o.o_bs0;
-        o.m_split = N;
-        o.o_rs = p->Lo2;
-        o.batch = nodes;
-        o.accumulate = 0;
-        o.j0 = 0;
+    std::vector<ProjArgs> pv;
+    for (int l = 0; l < (lw ? p->lmax_out + 1 : 1); ++l) {
+        const int jo = lw ? l * l : 0;
+        for (int s = 0; s < 2; ++s) {
+            pv.emplace_back();
+            ProjArgs& o = pv.back();
+            o.X = Tn[s];
+            o.x_bs = (int64_t)Cpar[s] * tstr;
+            o.x_rs = tstr;
+            o.W = W_out + (lw ? (size_t)l * N * C : 0);
+            o.ldw_m = C;
+            o.ldw_k = 1;
+            o.idx_m = nullptr;
+            o.idx_k = cp->perm_dev + (s ? cp->Ce : 0);
+            o.M = N;
+            o.K = Cpar[s];
+            o.J = lw ? 2 * l + 1 : p->Lo2;
+            o.out0 = out + (size_t)s * N * p->Lo2 + jo;
+            o.o_bs0 = (int64_t)2 * N * p->Lo2;
+            o.out1 = o.out0;
+            o.o_bs1 = o.o_bs0;
+            o.m_split = N;
+            o.o_rs = p->Lo2;
+            o.batch = nodes;
+            o.accumulate = 0;
+            o.j0 = jo;
+        }
     }
     return launch_proj_degrees(pv, 2, K_PROJ_OUT, st);
+}
+
+int cgtp_message_field(const float* node_feats, const int64_t* edge_index, const float* edge_feats, const float* W_edge,
+                       const float* W_node, const float* W_out, int lmax, int lmax_out, int N, int Ne, int C,
+                       const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* workspace,
+                       size_t workspace_bytes, void* cuda_stream)
+{
+    return cgtp_message_field_bipartite(node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C,
+                                        parity_mask, out, nodes, nodes, E, workspace, workspace_bytes, cuda_stream);
+}
+
+int cgtp_message_field_bipartite(const float* node_feats, const int64_t* edge_index, const float* edge_feats,
+                                 const float* W_edge, const float* W_node, const float* W_out, int lmax, int lmax_out, int N,
+                                 int Ne, int C, const uint8_t* parity_mask, float* out, int64_t n_send, int64_t nodes,
+                                 int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    return field_entry(false, node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C, parity_mask,
+                       out, n_send, nodes, E, workspace, workspace_bytes, cuda_stream);
+}
+
+int cgtp_message_field_lw(const float* node_feats, const int64_t* edge_index, const float* edge_feats, const float* W_edge,
+                          const float* W_node, const float* W_out, int lmax, int lmax_out, int N, int Ne, int C,
+                          const uint8_t* parity_mask, float* out, int64_t nodes, int64_t E, void* workspace,
+                          size_t workspace_bytes, void* cuda_stream)
+{
+    return field_entry(true, node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C, parity_mask,
+                       out, nodes, nodes, E, workspace, workspace_bytes, cuda_stream);
 }
 
 // ------------------------------------------------------------------------------ parity-slot entry points

@@ -187,3 +187,16 @@ def test_field_bipartite_shards_reproduce_the_full_call():
         torch.cuda.synchronize()
         rows.append(out.cpu().numpy())
     assert np.array_equal(np.concatenate(rows), full)  # bit-identical rows
+
+
+@pytest.mark.parametrize("lmax,lmax_out,N,Ne,C,nodes", [(4, 4, 16, 8, 64, 30), (3, 5, 6, 4, 5, 21), (6, 6, 8, 8, 16, 12)])
+def test_field_lw_vs_oracle(lmax, lmax_out, N, Ne, C, nodes):
+    m = synthetic.make_message(lmax, lmax_out, N, C, nodes, _ragged(nodes, 5, lmax), seed=31 + lmax)
+    XE, _ = synthetic.make_edge_field(m, Ne, seed=31)
+    (Wn,), Wo = synthetic.lw_weights(lmax, lmax_out, N, C, seed=31, n_in=1)
+    (We,), _ = synthetic.lw_weights(lmax, lmax_out, Ne, C, seed=37, n_in=1)
+    out = cg.cgtp_message_field_lw(_cuda(m.node_feats), _cuda(m.edge_index), _cuda(XE), _cuda(We), _cuda(Wn), _cuda(Wo),
+                                   lmax, lmax_out, N, Ne, C, m.parity_mask, check=True)
+    torch.cuda.synchronize()
+    ref = orc.message_field_lw(m.node_feats, m.edge_index, XE, We, Wn, Wo, lmax, lmax_out, m.parity_mask)
+    assert sector_err(out.cpu().numpy(), ref) <= TOL
