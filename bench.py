@@ -641,8 +641,9 @@ def run_edge_field(args, cg, synthetic, dev, fp32_peak_tflops):
     C channels plus the edge projection 2 C Ne L^2; per node 2 C N L^2 (node projection) + 2 N C L_o^2 (output)."""
     import torch
     res = []
-    for (lmax, N, Ne, C, nodes, degree) in [(4, 128, 128, 128, 2048, 16), (4, 128, 8, 128, 2048, 16)]:
-        m = synthetic.make_message(lmax, lmax, N, C, nodes, degree, seed=0)
+    for (lmax, N, Ne, C, nodes, degree) in [(4, 128, 128, 128, 2048, 16), (4, 128, 8, 128, 2048, 16),
+                                            (8, 128, 8, 128, 16384, 32)]:   # last: the graph of configs[4], 16 edge chunks
+        m = synthetic.make_message(lmax, lmax, N, C, nodes, degree, r_max=5.0 if nodes == 2048 else 6.0, seed=0)
         XE, W_edge = synthetic.make_edge_field(m, Ne, seed=0)
         nsets = max(2, int(300e6 // XE.nbytes) + 1)   # rotating edge fields so that no step finds them in L2
         XEs = [torch.from_numpy(XE).to(dev) for _ in range(nsets)]
@@ -686,7 +687,7 @@ def run_edge_field(args, cg, synthetic, dev, fp32_peak_tflops):
             del got_tc
         finally:
             cg.cgtp_set_math_mode(cg.MATH_FP32)
-        res.append({"workload": f"configs[2] graph ({nodes} nodes, {m.E} edges), lmax=lmax_out={lmax}, N=C={N}, edge field "
+        res.append({"workload": f"configs[{2 if nodes == 2048 else 4}] graph ({nodes} nodes, {m.E} edges), lmax=lmax_out={lmax}, N=C={N}, edge field "
                                 f"[E, {Ne}, {L2}] ({XE.nbytes / 1e6:.0f} MB, {nsets} rotating sets), half odd channels",
                     "ms_per_step": ms, "edges_per_s": m.E / (ms * 1e-3),
                     "alg_tflops": flops / (ms * 1e-3) / 1e12, "frac_fp32_peak": flops / (ms * 1e-3) / 1e12 / fp32_peak_tflops,

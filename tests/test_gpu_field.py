@@ -200,3 +200,20 @@ def test_field_lw_vs_oracle(lmax, lmax_out, N, Ne, C, nodes):
     torch.cuda.synchronize()
     ref = orc.message_field_lw(m.node_feats, m.edge_index, XE, We, Wn, Wo, lmax, lmax_out, m.parity_mask)
     assert sector_err(out.cpu().numpy(), ref) <= TOL
+
+
+def test_field_configs4_graph_sampled_receivers():
+    """The graph of BASELINE.json configs[4] (16384 nodes, 524288 edges, lmax 8, N = C = 128, half odd) with an edge
+    field of 8 channels: 16 edge chunks, 16-column groups reading the sender's field in place; sampled receivers
+    against the oracle on the edge list restricted to them."""
+    lmax, N, Ne, C, nodes, degree = 8, 128, 8, 128, 16384, 32
+    m = synthetic.make_message(lmax, lmax, N, C, nodes, degree, r_max=6.0, seed=0)
+    XE, W_edge = synthetic.make_edge_field(m, Ne, seed=0)
+    got = run_field(m, XE, W_edge, check=True)
+    rng = np.random.default_rng(1)
+    recv = np.unique(np.concatenate([[0, 1023, 1024, nodes - 1], rng.integers(0, nodes, 4)]))  # 1023 | 1024: a chunk boundary
+    keep = np.isin(m.edge_index[1], recv)
+    ref = orc.message_field(m.node_feats, m.edge_index[:, keep], XE[keep], W_edge, m.W_node, m.W_out, lmax, lmax,
+                            m.parity_mask)
+    assert sector_err(got[recv], ref[recv]) <= TOL, sector_err(got[recv], ref[recv])
+    assert np.abs(got[:, 1, :, 0]).max() <= TOL * np.abs(got[:, 1]).max()
