@@ -36,6 +36,29 @@ __global__ void __launch_bounds__(256) field_pool_kernel(const float* __restrict
         const bool first = r0 >= e0;
         if (lo >= hi && !(r0 == r1 && e0 == 0)) continue;
         float* dst = Tn + (size_t)i * blk;
+        if ((blk & 3) == 0) {
+            // blocks of a multiple of 4 floats start 16-byte aligned (the buffers are 256-byte aligned): 128-bit loads,
+            // two vectors per thread in flight; every component still adds its edges in edge order
+            const float4* T4 = reinterpret_cast<const float4*>(T);
+            float4* dst4 = reinterpret_cast<float4*>(dst);
+            const int blk4 = blk >> 2;
+            for (int q = threadIdx.x; q < blk4; q += 2 * blockDim.x) {
+                const int q1 = q + blockDim.x;
+                const bool two = q1 < blk4;
+                float4 a0 = first ? make_float4(0.f, 0.f, 0.f, 0.f) : dst4[q];
+                float4 a1 = (first || !two) ? make_float4(0.f, 0.f, 0.f, 0.f) : dst4[q1];
+                for (long long e = lo; e < hi; ++e) {
+                    const float4* t = T4 + (size_t)(e - e0) * blk4;
+                    const float4 v0 = __ldg(t + q);
+                    const float4 v1 = two ? __ldg(t + q1) : make_float4(0.f, 0.f, 0.f, 0.f);
+                    a0.x += v0.x; a0.y += v0.y; a0.z += v0.z; a0.w += v0.w;
+                    a1.x += v1.x; a1.y += v1.y; a1.z += v1.z; a1.w += v1.w;
+                }
+                dst4[q] = a0;
+                if (two) dst4[q1] = a1;
+            }
+            continue;
+        }
         for (int q = threadIdx.x; q < blk; q += blockDim.x) {
             float acc = first ? 0.f : dst[q];
             for (long long e = lo; e < hi; ++e) acc += __ldg(T + (size_t)(e - e0) * blk + q);
