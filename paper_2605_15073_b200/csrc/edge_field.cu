@@ -19,6 +19,12 @@ __global__ void __launch_bounds__(256) field_gather_kernel(const float* __restri
     for (long long e = blockIdx.x; e < ne; e += gridDim.x) {
         const float* src = Hn + (size_t)send[e] * blk;
         float* dst = Hb + (size_t)e * blk;
+        if ((blk & 3) == 0) {  // 16-byte aligned blocks: 128-bit copies
+            const float4* s4 = reinterpret_cast<const float4*>(src);
+            float4* d4 = reinterpret_cast<float4*>(dst);
+            for (int q = threadIdx.x; q < (blk >> 2); q += blockDim.x) d4[q] = __ldg(s4 + q);
+            continue;
+        }
         for (int q = threadIdx.x; q < blk; q += blockDim.x) dst[q] = __ldg(src + q);
     }
 }
