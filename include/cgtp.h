@@ -333,6 +333,38 @@ int cgtp_set_math_mode(int mode);
 int cgtp_get_math_mode(void);
 
 /* ---------------------------------------------------------------------------------------------
+ * Kernel-path switch (test instrumentation; never needed for results).  Several stages have a specialised kernel and
+ * a generic one that computes the same thing with a different mapping to the machine; a set bit forces the generic
+ * kernel, so that tests/ can cross-check the two on whole full-size batches (the oracle anchors both on samples):
+ *   CGTP_PATH_GENERIC_CORE   S2-S4: onsite_generic.cu instead of the lane = column core (onsite_core.cu)
+ *   CGTP_PATH_GENERIC_EDGE   M3-M4: one CTA per (receiver, channel block) with direct loads (message.cu) instead of
+ *                            the persistent TMA-ring kernel (edge_ring.cu)
+ *   CGTP_PATH_GENERIC_PROJ   S1/S5/M1/M6: register-tiled SIMT GEMM (proj.cu) instead of proj_fast.cu / proj_multi.cu
+ *   CGTP_PATH_GENERIC_SYNTH  M2: node_synth_kernel instead of the lane = column synthesis (sht_fast.cu)
+ *   CGTP_PATH_UNFUSED_ONSITE S1-S5: the four-launch on-site step (projection, core per parity, projection) instead of
+ *                            the single fused kernel (onsite_fused.cu)
+ * Process-wide, read at every call; 0 (default) = every specialised kernel.  CGTP_ERR_INVALID for unknown bits.
+ * ------------------------------------------------------------------------------------------- */
+#define CGTP_PATH_GENERIC_CORE 1
+#define CGTP_PATH_GENERIC_EDGE 2
+#define CGTP_PATH_GENERIC_PROJ 4
+#define CGTP_PATH_GENERIC_SYNTH 8
+#define CGTP_PATH_UNFUSED_ONSITE 16
+int cgtp_set_kernel_path(int flags);
+int cgtp_get_kernel_path(void);
+
+/* ---------------------------------------------------------------------------------------------
+ * FP32 pipe calibration: the denominator of the "alu" roofline of the on-site path ("measure the
+ * real sustained FP32 peak with an FMA micro-benchmark on the box").  Runs a register-only kernel of dependent-chain
+ * fused multiply-adds on every SM (16 independent chains per thread, 8 warps x 4 CTAs per SM) for about `ms_target`
+ * milliseconds and returns the sustained rate in *tflops (2 flop per FMA lane):
+ *   packed = 0  scalar FFMA (fma.rn.f32)        packed = 1  FFMA2 (fma.rn.f32x2, two lanes per instruction)
+ * Synchronises `cuda_stream`.  *sm_mhz_est (may be NULL) receives flop rate / (SMs x 128 lanes x 2), the clock the
+ * rate would correspond to at one FMA per lane per cycle.
+ * ------------------------------------------------------------------------------------------- */
+int cgtp_fma_peak(int packed, double ms_target, double* tflops, double* sm_mhz_est, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Instrumentation (used by bench.py; never needed for results).
  * cgtp_launch_count: number of kernels this library has launched since it was loaded.
  * cgtp_profile_enable(1): record a CUDA-event pair around every kernel launch (on the launching

@@ -95,6 +95,11 @@ def lib() -> ctypes.CDLL:
     L.cgtp_set_math_mode.restype = i
     L.cgtp_set_math_mode.argtypes = [i]
     L.cgtp_get_math_mode.restype = i
+    L.cgtp_set_kernel_path.restype = i
+    L.cgtp_set_kernel_path.argtypes = [i]
+    L.cgtp_get_kernel_path.restype = i
+    L.cgtp_fma_peak.restype = i
+    L.cgtp_fma_peak.argtypes = [i, ctypes.c_double, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), vp]
     L.cgtp_launch_count.restype = i64
     L.cgtp_profile_kinds.restype = i
     L.cgtp_profile_kind_name.restype = ctypes.c_char_p
@@ -132,18 +137,33 @@ def _stream_ptr(stream) -> int:
     return s.cuda_stream
 
 
+def _out(out, shape, device) -> torch.Tensor:
+    """The caller's `out` (contiguous FP32 CUDA tensor of exactly `shape`: the kernels write all of it) or a new one."""
+    if out is None:
+        return torch.empty(shape, dtype=torch.float32, device=device)
+    _dev(out, torch.float32, "out")
+    if tuple(out.shape) != tuple(shape) or out.device != device:
+        raise ValueError(f"out must be a tensor of shape {tuple(shape)} on {device}, got {tuple(out.shape)} on {out.device}")
+    return out
+
+
 _ws_cache: dict = {}
 
 
-def _workspace(device, nbytes: int) -> torch.Tensor:
-    """One grow-only scratch buffer per device (torch allocations are 512-byte aligned)."""
-    key = (device.type, device.index)
-    ws = _ws_cache.get(key)
-    if ws is None or ws.numel() < nbytes:
-        _ws_cache.pop(key, None)
-        ws = None
-        ws = torch.empty(int(nbytes), dtype=torch.uint8, device=device)
-        _ws_cache[key] = ws
+def _workspace(device, nbytes: int, stream=None) -> torch.Tensor:
+    """One grow-only scratch buffer per (device, stream): calls issued on different streams never share scratch, and a
+    buffer that is replaced by a larger one is handed back to the caching allocator only after the work queued on its
+    stream has run (record_stream).  torch allocations are 512-byte aligned."""
+    with torch.cuda.device(device):
+        s = torch.cuda.current_stream() if stream is None else stream
+        key = (device.index if device.index is not None else torch.cuda.current_device(), s.cuda_stream)
+        ws = _ws_cache.get(key)
+        if ws is None or ws.numel() < nbytes:
+            _ws_cache.pop(key, None)
+            ws = None  # drops the old buffer; its record_stream defers reuse until the stream has passed this point
+            ws = torch.empty(int(nbytes), dtype=torch.uint8, device=device)
+            ws.record_stream(s)
+            _ws_cache[key] = ws
     return ws
 
 
@@ -177,14 +197,9 @@ def cgtp_onsite(A, B, W_a, W_b, W_out, lmax, lmax_out, N, C, parity_mask, out=No
     if tuple(W_a.shape) != (C, N) or tuple(W_b.shape) != (C, N) or tuple(W_out.shape) != (N, C):
         raise ValueError("W_a, W_b must be [C, N] and W_out [N, C]")
     mask = _mask(parity_mask, C)
-    if out is None:
-        out = torch.empty((batch, 2, N, Lo2), dtype=f32, device=A.device)
-    else:
-        _dev(out, f32, "out")
-        if tuple(out.shape) != (batch, 2, N, Lo2):
-            raise ValueError("out must be [batch, 2, N, (lmax_out+1)^2]")
+    out = _out(out, (batch, 2, N, Lo2), A.device)
     nbytes = cgtp_onsite_workspace_bytes(lmax, lmax_out, N, C, batch)
-    ws = _workspace(A.device, nbytes) if workspace is None else workspace
+    ws = _workspace(A.device, nbytes, stream) if workspace is None else workspace
     with torch.cuda.device(A.device):
         rc = lib().cgtp_onsite(A.data_ptr(), B.data_ptr(), W_a.data_ptr(), W_b.data_ptr(), W_out.data_ptr(),
                                lmax, lmax_out, N, C, mask.ctypes.data, out.data_ptr(), batch,
@@ -213,14 +228,9 @@ def cgtp_onsite_nbody(X, W_in, W_out, nu, lmax, lmax_out, N, C, out=None, worksp
     batch = X.shape[1]
     if tuple(W_in.shape) != (nu, C, N) or tuple(W_out.shape) != (N, C):
         raise ValueError("W_in must be [nu, C, N] and W_out [N, C]")
-    if out is None:
-        out = torch.empty((batch, N, Lo2), dtype=f32, device=X.device)
-    else:
-        _dev(out, f32, "out")
-        if tuple(out.shape) != (batch, N, Lo2):
-            raise ValueError("out must be [batch, N, (lmax_out+1)^2]")
+    out = _out(out, (batch, N, Lo2), X.device)
     nbytes = cgtp_onsite_nbody_workspace_bytes(nu, lmax, lmax_out, N, C, batch)
-    ws = _workspace(X.device, nbytes) if workspace is None else workspace
+    ws = _workspace(X.device, nbytes, stream) if workspace is None else workspace
     with torch.cuda.device(X.device):
         rc = lib().cgtp_onsite_nbody(X.data_ptr(), W_in.data_ptr(), W_out.data_ptr(), nu, lmax, lmax_out, N, C,
                                      out.data_ptr(), batch, ws.data_ptr(), ws.numel(), _stream_ptr(stream))
@@ -251,12 +261,9 @@ def cgtp_message(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out, l
     if tuple(W_node.shape) != (C, N) or tuple(W_out.shape) != (N, C):
         raise ValueError("W_node must be [C, N] and W_out [N, C]")
     mask = _mask(parity_mask, C)
-    if out is None:
-        out = torch.empty((nodes, 2, N, Lo2), dtype=f32, device=X.device)
-    else:
-        _dev(out, f32, "out")
+    out = _out(out, (nodes, 2, N, Lo2), X.device)
     nbytes = lib().cgtp_message_workspace_bytes(lmax, lmax_out, N, C, mask.ctypes.data, nodes, E)
-    ws = _workspace(X.device, nbytes) if workspace is None else workspace
+    ws = _workspace(X.device, nbytes, stream) if workspace is None else workspace
     sp = _stream_ptr(stream)
     with torch.cuda.device(X.device):
         rc = lib().cgtp_message(X.data_ptr(), ei.data_ptr(), ev.data_ptr(), er.data_ptr(), W_node.data_ptr(),
@@ -296,12 +303,9 @@ def cgtp_message_field(node_feats, edge_index, edge_feats, W_edge, W_node, W_out
             or tuple(W_out.shape) != pre_out + (N, C)):
         raise ValueError("W_edge must be [C, Ne], W_node [C, N] and W_out [N, C] (with a leading degree axis for _lw)")
     mask = _mask(parity_mask, C)
-    if out is None:
-        out = torch.empty((nodes, 2, N, Lo2), dtype=f32, device=X.device)
-    else:
-        _dev(out, f32, "out")
+    out = _out(out, (nodes, 2, N, Lo2), X.device)
     nbytes = cgtp_message_field_workspace_bytes(lmax, lmax_out, N, Ne, C, nodes, E)
-    ws = _workspace(X.device, nbytes) if workspace is None else workspace
+    ws = _workspace(X.device, nbytes, stream) if workspace is None else workspace
     sp = _stream_ptr(stream)
     with torch.cuda.device(X.device):
         entry = lib().cgtp_message_field_lw if _lw else lib().cgtp_message_field
@@ -329,12 +333,9 @@ def cgtp_message_field_bipartite(node_feats, edge_index, edge_feats, W_edge, W_n
     if tuple(W_edge.shape) != (C, Ne) or tuple(W_node.shape) != (C, N) or tuple(W_out.shape) != (N, C):
         raise ValueError("W_edge must be [C, Ne], W_node [C, N] and W_out [N, C]")
     mask = _mask(parity_mask, C)
-    if out is None:
-        out = torch.empty((n_recv, 2, N, Lo2), dtype=f32, device=X.device)
-    else:
-        _dev(out, f32, "out")
+    out = _out(out, (n_recv, 2, N, Lo2), X.device)
     nbytes = lib().cgtp_message_field_bipartite_workspace_bytes(lmax, lmax_out, N, Ne, C, n_send, n_recv, E)
-    ws = _workspace(X.device, nbytes) if workspace is None else workspace
+    ws = _workspace(X.device, nbytes, stream) if workspace is None else workspace
     sp = _stream_ptr(stream)
     with torch.cuda.device(X.device):
         rc = lib().cgtp_message_field_bipartite(X.data_ptr(), ei.data_ptr(), XE.data_ptr(), W_edge.data_ptr(),
@@ -365,14 +366,9 @@ def cgtp_message_bipartite(node_feats, edge_index, edge_vec, edge_radial, W_node
     if tuple(W_node.shape) != (C, N) or tuple(W_out.shape) != (N, C):
         raise ValueError("W_node must be [C, N] and W_out [N, C]")
     mask = _mask(parity_mask, C)
-    if out is None:
-        out = torch.empty((n_recv, 2, N, Lo2), dtype=f32, device=X.device)
-    else:
-        _dev(out, f32, "out")
-        if tuple(out.shape) != (n_recv, 2, N, Lo2):
-            raise ValueError("out must be [n_recv, 2, N, (lmax_out+1)^2]")
+    out = _out(out, (n_recv, 2, N, Lo2), X.device)
     nbytes = lib().cgtp_message_bipartite_workspace_bytes(lmax, lmax_out, N, C, mask.ctypes.data, n_send, n_recv, E)
-    ws = _workspace(X.device, nbytes) if workspace is None else workspace
+    ws = _workspace(X.device, nbytes, stream) if workspace is None else workspace
     sp = _stream_ptr(stream)
     with torch.cuda.device(X.device):
         rc = lib().cgtp_message_bipartite(X.data_ptr(), ei.data_ptr(), ev.data_ptr(), er.data_ptr(), W_node.data_ptr(),
@@ -396,14 +392,9 @@ def cgtp_onsite_parity(A, B, W_a, W_b, W_out, lmax, lmax_out, N, C, out=None, wo
         raise ValueError("A, B must be [batch, 2, N, (lmax+1)^2]")
     if tuple(W_a.shape) != (16, C, N) or tuple(W_b.shape) != (16, C, N) or tuple(W_out.shape) != (16, N, C):
         raise ValueError("W_a, W_b must be [16, C, N] and W_out [16, N, C]")
-    if out is None:
-        out = torch.empty((batch, 2, N, Lo2), dtype=f32, device=A.device)
-    else:
-        _dev(out, f32, "out")
-        if tuple(out.shape) != (batch, 2, N, Lo2):
-            raise ValueError("out must be [batch, 2, N, (lmax_out+1)^2]")
+    out = _out(out, (batch, 2, N, Lo2), A.device)
     nbytes = lib().cgtp_onsite_parity_workspace_bytes(lmax, lmax_out, N, C, batch)
-    ws = _workspace(A.device, nbytes) if workspace is None else workspace
+    ws = _workspace(A.device, nbytes, stream) if workspace is None else workspace
     with torch.cuda.device(A.device):
         rc = lib().cgtp_onsite_parity(A.data_ptr(), B.data_ptr(), W_a.data_ptr(), W_b.data_ptr(), W_out.data_ptr(),
                                       lmax, lmax_out, N, C, out.data_ptr(), batch, ws.data_ptr(), ws.numel(),
@@ -429,14 +420,9 @@ def cgtp_message_parity(node_feats, edge_index, edge_vec, edge_radial, W_node, W
         raise ValueError("edge_index [2,E], edge_vec [E,3], edge_radial [E,8,C] expected")
     if tuple(W_node.shape) != (8, C, N) or tuple(W_out.shape) != (8, N, C):
         raise ValueError("W_node must be [8, C, N] and W_out [8, N, C]")
-    if out is None:
-        out = torch.empty((nodes, 2, N, Lo2), dtype=f32, device=X.device)
-    else:
-        _dev(out, f32, "out")
-        if tuple(out.shape) != (nodes, 2, N, Lo2):
-            raise ValueError("out must be [nodes, 2, N, (lmax_out+1)^2]")
+    out = _out(out, (nodes, 2, N, Lo2), X.device)
     nbytes = lib().cgtp_message_parity_workspace_bytes(lmax, lmax_out, N, C, nodes, E)
-    ws = _workspace(X.device, nbytes) if workspace is None else workspace
+    ws = _workspace(X.device, nbytes, stream) if workspace is None else workspace
     sp = _stream_ptr(stream)
     with torch.cuda.device(X.device):
         rc = lib().cgtp_message_parity(X.data_ptr(), ei.data_ptr(), ev.data_ptr(), er.data_ptr(), W_node.data_ptr(),
@@ -460,14 +446,9 @@ def cgtp_onsite_lw(A, B, W_a, W_b, W_out, lmax, lmax_out, N, C, parity_mask, out
     if tuple(W_a.shape) != (lmax + 1, C, N) or tuple(W_b.shape) != (lmax + 1, C, N) or tuple(W_out.shape) != (lmax_out + 1, N, C):
         raise ValueError("W_a, W_b must be [lmax+1, C, N] and W_out [lmax_out+1, N, C]")
     mask = _mask(parity_mask, C)
-    if out is None:
-        out = torch.empty((batch, 2, N, Lo2), dtype=f32, device=A.device)
-    else:
-        _dev(out, f32, "out")
-        if tuple(out.shape) != (batch, 2, N, Lo2):
-            raise ValueError("out must be [batch, 2, N, (lmax_out+1)^2]")
+    out = _out(out, (batch, 2, N, Lo2), A.device)
     nbytes = cgtp_onsite_workspace_bytes(lmax, lmax_out, N, C, batch)
-    ws = _workspace(A.device, nbytes) if workspace is None else workspace
+    ws = _workspace(A.device, nbytes, stream) if workspace is None else workspace
     with torch.cuda.device(A.device):
         rc = lib().cgtp_onsite_lw(A.data_ptr(), B.data_ptr(), W_a.data_ptr(), W_b.data_ptr(), W_out.data_ptr(),
                                   lmax, lmax_out, N, C, mask.ctypes.data, out.data_ptr(), batch,
@@ -494,12 +475,9 @@ def cgtp_message_lw(node_feats, edge_index, edge_vec, edge_radial, W_node, W_out
     if tuple(W_node.shape) != (lmax + 1, C, N) or tuple(W_out.shape) != (lmax_out + 1, N, C):
         raise ValueError("W_node must be [lmax+1, C, N] and W_out [lmax_out+1, N, C]")
     mask = _mask(parity_mask, C)
-    if out is None:
-        out = torch.empty((nodes, 2, N, Lo2), dtype=f32, device=X.device)
-    else:
-        _dev(out, f32, "out")
+    out = _out(out, (nodes, 2, N, Lo2), X.device)
     nbytes = lib().cgtp_message_workspace_bytes(lmax, lmax_out, N, C, mask.ctypes.data, nodes, E)
-    ws = _workspace(X.device, nbytes) if workspace is None else workspace
+    ws = _workspace(X.device, nbytes, stream) if workspace is None else workspace
     sp = _stream_ptr(stream)
     with torch.cuda.device(X.device):
         fn = lib().cgtp_message_lwr if radial_l1 else lib().cgtp_message_lw
@@ -520,8 +498,15 @@ def cgtp_message_lwr(node_feats, edge_index, edge_vec, edge_radial, W_node, W_ou
 
 
 def cgtp_message_status(workspace=None, device=None, stream=None) -> int:
-    ws = workspace if workspace is not None else _ws_cache[(device.type, device.index)]
-    return lib().cgtp_message_status(ws.data_ptr(), _stream_ptr(stream))
+    """Graph status word of the last message-passing call that used `workspace` (default: the binding's own scratch
+    buffer of (device, stream)); synchronises the stream."""
+    if workspace is None:
+        device = torch.device("cuda", torch.cuda.current_device()) if device is None else device
+        with torch.cuda.device(device):
+            s = torch.cuda.current_stream() if stream is None else stream
+            workspace = _ws_cache[(device.index, s.cuda_stream)]
+            return lib().cgtp_message_status(workspace.data_ptr(), s.cuda_stream)
+    return lib().cgtp_message_status(workspace.data_ptr(), _stream_ptr(stream))
 
 
 def cgtp_build_segments(edge_index, nodes: int, stream=None):
@@ -576,6 +561,24 @@ def cgtp_message_host(node_feats, edge_index, edge_vec, edge_radial, W_node, W_o
 
 
 MATH_FP32, MATH_3XTF32, MATH_TF32 = 0, 1, 2
+PATH_GENERIC_CORE, PATH_GENERIC_EDGE, PATH_GENERIC_PROJ, PATH_GENERIC_SYNTH, PATH_UNFUSED_ONSITE = 1, 2, 4, 8, 16
+
+
+def cgtp_set_kernel_path(flags: int) -> None:
+    """Test switch: force the generic kernel of a stage (PATH_* bits, include/cgtp.h); 0 = the specialised kernels."""
+    _check(lib().cgtp_set_kernel_path(int(flags)))
+
+
+def cgtp_get_kernel_path() -> int:
+    return lib().cgtp_get_kernel_path()
+
+
+def cgtp_fma_peak(packed: bool, ms_target: float = 20.0, stream=None):
+    """(TFLOP/s, equivalent SM MHz) of the register-only FFMA (packed=False) / FFMA2 (packed=True) micro-kernel."""
+    tf, mhz = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(lib().cgtp_fma_peak(int(bool(packed)), float(ms_target), ctypes.byref(tf), ctypes.byref(mhz),
+                               _stream_ptr(stream)))
+    return tf.value, mhz.value
 
 
 def cgtp_set_math_mode(mode: int) -> None:

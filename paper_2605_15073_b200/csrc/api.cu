@@ -74,7 +74,7 @@ static size_t message_ws_bytes(int lmax, int lmax_out, int C, int Co, int64_t n_
 // `group` problems per launch (the factors / sectors of one degree).
 static int launch_proj_degrees(const std::vector<ProjArgs>& v, int group, Kind kind, cudaStream_t st)
 {
-    if ((int)v.size() > group && get_math_mode() == CGTP_MATH_FP32) {
+    if ((int)v.size() > group && get_math_mode() == CGTP_MATH_FP32 && !(kernel_path() & PATH_GENERIC_PROJ)) {
         bool handled = false;
         const int rc = launch_proj_multi(v.data(), (int)v.size(), kind, st, &handled);
         if (rc != CGTP_OK || handled) return rc;
@@ -112,7 +112,8 @@ static int onsite_pass(const Plan* p, int N, const OnsitePass& q, int64_t batch,
 {
     const int Ce = q.Ce, Co = q.Co;
     // fast core (onsite_core.cu) when both parities fit; it wants odd row strides and 32-column groups
-    const bool fast = (Ce == 0 || onsite_fast_supported(p, false)) && (Co == 0 || onsite_fast_supported(p, true));
+    const bool fast = !(kernel_path() & PATH_GENERIC_CORE) && (Ce == 0 || onsite_fast_supported(p, false)) &&
+                      (Co == 0 || onsite_fast_supported(p, true));
     const int hstr = fast ? onsite_fast_hstride(p) : p->L2p;
     const int tstr = fast ? onsite_fast_tstride(p) : p->Lo2p;
     const size_t ncol_e = (size_t)round_up((int)((size_t)batch * Ce % 32), 32) + (size_t)batch * Ce / 32 * 32;
@@ -267,7 +268,7 @@ static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_
     Carver cv(workspace);
     int32_t* status = cv.take<int32_t>(1);
     int64_t* row_ptr = cv.take<int64_t>((size_t)nodes + 1);
-    const bool fast_synth = synth_fast_supported(p);
+    const bool fast_synth = !(kernel_path() & PATH_GENERIC_SYNTH) && synth_fast_supported(p);
     const int hstr = fast_synth ? synth_fast_hstride(p) : p->L2p;
     float* H_e = cv.take<float>((size_t)round_up64(n_send * Ce, 32) * hstr);
     float* H_o = cv.take<float>((size_t)round_up64(n_send * Co, 32) * hstr);
@@ -782,7 +783,8 @@ static int field_entry(bool lw, const float* node_feats, const int64_t* edge_ind
     const ChannelPlan* cp = get_channel_plan(C, parity_mask);
     if (!cp) return CGTP_ERR_CUDA;
     const int Cpar[2] = {cp->Ce, cp->Co};
-    const bool fast = (Cpar[0] == 0 || onsite_fast_supported(p, false)) && (Cpar[1] == 0 || onsite_fast_supported(p, true));
+    const bool fast = !(kernel_path() & PATH_GENERIC_CORE) && (Cpar[0] == 0 || onsite_fast_supported(p, false)) &&
+                      (Cpar[1] == 0 || onsite_fast_supported(p, true));
     const int hstr = fast ? onsite_fast_hstride(p) : p->L2p;
     const int tstr = fast ? onsite_fast_tstride(p) : p->Lo2p;
     const int64_t ec_max = field_chunk(C, E);
@@ -804,6 +806,9 @@ static int field_entry(bool lw, const float* node_feats, const int64_t* edge_ind
     // M0
     rc = launch_segments(edge_index, E, nodes, n_send, row_ptr, status, st);
     if (rc) return rc;
+    // the pool kernel leaves Tn alone when M0 flags the edge list: define it, so that `out` is zeros plus the flag
+    for (int s = 0; s < 2; ++s)
+        if (Cpar[s] > 0 && nodes > 0) CGTP_CUDA_CHECK(cudaMemsetAsync(Tn[s], 0, (size_t)nodes * Cpar[s] * tstr * 4, st));
 
     // factor 2: Hn = W_node . node_feats, once per node (Eq.(47) :398)
     ProjArgs a;
@@ -1082,15 +1087,15 @@ int cgtp_message_parity(const float* node_feats, const int64_t* edge_index, cons
 // memory back to the driver at every synchronisation and the next call pays for a fresh allocation.
 static void keep_pool_memory()
 {
-    static bool done = false;
-    if (done) return;
-    int dev = 0;
+    static bool done[64] = {false};
+    const int dev = current_device();
+    if (dev < 0 || dev >= 64 || done[dev]) return;
     cudaMemPool_t pool;
-    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+    if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
         uint64_t keep = UINT64_MAX;
         cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
     }
-    done = true;
+    done[dev] = true;
 }
 
 // Streams, events and chunk buffers of cgtp_onsite_host live for the life of the process (grow-only): creating and
@@ -1105,12 +1110,12 @@ struct HostCtx {
     cudaStream_t s_h2d, s_comp, s_d2h;
     cudaEvent_t start, ev_h2d[kHostStreams], ev_comp[kHostStreams], ev_d2h[kHostStreams], ev_end;
     float *dA[kHostStreams] = {}, *dB[kHostStreams] = {}, *dO[kHostStreams] = {};
-    void* dws[kHostStreams] = {};
+    void* dws = nullptr;  // one workspace: the chunks' kernels run in order on s_comp
     size_t in_bytes = 0, out_bytes = 0, ws_bytes = 0;
     float* dW = nullptr;  // W_a | W_b | W_out
     size_t w_bytes = 0;
 };
-HostCtx g_host;
+HostCtx g_host[64];  // one per CUDA device ordinal
 
 int host_ctx_reserve(HostCtx& h, size_t in_bytes, size_t out_bytes, size_t ws_bytes, size_t w_bytes)
 {
@@ -1130,10 +1135,11 @@ int host_ctx_reserve(HostCtx& h, size_t in_bytes, size_t out_bytes, size_t ws_by
     if (in_bytes > h.in_bytes || out_bytes > h.out_bytes || ws_bytes > h.ws_bytes) {
         CGTP_CUDA_CHECK(cudaDeviceSynchronize());
         for (int s = 0; s < kHostStreams; ++s) {
-            cudaFree(h.dA[s]); cudaFree(h.dB[s]); cudaFree(h.dO[s]); cudaFree(h.dws[s]);
+            cudaFree(h.dA[s]); cudaFree(h.dB[s]); cudaFree(h.dO[s]);
             h.dA[s] = h.dB[s] = h.dO[s] = nullptr;
-            h.dws[s] = nullptr;
         }
+        cudaFree(h.dws);
+        h.dws = nullptr;
         h.in_bytes = std::max(h.in_bytes, in_bytes);
         h.out_bytes = std::max(h.out_bytes, out_bytes);
         h.ws_bytes = std::max(h.ws_bytes, ws_bytes);
@@ -1141,8 +1147,8 @@ int host_ctx_reserve(HostCtx& h, size_t in_bytes, size_t out_bytes, size_t ws_by
             CGTP_CUDA_CHECK(cudaMalloc(&h.dA[s], h.in_bytes));
             CGTP_CUDA_CHECK(cudaMalloc(&h.dB[s], h.in_bytes));
             CGTP_CUDA_CHECK(cudaMalloc(&h.dO[s], h.out_bytes));
-            CGTP_CUDA_CHECK(cudaMalloc(&h.dws[s], h.ws_bytes));
         }
+        CGTP_CUDA_CHECK(cudaMalloc(&h.dws, h.ws_bytes));
     }
     if (w_bytes > h.w_bytes) {
         CGTP_CUDA_CHECK(cudaDeviceSynchronize());
@@ -1181,7 +1187,9 @@ int cgtp_onsite_host(const float* A, const float* B, const float* W_a, const flo
     const int64_t chunk = std::min<int64_t>(batch, 8 * unit);  // largest chunk: sizes the buffers
     const size_t wsb = onsite_ws_bytes(lmax, lmax_out, C, chunk);
 
-    HostCtx& h = g_host;
+    const int dev = current_device();
+    if (dev < 0 || dev >= 64) { set_error("no current CUDA device"); return CGTP_ERR_CUDA; }
+    HostCtx& h = g_host[dev];
     std::lock_guard<std::mutex> lock(h.mu);
     rc = host_ctx_reserve(h, (size_t)chunk * in_per, (size_t)chunk * out_per, wsb, 3 * wfl * 4);
     if (rc) return rc;
@@ -1205,7 +1213,7 @@ int cgtp_onsite_host(const float* A, const float* B, const float* W_a, const flo
         // kernels: need the inputs, and the output buffer back from the copy of the chunk that used it last
         CGTP_CUDA_CHECK(cudaStreamWaitEvent(h.s_comp, h.ev_h2d[s], 0));
         if (k >= kHostStreams) CGTP_CUDA_CHECK(cudaStreamWaitEvent(h.s_comp, h.ev_d2h[s], 0));
-        rc = cgtp_onsite(h.dA[s], h.dB[s], dWa, dWb, dWo, lmax, lmax_out, N, C, parity_mask, h.dO[s], nb, h.dws[0], wsb,
+        rc = cgtp_onsite(h.dA[s], h.dB[s], dWa, dWb, dWo, lmax, lmax_out, N, C, parity_mask, h.dO[s], nb, h.dws, wsb,
                          h.s_comp);
         if (rc) return rc;
         CGTP_CUDA_CHECK(cudaEventRecord(h.ev_comp[s], h.s_comp));
@@ -1239,17 +1247,28 @@ int cgtp_message_host(const float* node_feats, const int64_t* edge_index, const 
     const size_t xb = (size_t)nodes * N * L2 * 4, ob = (size_t)nodes * 2 * N * Lo2 * 4, wb = (size_t)C * N * 4;
     const size_t eib = (size_t)2 * (E > 0 ? E : 1) * 8, evb = (size_t)(E > 0 ? E : 1) * 3 * 4, erb = (size_t)(E > 0 ? E : 1) * C * 4;
     const size_t wsb = cgtp_message_workspace_bytes(lmax, lmax_out, N, C, parity_mask, nodes, E);
+    // stream-ordered allocations, released on every exit path
+    struct Pool {
+        cudaStream_t st;
+        std::vector<void*> ptrs;
+        ~Pool()
+        {
+            for (void* q : ptrs) cudaFreeAsync(q, st);
+        }
+        int take(void** q, size_t bytes)
+        {
+            CGTP_CUDA_CHECK(cudaMallocAsync(q, bytes, st));
+            ptrs.push_back(*q);
+            return CGTP_OK;
+        }
+    } pool{st, {}};
     float *dX, *dO, *dWn, *dWo, *dEv, *dEr;
     int64_t* dEi;
     void* dws;
-    CGTP_CUDA_CHECK(cudaMallocAsync(&dX, xb, st));
-    CGTP_CUDA_CHECK(cudaMallocAsync(&dO, ob, st));
-    CGTP_CUDA_CHECK(cudaMallocAsync(&dWn, wb, st));
-    CGTP_CUDA_CHECK(cudaMallocAsync(&dWo, wb, st));
-    CGTP_CUDA_CHECK(cudaMallocAsync(&dEi, eib, st));
-    CGTP_CUDA_CHECK(cudaMallocAsync(&dEv, evb, st));
-    CGTP_CUDA_CHECK(cudaMallocAsync(&dEr, erb, st));
-    CGTP_CUDA_CHECK(cudaMallocAsync(&dws, wsb, st));
+    if ((rc = pool.take((void**)&dX, xb)) || (rc = pool.take((void**)&dO, ob)) || (rc = pool.take((void**)&dWn, wb)) ||
+        (rc = pool.take((void**)&dWo, wb)) || (rc = pool.take((void**)&dEi, eib)) || (rc = pool.take((void**)&dEv, evb)) ||
+        (rc = pool.take((void**)&dEr, erb)) || (rc = pool.take(&dws, wsb)))
+        return rc;
     CGTP_CUDA_CHECK(cudaMemcpyAsync(dX, node_feats, xb, cudaMemcpyHostToDevice, st));
     CGTP_CUDA_CHECK(cudaMemcpyAsync(dWn, W_node, wb, cudaMemcpyHostToDevice, st));
     CGTP_CUDA_CHECK(cudaMemcpyAsync(dWo, W_out, wb, cudaMemcpyHostToDevice, st));
@@ -1261,16 +1280,7 @@ int cgtp_message_host(const float* node_feats, const int64_t* edge_index, const 
     rc = cgtp_message(dX, dEi, dEv, dEr, dWn, dWo, lmax, lmax_out, N, C, parity_mask, dO, nodes, E, dws, wsb, st);
     if (rc) return rc;
     CGTP_CUDA_CHECK(cudaMemcpyAsync(out, dO, ob, cudaMemcpyDeviceToHost, st));
-    int grc = cgtp_message_status(dws, st);
-    CGTP_CUDA_CHECK(cudaFreeAsync(dX, st));
-    CGTP_CUDA_CHECK(cudaFreeAsync(dO, st));
-    CGTP_CUDA_CHECK(cudaFreeAsync(dWn, st));
-    CGTP_CUDA_CHECK(cudaFreeAsync(dWo, st));
-    CGTP_CUDA_CHECK(cudaFreeAsync(dEi, st));
-    CGTP_CUDA_CHECK(cudaFreeAsync(dEv, st));
-    CGTP_CUDA_CHECK(cudaFreeAsync(dEr, st));
-    CGTP_CUDA_CHECK(cudaFreeAsync(dws, st));
-    CGTP_CUDA_CHECK(cudaStreamSynchronize(st));
+    const int grc = cgtp_message_status(dws, st);  // synchronises the stream
     return grc;
 }
 
@@ -1283,6 +1293,16 @@ int cgtp_set_math_mode(int mode)
     return CGTP_OK;
 }
 int cgtp_get_math_mode(void) { return cgtp::get_math_mode(); }
+
+// ------------------------------------------------------------------------------------------ kernel path
+int cgtp_set_kernel_path(int flags)
+{
+    clear_error();
+    if (flags < 0 || flags > 31) { set_error("unknown kernel-path flags %d", flags); return CGTP_ERR_INVALID; }
+    cgtp::set_kernel_path(flags);
+    return CGTP_OK;
+}
+int cgtp_get_kernel_path(void) { return cgtp::kernel_path(); }
 
 // ------------------------------------------------------------------------------------ instrumentation
 int64_t cgtp_launch_count(void) { return cgtp::launch_count(); }

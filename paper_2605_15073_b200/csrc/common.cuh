@@ -23,6 +23,21 @@ inline int kernel_band(int b)
     return -1;
 }
 
+// Ordinal of the calling thread's current CUDA device (-1 on error).  The plan / table / scratch caches hold device
+// pointers, so each of them is keyed by this ordinal: a process that drives several GPUs gets one entry per device.
+inline int current_device()
+{
+    int d = -1;
+    return cudaGetDevice(&d) == cudaSuccess ? d : -1;
+}
+// Multiprocessor count of the current device (cached per ordinal).
+int num_sms();
+
+// Test-only kernel-path switch (cgtp_set_kernel_path): bit set = take the generic kernel where a specialised one exists.
+enum : int { PATH_GENERIC_CORE = 1, PATH_GENERIC_EDGE = 2, PATH_GENERIC_PROJ = 4, PATH_GENERIC_SYNTH = 8, PATH_UNFUSED_ONSITE = 16 };
+int kernel_path();
+void set_kernel_path(int flags);
+
 __host__ __device__ constexpr int round_up(int x, int m) { return (x + m - 1) / m * m; }
 __host__ __device__ constexpr int tri_index(int l, int m) { return l * (l + 1) / 2 + m; }
 
@@ -37,6 +52,7 @@ __host__ __device__ constexpr int tri_index(int l, int m) { return l * (l + 1) /
 // P~_l^m(-x) = (-1)^(l+m) P~_l^m(x) and cos/sin(m (2pi - phi)).
 // ---------------------------------------------------------------------------------------------
 struct Plan {
+    int dev;   // CUDA device ordinal the tables live on: every cache of the library is keyed by it
     int lmax, lmax_out;
     int nu;    // body order the grid is exact for (2 everywhere except the nu-body entry point)
     int LB;    // kernel band limit = kernel_band(max(lmax, lmax_out)); tables cover 0 <= m <= l <= LB
@@ -76,6 +92,7 @@ const Plan* get_plan_nu(int lmax, int lmax_out, int nu);
 // Channel plan: parity_mask -> permutation that lists the even channels first (stable).
 // ---------------------------------------------------------------------------------------------
 struct ChannelPlan {
+    int dev;
     int C, Ce, Co;
     const int* perm_dev;  // device [C]: perm[k] = original channel index of sorted position k
     int perm_host[1024];
@@ -86,6 +103,7 @@ const ChannelPlan* get_channel_plan(int C, const uint8_t* parity_mask);
 // Parity plan (parity.cu): weight-row / weight-column index tables of the passes of the parity-slot entry points.
 // ---------------------------------------------------------------------------------------------
 struct ParityPlan {
+    int ordinal;     // CUDA device ordinal of `dev`
     int C, N;
     bool message;
     int npass;       // 4 on-site passes (s1, s2), 2 message passes (s_in)

@@ -319,17 +319,6 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
 // ------------------------------------------------------------------------------------------------
 // Host
 // ------------------------------------------------------------------------------------------------
-static int er_num_sms()
-{
-    static int n = 0;
-    if (!n) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-        if (n <= 0) n = 148;
-    }
-    return n;
-}
 
 template <bool ODD, int NSBT, int NA>
 static int launch_ring_t(const EdgeRingArgs& a, size_t smem, int grid, cudaStream_t st)
@@ -417,7 +406,7 @@ int launch_edge_ring(const Plan* p, bool odd, const float* G, const int64_t* row
     a.geo_bytes = (int)geo_bytes;
     const size_t smem = fixed + (size_t)NST * stage_bytes;
     const int64_t nitems = nodes * nblk;
-    const int grid = (int)std::min<int64_t>(nitems, er_num_sms());
+    const int grid = (int)std::min<int64_t>(nitems, num_sms());
 
     LaunchScope scope(odd ? K_EDGE_ODD : K_EDGE_EVEN, st);
     int rc = CGTP_OK;

@@ -342,7 +342,7 @@ int launch_edge(const Plan* p, bool odd, const float* G, const int64_t* row_ptr,
                 int64_t nodes, const int32_t* status, cudaStream_t st)
 {
     if (Cpar <= 0 || nodes <= 0) return CGTP_OK;
-    {
+    if (!(kernel_path() & PATH_GENERIC_EDGE)) {
         bool handled = false;
         const int rc = launch_edge_ring(p, odd, G, row_ptr, edge_index, E, edge_vec, edge_radial, perm_par, Cpar, C, S,
                                         nodes, status, st, &handled);
@@ -355,9 +355,6 @@ int launch_edge(const Plan* p, bool odd, const float* G, const int64_t* row_ptr,
     int cb = (Cpar + nblk - 1) / nblk;
     const int nf = odd ? 2 : 1;
     size_t smem = (size_t)EDGE_EC * nf * p->UVp * 4 + (size_t)round_up(EDGE_EC * cb, 4) * 4 + EDGE_EC * 8;
-    if (nodes > 65535) {
-        // blockIdx.y limit: fold receivers into x instead
-    }
     dim3 grid(nblk, 1, 1);
     LaunchScope scope(odd ? K_EDGE_ODD : K_EDGE_EVEN, st);
     // receivers go on grid.y (max 65535) in slabs

@@ -39,6 +39,7 @@ struct CoreTab {
 };
 
 struct CorePlan {
+    int dev;  // CUDA device ordinal of `blob`
     int lmax, lmax_out;
     bool odd;
     CoreTab tab;
@@ -115,7 +116,7 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
 {
     std::lock_guard<std::mutex> lk(g_core_mu);
     for (CorePlan* c : g_core_plans)
-        if (c->lmax == p->lmax && c->lmax_out == p->lmax_out && c->odd == odd) return c;
+        if (c->dev == p->dev && c->lmax == p->lmax && c->lmax_out == p->lmax_out && c->odd == odd) return c;
 
     const int LB = p->LB, U = p->U, Uh = p->Uh, V = p->V, Vh = p->Vh;
     const int LL = LB + 1;
@@ -237,6 +238,7 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
         return nullptr;
     }
     CorePlan* c = new CorePlan;
+    c->dev = p->dev;
     c->lmax = p->lmax;
     c->lmax_out = p->lmax_out;
     c->odd = odd;
@@ -730,17 +732,6 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
 // ------------------------------------------------------------------------------------------------
 // Launch
 // ------------------------------------------------------------------------------------------------
-static int g_num_sms = 0;
-static int num_sms()
-{
-    if (!g_num_sms) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
-        if (g_num_sms <= 0) g_num_sms = 148;
-    }
-    return g_num_sms;
-}
 
 constexpr size_t kSmemPerSm = 227 * 1024;
 

@@ -60,9 +60,10 @@ static std::vector<ParityPlan*> g_pp;
 
 const ParityPlan* get_parity_plan(int C, int N, bool message)
 {
+    const int ordinal = current_device();
     std::lock_guard<std::mutex> lock(g_pp_mutex);
     for (ParityPlan* q : g_pp)
-        if (q->C == C && q->N == N && q->message == message) return q;
+        if (q->ordinal == ordinal && q->C == C && q->N == N && q->message == message) return q;
     const int npass = message ? 2 : 4;
     std::vector<int> h((size_t)npass * 8 * C);
     for (int ps = 0; ps < npass; ++ps)
@@ -79,6 +80,7 @@ const ParityPlan* get_parity_plan(int C, int N, bool message)
         return nullptr;
     }
     ParityPlan* q = new ParityPlan;
+    q->ordinal = ordinal;
     q->C = C;
     q->N = N;
     q->message = message;

@@ -161,7 +161,7 @@ int launch_proj(const ProjArgs* args_in, int nargs_in, Kind kind, cudaStream_t s
         const int rc = launch_proj_tc(args, nargs, kind, st, &handled);
         if (rc != CGTP_OK || handled) return rc;
     }
-    {
+    if (!(kernel_path() & PATH_GENERIC_PROJ)) {
         bool handled = false;
         const int rc = launch_proj_fast(args, nargs, kind, st, &handled);
         if (rc != CGTP_OK || handled) return rc;

@@ -301,17 +301,6 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
 // ------------------------------------------------------------------------------------------------
 // Host: configuration search and launch
 // ------------------------------------------------------------------------------------------------
-static int pf_num_sms()
-{
-    static int n = 0;
-    if (!n) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-        if (n <= 0) n = 148;
-    }
-    return n;
-}
 
 static inline bool al16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
@@ -372,7 +361,7 @@ int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st
         }
     }
     if (best < 0.0) return CGTP_OK;
-    const int slots_total = pf_num_sms();
+    const int slots_total = num_sms();
 
     // Window tiles: a tile is CWT consecutive flattened (atom, j) columns, so every tile is full and atoms straddle
     // tile boundaries; the stage then holds every atom the window touches (up to ABw).  Taken when it saves rounds of
@@ -425,7 +414,7 @@ int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st
     a.jmagic = (uint32_t)((1ull << 32) / (uint64_t)J) + 1u;
     const size_t smem = 64 + wbytes + (size_t)bNS * a.stage_floats * 4;
     const int ctas_per_sm = 1;
-    const int slots = pf_num_sms() * ctas_per_sm;
+    const int slots = num_sms() * ctas_per_sm;
 
     // split the CTAs among (problem, row block) in proportion to their work (~ K per row block)
     int nrb[2] = {0, 0}, tot_rb = 0;

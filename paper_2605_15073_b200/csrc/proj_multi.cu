@@ -295,17 +295,6 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_multi_kernel(const __grid_
 // ------------------------------------------------------------------------------------------------
 // Host
 // ------------------------------------------------------------------------------------------------
-static int pm_num_sms()
-{
-    static int n = 0;
-    if (!n) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-        if (n <= 0) n = 148;
-    }
-    return n;
-}
 
 static inline bool pm_al16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
@@ -389,7 +378,7 @@ int launch_proj_multi(const ProjArgs* args, int nargs, Kind kind, cudaStream_t s
     a.stage_floats = maxAB * bKC * x_rs;
     const size_t smem = 64 + wbytes + (size_t)bNS * a.stage_floats * 4;
     if (smem > budget) return CGTP_OK;
-    const int slots = pm_num_sms();
+    const int slots = num_sms();
     int begin = 0;
     for (int i = 0; i < nargs; ++i) {
         PmProblem& q = a.p[i];

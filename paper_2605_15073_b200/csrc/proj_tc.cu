@@ -347,17 +347,6 @@ static int g_math_mode = 0;
 void set_math_mode(int m) { g_math_mode = m; }
 int get_math_mode() { return g_math_mode; }
 
-static int tc_num_sms()
-{
-    static int n = 0;
-    if (!n) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-        if (n <= 0) n = 148;
-    }
-    return n;
-}
 
 // *handled = false: not in a tensor-core math mode, or the shapes do not fit (caller uses the FP32 kernels).
 int launch_proj_tc(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st, bool* handled)
@@ -403,7 +392,7 @@ int launch_proj_tc(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st, 
     a.tmem_cols = tmem_cols;
     const size_t smem = 128 + (size_t)nsplit * Kpad * Npad * 4 + (size_t)TC_STAGES * nsplit * KC * TC_COLS * 4;
     const int64_t ntiles = (batch * (int64_t)J + TC_COLS - 1) / TC_COLS;
-    const int slots = tc_num_sms();
+    const int slots = num_sms();
     double wsum = 0.0;
     for (int i = 0; i < nargs; ++i) wsum += args[i].K;
     int begin = 0;

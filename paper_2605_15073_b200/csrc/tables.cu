@@ -26,6 +26,26 @@ void set_error(const char* fmt, ...)
 void clear_error() { g_err[0] = 0; }
 const char* last_error() { return g_err; }
 
+// ------------------------------------------------------------------- per-device facts, path switch
+static std::mutex g_dev_mu;
+static int g_sms[64] = {0};
+int num_sms()
+{
+    const int dev = current_device();
+    if (dev < 0 || dev >= 64) return 148;
+    std::lock_guard<std::mutex> lk(g_dev_mu);
+    if (!g_sms[dev]) {
+        int n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+        g_sms[dev] = n;
+    }
+    return g_sms[dev];
+}
+
+static int g_kernel_path = 0;
+int kernel_path() { return g_kernel_path; }
+void set_kernel_path(int flags) { g_kernel_path = flags; }
+
 // --------------------------------------------------------------------------- launch accounting
 static std::mutex g_prof_mu;
 static int64_t g_launches = 0;
@@ -170,12 +190,14 @@ const Plan* get_plan(int lmax, int lmax_out) { return get_plan_nu(lmax, lmax_out
 
 const Plan* get_plan_nu(int lmax, int lmax_out, int nu)
 {
+    const int dev = current_device();
     std::lock_guard<std::mutex> lk(g_plan_mu);
     for (Plan* p : g_plans)
-        if (p->lmax == lmax && p->lmax_out == lmax_out && p->nu == nu) return p;
+        if (p->dev == dev && p->lmax == lmax && p->lmax_out == lmax_out && p->nu == nu) return p;
 
     Plan* p = new Plan;
     std::memset(p, 0, sizeof *p);
+    p->dev = dev;
     p->lmax = lmax;
     p->lmax_out = lmax_out;
     p->nu = nu;
@@ -283,11 +305,13 @@ static std::vector<ChanEntry*> g_chans;
 
 const ChannelPlan* get_channel_plan(int C, const uint8_t* mask)
 {
+    const int dev = current_device();
     std::lock_guard<std::mutex> lk(g_chan_mu);
     for (ChanEntry* e : g_chans)
-        if (e->plan.C == C && std::memcmp(e->mask.data(), mask, C) == 0) return &e->plan;
+        if (e->plan.dev == dev && e->plan.C == C && std::memcmp(e->mask.data(), mask, C) == 0) return &e->plan;
     ChanEntry* e = new ChanEntry;
     e->mask.assign(mask, mask + C);
+    e->plan.dev = dev;
     e->plan.C = C;
     int k = 0;
     for (int c = 0; c < C; ++c)

@@ -9,14 +9,9 @@ from oracle import cgtp_oracle as orc
 from paper_2605_15073_b200 import binding as cg
 from paper_2605_15073_b200 import synthetic
 from tests import shref
+from tests.parity_util import TOL, cuda as _cuda, sample_rows, sector_errs
 
 pytestmark = pytest.mark.gpu
-
-TOL = 1e-5
-
-
-def _cuda(a):
-    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
 def run_field(m, XE, W_edge, **kw):
@@ -31,19 +26,8 @@ def oracle_field(m, XE, W_edge):
 
 
 def sector_err(got, ref):
-    """max|got - ref| / max|ref| per sector; a sector that vanishes identically in the reference (the curl pairing has
-    no l = 0 component, so the odd sector is zero at lmax_out = 0) is measured against the norm of the whole output."""
-    errs = []
-    whole = np.abs(ref).max()
-    for s in range(2):
-        den = np.abs(ref[:, s]).max()
-        if den == 0.0:
-            den = whole
-        if den > 0:
-            errs.append(np.abs(got[:, s].astype(np.float64) - ref[:, s]).max() / den)
-        else:
-            assert np.abs(got[:, s]).max() == 0.0
-    return max(errs) if errs else 0.0
+    """max over the sectors of the R14 / R22 error norm (tests/parity_util.py)."""
+    return max(sector_errs(got, ref))
 
 
 def _ragged(nodes, hi, seed):
@@ -160,8 +144,7 @@ def test_field_full_size_bench_configuration_sampled_receivers():
     m = synthetic.make_message(lmax, lmax, N, C, nodes, degree, seed=0)
     XE, W_edge = synthetic.make_edge_field(m, Ne, seed=0)
     got = run_field(m, XE, W_edge, check=True)
-    rng = np.random.default_rng(0)
-    recv = np.unique(np.concatenate([[0, nodes - 1], np.arange(0, nodes, 257), rng.integers(0, nodes, 6)]))
+    recv = sample_rows(nodes, 128, seed=0)
     keep = np.isin(m.edge_index[1], recv)
     ref = orc.message_field(m.node_feats, m.edge_index[:, keep], XE[keep], W_edge, m.W_node, m.W_out, lmax, lmax,
                             m.parity_mask)
@@ -204,14 +187,16 @@ def test_field_lw_vs_oracle(lmax, lmax_out, N, Ne, C, nodes):
 
 def test_field_configs4_graph_sampled_receivers():
     """The graph of BASELINE.json configs[4] (16384 nodes, 524288 edges, lmax 8, N = C = 128, half odd) with an edge
-    field of 8 channels: 16 edge chunks, 16-column groups reading the sender's field in place; sampled receivers
+    field of 8 channels: 16 edge chunks, 16-column groups reading the sender's field in place; >= 128 sampled receivers
     against the oracle on the edge list restricted to them."""
     lmax, N, Ne, C, nodes, degree = 8, 128, 8, 128, 16384, 32
     m = synthetic.make_message(lmax, lmax, N, C, nodes, degree, r_max=6.0, seed=0)
     XE, W_edge = synthetic.make_edge_field(m, Ne, seed=0)
     got = run_field(m, XE, W_edge, check=True)
-    rng = np.random.default_rng(1)
-    recv = np.unique(np.concatenate([[0, 1023, 1024, nodes - 1], rng.integers(0, nodes, 4)]))  # 1023 | 1024: a chunk boundary
+    # >= 128 receivers (SURVEY.md 8(c)), both sides of every chunk boundary (chunks of 2^22 / C = 32768 edges = 1024 receivers)
+    bounds = [b + d for b in range(1024, nodes, 1024) for d in (-1, 0)]
+    recv = sample_rows(nodes, 128, seed=1, extra=bounds)
+    assert recv.size >= 128
     keep = np.isin(m.edge_index[1], recv)
     ref = orc.message_field(m.node_feats, m.edge_index[:, keep], XE[keep], W_edge, m.W_node, m.W_out, lmax, lmax,
                             m.parity_mask)

@@ -11,24 +11,9 @@ from oracle import cgtp_oracle as orc
 from paper_2605_15073_b200 import binding as cg
 from paper_2605_15073_b200 import synthetic
 from tests import shref
+from tests.parity_util import TOL, cuda as _cuda, sector_errs as sector_err
 
 pytestmark = pytest.mark.gpu
-
-TOL = 1e-5
-
-
-def _cuda(a):
-    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
-
-
-def sector_err(got, ref):
-    got = np.asarray(got, np.float64)
-    errs = []
-    for s in (0, 1):
-        d = np.abs(got[:, s] - ref[:, s]).max() if got.size else 0.0
-        m = np.abs(ref[:, s]).max() if ref.size else 0.0
-        errs.append(d / m if m > 0 else d)
-    return errs
 
 
 def run_onsite(inp, **kw):
@@ -110,24 +95,6 @@ def test_onsite_window_tiles_ragged(lmax, N, C, batch):
     got, ref = run_onsite(inp), oracle_onsite(inp)
     e = sector_err(got, ref)
     assert max(e) < TOL, e
-
-
-@pytest.mark.parametrize("lmax", [2, 4, 8, 12, 16, 20])
-def test_onsite_config3_sweep_sampled(lmax):
-    """BASELINE.json configs[3]: N=C=32, batch=16384 on the GPU; the oracle evaluates a deterministic
-    sample of atoms (first, last, strided, seeded random)."""
-    inp = synthetic.config(3, lmax=lmax)
-    got = run_onsite(inp)
-    n = {2: 512, 4: 512, 8: 256, 12: 128, 16: 64, 20: 48}[lmax]
-    rng = np.random.default_rng(lmax)
-    idx = np.unique(np.concatenate([[0, 1, inp.batch - 1, inp.batch - 2], np.arange(0, inp.batch, inp.batch // (n // 2)),
-                                    rng.integers(0, inp.batch, n // 2)]))
-    ref = oracle_onsite(inp, idx)
-    e = sector_err(got[idx], ref)
-    assert max(e) < TOL, e
-    assert np.isfinite(got).all()
-    # the whole batch has the same statistics as the checked sample (catches tiles that were never written)
-    assert abs(np.abs(got[:, 0]).mean() / np.abs(got[idx][:, 0]).mean() - 1) < 0.2
 
 
 def test_onsite_invariants_full_size():
@@ -276,20 +243,6 @@ def test_message_config2_full_even_and_halfhalf():
     got, ref = run_message(m, check=True), oracle_message(m)
     e = sector_err(got, ref)
     assert max(e) < TOL, e
-
-
-def test_message_config4_sampled():
-    """BASELINE.json configs[4]: 16384 nodes x 32 in-edges, lmax=8, N=C=128, half odd channels; the oracle
-    evaluates a deterministic sample of receiver segments."""
-    m = synthetic.config(4)
-    got = run_message(m, check=True)
-    rng = np.random.default_rng(4)
-    recv = np.unique(np.concatenate([[0, 1, m.nodes - 1], np.arange(0, m.nodes, m.nodes // 24), rng.integers(0, m.nodes, 24)]))
-    ref = oracle_message(m, recv)
-    e = sector_err(got[recv], ref)
-    assert max(e) < TOL, e
-    assert np.isfinite(got).all()
-    assert abs(np.abs(got[:, 1]).mean() / np.abs(got[recv][:, 1]).mean() - 1) < 0.2
 
 
 def test_message_reproducible_and_graph_error():
