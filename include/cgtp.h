@@ -343,6 +343,8 @@ int cgtp_get_math_mode(void);
  *   CGTP_PATH_GENERIC_SYNTH  M2: node_synth_kernel instead of the lane = column synthesis (sht_fast.cu)
  *   CGTP_PATH_UNFUSED_ONSITE S1-S5: the four-launch on-site step (projection, core per parity, projection) instead of
  *                            the single fused kernel (onsite_fused.cu)
+ *   CGTP_PATH_FUSED_ONSITE   S1-S5: the single fused kernel for every shape it supports, also where the library's own
+ *                            choice is the four-launch step (narrow projections N * C < 4096)
  * Process-wide, read at every call; 0 (default) = every specialised kernel.  CGTP_ERR_INVALID for unknown bits.
  * ------------------------------------------------------------------------------------------- */
 #define CGTP_PATH_GENERIC_CORE 1
@@ -350,6 +352,7 @@ int cgtp_get_math_mode(void);
 #define CGTP_PATH_GENERIC_PROJ 4
 #define CGTP_PATH_GENERIC_SYNTH 8
 #define CGTP_PATH_UNFUSED_ONSITE 16
+#define CGTP_PATH_FUSED_ONSITE 32
 int cgtp_set_kernel_path(int flags);
 int cgtp_get_kernel_path(void);
 

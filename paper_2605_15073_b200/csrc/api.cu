@@ -15,7 +15,8 @@ int profile_collect(double* ms, int64_t* launches);
 
 static const char* kKindNames[K_COUNT] = {
     "proj_in",        "onsite_core_even", "onsite_core_odd", "proj_out",      "segments",      "node_synth_even",
-    "node_synth_odd", "edge_even",        "edge_odd",        "analysis_even", "analysis_odd",  "misc"};
+    "node_synth_odd", "edge_even",        "edge_odd",        "analysis_even", "analysis_odd",  "misc",
+    "onsite_fused"};
 
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 static inline int64_t round_up64(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
@@ -111,6 +112,15 @@ struct OnsitePass {
 static int onsite_pass(const Plan* p, int N, const OnsitePass& q, int64_t batch, void* workspace, cudaStream_t st)
 {
     const int Ce = q.Ce, Co = q.Co;
+    // the whole step in one kernel (onsite_fused.cu) when the shape fits and nothing but the plain contraction is asked
+    if (!(kernel_path() & (PATH_UNFUSED_ONSITE | PATH_GENERIC_CORE | PATH_GENERIC_PROJ)) && get_math_mode() == CGTP_MATH_FP32 &&
+        !q.lw_in && !q.lw_out && q.sigma_C == 0 && !q.accumulate && q.x_bs == (int64_t)N * p->L2 &&
+        q.out_o == q.out_e + (size_t)N * p->Lo2 && q.o_bs == (int64_t)2 * N * p->Lo2) {
+        bool handled = false;
+        const int rc = launch_onsite_fused(p, N, Ce + Co, Ce, Co, q.A, q.B, q.W_a, q.W_b, q.idx_in, q.W_out, q.ldw_out,
+                                           q.idx_out_e, q.idx_out_o, q.out_e, batch, st, &handled);
+        if (rc != CGTP_OK || handled) return rc;
+    }
     // fast core (onsite_core.cu) when both parities fit; it wants odd row strides and 32-column groups
     const bool fast = !(kernel_path() & PATH_GENERIC_CORE) && (Ce == 0 || onsite_fast_supported(p, false)) &&
                       (Co == 0 || onsite_fast_supported(p, true));
@@ -1298,7 +1308,7 @@ int cgtp_get_math_mode(void) { return cgtp::get_math_mode(); }
 int cgtp_set_kernel_path(int flags)
 {
     clear_error();
-    if (flags < 0 || flags > 31) { set_error("unknown kernel-path flags %d", flags); return CGTP_ERR_INVALID; }
+    if (flags < 0 || flags > 63) { set_error("unknown kernel-path flags %d", flags); return CGTP_ERR_INVALID; }
     cgtp::set_kernel_path(flags);
     return CGTP_OK;
 }

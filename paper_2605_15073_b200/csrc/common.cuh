@@ -34,7 +34,7 @@ inline int current_device()
 int num_sms();
 
 // Test-only kernel-path switch (cgtp_set_kernel_path): bit set = take the generic kernel where a specialised one exists.
-enum : int { PATH_GENERIC_CORE = 1, PATH_GENERIC_EDGE = 2, PATH_GENERIC_PROJ = 4, PATH_GENERIC_SYNTH = 8, PATH_UNFUSED_ONSITE = 16 };
+enum : int { PATH_GENERIC_CORE = 1, PATH_GENERIC_EDGE = 2, PATH_GENERIC_PROJ = 4, PATH_GENERIC_SYNTH = 8, PATH_UNFUSED_ONSITE = 16, PATH_FUSED_ONSITE = 32 };
 int kernel_path();
 void set_kernel_path(int flags);
 
@@ -134,6 +134,7 @@ enum Kind {
     K_ANALYSIS_EVEN,
     K_ANALYSIS_ODD,
     K_MISC,
+    K_ONSITE_FUSED,
     K_COUNT
 };
 
@@ -209,6 +210,14 @@ inline int onsite_fast_hstride(const Plan* p) { return p->L2 | 1; }
 inline int onsite_fast_tstride(const Plan* p) { return p->Lo2 | 1; }
 int launch_onsite_fast(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols,
                        cudaStream_t st);
+
+// S1-S5 in one kernel (onsite_fused.cu): reads A, B once, writes out once, H and T stay in shared memory.  idx_in[k] = row
+// of W_a / W_b of internal (parity-sorted) channel k; idx_out_e / idx_out_o = column of W_out of the even / odd channels;
+// `out` must be the dense [batch][2][N][Lo2] block.  *handled = false when the shape does not fit (band limit > 8,
+// lmax_out > lmax, shared memory): the caller runs the four-launch path.
+int launch_onsite_fused(const Plan* p, int N, int C, int Ce, int Co, const float* A, const float* B, const float* W_a,
+                        const float* W_b, const int* idx_in, const float* W_out, int ldw_out, const int* idx_out_e,
+                        const int* idx_out_o, float* out, int64_t batch, cudaStream_t st, bool* handled);
 
 // Same core with factor 2 read through the edge list (two-field coupling, Eq.(28)): column e * cpar + k of
 // Ha pairs with column send[e] * cpar + k of Hn.  *handled = false when the kernel's group width does not divide cpar.

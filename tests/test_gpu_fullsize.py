@@ -59,6 +59,19 @@ def test_onsite_config3_sweep_sampled_oracle_and_full_batch_cross_check(lmax):
     assert torch.isfinite(got).all()
 
 
+@pytest.mark.parametrize("lmax", [2, 4, 8])
+def test_onsite_config3_fused_kernel_whole_batch(lmax):
+    """configs[3] at the band limits the single-kernel step supports, forced (the library's own choice for N = C = 32 is
+    the four-launch step): every element against the default path."""
+    inp = synthetic.config(3, lmax=lmax)
+    A, B = cuda(inp.A), cuda(inp.B)
+    got = onsite_dev(inp, A, B).clone()
+    cg.cgtp_set_kernel_path(cg.PATH_FUSED_ONSITE)
+    alt = onsite_dev(inp, A, B)
+    e = sector_errs_torch(got, alt)
+    assert max(e) < TOL, e
+
+
 def test_onsite_config1_every_kernel_path_agrees():
     """configs[1] (the bench workload; the oracle checks every output in test_gpu_parity.py): fused step, four-launch
     step and the generic kernels agree element by element."""

@@ -79,6 +79,49 @@ def test_onsite_small_shapes(lmax, lmax_out, N, C, batch, mask):
             assert np.abs(got[:, s]).max() == 0.0
 
 
+@pytest.fixture
+def default_path_after():
+    yield
+    cg.cgtp_set_kernel_path(0)
+
+
+@pytest.mark.parametrize("lmax,lmax_out,N,C,batch,mask", [
+    (2, 2, 8, 8, 64, None),                        # configs[0]: 8 atoms per tile, two buffers, all groups per barrier
+    (2, 2, 8, 8, 61, None),                        # ragged last tile
+    (1, 1, 4, 8, 19, [0] * 4 + [1] * 4),           # odd lmax: aligned coefficient rows (L2 = 4)
+    (3, 2, 8, 16, 33, [0] * 8 + [1] * 8),          # lmax_out < lmax, L2 = 16
+    (4, 4, 32, 32, 300, None),                     # configs[3] shape at lmax 4
+    (4, 4, 16, 32, 77, [0] * 24 + [1] * 8),        # unbalanced sectors: 24 pointwise + 8 curl channels
+    (5, 5, 8, 16, 21, [1] * 16),                   # all odd: every warp on the curl sub-group; sector 0 must be zero
+    (6, 6, 8, 16, 21, [0] * 16),                   # all even
+    (6, 6, 64, 64, 301, None),                     # configs[1] shape: tight layout (one A/B buffer under the F planes)
+    (6, 4, 32, 64, 150, None),                     # N != C, lmax_out < lmax
+    (7, 7, 8, 32, 40, None),                       # band 7 on the LB = 8 instantiation, aligned rows (L2 = 64)
+    (8, 8, 8, 16, 30, [0] * 16),                   # band 8 fits with one parity only (the F planes of both do not)
+])
+def test_onsite_fused_kernel_shapes(lmax, lmax_out, N, C, batch, mask, default_path_after):
+    """The single-kernel step (onsite_fused.cu) forced for every shape it supports (CGTP_PATH_FUSED_ONSITE), against the
+    oracle; then the four-launch step on the same inputs (the two must agree to rounding)."""
+    inp = synthetic.make_onsite(lmax, lmax_out, N, C, batch, seed=900 + 10 * lmax + lmax_out, parity_mask=mask)
+    ref = oracle_onsite(inp)
+    cg.cgtp_set_kernel_path(cg.PATH_FUSED_ONSITE)
+    n0 = cg.cgtp_launch_count()
+    got = run_onsite(inp)
+    assert cg.cgtp_launch_count() - n0 == 1  # one launch: the fused kernel took the shape
+    e = sector_err(got, ref)
+    assert max(e) < TOL, e
+    for s in (0, 1):
+        if np.abs(ref[:, s]).max() == 0.0:
+            assert np.abs(got[:, s]).max() == 0.0
+    assert np.array_equal(got, run_onsite(inp))  # bitwise reproducible
+    cg.cgtp_set_kernel_path(cg.PATH_UNFUSED_ONSITE)
+    n0 = cg.cgtp_launch_count()
+    alt = run_onsite(inp)
+    assert cg.cgtp_launch_count() - n0 >= 3
+    e = sector_err(alt, ref)
+    assert max(e) < TOL, e
+
+
 def test_onsite_config1_full():
     """BASELINE.json configs[1] (the bench workload): lmax=6, N=C=64, batch=4096, every output checked."""
     inp = synthetic.config(1)
@@ -136,7 +179,13 @@ def test_onsite_host_entry_matches_device_entry():
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     host = cg.cgtp_onsite_host(pin(inp.A), pin(inp.B), pin(inp.W_a), pin(inp.W_b), pin(inp.W_out), 4, 4, 16, 16,
                                inp.parity_mask).numpy()
-    assert np.array_equal(dev, host)
+    # the host entry works in batch chunks, and the library chooses the kernels per call size (onsite_fused.cu for small
+    # calls): the two results agree to rounding, not bit for bit
+    for s in (0, 1):
+        assert np.abs(dev[:, s] - host[:, s]).max() <= 2e-6 * np.abs(dev[:, s]).max()
+    host2 = cg.cgtp_onsite_host(pin(inp.A), pin(inp.B), pin(inp.W_a), pin(inp.W_b), pin(inp.W_out), 4, 4, 16, 16,
+                                inp.parity_mask).numpy()
+    assert np.array_equal(host, host2)
 
 
 def test_onsite_argument_errors():
