@@ -58,6 +58,7 @@ def onsite_flops_per_atom(lmax, lmax_out, N, C, Ce, Co):
         "onsite_core_odd": Co * (8 * U * L2 + 8 * U * V * M + 3 * U * V + 2 * U * V * Mo + 2 * U * Lo2),
         "proj_out": 2 * N * C * Lo2,
     }
+    k["onsite_fused"] = sum(k.values())  # the single-kernel step (onsite_fused.cu) does all four
     return k
 
 
@@ -250,6 +251,11 @@ def main():
         A, B = sets[i % NSETS]
         cg.cgtp_onsite(A, B, Wa, Wb, Wo, lmax, lmax_out, N, C, mask, out=out)
 
+    # FP32 pipe calibration in the same run: register-only FFMA / FFMA2 chains on every SM
+    ffma_tf, ffma_mhz = cg.cgtp_fma_peak(False, 30.0)
+    ffma2_tf, ffma2_mhz = cg.cgtp_fma_peak(True, 30.0)
+    fp32_peak_measured = max(ffma_tf, ffma2_tf)
+
     sampler = ClockSampler(local_rank).start()
     for i in range(args.warmup):
         step(i)
@@ -285,6 +291,7 @@ def main():
     cg.cgtp_profile_enable(False)
 
     fl = onsite_flops_per_atom(lmax, lmax_out, N, C, Ce, Co)
+    step_flops = fl["proj_in"] + fl["onsite_core_even"] + fl["onsite_core_odd"] + fl["proj_out"]
     sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz", 1965.0)
     fp32_peak_tflops = SM_COUNT * FMA_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     kernels = {}
@@ -299,18 +306,29 @@ def main():
     for name, (ms, cnt) in prof.items():
         kernels[name]["share"] = ms / tot_ms
     dom = max(prof, key=lambda n: prof[n][0])
-    traffic = None
+    traffic = pipe_util = None
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tp):
-        traffic = json.load(open(tp)).get(f"config1:{dom}")
+        tj = json.load(open(tp))
+        traffic = tj.get(f"config1:{dom}")
+        pipe_util = tj.get(f"config1:{dom}:pipe_util")
     roofline = {
         "kernel": dom, "bound": "alu", "achieved": kernels[dom]["alg_tflops"], "peak": fp32_peak_tflops,
         "unit": "TFLOP/s", "frac": kernels[dom]["alg_tflops"] / fp32_peak_tflops, "traffic": traffic,
         "peak_source": f"derived: {SM_COUNT} SMs x {FMA_LANES_PER_SM} FP32 FMA lanes x 2 x {sm_max:.0f} MHz (DESIGN.md)",
+        "peak_measured": fp32_peak_measured,
+        "peak_measured_source": "cgtp_fma_peak in this run: register-only dependent chains on every SM, 30 ms each: "
+                                f"FFMA {ffma_tf:.1f} TFLOP/s (= {ffma_mhz:.0f} MHz x 148 x 128 x 2), FFMA2 {ffma2_tf:.1f} TFLOP/s",
+        "frac_of_measured": kernels[dom]["alg_tflops"] / fp32_peak_measured,
+        "pipe_util": pipe_util,
+        "pipe_util_definition": "ncu counters of the kept capture of this kernel (file named inside): FMA-pipe cycles "
+                                "active, issue slots used, shared-memory wavefronts -- `frac` counts the paper's dense "
+                                "transforms, the kernel folds symmetries, so frac > pipe utilisation is expected",
         "achieved_definition": "algorithmic FP32 flops of this kernel per launch (SURVEY.md 8(d) formula, dense DFT, "
                                "no symmetry folding) / mean CUDA-event duration",
-        "step_alg_tflops": sum(fl.values()) * batch / (ms_per_step * 1e-3) / 1e12,
-        "step_frac_fp32_peak": sum(fl.values()) * batch / (ms_per_step * 1e-3) / 1e12 / fp32_peak_tflops,
+        "step_alg_tflops": step_flops * batch / (ms_per_step * 1e-3) / 1e12,
+        "step_frac_fp32_peak": step_flops * batch / (ms_per_step * 1e-3) / 1e12 / fp32_peak_tflops,
+        "step_frac_of_measured": step_flops * batch / (ms_per_step * 1e-3) / 1e12 / fp32_peak_measured,
         "step_hbm_gbs_algorithmic": onsite_bytes_per_atom(lmax, lmax_out, N) * batch / (ms_per_step * 1e-3) / 1e9,
         "hbm_peak_gbs": peaks["hbm_gbs"], "hbm_peak_source": peak_src,
     }
@@ -344,8 +362,13 @@ def main():
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "kernels": kernels,
     }
 
+    # ------------------------------------------------------------------ receiver-sharded message passing (every N)
+    if not args.no_extras:
+        line["message_sharded"] = run_message_sharded(args, cg, synthetic, dev, rank, world, peaks, barrier, max_over_ranks)
+
     # ------------------------------------------------------------------ extras (rank 0, 1 GPU)
     if world == 1 and not args.no_extras:
+        sampler2 = ClockSampler(local_rank, period=0.05).start()  # the extras get their own clock record
         rate, dt_cpu, cores = oracle_onsite_rate(base, batch)
         line["cpu_baseline"] = {"value": rate, "unit": "contractions/s", "cores": cores, "kind": "oracle",
                                 "sample": f"all {batch} atoms of configs[1] once ({dt_cpu:.1f} s wall)"}
@@ -356,6 +379,8 @@ def main():
         line["l_dependent_weights"] = run_lw(args, cg, synthetic, dev, ms_per_step)
         line["nbody"] = run_nbody(args, cg, synthetic, dev, fp32_peak_tflops)
         line["edge_field"] = run_edge_field(args, cg, synthetic, dev, fp32_peak_tflops)
+        line["unfused_onsite"] = run_unfused(args, cg, step, fl, batch, fp32_peak_tflops, fp32_peak_measured)
+        line["clocks_extras"] = sampler2.stop()
     elif world == 1:
         rate, dt_cpu, cores = oracle_onsite_rate(base, 1024)
         line["cpu_baseline"] = {"value": rate, "unit": "contractions/s", "cores": cores, "kind": "oracle",
@@ -379,6 +404,88 @@ def time_steps(fn, steps, warmup):
     ev1.record()
     torch.cuda.synchronize()
     return ev0.elapsed_time(ev1) / steps
+
+
+def run_message_sharded(args, cg, synthetic, dev, rank, world, peaks, barrier, max_over_ranks):
+    """BASELINE.json configs[4] split over the ranks by receivers: every rank owns a
+    contiguous receiver range, its in-edges and its rows of node_feats; one all-gather of node_feats (NCCL), then
+    cgtp_message_bipartite over the local in-edges.  Strong scaling: the graph is fixed, edges/s = E / max-over-ranks
+    time of (all-gather + kernels).  At N = 1 the all-gather is the identity and the call is cgtp_message itself."""
+    import torch
+    import torch.distributed as dist
+    from paper_2605_15073_b200 import parallel
+    m = synthetic.config(4)
+    rp = parallel.row_ptr_from_receivers(m.edge_index[1], m.nodes)
+    bounds = parallel.shard_receivers(rp, world)
+    t = torch.from_numpy
+    sh = parallel.make_shard(t(m.node_feats), t(m.edge_index), t(m.edge_vec), t(m.edge_radial), bounds, rank, row_ptr=rp)
+    local = sh.node_feats.to(dev)
+    ei, ev, er = sh.edge_index.to(dev), sh.edge_vec.to(dev), sh.edge_radial.to(dev)
+    Wn, Wo = t(m.W_node).to(dev), t(m.W_out).to(dev)
+    feats = torch.empty((m.nodes, m.N, (m.lmax + 1) ** 2), device=dev)
+    out = torch.empty((sh.hi - sh.lo, 2, m.N, (m.lmax_out + 1) ** 2), device=dev)
+    steps = max(3, min(args.steps, 10))
+    ev_a0, ev_a1, ev_k1 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+    ag_ms, tot_ms = [], []
+
+    def one(timed):
+        ev_a0.record()
+        full = parallel.all_gather_node_feats(local, bounds, out=feats) if world > 1 else local
+        ev_a1.record()
+        cg.cgtp_message_bipartite(full, ei, ev, er, Wn, Wo, m.lmax, m.lmax_out, m.N, m.C, m.parity_mask, sh.hi - sh.lo, out=out)
+        ev_k1.record()
+        if timed:
+            torch.cuda.synchronize()
+            ag_ms.append(ev_a0.elapsed_time(ev_a1))
+            tot_ms.append(ev_a0.elapsed_time(ev_k1))
+    for _ in range(3):
+        one(False)
+    for _ in range(steps):
+        barrier()
+        one(True)
+    step_ms = max_over_ranks(float(np.mean(tot_ms)))
+    gather_ms = max_over_ranks(float(np.mean(ag_ms)))
+    gathered_bytes = feats.numel() * 4 * (world - 1) / max(world, 1)  # bytes every rank receives
+    return {"workload": f"BASELINE.json configs[4] over {world} receiver shard(s): nodes={m.nodes} E={m.E}, rank 0 owns "
+                        f"receivers [{int(bounds[0])}, {int(bounds[1])}) with {int(ei.shape[1])} in-edges",
+            "scaling": "strong", "ranks": world,
+            "backend": dist.get_backend() if world > 1 else "none (single process)",
+            "ms_per_step": step_ms, "edges_per_s": m.E / (step_ms * 1e-3),
+            "all_gather_ms": gather_ms,
+            "all_gather_gbs_per_rank": (gathered_bytes / (gather_ms * 1e-3) / 1e9) if world > 1 and gather_ms > 0 else None,
+            "all_gather_bytes_per_rank": int(gathered_bytes), "steps": steps,
+            "timing": "CUDA events on the launch stream around all-gather + kernels, mean over steps, max over ranks"}
+
+
+def run_unfused(args, cg, step, fl, batch, fp32_peak_tflops, fp32_peak_measured):
+    """configs[1] through the four-launch step (proj_fast + onsite_core x 2 + proj_fast), forced with
+    CGTP_PATH_UNFUSED_ONSITE: what the single-kernel step is measured against."""
+    import torch
+    try:
+        cg.cgtp_set_kernel_path(cg.PATH_UNFUSED_ONSITE)
+        it = [0]
+
+        def fn():
+            it[0] += 1
+            step(it[0])
+        ms = time_steps(fn, max(args.steps // 2, 5), 3)
+        cg.cgtp_profile_enable(True)
+        for _ in range(20):
+            fn()
+        torch.cuda.synchronize()
+        prof = cg.cgtp_profile_collect()
+        cg.cgtp_profile_enable(False)
+    finally:
+        cg.cgtp_set_kernel_path(0)
+    kern = {}
+    for k, (kms, cnt) in prof.items():
+        a = kms / cnt
+        kern[k] = {"avg_ms": a}
+        if k in fl:
+            kern[k]["alg_tflops"] = fl[k] * batch / (a * 1e-3) / 1e12
+            kern[k]["frac_fp32_peak"] = kern[k]["alg_tflops"] / fp32_peak_tflops
+            kern[k]["frac_of_measured"] = kern[k]["alg_tflops"] / fp32_peak_measured
+    return {"ms_per_step": ms, "contractions_per_s": batch / (ms * 1e-3), "kernels": kern}
 
 
 def run_tensor_core(args, cg, step, out, lmax, lmax_out, N, C, Ce, Co, batch, peaks, peak_src):
@@ -447,7 +554,7 @@ def run_sweep(args, cg, synthetic, dev, fp32_peak_tflops, peaks):
         prof = cg.cgtp_profile_collect()
         cg.cgtp_profile_enable(False)
         fls = onsite_flops_per_atom(lmax, lmax, N, C, C // 2, C // 2)
-        fl = sum(fls.values())
+        fl = fls["onsite_fused"]
         by = onsite_bytes_per_atom(lmax, lmax, N)
         res.append({"lmax": lmax, "ms_per_step": ms, "contractions_per_s": batch / (ms * 1e-3),
                     "kernel_ms": {k: v[0] / v[1] * (v[1] / steps) for k, v in prof.items()},
@@ -475,7 +582,7 @@ def run_message(args, cg, synthetic, dev, peaks, peak_src):
         Wn, Wo = cu(m.W_node), cu(m.W_out)
         out = torch.empty((m.nodes, 2, m.N, (m.lmax_out + 1) ** 2), device=dev)
         fn = lambda: cg.cgtp_message(X, ei, ev, er, Wn, Wo, m.lmax, m.lmax_out, m.N, m.C, m.parity_mask, out=out)
-        steps = 10 if idx == 2 else 3
+        steps = max(3, min(args.steps, 50 if idx == 2 else 10))
         ms = time_steps(fn, steps, 3)
         cg.cgtp_profile_enable(True)
         for _ in range(steps):
@@ -506,6 +613,17 @@ def run_message(args, cg, synthetic, dev, peaks, peak_src):
                          "peak_source": peak_src, "traffic": ncu_traffic.get(f"config{idx}:{dom}") if halfhalf else None},
             "kernels": kern,
         }
+        if idx == 2:
+            # the node-grid table the edges gather from (95 MB) is written by M2 in the same step and stays in the 126 MB
+            # L2 (SURVEY.md 8(d) says so): the gather is an L2 read, the algorithmic rate is not an HBM measurement
+            r = res[name]["roofline"]
+            r.update({"bound": "l2", "peak": None, "frac": None, "peak_source": None,
+                      "note": "gathered table is L2-resident; `achieved` = algorithmic gather bytes / time; the ncu "
+                              "capture (lts__t_bytes, dram__bytes) is in profiles/, see traffic.json",
+                      "traffic": ncu_traffic.get(f"config2:{dom}"), "l2_bytes": ncu_traffic.get(f"config2:{dom}:lts_bytes")})
+            for kk in kern.values():
+                kk.pop("frac_hbm_peak", None)
+            res[name].pop("frac_hbm_peak_whole_step", None)
         del X, ei, ev, er, out
         torch.cuda.empty_cache()
     return res

@@ -80,39 +80,68 @@ class MessageShard:
     node_feats: torch.Tensor   # [hi - lo, N, (lmax+1)^2]
 
 
+def row_ptr_on_device(receivers: torch.Tensor, nodes: int) -> torch.Tensor:
+    """CSR offsets of a receiver-sorted edge list, computed where the list lives (no host copy)."""
+    probe = torch.arange(nodes + 1, dtype=torch.int64, device=receivers.device)
+    return torch.searchsorted(receivers.contiguous(), probe, right=False)
+
+
 def make_shard(node_feats: torch.Tensor, edge_index: torch.Tensor, edge_vec: torch.Tensor,
-               edge_radial: torch.Tensor, bounds: Sequence[int], rank: int) -> MessageShard:
+               edge_radial: torch.Tensor, bounds: Sequence[int], rank: int, row_ptr=None) -> MessageShard:
     """Cuts rank `rank`'s shard out of a full (replicated) problem; used by tests and by callers that
-    load the whole graph on every rank."""
+    load the whole graph on every rank.  `row_ptr` (device or host, int64 [nodes+1]) is reused when given; otherwise the
+    two offsets the shard needs are found on the device the edge list lives on."""
     nodes = node_feats.shape[0]
-    rp = row_ptr_from_receivers(edge_index[1].cpu().numpy(), nodes)
     lo, hi = int(bounds[rank]), int(bounds[rank + 1])
-    e0, e1 = local_edge_slice(rp, lo, hi)
+    if row_ptr is None:
+        probe = torch.tensor([lo, hi], dtype=torch.int64, device=edge_index.device)
+        e0, e1 = (int(v) for v in torch.searchsorted(edge_index[1].contiguous(), probe, right=False).tolist())
+    else:
+        e0, e1 = int(row_ptr[lo]), int(row_ptr[hi])
+    if not (0 <= lo <= hi <= nodes):
+        raise ValueError("receiver bounds outside [0, nodes]")
     ei = edge_index[:, e0:e1].clone()
     ei[1] -= lo
     return MessageShard(lo, hi, ei.contiguous(), edge_vec[e0:e1].contiguous(), edge_radial[e0:e1].contiguous(),
                         node_feats[lo:hi].contiguous())
 
 
-def all_gather_node_feats(local: torch.Tensor, bounds: Sequence[int], group=None) -> torch.Tensor:
+def all_gather_node_feats(local: torch.Tensor, bounds: Sequence[int], group=None, out: Optional[torch.Tensor] = None) -> torch.Tensor:
     """All-gather of the per-rank node-feature blocks into [nodes, N, L^2] (the one exchange step).
 
-    Ranges may differ in length, so every rank pads its block to the longest range, one
-    all_gather_into_tensor moves the padded blocks (NCCL on GPUs, gloo on CPU), and the padding is
-    dropped on arrival."""
+    The blocks land directly in their rows of the result: one all_gather_into_tensor when every range has the same
+    length (the balanced case), else one all_gather over views of the result with per-rank lengths (NCCL moves uneven
+    blocks as grouped broadcasts).  Only the gloo backend (CPU tests) needs equal blocks and goes through a padded
+    staging copy.  A single process (no process group) has nothing to exchange."""
+    if not (dist.is_available() and dist.is_initialized()):
+        if local.shape[0] != int(bounds[-1] - bounds[0]):
+            raise ValueError("local block does not match the receiver bounds")
+        return local
     world = dist.get_world_size(group)
     rank = dist.get_rank(group)
     sizes = [int(bounds[r + 1] - bounds[r]) for r in range(world)]
     if local.shape[0] != sizes[rank]:
         raise ValueError("local block does not match the receiver bounds")
-    longest = max(max(sizes), 1)
     tail = tuple(local.shape[1:])
+    if out is None:
+        out = local.new_empty((sum(sizes),) + tail)
+    if len(set(sizes)) == 1:
+        dist.all_gather_into_tensor(out, local.contiguous(), group=group)
+        return out
+    if dist.get_backend(group) != "gloo":
+        dist.all_gather(list(out.split(sizes, dim=0)), local.contiguous(), group=group)
+        return out
+    longest = max(max(sizes), 1)
     send = local.new_zeros((longest,) + tail)
     send[: sizes[rank]] = local
     recv = local.new_empty((world * longest,) + tail)
     dist.all_gather_into_tensor(recv, send, group=group)
     recv = recv.view((world, longest) + tail)
-    return torch.cat([recv[r, : sizes[r]] for r in range(world)], dim=0)
+    off = 0
+    for r in range(world):
+        out[off: off + sizes[r]] = recv[r, : sizes[r]]
+        off += sizes[r]
+    return out
 
 
 def message_sharded(shard: MessageShard, bounds: Sequence[int], W_node: torch.Tensor, W_out: torch.Tensor,
@@ -143,10 +172,9 @@ class FieldShard:
 
 def make_field_shard(node_feats: torch.Tensor, edge_index: torch.Tensor, edge_feats: torch.Tensor,
                      bounds: Sequence[int], rank: int) -> FieldShard:
-    nodes = node_feats.shape[0]
-    rp = row_ptr_from_receivers(edge_index[1].cpu().numpy(), nodes)
     lo, hi = int(bounds[rank]), int(bounds[rank + 1])
-    e0, e1 = local_edge_slice(rp, lo, hi)
+    probe = torch.tensor([lo, hi], dtype=torch.int64, device=edge_index.device)
+    e0, e1 = (int(v) for v in torch.searchsorted(edge_index[1].contiguous(), probe, right=False).tolist())
     ei = edge_index[:, e0:e1].clone()
     ei[1] -= lo
     return FieldShard(lo, hi, ei.contiguous(), edge_feats[e0:e1].contiguous(), node_feats[lo:hi].contiguous())
