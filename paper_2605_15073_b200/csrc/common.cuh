@@ -75,6 +75,9 @@ struct Plan {
     const float* WV;  // [round_up(Vh,4)]: (2 pi / V), halved for self-mirrored v'   (Eq.(39), :339)
     // Grid geometry for the edge factor, [8][UVp]: Omega_xyz, theta_hat_xyz, phi_hat_xy (zero padded)
     const float* geo;
+    // host copies of QC, QS, WV: kernels that take the azimuthal tables as kernel parameters (constant bank, read on the
+    // uniform datapath instead of through shared memory) copy them from here
+    const float *hQC, *hQS, *hWV;
 };
 
 // FP64 host helpers of the table builder (tables.cu), shared with the packed tables of onsite_core.cu.

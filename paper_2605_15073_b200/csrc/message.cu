@@ -12,6 +12,8 @@
 //   K_e(Omega) = sum_{l<=lmax} (2l+1)/(4 pi) P_l(r_e . Omega)     (addition theorem)
 // and for the odd channels its surface gradient in the (theta_hat, phi_hat) frame:
 //   d_theta K_e = k'(t) (r_e . theta_hat),  (1/sin theta) d_phi K_e = k'(t) (r_e . phi_hat),  t = r_e . Omega.
+#include <mutex>
+
 #include "sht.cuh"
 
 namespace cgtp {
@@ -396,9 +398,7 @@ static AnaSmem ana_smem_layout(const Plan* p, bool odd, int NC)
     int off = 0;
     s.bar = off; off += 16;
     s.wp = off; off += nf * s.tab_bytes;
-    s.qc = off; off += s.q_bytes;
-    s.qs = off; off += s.q_bytes;
-    s.wv = off; off += s.wv_bytes;
+    s.qc = s.qs = s.wv = off;  // the azimuthal tables are a kernel parameter (QParam)
     s.ss = off; off += NC * nf * p->UVp * 4;
     s.t = off; off += nf * round_up(M * J, 4) * 4;
     s.total = off;
@@ -406,17 +406,15 @@ static AnaSmem ana_smem_layout(const Plan* p, bool odd, int NC)
 }
 
 template <int LB, bool ODD>
-__global__ void __launch_bounds__(256) analysis_kernel(Plan p, AnaSmem lay, const float* __restrict__ S,
-                                                      float* __restrict__ T, long long ncols, int NC)
+__global__ void __launch_bounds__(256) analysis_kernel(Plan p, AnaSmem lay, const __grid_constant__ QParam<LB> qp,
+                                                      const float* __restrict__ S, float* __restrict__ T, long long ncols,
+                                                      int NC)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int M = 2 * LB + 1;
     constexpr int NF = ODD ? 2 : 1;
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + lay.bar);
     float* wp = reinterpret_cast<float*>(smem + lay.wp);
-    float* qc = reinterpret_cast<float*>(smem + lay.qc);
-    float* qs = reinterpret_cast<float*>(smem + lay.qs);
-    float* wv = reinterpret_cast<float*>(smem + lay.wv);
     float* Ss = reinterpret_cast<float*>(smem + lay.ss);
     float* Tm = reinterpret_cast<float*>(smem + lay.t);
 
@@ -432,7 +430,7 @@ __global__ void __launch_bounds__(256) analysis_kernel(Plan p, AnaSmem lay, cons
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        const uint32_t total = NF * lay.tab_bytes + 2 * lay.q_bytes + lay.wv_bytes + sbytes;
+        const uint32_t total = NF * lay.tab_bytes + sbytes;
         mbar_arrive_expect_tx(bar, total);
         if (!ODD) {
             tma_load_span(wp, p.WP, lay.tab_bytes, bar);
@@ -440,9 +438,6 @@ __global__ void __launch_bounds__(256) analysis_kernel(Plan p, AnaSmem lay, cons
             tma_load_span(wp, p.WD, lay.tab_bytes, bar);
             tma_load_span(wp + lay.tab_bytes / 4, p.WS, lay.tab_bytes, bar);
         }
-        tma_load_span(qc, p.QC, lay.q_bytes, bar);
-        tma_load_span(qs, p.QS, lay.q_bytes, bar);
-        tma_load_span(wv, p.WV, lay.wv_bytes, bar);
         tma_load_span(Ss, S + col0 * NF * p.UVp, sbytes, bar);
     }
     mbar_wait(bar, 0);
@@ -451,7 +446,7 @@ __global__ void __launch_bounds__(256) analysis_kernel(Plan p, AnaSmem lay, cons
     for (int item = threadIdx.x; item < NF * rows; item += blockDim.x) {
         const int f = item / rows, j = item - f * rows;
         const int col = j / p.U, u = j - col * p.U;
-        dft_inverse_row<LB>(Ss + ((size_t)col * NF + f) * p.UVp + u * p.V, Tm + (size_t)f * MJ, J, j, qc, qs, wv, p.V, p.Vh);
+        dft_inverse_row_p<LB>(Ss + ((size_t)col * NF + f) * p.UVp + u * p.V, Tm + (size_t)f * MJ, J, j, qp, p.V, p.Vh);
     }
     __syncthreads();
     if (!ODD)
@@ -482,7 +477,9 @@ static int launch_analysis_t(const Plan* p, const float* S, float* T, int64_t nc
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, lay.total));
     int64_t grid = (ncols + NC - 1) / NC;
     LaunchScope scope(ODD ? K_ANALYSIS_ODD : K_ANALYSIS_EVEN, st);
-    kern<<<(unsigned)grid, 256, lay.total, st>>>(*p, lay, S, T, (long long)ncols, NC);
+    QParam<LB> qp;
+    fill_qparam<LB>(p, qp);
+    kern<<<(unsigned)grid, 256, lay.total, st>>>(*p, lay, qp, S, T, (long long)ncols, NC);
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
 }

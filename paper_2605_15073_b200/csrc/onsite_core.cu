@@ -28,6 +28,7 @@ struct CorePlan {
     bool odd;
     CoreTab tab;
     const void* blob;  // device
+    std::vector<float> QF, QI;  // host copies of the azimuthal tables (kernel parameter CoreQParam)
 };
 
 // Host: packed tables + static schedules
@@ -224,6 +225,8 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
     c->odd = odd;
     c->tab = t;
     c->blob = d;
+    c->QF = QF;
+    c->QI = QI;
     g_core_plans.push_back(c);
     return c;
 }
@@ -249,7 +252,7 @@ struct CoreArgs {
 };
 
 template <int LB, bool ODD>
-__global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
+__global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a, const __grid_constant__ CoreQParam<LB> qp)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int MR = 2 * LB + 1;
@@ -346,7 +349,7 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a)
                 if constexpr (TWO_TERM)
                     stage_b_two_term<LB, RB, GW>(qf, qi, a.tab.QFS, a.tab.QIS, a.tab.SOFF, F, plane, lr, a.Vh, col);
                 else
-                    stage_b<LB, ODD, RB, GW>(qf, qi, a.tab.QFS, a.tab.QIS, a.tab.SOFF, F, plane, lr, a.Vh, col);
+                    stage_b_p<LB, ODD, RB, GW>(qp, F, plane, lr, a.Vh, col);
             }
             // the previous group's bulk store must have finished reading Ts before stage C rewrites it
             if (blk == 0 && threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
@@ -431,8 +434,12 @@ static int launch_fast_t(const Plan* p, const CorePlan* c, const float* Ha, cons
     if (ctas_per_sm < 1) ctas_per_sm = 1;
     int64_t grid = (int64_t)num_sms() * ctas_per_sm;
     if (grid > a.ngroups) grid = a.ngroups;
+    CoreQParam<LB> qp;
+    std::memset(&qp, 0, sizeof qp);
+    std::memcpy(qp.qf, c->QF.data(), std::min(sizeof qp.qf, c->QF.size() * sizeof(float)));
+    std::memcpy(qp.qi, c->QI.data(), std::min(sizeof qp.qi, c->QI.size() * sizeof(float)));
     LaunchScope scope(ODD ? K_ONSITE_ODD : K_ONSITE_EVEN, st);
-    kern<<<(unsigned)grid, 32 * c->tab.NW, smem, st>>>(a);
+    kern<<<(unsigned)grid, 32 * c->tab.NW, smem, st>>>(a, qp);
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
 }

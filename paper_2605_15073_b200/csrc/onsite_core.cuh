@@ -174,6 +174,19 @@ __device__ __forceinline__ void stage_a_odd(const float* __restrict__ ta, int UP
 //   f(phi) = Ce+Co+Se+So,  f(-phi) = Ce+Co-Se-So,  f(pi+phi) = Ce-Co+Se-So,  f(pi-phi) = Ce-Co-Se+So,
 // and the inverse transform needs only  A+-B (cosine rows, even/odd m) and Cd+-D (sine rows) with
 // A = s1+s2, B = s3+s4, Cd = s1-s2, D = s4-s3.  The result rows overwrite plane 0 in place.
+// The azimuthal tables of stage B as a kernel parameter (constant bank): with the row loop fully unrolled every table
+// index is a compile-time constant and the values are operands of the FMAs (uniform registers filled by LDCU), instead
+// of 128-bit broadcast loads from shared memory, which cost two shared-memory wavefronts each -- the shared-memory pipe,
+// not the FMA pipe, bound this stage (ncu: 75 % of the wavefront peak against 52 % FMA-pipe cycles).
+template <int LB>
+struct CoreQParam {
+    static constexpr int QFS = round_up(2 * LB + 1, 4);
+    static constexpr int SOFF = round_up(LB + 1, 2);
+    static constexpr int QIS = round_up(SOFF + LB, 4);
+    static constexpr int NQMAX = round_up(3 * LB + 1, 4) / 4 + 1;  // V4/4 + 1 at lmax = lmax_out = LB
+    float qf[NQMAX * QFS], qi[NQMAX * QIS];
+};
+
 template <int LB, bool ODD, int RB, int GW>
 __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const float* __restrict__ qi, int QFS, int QIS,
                                         int SOFF, float* __restrict__ F, int plane_stride, int lr, int NQ, int lane)
@@ -257,6 +270,98 @@ __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const floa
         for (int k = 0; k < NTC; ++k) tc[k] = ffma2(qc2[k], mc, tc[k]);
 #pragma unroll
         for (int k = 0; k < NTS; ++k) ts[k] = ffma2(qs2[k], ms, ts[k]);
+    }
+#pragma unroll
+    for (int m = 0; m <= LB; ++m) F[(m * RB + lr) * GW + lane] = (m & 1) ? tc[m / 2].y : tc[m / 2].x;
+#pragma unroll
+    for (int m = 1; m <= LB; ++m) F[((LB + m) * RB + lr) * GW + lane] = ((m - 1) & 1) ? ts[(m - 1) / 2].y : ts[(m - 1) / 2].x;
+}
+
+template <int LB, bool ODD, int RB, int GW>
+__device__ __forceinline__ void stage_b_p(const CoreQParam<LB>& qp, float* __restrict__ F, int plane_stride, int lr, int NQ,
+                                          int lane)
+{
+    constexpr int MR = 2 * LB + 1;
+    constexpr int NTC = (LB + 2) / 2;  // pairs of cos rows (m = 2k, 2k+1)
+    constexpr int NTS = (LB + 1) / 2;  // pairs of sin rows (m = 2k+1, 2k+2)
+    constexpr int NP = ODD ? 2 : 1;
+    // f[k][r]: even: k = 0, pair (A, B); odd: k = 0 pair (A_theta, A_phi), k = 1 pair (B_theta, B_phi)
+    float2 f[NP][MR];
+#pragma unroll
+    for (int r = 0; r < MR; ++r) {
+        const int idx = (r * RB + lr) * GW + lane;
+        f[0][r] = make_float2(F[idx], F[idx + plane_stride]);
+        if (ODD) f[NP - 1][r] = make_float2(F[idx + 2 * plane_stride], F[idx + 3 * plane_stride]);
+    }
+    float2 tc[NTC], ts[NTS > 0 ? NTS : 1];
+#pragma unroll
+    for (int k = 0; k < NTC; ++k) tc[k] = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int k = 0; k < NTS; ++k) ts[k] = make_float2(0.f, 0.f);
+
+    constexpr int QFS = CoreQParam<LB>::QFS, QIS = CoreQParam<LB>::QIS, SOFF = CoreQParam<LB>::SOFF;
+    // fully unrolled over the largest table of the band limit: every table index is a compile-time constant, the values
+    // are constant-bank / uniform-register operands of the FMAs
+#pragma unroll
+    for (int vq = 0; vq < CoreQParam<LB>::NQMAX; ++vq) {
+        if (vq >= NQ) break;
+        float2 Ce[NP], Co[NP], Se[NP], So[NP];
+#pragma unroll
+        for (int k = 0; k < NP; ++k) Ce[k] = Co[k] = Se[k] = So[k] = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int r = 0; r < MR; r += 4) {
+            const float qv[4] = {qp.qf[vq * QFS + r], qp.qf[vq * QFS + r + 1], qp.qf[vq * QFS + r + 2], qp.qf[vq * QFS + r + 3]};
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                const int rr = r + h;
+                if (rr >= MR) break;
+                const float2 q2 = make_float2(qv[h], qv[h]);
+                const int m = (rr <= LB) ? rr : rr - LB;
+#pragma unroll
+                for (int k = 0; k < NP; ++k) {
+                    if (rr <= LB) {
+                        if (m & 1) Co[k] = ffma2(f[k][rr], q2, Co[k]);
+                        else Ce[k] = ffma2(f[k][rr], q2, Ce[k]);
+                    } else {
+                        if (m & 1) So[k] = ffma2(f[k][rr], q2, So[k]);
+                        else Se[k] = ffma2(f[k][rr], q2, Se[k]);
+                    }
+                }
+            }
+        }
+        float2 g1[NP], g2[NP], g3[NP], g4[NP];
+#pragma unroll
+        for (int k = 0; k < NP; ++k) {
+            const float2 P = fadd2(Ce[k], Co[k]), Q = fsub2(Ce[k], Co[k]);
+            const float2 R = fadd2(Se[k], So[k]), T = fsub2(Se[k], So[k]);
+            g1[k] = fadd2(P, R);  // phi
+            g2[k] = fsub2(P, R);  // -phi
+            g4[k] = fadd2(Q, T);  // pi + phi
+            g3[k] = fsub2(Q, T);  // pi - phi
+        }
+        float s1, s2, s3, s4;
+        if (!ODD) {
+            // Eq.(38): A~ B~ at the four azimuths
+            s1 = g1[0].x * g1[0].y;
+            s2 = g2[0].x * g2[0].y;
+            s3 = g3[0].x * g3[0].y;
+            s4 = g4[0].x * g4[0].y;
+        } else {
+            // Eq.(11): {A,B} = A_theta B_phi - A_phi B_theta  (A factor 1, B factor 2)
+            s1 = fmaf(g1[0].x, g1[NP - 1].y, -g1[0].y * g1[NP - 1].x);
+            s2 = fmaf(g2[0].x, g2[NP - 1].y, -g2[0].y * g2[NP - 1].x);
+            s3 = fmaf(g3[0].x, g3[NP - 1].y, -g3[0].y * g3[NP - 1].x);
+            s4 = fmaf(g4[0].x, g4[NP - 1].y, -g4[0].y * g4[NP - 1].x);
+        }
+        const float A = s1 + s2, B = s3 + s4, Cd = s1 - s2, D = s4 - s3;
+        const float2 mc = make_float2(A + B, A - B);    // cosine rows: (even m, odd m)
+        const float2 ms = make_float2(Cd - D, Cd + D);  // sine rows:   (odd m, even m)
+#pragma unroll
+        for (int k = 0; k < NTC; ++k)
+            tc[k] = ffma2(make_float2(qp.qi[vq * QIS + 2 * k], qp.qi[vq * QIS + 2 * k + 1]), mc, tc[k]);
+#pragma unroll
+        for (int k = 0; k < NTS; ++k)
+            ts[k] = ffma2(make_float2(qp.qi[vq * QIS + SOFF + 2 * k], qp.qi[vq * QIS + SOFF + 2 * k + 1]), ms, ts[k]);
     }
 #pragma unroll
     for (int m = 0; m <= LB; ++m) F[(m * RB + lr) * GW + lane] = (m & 1) ? tc[m / 2].y : tc[m / 2].x;

@@ -122,8 +122,8 @@ __device__ __forceinline__ void proj_tile(float2 (&acc)[2][kTJ], uint32_t x0, ui
 
 // S2a-S4b for the groups of one parity, run by the nsub warps of a sub-group (2 workers = half-warps per warp).
 template <int LB, bool ODD>
-__device__ __forceinline__ void core_groups(const FusedArgs& a, const float* __restrict__ ta, const float* __restrict__ wp,
-                                            const float* __restrict__ qf, const float* __restrict__ qi,
+__device__ __forceinline__ void core_groups(const FusedArgs& a, const CoreQParam<LB>& qp, const float* __restrict__ ta,
+                                            const float* __restrict__ wp,
                                             const int* __restrict__ sched, int MAXI, float* __restrict__ F,
                                             float* __restrict__ Ha, const float* __restrict__ Hb, int col_base, int ngroups,
                                             int sub_warp, int nsub, int bar_id, int lane)
@@ -162,7 +162,7 @@ __device__ __forceinline__ void core_groups(const FusedArgs& a, const float* __r
             const int gi = it / RB, lr = it - gi * RB;
             const int e = (lr < UB) ? lr : lr - UB;
             if (e >= ne || (lr >= UB && e == eq)) continue;
-            stage_b<LB, ODD, RB, GW>(qf, qi, a.tab.QFS, a.tab.QIS, a.tab.SOFF, F + (size_t)gi * fgroup, plane, lr, a.tab.NQ, col);
+            stage_b_p<LB, ODD, RB, GW>(qp, F + (size_t)gi * fgroup, plane, lr, a.tab.NQ, col);
         }
         bar_sync(bar_id, nsub * 32);
         // stage C: T overwrites the column's factor-1 row of H, dead since stage A
@@ -251,7 +251,8 @@ __device__ __forceinline__ void phase_q(const FusedArgs& a, int wwarp, int lane,
 }
 
 template <int LB>
-__global__ void __launch_bounds__(kFusedThreads, 1) onsite_fused_kernel(const __grid_constant__ FusedArgs a)
+__global__ void __launch_bounds__(kFusedThreads, 1) onsite_fused_kernel(const __grid_constant__ FusedArgs a,
+                                                                        const __grid_constant__ CoreQParam<LB> qp)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* bar_tab = reinterpret_cast<uint64_t*>(smem);
@@ -327,8 +328,6 @@ __global__ void __launch_bounds__(kFusedThreads, 1) onsite_fused_kernel(const __
     const float* ta_e = reinterpret_cast<const float*>(blob + a.tab.ta_e);
     const float* ta_o = reinterpret_cast<const float*>(blob + a.tab.ta_o);
     const float* wp = reinterpret_cast<const float*>(blob + a.tab.wp);
-    const float* qf = reinterpret_cast<const float*>(blob + a.tab.qf);
-    const float* qi = reinterpret_cast<const float*>(blob + a.tab.qi);
     const int* sched_e = reinterpret_cast<const int*>(blob + a.tab.sched_e);
     const int* sched_o = reinterpret_cast<const int*>(blob + a.tab.sched_o);
 
@@ -355,11 +354,11 @@ __global__ void __launch_bounds__(kFusedThreads, 1) onsite_fused_kernel(const __
         // ---- core (S2a-S4b): even and odd sub-groups side by side
         if (wwarp < a.tab.we) {
             if (Ce > 0)
-                core_groups<LB, false>(a, ta_e, wp, qf, qi, sched_e, a.tab.maxi_e, reinterpret_cast<float*>(wgm + a.off_fe), Ha,
+                core_groups<LB, false>(a, qp, ta_e, wp, sched_e, a.tab.maxi_e, reinterpret_cast<float*>(wgm + a.off_fe), Ha,
                                        Hb, 0, NA * Ce / kFusedGW, wwarp, a.tab.we, bar_e, lane);
         } else {
             if (Co > 0)
-                core_groups<LB, true>(a, ta_o, wp, qf, qi, sched_o, a.tab.maxi_o,
+                core_groups<LB, true>(a, qp, ta_o, wp, sched_o, a.tab.maxi_o,
                                       reinterpret_cast<float*>(wgm + a.off_fo), Ha, Hb, NA * Ce, NA * Co / kFusedGW,
                                       wwarp - a.tab.we, a.tab.wo, bar_o, lane);
         }
@@ -387,6 +386,7 @@ struct FusedPlan {
     int dev, lmax, lmax_out, we, wo;
     FusedTab tab;
     const void* blob;
+    std::vector<float> QF, QI;  // host copies of the azimuthal tables: passed to the kernel as a parameter (CoreQParam)
 };
 static std::mutex g_fused_mu;
 static std::vector<FusedPlan*> g_fused_plans;
@@ -457,6 +457,8 @@ static const FusedPlan* get_fused_plan(const Plan* p, int we, int wo)
     f->dev = p->dev; f->lmax = p->lmax; f->lmax_out = p->lmax_out; f->we = we; f->wo = wo;
     f->tab = t;
     f->blob = d;
+    f->QF = QF;
+    f->QI = QI;
     g_fused_plans.push_back(f);
     return f;
 }
@@ -470,12 +472,16 @@ static inline int num_slices(int L)
 }
 
 template <int LB>
-static int launch_fused_t(const FusedArgs& a, int smem, int64_t grid, cudaStream_t st)
+static int launch_fused_t(const FusedArgs& a, const FusedPlan* fp, int smem, int64_t grid, cudaStream_t st)
 {
+    CoreQParam<LB> qp;
+    std::memset(&qp, 0, sizeof qp);
+    std::memcpy(qp.qf, fp->QF.data(), std::min(sizeof qp.qf, fp->QF.size() * sizeof(float)));
+    std::memcpy(qp.qi, fp->QI.data(), std::min(sizeof qp.qi, fp->QI.size() * sizeof(float)));
     auto kern = onsite_fused_kernel<LB>;
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     LaunchScope scope(K_ONSITE_FUSED, st);
-    kern<<<(unsigned)grid, kFusedThreads, smem, st>>>(a);
+    kern<<<(unsigned)grid, kFusedThreads, smem, st>>>(a, qp);
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
 }
@@ -567,7 +573,7 @@ int launch_onsite_fused(const Plan* p, int N, int C, int Ce, int Co, const float
     switch (LB) {
 #define CGTP_CASE(Bn) \
     case Bn:          \
-        return launch_fused_t<Bn>(a, smem, grid, st);
+        return launch_fused_t<Bn>(a, fp, smem, grid, st);
         CGTP_CASE(1) CGTP_CASE(2) CGTP_CASE(3) CGTP_CASE(4) CGTP_CASE(5) CGTP_CASE(6) CGTP_CASE(8)
 #undef CGTP_CASE
     }

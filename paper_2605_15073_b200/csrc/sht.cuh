@@ -342,6 +342,50 @@ __device__ __forceinline__ void dft_inverse_row(const float* srow, float* T, int
     for (int r = 0; r < M; ++r) T[r * J + j] = t[r];
 }
 
+// The azimuthal tables of one plan as a kernel parameter (constant bank): the table index depends only on the loop counter,
+// so the loads run on the uniform datapath (LDCU) and the FMAs take the value as a uniform-register operand -- no
+// shared-memory wavefronts, where the broadcast 128-bit loads of the shared-memory form cost two each (measured:
+// the shared-memory pipe, not the FMA pipe, bound the transforms).
+template <int LB>
+struct QParam {
+    static constexpr int QSTR = round_up(LB + 1, 4);
+    static constexpr int VHMAX = (3 * LB + 1) / 2 + 1;  // Vh of the bilinear grid at lmax = lmax_out = LB
+    float qc[VHMAX * QSTR], qs[VHMAX * QSTR], wv[round_up(VHMAX, 4)];
+};
+template <int LB>
+inline void fill_qparam(const Plan* p, QParam<LB>& q)
+{
+    for (int i = 0; i < p->Vh * p->QSTR; ++i) { q.qc[i] = p->hQC[i]; q.qs[i] = p->hQS[i]; }
+    for (int i = 0; i < round_up(p->Vh, 4); ++i) q.wv[i] = p->hWV[i];
+}
+
+// dft_inverse_row with the tables read from a QParam kernel parameter.
+template <int LB>
+__device__ __forceinline__ void dft_inverse_row_p(const float* srow, float* T, int J, int j, const QParam<LB>& q, int V, int Vh)
+{
+    constexpr int M = 2 * LB + 1;
+    constexpr int QSTR = QParam<LB>::QSTR;
+    float t[M];
+#pragma unroll
+    for (int r = 0; r < M; ++r) t[r] = 0.f;
+    // fully unrolled over the largest Vh of the band limit: every table index is a compile-time constant, so the table
+    // values are constant-bank operands of the FMAs themselves (no load instruction at all)
+#pragma unroll
+    for (int vp = 0; vp < QParam<LB>::VHMAX; ++vp) {
+        if (vp >= Vh) break;
+        const float s1 = srow[vp];
+        const float s2 = srow[vp == 0 ? 0 : V - vp];
+        const float w = q.wv[vp];
+        const float sp = w * (s1 + s2), sm = w * (s1 - s2);
+#pragma unroll
+        for (int m = 0; m <= LB; ++m) t[m] = fmaf(q.qc[vp * QSTR + m], sp, t[m]);
+#pragma unroll
+        for (int m = 1; m <= LB; ++m) t[LB + m] = fmaf(q.qs[vp * QSTR + m], sm, t[LB + m]);
+    }
+#pragma unroll
+    for (int r = 0; r < M; ++r) T[r * J + j] = t[r];
+}
+
 // --------------------------------------------------------------------------- Legendre analysis
 // Rows S4b / M5 second half (Eq.(40), Eq.(54) :422): Gauss-Legendre quadrature.
 // T0 (+ T1 if not null): [M][J] shared, the azimuthal coefficients per grid row; WP: [Uh][NTRI] table

@@ -41,8 +41,7 @@ static SfLayout sf_layout(const Plan* p, int hstride, int nfield)
     s.HS = hstride;
     int off = 0;
     s.ptt = off; off += round_up(nfield * ntri * s.UP, 4);
-    s.qc = off; off += p->Vh * p->QSTR;
-    s.qs = off; off += p->Vh * p->QSTR;
+    s.qc = s.qs = off;  // the azimuthal tables are a kernel parameter (QParam)
     s.f = off; off += nfield * M * p->U * 32;
     s.gt = off; off += std::max(round_up(32 * s.GS, 4), round_up(32 * hstride, 4));
     s.hs = s.gt;  // the coefficients are dead once the Legendre stage has run; the grid tile reuses their space
@@ -54,8 +53,9 @@ static SfLayout sf_layout(const Plan* p, int hstride, int nfield)
 // M2: value grid field of 32 columns per group.  H: [col][hstride] (hstride odd), G: [col][UVp].
 // ------------------------------------------------------------------------------------------------
 template <int LB>
-__global__ void __launch_bounds__(SF_THREADS) synth_fast_kernel(Plan p, SfLayout lay, const float* __restrict__ H,
-                                                               float* __restrict__ G, long long ncols)
+__global__ void __launch_bounds__(SF_THREADS) synth_fast_kernel(Plan p, SfLayout lay, const __grid_constant__ QParam<LB> qp,
+                                                               const float* __restrict__ H, float* __restrict__ G,
+                                                               long long ncols)
 {
     extern __shared__ __align__(16) float sm[];
     constexpr int M = 2 * LB + 1;
@@ -63,8 +63,6 @@ __global__ void __launch_bounds__(SF_THREADS) synth_fast_kernel(Plan p, SfLayout
     constexpr int UHMAX = ((3 * LB + 2) / 2 + 1) / 2;
     constexpr int UP = round_up(UHMAX, 4);
     float* PTt = sm + lay.ptt;  // [tri][UP]
-    float* QC = sm + lay.qc;
-    float* QS = sm + lay.qs;
     float* Hs = sm + lay.hs;    // [32][HS]
     float* F = sm + lay.f;      // [M][U][32]
     float* Gt = sm + lay.gt;    // [32][GS]
@@ -76,10 +74,6 @@ __global__ void __launch_bounds__(SF_THREADS) synth_fast_kernel(Plan p, SfLayout
     for (int i = tid; i < ntri * UP; i += SF_THREADS) {
         const int t = i / UP, u = i - t * UP;
         PTt[i] = (u < Uh) ? p.PT[u * p.NTRI + t] : 0.f;
-    }
-    for (int i = tid; i < Vh * QSTR; i += SF_THREADS) {
-        QC[i] = p.QC[i];
-        QS[i] = p.QS[i];
     }
     // coefficient rows above lmax (kernel band limit LB > lmax) stay zero for the whole kernel
     for (int i = tid; i < M * U * 32; i += SF_THREADS) F[i] = 0.f;
@@ -147,34 +141,33 @@ __global__ void __launch_bounds__(SF_THREADS) synth_fast_kernel(Plan p, SfLayout
             for (int r = 0; r < M; ++r) f[r] = make_float2(F[(r * U + un) * 32 + lane], F[(r * U + us) * 32 + lane]);
             float* gn = Gt + lane * GS + un * V;
             float* gs = Gt + lane * GS + us * V;
-            // two azimuths per pass: four independent accumulation chains
-            for (int vp0 = 0; vp0 < Vh; vp0 += 2) {
+            // two azimuths per pass: four independent accumulation chains.  The azimuth loop is fully unrolled over the
+            // largest table of the band limit, so every table value is a constant-bank operand (QParam, sht.cuh): no
+            // shared-memory wavefronts for the tables (this stage ran the shared-memory pipe above the FMA pipe)
+#pragma unroll
+            for (int vp0 = 0; vp0 < QParam<LB>::VHMAX; vp0 += 2) {
+                if (vp0 >= Vh) break;
                 float2 ce[2], so[2];
 #pragma unroll
                 for (int w = 0; w < 2; ++w) ce[w] = so[w] = make_float2(0.f, 0.f);
-                const int vp1 = (vp0 + 1 < Vh) ? vp0 + 1 : vp0;
+                const bool two = vp0 + 1 < Vh;
 #pragma unroll
-                for (int k = 0; k < QSTR / 4; ++k) {
-                    const float4 c0 = reinterpret_cast<const float4*>(QC + vp0 * QSTR)[k];
-                    const float4 s0 = reinterpret_cast<const float4*>(QS + vp0 * QSTR)[k];
-                    const float4 c1 = reinterpret_cast<const float4*>(QC + vp1 * QSTR)[k];
-                    const float4 s1 = reinterpret_cast<const float4*>(QS + vp1 * QSTR)[k];
-                    const float cv[2][4] = {{c0.x, c0.y, c0.z, c0.w}, {c1.x, c1.y, c1.z, c1.w}};
-                    const float sv[2][4] = {{s0.x, s0.y, s0.z, s0.w}, {s1.x, s1.y, s1.z, s1.w}};
+                for (int m = 0; m <= LB; ++m) {
 #pragma unroll
-                    for (int hh = 0; hh < 4; ++hh) {
-                        const int m = 4 * k + hh;
-#pragma unroll
-                        for (int w = 0; w < 2; ++w) {
-                            if (m <= LB) ce[w] = __ffma2_rn(f[m], make_float2(cv[w][hh], cv[w][hh]), ce[w]);
-                            if (m >= 1 && m <= LB) so[w] = __ffma2_rn(f[LB + m], make_float2(sv[w][hh], sv[w][hh]), so[w]);
+                    for (int w = 0; w < 2; ++w) {
+                        if (vp0 + w >= QParam<LB>::VHMAX) continue;
+                        const float c = qp.qc[(vp0 + w) * QSTR + m];
+                        ce[w] = __ffma2_rn(f[m], make_float2(c, c), ce[w]);
+                        if (m >= 1) {
+                            const float sn = qp.qs[(vp0 + w) * QSTR + m];
+                            so[w] = __ffma2_rn(f[LB + m], make_float2(sn, sn), so[w]);
                         }
                     }
                 }
 #pragma unroll
                 for (int w = 0; w < 2; ++w) {
-                    const int vp = w ? vp1 : vp0;
-                    if (w && vp1 == vp0) break;
+                    if (w && !two) break;
+                    const int vp = vp0 + w;
                     const float2 a = __fadd2_rn(ce[w], so[w]), b = __fadd2_rn(ce[w], make_float2(-so[w].x, -so[w].y));
                     gn[vp] = a.x;
                     gs[vp] = a.y;
@@ -217,7 +210,9 @@ static int launch_synth_fast_t(const Plan* p, Kind kind, const float* H, int hst
     const int64_t ngroups = (ncols + 31) / 32;
     const int grid = (int)std::min<int64_t>(ngroups, (int64_t)148 * per_sm);
     LaunchScope scope(kind, st);
-    kern<<<grid, SF_THREADS, smem, st>>>(*p, lay, H, G, (long long)ncols);
+    QParam<LB> qp;
+    fill_qparam<LB>(p, qp);
+    kern<<<grid, SF_THREADS, smem, st>>>(*p, lay, qp, H, G, (long long)ncols);
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
 }

@@ -291,6 +291,14 @@ const Plan* get_plan_nu(int lmax, int lmax_out, int nu)
         delete p;
         return nullptr;
     }
+    auto keep = [](const std::vector<float>& v) {
+        float* h = new float[v.size()];
+        std::memcpy(h, v.data(), v.size() * sizeof(float));
+        return h;
+    };
+    p->hQC = keep(QC);
+    p->hQS = keep(QS);
+    p->hWV = keep(WV);
     g_plans.push_back(p);
     return p;
 }
