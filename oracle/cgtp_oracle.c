@@ -43,6 +43,10 @@
  * fine-grid quadrature of the pooled pointwise product, one-edge receivers = oracle_onsite, edge order inside a
  * segment and rotation, and its l-dependent-weight form (oracle_message_field_lw) against it (equal weights, degree
  * selection, per-degree numpy projections around it) (tests/test_oracle_field.py).
+ * oracle_message_field_parity (Eq.(28) with the parity labels of both fields, Sec. VII C f :471) is pinned
+ * (tests/test_oracle_field_parity.py) to oracle_message_field per run (one slot pair populated), to oracle_onsite_parity on
+ * one-edge receivers, to B7-style exact vanishing in the wrong sector (:647), to inversion with the slots' labels and to
+ * Wigner-D rotation.
  * No function here is "parity unpinned".
  *
  * Plain C99 + OpenMP, double precision (long double inside the Racah sum).
@@ -994,6 +998,81 @@ int oracle_message_field_lw(const double *node_feats, const int64_t *edge_index,
 {
     return message_field_impl(node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C,
                               parity_mask, out, nodes, E, 1);
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Two parity-bearing fields, Eq.(28) with the parity labels of both fields        */
+/* (Sec. VI E :232-:240; Sec. VII C f :471).  Slot axes as in oracle_onsite_parity (R19): */
+/* slot 0 = natural parity (-1)^l, slot 1 = opposite parity.  Runs r = 8 cat + 4 s1 + 2 s2 + tau    */
+/* (R20): category cat (0: Gaunt, 1: curl), slot s1 of the edge field (factor 1, R10), slot s2 of   */
+/* the node field, output-degree parity tau.  Every non-zero coupling term is routed by p = p1 p2   */
+/* (:236 "The output parity is p = p1 p2") to the output slot whose label it carries.               */
+/*   edge_feats [E][2][Ne][L2], node_feats [nodes][2][N][L2],                                       */
+/*   W_edge [16][C][Ne], W_node [16][C][N], W_out [16][N][C], out [nodes][2][N][Lo2].               */
+/* ------------------------------------------------------------------------------------------ */
+int oracle_message_field_parity(const double *node_feats, const int64_t *edge_index, const double *edge_feats,
+                                const double *W_edge, const double *W_node, const double *W_out, int lmax,
+                                int lmax_out, int N, int Ne, int C, double *out, int64_t nodes, int64_t E)
+{
+    enum { R = 16 };
+    int L2 = (lmax + 1) * (lmax + 1), Lo2 = (lmax_out + 1) * (lmax_out + 1);
+    const coupling_t *tab[2];
+    tab[0] = get_coupling(lmax, lmax_out, 0);
+    tab[1] = get_coupling(lmax, lmax_out, 1);
+    if (!tab[0] || !tab[1]) return 2;
+    int64_t *row_ptr = malloc((size_t)(nodes + 1) * sizeof(int64_t));
+    int rc = oracle_segments(edge_index, E, nodes, row_ptr);
+    if (rc) { free(row_ptr); return rc; }
+    const int64_t *snd = edge_index;
+#pragma omp parallel
+    {
+        double *a = malloc((size_t)C * L2 * sizeof(double));
+        double *h = malloc((size_t)C * L2 * sizeof(double));
+        double *T = malloc((size_t)2 * C * Lo2 * sizeof(double)); /* [output slot][c][lm] of one run */
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t i = 0; i < nodes; ++i) {
+            double *ob = out + i * 2 * (int64_t)N * Lo2;
+            for (size_t k = 0; k < (size_t)2 * N * Lo2; ++k) ob[k] = 0.0;
+            for (int run = 0; run < R; ++run) {
+                int cat = run >> 3, s1 = (run >> 2) & 1, s2 = (run >> 1) & 1, tau = run & 1;
+                const coupling_t *t = tab[cat];
+                for (size_t k = 0; k < (size_t)2 * C * Lo2; ++k) T[k] = 0.0;
+                for (int64_t e = row_ptr[i]; e < row_ptr[i + 1]; ++e) {
+                    const double *xe = edge_feats + (e * 2 + s1) * (int64_t)Ne * L2;
+                    const double *xj = node_feats + (snd[e] * 2 + s2) * (int64_t)N * L2;
+                    for (int c = 0; c < C; ++c)
+                        for (int q = 0; q < L2; ++q) {
+                            double sa = 0.0, sh = 0.0;
+                            for (int n = 0; n < Ne; ++n) sa += W_edge[((size_t)run * C + c) * Ne + n] * xe[n * L2 + q];
+                            for (int n = 0; n < N; ++n) sh += W_node[((size_t)run * C + c) * N + n] * xj[n * L2 + q];
+                            a[c * L2 + q] = sa;
+                            h[c * L2 + q] = sh;
+                        }
+                    for (int64_t k = 0; k < t->nnz; ++k) {
+                        int l1 = isqrt_floor(t->i1[k]), l2 = isqrt_floor(t->i2[k]), l = isqrt_floor(t->io[k]);
+                        int p1 = sgn_pow(s1) * sgn_pow(l1), p2 = sgn_pow(s2) * sgn_pow(l2);
+                        int p = p1 * p2;                        /* Eq.(28): output parity p = p1 p2 (:236)      */
+                        int so = (p == sgn_pow(l)) ? 0 : 1;
+                        if ((l & 1) != tau) continue;           /* this run feeds (-1)^l = sigma only (Eq.(54)) */
+                        for (int c = 0; c < C; ++c)
+                            T[((size_t)so * C + c) * Lo2 + t->io[k]] +=
+                                t->val[k] * a[(size_t)c * L2 + t->i1[k]] * h[(size_t)c * L2 + t->i2[k]];
+                    }
+                }
+                for (int so = 0; so < 2; ++so)
+                    for (int n = 0; n < N; ++n)
+                        for (int q = 0; q < Lo2; ++q) {
+                            double acc = 0.0;
+                            for (int c = 0; c < C; ++c)
+                                acc += W_out[((size_t)run * N + n) * C + c] * T[((size_t)so * C + c) * Lo2 + q];
+                            ob[((size_t)so * N + n) * Lo2 + q] += acc;
+                        }
+            }
+        }
+        free(a); free(h); free(T);
+    }
+    free(row_ptr);
+    return 0;
 }
 
 int oracle_num_threads(void)

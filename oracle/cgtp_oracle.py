@@ -76,6 +76,8 @@ def _load():
     lib.oracle_message_field.argtypes = [p, p, p, p, p, p, i, i, i, i, i, p, p, i64, i64]
     lib.oracle_message_field_lw.restype = i
     lib.oracle_message_field_lw.argtypes = lib.oracle_message_field.argtypes
+    lib.oracle_message_field_parity.restype = i
+    lib.oracle_message_field_parity.argtypes = [p, p, p, p, p, p, i, i, i, i, i, p, i64, i64]
     lib.oracle_num_threads.restype = i
     lib.oracle_num_threads.argtypes = []
     _lib = lib
@@ -322,6 +324,25 @@ def message_field(node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lma
                                       lmax_out, N, Ne, C, _ptr(mask), _ptr(out), nodes, E)
     if rc:
         raise RuntimeError(f"oracle_message_field failed with code {rc}")
+    return out
+
+
+def message_field_parity(node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out) -> np.ndarray:
+    """Two parity-bearing fields, Eq.(28) with slot axes: node_feats [nodes,2,N,L2], edge_feats [E,2,Ne,L2] (slot 0 natural,
+    1 opposite parity); W_edge [16,C,Ne], W_node [16,C,N], W_out [16,N,C], run = 8*cat + 4*s1 + 2*s2 + tau (s1: edge slot,
+    s2: node slot).  out [nodes, 2, N, (lmax_out+1)^2]."""
+    X, XE, W_edge, W_node, W_out = map(_f64, (node_feats, edge_feats, W_edge, W_node, W_out))
+    ei = np.ascontiguousarray(np.asarray(edge_index), dtype=np.int64)
+    nodes, two, N, L2 = X.shape
+    E, two_e, Ne, _ = XE.shape
+    C = W_node.shape[1]
+    assert two == 2 and two_e == 2 and L2 == (lmax + 1) ** 2 and XE.shape == (E, 2, Ne, L2) and ei.shape == (2, E)
+    assert W_edge.shape == (16, C, Ne) and W_node.shape == (16, C, N) and W_out.shape == (16, N, C)
+    out = np.zeros((nodes, 2, N, (lmax_out + 1) ** 2), np.float64)
+    rc = _load().oracle_message_field_parity(_ptr(X), _ptr(ei), _ptr(XE), _ptr(W_edge), _ptr(W_node), _ptr(W_out), lmax,
+                                             lmax_out, N, Ne, C, _ptr(out), nodes, E)
+    if rc:
+        raise RuntimeError(f"oracle_message_field_parity failed with code {rc}")
     return out
 
 

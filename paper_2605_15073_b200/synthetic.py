@@ -206,6 +206,39 @@ def make_message_parity(lmax: int, lmax_out: int, N: int, C: int, nodes: int, de
                                W_node, W_out, g.degree)
 
 
+@dataclass
+class FieldParityInputs:
+    lmax: int
+    lmax_out: int
+    N: int
+    Ne: int
+    C: int
+    nodes: int
+    E: int
+    node_feats: np.ndarray   # [nodes, 2, N, L2]
+    edge_index: np.ndarray   # [2, E]
+    edge_feats: np.ndarray   # [E, 2, Ne, L2]
+    W_edge: np.ndarray       # [16, C, Ne]
+    W_node: np.ndarray       # [16, C, N]
+    W_out: np.ndarray        # [16, N, C]
+    degree: np.ndarray
+
+
+def make_field_parity(lmax: int, lmax_out: int, N: int, Ne: int, C: int, nodes: int, degree, seed: int = 0) -> FieldParityInputs:
+    """Two parity-bearing fields (Eq.(28), Sec. VII C f :471): the graph of make_message (same seed -> same
+    graph), node and edge feature fields ~N(0,1) in both parity slots, one weight set per run (16 runs)."""
+    g = make_message(lmax, lmax_out, 1, 1, nodes, degree, 0.8, 5.0, seed)
+    L2 = (lmax + 1) ** 2
+    rX, rE, rWe, rWn, rWo = _streams(seed + 104729, 5)
+    node_feats = rX.standard_normal((nodes, 2, N, L2), dtype=np.float32)
+    edge_feats = rE.standard_normal((g.E, 2, Ne, L2), dtype=np.float32)
+    W_edge = (rWe.standard_normal((16, C, Ne), dtype=np.float32) / np.float32(np.sqrt(Ne))).astype(np.float32)
+    W_node = (rWn.standard_normal((16, C, N), dtype=np.float32) / np.float32(np.sqrt(N))).astype(np.float32)
+    W_out = (rWo.standard_normal((16, N, C), dtype=np.float32) / np.float32(np.sqrt(C))).astype(np.float32)
+    return FieldParityInputs(lmax, lmax_out, N, Ne, C, nodes, g.E, node_feats, g.edge_index, edge_feats, W_edge, W_node,
+                             W_out, g.degree)
+
+
 # ---------------------------------------------------------------------------------------------
 # l-dependent CP weights (SURVEY.md 8(f) NEXT-2; PAPER.md Eq.(35) :322, Eq.(41) :346, Eq.(47) :398): the same inputs as
 # make_onsite / make_message with one weight matrix per degree l.
