@@ -333,6 +333,29 @@ int cgtp_set_math_mode(int mode);
 int cgtp_get_math_mode(void);
 
 /* ---------------------------------------------------------------------------------------------
+ * Two parity-bearing fields, Eq.(28) with the parity labels of both fields (Sec. VI E :232-:240,
+ * Sec. VII C f :471: "The dispatch reads from both I^(E) and I^(N) with independent parity-slot selections at (l1,p1) and
+ * (l2,p2) ... four input-parity combinations, two output-l parities, and Categories alpha and beta").  Slot axes as in
+ * cgtp_onsite_parity (R19): slot 0 = natural parity (-1)^l, slot 1 = opposite parity.
+ *
+ *   run r = 8 cat + 4 s1 + 2 s2 + tau   (cat: 0 alpha = Gaunt coupling, 1 beta = surface-curl coupling; s1 / s2: slot of
+ *                                        the edge field / the node field; tau: output-degree parity (-1)^l = sigma, Eq.(54))
+ *   a_r[e,c,:] = W_edge[r,c,:] . edge_feats[e,s1]        H_r[j,c,:] = W_node[r,c,:] . node_feats[j,s2]
+ *   T_r[i,c,lm] = sum_{e -> i} coupling_cat(a_r[e,c], H_r[send(e),c])_lm   kept at the degrees l with (l & 1) == tau
+ *   out[i, s, n, lm] += sum_c W_out[r,n,c] T_r[i,c,lm]   with s = s1 ^ s2 (alpha) or 1 ^ s1 ^ s2 (beta): p = p1 p2 (:236)
+ *
+ * node_feats device [nodes, 2, N, (lmax+1)^2]     edge_feats device [E, 2, Ne, (lmax+1)^2]
+ * W_edge device [16, C, Ne]   W_node device [16, C, N]   W_out device [16, N, C]
+ * out device [nodes, 2, N, (lmax_out+1)^2], fully overwritten; everything else as cgtp_message_field.  Four passes of the
+ * two-field pipeline over 4 C internal rank channels (cost: the paper's upper bound 24 x, Eq.(61)); C <= 256.
+ * ------------------------------------------------------------------------------------------- */
+size_t cgtp_message_field_parity_workspace_bytes(int lmax, int lmax_out, int N, int Ne, int C, int64_t nodes, int64_t E);
+int cgtp_message_field_parity(const float* node_feats, const int64_t* edge_index, const float* edge_feats,
+                              const float* W_edge, const float* W_node, const float* W_out,
+                              int lmax, int lmax_out, int N, int Ne, int C, float* out,
+                              int64_t nodes, int64_t E, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Kernel-path switch (test instrumentation; never needed for results).  Several stages have a specialised kernel and
  * a generic one that computes the same thing with a different mapping to the machine; a set bit forces the generic
  * kernel, so that tests/ can cross-check the two on whole full-size batches (the oracle anchors both on samples):

@@ -72,6 +72,10 @@ def lib() -> ctypes.CDLL:
     L.cgtp_message_field_bipartite_workspace_bytes.argtypes = [i, i, i, i, i, i64, i64, i64]
     L.cgtp_message_field_bipartite.restype = i
     L.cgtp_message_field_bipartite.argtypes = [vp, vp, vp, vp, vp, vp, i, i, i, i, i, vp, vp, i64, i64, i64, vp, sz, vp]
+    L.cgtp_message_field_parity_workspace_bytes.restype = sz
+    L.cgtp_message_field_parity_workspace_bytes.argtypes = [i, i, i, i, i, i64, i64]
+    L.cgtp_message_field_parity.restype = i
+    L.cgtp_message_field_parity.argtypes = [vp, vp, vp, vp, vp, vp, i, i, i, i, i, vp, i64, i64, vp, sz, vp]
     L.cgtp_onsite_nbody_workspace_bytes.restype = sz
     L.cgtp_onsite_nbody_workspace_bytes.argtypes = [i, i, i, i, i, i64]
     L.cgtp_onsite_nbody.restype = i
@@ -312,6 +316,34 @@ def cgtp_message_field(node_feats, edge_index, edge_feats, W_edge, W_node, W_out
         rc = entry(X.data_ptr(), ei.data_ptr(), XE.data_ptr(), W_edge.data_ptr(), W_node.data_ptr(),
                                       W_out.data_ptr(), lmax, lmax_out, N, Ne, C, mask.ctypes.data, out.data_ptr(),
                                       nodes, E, ws.data_ptr(), ws.numel(), sp)
+        _check(rc)
+        if check:
+            _check(lib().cgtp_message_status(ws.data_ptr(), sp))
+    return out
+
+
+def cgtp_message_field_parity(node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C, out=None,
+                              workspace=None, stream=None, check: bool = False):
+    """out[nodes, 2, N, (lmax_out+1)^2] = two parity-bearing fields, Eq.(28) with slot axes: node_feats [nodes,2,N,L2],
+    edge_feats [E,2,Ne,L2], W_edge [16,C,Ne], W_node [16,C,N], W_out [16,N,C] (see include/cgtp.h)."""
+    f32 = torch.float32
+    X, XE = _dev(node_feats, f32, "node_feats"), _dev(edge_feats, f32, "edge_feats")
+    ei = _dev(edge_index, torch.int64, "edge_index")
+    W_edge, W_node, W_out = _dev(W_edge, f32, "W_edge"), _dev(W_node, f32, "W_node"), _dev(W_out, f32, "W_out")
+    nodes, E = X.shape[0], ei.shape[1]
+    L2, Lo2 = (lmax + 1) ** 2, (lmax_out + 1) ** 2
+    if tuple(X.shape) != (nodes, 2, N, L2) or tuple(XE.shape) != (E, 2, Ne, L2) or tuple(ei.shape) != (2, E):
+        raise ValueError("node_feats [nodes,2,N,(lmax+1)^2], edge_feats [E,2,Ne,(lmax+1)^2], edge_index [2,E] expected")
+    if tuple(W_edge.shape) != (16, C, Ne) or tuple(W_node.shape) != (16, C, N) or tuple(W_out.shape) != (16, N, C):
+        raise ValueError("W_edge must be [16, C, Ne], W_node [16, C, N] and W_out [16, N, C]")
+    out = _out(out, (nodes, 2, N, Lo2), X.device)
+    nbytes = lib().cgtp_message_field_parity_workspace_bytes(lmax, lmax_out, N, Ne, C, nodes, E)
+    ws = _workspace(X.device, nbytes, stream) if workspace is None else workspace
+    sp = _stream_ptr(stream)
+    with torch.cuda.device(X.device):
+        rc = lib().cgtp_message_field_parity(X.data_ptr(), ei.data_ptr(), XE.data_ptr(), W_edge.data_ptr(), W_node.data_ptr(),
+                                             W_out.data_ptr(), lmax, lmax_out, N, Ne, C, out.data_ptr(), nodes, E,
+                                             ws.data_ptr(), ws.numel(), sp)
         _check(rc)
         if check:
             _check(lib().cgtp_message_status(ws.data_ptr(), sp))

@@ -762,37 +762,34 @@ size_t cgtp_message_field_workspace_bytes(int lmax, int lmax_out, int N, int Ne,
 
 // lw: l-dependent weights W_edge [lmax+1, C, Ne], W_node [lmax+1, C, N], W_out [lmax_out+1, N, C] (Eq.(35), (41), (47), (55)):
 // every projection becomes one problem per degree l over the columns l^2 .. l^2 + 2l (one launch with proj_multi).
-static int field_entry(bool lw, const float* node_feats, const int64_t* edge_index, const float* edge_feats,
-                       const float* W_edge, const float* W_node, const float* W_out, int lmax, int lmax_out, int N, int Ne,
-                       int C, const uint8_t* parity_mask, float* out, int64_t n_send, int64_t nodes, int64_t E,
-                       void* workspace, size_t workspace_bytes, void* cuda_stream)
+// One run of the two-field pipeline (Eq.(28)) over Ce even + Co odd rank channels; cgtp_message_field is one
+// pass, cgtp_message_field_parity four (one per pair of input slots).
+struct FieldPass {
+    const float* node_feats;  // first sender's [N, L2] block
+    int64_t x_bs_node;        // floats between consecutive senders
+    const float* edge_feats;  // first edge's [Ne, L2] block
+    int64_t x_bs_edge;        // floats between consecutive edges
+    const float *W_edge, *W_node;
+    const int* idx_in;        // [Ce+Co] device: row of W_edge (row length Ne) and of W_node (row length N) of channel k
+    const float* W_out;
+    int ldw_out;
+    const int *idx_out_e, *idx_out_o;
+    int Ce, Co;
+    float *out_e, *out_o;
+    int64_t o_bs;
+    int accumulate;
+    int sigma_C;              // as OnsitePass::sigma_C
+    bool segments_done;
+    bool lw;
+};
+
+static int field_pass(const Plan* p, int N, int Ne, const FieldPass& q, const int64_t* edge_index, int64_t n_send,
+                      int64_t nodes, int64_t E, void* workspace, cudaStream_t st)
 {
-    clear_error();
-    int rc = check_common(lmax, lmax_out, N, C, parity_mask);
-    if (rc) return rc;
-    if (Ne <= 0) { set_error("Ne must be positive (Ne=%d)", Ne); return CGTP_ERR_INVALID; }
-    if (nodes < 0 || n_send < 0 || E < 0) { set_error("negative size"); return CGTP_ERR_INVALID; }
-    if (nodes == 0) return CGTP_OK;
-    if (n_send == 0 && E > 0) { set_error("edges without sender nodes"); return CGTP_ERR_INVALID; }
-    if ((!node_feats && n_send > 0) || !W_edge || !W_node || !W_out || !out || !workspace || (E > 0 && (!edge_index || !edge_feats))) {
-        set_error("null pointer argument");
-        return CGTP_ERR_INVALID;
-    }
-    if (!aligned16(node_feats) || !aligned16(out) || !aligned16(W_edge) || !aligned16(W_node) || !aligned16(W_out) ||
-        (E > 0 && (!aligned16(edge_index) || !aligned16(edge_feats))) || (reinterpret_cast<uintptr_t>(workspace) & 255u)) {
-        set_error("misaligned pointer (tensors need 16-byte, workspace 256-byte alignment)");
-        return CGTP_ERR_INVALID;
-    }
-    if (workspace_bytes < field_ws_bytes(lmax, lmax_out, C, n_send, nodes, E)) {
-        set_error("workspace too small: %zu < %zu bytes", workspace_bytes, field_ws_bytes(lmax, lmax_out, C, n_send, nodes, E));
-        return CGTP_ERR_INVALID;
-    }
-    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const Plan* p = get_plan(lmax, lmax_out);
-    if (!p) return CGTP_ERR_CUDA;
-    const ChannelPlan* cp = get_channel_plan(C, parity_mask);
-    if (!cp) return CGTP_ERR_CUDA;
-    const int Cpar[2] = {cp->Ce, cp->Co};
+    const int C = q.Ce + q.Co;
+    const int Cpar[2] = {q.Ce, q.Co};
+    const bool lw = q.lw;
+    int rc = CGTP_OK;
     const bool fast = !(kernel_path() & PATH_GENERIC_CORE) && (Cpar[0] == 0 || onsite_fast_supported(p, false)) &&
                       (Cpar[1] == 0 || onsite_fast_supported(p, true));
     const int hstr = fast ? onsite_fast_hstride(p) : p->L2p;
@@ -814,21 +811,23 @@ static int field_entry(bool lw, const float* node_feats, const int64_t* edge_ind
     }
 
     // M0
-    rc = launch_segments(edge_index, E, nodes, n_send, row_ptr, status, st);
-    if (rc) return rc;
+    if (!q.segments_done) {
+        rc = launch_segments(edge_index, E, nodes, n_send, row_ptr, status, st);
+        if (rc) return rc;
+    }
     // the pool kernel leaves Tn alone when M0 flags the edge list: define it, so that `out` is zeros plus the flag
     for (int s = 0; s < 2; ++s)
         if (Cpar[s] > 0 && nodes > 0) CGTP_CUDA_CHECK(cudaMemsetAsync(Tn[s], 0, (size_t)nodes * Cpar[s] * tstr * 4, st));
 
     // factor 2: Hn = W_node . node_feats, once per node (Eq.(47) :398)
     ProjArgs a;
-    a.X = node_feats;
-    a.x_bs = (int64_t)N * p->L2;
+    a.X = q.node_feats;
+    a.x_bs = q.x_bs_node;
     a.x_rs = p->L2;
-    a.W = W_node;
+    a.W = q.W_node;
     a.ldw_m = N;
     a.ldw_k = 1;
-    a.idx_m = cp->perm_dev;
+    a.idx_m = q.idx_in;
     a.idx_k = nullptr;
     a.M = C;
     a.K = N;
@@ -858,7 +857,7 @@ static int field_entry(bool lw, const float* node_feats, const int64_t* edge_ind
         return v;
     };
     if (n_send > 0) {
-        rc = launch_proj_degrees(per_degree(a, W_node, N), 1, K_PROJ_IN, st);
+        rc = launch_proj_degrees(per_degree(a, q.W_node, N), 1, K_PROJ_IN, st);
         if (rc) return rc;
     }
 
@@ -867,15 +866,15 @@ static int field_entry(bool lw, const float* node_feats, const int64_t* edge_ind
         if (ec > 0) {
             // factor 1: Ha = W_edge . edge_feats ("an explicit radial contraction ... on the edge side", :471)
             ProjArgs b = a;
-            b.X = edge_feats + (size_t)e0 * Ne * p->L2;
-            b.x_bs = (int64_t)Ne * p->L2;
-            b.W = W_edge;
+            b.X = q.edge_feats + (size_t)e0 * q.x_bs_edge;
+            b.x_bs = q.x_bs_edge;
+            b.W = q.W_edge;
             b.ldw_m = Ne;
             b.K = Ne;
             b.out0 = Ha[0];
             b.out1 = Ha[1];
             b.batch = ec;
-            rc = launch_proj_degrees(per_degree(b, W_edge, Ne), 1, K_PROJ_IN, st);
+            rc = launch_proj_degrees(per_degree(b, q.W_edge, Ne), 1, K_PROJ_IN, st);
             if (rc) return rc;
         }
         for (int s = 0; s < 2; ++s) {
@@ -911,6 +910,13 @@ static int field_entry(bool lw, const float* node_feats, const int64_t* edge_ind
         if (E == 0) break;
     }
 
+    if (q.sigma_C > 0)
+        for (int s = 0; s < 2; ++s)
+            if (Cpar[s] > 0) {
+                rc = launch_sigma_mask(Tn[s], tstr, nodes * Cpar[s], Cpar[s], q.sigma_C, p->Lo2, st);
+                if (rc) return rc;
+            }
+
     // output projection per receiver (Eq.(55), (58))
     std::vector<ProjArgs> pv;
     for (int l = 0; l < (lw ? p->lmax_out + 1 : 1); ++l) {
@@ -921,26 +927,81 @@ static int field_entry(bool lw, const float* node_feats, const int64_t* edge_ind
             o.X = Tn[s];
             o.x_bs = (int64_t)Cpar[s] * tstr;
             o.x_rs = tstr;
-            o.W = W_out + (lw ? (size_t)l * N * C : 0);
-            o.ldw_m = C;
+            o.W = q.W_out + (lw ? (size_t)l * N * C : 0);
+            o.ldw_m = q.ldw_out;
             o.ldw_k = 1;
             o.idx_m = nullptr;
-            o.idx_k = cp->perm_dev + (s ? cp->Ce : 0);
+            o.idx_k = s ? q.idx_out_o : q.idx_out_e;
             o.M = N;
             o.K = Cpar[s];
             o.J = lw ? 2 * l + 1 : p->Lo2;
-            o.out0 = out + (size_t)s * N * p->Lo2 + jo;
-            o.o_bs0 = (int64_t)2 * N * p->Lo2;
+            o.out0 = (s ? q.out_o : q.out_e) + jo;
+            o.o_bs0 = q.o_bs;
             o.out1 = o.out0;
             o.o_bs1 = o.o_bs0;
             o.m_split = N;
             o.o_rs = p->Lo2;
             o.batch = nodes;
-            o.accumulate = 0;
+            o.accumulate = q.accumulate;
             o.j0 = jo;
         }
     }
     return launch_proj_degrees(pv, 2, K_PROJ_OUT, st);
+}
+
+
+static int field_entry(bool lw, const float* node_feats, const int64_t* edge_index, const float* edge_feats,
+                       const float* W_edge, const float* W_node, const float* W_out, int lmax, int lmax_out, int N, int Ne,
+                       int C, const uint8_t* parity_mask, float* out, int64_t n_send, int64_t nodes, int64_t E,
+                       void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    clear_error();
+    int rc = check_common(lmax, lmax_out, N, C, parity_mask);
+    if (rc) return rc;
+    if (Ne <= 0) { set_error("Ne must be positive (Ne=%d)", Ne); return CGTP_ERR_INVALID; }
+    if (nodes < 0 || n_send < 0 || E < 0) { set_error("negative size"); return CGTP_ERR_INVALID; }
+    if (nodes == 0) return CGTP_OK;
+    if (n_send == 0 && E > 0) { set_error("edges without sender nodes"); return CGTP_ERR_INVALID; }
+    if ((!node_feats && n_send > 0) || !W_edge || !W_node || !W_out || !out || !workspace || (E > 0 && (!edge_index || !edge_feats))) {
+        set_error("null pointer argument");
+        return CGTP_ERR_INVALID;
+    }
+    if (!aligned16(node_feats) || !aligned16(out) || !aligned16(W_edge) || !aligned16(W_node) || !aligned16(W_out) ||
+        (E > 0 && (!aligned16(edge_index) || !aligned16(edge_feats))) || (reinterpret_cast<uintptr_t>(workspace) & 255u)) {
+        set_error("misaligned pointer (tensors need 16-byte, workspace 256-byte alignment)");
+        return CGTP_ERR_INVALID;
+    }
+    if (workspace_bytes < field_ws_bytes(lmax, lmax_out, C, n_send, nodes, E)) {
+        set_error("workspace too small: %zu < %zu bytes", workspace_bytes, field_ws_bytes(lmax, lmax_out, C, n_send, nodes, E));
+        return CGTP_ERR_INVALID;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const Plan* p = get_plan(lmax, lmax_out);
+    if (!p) return CGTP_ERR_CUDA;
+    const ChannelPlan* cp = get_channel_plan(C, parity_mask);
+    if (!cp) return CGTP_ERR_CUDA;
+    FieldPass q;
+    q.node_feats = node_feats;
+    q.x_bs_node = (int64_t)N * p->L2;
+    q.edge_feats = edge_feats;
+    q.x_bs_edge = (int64_t)Ne * p->L2;
+    q.W_edge = W_edge;
+    q.W_node = W_node;
+    q.idx_in = cp->perm_dev;
+    q.W_out = W_out;
+    q.ldw_out = C;
+    q.idx_out_e = cp->perm_dev;
+    q.idx_out_o = cp->perm_dev + cp->Ce;
+    q.Ce = cp->Ce;
+    q.Co = cp->Co;
+    q.out_e = out;
+    q.out_o = out + (size_t)N * p->Lo2;
+    q.o_bs = (int64_t)2 * N * p->Lo2;
+    q.accumulate = 0;
+    q.sigma_C = 0;
+    q.segments_done = false;
+    q.lw = lw;
+    return field_pass(p, N, Ne, q, edge_index, n_send, nodes, E, workspace, st);
 }
 
 int cgtp_message_field(const float* node_feats, const int64_t* edge_index, const float* edge_feats, const float* W_edge,
@@ -968,6 +1029,76 @@ int cgtp_message_field_lw(const float* node_feats, const int64_t* edge_index, co
 {
     return field_entry(true, node_feats, edge_index, edge_feats, W_edge, W_node, W_out, lmax, lmax_out, N, Ne, C, parity_mask,
                        out, nodes, nodes, E, workspace, workspace_bytes, cuda_stream);
+}
+
+size_t cgtp_message_field_parity_workspace_bytes(int lmax, int lmax_out, int N, int Ne, int C, int64_t nodes, int64_t E)
+{
+    (void)N;
+    (void)Ne;
+    if (lmax < 0 || lmax_out < 0 || C <= 0 || nodes < 0 || E < 0) return 0;
+    return field_ws_bytes(lmax, lmax_out, 4 * C, nodes, nodes, E);
+}
+
+int cgtp_message_field_parity(const float* node_feats, const int64_t* edge_index, const float* edge_feats,
+                              const float* W_edge, const float* W_node, const float* W_out, int lmax, int lmax_out, int N,
+                              int Ne, int C, float* out, int64_t nodes, int64_t E, void* workspace, size_t workspace_bytes,
+                              void* cuda_stream)
+{
+    clear_error();
+    if (C <= 0 || C > 256) { set_error("C=%d outside [1, 256] (4*C internal rank channels per pass)", C); return C <= 0 ? CGTP_ERR_INVALID : CGTP_ERR_UNSUPPORTED; }
+    uint8_t mask[1024];
+    for (int k = 0; k < 4 * C; ++k) mask[k] = k >= 2 * C;
+    int rc = check_common(lmax, lmax_out, N, 4 * C, mask);
+    if (rc) return rc;
+    if (Ne <= 0) { set_error("Ne must be positive (Ne=%d)", Ne); return CGTP_ERR_INVALID; }
+    if (nodes < 0 || E < 0) { set_error("negative size"); return CGTP_ERR_INVALID; }
+    if (nodes == 0) return CGTP_OK;
+    if (!node_feats || !W_edge || !W_node || !W_out || !out || !workspace || (E > 0 && (!edge_index || !edge_feats))) {
+        set_error("null pointer argument");
+        return CGTP_ERR_INVALID;
+    }
+    if (!aligned16(node_feats) || !aligned16(out) || !aligned16(W_edge) || !aligned16(W_node) || !aligned16(W_out) ||
+        (E > 0 && (!aligned16(edge_index) || !aligned16(edge_feats))) || (reinterpret_cast<uintptr_t>(workspace) & 255u)) {
+        set_error("misaligned pointer (tensors need 16-byte, workspace 256-byte alignment)");
+        return CGTP_ERR_INVALID;
+    }
+    if (workspace_bytes < field_ws_bytes(lmax, lmax_out, 4 * C, nodes, nodes, E)) {
+        set_error("workspace too small: %zu < %zu bytes", workspace_bytes, field_ws_bytes(lmax, lmax_out, 4 * C, nodes, nodes, E));
+        return CGTP_ERR_INVALID;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const Plan* p = get_plan(lmax, lmax_out);
+    if (!p) return CGTP_ERR_CUDA;
+    const ParityPlan* pp = get_parity_plan(C, N, false);  // the run index 8 cat + 4 s1 + 2 s2 + tau of the on-site dispatch
+    if (!pp) return CGTP_ERR_CUDA;
+    const size_t nslot = (size_t)N * p->L2, eslot = (size_t)Ne * p->L2, sector = (size_t)N * p->Lo2;
+    for (int ps = 0; ps < 4; ++ps) {
+        const int s1 = ps >> 1, s2 = ps & 1;  // slot of the edge field (factor 1, R10) and of the node field (factor 2)
+        FieldPass q;
+        q.edge_feats = edge_feats + (size_t)s1 * eslot;
+        q.x_bs_edge = (int64_t)2 * eslot;
+        q.node_feats = node_feats + (size_t)s2 * nslot;
+        q.x_bs_node = (int64_t)2 * nslot;
+        q.W_edge = W_edge;
+        q.W_node = W_node;
+        q.idx_in = pp->idx_in(ps);
+        q.W_out = W_out;
+        q.ldw_out = C;
+        q.idx_out_e = pp->idx_out(ps);
+        q.idx_out_o = pp->idx_out(ps) + 2 * C;
+        q.Ce = 2 * C;
+        q.Co = 2 * C;
+        q.out_e = out + (size_t)(s1 ^ s2) * sector;      // alpha: p = p1 p2 with l1+l2+l even -> slot s1 ^ s2 (Eq.(28) :236)
+        q.out_o = out + (size_t)(1 ^ s1 ^ s2) * sector;  // beta: l1+l2+l odd -> the other slot
+        q.o_bs = (int64_t)2 * sector;
+        q.accumulate = ps > 0;
+        q.sigma_C = C;
+        q.segments_done = ps > 0;
+        q.lw = false;
+        rc = field_pass(p, N, Ne, q, edge_index, nodes, nodes, E, workspace, st);
+        if (rc) return rc;
+    }
+    return CGTP_OK;
 }
 
 // ------------------------------------------------------------------------------ parity-slot entry points

@@ -202,3 +202,83 @@ def test_field_configs4_graph_sampled_receivers():
                             m.parity_mask)
     assert sector_err(got[recv], ref[recv]) <= TOL, sector_err(got[recv], ref[recv])
     assert np.abs(got[:, 1, :, 0]).max() <= TOL * np.abs(got[:, 1]).max()
+
+
+# ------------------------------------------------ two parity-bearing fields with slot axes
+def run_field_parity(q, **kw):
+    out = cg.cgtp_message_field_parity(_cuda(q.node_feats), _cuda(q.edge_index), _cuda(q.edge_feats), _cuda(q.W_edge),
+                                       _cuda(q.W_node), _cuda(q.W_out), q.lmax, q.lmax_out, q.N, q.Ne, q.C, **kw)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+@pytest.mark.parametrize("lmax,lmax_out,N,Ne,C,nodes", [
+    (0, 0, 2, 2, 2, 5),
+    (1, 2, 3, 2, 2, 17),     # odd N * L2: slot blocks not 16-byte aligned -> generic projection kernel
+    (2, 2, 8, 4, 8, 40),
+    (3, 5, 4, 3, 3, 21),     # lmax_out > lmax
+    (4, 4, 8, 8, 8, 30),     # 16 columns per parity block: sender fields read in place through the edge list
+    (6, 6, 8, 4, 4, 25),
+    (8, 8, 4, 4, 4, 12),
+])
+def test_field_parity_slots_vs_oracle(lmax, lmax_out, N, Ne, C, nodes):
+    """cgtp_message_field_parity (Eq.(28) with the parity labels of both fields, Sec. VII C f :471) against the
+    term-by-term oracle: 16 runs, ragged graphs with empty first receiver and a long last segment."""
+    rng = np.random.default_rng(600 + lmax)
+    deg = rng.integers(0, 7, nodes)
+    deg[0] = 0
+    deg[-1] = 19
+    q = synthetic.make_field_parity(lmax, lmax_out, N, Ne, C, nodes, deg, seed=600 + lmax)
+    got = run_field_parity(q, check=True)
+    ref = orc.message_field_parity(q.node_feats, q.edge_index, q.edge_feats, q.W_edge, q.W_node, q.W_out, lmax, lmax_out)
+    assert sector_err(got, ref) <= TOL, sector_errs(got, ref)
+    assert np.abs(got[deg == 0]).max() == 0.0
+    assert np.array_equal(got, run_field_parity(q))  # bitwise reproducible
+
+
+def test_field_parity_reduces_to_the_natural_parity_call():
+    """Slot 1 of both fields empty: sector 0 / 1 at (-1)^l = sigma equal cgtp_message_field with the weights of the runs
+    (alpha, 0, 0, tau) / (beta, 0, 0, tau) -- the two entry points agree to rounding."""
+    lmax, N, Ne, C, nodes = 4, 8, 4, 4, 30
+    q = synthetic.make_field_parity(lmax, lmax, N, Ne, C, nodes, _ragged(nodes, 6, 2), seed=77)
+    q.node_feats[:, 1] = 0
+    q.edge_feats[:, 1] = 0
+    got = run_field_parity(q)
+    lv = np.concatenate([np.full(2 * l + 1, l) for l in range(lmax + 1)])
+    for tau in (0, 1):
+        We = np.concatenate([q.W_edge[tau], q.W_edge[8 + tau]])
+        Wn = np.concatenate([q.W_node[tau], q.W_node[8 + tau]])
+        Wo = np.concatenate([q.W_out[tau], q.W_out[8 + tau]], axis=1)
+        nat = cg.cgtp_message_field(_cuda(q.node_feats[:, 0]), _cuda(q.edge_index), _cuda(q.edge_feats[:, 0]), _cuda(We),
+                                    _cuda(Wn), _cuda(Wo), lmax, lmax, N, Ne, 2 * C, [0] * C + [1] * C).cpu().numpy()
+        sel = (lv % 2) == tau
+        for s in (0, 1):
+            d = np.abs(got[:, s][:, :, sel] - nat[:, s][:, :, sel]).max()
+            assert d <= 2e-6 * np.abs(nat[:, s]).max(), (tau, s, d)
+
+
+def test_field_parity_inversion_rotation_and_errors_on_gpu():
+    lmax, N, Ne, C, nodes = 4, 4, 4, 4, 20
+    q = synthetic.make_field_parity(lmax, lmax, N, Ne, C, nodes, 5, seed=91)
+    base = run_field_parity(q).astype(np.float64)
+    sign = np.concatenate([np.full(2 * l + 1, (-1.0) ** l) for l in range(lmax + 1)]).astype(np.float32)
+    qi = synthetic.make_field_parity(lmax, lmax, N, Ne, C, nodes, 5, seed=91)
+    qi.node_feats[:, 0] *= sign
+    qi.node_feats[:, 1] *= -sign
+    qi.edge_feats[:, 0] *= sign
+    qi.edge_feats[:, 1] *= -sign
+    inv = run_field_parity(qi)
+    assert np.abs(inv[:, 0] - base[:, 0] * sign).max() < TOL * np.abs(base[:, 0]).max()
+    assert np.abs(inv[:, 1] + base[:, 1] * sign).max() < TOL * np.abs(base[:, 1]).max()
+    D = shref.wigner_D_real(lmax, shref.random_rotation(np.random.default_rng(8)))
+    qr = synthetic.make_field_parity(lmax, lmax, N, Ne, C, nodes, 5, seed=91)
+    qr.node_feats = np.einsum("ab,...b->...a", D, q.node_feats.astype(np.float64)).astype(np.float32)
+    qr.edge_feats = np.einsum("ab,...b->...a", D, q.edge_feats.astype(np.float64)).astype(np.float32)
+    rot = run_field_parity(qr)
+    assert sector_err(rot, np.einsum("ab,...b->...a", D, base)) <= TOL
+    bad = synthetic.make_field_parity(lmax, lmax, N, Ne, C, nodes, 5, seed=91)
+    bad.edge_index[1] = bad.edge_index[1][::-1].copy()
+    with pytest.raises(cg.CgtpError) as ei:
+        run_field_parity(bad, check=True)
+    assert ei.value.code == cg.ERR_GRAPH
+    assert np.abs(run_field_parity(bad)).max() == 0.0  # zeros plus the flag
