@@ -348,8 +348,10 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a,
                 if (e >= ne || (lr >= UB && e == eq)) continue;
                 if constexpr (TWO_TERM)
                     stage_b_two_term<LB, RB, GW>(qf, qi, a.tab.QFS, a.tab.QIS, a.tab.SOFF, F, plane, lr, a.Vh, col);
-                else
-                    stage_b_p<LB, ODD, RB, GW>(qp, F, plane, lr, a.Vh, col);
+                else if constexpr (LB <= 12)
+                    stage_b_p<LB, ODD, RB, GW>(qp, F, plane, lr, a.Vh, col);  // tables as constant-bank operands
+                else  // the fully unrolled form outgrows the instruction cache at band limits 16 and 20 (measured slower)
+                    stage_b<LB, ODD, RB, GW>(qf, qi, a.tab.QFS, a.tab.QIS, a.tab.SOFF, F, plane, lr, a.Vh, col);
             }
             // the previous group's bulk store must have finished reading Ts before stage C rewrites it
             if (blk == 0 && threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
