@@ -368,8 +368,6 @@ int cgtp_message_field_parity(const float* node_feats, const int64_t* edge_index
  *                            the single fused kernel (onsite_fused.cu)
  *   CGTP_PATH_FUSED_ONSITE   S1-S5: the single fused kernel for every shape it supports, also where the library's own
  *                            choice is the four-launch step (narrow projections N * C < 4096)
- *   CGTP_PATH_FUSED_WG       S1-S5: the warp-group form of the single fused kernel (two independent groups of 8 warps)
- *                            instead of the pipelined form (12 warps with fixed roles)
  * Process-wide, read at every call; 0 (default) = every specialised kernel.  CGTP_ERR_INVALID for unknown bits.
  * ------------------------------------------------------------------------------------------- */
 #define CGTP_PATH_GENERIC_CORE 1
@@ -378,7 +376,6 @@ int cgtp_message_field_parity(const float* node_feats, const int64_t* edge_index
 #define CGTP_PATH_GENERIC_SYNTH 8
 #define CGTP_PATH_UNFUSED_ONSITE 16
 #define CGTP_PATH_FUSED_ONSITE 32
-#define CGTP_PATH_FUSED_WG 64
 int cgtp_set_kernel_path(int flags);
 int cgtp_get_kernel_path(void);
 

@@ -34,7 +34,7 @@ inline int current_device()
 int num_sms();
 
 // Test-only kernel-path switch (cgtp_set_kernel_path): bit set = take the generic kernel where a specialised one exists.
-enum : int { PATH_GENERIC_CORE = 1, PATH_GENERIC_EDGE = 2, PATH_GENERIC_PROJ = 4, PATH_GENERIC_SYNTH = 8, PATH_UNFUSED_ONSITE = 16, PATH_FUSED_ONSITE = 32, PATH_FUSED_WG = 64 };
+enum : int { PATH_GENERIC_CORE = 1, PATH_GENERIC_EDGE = 2, PATH_GENERIC_PROJ = 4, PATH_GENERIC_SYNTH = 8, PATH_UNFUSED_ONSITE = 16, PATH_FUSED_ONSITE = 32 };
 int kernel_path();
 void set_kernel_path(int flags);
 

@@ -64,8 +64,6 @@ struct FusedArgs {
     // one, overlaid by the F planes and refilled during Q), the staged `out` block, the F planes of the two sub-groups
     // (gc column groups each, so that gc groups share one barrier per stage), then Ha | Hb
     int off_ab0, off_ab1, off_ost, off_fe, off_fo, off_h;
-    int off_h1;  // pipelined kernel: second H buffer
-    int debug;   // timing experiments only: bit 0 skips the core, bit 1 the projections (results are then meaningless)
     int dbl, gc;
 };
 
@@ -84,11 +82,6 @@ __device__ __forceinline__ float2 fz_lds64(uint32_t addr)
 __device__ __forceinline__ void bar_sync(int id, int nthreads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-
-__device__ __forceinline__ void bar_arrive(int id, int nthreads)
-{
-    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
 // One contraction index of a projection tile: acc[p][t] += (w[2p], w[2p+1]) * x[t] for the thread's 4 output rows (2 packed
@@ -188,18 +181,18 @@ __device__ __forceinline__ void core_groups(const FusedArgs& a, const CoreQParam
 
 // P: thread item = (factor, atom, column tile sl, row tile ct); rows (rank channels, parity-sorted order) ct + nct * i.
 __device__ __forceinline__ void phase_p(const FusedArgs& a, int wwarp, int lane, uint32_t sAB, uint32_t sW, float* Ha,
-                                        float* Hb, int tile_floats, int nwarps = kWgWarps, int f0 = 0, int f1 = 2)
+                                        float* Hb, int tile_floats)
 {
     const int N = a.N, C = a.C, Ce = a.Ce, Co = a.Co, NA = a.NA, L2 = a.L2, L2s = a.L2s;
     const int nct = C / kTM, nsl = a.nsl_in;
-    const int total = (f1 - f0) * NA * nsl * nct;
+    const int total = 2 * NA * nsl * nct;
     const bool mis = (L2 & 3) == 1;
-    for (int q = wwarp * 32 + lane; q < total; q += nwarps * 32) {
+    for (int q = wwarp * 32 + lane; q < total; q += kWgWarps * 32) {
         const int ct = q % nct;
         int r = q / nct;
         const int sl = r % nsl;
         r /= nsl;
-        const int at = r % NA, f = f0 + r / NA;
+        const int at = r % NA, f = r / NA;
         const int lm0 = sl * kTW;
         const int hi = (sl == nsl - 1) ? L2 : lm0 + kTW;
         float2 acc[2][kTJ];
@@ -225,13 +218,12 @@ __device__ __forceinline__ void phase_p(const FusedArgs& a, int wwarp, int lane,
 
 // Q: thread item = (sector, atom, column tile, row tile); rows = output channels jt + nnt * i; the T rows sit in place of
 // the factor-1 rows of H (stride L2s, 1 mod 4).
-__device__ __forceinline__ void phase_q(const FusedArgs& a, int wwarp, int lane, uint32_t sHa, uint32_t sW, float* OST,
-                                        int nwarps = kWgWarps)
+__device__ __forceinline__ void phase_q(const FusedArgs& a, int wwarp, int lane, uint32_t sHa, uint32_t sW, float* OST)
 {
     const int N = a.N, C = a.C, Ce = a.Ce, Co = a.Co, NA = a.NA, Lo2 = a.Lo2, L2s = a.L2s;
     const int nnt = N / kTM, nsl = a.nsl_out;
     const int total = 2 * NA * nsl * nnt;
-    for (int q = wwarp * 32 + lane; q < total; q += nwarps * 32) {
+    for (int q = wwarp * 32 + lane; q < total; q += kWgWarps * 32) {
         const int jt = q % nnt;
         int r = q / nnt;
         const int sl = r % nsl;
@@ -344,13 +336,6 @@ __global__ void __launch_bounds__(kFusedThreads, 1) onsite_fused_kernel(const __
 
     uint32_t phases = 0;  // bit b: parity to wait for on buffer b
     int buf = 0;
-    // The two warp groups do equal work per tile, so whatever phase relation they start with persists.  Started together
-    // they run P, core and Q in lockstep and the kernel time is the SUM of the FMA-bound projections and the latency-bound
-    // transforms (measured: 88 + 112 us + 47 us of exposed copies = 255 us at configs[1]); started half a tile apart, the
-    // projections of one group fill the issue slots the other group's transforms leave idle.
-    const bool stagger = (blockIdx.x * 2 + 1 < a.ntiles) && !(a.debug & 4);
-    bool first = true;
-    if (wg == 1 && stagger && tile < a.ntiles) bar_sync(7, 2 * kWgWarps * 32);
     for (; tile < a.ntiles; tile += tile_step) {
         const long long b0 = (long long)tile * NA;
         const int nb = (int)((a.batch - b0 < NA) ? (a.batch - b0) : NA);
@@ -361,16 +346,13 @@ __global__ void __launch_bounds__(kFusedThreads, 1) onsite_fused_kernel(const __
         const uint32_t sAB = smem_u32(ABuf[buf]);
 
         // ---- P (S1, Eq.(35)): H_f[col][lm] = sum_n W_f[c][n] X_f[a][n][lm]
-        if (!(a.debug & 2)) phase_p(a, wwarp, lane, sAB, sW, Ha, Hb, tile_floats);
-        if (first && wg == 0 && stagger) bar_arrive(7, 2 * kWgWarps * 32);  // release the other group after this group's first P
-        first = false;
+        phase_p(a, wwarp, lane, sAB, sW, Ha, Hb, tile_floats);
         // the previous tile's bulk store must have read OST before the F planes (which overlay it) are rewritten
         if (wtid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         bar_sync(bar_full, kWgWarps * 32);
 
         // ---- core (S2a-S4b): even and odd sub-groups side by side
-        if (a.debug & 1) {
-        } else if (wwarp < a.tab.we) {
+        if (wwarp < a.tab.we) {
             if (Ce > 0)
                 core_groups<LB, false>(a, qp, ta_e, wp, sched_e, a.tab.maxi_e, reinterpret_cast<float*>(wgm + a.off_fe), Ha,
                                        Hb, 0, NA * Ce / kFusedGW, wwarp, a.tab.we, bar_e, lane);
@@ -385,7 +367,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) onsite_fused_kernel(const __
         if (!a.dbl && wtid == 0 && tile + tile_step < a.ntiles) load_tile(tile + tile_step, 0);
 
         // ---- Q (S5, Eq.(41)): out[a][s][n][lm] = sum_{k in sector s} W_out[n][c_k] T[col(a,k)][lm]
-        if (!(a.debug & 2)) phase_q(a, wwarp, lane, sHa, sW, OST);
+        phase_q(a, wwarp, lane, sHa, sW, OST);
         fence_async_smem();
         bar_sync(bar_full, kWgWarps * 32);
         if (wtid == 0) {
@@ -395,164 +377,6 @@ __global__ void __launch_bounds__(kFusedThreads, 1) onsite_fused_kernel(const __
         if (a.dbl) buf ^= 1;
     }
     if (wtid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
-}
-
-// ------------------------------------------------------------------------------------------------
-// Pipelined form: ONE group of 12 warps per SM with fixed roles, three tiles in flight:
-//   warps 0-3  (one per scheduler): P of tile i+1, then Q of tile i-1 -- the FMA-dense projections, which one warp per
-//              scheduler already runs at the issue limit of packed FMAs;
-//   warps 4-11: the core of tile i, even sub-group and odd sub-group side by side (as in the warp-group form).
-// H is double-buffered, T overwrites the dead H rows in place, so P(i+1) fills one buffer while the core works in the
-// other and Q(i-1) drains it.  Hand-over by named barriers (bar.arrive by the producer role, bar.sync by the consumer
-// role); A and B arrive by separate TMA bulk copies, each re-issued as soon as the projection of its factor has read the
-// buffer, so the copy of tile i+2 flies under Q(i) and the other factor's projection.
-// ------------------------------------------------------------------------------------------------
-constexpr int kPipeProj = 4;                   // projection warps
-constexpr int kPipeThreads = 32 * (kPipeProj + 8);
-enum { BAR_PROJ = 1, BAR_EVEN = 2, BAR_ODD = 3, BAR_HFULL = 4, BAR_TFULL = 6 };
-
-template <int LB>
-__global__ void __launch_bounds__(kPipeThreads, 1) onsite_pipe_kernel(const __grid_constant__ FusedArgs a,
-                                                                      const __grid_constant__ CoreQParam<LB> qp)
-{
-    extern __shared__ __align__(128) unsigned char smem[];
-    uint64_t* bar_tab = reinterpret_cast<uint64_t*>(smem);
-    uint64_t* bar_in = reinterpret_cast<uint64_t*>(smem + 16);  // [2]: A, B of the current tile
-    const unsigned char* blob = smem + a.off_blob;
-    float* Wsm = reinterpret_cast<float*>(smem + a.off_w);
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int N = a.N, C = a.C, Ce = a.Ce, Co = a.Co, NA = a.NA, L2 = a.L2, Lo2 = a.Lo2, L2s = a.L2s;
-
-    if (tid == 0) {
-        mbar_init(bar_tab, 1);
-        mbar_init(&bar_in[0], 1);
-        mbar_init(&bar_in[1], 1);
-        mbar_fence_init();
-    }
-    __syncthreads();
-    if (tid == 0) {
-        mbar_arrive_expect_tx(bar_tab, (uint32_t)a.tab.bytes);
-        tma_load_span(smem + a.off_blob, a.blob, (uint32_t)a.tab.bytes, bar_tab);
-    }
-    unsigned char* base = smem + a.off_wg;
-    float* AB = reinterpret_cast<float*>(base + a.off_ab0);
-    float* OST = reinterpret_cast<float*>(base + a.off_ost);
-    float* Hbuf[2] = {reinterpret_cast<float*>(base + a.off_h), reinterpret_cast<float*>(base + a.off_h1)};
-    const int ncol = NA * C;
-    const int tile_floats = NA * N * L2;
-    const int n_mine = ((int)blockIdx.x < a.ntiles) ? (a.ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
-
-    auto load_half = [&](int tile, int f) {  // one thread
-        const long long b0 = (long long)tile * NA;
-        const int nb = (int)((a.batch - b0 < NA) ? (a.batch - b0) : NA);
-        const uint32_t bytes = (uint32_t)nb * N * L2 * 4u;
-        mbar_arrive_expect_tx(&bar_in[f], bytes);
-        tma_load_span(AB + (size_t)f * tile_floats, (f ? a.B : a.A) + b0 * N * L2, bytes, &bar_in[f]);
-    };
-    if (tid == 0 && n_mine > 0) {
-        load_half(blockIdx.x, 0);
-        load_half(blockIdx.x, 1);
-    }
-
-    // ---- weights -> shared memory in the order the projection tiles read them (see onsite_fused_kernel)
-    {
-        const int nct = C / kTM, nnt = N / kTM;
-        float* Wa_p = Wsm;
-        float* Wb_p = Wsm + (size_t)N * C;
-        for (int t = tid; t < N * C; t += kPipeThreads) {
-            const int c = t / N, k = t - c * N;
-            const int row = a.idx_in ? __ldg(a.idx_in + c) : c;
-            const int d = (k * nct + c % nct) * kTM + c / nct;
-            Wa_p[d] = __ldg(a.W_a + (size_t)row * N + k);
-            Wb_p[d] = __ldg(a.W_b + (size_t)row * N + k);
-        }
-        float* Wo = Wsm + (size_t)2 * N * C;
-        for (int s = 0; s < 2; ++s) {
-            const int Cs = s ? Co : Ce;
-            const int* idx = s ? a.idx_out_o : a.idx_out_e;
-            float* Wo_s = Wo + (s ? (size_t)Ce * N : 0);
-            for (int t = tid; t < N * Cs; t += kPipeThreads) {
-                const int n = t / Cs, k = t - n * Cs;
-                const int cidx = idx ? __ldg(idx + k) : (s ? Ce + k : k);
-                Wo_s[(k * nnt + n % nnt) * kTM + n / nnt] = __ldg(a.W_out + (size_t)n * a.ldw_out + cidx);
-            }
-        }
-    }
-    mbar_wait(bar_tab, 0);
-    __syncthreads();
-
-    const int we = a.tab.we, wo = a.tab.wo;
-    const int count_x = 32 * (kPipeProj + we + wo);  // threads of a hand-over barrier: both roles
-    const uint32_t sW = smem_u32(Wsm), sAB = smem_u32(AB);
-
-    if (warp < kPipeProj) {
-        // =============================== projection warps ===============================
-        const int ptid = tid;
-        uint32_t ph = 0;
-        for (int it = 0; it <= n_mine; ++it) {
-            if (it < n_mine) {
-                const int next = blockIdx.x + (it + 1) * gridDim.x;
-                float* Ha = Hbuf[it & 1];
-                float* Hb = Ha + (size_t)ncol * L2s;
-                // P (S1, Eq.(35)), factor by factor; each half of the input buffer is refilled as soon as it has been read
-                mbar_wait(&bar_in[0], ph);
-                if (!(a.debug & 2)) phase_p(a, warp, lane, sAB, sW, Ha, Hb, tile_floats, kPipeProj, 0, 1);
-                bar_sync(BAR_PROJ, 32 * kPipeProj);
-                if (ptid == 0 && it + 1 < n_mine) load_half(next, 0);
-                mbar_wait(&bar_in[1], ph);
-                if (!(a.debug & 2)) phase_p(a, warp, lane, sAB, sW, Ha, Hb, tile_floats, kPipeProj, 1, 2);
-                bar_sync(BAR_PROJ, 32 * kPipeProj);
-                if (ptid == 0 && it + 1 < n_mine) load_half(next, 1);
-                ph ^= 1u;
-                __threadfence_block();
-                bar_arrive(BAR_HFULL + (it & 1), count_x);  // H of tile `it` is complete
-            }
-            if (it >= 1) {
-                const int jt = it - 1;
-                const long long b0 = (long long)(blockIdx.x + jt * gridDim.x) * NA;
-                const int nb = (int)((a.batch - b0 < NA) ? (a.batch - b0) : NA);
-                bar_sync(BAR_TFULL + (jt & 1), count_x);    // T of tile jt is complete
-                if (ptid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // OST is free again
-                bar_sync(BAR_PROJ, 32 * kPipeProj);
-                // Q (S5, Eq.(41))
-                if (!(a.debug & 2)) phase_q(a, warp, lane, smem_u32(Hbuf[jt & 1]), sW, OST, kPipeProj);
-                fence_async_smem();
-                bar_sync(BAR_PROJ, 32 * kPipeProj);  // also: every projection warp has read T before P(it+1) refills the buffer
-                if (ptid == 0) {
-                    tma_store_1d(a.out + b0 * 2 * N * Lo2, OST, (uint32_t)nb * 2u * N * Lo2 * 4u);
-                    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-                }
-            }
-        }
-        if (ptid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
-        return;
-    }
-
-    // ================================== core warps ==================================
-    const int cw = warp - kPipeProj;
-    if (cw >= we + wo) return;
-    const float* ta_e = reinterpret_cast<const float*>(blob + a.tab.ta_e);
-    const float* ta_o = reinterpret_cast<const float*>(blob + a.tab.ta_o);
-    const float* wp = reinterpret_cast<const float*>(blob + a.tab.wp);
-    const int* sched_e = reinterpret_cast<const int*>(blob + a.tab.sched_e);
-    const int* sched_o = reinterpret_cast<const int*>(blob + a.tab.sched_o);
-    for (int it = 0; it < n_mine; ++it) {
-        float* Ha = Hbuf[it & 1];
-        float* Hb = Ha + (size_t)ncol * L2s;
-        bar_sync(BAR_HFULL + (it & 1), count_x);
-        if (a.debug & 1) {
-        } else if (cw < we) {
-            if (Ce > 0)
-                core_groups<LB, false>(a, qp, ta_e, wp, sched_e, a.tab.maxi_e, reinterpret_cast<float*>(base + a.off_fe), Ha, Hb, 0,
-                                       NA * Ce / kFusedGW, cw, we, BAR_EVEN, lane);
-        } else {
-            if (Co > 0)
-                core_groups<LB, true>(a, qp, ta_o, wp, sched_o, a.tab.maxi_o, reinterpret_cast<float*>(base + a.off_fo), Ha, Hb,
-                                      NA * Ce, NA * Co / kFusedGW, cw - we, wo, BAR_ODD, lane);
-        }
-        __threadfence_block();
-        bar_arrive(BAR_TFULL + (it & 1), count_x);
-    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -662,21 +486,6 @@ static int launch_fused_t(const FusedArgs& a, const FusedPlan* fp, int smem, int
     return CGTP_OK;
 }
 
-template <int LB>
-static int launch_pipe_t(const FusedArgs& a, const FusedPlan* fp, int smem, int64_t grid, cudaStream_t st)
-{
-    CoreQParam<LB> qp;
-    std::memset(&qp, 0, sizeof qp);
-    std::memcpy(qp.qf, fp->QF.data(), std::min(sizeof qp.qf, fp->QF.size() * sizeof(float)));
-    std::memcpy(qp.qi, fp->QI.data(), std::min(sizeof qp.qi, fp->QI.size() * sizeof(float)));
-    auto kern = onsite_pipe_kernel<LB>;
-    CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    LaunchScope scope(K_ONSITE_FUSED, st);
-    kern<<<(unsigned)grid, kPipeThreads, smem, st>>>(a, qp);
-    CGTP_CUDA_CHECK(cudaGetLastError());
-    return CGTP_OK;
-}
-
 int launch_onsite_fused(const Plan* p, int N, int C, int Ce, int Co, const float* A, const float* B, const float* W_a,
                         const float* W_b, const int* idx_in, const float* W_out, int ldw_out, const int* idx_out_e,
                         const int* idx_out_o, float* out, int64_t batch, cudaStream_t st, bool* handled)
@@ -706,7 +515,6 @@ int launch_onsite_fused(const Plan* p, int N, int C, int Ce, int Co, const float
     FusedArgs a;
     std::memset(&a, 0, sizeof a);
     a.N = N; a.C = C; a.Ce = Ce; a.Co = Co;
-    a.debug = (kernel_path() >> 8) & 7;
     a.lmax = p->lmax; a.lmax_out = p->lmax_out; a.L2 = p->L2; a.Lo2 = p->Lo2; a.L2s = p->L2 | 1; a.U = p->U; a.Uh = p->Uh;
     a.nsl_in = num_slices(p->L2);
     a.nsl_out = num_slices(p->Lo2);
@@ -716,52 +524,6 @@ int launch_onsite_fused(const Plan* p, int N, int C, int Ce, int Co, const float
     a.off_w = al128(a.off_blob + fp->tab.bytes);
     a.off_wg = al128(a.off_w + 3 * N * C * 4);
     const int fe_bytes = (Ce > 0 ? 2 : 0) * MR * RB * kFusedGW * 4, fo_bytes = (Co > 0 ? 4 : 0) * MR * RB * kFusedGW * 4;
-    // ---- pipelined kernel (12 warps with fixed roles, three tiles in flight) when its buffers fit: one A/B block, the
-    // staged `out` block, the F planes of gc groups per parity, two H buffers
-    if (!(kernel_path() & PATH_FUSED_WG)) {
-        auto plan_pipe = [&](int na, int gc) -> int {
-            int off = 0;
-            a.off_ab0 = off; off += al128(2 * na * N * p->L2 * 4 + 64);
-            a.off_ost = off; off += al128(na * 2 * N * p->Lo2 * 4);
-            a.off_fe = off; off += al128(gc * fe_bytes);
-            a.off_fo = off; off += al128(gc * fo_bytes);
-            const int hbytes = al128(2 * na * C * a.L2s * 4 + 64);
-            a.off_h = off; off += hbytes;
-            a.off_h1 = off; off += hbytes;
-            a.dbl = 0; a.gc = gc; a.wg_bytes = off;
-            const int total = a.off_wg + off;
-            return total <= 227 * 1024 ? total : 0;
-        };
-        int NAp = 0, smem_p = 0;
-        for (int na = 8; na >= 1 && !NAp; na /= 2) {
-            if ((na * Ce) % kFusedGW != 0 || (na * Co) % kFusedGW != 0) continue;
-            if (na > 1 && (batch + na - 1) / na < (int64_t)6 * num_sms()) continue;  // keep a few tiles per SM
-            const int ng = std::max(na * Ce, na * Co) / kFusedGW;
-            for (int gc = std::min(ng, 8); gc >= 1 && !NAp; gc /= 2)
-                if ((smem_p = plan_pipe(na, gc)) != 0) NAp = na;
-        }
-        if (NAp) {
-            a.NA = NAp;
-            *handled = true;
-            a.A = A; a.B = B; a.W_a = W_a; a.W_b = W_b; a.W_out = W_out;
-            a.idx_in = idx_in; a.idx_out_e = idx_out_e; a.idx_out_o = idx_out_o; a.ldw_out = ldw_out;
-            a.out = out;
-            a.batch = batch;
-            const int64_t ntiles = (batch + NAp - 1) / NAp;
-            if (ntiles > 2147483647LL / 4) { set_error("onsite fused: batch too large"); return CGTP_ERR_UNSUPPORTED; }
-            a.ntiles = (int)ntiles;
-            const int64_t grid = std::min<int64_t>(num_sms(), ntiles);
-            switch (LB) {
-#define CGTP_CASE(Bn) \
-    case Bn:          \
-        return launch_pipe_t<Bn>(a, fp, smem_p, grid, st);
-                CGTP_CASE(1) CGTP_CASE(2) CGTP_CASE(3) CGTP_CASE(4) CGTP_CASE(5) CGTP_CASE(6) CGTP_CASE(8)
-#undef CGTP_CASE
-            }
-            *handled = false;
-            return CGTP_OK;
-        }
-    }
     // Atoms per tile NA (whole column groups), concurrent groups gc and buffering: a roomy layout (two A/B buffers, the F
     // planes of gc groups next to them) when shared memory holds it -- more atoms per tile and fewer barriers amortise the
     // per-tile latencies of small shapes --, else the tight layout (one A/B buffer under the F planes, one group at a time).
