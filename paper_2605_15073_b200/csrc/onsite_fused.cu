@@ -28,15 +28,13 @@
 #include <mutex>
 
 #include "onsite_core.cuh"
+#include "proj_tile.cuh"
 
 namespace cgtp {
 
 constexpr int kFusedThreads = 512;
 constexpr int kWgWarps = 8;
 constexpr int kFusedGW = 16;   // columns per core group
-constexpr int kTM = 4;         // output rows per thread of a projection tile
-constexpr int kTW = 12;        // columns per projection tile (the last tile of a row may hold 13)
-constexpr int kTJ = 13;
 
 struct FusedTab {
     int ta_e, ta_o, wp, qf, qi, sched_e, sched_o, bytes;  // byte offsets into the table blob
@@ -67,57 +65,9 @@ struct FusedArgs {
     int dbl, gc;
 };
 
-__device__ __forceinline__ float4 fz_lds128(uint32_t addr)
-{
-    float4 v;
-    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ float2 fz_lds64(uint32_t addr)
-{
-    float2 v;
-    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
-    return v;
-}
 __device__ __forceinline__ void bar_sync(int id, int nthreads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-
-// One contraction index of a projection tile: acc[p][t] += (w[2p], w[2p+1]) * x[t] for the thread's 4 output rows (2 packed
-// pairs) and 13 columns.  x = 13 consecutive floats starting SHIFT floats after the 16-byte aligned shared-memory address
-// xb (loads the compiler finds unused are dropped); the 4 weights are one 128-bit load at wb.
-template <int SHIFT>
-__device__ __forceinline__ void tile_fma(float2 (&acc)[2][kTJ], uint32_t xb, uint32_t wb)
-{
-    const float4 a = fz_lds128(xb), b = fz_lds128(xb + 16), c = fz_lds128(xb + 32), d = fz_lds128(xb + 48);
-    const float v[16] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w, c.x, c.y, c.z, c.w, d.x, d.y, d.z, d.w};
-    const float4 w4 = fz_lds128(wb);
-    const float2 w0 = make_float2(w4.x, w4.y), w1 = make_float2(w4.z, w4.w);
-#pragma unroll
-    for (int t = 0; t < kTJ; ++t) {
-        const float2 x = make_float2(v[SHIFT + t], v[SHIFT + t]);
-        acc[0][t] = __ffma2_rn(w0, x, acc[0][t]);
-        acc[1][t] = __ffma2_rn(w1, x, acc[1][t]);
-    }
-}
-
-// A projection tile: acc[p][t] = sum_k W[k][rows 2p, 2p+1] * X[row k][lm0 + t].  x0 = byte address of (row 0, lm0), 16-byte
-// aligned; rows are row_bytes apart.  MIS: the row stride is 1 mod 4 floats, so row k starts k mod 4 floats past a 16-byte
-// boundary and the window is read from the boundary below it (static under the 4-fold unrolling); otherwise every row is
-// aligned.  w0 = byte address of the thread's 4 weights of k = 0, w_kstride bytes between k.  K is a multiple of 4.
-template <bool MIS>
-__device__ __forceinline__ void proj_tile(float2 (&acc)[2][kTJ], uint32_t x0, uint32_t row_bytes, uint32_t w0,
-                                          uint32_t w_kstride, int K)
-{
-#pragma unroll 2
-    for (int k0 = 0; k0 < K; k0 += 4) {
-        const uint32_t xb = x0 + (uint32_t)k0 * row_bytes, wb = w0 + (uint32_t)k0 * w_kstride;
-        tile_fma<0>(acc, xb, wb);
-        tile_fma<MIS ? 1 : 0>(acc, xb + row_bytes - (MIS ? 4u : 0u), wb + w_kstride);
-        tile_fma<MIS ? 2 : 0>(acc, xb + 2 * row_bytes - (MIS ? 8u : 0u), wb + 2 * w_kstride);
-        tile_fma<MIS ? 3 : 0>(acc, xb + 3 * row_bytes - (MIS ? 12u : 0u), wb + 3 * w_kstride);
-    }
 }
 
 // S2a-S4b for the groups of one parity, run by the nsub warps of a sub-group (2 workers = half-warps per warp).
@@ -464,13 +414,6 @@ static const FusedPlan* get_fused_plan(const Plan* p, int we, int wo)
 }
 
 static inline int al128(int x) { return (x + 127) / 128 * 128; }
-// column tiles per row: 12 wide, the last one up to 13 (13 + 3 floats of misalignment fill the 16-float window)
-static inline int num_slices(int L)
-{
-    if (L <= kTJ) return 1;
-    return (L % kTW == 1) ? (L - 1) / kTW : (L + kTW - 1) / kTW;
-}
-
 template <int LB>
 static int launch_fused_t(const FusedArgs& a, const FusedPlan* fp, int smem, int64_t grid, cudaStream_t st)
 {
@@ -516,8 +459,8 @@ int launch_onsite_fused(const Plan* p, int N, int C, int Ce, int Co, const float
     std::memset(&a, 0, sizeof a);
     a.N = N; a.C = C; a.Ce = Ce; a.Co = Co;
     a.lmax = p->lmax; a.lmax_out = p->lmax_out; a.L2 = p->L2; a.Lo2 = p->Lo2; a.L2s = p->L2 | 1; a.U = p->U; a.Uh = p->Uh;
-    a.nsl_in = num_slices(p->L2);
-    a.nsl_out = num_slices(p->Lo2);
+    a.nsl_in = proj_num_slices(p->L2);
+    a.nsl_out = proj_num_slices(p->Lo2);
     a.tab = fp->tab;
     a.blob = fp->blob;
     a.off_blob = 64;
