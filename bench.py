@@ -146,15 +146,22 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 # reference arm = the oracle on the host cores
 # ------------------------------------------------------------------------------------------------
-def oracle_onsite_rate(inp, n_atoms):
+def oracle_onsite_rate(inp, n_atoms, min_wall_s=0.0):
+    """The oracle as it stands on the host cores: passes over the first n_atoms atoms until min_wall_s of wall time has
+    gone by (at least one pass).  Returns (atoms/s, wall seconds, threads, passes)."""
     from oracle import cgtp_oracle as orc
     n = min(n_atoms, inp.batch)
     orc.real_coupling(inp.lmax, inp.lmax_out, False)
     orc.real_coupling(inp.lmax, inp.lmax_out, True)  # tables are set-up, not the timed work
     t0 = time.perf_counter()
-    orc.onsite(inp.A[:n], inp.B[:n], inp.W_a, inp.W_b, inp.W_out, inp.lmax, inp.lmax_out, inp.parity_mask)
-    dt = time.perf_counter() - t0
-    return n / dt, dt, orc.num_threads()
+    passes = 0
+    while True:
+        orc.onsite(inp.A[:n], inp.B[:n], inp.W_a, inp.W_b, inp.W_out, inp.lmax, inp.lmax_out, inp.parity_mask)
+        passes += 1
+        dt = time.perf_counter() - t0
+        if dt >= min_wall_s:
+            break
+    return n * passes / dt, dt, orc.num_threads(), passes
 
 
 def run_reference(args, rank, world):
@@ -369,9 +376,10 @@ def main():
     # ------------------------------------------------------------------ extras (rank 0, 1 GPU)
     if world == 1 and not args.no_extras:
         sampler2 = ClockSampler(local_rank, period=0.05).start()  # the extras get their own clock record
-        rate, dt_cpu, cores = oracle_onsite_rate(base, batch)
+        rate, dt_cpu, cores, passes = oracle_onsite_rate(base, batch, min_wall_s=1.5)
         line["cpu_baseline"] = {"value": rate, "unit": "contractions/s", "cores": cores, "kind": "oracle",
-                                "sample": f"all {batch} atoms of configs[1] once ({dt_cpu:.1f} s wall)"}
+                                "sample": f"all {batch} atoms of configs[1], {passes} passes ({dt_cpu:.1f} s wall, "
+                                          f"{dt_cpu * cores:.0f} s of CPU work)"}
         line["tensor_core"] = run_tensor_core(args, cg, step, out, lmax, lmax_out, N, C, Ce, Co, batch, peaks, peak_src)
         line["sweep"] = run_sweep(args, cg, synthetic, dev, fp32_peak_tflops, peaks)
         line["message"] = run_message(args, cg, synthetic, dev, peaks, peak_src)
@@ -382,9 +390,9 @@ def main():
         line["unfused_onsite"] = run_unfused(args, cg, step, fl, batch, fp32_peak_tflops, fp32_peak_measured)
         line["clocks_extras"] = sampler2.stop()
     elif world == 1:
-        rate, dt_cpu, cores = oracle_onsite_rate(base, 1024)
+        rate, dt_cpu, cores, passes = oracle_onsite_rate(base, 1024, min_wall_s=1.0)
         line["cpu_baseline"] = {"value": rate, "unit": "contractions/s", "cores": cores, "kind": "oracle",
-                                "sample": f"first 1024 atoms of configs[1] once ({dt_cpu:.1f} s wall)"}
+                                "sample": f"first 1024 atoms of configs[1], {passes} passes ({dt_cpu:.1f} s wall)"}
 
     if rank == 0:
         print(json.dumps(line), flush=True)
