@@ -839,7 +839,7 @@ int oracle_message_lwr(const double *node_feats, const int64_t *edge_index, cons
 /* truncating it earlier would change the result):                                               */
 /*   P_1 = H(1);  P_k[i] = sum_{a,b} Gr(a,b;i) P_{k-1}[a] H(k)[b],  band k*lmax;                 */
 /*   T = P_nu restricted to l <= lmax_out.                                                       */
-/* Nothing here touches a quadrature grid.  Reading R19: l-shared weights, rank       */
+/* Nothing here touches a quadrature grid.  Reading R23: l-shared weights, rank       */
 /* channels of the pointwise (even) kind only -- the curl pairing is bilinear and the paper       */
 /* gives no nu-body form of it.  Layouts: X [nu,batch,N,(lmax+1)^2]; W_in [nu,C,N]; W_out [N,C];  */
 /* out [batch,N,(lmax_out+1)^2].                                                                  */

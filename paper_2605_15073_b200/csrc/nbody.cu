@@ -8,7 +8,7 @@
 // (Eq.(39) :339), all in registers -> Gauss-Legendre analysis (Eq.(40) :342).  The grid is the plan's
 // U = ceil((nu lmax + lmax_out + 1)/2) x V = nu lmax + lmax_out + 1, on which the quadrature of the degree
 // nu lmax + lmax_out integrand is exact.  Grid fields exist only in registers, the per-row azimuthal coefficients only
-// in shared memory.  Pointwise (even) channels only: the curl pairing is bilinear (R19).
+// in shared memory.  Pointwise (even) channels only: the curl pairing is bilinear (R23).
 #include "sht.cuh"
 
 namespace cgtp {
