@@ -879,6 +879,15 @@ static int field_pass(const Plan* p, int N, int Ne, const FieldPass& q, const in
         }
         for (int s = 0; s < 2; ++s) {
             const int64_t nc = ec * Cpar[s];
+            if (nc > 0 && fast && !(kernel_path() & PATH_FIELD_PER_EDGE)) {
+                // neighbour sum on the grid inside the core (Eq.(52) :415): one inverse transform and one analysis per
+                // receiver, nothing per edge written to HBM
+                bool pooled = false;
+                rc = launch_field_pool_core(p, s == 1, Ha[s], Hn[s], edge_index, row_ptr, Cpar[s], status, Tn[s], nodes, e0,
+                                            e0 + ec, st, &pooled);
+                if (rc) return rc;
+                if (pooled) continue;
+            }
             if (nc > 0) {
                 // S2-S4 per edge: the edge field is factor 1 (R10), the sender's field factor 2 -- read in place through
                 // the edge list when the core's column groups do not straddle edges, else gathered into Hb first
@@ -1439,7 +1448,7 @@ int cgtp_get_math_mode(void) { return cgtp::get_math_mode(); }
 int cgtp_set_kernel_path(int flags)
 {
     clear_error();
-    if (flags < 0 || flags > 63) { set_error("unknown kernel-path flags %d", flags); return CGTP_ERR_INVALID; }
+    if (flags < 0 || flags > 127) { set_error("unknown kernel-path flags %d", flags); return CGTP_ERR_INVALID; }
     cgtp::set_kernel_path(flags);
     return CGTP_OK;
 }

@@ -34,7 +34,7 @@ inline int current_device()
 int num_sms();
 
 // Test-only kernel-path switch (cgtp_set_kernel_path): bit set = take the generic kernel where a specialised one exists.
-enum : int { PATH_GENERIC_CORE = 1, PATH_GENERIC_EDGE = 2, PATH_GENERIC_PROJ = 4, PATH_GENERIC_SYNTH = 8, PATH_UNFUSED_ONSITE = 16, PATH_FUSED_ONSITE = 32 };
+enum : int { PATH_GENERIC_CORE = 1, PATH_GENERIC_EDGE = 2, PATH_GENERIC_PROJ = 4, PATH_GENERIC_SYNTH = 8, PATH_UNFUSED_ONSITE = 16, PATH_FUSED_ONSITE = 32, PATH_FIELD_PER_EDGE = 64 };
 int kernel_path();
 void set_kernel_path(int flags);
 
@@ -226,6 +226,11 @@ int launch_onsite_fused(const Plan* p, int N, int C, int Ce, int Co, const float
 // Ha pairs with column send[e] * cpar + k of Hn.  *handled = false when the kernel's group width does not divide cpar.
 int launch_onsite_fast_gather(const Plan* p, bool odd, const float* Ha, const float* Hn, const int64_t* send, int cpar,
                               const int32_t* status, float* T, int64_t ncols, cudaStream_t st, bool* handled);
+
+// Two-field coupling with the neighbour sum on the grid (onsite_core.cu, field_pool_core_kernel): see there.
+int launch_field_pool_core(const Plan* p, bool odd, const float* Ha, const float* Hn, const int64_t* send,
+                           const int64_t* row_ptr, int cpar, const int32_t* status, float* Tn, int64_t nodes, int64_t e0,
+                           int64_t e1, cudaStream_t st, bool* handled);
 
 // nu-body form of S2-S4 (nbody.cu): T[col][Lo2p] = analysis of prod_s synthesis(H[s][col]); H holds nu blocks at
 // distance nbody_hfstride(p, ncols) floats, each [ncols][nbody_hstride(p)] (odd row stride), plus 4 rows of padding at

@@ -465,6 +465,226 @@ int launch_onsite_fast(const Plan* p, bool odd, const float* Ha, const float* Hb
     return CGTP_ERR_UNSUPPORTED;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Two-field coupling with the neighbour sum ON THE GRID (Eq.(52) PAPER.md:415 for Eq.(28) :236): one work item = (receiver,
+// group of GW rank channels).  The CTA walks the receiver's in-edges inside the chunk [e0, e1): per edge stage A of both
+// factors (the edge field's block of Ha, the sender's block of Hn through the edge list, TMA double-buffered) and the
+// forward half of stage B, whose quarter-wave combinations are summed over the edges in registers; then ONE inverse
+// transform and ONE Legendre analysis per receiver, added to Tn (a segment continued in the next chunk adds its part
+// there: fixed order, no floating-point atomics).  Against one full core pass per edge plus a pooling kernel this drops the
+// per-edge inverse transform, the per-edge analysis and the T round trip.
+// ------------------------------------------------------------------------------------------------
+struct PoolArgs {
+    CoreTab tab;
+    const void* blob;
+    const float* Ha;            // [e1 - e0][cpar][L2s]: projected edge field of the chunk
+    const float* Hn;            // [senders][cpar][L2s]
+    const long long* send;      // senders of the whole edge list
+    const long long* row_ptr;   // [nodes + 1]
+    float* Tn;                  // [nodes][cpar][Lo2s]
+    const int32_t* status;
+    long long nodes, e0, e1;
+    int cpar, lmax, lmax_out, U, Uh, NQ, L2s, Lo2s;
+    int off_blob, off_hs, off_f, off_ts, hs_bytes;
+};
+
+template <int LB, bool ODD>
+__global__ void __launch_bounds__(32 * kMaxWarps) field_pool_core_kernel(PoolArgs a, const __grid_constant__ CoreQParam<LB> qp)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    constexpr int MR = 2 * LB + 1;
+    constexpr int UB = core_ub(LB, ODD), RB = 2 * UB;
+    constexpr int GW = core_gw(LB, ODD), NH = 32 / GW;
+    constexpr int MAXR = (GW == 32) ? 3 : 2;  // grid rows per worker (host-checked)
+    constexpr int NQM = CoreQParam<LB>::NQMAX;
+    uint64_t* bar_tab = reinterpret_cast<uint64_t*>(smem);
+    uint64_t* bar_h = reinterpret_cast<uint64_t*>(smem + 16);  // [2]
+    const unsigned char* blob = smem + a.off_blob;
+    const float* ta = reinterpret_cast<const float*>(blob + a.tab.ta);
+    const float* wp = reinterpret_cast<const float*>(blob + a.tab.wp);
+    const int* sched = reinterpret_cast<const int*>(blob + a.tab.sched);
+    float* F = reinterpret_cast<float*>(smem + a.off_f);
+    float* Ts = reinterpret_cast<float*>(smem + a.off_ts);
+    constexpr int plane = MR * RB * GW;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, NW = blockDim.x >> 5;
+    const int col = lane & (GW - 1);
+    const int worker = warp * NH + lane / GW, nworkers = NW * NH;
+    const int hfl = GW * a.L2s;
+    const uint32_t hbytes = (uint32_t)hfl * 4;
+    const int ngrp = a.cpar / GW;
+    if (*a.status != 0) return;  // M0 flagged the edge list: send[] may not be dereferenced (Tn stays zero)
+
+    if (tid == 0) {
+        mbar_init(bar_tab, 1);
+        mbar_init(&bar_h[0], 1);
+        mbar_init(&bar_h[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (tid == 0) {
+        mbar_arrive_expect_tx(bar_tab, (uint32_t)a.tab.bytes);
+        tma_load_span(smem + a.off_blob, a.blob, (uint32_t)a.tab.bytes, bar_tab);
+    }
+    auto load_h = [&](long long e, int g, int buf) {
+        float* dst = reinterpret_cast<float*>(smem + a.off_hs + (size_t)buf * a.hs_bytes);
+        mbar_arrive_expect_tx(&bar_h[buf], 2 * hbytes);
+        tma_load_span(dst, a.Ha + ((size_t)(e - a.e0) * a.cpar + (size_t)g * GW) * a.L2s, hbytes, &bar_h[buf]);
+        tma_load_span(dst + hfl, a.Hn + ((size_t)a.send[e] * a.cpar + (size_t)g * GW) * a.L2s, hbytes, &bar_h[buf]);
+    };
+    mbar_wait(bar_tab, 0);
+
+    const int MAXI = a.tab.MAXI;
+    const int na = sched[0 * kMaxWorkers + worker], nc = sched[2 * kMaxWorkers + worker];
+    const int* ia = sched + 3 * kMaxWorkers + (0 * kMaxWorkers + worker) * MAXI;
+    const int* ic = sched + 3 * kMaxWorkers + (2 * kMaxWorkers + worker) * MAXI;
+    const int ne = a.Uh;
+    const int eq = (a.U & 1) ? a.Uh - 1 : -1;
+
+    int buf = 0;
+    uint32_t phases = 0u;
+    const long long nitems = a.nodes * ngrp;
+    for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
+        const long long i = item / ngrp;
+        const int g = (int)(item - i * ngrp);
+        const long long lo = a.row_ptr[i] > a.e0 ? a.row_ptr[i] : a.e0;
+        const long long hi = a.row_ptr[i + 1] < a.e1 ? a.row_ptr[i + 1] : a.e1;
+        if (lo >= hi) continue;
+        float2 acc[MAXR][NQM][2];
+#pragma unroll
+        for (int r = 0; r < MAXR; ++r)
+#pragma unroll
+            for (int v = 0; v < NQM; ++v) acc[r][v][0] = acc[r][v][1] = make_float2(0.f, 0.f);
+        if (tid == 0) load_h(lo, g, buf);
+        for (long long e = lo; e < hi; ++e) {
+            if (tid == 0 && e + 1 < hi) load_h(e + 1, g, buf ^ 1);
+            mbar_wait(&bar_h[buf], (phases >> buf) & 1u);
+            phases ^= 1u << buf;
+            const float* hs = reinterpret_cast<const float*>(smem + a.off_hs + (size_t)buf * a.hs_bytes);
+            const float* ha = hs + col * a.L2s;
+            const float* hb = hs + hfl + col * a.L2s;
+            for (int k = 0; k < na; ++k) {
+                if (!ODD) {
+                    stage_a_even<LB, UB, GW>(ta, a.tab.UP4, ha, hb, F, F + plane, ia[k], a.lmax, 0, ne, col);
+                } else {
+                    const int m = ia[k] >> 1, f = ia[k] & 1;
+                    stage_a_odd<LB, UB, GW>(ta, a.tab.UP2, f ? hb : ha, F + (2 * f) * plane, F + (2 * f + 1) * plane, m, a.lmax,
+                                            0, ne, col);
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int r = 0; r < MAXR; ++r) {
+                const int lr = worker + r * nworkers;
+                if (lr < RB) {
+                    const int e_ = (lr < UB) ? lr : lr - UB;
+                    if (!(e_ >= ne || (lr >= UB && e_ == eq)))
+                        stage_b_fwd_p<LB, ODD, RB, GW>(qp, F, plane, lr, a.NQ, col, acc[r]);
+                }
+            }
+            __syncthreads();  // F and this H buffer are free again
+            buf ^= 1;
+        }
+        // one inverse transform and one analysis for the pooled grid of the receiver
+#pragma unroll
+        for (int r = 0; r < MAXR; ++r) {
+            const int lr = worker + r * nworkers;
+            if (lr < RB) {
+                const int e_ = (lr < UB) ? lr : lr - UB;
+                if (!(e_ >= ne || (lr >= UB && e_ == eq))) stage_b_inv_p<LB, RB, GW>(qp, acc[r], F, lr, a.NQ, col);
+            }
+        }
+        __syncthreads();
+        for (int k = 0; k < nc; ++k) stage_c<LB, UB, GW>(wp, a.tab.UP4, F, Ts + col * a.Lo2s, ic[k], a.lmax_out, 0, ne, eq, true, col);
+        __syncthreads();
+        {
+            float* dst = a.Tn + ((size_t)i * a.cpar + (size_t)g * GW) * a.Lo2s;
+            const int n = GW * a.Lo2s;
+            for (int idx = tid; idx < n; idx += blockDim.x) dst[idx] += Ts[idx];
+        }
+        __syncthreads();
+    }
+}
+
+template <int LB, bool ODD>
+static int launch_pool_t(const Plan* p, const CorePlan* c, const float* Ha, const float* Hn, const int64_t* send,
+                         const int64_t* row_ptr, int cpar, const int32_t* status, float* Tn, int64_t nodes, int64_t e0,
+                         int64_t e1, cudaStream_t st, bool* handled)
+{
+    constexpr int GW = core_gw(LB, ODD), NH = 32 / GW, RB = 2 * core_ub(LB, ODD);
+    constexpr int MAXR = (GW == 32) ? 3 : 2;
+    *handled = false;
+    if (cpar % GW != 0) return CGTP_OK;
+    if ((RB + c->tab.NW * NH - 1) / (c->tab.NW * NH) > MAXR) return CGTP_OK;
+    const size_t smem = core_smem_bytes(p, ODD, c->tab, true);
+    if (smem + 1024 > kSmemPerSm) return CGTP_OK;
+    PoolArgs a;
+    a.tab = c->tab;
+    a.blob = c->blob;
+    a.Ha = Ha;
+    a.Hn = Hn;
+    a.send = reinterpret_cast<const long long*>(send);
+    a.row_ptr = reinterpret_cast<const long long*>(row_ptr);
+    a.Tn = Tn;
+    a.status = status;
+    a.nodes = nodes;
+    a.e0 = e0;
+    a.e1 = e1;
+    a.cpar = cpar;
+    a.lmax = p->lmax;
+    a.lmax_out = p->lmax_out;
+    a.U = p->U;
+    a.Uh = p->Uh;
+    a.NQ = c->tab.NQ;
+    a.L2s = onsite_fast_hstride(p);
+    a.Lo2s = onsite_fast_tstride(p);
+    a.hs_bytes = 2 * GW * a.L2s * 4;
+    a.off_blob = 64;
+    a.off_hs = a.off_blob + c->tab.bytes;
+    a.off_f = a.off_hs + 2 * a.hs_bytes;
+    a.off_ts = a.off_f + (ODD ? 4 : 2) * (2 * LB + 1) * RB * GW * 4;
+    auto kern = field_pool_core_kernel<LB, ODD>;
+    CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int ctas_per_sm = 0;
+    CGTP_CUDA_CHECK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, 32 * c->tab.NW, smem));
+    if (ctas_per_sm < 1) ctas_per_sm = 1;
+    const int64_t nitems = nodes * (cpar / GW);
+    int64_t grid = (int64_t)num_sms() * ctas_per_sm;
+    if (grid > nitems) grid = nitems;
+    CoreQParam<LB> qp;
+    std::memset(&qp, 0, sizeof qp);
+    std::memcpy(qp.qf, c->QF.data(), std::min(sizeof qp.qf, c->QF.size() * sizeof(float)));
+    std::memcpy(qp.qi, c->QI.data(), std::min(sizeof qp.qi, c->QI.size() * sizeof(float)));
+    *handled = true;
+    LaunchScope scope(ODD ? K_ONSITE_ODD : K_ONSITE_EVEN, st);
+    kern<<<(unsigned)grid, 32 * c->tab.NW, smem, st>>>(a, qp);
+    CGTP_CUDA_CHECK(cudaGetLastError());
+    return CGTP_OK;
+}
+
+// Ha: projected edge field of the edges [e0, e1) (columns (e - e0) * cpar + k), Hn: projected node field, send / row_ptr: the
+// whole receiver-sorted edge list; Tn[i] += analysis of the pooled product grids of receiver i's in-edges inside the chunk.
+// *handled = false when the shape is outside the kernel's limits (band limit > 8, cpar not a multiple of the group width):
+// the caller then runs the per-edge core and the pooling kernel.
+int launch_field_pool_core(const Plan* p, bool odd, const float* Ha, const float* Hn, const int64_t* send,
+                           const int64_t* row_ptr, int cpar, const int32_t* status, float* Tn, int64_t nodes, int64_t e0,
+                           int64_t e1, cudaStream_t st, bool* handled)
+{
+    *handled = false;
+    if (cpar <= 0 || nodes <= 0 || e1 <= e0 || p->LB > 8) return CGTP_OK;
+    const CorePlan* c = get_core_plan(p, odd);
+    if (!c) return CGTP_ERR_CUDA;
+    switch (p->LB) {
+#define CGTP_CASE(B)                                                                                              \
+    case B:                                                                                                       \
+        return odd ? launch_pool_t<B, true>(p, c, Ha, Hn, send, row_ptr, cpar, status, Tn, nodes, e0, e1, st, handled)  \
+                   : launch_pool_t<B, false>(p, c, Ha, Hn, send, row_ptr, cpar, status, Tn, nodes, e0, e1, st, handled);
+        CGTP_CASE(1) CGTP_CASE(2) CGTP_CASE(3) CGTP_CASE(4) CGTP_CASE(5) CGTP_CASE(6) CGTP_CASE(8)
+#undef CGTP_CASE
+    }
+    return CGTP_OK;
+}
+
 // Factor 2 gathered through the edge list (two-field coupling): column e * cpar + k pairs Ha's column with the block
 // of sender send[e] in Hn.  *handled = false when the group width does not divide cpar (the caller gathers into a
 // dense Hb and uses launch_onsite_fast).

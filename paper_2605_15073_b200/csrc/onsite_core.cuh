@@ -369,6 +369,102 @@ __device__ __forceinline__ void stage_b_p(const CoreQParam<LB>& qp, float* __res
     for (int m = 1; m <= LB; ++m) F[((LB + m) * RB + lr) * GW + lane] = ((m - 1) & 1) ? ts[(m - 1) / 2].y : ts[(m - 1) / 2].x;
 }
 
+// Stage B split in two for sums of products over several (factor 1, factor 2) pairs before ONE inverse transform (the
+// neighbour sum on the grid of Eq.(52) PAPER.md:415 for the two-field coupling Eq.(28): the product grids of a receiver's
+// in-edges are pooled before the analysis).  stage_b_fwd_p: forward transform and product of one grid row, the four
+// quarter-wave combinations of every table row ADDED to acc[vq] = (mc, ms); stage_b_inv_p: inverse transform of the
+// accumulated combinations into plane 0 of F.  Same arithmetic as stage_b_p, which is fwd + inv on a zero accumulator.
+template <int LB, bool ODD, int RB, int GW>
+__device__ __forceinline__ void stage_b_fwd_p(const CoreQParam<LB>& qp, const float* __restrict__ F, int plane_stride, int lr,
+                                              int NQ, int lane, float2 (&acc)[CoreQParam<LB>::NQMAX][2])
+{
+    constexpr int MR = 2 * LB + 1;
+    constexpr int NP = ODD ? 2 : 1;
+    float2 f[NP][MR];
+#pragma unroll
+    for (int r = 0; r < MR; ++r) {
+        const int idx = (r * RB + lr) * GW + lane;
+        f[0][r] = make_float2(F[idx], F[idx + plane_stride]);
+        if (ODD) f[NP - 1][r] = make_float2(F[idx + 2 * plane_stride], F[idx + 3 * plane_stride]);
+    }
+    constexpr int QFS = CoreQParam<LB>::QFS;
+#pragma unroll
+    for (int vq = 0; vq < CoreQParam<LB>::NQMAX; ++vq) {
+        if (vq >= NQ) break;
+        float2 Ce[NP], Co[NP], Se[NP], So[NP];
+#pragma unroll
+        for (int k = 0; k < NP; ++k) Ce[k] = Co[k] = Se[k] = So[k] = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int rr = 0; rr < MR; ++rr) {
+            const float qv = qp.qf[vq * QFS + rr];
+            const float2 q2 = make_float2(qv, qv);
+            const int m = (rr <= LB) ? rr : rr - LB;
+#pragma unroll
+            for (int k = 0; k < NP; ++k) {
+                if (rr <= LB) {
+                    if (m & 1) Co[k] = ffma2(f[k][rr], q2, Co[k]);
+                    else Ce[k] = ffma2(f[k][rr], q2, Ce[k]);
+                } else {
+                    if (m & 1) So[k] = ffma2(f[k][rr], q2, So[k]);
+                    else Se[k] = ffma2(f[k][rr], q2, Se[k]);
+                }
+            }
+        }
+        float2 g1[NP], g2[NP], g3[NP], g4[NP];
+#pragma unroll
+        for (int k = 0; k < NP; ++k) {
+            const float2 P = fadd2(Ce[k], Co[k]), Q = fsub2(Ce[k], Co[k]);
+            const float2 R = fadd2(Se[k], So[k]), T = fsub2(Se[k], So[k]);
+            g1[k] = fadd2(P, R);
+            g2[k] = fsub2(P, R);
+            g4[k] = fadd2(Q, T);
+            g3[k] = fsub2(Q, T);
+        }
+        float s1, s2, s3, s4;
+        if (!ODD) {
+            s1 = g1[0].x * g1[0].y;
+            s2 = g2[0].x * g2[0].y;
+            s3 = g3[0].x * g3[0].y;
+            s4 = g4[0].x * g4[0].y;
+        } else {
+            s1 = fmaf(g1[0].x, g1[NP - 1].y, -g1[0].y * g1[NP - 1].x);
+            s2 = fmaf(g2[0].x, g2[NP - 1].y, -g2[0].y * g2[NP - 1].x);
+            s3 = fmaf(g3[0].x, g3[NP - 1].y, -g3[0].y * g3[NP - 1].x);
+            s4 = fmaf(g4[0].x, g4[NP - 1].y, -g4[0].y * g4[NP - 1].x);
+        }
+        const float A = s1 + s2, B = s3 + s4, Cd = s1 - s2, D = s4 - s3;
+        acc[vq][0] = fadd2(acc[vq][0], make_float2(A + B, A - B));    // cosine rows: (even m, odd m)
+        acc[vq][1] = fadd2(acc[vq][1], make_float2(Cd - D, Cd + D));  // sine rows:   (odd m, even m)
+    }
+}
+
+template <int LB, int RB, int GW>
+__device__ __forceinline__ void stage_b_inv_p(const CoreQParam<LB>& qp, const float2 (&acc)[CoreQParam<LB>::NQMAX][2],
+                                              float* __restrict__ F, int lr, int NQ, int lane)
+{
+    constexpr int NTC = (LB + 2) / 2, NTS = (LB + 1) / 2;
+    constexpr int QIS = CoreQParam<LB>::QIS, SOFF = CoreQParam<LB>::SOFF;
+    float2 tc[NTC], ts[NTS > 0 ? NTS : 1];
+#pragma unroll
+    for (int k = 0; k < NTC; ++k) tc[k] = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int k = 0; k < NTS; ++k) ts[k] = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int vq = 0; vq < CoreQParam<LB>::NQMAX; ++vq) {
+        if (vq >= NQ) break;
+#pragma unroll
+        for (int k = 0; k < NTC; ++k)
+            tc[k] = ffma2(make_float2(qp.qi[vq * QIS + 2 * k], qp.qi[vq * QIS + 2 * k + 1]), acc[vq][0], tc[k]);
+#pragma unroll
+        for (int k = 0; k < NTS; ++k)
+            ts[k] = ffma2(make_float2(qp.qi[vq * QIS + SOFF + 2 * k], qp.qi[vq * QIS + SOFF + 2 * k + 1]), acc[vq][1], ts[k]);
+    }
+#pragma unroll
+    for (int m = 0; m <= LB; ++m) F[(m * RB + lr) * GW + lane] = (m & 1) ? tc[m / 2].y : tc[m / 2].x;
+#pragma unroll
+    for (int m = 1; m <= LB; ++m) F[((LB + m) * RB + lr) * GW + lane] = ((m - 1) & 1) ? ts[(m - 1) / 2].y : ts[(m - 1) / 2].x;
+}
+
 // Stage B for odd channels at band limits whose four coefficient vectors do not fit the register file: the curl
 // pairing {A,B} = A_theta B_phi - A_phi B_theta is evaluated as two product terms, each with its own forward
 // transform of one (factor-1 field, factor-2 field) pair, sharing the inverse-transform accumulators by linearity.

@@ -282,3 +282,47 @@ def test_field_parity_inversion_rotation_and_errors_on_gpu():
         run_field_parity(bad, check=True)
     assert ei.value.code == cg.ERR_GRAPH
     assert np.abs(run_field_parity(bad)).max() == 0.0  # zeros plus the flag
+
+
+# ------------------------------------------------------------ neighbour sum on the grid inside the core vs per-edge passes
+@pytest.fixture
+def default_path_after():
+    yield
+    cg.cgtp_set_kernel_path(0)
+
+
+@pytest.mark.parametrize("lmax,lmax_out,N,Ne,C,nodes,degree", [
+    (2, 2, 8, 4, 32, 40, "ragged"), (4, 4, 16, 8, 64, 61, "ragged"), (6, 6, 16, 16, 32, 50, 5), (8, 8, 8, 8, 32, 20, 40),
+    (3, 5, 6, 3, 32, 33, "ragged"),
+])
+def test_field_per_edge_path_vs_oracle(lmax, lmax_out, N, Ne, C, nodes, degree, default_path_after):
+    """The per-edge form (one full core pass per edge + pooling kernel, CGTP_PATH_FIELD_PER_EDGE) stays covered: against the
+    oracle, and against the default form (neighbour sum on the grid inside the core) to rounding."""
+    deg = _ragged(nodes, 9, lmax) if degree == "ragged" else degree
+    m = synthetic.make_message(lmax, lmax_out, N, C, nodes, deg, seed=70 + lmax)
+    XE, W_edge = synthetic.make_edge_field(m, Ne, seed=70)
+    ref = oracle_field(m, XE, W_edge)
+    got = run_field(m, XE, W_edge, check=True)
+    assert sector_err(got, ref) <= TOL
+    cg.cgtp_set_kernel_path(cg.PATH_FIELD_PER_EDGE)
+    n0 = cg.cgtp_launch_count()
+    alt = run_field(m, XE, W_edge, check=True)
+    n1 = cg.cgtp_launch_count()
+    assert sector_err(alt, ref) <= TOL
+    cg.cgtp_set_kernel_path(0)
+    run_field(m, XE, W_edge)
+    assert cg.cgtp_launch_count() - n1 <= n1 - n0  # the default form has no pooling launches where its group width divides the channels
+
+
+def test_field_configs4_graph_every_element_both_forms(default_path_after):
+    """The configs[4] graph (16 edge chunks, segments meeting chunk boundaries): the two forms agree on every element."""
+    lmax, N, Ne, C, nodes, degree = 8, 128, 8, 128, 16384, 32
+    m = synthetic.make_message(lmax, lmax, N, C, nodes, degree, r_max=6.0, seed=0)
+    XE, W_edge = synthetic.make_edge_field(m, Ne, seed=0)
+    T = [_cuda(x) for x in (m.node_feats, m.edge_index, XE, W_edge, m.W_node, m.W_out)]
+    f = lambda: cg.cgtp_message_field(*T, lmax, lmax, N, Ne, C, m.parity_mask, check=True)
+    a = f().clone()
+    cg.cgtp_set_kernel_path(cg.PATH_FIELD_PER_EDGE)
+    b = f()
+    for s in (0, 1):
+        assert ((a[:, s] - b[:, s]).abs().max() / b[:, s].abs().max()).item() < TOL

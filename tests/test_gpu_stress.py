@@ -110,6 +110,12 @@ def test_edge_lr_nbody_and_field_families_repeatable_and_in_bounds():
     ws = cg.cgtp_message_field_workspace_bytes(lmax, lmax, N, 4, C, nodes, m.E)
     _stress(lambda out, w: cg.cgtp_message_field(*F, lmax, lmax, N, 4, C, m.parity_mask, out=out, workspace=w),
             (nodes, 2, N, (lmax + 1) ** 2), ws)
+    m32 = synthetic.make_message(lmax, lmax, N, 32, nodes, np.random.default_rng(3).integers(0, 15, nodes), seed=46)
+    XE, We = synthetic.make_edge_field(m32, 4, seed=46)  # 16 channels per parity: the pooled core (field_pool_core_kernel)
+    F = [cuda(x) for x in (m32.node_feats, m32.edge_index, XE, We, m32.W_node, m32.W_out)]
+    ws = cg.cgtp_message_field_workspace_bytes(lmax, lmax, N, 4, 32, nodes, m32.E)
+    _stress(lambda out, w: cg.cgtp_message_field(*F, lmax, lmax, N, 4, 32, m32.parity_mask, out=out, workspace=w),
+            (nodes, 2, N, (lmax + 1) ** 2), ws)
     nb = synthetic.make_nbody(3, 3, 3, 8, 8, 130, seed=47)
     Xn = [cuda(x) for x in (nb.X, nb.W_in, nb.W_out)]
     ws = cg.cgtp_onsite_nbody_workspace_bytes(3, 3, 3, 8, 8, 130)
