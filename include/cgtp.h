@@ -159,7 +159,8 @@ int cgtp_message_field_bipartite(const float* node_feats, const int64_t* edge_in
  * X      device [nu, batch, N, (lmax+1)^2]     W_in  device [nu, C, N]     W_out  device [N, C]
  * out    device [batch, N, (lmax_out+1)^2]
  * workspace device, >= cgtp_onsite_nbody_workspace_bytes(...) bytes, 256-byte aligned (scratch)
- * 1 <= nu <= 4, max(lmax, lmax_out) <= 8 (CGTP_ERR_UNSUPPORTED beyond), 0 <= lmax_out <= nu*lmax
+ * 1 <= nu <= 4, max(lmax, lmax_out) <= cgtp_max_lmax() (CGTP_ERR_UNSUPPORTED beyond, and where fewer than four columns of
+ * the nu fields fit the shared memory of an SM: nu = 4 at band limit 20), 0 <= lmax_out <= nu*lmax
  * (CGTP_ERR_INVALID otherwise).  batch may be 0.  Asynchronous on cuda_stream, bitwise reproducible.
  * ------------------------------------------------------------------------------------------- */
 size_t cgtp_onsite_nbody_workspace_bytes(int nu, int lmax, int lmax_out, int N, int C, int64_t batch);

@@ -13,7 +13,7 @@
 
 namespace cgtp {
 
-constexpr int kNbodyMaxBand = 8;
+constexpr int kNbodyMaxBand = 20;
 constexpr int kNbodyMaxNu = 4;
 
 // H rows have the odd stride L2 | 1 (written so by S1): with lane = column the coefficient loads of the synthesis are
@@ -246,7 +246,7 @@ __device__ __forceinline__ void nbody_analysis(const float* Tr, const float* __r
 }
 
 template <int LB, int NU>
-__global__ void __launch_bounds__(256, 2) nbody_core_kernel(Plan p, NbodySmem lay, const float* __restrict__ H,
+__global__ void __launch_bounds__(256, (LB <= 8 ? 2 : 1)) nbody_core_kernel(Plan p, NbodySmem lay, const float* __restrict__ H,
                                                             long long hfs, float* __restrict__ T, long long ncols, int NC)
 {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -358,7 +358,7 @@ static int launch_nbody_t(const Plan* p, const float* H, float* T, int64_t ncols
     return CGTP_OK;
 }
 
-#define CGTP_FOR_EACH_NBODY_BAND(X) X(1) X(2) X(3) X(4) X(5) X(6) X(8)
+#define CGTP_FOR_EACH_NBODY_BAND(X) X(1) X(2) X(3) X(4) X(5) X(6) X(8) X(10) X(12) X(16) X(20)
 
 int launch_nbody(const Plan* p, const float* H, float* T, int64_t ncols, cudaStream_t st)
 {

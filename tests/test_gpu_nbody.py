@@ -34,6 +34,8 @@ def rel_err(got, ref):
     (3, 2, 2, 8, 8, 64), (3, 2, 6, 6, 5, 37), (4, 2, 2, 8, 8, 50), (4, 2, 8, 4, 6, 21), (3, 4, 4, 16, 12, 133),
     (2, 3, 5, 8, 8, 40), (1, 3, 2, 8, 4, 17), (3, 6, 6, 16, 16, 67), (4, 3, 3, 12, 10, 91), (3, 7, 7, 8, 8, 19),
     (3, 1, 3, 2, 2, 3), (4, 8, 8, 8, 4, 9), (3, 3, 0, 8, 8, 33),
+    # band limits above 8 (round 2): row counts U up to 41, one CTA per SM
+    (3, 12, 12, 8, 8, 21), (2, 16, 16, 4, 8, 13), (4, 10, 6, 4, 4, 9), (3, 9, 14, 4, 4, 7), (2, 20, 20, 4, 4, 6), (3, 16, 8, 4, 4, 5),
 ])
 def test_nbody_vs_oracle(nu, lmax, lmax_out, N, C, batch):
     inp = synthetic.make_nbody(nu, lmax, lmax_out, N, C, batch, seed=1000 * nu + 10 * lmax + lmax_out)
@@ -81,5 +83,5 @@ def test_nbody_grid_shape_and_errors():
         run_nbody(synthetic.make_nbody(5, 2, 2, 4, 4, 2))  # body order above the compiled limit
     assert e.value.code == cg.ERR_UNSUPPORTED
     with pytest.raises(cg.CgtpError) as e:
-        run_nbody(synthetic.make_nbody(3, 10, 10, 4, 4, 2))  # band limit above the nu-body limit
+        run_nbody(synthetic.make_nbody(4, 20, 20, 4, 4, 2))  # four fields of band 20 do not fit the shared memory of an SM
     assert e.value.code == cg.ERR_UNSUPPORTED
