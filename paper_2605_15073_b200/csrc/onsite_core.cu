@@ -65,7 +65,8 @@ void stage_items(const Plan* p, bool odd, std::vector<std::pair<int, int>> (&ite
         }
     }
     // stage B: one item per grid row of a row block, equal cost (the kernel deals them round-robin)
-    const int rows = LB <= 8 ? p->U : 2 * core_ub(LB, odd);
+    // (core_split: two half-rows per grid row)
+    const int rows = (LB <= 8 ? p->U : 2 * core_ub(LB, odd)) * (core_split(LB, odd) ? 2 : 1);
     for (int u = 0; u < rows; ++u) items[1].push_back({4, u});
     // stage C: one item per m <= lmax_out
     for (int m = 0; m <= p->lmax_out; ++m) items[2].push_back({(p->lmax_out - m + 1) + 1, m});
@@ -181,6 +182,7 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
         if (eff > best + 1e-9) { best = eff; bestNW = NW; }
     }
     t.NW = bestNW;
+    if (core_split(LB, odd)) t.NW = 2 * (2 * core_ub(LB, odd)) / NH;  // every (grid row, half of the azimuth rows) has its own half-warp: one pass
     std::vector<std::vector<int>> asg[3];
     int maxi = 1;
     for (int s = 0; s < 3; ++s) {
@@ -251,12 +253,12 @@ struct CoreArgs {
     const int32_t* status;
 };
 
-template <int LB, bool ODD>
+template <int LB, bool ODD, int UB = core_ub(LB, ODD), bool SPLIT = core_split(LB, ODD)>
 __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a, const __grid_constant__ CoreQParam<LB> qp)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int MR = 2 * LB + 1;
-    constexpr int UB = core_ub(LB, ODD), RB = 2 * UB;
+    constexpr int RB = 2 * UB;
     constexpr int GW = core_gw(LB, ODD), NH = 32 / GW;  // columns per group; schedule slots (workers) per warp
     constexpr bool TWO_TERM = ODD && LB >= 20;     // four coefficient vectors of 2 LB + 1 pairs exceed the registers
     uint64_t* bar_tab = reinterpret_cast<uint64_t*>(smem);
@@ -343,6 +345,20 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a,
 
             // ---- stage B: one local grid row per worker pass (north rows 0..ne-1, south rows UB..UB+ne-1; the
             // equator's southern copy is skipped)
+            if constexpr (SPLIT) {
+                // two warps per grid row, each with half of the azimuth rows; one pass (NW * NH == 2 RB)
+                const int nwh = NW >> 1, vh = warp / nwh;
+                const int lr = (warp - vh * nwh) * NH + lane / GW;
+                const int e = (lr < UB) ? lr : lr - UB;
+                const bool act = lr < RB && e < ne && !(lr >= UB && e == eq);
+                const int vqm = (a.Vh + 1) >> 1;
+                if constexpr (TWO_TERM)
+                    stage_b_two_term<LB, RB, GW, true>(qf, qi, a.tab.QFS, a.tab.QIS, a.tab.SOFF, F, plane, lr,
+                                                       vh ? a.Vh : vqm, col, act, vh ? vqm : 0, vh);
+                else
+                    stage_b<LB, ODD, RB, GW, true>(qf, qi, a.tab.QFS, a.tab.QIS, a.tab.SOFF, F, plane, lr,
+                                                   vh ? a.Vh : vqm, col, act, vh ? vqm : 0, vh);
+            } else
             for (int lr = worker; lr < RB; lr += nworkers) {
                 const int e = (lr < UB) ? lr : lr - UB;
                 if (e >= ne || (lr >= UB && e == eq)) continue;
@@ -359,7 +375,8 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a,
 
             // ---- stage C: quadrature over the block's rows, accumulated over the blocks
             for (int k = 0; k < nc; ++k)
-                stage_c<LB, UB, GW>(wp, a.tab.UP4, F, Ts + col * a.Lo2s, ic[k], a.lmax_out, e0, ne, eq, blk == 0, col);
+                stage_c<LB, UB, GW, SPLIT>(wp, a.tab.UP4, F, Ts + col * a.Lo2s, ic[k], a.lmax_out, e0, ne, eq, blk == 0, col,
+                                           plane);
             if (blk == nblk - 1) fence_async_smem();
             __syncthreads();
         }
@@ -397,7 +414,7 @@ bool onsite_fast_supported(const Plan* p, bool odd)
     return core_config(p, odd, c, &dbl) != 0;
 }
 
-template <int LB, bool ODD>
+template <int LB, bool ODD, int UB = core_ub(LB, ODD), bool SPLIT = core_split(LB, ODD)>
 static int launch_fast_t(const Plan* p, const CorePlan* c, const float* Ha, const float* Hb, float* T, int64_t ncols,
                          cudaStream_t st, const int64_t* send = nullptr, int cpar = 0, const int32_t* status = nullptr)
 {
@@ -427,8 +444,8 @@ static int launch_fast_t(const Plan* p, const CorePlan* c, const float* Ha, cons
     a.off_blob = 64;
     a.off_hs = a.off_blob + c->tab.bytes;
     a.off_f = a.off_hs + (dbl ? 2 : 1) * a.hs_bytes;
-    a.off_ts = a.off_f + (ODD ? 4 : 2) * (2 * LB + 1) * (2 * core_ub(LB, ODD)) * GW * 4;
-    auto kern = onsite_fast_kernel<LB, ODD>;
+    a.off_ts = a.off_f + (ODD ? 4 : 2) * (2 * LB + 1) * (2 * UB) * GW * 4;
+    auto kern = onsite_fast_kernel<LB, ODD, UB, SPLIT>;
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     // persistent CTAs: exactly as many as are resident at once (shared memory and registers both count)
     int ctas_per_sm = 0;

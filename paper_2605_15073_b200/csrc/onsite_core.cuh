@@ -36,8 +36,13 @@ __host__ __device__ constexpr int core_uhmax(int LB) { return ((3 * LB + 2) / 2 
 // (kept at 32); lmax 2 and 4 are slower with 16.
 __host__ __device__ constexpr int core_gw(int LB, bool odd) { return (LB >= 8 || (LB == 6 && odd)) ? 16 : 32; }
 // Northern nodes per row block of the fast kernel: all of them (one block) for band limits <= 8; four for the
-// larger ones.
-__host__ __device__ constexpr int core_ub(int LB, bool odd) { return LB <= 8 ? core_uhmax(LB) : 4; }
+// larger ones (eight for the odd channels at 16), and at band limit 20 two warps share a grid row in stage B
+// (core_split, see stage_b).  At 16 / 20 one group's H, T and F planes leave room for ONE CTA per SM, and with four-node
+// blocks that CTA had 4 warps (ncu: one warp per scheduler, issue slots 23-30 % used).  Measured on configs[3], core even /
+// odd in ms -- lmax 16: blocks of 4: 1.62 / 3.75 (even: 2 CTAs x 4 warps), split: 2.32 / 3.12, blocks of 8: 3.23 / 2.81;
+// lmax 20: blocks of 4: 4.67 / 6.18, split: 3.37 / 5.13, blocks of 8: 3.63 / does not fit.
+__host__ __device__ constexpr int core_ub(int LB, bool odd) { return LB <= 8 ? core_uhmax(LB) : (LB == 16 && odd) ? 8 : 4; }
+__host__ __device__ constexpr bool core_split(int LB, bool odd) { return LB >= 20; }
 
 
 // Host (onsite_core.cu): longest-processing-time assignment of (cost, id) items to NW workers.
@@ -187,9 +192,15 @@ struct CoreQParam {
     float qf[NQMAX * QFS], qi[NQMAX * QIS];
 };
 
-template <int LB, bool ODD, int RB, int GW>
+//
+// SPLIT (band limits whose shared-memory footprint leaves room for one small CTA only): two warps share a grid row, each
+// takes the azimuth rows [vq0, vq1) of the quarter-wave tables, and the two partial inverse transforms go to planes 0 and 1
+// (stage C adds them).  Both planes are inputs of the partner warp, hence the CTA-wide barrier between the last load and
+// the first store; `act` = this thread has a row (threads without one still take the barrier).
+template <int LB, bool ODD, int RB, int GW, bool SPLIT = false>
 __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const float* __restrict__ qi, int QFS, int QIS,
-                                        int SOFF, float* __restrict__ F, int plane_stride, int lr, int NQ, int lane)
+                                        int SOFF, float* __restrict__ F, int plane_stride, int lr, int NQ, int lane,
+                                        bool act = true, int vq0 = 0, int out_plane = 0)
 {
     constexpr int MR = 2 * LB + 1;
     constexpr int NTC = (LB + 2) / 2;  // pairs of cos rows (m = 2k, 2k+1)
@@ -197,11 +208,13 @@ __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const floa
     constexpr int NP = ODD ? 2 : 1;
     // f[k][r]: even: k = 0, pair (A, B); odd: k = 0 pair (A_theta, A_phi), k = 1 pair (B_theta, B_phi)
     float2 f[NP][MR];
+    if (!SPLIT || act) {
 #pragma unroll
-    for (int r = 0; r < MR; ++r) {
-        const int idx = (r * RB + lr) * GW + lane;
-        f[0][r] = make_float2(F[idx], F[idx + plane_stride]);
-        if (ODD) f[NP - 1][r] = make_float2(F[idx + 2 * plane_stride], F[idx + 3 * plane_stride]);
+        for (int r = 0; r < MR; ++r) {
+            const int idx = (r * RB + lr) * GW + lane;
+            f[0][r] = make_float2(F[idx], F[idx + plane_stride]);
+            if (ODD) f[NP - 1][r] = make_float2(F[idx + 2 * plane_stride], F[idx + 3 * plane_stride]);
+        }
     }
     float2 tc[NTC], ts[NTS > 0 ? NTS : 1];
 #pragma unroll
@@ -210,7 +223,7 @@ __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const floa
     for (int k = 0; k < NTS; ++k) ts[k] = make_float2(0.f, 0.f);
 
 #pragma unroll 2
-    for (int vq = 0; vq < NQ; ++vq) {
+    for (int vq = (SPLIT ? (act ? vq0 : NQ) : 0); vq < NQ; ++vq) {
         const float4* q4 = reinterpret_cast<const float4*>(qf + (size_t)vq * QFS);
         float2 Ce[NP], Co[NP], Se[NP], So[NP];
 #pragma unroll
@@ -270,6 +283,11 @@ __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const floa
         for (int k = 0; k < NTC; ++k) tc[k] = ffma2(qc2[k], mc, tc[k]);
 #pragma unroll
         for (int k = 0; k < NTS; ++k) ts[k] = ffma2(qs2[k], ms, ts[k]);
+    }
+    if (SPLIT) {
+        __syncthreads();
+        if (!act) return;
+        F += (size_t)out_plane * plane_stride;
     }
 #pragma unroll
     for (int m = 0; m <= LB; ++m) F[(m * RB + lr) * GW + lane] = (m & 1) ? tc[m / 2].y : tc[m / 2].x;
@@ -469,10 +487,10 @@ __device__ __forceinline__ void stage_b_inv_p(const CoreQParam<LB>& qp, const fl
 // pairing {A,B} = A_theta B_phi - A_phi B_theta is evaluated as two product terms, each with its own forward
 // transform of one (factor-1 field, factor-2 field) pair, sharing the inverse-transform accumulators by linearity.
 // F planes: 0 = A_theta, 1 = A_phi, 2 = B_theta, 3 = B_phi.
-template <int LB, int RB, int GW>
+template <int LB, int RB, int GW, bool SPLIT = false>
 __device__ __forceinline__ void stage_b_two_term(const float* __restrict__ qf, const float* __restrict__ qi, int QFS,
                                                  int QIS, int SOFF, float* __restrict__ F, int plane_stride, int lr,
-                                                 int NQ, int lane)
+                                                 int NQ, int lane, bool act = true, int vq0 = 0, int out_plane = 0)
 {
     constexpr int MR = 2 * LB + 1;
     constexpr int NTC = (LB + 2) / 2, NTS = (LB + 1) / 2;
@@ -486,13 +504,15 @@ __device__ __forceinline__ void stage_b_two_term(const float* __restrict__ qf, c
         const int pa = term ? 1 : 0, pb = term ? 2 : 3;
         const float sgn = term ? -1.f : 1.f;
         float2 f[MR];
+        if (!SPLIT || act) {
 #pragma unroll
-        for (int r = 0; r < MR; ++r) {
-            const int idx = (r * RB + lr) * GW + lane;
-            f[r] = make_float2(F[idx + pa * plane_stride], F[idx + pb * plane_stride]);
+            for (int r = 0; r < MR; ++r) {
+                const int idx = (r * RB + lr) * GW + lane;
+                f[r] = make_float2(F[idx + pa * plane_stride], F[idx + pb * plane_stride]);
+            }
         }
 #pragma unroll 2
-        for (int vq = 0; vq < NQ; ++vq) {
+        for (int vq = (SPLIT ? (act ? vq0 : NQ) : 0); vq < NQ; ++vq) {
             const float4* q4 = reinterpret_cast<const float4*>(qf + (size_t)vq * QFS);
             float2 Ce = make_float2(0.f, 0.f), Co = Ce, Se = Ce, So = Ce;
 #pragma unroll
@@ -528,6 +548,11 @@ __device__ __forceinline__ void stage_b_two_term(const float* __restrict__ qf, c
             for (int k = 0; k < NTS; ++k) ts[k] = ffma2(qs2[k], ms, ts[k]);
         }
     }
+    if (SPLIT) {
+        __syncthreads();
+        if (!act) return;
+        F += (size_t)out_plane * plane_stride;
+    }
 #pragma unroll
     for (int m = 0; m <= LB; ++m) F[(m * RB + lr) * GW + lane] = (m & 1) ? tc[m / 2].y : tc[m / 2].x;
 #pragma unroll
@@ -538,10 +563,10 @@ __device__ __forceinline__ void stage_b_two_term(const float* __restrict__ qf, c
 // (column, |m|); pairs are (+m, -m).  Ts: [32][Lo2s] staging for the bulk store; `first` = first block of the
 // group (store), later blocks accumulate.  eq = index e of the equator row in this block (its mirror image is the
 // row itself and stage B ran on the northern copy only), or -1.
-template <int LB, int UB, int GW>
+template <int LB, int UB, int GW, bool SPLIT = false>
 __device__ __forceinline__ void stage_c(const float* __restrict__ wp, int UP4, const float* __restrict__ F,
                                         float* __restrict__ ts_col, int m, int lmax_out, int e0, int ne, int eq,
-                                        bool first, int lane)
+                                        bool first, int lane, int plane_stride = 0)
 {
     constexpr int RB = 2 * UB;
     float2 tp[UB], tm[UB];
@@ -555,6 +580,12 @@ __device__ __forceinline__ void stage_c(const float* __restrict__ wp, int UP4, c
             n.x = F[rn];
             s.x = F[rs];
             if (m > 0) { n.y = F[rn + off]; s.y = F[rs + off]; }
+            if (SPLIT) {  // the two halves of the azimuth sum (stage_b, SPLIT)
+                const float* F1 = F + plane_stride;
+                n.x += F1[rn];
+                s.x += F1[rs];
+                if (m > 0) { n.y += F1[rn + off]; s.y += F1[rs + off]; }
+            }
         }
         tp[e] = fadd2(n, s);
         tm[e] = fsub2(n, s);
