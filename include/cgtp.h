@@ -371,6 +371,8 @@ int cgtp_message_field_parity(const float* node_feats, const int64_t* edge_index
  *                            choice is the four-launch step (narrow projections N * C < 4096)
  *   CGTP_PATH_FIELD_PER_EDGE two-field coupling: one full core pass per edge and a pooling kernel (edge_field.cu) instead of
  *                            the neighbour sum on the grid inside the core (field_pool_core_kernel, onsite_core.cu)
+ *   CGTP_PATH_SMEM_CORE      S2-S4 at band limits <= 6: the warp-scheduled shared-memory core (onsite_core.cu) instead of
+ *                            the one-thread-per-column register core (onsite_reg.cu)
  * Process-wide, read at every call; 0 (default) = every specialised kernel.  CGTP_ERR_INVALID for unknown bits.
  * ------------------------------------------------------------------------------------------- */
 #define CGTP_PATH_GENERIC_CORE 1
@@ -380,6 +382,7 @@ int cgtp_message_field_parity(const float* node_feats, const int64_t* edge_index
 #define CGTP_PATH_UNFUSED_ONSITE 16
 #define CGTP_PATH_FUSED_ONSITE 32
 #define CGTP_PATH_FIELD_PER_EDGE 64
+#define CGTP_PATH_SMEM_CORE 128
 int cgtp_set_kernel_path(int flags);
 int cgtp_get_kernel_path(void);
 

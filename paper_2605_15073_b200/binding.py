@@ -596,6 +596,7 @@ MATH_FP32, MATH_3XTF32, MATH_TF32 = 0, 1, 2
 PATH_GENERIC_CORE, PATH_GENERIC_EDGE, PATH_GENERIC_PROJ, PATH_GENERIC_SYNTH, PATH_UNFUSED_ONSITE = 1, 2, 4, 8, 16
 PATH_FUSED_ONSITE = 32
 PATH_FIELD_PER_EDGE = 64
+PATH_SMEM_CORE = 128
 
 
 def cgtp_set_kernel_path(flags: int) -> None:

@@ -1448,7 +1448,7 @@ int cgtp_get_math_mode(void) { return cgtp::get_math_mode(); }
 int cgtp_set_kernel_path(int flags)
 {
     clear_error();
-    if (flags < 0 || flags > 127) { set_error("unknown kernel-path flags %d", flags); return CGTP_ERR_INVALID; }
+    if (flags < 0 || flags > 255) { set_error("unknown kernel-path flags %d", flags); return CGTP_ERR_INVALID; }
     cgtp::set_kernel_path(flags);
     return CGTP_OK;
 }

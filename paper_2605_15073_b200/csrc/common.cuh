@@ -34,7 +34,7 @@ inline int current_device()
 int num_sms();
 
 // Test-only kernel-path switch (cgtp_set_kernel_path): bit set = take the generic kernel where a specialised one exists.
-enum : int { PATH_GENERIC_CORE = 1, PATH_GENERIC_EDGE = 2, PATH_GENERIC_PROJ = 4, PATH_GENERIC_SYNTH = 8, PATH_UNFUSED_ONSITE = 16, PATH_FUSED_ONSITE = 32, PATH_FIELD_PER_EDGE = 64 };
+enum : int { PATH_GENERIC_CORE = 1, PATH_GENERIC_EDGE = 2, PATH_GENERIC_PROJ = 4, PATH_GENERIC_SYNTH = 8, PATH_UNFUSED_ONSITE = 16, PATH_FUSED_ONSITE = 32, PATH_FIELD_PER_EDGE = 64, PATH_SMEM_CORE = 128 };
 int kernel_path();
 void set_kernel_path(int flags);
 
@@ -213,6 +213,12 @@ inline int onsite_fast_hstride(const Plan* p) { return p->L2 | 1; }
 inline int onsite_fast_tstride(const Plan* p) { return p->Lo2 | 1; }
 int launch_onsite_fast(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols,
                        cudaStream_t st);
+// Register-resident core for small band limits (onsite_reg.cu): one thread per column, nothing exchanged between
+// threads; same buffers and strides as the fast kernel, which hands the band limits of onsite_reg_supported() over to it
+// unless CGTP_PATH_SMEM_CORE is set.  send / cpar / status as in launch_onsite_fast_field (cpar a multiple of 32).
+bool onsite_reg_supported(const Plan* p, bool odd);
+int launch_onsite_reg(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols, cudaStream_t st,
+                      const int64_t* send, int cpar, const int32_t* status);
 
 // S1-S5 in one kernel (onsite_fused.cu): reads A, B once, writes out once, H and T stay in shared memory.  idx_in[k] = row
 // of W_a / W_b of internal (parity-sorted) channel k; idx_out_e / idx_out_o = column of W_out of the even / odd channels;

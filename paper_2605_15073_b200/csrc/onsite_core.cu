@@ -467,6 +467,8 @@ int launch_onsite_fast(const Plan* p, bool odd, const float* Ha, const float* Hb
                        cudaStream_t st)
 {
     if (ncols <= 0) return CGTP_OK;
+    if (onsite_reg_supported(p, odd) && !(kernel_path() & PATH_SMEM_CORE))
+        return launch_onsite_reg(p, odd, Ha, Hb, T, ncols, st, nullptr, 0, nullptr);
     const CorePlan* c = get_core_plan(p, odd);
     if (!c) return CGTP_ERR_CUDA;
     switch (p->LB) {

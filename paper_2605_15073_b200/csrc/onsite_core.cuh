@@ -295,31 +295,20 @@ __device__ __forceinline__ void stage_b(const float* __restrict__ qf, const floa
     for (int m = 1; m <= LB; ++m) F[((LB + m) * RB + lr) * GW + lane] = ((m - 1) & 1) ? ts[(m - 1) / 2].y : ts[(m - 1) / 2].x;
 }
 
-template <int LB, bool ODD, int RB, int GW>
-__device__ __forceinline__ void stage_b_p(const CoreQParam<LB>& qp, float* __restrict__ F, int plane_stride, int lr, int NQ,
-                                          int lane)
+// Stage B of one (column, grid row) on registers.  f[k][r]: coefficient rows r = m (cosine, 0..LB), LB + m (sine); even
+// channels: k = 0, pair (A, B); odd channels: PAIR_AB = false: f[0] = (A_theta, A_phi), f[1] = (B_theta, B_phi);
+// PAIR_AB = true: f[0] = (A_theta, B_theta), f[1] = (A_phi, B_phi).  Result: tc[k] = cosine rows (m = 2k, 2k+1),
+// ts[k] = sine rows (m = 2k+1, 2k+2), ADDED to the caller's values.  Fully unrolled over the largest table of the band
+// limit: every table index is a compile-time constant, the values are constant-bank / uniform-register operands.
+template <int LB, bool ODD, bool PAIR_AB = false>
+__device__ __forceinline__ void stage_b_regs(const CoreQParam<LB>& qp, const float2 (&f)[ODD ? 2 : 1][2 * LB + 1], int NQ,
+                                             float2 (&tc)[(LB + 2) / 2], float2 (&ts)[(LB + 1) / 2 > 0 ? (LB + 1) / 2 : 1])
 {
     constexpr int MR = 2 * LB + 1;
     constexpr int NTC = (LB + 2) / 2;  // pairs of cos rows (m = 2k, 2k+1)
     constexpr int NTS = (LB + 1) / 2;  // pairs of sin rows (m = 2k+1, 2k+2)
     constexpr int NP = ODD ? 2 : 1;
-    // f[k][r]: even: k = 0, pair (A, B); odd: k = 0 pair (A_theta, A_phi), k = 1 pair (B_theta, B_phi)
-    float2 f[NP][MR];
-#pragma unroll
-    for (int r = 0; r < MR; ++r) {
-        const int idx = (r * RB + lr) * GW + lane;
-        f[0][r] = make_float2(F[idx], F[idx + plane_stride]);
-        if (ODD) f[NP - 1][r] = make_float2(F[idx + 2 * plane_stride], F[idx + 3 * plane_stride]);
-    }
-    float2 tc[NTC], ts[NTS > 0 ? NTS : 1];
-#pragma unroll
-    for (int k = 0; k < NTC; ++k) tc[k] = make_float2(0.f, 0.f);
-#pragma unroll
-    for (int k = 0; k < NTS; ++k) ts[k] = make_float2(0.f, 0.f);
-
     constexpr int QFS = CoreQParam<LB>::QFS, QIS = CoreQParam<LB>::QIS, SOFF = CoreQParam<LB>::SOFF;
-    // fully unrolled over the largest table of the band limit: every table index is a compile-time constant, the values
-    // are constant-bank / uniform-register operands of the FMAs
 #pragma unroll
     for (int vq = 0; vq < CoreQParam<LB>::NQMAX; ++vq) {
         if (vq >= NQ) break;
@@ -364,12 +353,17 @@ __device__ __forceinline__ void stage_b_p(const CoreQParam<LB>& qp, float* __res
             s2 = g2[0].x * g2[0].y;
             s3 = g3[0].x * g3[0].y;
             s4 = g4[0].x * g4[0].y;
-        } else {
+        } else if (!PAIR_AB) {
             // Eq.(11): {A,B} = A_theta B_phi - A_phi B_theta  (A factor 1, B factor 2)
             s1 = fmaf(g1[0].x, g1[NP - 1].y, -g1[0].y * g1[NP - 1].x);
             s2 = fmaf(g2[0].x, g2[NP - 1].y, -g2[0].y * g2[NP - 1].x);
             s3 = fmaf(g3[0].x, g3[NP - 1].y, -g3[0].y * g3[NP - 1].x);
             s4 = fmaf(g4[0].x, g4[NP - 1].y, -g4[0].y * g4[NP - 1].x);
+        } else {
+            s1 = fmaf(g1[0].x, g1[NP - 1].y, -g1[NP - 1].x * g1[0].y);
+            s2 = fmaf(g2[0].x, g2[NP - 1].y, -g2[NP - 1].x * g2[0].y);
+            s3 = fmaf(g3[0].x, g3[NP - 1].y, -g3[NP - 1].x * g3[0].y);
+            s4 = fmaf(g4[0].x, g4[NP - 1].y, -g4[NP - 1].x * g4[0].y);
         }
         const float A = s1 + s2, B = s3 + s4, Cd = s1 - s2, D = s4 - s3;
         const float2 mc = make_float2(A + B, A - B);    // cosine rows: (even m, odd m)
@@ -381,6 +375,28 @@ __device__ __forceinline__ void stage_b_p(const CoreQParam<LB>& qp, float* __res
         for (int k = 0; k < NTS; ++k)
             ts[k] = ffma2(make_float2(qp.qi[vq * QIS + SOFF + 2 * k], qp.qi[vq * QIS + SOFF + 2 * k + 1]), ms, ts[k]);
     }
+}
+
+template <int LB, bool ODD, int RB, int GW>
+__device__ __forceinline__ void stage_b_p(const CoreQParam<LB>& qp, float* __restrict__ F, int plane_stride, int lr, int NQ,
+                                          int lane)
+{
+    constexpr int MR = 2 * LB + 1;
+    constexpr int NTC = (LB + 2) / 2, NTS = (LB + 1) / 2;
+    constexpr int NP = ODD ? 2 : 1;
+    float2 f[NP][MR];
+#pragma unroll
+    for (int r = 0; r < MR; ++r) {
+        const int idx = (r * RB + lr) * GW + lane;
+        f[0][r] = make_float2(F[idx], F[idx + plane_stride]);
+        if (ODD) f[NP - 1][r] = make_float2(F[idx + 2 * plane_stride], F[idx + 3 * plane_stride]);
+    }
+    float2 tc[NTC], ts[NTS > 0 ? NTS : 1];
+#pragma unroll
+    for (int k = 0; k < NTC; ++k) tc[k] = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int k = 0; k < NTS; ++k) ts[k] = make_float2(0.f, 0.f);
+    stage_b_regs<LB, ODD>(qp, f, NQ, tc, ts);
 #pragma unroll
     for (int m = 0; m <= LB; ++m) F[(m * RB + lr) * GW + lane] = (m & 1) ? tc[m / 2].y : tc[m / 2].x;
 #pragma unroll

@@ -41,7 +41,8 @@ def sanitize():
 
     onsite(2, 8, 8, 64)                                  # configs[0]: onsite_fused (roomy layout)
     onsite(6, 64, 64, 20)                                # onsite_fused (tight layout)
-    onsite(6, 64, 64, 70, path=cg.PATH_UNFUSED_ONSITE)   # proj_fast + onsite_fast
+    onsite(6, 64, 64, 70, path=cg.PATH_UNFUSED_ONSITE | cg.PATH_SMEM_CORE)  # proj_fast + onsite_fast
+    onsite(4, 16, 16, 70, path=cg.PATH_UNFUSED_ONSITE)   # onsite_reg (one thread per column)
     onsite(12, 8, 8, 40, path=cg.PATH_UNFUSED_ONSITE)    # onsite_fast, row blocks
     onsite(4, 16, 16, 50, path=cg.PATH_UNFUSED_ONSITE | cg.PATH_GENERIC_CORE | cg.PATH_GENERIC_PROJ)
     onsite(4, 24, 40, 70, path=cg.PATH_UNFUSED_ONSITE, mode=cg.MATH_3XTF32)  # proj_tc (tcgen05)

@@ -72,14 +72,28 @@ def test_onsite_config3_fused_kernel_whole_batch(lmax):
     assert max(e) < TOL, e
 
 
+@pytest.mark.parametrize("lmax", [2, 4])
+def test_onsite_config3_both_cores_whole_batch(lmax):
+    """configs[3] at small band limits: the one-thread-per-column register core (onsite_reg.cu, the library's choice) and
+    the warp-scheduled shared-memory core (onsite_core.cu, CGTP_PATH_SMEM_CORE) on the whole batch, element by element."""
+    inp = synthetic.config(3, lmax=lmax)
+    A, B = cuda(inp.A), cuda(inp.B)
+    cg.cgtp_set_kernel_path(cg.PATH_UNFUSED_ONSITE)
+    got = onsite_dev(inp, A, B).clone()
+    cg.cgtp_set_kernel_path(cg.PATH_UNFUSED_ONSITE | cg.PATH_SMEM_CORE)
+    alt = onsite_dev(inp, A, B)
+    e = sector_errs_torch(got, alt)
+    assert max(e) < TOL, e
+
+
 def test_onsite_config1_every_kernel_path_agrees():
     """configs[1] (the bench workload; the oracle checks every output in test_gpu_parity.py): fused step, four-launch
     step and the generic kernels agree element by element."""
     inp = synthetic.config(1)
     A, B = cuda(inp.A), cuda(inp.B)
     got = onsite_dev(inp, A, B).clone()
-    for flags in (cg.PATH_UNFUSED_ONSITE, cg.PATH_UNFUSED_ONSITE | cg.PATH_GENERIC_CORE,
-                  cg.PATH_UNFUSED_ONSITE | cg.PATH_GENERIC_PROJ, GENERIC_ALL):
+    for flags in (cg.PATH_UNFUSED_ONSITE, cg.PATH_UNFUSED_ONSITE | cg.PATH_SMEM_CORE,
+                  cg.PATH_UNFUSED_ONSITE | cg.PATH_GENERIC_CORE, cg.PATH_UNFUSED_ONSITE | cg.PATH_GENERIC_PROJ, GENERIC_ALL):
         cg.cgtp_set_kernel_path(flags)
         assert cg.cgtp_get_kernel_path() == flags
         alt = onsite_dev(inp, A, B)

@@ -122,6 +122,35 @@ def test_onsite_fused_kernel_shapes(lmax, lmax_out, N, C, batch, mask, default_p
     assert max(e) < TOL, e
 
 
+@pytest.mark.parametrize("lmax,lmax_out,N,C,batch,mask", [
+    (1, 1, 8, 8, 70, None),
+    (2, 2, 8, 16, 129, None),
+    (3, 3, 8, 8, 300, [0, 0, 0, 1, 1, 1, 1, 1]),   # 3 even + 5 odd channels: ragged column groups in both parities
+    (4, 4, 32, 32, 300, None),                     # configs[3] shape at lmax 4
+    (4, 2, 8, 8, 33, None),                        # lmax_out < lmax: T shorter than H
+    (2, 4, 8, 8, 33, None),                        # lmax_out > lmax: band limit 4 kernel, H has 9 coefficients
+    (5, 5, 8, 16, 65, None),                       # H re-read from shared memory per grid row (band limits 5, 6)
+    (3, 6, 8, 8, 21, None),                        # band limit 6: register core for the odd channels only
+    (6, 6, 16, 16, 47, [1] * 16),                  # all odd at band limit 6
+    (4, 4, 8, 8, 1, None),                         # one atom: a single partly filled group
+])
+def test_onsite_register_and_shared_memory_cores(lmax, lmax_out, N, C, batch, mask, default_path_after):
+    """S2a-S4b at small band limits have two cores: one thread per column with everything in registers (onsite_reg.cu, the
+    library's choice for band limits <= 5 and the odd channels at 6) and the warp-scheduled shared-memory core
+    (onsite_core.cu, CGTP_PATH_SMEM_CORE).  Both against the oracle on the four-launch step."""
+    inp = synthetic.make_onsite(lmax, lmax_out, N, C, batch, seed=700 + 10 * lmax + lmax_out, parity_mask=mask)
+    ref = oracle_onsite(inp)
+    outs = []
+    for flags in (cg.PATH_UNFUSED_ONSITE, cg.PATH_UNFUSED_ONSITE | cg.PATH_SMEM_CORE):
+        cg.cgtp_set_kernel_path(flags)
+        got = run_onsite(inp)
+        e = sector_err(got, ref)
+        assert max(e) < TOL, (flags, e)
+        assert np.array_equal(got, run_onsite(inp))  # bitwise reproducible
+        outs.append(got)
+    assert not np.array_equal(outs[0], outs[1])  # two different kernels did run (different summation orders)
+
+
 def test_onsite_config1_full():
     """BASELINE.json configs[1] (the bench workload): lmax=6, N=C=64, batch=4096, every output checked."""
     inp = synthetic.config(1)

@@ -65,7 +65,10 @@ def defaults_after():
     ("fused_roomy", 2, 8, 8, 203, cg.PATH_FUSED_ONSITE, 0),
     ("fused_tight", 6, 64, 64, 333, 0, 0),
     ("fused_mid", 4, 32, 32, 1001, cg.PATH_FUSED_ONSITE, 0),
-    ("proj_fast+onsite_fast", 6, 64, 64, 333, cg.PATH_UNFUSED_ONSITE, 0),
+    ("proj_fast+onsite_fast", 6, 64, 64, 333, cg.PATH_UNFUSED_ONSITE | cg.PATH_SMEM_CORE, 0),
+    ("proj_fast+onsite_reg", 6, 64, 64, 333, cg.PATH_UNFUSED_ONSITE, 0),
+    ("onsite_reg_lb4", 4, 32, 32, 1001, cg.PATH_UNFUSED_ONSITE, 0),
+    ("onsite_reg_lb2", 2, 8, 24, 517, cg.PATH_UNFUSED_ONSITE, 0),
     ("onsite_fast_rowblocks", 12, 8, 8, 75, cg.PATH_UNFUSED_ONSITE, 0),
     ("generic", 5, 12, 20, 99, cg.PATH_UNFUSED_ONSITE | cg.PATH_GENERIC_CORE | cg.PATH_GENERIC_PROJ, 0),
     ("proj_tc_3xtf32", 4, 24, 40, 170, cg.PATH_UNFUSED_ONSITE, cg.MATH_3XTF32),
