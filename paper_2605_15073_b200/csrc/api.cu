@@ -621,8 +621,10 @@ int cgtp_message_status(const void* workspace, void* cuda_stream)
 static size_t nbody_ws_bytes(int nu, int lmax, int lmax_out, int C, int64_t batch)
 {
     const size_t L2p = round_up((lmax + 1) * (lmax + 1), 4), Lo2p = round_up((lmax_out + 1) * (lmax_out + 1), 4);
-    // H rows have the odd stride L2 | 1 <= L2p + 1; every factor block is padded to whole groups of 4 columns
-    return (((size_t)batch * C + 4) * (size_t)nu * (L2p + 1) + 4 * (L2p + 1) + (size_t)batch * C * Lo2p) * sizeof(float) + 4 * 256;
+    // H rows have the odd stride L2 | 1 <= L2p + 1; every factor block is padded to whole groups of 4 columns (nu = 2
+    // runs on the bilinear core: groups of 32 columns, T rows of stride Lo2 | 1)
+    return (((size_t)batch * C + 32) * (size_t)nu * (L2p + 1) + 4 * (L2p + 1) + ((size_t)batch * C + 32) * (Lo2p + 1)) * sizeof(float) +
+           4 * 256;
 }
 
 size_t cgtp_onsite_nbody_workspace_bytes(int nu, int lmax, int lmax_out, int N, int C, int64_t batch)
@@ -644,7 +646,7 @@ int cgtp_onsite_nbody(const float* X, const float* W_in, const float* W_out, int
     if (N <= 0 || C <= 0) { set_error("N and C must be positive (N=%d, C=%d)", N, C); return CGTP_ERR_INVALID; }
     const int LB = kernel_band(lmax > lmax_out ? lmax : lmax_out);
     if (!nbody_supported(LB, nu)) {
-        set_error("nu-body product: max(lmax,lmax_out)=%d / nu=%d exceed the compiled limits (band limit 8, nu 4)",
+        set_error("nu-body product: max(lmax,lmax_out)=%d / nu=%d exceed the compiled limits (band limit 20, nu 4)",
                   lmax > lmax_out ? lmax : lmax_out, nu);
         return CGTP_ERR_UNSUPPORTED;
     }
@@ -666,9 +668,14 @@ int cgtp_onsite_nbody(const float* X, const float* W_in, const float* W_out, int
     const int64_t ncols = batch * C;
     Carver cv(workspace);
     const int hstr = nbody_hstride(p);
-    const int64_t hfs = nbody_hfstride(p, ncols);
+    // nu = 2 is the pointwise product of the bilinear step (Eq.(38) PAPER.md:332 with every channel even): the bilinear
+    // core runs it (H blocks padded to groups of 32 columns, T rows of its odd stride)
+    const Plan* p2 = (nu == 2 && !(kernel_path() & PATH_GENERIC_CORE)) ? get_plan(lmax, lmax_out) : nullptr;
+    const bool bilinear = p2 && onsite_fast_supported(p2, false) && onsite_fast_hstride(p2) == hstr;
+    const int64_t hfs = bilinear ? (int64_t)round_up64(ncols, 32) * hstr : nbody_hfstride(p, ncols);
+    const int tstr = bilinear ? onsite_fast_tstride(p2) : p->Lo2p;
     float* H = cv.take<float>((size_t)nu * hfs + 4 * hstr);
-    float* T = cv.take<float>((size_t)ncols * p->Lo2p);
+    float* T = cv.take<float>((size_t)(bilinear ? round_up64(ncols, 32) : ncols) * tstr);
 
     // S1 per factor: H[s] = W_in[s] . X[s] (Eq.(35)), one launch over the nu problems
     std::vector<ProjArgs> pv(nu);
@@ -698,15 +705,15 @@ int cgtp_onsite_nbody(const float* X, const float* W_in, const float* W_out, int
     int rc = launch_proj_degrees(pv, 2, K_PROJ_IN, st);
     if (rc) return rc;
     // S2-S4 with nu factors
-    rc = launch_nbody(p, H, T, ncols, st);
+    rc = bilinear ? launch_onsite_fast(p2, false, H, H + hfs, T, round_up64(ncols, 32), st) : launch_nbody(p, H, T, ncols, st);
     if (rc) return rc;
     // S5: out[b] = W_out . T[b] (Eq.(41) :346)
     std::vector<ProjArgs> po(1);
     {
         ProjArgs& a = po[0];
         a.X = T;
-        a.x_bs = (int64_t)C * p->Lo2p;
-        a.x_rs = p->Lo2p;
+        a.x_bs = (int64_t)C * tstr;
+        a.x_rs = tstr;
         a.W = W_out;
         a.ldw_m = C;
         a.ldw_k = 1;

@@ -47,6 +47,24 @@ def test_nbody_vs_oracle(nu, lmax, lmax_out, N, C, batch):
     assert np.array_equal(got, again)  # bitwise reproducible
 
 
+@pytest.mark.parametrize("lmax,lmax_out,N,C,batch", [(3, 5, 8, 8, 40), (6, 6, 16, 16, 67), (2, 4, 8, 4, 33), (16, 16, 4, 8, 13)])
+def test_nbody_nu2_both_cores_vs_oracle(lmax, lmax_out, N, C, batch):
+    """nu = 2 runs on the bilinear core (the pointwise product of Eq.(38) with every channel even); under
+    CGTP_PATH_GENERIC_CORE the nu-body kernel takes it.  Both against the oracle."""
+    inp = synthetic.make_nbody(2, lmax, lmax_out, N, C, batch, seed=77 + lmax)
+    ref = orc.onsite_nbody(inp.X, inp.W_in, inp.W_out, lmax, lmax_out)
+    outs = []
+    try:
+        for flags in (0, cg.PATH_GENERIC_CORE):
+            cg.cgtp_set_kernel_path(flags)
+            got = run_nbody(inp)
+            assert rel_err(got, ref) <= TOL, (flags, rel_err(got, ref))
+            outs.append(got)
+    finally:
+        cg.cgtp_set_kernel_path(0)
+    assert not np.array_equal(outs[0], outs[1])  # two different kernels did run
+
+
 def test_nbody_nu2_matches_bilinear_entry_point():
     lmax, lmax_out, N, C, batch = 4, 4, 16, 16, 100
     o = synthetic.make_onsite(lmax, lmax_out, N, C, batch, seed=5, parity_mask=np.zeros(C, np.uint8))
