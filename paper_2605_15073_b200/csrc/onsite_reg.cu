@@ -19,27 +19,12 @@
 #include <cstring>
 #include <mutex>
 
-#include "onsite_core.cuh"
+#include "onsite_reg.cuh"
 
 namespace cgtp {
 
-namespace {
-
-struct RegPlan {
-    int dev, lmax, lmax_out;
-    bool odd;
-    int NT4, U, NQ, bytes;
-    const void* blob;  // device: even: P[U][NT4], WP[U][NT4]; odd: DP[U][NT4], MP[U][NT4], WP[U][NT4]
-    std::vector<float> QF, QI;
-};
-std::mutex g_mu;
-std::vector<RegPlan*> g_plans;
-
-const RegPlan* get_reg_plan(const Plan* p, bool odd)
+int reg_host_tables(const Plan* p, bool odd, std::vector<float>& tab)
 {
-    std::lock_guard<std::mutex> lk(g_mu);
-    for (RegPlan* c : g_plans)
-        if (c->dev == p->dev && c->lmax == p->lmax && c->lmax_out == p->lmax_out && c->odd == odd) return c;
     const int LB = p->LB, U = p->U, LL = LB + 1;
     const int NT = (LB + 1) * (LB + 2) / 2, NT4 = round_up(NT, 4);
     std::vector<double> x, w, P;
@@ -47,7 +32,7 @@ const RegPlan* get_reg_plan(const Plan* p, bool odd)
     legendre_values(U, LB, x, P);
     auto at = [&](int u, int l, int m) -> double { return P[((size_t)u * LL + l) * LL + m]; };
     const int ntab = odd ? 3 : 2;
-    std::vector<float> tab((size_t)ntab * U * NT4, 0.f);
+    tab.assign((size_t)ntab * U * NT4, 0.f);
     for (int u = 0; u < U; ++u) {
         const double ct = x[u], st = std::sqrt(1.0 - ct * ct);
         for (int l = 0; l <= LB; ++l)
@@ -68,6 +53,29 @@ const RegPlan* get_reg_plan(const Plan* p, bool odd)
                 if (l <= p->lmax_out) tab[(size_t)(ntab - 1) * U * NT4 + k] = (float)(w[u] * pv);
             }
     }
+    return NT4;
+}
+
+namespace {
+
+struct RegPlan {
+    int dev, lmax, lmax_out;
+    bool odd;
+    int NT4, U, NQ, bytes;
+    const void* blob;  // device: even: P[U][NT4], WP[U][NT4]; odd: DP[U][NT4], MP[U][NT4], WP[U][NT4]
+    std::vector<float> QF, QI;
+};
+std::mutex g_mu;
+std::vector<RegPlan*> g_plans;
+
+const RegPlan* get_reg_plan(const Plan* p, bool odd)
+{
+    std::lock_guard<std::mutex> lk(g_mu);
+    for (RegPlan* c : g_plans)
+        if (c->dev == p->dev && c->lmax == p->lmax && c->lmax_out == p->lmax_out && c->odd == odd) return c;
+    std::vector<float> tab;
+    const int NT4 = reg_host_tables(p, odd, tab);
+    const int U = p->U;
     CoreTab t;
     std::memset(&t, 0, sizeof t);
     std::vector<float> TA, WP, QF, QI;
@@ -111,14 +119,14 @@ struct RegArgs {
 
 constexpr int kRegWarps = 4;
 
-template <int LB, bool ODD, bool HREG>
+template <int LB, bool ODD, bool HREG, int NBUF>
+// (register caps for more resident warps at band limits 5 / 6 -- __launch_bounds__(128, 3 or 4): 170 / 128 registers, 200-390
+// bytes spilled -- measured slower: lmax 6 odd 111 -> 152 / 119 us, lmax 5 odd 72 -> 78 / 99 us on configs[3])
 __global__ void __launch_bounds__(32 * kRegWarps) onsite_reg_kernel(const RegArgs a, const __grid_constant__ CoreQParam<LB> qp)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int NT = (LB + 1) * (LB + 2) / 2, NT4 = round_up(NT, 4), L2B = (LB + 1) * (LB + 1);
-    constexpr int MR = 2 * LB + 1, NP = ODD ? 2 : 1;
-    constexpr int NTC = (LB + 2) / 2, NTS = (LB + 1) / 2;
-    constexpr int NBUF = HREG ? 1 : 2;
+    static_assert(!HREG || NBUF == 1, "register-resident H refills its one buffer");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (a.status && *a.status != 0) return;
 
@@ -158,7 +166,7 @@ __global__ void __launch_bounds__(32 * kRegWarps) onsite_reg_kernel(const RegArg
     uint32_t phases = 0u;
     for (; g < a.ngroups; g += stride) {
         const long long gn = g + stride;
-        if (!HREG && lane == 0 && gn < a.ngroups) load_h(gn, buf ^ 1);
+        if (NBUF == 2 && lane == 0 && gn < a.ngroups) load_h(gn, buf ^ 1);
         mbar_wait(&bar[buf], (phases >> buf) & 1u);
         phases ^= 1u << buf;
         const float* ha = hbuf + (size_t)buf * 2 * hfl + lane * a.L2s;
@@ -174,82 +182,12 @@ __global__ void __launch_bounds__(32 * kRegWarps) onsite_reg_kernel(const RegArg
 #pragma unroll
         for (int k = 0; k < L2B; ++k) T[k] = 0.f;
 
-#pragma unroll 1
-        for (int u = 0; u < a.U; ++u) {
-            // ---- stage A: coefficient rows of grid row u.  Pairs are the two factors (A, B); table values are scalars.
-            float2 f[NP][MR];
-#pragma unroll
-            for (int k = 0; k < NP; ++k)
-#pragma unroll
-                for (int r = 0; r < MR; ++r) f[k][r] = make_float2(0.f, 0.f);
-            {
-                float t0[NT4], t1[ODD ? NT4 : 1];
-#pragma unroll
-                for (int j = 0; j < NT4; j += 4) {
-                    const float4 v = *reinterpret_cast<const float4*>(tab0 + u * NT4 + j);
-                    t0[j] = v.x; t0[j + 1] = v.y; t0[j + 2] = v.z; t0[j + 3] = v.w;
-                    if (ODD) {
-                        const float4 q = *reinterpret_cast<const float4*>(tab1 + u * NT4 + j);
-                        t1[j] = q.x; t1[j + 1] = q.y; t1[j + 2] = q.z; t1[j + 3] = q.w;
-                    }
-                }
-#pragma unroll
-                for (int l = 0; l <= LB; ++l) {
-#pragma unroll
-                    for (int m = 0; m <= l; ++m) {
-                        const int t = tri_index(l, m), ip = l * l + l + m, im = l * l + l - m;
-                        float2 xp, xm;
-                        if (HREG) {
-                            xp = hh[ip];
-                            xm = hh[im];
-                        } else {
-                            const bool in = ip < a.L2;  // l <= lmax
-                            xp = in ? make_float2(ha[ip], hb[ip]) : make_float2(0.f, 0.f);
-                            xm = (in && m > 0) ? make_float2(ha[im], hb[im]) : xp;
-                        }
-                        const float2 p2 = make_float2(t0[t], t0[t]);
-                        f[0][m] = ffma2(xp, p2, f[0][m]);
-                        if (m > 0) f[0][LB + m] = ffma2(xm, p2, f[0][LB + m]);
-                        if (ODD && m > 0) {
-                            // the phi derivative swaps the cosine and sine rows: cos row m takes
-                            // +m (sine coefficient), sin row m takes -m (cosine coefficient)
-                            f[NP - 1][m] = ffma2(xm, make_float2(t1[t], t1[t]), f[NP - 1][m]);
-                            f[NP - 1][LB + m] = ffma2(xp, make_float2(-t1[t], -t1[t]), f[NP - 1][LB + m]);
-                        }
-                    }
-                }
-            }
-            // ---- stage B
-            float2 tc[NTC], ts[NTS > 0 ? NTS : 1];
-#pragma unroll
-            for (int k = 0; k < NTC; ++k) tc[k] = make_float2(0.f, 0.f);
-#pragma unroll
-            for (int k = 0; k < NTS; ++k) ts[k] = make_float2(0.f, 0.f);
-            stage_b_regs<LB, ODD, true>(qp, f, a.NQ, tc, ts);
-            // ---- stage C: this row's term of the quadrature
-            {
-                float wv[NT4];
-#pragma unroll
-                for (int j = 0; j < NT4; j += 4) {
-                    const float4 v = *reinterpret_cast<const float4*>(tabw + u * NT4 + j);
-                    wv[j] = v.x; wv[j + 1] = v.y; wv[j + 2] = v.z; wv[j + 3] = v.w;
-                }
-#pragma unroll
-                for (int l = 0; l <= LB; ++l) {
-#pragma unroll
-                    for (int m = 0; m <= l; ++m) {
-                        const int t = tri_index(l, m);
-                        const float gc = (m & 1) ? tc[m / 2].y : tc[m / 2].x;
-                        T[l * l + l + m] = fmaf(wv[t], gc, T[l * l + l + m]);
-                        if (m > 0) {
-                            const float gs = ((m - 1) & 1) ? ts[(m - 1) / 2].y : ts[(m - 1) / 2].x;
-                            T[l * l + l - m] = fmaf(wv[t], gs, T[l * l + l - m]);
-                        }
-                    }
-                }
-            }
-        }
+        reg_column_rows<LB, ODD, HREG>(qp, tab0, tab1, tabw, a.U, a.NQ, a.L2, ha, hb, hh, T);
 
+        if (!HREG && NBUF == 1) {  // the rows of H are dead: refill the one buffer while T is stored
+            __syncwarp();
+            if (lane == 0 && gn < a.ngroups) load_h(gn, 0);
+        }
         // ---- T leaves through the warp's staging rows
         if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         __syncwarp();
@@ -262,18 +200,17 @@ __global__ void __launch_bounds__(32 * kRegWarps) onsite_reg_kernel(const RegArg
             tma_store_1d(a.T + g * 32 * a.Lo2s, Ts, (uint32_t)(32 * a.Lo2s * 4));
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
-        if (!HREG) buf ^= 1;
+        if (NBUF == 2) buf ^= 1;
     }
     if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
-
-constexpr size_t kSmemPerSm = 227 * 1024;
 
 template <int LB, bool ODD>
 int launch_reg_t(const Plan* p, const RegPlan* c, const float* Ha, const float* Hb, float* T, int64_t ncols, cudaStream_t st,
                  const int64_t* send, int cpar, const int32_t* status)
 {
     constexpr bool HREG = LB <= 4;
+    constexpr int NBUF = 1;
     RegArgs a;
     a.tab = reinterpret_cast<const float*>(c->blob);
     a.tab_floats = c->bytes / 4;
@@ -291,11 +228,11 @@ int launch_reg_t(const Plan* p, const RegPlan* c, const float* Ha, const float* 
     a.cpar = cpar;
     a.status = status;
     const int hbytes = 2 * 32 * a.L2s * 4;
-    a.off_ts = 16 + (HREG ? 1 : 2) * hbytes;
+    a.off_ts = 16 + NBUF * hbytes;
     a.warp_bytes = round_up(a.off_ts + 32 * a.Lo2s * 4, 128);
     a.off_warp = round_up(c->bytes, 128);
     const size_t smem = (size_t)a.off_warp + (size_t)kRegWarps * a.warp_bytes;
-    auto kern = onsite_reg_kernel<LB, ODD, HREG>;
+    auto kern = onsite_reg_kernel<LB, ODD, HREG, NBUF>;
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int ctas_per_sm = 0;
     CGTP_CUDA_CHECK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, 32 * kRegWarps, smem));
@@ -317,7 +254,8 @@ int launch_reg_t(const Plan* p, const RegPlan* c, const float* Ha, const float* 
 
 // Measured on configs[3] (N = C = 32, 16384 atoms; core even / odd in us, this kernel against onsite_fast_kernel):
 // lmax 1: 10.5 / 10.7 vs 15.8 / 19.0; 2: 14.8 / 18.9 vs 24.0 / 31.0; 3: 21.0 / 29.1 vs 35.3 / 51.4; 4: 37.3 / 51.7 vs
-// 49.7 / 84.4; 5: 55.7 / 72.1 vs 61.9 / 99.0; 6: 100.8 / 133.2 vs 93.0 / 170.4 (216 / 255 registers: 8 warps per SM).
+// 49.7 / 84.4; 5: 55.7 / 72.1 vs 61.9 / 99.0; 6: 100.8 / 110.9 vs 93.0 / 170.4 (223 / 254 registers: 8 warps per SM);
+// configs[1] (N = C = 64, 4096 atoms, lmax 6): odd 68.0 vs 88.3.
 bool onsite_reg_supported(const Plan* p, bool odd) { return p->LB <= 5 || (p->LB == 6 && odd); }
 
 int launch_onsite_reg(const Plan* p, bool odd, const float* Ha, const float* Hb, float* T, int64_t ncols, cudaStream_t st,
