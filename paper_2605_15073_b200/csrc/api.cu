@@ -672,10 +672,13 @@ int cgtp_onsite_nbody(const float* X, const float* W_in, const float* W_out, int
     // core runs it (H blocks padded to groups of 32 columns, T rows of its odd stride)
     const Plan* p2 = (nu == 2 && !(kernel_path() & PATH_GENERIC_CORE)) ? get_plan(lmax, lmax_out) : nullptr;
     const bool bilinear = p2 && onsite_fast_supported(p2, false) && onsite_fast_hstride(p2) == hstr;
-    const int64_t hfs = bilinear ? (int64_t)round_up64(ncols, 32) * hstr : nbody_hfstride(p, ncols);
-    const int tstr = bilinear ? onsite_fast_tstride(p2) : p->Lo2p;
+    // nu >= 3 at small band limits: one thread per column (nbody_reg.cu), same padded layout
+    const bool regcore = !bilinear && !(kernel_path() & PATH_SMEM_CORE) && nbody_reg_supported(p);
+    const bool pad32 = bilinear || regcore;
+    const int64_t hfs = pad32 ? (int64_t)round_up64(ncols, 32) * hstr : nbody_hfstride(p, ncols);
+    const int tstr = pad32 ? (p->Lo2 | 1) : p->Lo2p;
     float* H = cv.take<float>((size_t)nu * hfs + 4 * hstr);
-    float* T = cv.take<float>((size_t)(bilinear ? round_up64(ncols, 32) : ncols) * tstr);
+    float* T = cv.take<float>((size_t)(pad32 ? round_up64(ncols, 32) : ncols) * tstr);
 
     // S1 per factor: H[s] = W_in[s] . X[s] (Eq.(35)), one launch over the nu problems
     std::vector<ProjArgs> pv(nu);
@@ -705,7 +708,9 @@ int cgtp_onsite_nbody(const float* X, const float* W_in, const float* W_out, int
     int rc = launch_proj_degrees(pv, 2, K_PROJ_IN, st);
     if (rc) return rc;
     // S2-S4 with nu factors
-    rc = bilinear ? launch_onsite_fast(p2, false, H, H + hfs, T, round_up64(ncols, 32), st) : launch_nbody(p, H, T, ncols, st);
+    rc = bilinear  ? launch_onsite_fast(p2, false, H, H + hfs, T, round_up64(ncols, 32), st)
+         : regcore ? launch_nbody_reg(p, H, hfs, T, ncols, st)
+                   : launch_nbody(p, H, T, ncols, st);
     if (rc) return rc;
     // S5: out[b] = W_out . T[b] (Eq.(41) :346)
     std::vector<ProjArgs> po(1);

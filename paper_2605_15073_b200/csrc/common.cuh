@@ -245,6 +245,10 @@ bool nbody_supported(int LB, int nu);
 int nbody_hstride(const Plan* p);
 int64_t nbody_hfstride(const Plan* p, int64_t ncols);
 int launch_nbody(const Plan* p, const float* H, float* T, int64_t ncols, cudaStream_t st);
+// Register-resident form for small band limits (nbody_reg.cu): one thread per column.  H: [nu][hfs] with rows of stride
+// L2 | 1 and every factor block padded to whole groups of 32 columns; T rows of stride Lo2 | 1, padded likewise.
+bool nbody_reg_supported(const Plan* p);
+int launch_nbody_reg(const Plan* p, const float* H, int64_t hfs, float* T, int64_t ncols, cudaStream_t st);
 
 // M0: row_ptr over `nodes` receivers; senders are validated against n_send
 int launch_segments(const int64_t* edge_index, int64_t E, int64_t nodes, int64_t n_send, int64_t* row_ptr,

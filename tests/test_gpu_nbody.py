@@ -47,6 +47,29 @@ def test_nbody_vs_oracle(nu, lmax, lmax_out, N, C, batch):
     assert np.array_equal(got, again)  # bitwise reproducible
 
 
+@pytest.mark.parametrize("nu,lmax,lmax_out,N,C,batch", [
+    (3, 2, 2, 8, 8, 64), (4, 2, 2, 8, 8, 50), (3, 4, 4, 16, 12, 133), (4, 3, 3, 12, 10, 91), (3, 1, 3, 2, 2, 3),
+    (3, 3, 0, 8, 8, 33), (4, 1, 4, 8, 8, 70), (3, 3, 3, 32, 32, 257), (4, 4, 2, 8, 16, 45), (3, 6, 6, 16, 16, 67),
+    (4, 5, 5, 8, 8, 21), (3, 2, 6, 6, 5, 37),
+])
+def test_nbody_register_and_shared_memory_cores(nu, lmax, lmax_out, N, C, batch):
+    """nu >= 3 at band limits <= 6 runs with one thread per column on registers (nbody_reg.cu); CGTP_PATH_SMEM_CORE keeps
+    the CTA-tiled kernel of nbody.cu.  Both against the oracle."""
+    inp = synthetic.make_nbody(nu, lmax, lmax_out, N, C, batch, seed=500 + 100 * nu + 10 * lmax + lmax_out)
+    ref = orc.onsite_nbody(inp.X, inp.W_in, inp.W_out, lmax, lmax_out)
+    outs = []
+    try:
+        for flags in (0, cg.PATH_SMEM_CORE):
+            cg.cgtp_set_kernel_path(flags)
+            got = run_nbody(inp)
+            assert rel_err(got, ref) <= TOL, (flags, rel_err(got, ref))
+            assert np.array_equal(got, run_nbody(inp))
+            outs.append(got)
+    finally:
+        cg.cgtp_set_kernel_path(0)
+    assert not np.array_equal(outs[0], outs[1])  # two different kernels did run
+
+
 @pytest.mark.parametrize("lmax,lmax_out,N,C,batch", [(3, 5, 8, 8, 40), (6, 6, 16, 16, 67), (2, 4, 8, 4, 33), (16, 16, 4, 8, 13)])
 def test_nbody_nu2_both_cores_vs_oracle(lmax, lmax_out, N, C, batch):
     """nu = 2 runs on the bilinear core (the pointwise product of Eq.(38) with every channel even); under
