@@ -621,6 +621,23 @@ def run_message(args, cg, synthetic, dev, peaks, peak_src):
                          "peak_source": peak_src, "traffic": ncu_traffic.get(f"config{idx}:{dom}") if halfhalf else None},
             "kernels": kern,
         }
+        if idx == 4:
+            # M1 / M6 on the tensor cores (tcgen05, 3xTF32: three TF32 products per FP32 product), reported beside the
+            # FP32-exact step, never inside it (north_star: "TF32/3xTF32 reported separately")
+            ref_out = out.clone()
+            cg.cgtp_set_math_mode(cg.MATH_3XTF32)
+            try:
+                ms_tc = time_steps(fn, steps, 3)
+                fn()
+                torch.cuda.synchronize()
+                diff = [float((out[:, s_] - ref_out[:, s_]).abs().max() / ref_out[:, s_].abs().max()) for s_ in (0, 1)]
+            finally:
+                cg.cgtp_set_math_mode(cg.MATH_FP32)
+            res[name]["projections_3xtf32"] = {
+                "ms_per_step": ms_tc, "edges_per_s": m.E / (ms_tc * 1e-3),
+                "frac_hbm_peak_whole_step": total_bytes / (ms_tc * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                "max_rel_diff_vs_fp32_path": diff}
+            del ref_out
         if idx == 2:
             # the node-grid table the edges gather from (95 MB) is written by M2 in the same step and stays in the 126 MB
             # L2 (SURVEY.md 8(d) says so): the gather is an L2 read, the algorithmic rate is not an HBM measurement

@@ -182,6 +182,9 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
         if (eff > best + 1e-9) { best = eff; bestNW = NW; }
     }
     t.NW = bestNW;
+    // where one CTA per SM is all that fits (band limit 16 odd: row blocks of eight) every grid row of a block gets its own
+    // half-warp: more resident warps count for more than the balance of the per-m lists
+    if (LB >= 16 && core_ub(LB, odd) >= 8) t.NW = std::min(kMaxWarps, 2 * core_ub(LB, odd) / NH);
     if (core_split(LB, odd)) t.NW = 2 * (2 * core_ub(LB, odd)) / NH;  // every (grid row, half of the azimuth rows) has its own half-warp: one pass
     std::vector<std::vector<int>> asg[3];
     int maxi = 1;

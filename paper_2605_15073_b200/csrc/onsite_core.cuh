@@ -35,14 +35,15 @@ __host__ __device__ constexpr int core_uhmax(int LB) { return ((3 * LB + 2) / 2 
 // four-node row blocks); 20 odd (four-node row blocks): 11.2 -> 6.0 ms; configs[1] odd 106 -> 97 us, even 56 -> 63 us
 // (kept at 32); lmax 2 and 4 are slower with 16.
 __host__ __device__ constexpr int core_gw(int LB, bool odd) { return (LB >= 8 || (LB == 6 && odd)) ? 16 : 32; }
-// Northern nodes per row block of the fast kernel: all of them (one block) for band limits <= 8; four for the
-// larger ones (eight for the odd channels at 16), and at band limit 20 two warps share a grid row in stage B
-// (core_split, see stage_b).  At 16 / 20 one group's H, T and F planes leave room for ONE CTA per SM, and with four-node
-// blocks that CTA had 4 warps (ncu: one warp per scheduler, issue slots 23-30 % used).  Measured on configs[3], core even /
-// odd in ms -- lmax 16: blocks of 4: 1.62 / 3.75 (even: 2 CTAs x 4 warps), split: 2.32 / 3.12, blocks of 8: 3.23 / 2.81;
-// lmax 20: blocks of 4: 4.67 / 6.18, split: 3.37 / 5.13, blocks of 8: 3.63 / does not fit.
-__host__ __device__ constexpr int core_ub(int LB, bool odd) { return LB <= 8 ? core_uhmax(LB) : (LB == 16 && odd) ? 8 : 4; }
-__host__ __device__ constexpr bool core_split(int LB, bool odd) { return LB >= 20; }
+// Northern nodes per row block of the fast kernel: all of them (one block) for band limits <= 8; four for the larger
+// ones, except eight for the odd channels at 16 and the even channels at 20; the odd channels at 20 give every grid row
+// of stage B to two warps (core_split, see stage_b).  At 16 / 20 one group's H, T and F planes leave room for ONE CTA per
+// SM, and with four-node blocks that CTA had 4 warps (ncu: one warp per scheduler, issue slots 23-30 % used); blocks of
+// eight run with 8 warps (one half-warp per grid row of the block).  Measured on configs[3], core even / odd in ms --
+// lmax 16: blocks of 4: 1.62 / 3.75 (even: 2 CTAs x 4 warps), split: 2.32 / 3.12, blocks of 8 on 8 warps: 1.99 / 2.15;
+// lmax 20: blocks of 4: 4.67 / 6.18, split: 3.37 / 5.13, blocks of 8 on 8 warps: 2.26 / does not fit.
+__host__ __device__ constexpr int core_ub(int LB, bool odd) { return LB <= 8 ? core_uhmax(LB) : ((LB == 16 && odd) || (LB == 20 && !odd)) ? 8 : 4; }
+__host__ __device__ constexpr bool core_split(int LB, bool odd) { return LB >= 20 && odd; }
 
 
 // Host (onsite_core.cu): longest-processing-time assignment of (cost, id) items to NW workers.
