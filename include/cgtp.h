@@ -85,6 +85,28 @@ int cgtp_onsite(const float* A, const float* B, const float* W_a, const float* W
                 int64_t batch, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * cgtp_onsite for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc).  Same operation, arguments, layouts and sectors as cgtp_onsite (Eq.(35)-(41)
+ * PAPER.md:322-346, odd channels Eq.(11)-(12) :107-:111), but NO workspace argument and NO allocation of any kind: the
+ * projected coefficients H and the rank-space results T live in a file-scope device array of
+ * CGTP_STATIC_SCRATCH_BYTES (16 MiB; every GPU that loads the library's module holds it until the process exits), the
+ * tables travel as kernel parameters, and the call makes no cudaMalloc / cudaFree / allocating library call and touches
+ * no plan cache of the library (first call included).
+ *
+ * Limits: max(lmax, lmax_out) <= 4 and C <= 256 (any N, any batch: persistent CTAs walk the batch); beyond them
+ * CGTP_ERR_UNSUPPORTED with a message naming the limit -- use cgtp_onsite with a workspace there.  Other errors as
+ * cgtp_onsite.  One plain FP32 kernel (no TMA, no tensor cores, math mode ignored): made for small shapes, not for speed.
+ *
+ * ALL CALLS SHARE THE ONE ARRAY.  It keeps the last call's contents; no call reads a word it has not written itself, so
+ * nothing needs clearing.  Calls that overlap on the GPU (different streams, concurrently replayed graphs) RACE on it;
+ * calls on one stream are ordered and safe.  Asynchronous on cuda_stream.  Not counted by cgtp_launch_count / profiling.
+ * ------------------------------------------------------------------------------------------- */
+#define CGTP_STATIC_SCRATCH_BYTES (16u << 20)
+int cgtp_onsite_static(const float* A, const float* B, const float* W_a, const float* W_b, const float* W_out,
+                       int lmax, int lmax_out, int N, int C, const uint8_t* parity_mask, float* out,
+                       int64_t batch, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Two feature fields (Eq.(28) :236, Sec. VI E :232-:240, Sec. VII C f :471):
  * "the deeper message-passing variant in which the edge-side message ... no longer factors as R.Y", written with
  * an edge field I^(E)[e, n1, l1 m1] and a node field I^(N)[j, n2, l2 m2].  At fixed CP rank (Eq.(3) :39; "an

@@ -46,6 +46,8 @@ def lib() -> ctypes.CDLL:
     L.cgtp_onsite_workspace_bytes.argtypes = [i, i, i, i, i64]
     L.cgtp_onsite.restype = i
     L.cgtp_onsite.argtypes = [vp, vp, vp, vp, vp, i, i, i, i, vp, vp, i64, vp, sz, vp]
+    L.cgtp_onsite_static.restype = i
+    L.cgtp_onsite_static.argtypes = [vp, vp, vp, vp, vp, i, i, i, i, vp, vp, i64, vp]
     L.cgtp_message_workspace_bytes.restype = sz
     L.cgtp_message_workspace_bytes.argtypes = [i, i, i, i, vp, i64, i64]
     L.cgtp_message.restype = i
@@ -208,6 +210,33 @@ def cgtp_onsite(A, B, W_a, W_b, W_out, lmax, lmax_out, N, C, parity_mask, out=No
         rc = lib().cgtp_onsite(A.data_ptr(), B.data_ptr(), W_a.data_ptr(), W_b.data_ptr(), W_out.data_ptr(),
                                lmax, lmax_out, N, C, mask.ctypes.data, out.data_ptr(), batch,
                                ws.data_ptr(), ws.numel(), _stream_ptr(stream))
+    _check(rc)
+    return out
+
+
+STATIC_SCRATCH_BYTES = 16 << 20
+
+
+def cgtp_onsite_static(A, B, W_a, W_b, W_out, lmax, lmax_out, N, C, parity_mask, out, stream=None):
+    """cgtp_onsite without any device allocation (include/cgtp.h): scratch in a 16 MiB file-scope device array, limits
+    max(lmax, lmax_out) <= 4 and C <= 256.  `out` [batch, 2, N, (lmax_out+1)^2] is the caller's (this wrapper allocates
+    nothing either).  All calls share the array: calls that overlap on the GPU race."""
+    f32 = torch.float32
+    A, B = _dev(A, f32, "A"), _dev(B, f32, "B")
+    W_a, W_b, W_out = _dev(W_a, f32, "W_a"), _dev(W_b, f32, "W_b"), _dev(W_out, f32, "W_out")
+    batch = A.shape[0]
+    L2, Lo2 = (lmax + 1) ** 2, (lmax_out + 1) ** 2
+    if tuple(A.shape) != (batch, N, L2) or tuple(B.shape) != (batch, N, L2):
+        raise ValueError("A, B must be [batch, N, (lmax+1)^2]")
+    if tuple(W_a.shape) != (C, N) or tuple(W_b.shape) != (C, N) or tuple(W_out.shape) != (N, C):
+        raise ValueError("W_a, W_b must be [C, N] and W_out [N, C]")
+    mask = _mask(parity_mask, C)
+    if out is None:
+        raise ValueError("cgtp_onsite_static allocates nothing: pass `out`")
+    out = _out(out, (batch, 2, N, Lo2), A.device)
+    with torch.cuda.device(A.device):
+        rc = lib().cgtp_onsite_static(A.data_ptr(), B.data_ptr(), W_a.data_ptr(), W_b.data_ptr(), W_out.data_ptr(),
+                                      lmax, lmax_out, N, C, mask.ctypes.data, out.data_ptr(), batch, _stream_ptr(stream))
     _check(rc)
     return out
 
