@@ -387,7 +387,10 @@ def main():
         line["l_dependent_weights"] = run_lw(args, cg, synthetic, dev, ms_per_step)
         line["nbody"] = run_nbody(args, cg, synthetic, dev, fp32_peak_tflops)
         line["edge_field"] = run_edge_field(args, cg, synthetic, dev, fp32_peak_tflops)
-        line["unfused_onsite"] = run_unfused(args, cg, step, fl, batch, fp32_peak_tflops, fp32_peak_measured)
+        # the other on-site path beside the library's own choice (four launches at configs[1] since the projections address
+        # with compile-time strides): the single fused kernel, forced
+        line["fused_onsite"] = run_other_path(args, cg, step, fl, batch, fp32_peak_tflops, fp32_peak_measured,
+                                              cg.PATH_FUSED_ONSITE)
         line["clocks_extras"] = sampler2.stop()
     elif world == 1:
         rate, dt_cpu, cores, passes = oracle_onsite_rate(base, 1024, min_wall_s=1.0)
@@ -465,12 +468,13 @@ def run_message_sharded(args, cg, synthetic, dev, rank, world, peaks, barrier, m
             "timing": "CUDA events on the launch stream around all-gather + kernels, mean over steps, max over ranks"}
 
 
-def run_unfused(args, cg, step, fl, batch, fp32_peak_tflops, fp32_peak_measured):
-    """configs[1] through the four-launch step (proj_fast + onsite_core x 2 + proj_fast), forced with
-    CGTP_PATH_UNFUSED_ONSITE: what the single-kernel step is measured against."""
+def run_other_path(args, cg, step, fl, batch, fp32_peak_tflops, fp32_peak_measured, path):
+    """configs[1] through the on-site path the library did NOT choose, forced with a CGTP_PATH_* flag
+    (CGTP_PATH_FUSED_ONSITE: S1-S5 in one kernel, onsite_fused.cu; CGTP_PATH_UNFUSED_ONSITE: proj_fast + core x 2 +
+    proj_fast): what the headline step is measured against."""
     import torch
     try:
-        cg.cgtp_set_kernel_path(cg.PATH_UNFUSED_ONSITE)
+        cg.cgtp_set_kernel_path(path)
         it = [0]
 
         def fn():
@@ -493,7 +497,7 @@ def run_unfused(args, cg, step, fl, batch, fp32_peak_tflops, fp32_peak_measured)
             kern[k]["alg_tflops"] = fl[k] * batch / (a * 1e-3) / 1e12
             kern[k]["frac_fp32_peak"] = kern[k]["alg_tflops"] / fp32_peak_tflops
             kern[k]["frac_of_measured"] = kern[k]["alg_tflops"] / fp32_peak_measured
-    return {"ms_per_step": ms, "contractions_per_s": batch / (ms * 1e-3), "kernels": kern}
+    return {"kernel_path": int(path), "ms_per_step": ms, "contractions_per_s": batch / (ms * 1e-3), "kernels": kern}
 
 
 def run_tensor_core(args, cg, step, out, lmax, lmax_out, N, C, Ce, Co, batch, peaks, peak_src):

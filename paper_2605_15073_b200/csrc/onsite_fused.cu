@@ -437,15 +437,16 @@ int launch_onsite_fused(const Plan* p, int N, int C, int Ce, int Co, const float
     const int LB = p->LB;
     if (LB > 8 || p->lmax_out > p->lmax || N % kTM != 0 || C % kTM != 0 || Ce % 4 != 0 || Co % 4 != 0 || batch <= 0)
         return CGTP_OK;
-    // Taken where it was measured faster than the four launches (B200): wide projections at band limits >= 6
-    // (configs[1]: 255 vs 259 us), narrow ones (N C <= 256) at band limits >= 4 (N = C = 16, 20000 atoms, lmax 4 / 5 / 6:
-    // 160 / 206 / 298 vs 195 / 269 / 389 us) and problems so small that launch latency dominates (configs[0]: 23 vs 38 us).
-    // Elsewhere the four launches win since the small band limits have the register core of onsite_reg.cu (N = C = 64,
-    // 4096 atoms, lmax 1-5: 51 / 63 / 92 / 130 / 178 vs 97 / 106 / 143 / 224 / 243 us; N = C = 32, configs[3], lmax 2 / 4:
-    // 79 / 183 vs 116 / 261 us); CGTP_PATH_FUSED_ONSITE forces the kernel there (tests, bench).
-    const bool wide = (int64_t)N * C >= 4096 && LB >= 6, narrow = (int64_t)N * C <= 256 && LB >= 4;
-    const bool tiny = batch * (int64_t)C * p->L2 <= (1 << 17);
-    if (!wide && !narrow && !tiny && !(kernel_path() & PATH_FUSED_ONSITE)) return CGTP_OK;
+    // Taken where it was measured faster than the four launches (B200, DESIGN.md 5.11 / 5.14): narrow projections
+    // (N C <= 256) at band limits >= 4 (N = C = 16, 20000 atoms, lmax 4 / 5 / 6: 160 / 206 / 298 vs 195 / 269 / 389 us) and
+    // problems so small that launch latency dominates (configs[0]: 23 vs 38 us).  Elsewhere the four launches win: the
+    // small band limits have the register core of onsite_reg.cu and the projections of proj_fast.cu address with
+    // compile-time strides (configs[1]: 243 us in four launches, 257 us here; N = C = 32, configs[3], lmax 2 / 4: 78 / 175 vs
+    // 116 / 261 us).  CGTP_PATH_FUSED_ONSITE forces the kernel for every shape it supports (tests, bench).
+    // (N = C = 8, 30000 atoms, lmax 2: 83 vs 123 us; N = C = 64, lmax 6, 256 atoms: 32 vs 48 us, 1024 atoms: 85 vs 83 us)
+    const bool narrow = (int64_t)N * C <= 64 || ((int64_t)N * C <= 256 && LB >= 4);
+    const bool tiny = batch * (int64_t)C * p->L2 <= (1 << 17) || batch <= 512;
+    if (!narrow && !tiny && !(kernel_path() & PATH_FUSED_ONSITE)) return CGTP_OK;
     // warps of the two sub-groups by estimated work: a curl group costs about 1.9 pointwise groups (configs[1]: 3 + 5 warps 260 us, 4 + 4 warps 304 us -- ten grid rows on ten half-warp workers is one round of stage B)
     int we = 8, wo = 0;
     if (Ce == 0) { we = 0; wo = 8; }

@@ -69,12 +69,23 @@ __device__ __forceinline__ float4 lds128(uint32_t addr)
     return v;
 }
 
+// store at a compile-time byte offset from a per-thread pointer: STG [R.64 + imm], no address arithmetic per store
+template <int OFF>
+__device__ __forceinline__ void stg_off(float* p, float v)
+{
+    asm volatile("st.global.f32 [%0+%1], %2;" ::"l"(p), "n"(OFF), "f"(v) : "memory");
+}
+
 __device__ __forceinline__ void mbar_arrive_cta(uint64_t* bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
-template <int RW, int CWP, bool ACC, bool WIN>
+// RS > 0: the row strides of X and of the output are both the compile-time constant RS (floats) -- the x loads of the
+// inner loop and the stores of the epilogue then address with immediate offsets (no per-load IMAD, no per-store address
+// arithmetic: 31 of 363 instructions per 8 k-steps and ~80 of 100 per 16 stores with run-time strides, ncu source
+// counters at configs[1]).  RS = 0: run-time strides.
+template <int RW, int CWP, bool ACC, bool WIN, int RS = 0>
 __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
 {
     constexpr int MW = 16 * RW;       // rows per CTA
@@ -94,7 +105,7 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
     const int pi = (a.nprob > 1 && (int)blockIdx.x >= a.p[1].cta_begin) ? 1 : 0;
     const float* const X = pi ? a.p[1].X : a.p[0].X;
     const int64_t x_bs = pi ? a.p[1].x_bs : a.p[0].x_bs;
-    const int x_rs = a.p[0].x_rs;  // common to both problems (host-checked)
+    const int x_rs = RS ? RS : a.p[0].x_rs;  // common to both problems (host-checked)
     const int M = pi ? a.p[1].M : a.p[0].M;
     const int K = pi ? a.p[1].K : a.p[0].K;
     const int cpr = pi ? a.p[1].ctas_per_rb : a.p[0].ctas_per_rb;
@@ -182,7 +193,7 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
 
     // ---- output addressing: row m of this warp's slab goes to out0 (m < m_split) or out1
     const int mrow0 = m0 + wr * 16;
-    const int o_rs = a.p[pi].o_rs, m_split = a.p[pi].m_split;
+    const int o_rs = RS ? RS : a.p[pi].o_rs, m_split = a.p[pi].m_split;
     const bool slab_uniform = (mrow0 + 16 <= m_split) || (mrow0 >= m_split);
     const int slab_dst = (mrow0 >= m_split) ? 1 : 0;
     const int nrow_live = (M - mrow0 < 16) ? (M - mrow0) : 16;  // may be <= 0
@@ -229,6 +240,10 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
             // stays on the uniform datapath, so the FMA pipe sees no address arithmetic
             const uint32_t ub = stage0 + (uint32_t)s * stage_bytes;
             const uint32_t wb = w0 + (uint32_t)(kc * KC) * (MW * 4);
+            // RS: the four column addresses of this chunk; row kk is then an immediate offset kk * RS * 4
+            uint32_t xb[4];
+#pragma unroll
+            for (int t = 0; t < 4; ++t) xb[t] = (uint32_t)xoff[t] + ub;
 #pragma unroll 8
             for (int kk = 0; kk < KC; ++kk) {
                 const uint32_t wa = wb + (uint32_t)kk * (MW * 4);
@@ -237,7 +252,7 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
                 float2 x[4];
 #pragma unroll
                 for (int t = 0; t < 4; ++t) {
-                    const float v = lds32(xoff[t] + rowb);
+                    const float v = RS ? lds32(xb[t] + (uint32_t)kk * (uint32_t)(RS * 4)) : lds32(xoff[t] + rowb);
                     x[t] = make_float2(v, v);
                 }
 #pragma unroll
@@ -261,7 +276,19 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
                 if (cc >= ncol) continue;
                 const int al = (J == 1) ? cc : (int)__umulhi((uint32_t)cc, jmagic), j = cc - al * J;
                 const int64_t b = (int64_t)b0 + al;
-                if (slab_uniform) {
+                if (slab_uniform && !ACC && nrow_live == 16) {
+                    // the common case: a full slab of 16 rows, no predicates (with RS the row offsets are immediates)
+                    float* dst = ob + b * obs + j;
+                    if constexpr (RS > 0) {
+#define CGTP_ST(r) stg_off<(r) * RS * 4>(dst, ((r) & 1) ? acc[(r) >> 1][t].y : acc[(r) >> 1][t].x);
+                        CGTP_ST(0) CGTP_ST(1) CGTP_ST(2) CGTP_ST(3) CGTP_ST(4) CGTP_ST(5) CGTP_ST(6) CGTP_ST(7)
+                        CGTP_ST(8) CGTP_ST(9) CGTP_ST(10) CGTP_ST(11) CGTP_ST(12) CGTP_ST(13) CGTP_ST(14) CGTP_ST(15)
+#undef CGTP_ST
+                    } else {
+#pragma unroll
+                        for (int r = 0; r < 16; ++r) dst[(int64_t)r * o_rs] = (r & 1) ? acc[r >> 1][t].y : acc[r >> 1][t].x;
+                    }
+                } else if (slab_uniform) {
                     float* dst = ob + b * obs + j;
                     float prev[16];
                     if (ACC) {
@@ -454,6 +481,22 @@ int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st
     else
         kern = wide ? (acc ? proj_fast_kernel<2, 4, true, false> : proj_fast_kernel<2, 4, false, false>)
                     : (acc ? proj_fast_kernel<4, 2, true, false> : proj_fast_kernel<4, 2, false, false>);
+    // compile-time row stride when X and every output share it ((lmax+1)^2 is odd for even lmax, so the odd strides of H
+    // and T equal the dense ones: S1, S5 and M1 at the band limits of BASELINE.json's configs)
+    bool same_rs = !acc;
+    for (int i = 0; i < nargs; ++i) same_rs = same_rs && args[i].o_rs == x_rs;
+    if (same_rs && !(kernel_path() & PATH_GENERIC_PROJ)) {
+        switch (x_rs) {
+#define CGTP_RS(V)                                                                                             \
+    case V:                                                                                                    \
+        kern = window ? (wide ? proj_fast_kernel<2, 4, false, true, V> : proj_fast_kernel<4, 2, false, true, V>)  \
+                      : (wide ? proj_fast_kernel<2, 4, false, false, V> : proj_fast_kernel<4, 2, false, false, V>); \
+        break;
+            CGTP_RS(9) CGTP_RS(25) CGTP_RS(49) CGTP_RS(81) CGTP_RS(169) CGTP_RS(289) CGTP_RS(441)
+#undef CGTP_RS
+            default: break;
+        }
+    }
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<grid, kPfThreads, smem, st>>>(a);
     CGTP_CUDA_CHECK(cudaGetLastError());
