@@ -26,6 +26,7 @@ struct CorePlan {
     int dev;  // CUDA device ordinal of `blob`
     int lmax, lmax_out;
     bool odd;
+    bool wide;  // 8-warp CTAs where the on-site kernel wants them (band limit 8, odd channels)
     CoreTab tab;
     const void* blob;  // device
     std::vector<float> QF, QI;  // host copies of the azimuthal tables (kernel parameter CoreQParam)
@@ -147,11 +148,14 @@ void core_host_tables(const Plan* p, bool odd, CoreTab& t, std::vector<float>& T
     t.NQ = NQ;
 }
 
-static const CorePlan* get_core_plan(const Plan* p, bool odd)
+// wide: the plan of launch_onsite_fast (see the warp count below); the two-field core and the single-kernel step keep the
+// heuristic's CTA size (8 warps cost the pooled core of the two-field step 69.0 -> 76.7 ms on the configs[4] graph)
+static const CorePlan* get_core_plan(const Plan* p, bool odd, bool wide = false)
 {
+    wide = wide && p->LB == 8 && odd;
     std::lock_guard<std::mutex> lk(g_core_mu);
     for (CorePlan* c : g_core_plans)
-        if (c->dev == p->dev && c->lmax == p->lmax && c->lmax_out == p->lmax_out && c->odd == odd) return c;
+        if (c->dev == p->dev && c->lmax == p->lmax && c->lmax_out == p->lmax_out && c->odd == odd && c->wide == wide) return c;
 
     const int LB = p->LB;
     CoreTab t;
@@ -185,6 +189,11 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
     // where one CTA per SM is all that fits (band limit 16 odd: row blocks of eight) every grid row of a block gets its own
     // half-warp: more resident warps count for more than the balance of the per-m lists
     if (LB >= 16 && core_ub(LB, odd) >= 8) t.NW = std::min(kMaxWarps, 2 * core_ub(LB, odd) / NH);
+    // band limit 8, odd channels: 14 grid rows per group = 16 half-warp workers in one round of stage B; the heuristic keeps
+    // 4 warps (two rounds, the same efficiency on paper), which leaves 8 warps per SM (two 93 KB CTAs) and 42 % of the issue
+    // slots used.  Measured (configs[3] lmax 8, odd core): 4 / 6 / 8 warps 374 / 362 / 343 us; 8 warps lose at band limit 12
+    // (row blocks of four: half the workers idle in stage B, 1.10 -> 1.61 ms) and for the even channels (193 -> 263 us)
+    if (wide) t.NW = kMaxWarps;
     if (core_split(LB, odd)) t.NW = 2 * (2 * core_ub(LB, odd)) / NH;  // every (grid row, half of the azimuth rows) has its own half-warp: one pass
     std::vector<std::vector<int>> asg[3];
     int maxi = 1;
@@ -228,6 +237,7 @@ static const CorePlan* get_core_plan(const Plan* p, bool odd)
     c->lmax = p->lmax;
     c->lmax_out = p->lmax_out;
     c->odd = odd;
+    c->wide = wide;
     c->tab = t;
     c->blob = d;
     c->QF = QF;
@@ -472,7 +482,7 @@ int launch_onsite_fast(const Plan* p, bool odd, const float* Ha, const float* Hb
     if (ncols <= 0) return CGTP_OK;
     if (onsite_reg_supported(p, odd) && !(kernel_path() & PATH_SMEM_CORE))
         return launch_onsite_reg(p, odd, Ha, Hb, T, ncols, st, nullptr, 0, nullptr);
-    const CorePlan* c = get_core_plan(p, odd);
+    const CorePlan* c = get_core_plan(p, odd, true);
     if (!c) return CGTP_ERR_CUDA;
     switch (p->LB) {
 #define CGTP_CASE(B)                                                              \
