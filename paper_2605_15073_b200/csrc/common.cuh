@@ -160,6 +160,36 @@ struct LaunchScope {
     } while (0)
 
 // ---------------------------------------------------------------------------------------------
+// Programmatic dependent launch (the kernels of the four-launch on-site step): a kernel launched with launch_pdl may be
+// scheduled while its predecessor in the stream is still running, once every CTA of the predecessor has executed
+// pdl_launch_dependents() (or exited).  It may then run the part of its prologue that touches nothing the predecessor
+// writes (tables, weights -> shared memory) and MUST execute pdl_wait() before its first access to such data: the wait
+// returns when the predecessor grid has completed and its writes are visible.  Launched without the attribute both
+// instructions are no-ops.  Only persistent kernels whose whole grid is resident use this (no CTA of the predecessor can be
+// kept off an SM by a waiting successor).
+// ---------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t st, Args&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+#endif
+
+// ---------------------------------------------------------------------------------------------
 // Stage launchers (one per row of SURVEY.md 8(a)); all asynchronous on `st`.
 // ---------------------------------------------------------------------------------------------
 

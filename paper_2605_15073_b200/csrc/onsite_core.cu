@@ -303,7 +303,11 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a,
         }
         tma_load_span(dst + hfl, hb, hbytes, &bar_h[buf]);
     };
-    if (a.status && *a.status != 0) return;
+    pdl_launch_dependents();
+    if (a.status) {  // written by an earlier kernel of the stream: nothing may be read before the predecessor is done
+        pdl_wait();
+        if (*a.status != 0) return;
+    }
 
     if (threadIdx.x == 0) {
         mbar_init(bar_tab, 1);
@@ -315,7 +319,8 @@ __global__ void __launch_bounds__(32 * kMaxWarps) onsite_fast_kernel(CoreArgs a,
     long long g = blockIdx.x;
     if (threadIdx.x == 0) {
         mbar_arrive_expect_tx(bar_tab, (uint32_t)a.tab.bytes);
-        tma_load_span(smem + a.off_blob, a.blob, (uint32_t)a.tab.bytes, bar_tab);
+        tma_load_span(smem + a.off_blob, a.blob, (uint32_t)a.tab.bytes, bar_tab);  // the plan's tables: independent
+        pdl_wait();  // H is the predecessor's output (this thread issues every load of it; T is written after H arrived)
         if (g < a.ngroups) load_h(g, 0);
     }
     mbar_wait(bar_tab, 0);
@@ -471,7 +476,7 @@ static int launch_fast_t(const Plan* p, const CorePlan* c, const float* Ha, cons
     std::memcpy(qp.qf, c->QF.data(), std::min(sizeof qp.qf, c->QF.size() * sizeof(float)));
     std::memcpy(qp.qi, c->QI.data(), std::min(sizeof qp.qi, c->QI.size() * sizeof(float)));
     LaunchScope scope(ODD ? K_ONSITE_ODD : K_ONSITE_EVEN, st);
-    kern<<<(unsigned)grid, 32 * c->tab.NW, smem, st>>>(a, qp);
+    CGTP_CUDA_CHECK(launch_pdl(kern, (unsigned)grid, 32u * c->tab.NW, smem, st, a, qp));
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
 }

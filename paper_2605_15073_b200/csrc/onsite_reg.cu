@@ -128,10 +128,14 @@ __global__ void __launch_bounds__(32 * kRegWarps) onsite_reg_kernel(const RegArg
     constexpr int NT = (LB + 1) * (LB + 2) / 2, NT4 = round_up(NT, 4), L2B = (LB + 1) * (LB + 1);
     static_assert(!HREG || NBUF == 1, "register-resident H refills its one buffer");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (a.status && *a.status != 0) return;
+    pdl_launch_dependents();
+    if (a.status) {  // written by an earlier kernel of the stream: nothing may be read before the predecessor is done
+        pdl_wait();
+        if (*a.status != 0) return;
+    }
 
     float* tabs = reinterpret_cast<float*>(smem);
-    for (int i = threadIdx.x; i < a.tab_floats; i += blockDim.x) tabs[i] = a.tab[i];
+    for (int i = threadIdx.x; i < a.tab_floats; i += blockDim.x) tabs[i] = a.tab[i];  // the plan's tables: independent
     unsigned char* wr = smem + a.off_warp + (size_t)warp * a.warp_bytes;
     uint64_t* bar = reinterpret_cast<uint64_t*>(wr);  // [NBUF]
     float* hbuf = reinterpret_cast<float*>(wr + 16);
@@ -158,6 +162,7 @@ __global__ void __launch_bounds__(32 * kRegWarps) onsite_reg_kernel(const RegArg
 
     const long long stride = (long long)gridDim.x * kRegWarps;
     long long g = (long long)blockIdx.x * kRegWarps + warp;
+    pdl_wait();  // H is the predecessor's output
     if (lane == 0 && g < a.ngroups) load_h(g, 0);
     const float* tab0 = tabs;                                   // even: P; odd: d_theta P
     const float* tab1 = tabs + (size_t)a.U * NT4;               // odd: m P / sin(theta)
@@ -245,7 +250,7 @@ int launch_reg_t(const Plan* p, const RegPlan* c, const float* Ha, const float* 
     std::memcpy(qp.qf, c->QF.data(), std::min(sizeof qp.qf, c->QF.size() * sizeof(float)));
     std::memcpy(qp.qi, c->QI.data(), std::min(sizeof qp.qi, c->QI.size() * sizeof(float)));
     LaunchScope scope(ODD ? K_ONSITE_ODD : K_ONSITE_EVEN, st);
-    kern<<<(unsigned)grid, 32 * kRegWarps, smem, st>>>(a, qp);
+    CGTP_CUDA_CHECK(launch_pdl(kern, (unsigned)grid, 32u * kRegWarps, smem, st, a, qp));
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
 }

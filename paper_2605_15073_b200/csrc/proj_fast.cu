@@ -169,6 +169,12 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_fast_kernel(PfArgs a)
         if (++p_kc == NCH) { p_kc = 0; p_ti += cpr; }
         if (++p_s == NSTAGE) p_s = 0;
     };
+    // Programmatic dependent launch (common.cuh): this kernel may be scheduled while its predecessor in the stream still
+    // runs.  Everything it reads from global memory is a caller input or the predecessor's output (X, and the weights too:
+    // the caller's previous kernel may have just written them), so it waits here; what overlaps is the launch itself and
+    // the barrier set-up above.
+    pdl_launch_dependents();
+    pdl_wait();
     for (int i = 0; i < NSTAGE - 1; ++i) produce();
 
     // ---- weights: Wd[k][r] = W[idx_m[m0+r]][idx_k[k]].  Thread = fixed row r,
@@ -498,7 +504,7 @@ int launch_proj_fast(const ProjArgs* args, int nargs, Kind kind, cudaStream_t st
         }
     }
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<grid, kPfThreads, smem, st>>>(a);
+    CGTP_CUDA_CHECK(launch_pdl(kern, (unsigned)grid, (unsigned)kPfThreads, smem, st, a));
     CGTP_CUDA_CHECK(cudaGetLastError());
     *handled = true;
     return CGTP_OK;
