@@ -160,13 +160,14 @@ struct LaunchScope {
     } while (0)
 
 // ---------------------------------------------------------------------------------------------
-// Programmatic dependent launch (the kernels of the four-launch on-site step): a kernel launched with launch_pdl may be
+// Programmatic dependent launch (the kernels of the four-launch on-site step and of message passing M1-M6): a kernel
+// launched with launch_pdl may be
 // scheduled while its predecessor in the stream is still running, once every CTA of the predecessor has executed
 // pdl_launch_dependents() (or exited).  It may then run the part of its prologue that touches nothing the predecessor
 // writes (tables, weights -> shared memory) and MUST execute pdl_wait() before its first access to such data: the wait
 // returns when the predecessor grid has completed and its writes are visible.  Launched without the attribute both
-// instructions are no-ops.  Only persistent kernels whose whole grid is resident use this (no CTA of the predecessor can be
-// kept off an SM by a waiting successor).
+// instructions are no-ops.  A successor is scheduled only after EVERY CTA of its predecessor has started (and signalled), so
+// a waiting successor cannot keep a predecessor's CTA off an SM, whether or not the predecessor's grid is resident at once.
 // ---------------------------------------------------------------------------------------------
 #ifdef __CUDACC__
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }

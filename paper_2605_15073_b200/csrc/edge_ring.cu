@@ -81,6 +81,8 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
     const int UVp = a.p.UVp, QP = UVp / 4;
     const int NST = a.NST, cs = a.cs, cb = a.cb, nblk = a.nblk, Cpar = a.Cpar;
 
+    pdl_launch_dependents();  // programmatic dependent launch, common.cuh: barriers, recurrence coefficients and the plan's
+                              // grid geometry below are independent of every earlier kernel
     if (tid == 0) {
         for (int s = 0; s < NST; ++s) {
             mbar_init(&full[s], 1);
@@ -96,6 +98,7 @@ __global__ void __launch_bounds__(ER_NT, 1) edge_ring_kernel(EdgeRingArgs a)
         for (int idx = tid; idx < a.geo_bytes / 4; idx += ER_NT) geo_s[idx] = a.p.geo[idx];
     __syncthreads();
 
+    pdl_wait();  // status / row_ptr (M0), G (M2) and the caller's edge arrays; S may still be read by an earlier kernel
     const bool graph_ok = (*a.status == 0);
     const long long nitems = a.nodes * nblk;
     int slot = 0;
@@ -325,7 +328,7 @@ static int launch_ring_t(const EdgeRingArgs& a, size_t smem, int grid, cudaStrea
 {
     auto kern = edge_ring_kernel<ODD, NSBT, NA>;
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<grid, ER_NT, smem, st>>>(a);
+    CGTP_CUDA_CHECK(launch_pdl(kern, (unsigned)grid, (unsigned)ER_NT, smem, st, a));
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
 }

@@ -118,12 +118,14 @@ __global__ void __launch_bounds__(256) node_synth_kernel(Plan p, SynthSmem lay, 
         mbar_fence_init();
     }
     __syncthreads();
+    pdl_launch_dependents();  // programmatic dependent launch, common.cuh
     if (threadIdx.x == 0) {
         const uint32_t total = lay.tab_bytes + 2 * lay.q_bytes + hbytes;
         mbar_arrive_expect_tx(bar, total);
-        tma_load_span(tab0, p.PT, lay.tab_bytes, bar);
+        tma_load_span(tab0, p.PT, lay.tab_bytes, bar);  // the plan's tables: independent of the predecessor
         tma_load_span(qc, p.QC, lay.q_bytes, bar);
         tma_load_span(qs, p.QS, lay.q_bytes, bar);
+        pdl_wait();  // H is the predecessor's output; G is written only after it has arrived
         tma_load_span(hs, H + col0 * p.L2p, hbytes, bar);
     }
 #pragma unroll
@@ -184,7 +186,7 @@ static int launch_node_synth_t(const Plan* p, Kind kind, const float* H, float* 
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, lay.total));
     int64_t grid = (ncols + NC - 1) / NC;
     LaunchScope scope(kind, st);
-    kern<<<(unsigned)grid, 256, lay.total, st>>>(*p, lay, H, G, (long long)ncols, NC);
+    CGTP_CUDA_CHECK(launch_pdl(kern, (unsigned)grid, 256u, (size_t)lay.total, st, *p, lay, H, G, (long long)ncols, NC));
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
 }
@@ -429,15 +431,17 @@ __global__ void __launch_bounds__(256) analysis_kernel(Plan p, AnaSmem lay, cons
         mbar_fence_init();
     }
     __syncthreads();
+    pdl_launch_dependents();  // programmatic dependent launch, common.cuh
     if (threadIdx.x == 0) {
         const uint32_t total = NF * lay.tab_bytes + sbytes;
         mbar_arrive_expect_tx(bar, total);
         if (!ODD) {
-            tma_load_span(wp, p.WP, lay.tab_bytes, bar);
+            tma_load_span(wp, p.WP, lay.tab_bytes, bar);  // the plan's tables: independent of the predecessor
         } else {
             tma_load_span(wp, p.WD, lay.tab_bytes, bar);
             tma_load_span(wp + lay.tab_bytes / 4, p.WS, lay.tab_bytes, bar);
         }
+        pdl_wait();  // S is the predecessor's output; T is written only after it has arrived
         tma_load_span(Ss, S + col0 * NF * p.UVp, sbytes, bar);
     }
     mbar_wait(bar, 0);
@@ -479,7 +483,7 @@ static int launch_analysis_t(const Plan* p, const float* S, float* T, int64_t nc
     LaunchScope scope(ODD ? K_ANALYSIS_ODD : K_ANALYSIS_EVEN, st);
     QParam<LB> qp;
     fill_qparam<LB>(p, qp);
-    kern<<<(unsigned)grid, 256, lay.total, st>>>(*p, lay, qp, S, T, (long long)ncols, NC);
+    CGTP_CUDA_CHECK(launch_pdl(kern, (unsigned)grid, 256u, (size_t)lay.total, st, *p, lay, qp, S, T, (long long)ncols, NC));
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
 }

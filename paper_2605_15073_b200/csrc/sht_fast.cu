@@ -71,6 +71,7 @@ __global__ void __launch_bounds__(SF_THREADS) synth_fast_kernel(Plan p, SfLayout
     const int HS = lay.HS, GS = lay.GS;
     constexpr int ntri = (LB + 1) * (LB + 2) / 2;
 
+    pdl_launch_dependents();  // programmatic dependent launch, common.cuh: the table set-up below touches only the plan
     for (int i = tid; i < ntri * UP; i += SF_THREADS) {
         const int t = i / UP, u = i - t * UP;
         PTt[i] = (u < Uh) ? p.PT[u * p.NTRI + t] : 0.f;
@@ -78,6 +79,7 @@ __global__ void __launch_bounds__(SF_THREADS) synth_fast_kernel(Plan p, SfLayout
     // coefficient rows above lmax (kernel band limit LB > lmax) stay zero for the whole kernel
     for (int i = tid; i < M * U * 32; i += SF_THREADS) F[i] = 0.f;
 
+    pdl_wait();  // H is the predecessor's output, G may still be read by an earlier kernel of the stream
     const long long ngroups = (ncols + 31) / 32;
     for (long long g = blockIdx.x; g < ngroups; g += gridDim.x) {
         __syncthreads();
@@ -212,7 +214,7 @@ static int launch_synth_fast_t(const Plan* p, Kind kind, const float* H, int hst
     LaunchScope scope(kind, st);
     QParam<LB> qp;
     fill_qparam<LB>(p, qp);
-    kern<<<grid, SF_THREADS, smem, st>>>(*p, lay, qp, H, G, (long long)ncols);
+    CGTP_CUDA_CHECK(launch_pdl(kern, (unsigned)grid, (unsigned)SF_THREADS, smem, st, *p, lay, qp, H, G, (long long)ncols));
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
 }
