@@ -84,8 +84,9 @@ __global__ void __launch_bounds__(32 * kNbRegWarps) nbody_reg_kernel(const NbReg
     constexpr int NP = NU / 2, NR = NU % 2;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
+    pdl_launch_dependents();  // programmatic dependent launch, common.cuh
     float* tabs = reinterpret_cast<float*>(smem);
-    for (int i = threadIdx.x; i < a.tab_floats; i += blockDim.x) tabs[i] = a.tab[i];
+    for (int i = threadIdx.x; i < a.tab_floats; i += blockDim.x) tabs[i] = a.tab[i];  // the plan's tables: independent
     unsigned char* wr = smem + a.off_warp + (size_t)warp * a.warp_bytes;
     uint64_t* bar = reinterpret_cast<uint64_t*>(wr);
     float* hbuf = reinterpret_cast<float*>(wr + 16);
@@ -104,6 +105,7 @@ __global__ void __launch_bounds__(32 * kNbRegWarps) nbody_reg_kernel(const NbReg
     };
     const long long stride = (long long)gridDim.x * kNbRegWarps;
     long long g = (long long)blockIdx.x * kNbRegWarps + warp;
+    pdl_wait();  // H is the predecessor's output
     if (lane == 0 && g < a.ngroups) load_h(g);
     const float* tabp = tabs;
     const float* tabw = tabs + a.off_w;
@@ -254,7 +256,7 @@ int launch_t(const Plan* p, const NbRegPlan* c, const float* H, int64_t hfs, flo
     const int64_t need = (a.ngroups + kNbRegWarps - 1) / kNbRegWarps;
     if (grid > need) grid = need;
     LaunchScope scope(K_ONSITE_EVEN, st);
-    kern<<<(unsigned)grid, 32 * kNbRegWarps, smem, st>>>(a);
+    CGTP_CUDA_CHECK(launch_pdl(kern, (unsigned)grid, 32u * kNbRegWarps, smem, st, a));
     CGTP_CUDA_CHECK(cudaGetLastError());
     return CGTP_OK;
 }

@@ -152,6 +152,9 @@ __global__ void __launch_bounds__(kPfThreads, 1) proj_multi_kernel(const __grid_
         if (++p_kc == NCH) { p_kc = 0; p_ti += cpr; }
         if (++p_s == NSTAGE) p_s = 0;
     };
+    // programmatic dependent launch (common.cuh): everything read below is a caller input or a predecessor's output
+    pdl_launch_dependents();
+    pdl_wait();
     for (int i = 0; i < NSTAGE - 1; ++i) produce();
 
     // ---- weights: Wd[k][r] = W[idx_m[m0+r]][idx_k[k]].  Thread = fixed row r,
@@ -395,7 +398,7 @@ int launch_proj_multi(const ProjArgs* args, int nargs, Kind kind, cudaStream_t s
     LaunchScope scope(kind, st);
     void (*kern)(const PmArgs) = wide ? proj_multi_kernel<2, 4> : proj_multi_kernel<4, 2>;
     CGTP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<grid, kPfThreads, smem, st>>>(a);
+    CGTP_CUDA_CHECK(launch_pdl(kern, (unsigned)grid, (unsigned)kPfThreads, smem, st, a));
     CGTP_CUDA_CHECK(cudaGetLastError());
     *handled = true;
     return CGTP_OK;
