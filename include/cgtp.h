@@ -395,6 +395,8 @@ int cgtp_message_field_parity(const float* node_feats, const int64_t* edge_index
  *                            the neighbour sum on the grid inside the core (field_pool_core_kernel, onsite_core.cu)
  *   CGTP_PATH_SMEM_CORE      S2-S4 at band limits <= 6: the warp-scheduled shared-memory core (onsite_core.cu) instead of
  *                            the one-thread-per-column register core (onsite_reg.cu)
+ *   CGTP_PATH_PLAIN_LAUNCH   every kernel launched in plain stream order instead of chained by programmatic dependent launch
+ *                            (the kernels are the same; only their overlap at the boundaries goes away)
  * Process-wide, read at every call; 0 (default) = every specialised kernel.  CGTP_ERR_INVALID for unknown bits.
  * ------------------------------------------------------------------------------------------- */
 #define CGTP_PATH_GENERIC_CORE 1
@@ -405,6 +407,7 @@ int cgtp_message_field_parity(const float* node_feats, const int64_t* edge_index
 #define CGTP_PATH_FUSED_ONSITE 32
 #define CGTP_PATH_FIELD_PER_EDGE 64
 #define CGTP_PATH_SMEM_CORE 128
+#define CGTP_PATH_PLAIN_LAUNCH 256
 int cgtp_set_kernel_path(int flags);
 int cgtp_get_kernel_path(void);
 

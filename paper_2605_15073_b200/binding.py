@@ -626,6 +626,7 @@ PATH_GENERIC_CORE, PATH_GENERIC_EDGE, PATH_GENERIC_PROJ, PATH_GENERIC_SYNTH, PAT
 PATH_FUSED_ONSITE = 32
 PATH_FIELD_PER_EDGE = 64
 PATH_SMEM_CORE = 128
+PATH_PLAIN_LAUNCH = 256
 
 
 def cgtp_set_kernel_path(flags: int) -> None:

@@ -112,6 +112,8 @@ struct OnsitePass {
 static int onsite_pass(const Plan* p, int N, const OnsitePass& q, int64_t batch, void* workspace, cudaStream_t st)
 {
     const int Ce = q.Ce, Co = q.Co;
+    // long steps (H of one factor beyond kPdlMaxBytes: configs[3] from lmax 12 up) launch their kernels in plain order
+    PdlScope pdl((size_t)batch * (size_t)(Ce + Co) * p->L2 * sizeof(float) > kPdlMaxBytes);
     // the whole step in one kernel (onsite_fused.cu) when the shape fits and nothing but the plain contraction is asked
     if (!(kernel_path() & (PATH_UNFUSED_ONSITE | PATH_GENERIC_CORE | PATH_GENERIC_PROJ)) && get_math_mode() == CGTP_MATH_FP32 &&
         !q.lw_in && !q.lw_out && q.sigma_C == 0 && !q.accumulate && q.x_bs == (int64_t)N * p->L2 &&
@@ -275,6 +277,8 @@ static int message_pass(const Plan* p, int N, const MessagePass& q, const int64_
                         int64_t n_send, int64_t nodes, int64_t E, void* workspace, cudaStream_t st)
 {
     const int Ce = q.Ce, Co = q.Co;
+    // long steps (node grids beyond kPdlMaxBytes: configs[4]) launch their kernels in plain order
+    PdlScope pdl((size_t)n_send * (size_t)(Ce + Co) * p->UVp * sizeof(float) > kPdlMaxBytes);
     Carver cv(workspace);
     int32_t* status = cv.take<int32_t>(1);
     int64_t* row_ptr = cv.take<int64_t>((size_t)nodes + 1);
@@ -666,6 +670,7 @@ int cgtp_onsite_nbody(const float* X, const float* W_in, const float* W_out, int
     const Plan* p = get_plan_nu(lmax, lmax_out, nu);
     if (!p) return CGTP_ERR_CUDA;
     const int64_t ncols = batch * C;
+    PdlScope pdl((size_t)ncols * p->L2 * sizeof(float) > kPdlMaxBytes);  // long steps: plain launch order (common.cuh)
     Carver cv(workspace);
     const int hstr = nbody_hstride(p);
     // nu = 2 is the pointwise product of the bilinear step (Eq.(38) PAPER.md:332 with every channel even): the bilinear
@@ -802,6 +807,7 @@ static int field_pass(const Plan* p, int N, int Ne, const FieldPass& q, const in
     const int Cpar[2] = {q.Ce, q.Co};
     const bool lw = q.lw;
     int rc = CGTP_OK;
+    PdlScope pdl((size_t)E * (size_t)C * p->L2 * sizeof(float) > kPdlMaxBytes);  // long steps: plain launch order (common.cuh)
     const bool fast = !(kernel_path() & PATH_GENERIC_CORE) && (Cpar[0] == 0 || onsite_fast_supported(p, false)) &&
                       (Cpar[1] == 0 || onsite_fast_supported(p, true));
     const int hstr = fast ? onsite_fast_hstride(p) : p->L2p;
@@ -1460,7 +1466,7 @@ int cgtp_get_math_mode(void) { return cgtp::get_math_mode(); }
 int cgtp_set_kernel_path(int flags)
 {
     clear_error();
-    if (flags < 0 || flags > 255) { set_error("unknown kernel-path flags %d", flags); return CGTP_ERR_INVALID; }
+    if (flags < 0 || flags > 511) { set_error("unknown kernel-path flags %d", flags); return CGTP_ERR_INVALID; }
     cgtp::set_kernel_path(flags);
     return CGTP_OK;
 }

@@ -34,7 +34,7 @@ inline int current_device()
 int num_sms();
 
 // Test-only kernel-path switch (cgtp_set_kernel_path): bit set = take the generic kernel where a specialised one exists.
-enum : int { PATH_GENERIC_CORE = 1, PATH_GENERIC_EDGE = 2, PATH_GENERIC_PROJ = 4, PATH_GENERIC_SYNTH = 8, PATH_UNFUSED_ONSITE = 16, PATH_FUSED_ONSITE = 32, PATH_FIELD_PER_EDGE = 64, PATH_SMEM_CORE = 128 };
+enum : int { PATH_GENERIC_CORE = 1, PATH_GENERIC_EDGE = 2, PATH_GENERIC_PROJ = 4, PATH_GENERIC_SYNTH = 8, PATH_UNFUSED_ONSITE = 16, PATH_FUSED_ONSITE = 32, PATH_FIELD_PER_EDGE = 64, PATH_SMEM_CORE = 128, PATH_PLAIN_LAUNCH = 256 };
 int kernel_path();
 void set_kernel_path(int flags);
 
@@ -169,6 +169,20 @@ struct LaunchScope {
 // instructions are no-ops.  A successor is scheduled only after EVERY CTA of its predecessor has started (and signalled), so
 // a waiting successor cannot keep a predecessor's CTA off an SM, whether or not the predecessor's grid is resident at once.
 // ---------------------------------------------------------------------------------------------
+// Per calling thread: true = launch_pdl launches in plain stream order.  Set for the duration of a call by the entry points
+// whose steps are long (PdlScope): chaining pays where the kernel boundaries are a visible share of the step (configs[1]
+// 0.240 -> 0.224 ms, configs[2] 0.521 -> 0.495 ms) and does not where the kernels run for milliseconds (configs[4]: 21.3 ms
+// chained against 21.0 ms plain, medians of six alternating runs on a power-capped box).
+bool pdl_plain();
+void set_pdl_plain(bool plain);
+struct PdlScope {
+    explicit PdlScope(bool plain) : prev(pdl_plain()) { set_pdl_plain(plain); }
+    ~PdlScope() { set_pdl_plain(prev); }
+    bool prev;
+};
+// intermediate data of a step (bytes) above which its kernels are launched in plain order
+constexpr size_t kPdlMaxBytes = (size_t)256 << 20;
+
 #ifdef __CUDACC__
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
@@ -185,7 +199,7 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned bl
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = ((kernel_path() & PATH_PLAIN_LAUNCH) || pdl_plain()) ? 0 : 1;  // test switch / long steps: plain order
     return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
 }
 #endif

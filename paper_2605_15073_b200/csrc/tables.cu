@@ -42,6 +42,10 @@ int num_sms()
     return g_sms[dev];
 }
 
+static thread_local bool g_pdl_plain = false;
+bool pdl_plain() { return g_pdl_plain; }
+void set_pdl_plain(bool plain) { g_pdl_plain = plain; }
+
 static int g_kernel_path = 0;
 int kernel_path() { return g_kernel_path; }
 void set_kernel_path(int flags) { g_kernel_path = flags; }

@@ -93,14 +93,17 @@ def test_onsite_config1_every_kernel_path_agrees():
     A, B = cuda(inp.A), cuda(inp.B)
     got = onsite_dev(inp, A, B).clone()
     for flags in (cg.PATH_UNFUSED_ONSITE, cg.PATH_UNFUSED_ONSITE | cg.PATH_SMEM_CORE,
-                  cg.PATH_UNFUSED_ONSITE | cg.PATH_GENERIC_CORE, cg.PATH_UNFUSED_ONSITE | cg.PATH_GENERIC_PROJ, GENERIC_ALL):
+                  cg.PATH_UNFUSED_ONSITE | cg.PATH_GENERIC_CORE, cg.PATH_UNFUSED_ONSITE | cg.PATH_GENERIC_PROJ, GENERIC_ALL,
+                  cg.PATH_PLAIN_LAUNCH):
         cg.cgtp_set_kernel_path(flags)
         assert cg.cgtp_get_kernel_path() == flags
         alt = onsite_dev(inp, A, B)
         e = sector_errs_torch(got, alt)
         assert max(e) < TOL, (flags, e)
+        if flags == cg.PATH_PLAIN_LAUNCH:  # the same kernels, launched in plain stream order instead of chained
+            assert torch.equal(got, alt)
     with pytest.raises(cg.CgtpError):
-        cg.cgtp_set_kernel_path(1 << 9)
+        cg.cgtp_set_kernel_path(1 << 10)
 
 
 @pytest.mark.parametrize("cfg,lmax", [(0, None), (1, None), (3, 2), (3, 4), (3, 8), (3, 12), (3, 16), (3, 20)])
