@@ -66,3 +66,20 @@ def test_binding_refuses_cpu_tensors():
     w = torch.zeros((4, 4))
     with pytest.raises(TypeError):
         cg.cgtp_onsite(z, z, w, w, w, 2, 2, 4, 4, [0, 0, 1, 1])
+
+
+def test_kernel_path_switch_bounds_without_gpu():
+    """cgtp_set_kernel_path only stores a process-wide word: every documented CGTP_PATH_* bit is accepted, anything above is
+    CGTP_ERR_INVALID, and the previous value stays in force after a refused call."""
+    L = _lib()
+    try:
+        for bit in (1, 2, 4, 8, 16, 32, 64, 128, 256):
+            assert L.cgtp_set_kernel_path(bit) == 0
+            assert L.cgtp_get_kernel_path() == bit
+        assert L.cgtp_set_kernel_path(511) == 0
+        assert L.cgtp_set_kernel_path(512) != 0
+        assert L.cgtp_set_kernel_path(-1) != 0
+        assert L.cgtp_get_kernel_path() == 511
+    finally:
+        assert L.cgtp_set_kernel_path(0) == 0
+
