@@ -123,3 +123,55 @@ def test_edge_lr_nbody_and_field_families_repeatable_and_in_bounds():
     Xn = [cuda(x) for x in (nb.X, nb.W_in, nb.W_out)]
     ws = cg.cgtp_onsite_nbody_workspace_bytes(3, 3, 3, 8, 8, 130)
     _stress(lambda out, w: cg.cgtp_onsite_nbody(*Xn, 3, 3, 3, 8, 8, out=out, workspace=w), (130, 8, 16), ws)
+
+
+def test_chained_launches_across_entry_points_share_one_workspace():
+    """The kernels of the on-site step, of message passing and of the nu-body product are chained by programmatic dependent
+    launch: a kernel may start while its predecessor in the stream still runs and waits before its first
+    access to anything a predecessor produced.  Different entry points issued back to back on one stream, all carving ONE
+    workspace buffer (so the H / T / G regions of one call are rewritten by the next): a missed wait is a write-after-read or
+    read-after-write race between kernels of different calls.  Every output must equal, bit for bit, the one obtained with
+    plain launches (CGTP_PATH_PLAIN_LAUNCH: the same kernels in the usual stream order), over several repetitions with
+    unrelated traffic on a second stream."""
+    o1 = synthetic.make_onsite(6, 6, 64, 64, 600, seed=71)          # four launches, register core for the odd channels
+    o2 = synthetic.make_onsite(2, 2, 32, 32, 3000, seed=72)         # short kernels: the boundaries overlap most
+    deg = np.random.default_rng(7).integers(0, 24, 300)
+    m = synthetic.make_message(4, 4, 16, 32, 300, deg, seed=73)
+    nb = synthetic.make_nbody(3, 3, 3, 16, 16, 700, seed=74)
+    To1 = [cuda(x) for x in (o1.A, o1.B, o1.W_a, o1.W_b, o1.W_out)]
+    To2 = [cuda(x) for x in (o2.A, o2.B, o2.W_a, o2.W_b, o2.W_out)]
+    Tm = [cuda(x) for x in (m.node_feats, m.edge_index, m.edge_vec, m.edge_radial, m.W_node, m.W_out)]
+    Tn = [cuda(x) for x in (nb.X, nb.W_in, nb.W_out)]
+    ws_bytes = max(cg.cgtp_onsite_workspace_bytes(6, 6, 64, 64, 600), cg.cgtp_onsite_workspace_bytes(2, 2, 32, 32, 3000),
+                   cg.cgtp_message_workspace_bytes(4, 4, 16, 32, m.parity_mask, 300, m.E),
+                   cg.cgtp_onsite_nbody_workspace_bytes(3, 3, 3, 16, 16, 700))
+    g_ws = Guarded(int(ws_bytes))
+    outs = [torch.empty((600, 2, 64, 49), device="cuda"), torch.empty((3000, 2, 32, 9), device="cuda"),
+            torch.empty((300, 2, 16, 25), device="cuda"), torch.empty((700, 16, 16), device="cuda")]
+
+    def sequence():
+        for o in outs:
+            o.fill_(float("nan"))
+        w = g_ws.view
+        cg.cgtp_onsite(*To1, 6, 6, 64, 64, o1.parity_mask, out=outs[0], workspace=w)
+        cg.cgtp_message(*Tm, 4, 4, 16, 32, m.parity_mask, out=outs[2], workspace=w)
+        cg.cgtp_onsite(*To2, 2, 2, 32, 32, o2.parity_mask, out=outs[1], workspace=w)
+        cg.cgtp_onsite_nbody(*Tn, 3, 3, 3, 16, 16, out=outs[3], workspace=w)
+        cg.cgtp_onsite(*To1, 6, 6, 64, 64, o1.parity_mask, out=outs[0], workspace=w)
+        torch.cuda.synchronize()
+        assert all(torch.isfinite(o).all() for o in outs)
+        assert g_ws.intact()
+        return [o.clone() for o in outs]
+
+    cg.cgtp_set_kernel_path(cg.PATH_PLAIN_LAUNCH)
+    ref = sequence()
+    cg.cgtp_set_kernel_path(0)
+    side = torch.cuda.Stream()
+    noise = torch.empty(1 << 24, device="cuda")
+    for r in range(8):
+        if r % 2:
+            with torch.cuda.stream(side):
+                noise.normal_()
+        got = sequence()
+        for k, (a, b) in enumerate(zip(got, ref)):
+            assert torch.equal(a, b), f"repetition {r}, output {k}: chained launches differ from plain launches"
